@@ -1,0 +1,278 @@
+/*
+ * pinsage_oracle.c -- TEST INFRASTRUCTURE, NOT PRODUCT CODE.
+ *
+ * A plain, slow, obviously-correct fp64 CPU statement of what the PinSage
+ * inference hot path computes, written from the paper text
+ * (/root/reference/PAPER.md = arXiv 1806.01973).  Only tests/, bench.py's
+ * cpu_baseline / --impl reference leg and __graft_entry__.smoke() may call it.
+ * It shares no code, header, table or helper with the CUDA path under
+ * paper_1806_01973_b200/csrc/ and neither includes the other.
+ *
+ * What is implemented (every function cites the passage it follows):
+ *   Algorithm 1 CONVOLVE
+ *     line 1: n_u = gamma({ReLU(Q h_v + q) | v in N(u)}, alpha)        :114
+ *             gamma = importance pooling = weighted mean with the
+ *             L1-normalised visit counts as weights                     :120-124
+ *     line 2: z_u = ReLU(W concat(h_u, n_u) + w)   (self first)         :115
+ *     line 3: z_u = z_u / ||z_u||_2                                     :116
+ *   Stacking K layers, layer 0 = input features    PAPER.md:126, Alg.2 l.8-14 :155-164
+ *   Head z_u = G2 ReLU(G1 h_u^(K) + g)             PAPER.md:166 (Alg.2 l.16), :130
+ *   Layer-wise ("MapReduce") schedule: project every node once, then join
+ *   + pool per destination                         PAPER.md:214-221 (sec. 3.4)
+ *
+ * Readings where the paper is silent / garbled:
+ *   A2  alpha[v][t] = (float)c[v][t] / (float)(sum_t c[v][t]) in IEEE binary32,
+ *       then used as given: the pool is a weighted SUM with weights summing to 1.
+ *   A3  ||z|| == 0  ->  the zero row (no NaN).
+ *   A5  concat order [h_u ; n_u]: the first d_in columns of W act on self.
+ *   A6  head has one bias (g, on G1), no activation / normalisation after G2.
+ *   A18 every matrix is stored "out x in" row-major, applied as M * vector.
+ *
+ * Parity pins (tests/test_oracle_pins.py, none of them re-types these loops):
+ *   numpy fp64 relu(H @ Q.T + q) for the dense steps; scipy.sparse SpMM for the
+ *   pool; hand-computed worked example (tests/golden/worked_example.txt);
+ *   closed forms (identity layer, graph-free self-loop MLP, sparse power step,
+ *   positive-scale invariance); invariants (unit rows, alpha rows sum to 1,
+ *   neighbour-order and node-relabelling invariance, entry splitting);
+ *   brute-force recursion over the K-hop tree == literal == layer-wise.
+ *   Nothing here is "parity unpinned".
+ *
+ * All arrays are row-major double unless stated; indices are int32 in [0, N).
+ * Build: gcc -O2 -std=c99 -ffp-contract=off -fopenmp -shared -fPIC (see oracle.py).
+ */
+#include <math.h>
+#include <stdint.h>
+#include <stdlib.h>
+#include <string.h>
+
+#ifdef _OPENMP
+#include <omp.h>
+#endif
+
+int oracle_num_threads(void)
+{
+#ifdef _OPENMP
+    return omp_get_max_threads();
+#else
+    return 1;
+#endif
+}
+
+static double relu(double x) { return x > 0.0 ? x : 0.0; }
+
+/* y[j] = ReLU(sum_i M[j][i] x[i] + b[j]),  M is [rows x cols] "out x in".
+ * b may be NULL (no bias); act = 0 disables the ReLU.                      */
+static void affine(const double *M, const double *b, int rows, int cols,
+                   const double *x, int act, double *y)
+{
+    for (int j = 0; j < rows; ++j) {
+        double s = 0.0;
+        for (int i = 0; i < cols; ++i)
+            s += M[(size_t)j * cols + i] * x[i];
+        if (b)
+            s += b[j];
+        y[j] = act ? relu(s) : s;
+    }
+}
+
+/* PAPER.md:120-124 + reading A2.  counts [N x T] int32 -> alpha [N x T] float. */
+void oracle_normalize_counts(int64_t N, int32_t T, const int32_t *counts, float *alpha)
+{
+    for (int64_t v = 0; v < N; ++v) {
+        int64_t tot = 0;
+        for (int t = 0; t < T; ++t)
+            tot += counts[v * T + t];
+        float ftot = (float)tot;
+        for (int t = 0; t < T; ++t)
+            alpha[v * T + t] = (float)counts[v * T + t] / ftot;
+    }
+}
+
+/*
+ * Algorithm 1 CONVOLVE for ONE node, literally.
+ *   h_u      [d_in]       current representation of u
+ *   h_nbr    [T x d_in]   current representations of v_0..v_{T-1} in N(u)
+ *   alpha    [T]          neighbour weights
+ *   Q [m x d_in], q [m], W [d x (d_in+m)], w [d]
+ *   out      [d]
+ * scratch must hold 2*m + d_in + m doubles (p_t, n, concat).
+ */
+void oracle_convolve_node(int32_t T, int32_t d_in, int32_t m, int32_t d,
+                          const double *h_u, const double *h_nbr, const double *alpha,
+                          const double *Q, const double *q, const double *W, const double *w,
+                          double *out, double *scratch)
+{
+    double *p = scratch;          /* [m]        */
+    double *n = scratch + m;      /* [m]        */
+    double *cat = scratch + 2 * m; /* [d_in + m] */
+    for (int j = 0; j < m; ++j)
+        n[j] = 0.0;
+    /* line 1: project each neighbour through Q (ReLU inside, A19), weight, sum */
+    for (int t = 0; t < T; ++t) {
+        affine(Q, q, m, d_in, h_nbr + (size_t)t * d_in, 1, p);
+        for (int j = 0; j < m; ++j)
+            n[j] += alpha[t] * p[j];
+    }
+    /* line 2: concat(self, neighbourhood), W, ReLU */
+    for (int i = 0; i < d_in; ++i)
+        cat[i] = h_u[i];
+    for (int j = 0; j < m; ++j)
+        cat[d_in + j] = n[j];
+    affine(W, w, d, d_in + m, cat, 1, out);
+    /* line 3: L2 normalise (A3: zero row stays zero) */
+    double ss = 0.0;
+    for (int j = 0; j < d; ++j)
+        ss += out[j] * out[j];
+    double nrm = sqrt(ss);
+    if (nrm > 0.0)
+        for (int j = 0; j < d; ++j)
+            out[j] /= nrm;
+}
+
+/* Mode A: one layer, literal Algorithm 1 applied node by node over all N nodes
+ * (every neighbour projection is recomputed for every (u,t) occurrence).     */
+void oracle_layer_literal(int64_t N, int32_t T, int32_t d_in, int32_t m, int32_t d,
+                          const double *H, const int32_t *idx, const float *alpha,
+                          const double *Q, const double *q, const double *W, const double *w,
+                          double *out)
+{
+#pragma omp parallel
+    {
+        double *scratch = (double *)malloc(sizeof(double) * (size_t)(3 * m + d_in));
+        double *nbr = (double *)malloc(sizeof(double) * (size_t)T * d_in);
+        double *a = (double *)malloc(sizeof(double) * (size_t)T);
+#pragma omp for schedule(static)
+        for (int64_t u = 0; u < N; ++u) {
+            for (int t = 0; t < T; ++t) {
+                memcpy(nbr + (size_t)t * d_in, H + (size_t)idx[u * T + t] * d_in,
+                       sizeof(double) * (size_t)d_in);
+                a[t] = (double)alpha[u * T + t];
+            }
+            oracle_convolve_node(T, d_in, m, d, H + (size_t)u * d_in, nbr, a, Q, q, W, w,
+                                 out + (size_t)u * d, scratch);
+        }
+        free(scratch);
+        free(nbr);
+        free(a);
+    }
+}
+
+/* S1 (PAPER.md:114 dense part; sec. 3.4 job 1 :218): P[v] = ReLU(Q H[v] + q), once per node.
+ * Also serves the head's dense layers (act / bias switchable).                */
+void oracle_dense(int64_t N, int32_t d_in, int32_t d_out, const double *H,
+                  const double *M, const double *b, int32_t act, double *P)
+{
+#pragma omp parallel for schedule(static)
+    for (int64_t v = 0; v < N; ++v)
+        affine(M, b, d_out, d_in, H + (size_t)v * d_in, act, P + (size_t)v * d_out);
+}
+
+/* S2 (PAPER.md:114 gamma, :124; sec. 3.4 job 2 :219): n[v] = sum_t alpha[v][t] * P[idx[v][t]]. */
+void oracle_pool(int64_t N, int32_t T, int32_t m, const double *P,
+                 const int32_t *idx, const float *alpha, double *n)
+{
+#pragma omp parallel for schedule(static)
+    for (int64_t v = 0; v < N; ++v) {
+        double *nv = n + (size_t)v * m;
+        for (int j = 0; j < m; ++j)
+            nv[j] = 0.0;
+        for (int t = 0; t < T; ++t) {
+            const double *pr = P + (size_t)idx[v * T + t] * m;
+            double a = (double)alpha[v * T + t];
+            for (int j = 0; j < m; ++j)
+                nv[j] += a * pr[j];
+        }
+    }
+}
+
+/* S3: out[v] = normalise(ReLU(W concat(H[v], n[v]) + w)). */
+void oracle_combine(int64_t N, int32_t d_in, int32_t m, int32_t d,
+                    const double *H, const double *n, const double *W, const double *w,
+                    double *out)
+{
+#pragma omp parallel
+    {
+        double *cat = (double *)malloc(sizeof(double) * (size_t)(d_in + m));
+#pragma omp for schedule(static)
+        for (int64_t v = 0; v < N; ++v) {
+            double *o = out + (size_t)v * d;
+            memcpy(cat, H + (size_t)v * d_in, sizeof(double) * (size_t)d_in);
+            memcpy(cat + d_in, n + (size_t)v * m, sizeof(double) * (size_t)m);
+            affine(W, w, d, d_in + m, cat, 1, o);
+            double ss = 0.0;
+            for (int j = 0; j < d; ++j)
+                ss += o[j] * o[j];
+            double nrm = sqrt(ss);
+            if (nrm > 0.0)
+                for (int j = 0; j < d; ++j)
+                    o[j] /= nrm;
+        }
+        free(cat);
+    }
+}
+
+/* Mode B: one layer in the layer-wise schedule of sec. 3.4:
+ * project every node once, then pool + combine per destination.  Same per-output
+ * arithmetic and loop order as the literal form, so the two agree bit for bit.
+ * P_ws [N x m] and n_ws [N x m] are caller-provided workspaces.               */
+void oracle_layer_layerwise(int64_t N, int32_t T, int32_t d_in, int32_t m, int32_t d,
+                            const double *H, const int32_t *idx, const float *alpha,
+                            const double *Q, const double *q, const double *W, const double *w,
+                            double *out, double *P_ws, double *n_ws)
+{
+    oracle_dense(N, d_in, m, H, Q, q, 1, P_ws);
+    oracle_pool(N, T, m, P_ws, idx, alpha, n_ws);
+    oracle_combine(N, d_in, m, d, H, n_ws, W, w, out);
+}
+
+/* Head (Alg. 2 l.16; A6): out[v] = G2 ReLU(G1 h[v] + g). */
+void oracle_head(int64_t N, int32_t d, int32_t g1, int32_t d_out, const double *H,
+                 const double *G1, const double *g, const double *G2, double *out)
+{
+#pragma omp parallel
+    {
+        double *a = (double *)malloc(sizeof(double) * (size_t)g1);
+#pragma omp for schedule(static)
+        for (int64_t v = 0; v < N; ++v) {
+            affine(G1, g, g1, d, H + (size_t)v * d, 1, a);
+            affine(G2, NULL, d_out, g1, a, 0, out + (size_t)v * d_out);
+        }
+        free(a);
+    }
+}
+
+/*
+ * Mode R: brute-force recursion over the K-hop computation tree (Fig. 1,
+ * PAPER.md:39; Alg. 2 l.8-14 with no sharing of any intermediate):
+ *   rec(u,0) = x_u ;  rec(u,k) = CONVOLVE_k(rec(u,k-1), {rec(v_t,k-1)}).
+ * Cost O(T^K) per node: tiny inputs only.
+ * dims[0..K] = d_0, d_1, ..., d_K ; ms[k-1] = m of layer k;
+ * Qs/qs/Ws/ws are arrays of K pointers.  out [dims[k]].
+ */
+void oracle_rec(int64_t u, int32_t k, int32_t T, const int32_t *dims, const int32_t *ms,
+                const double *X, const int32_t *idx, const float *alpha,
+                const double *const *Qs, const double *const *qs,
+                const double *const *Ws, const double *const *ws, double *out)
+{
+    if (k == 0) {
+        memcpy(out, X + (size_t)u * dims[0], sizeof(double) * (size_t)dims[0]);
+        return;
+    }
+    int32_t d_in = dims[k - 1], d = dims[k], m = ms[k - 1];
+    double *h_u = (double *)malloc(sizeof(double) * (size_t)d_in);
+    double *nbr = (double *)malloc(sizeof(double) * (size_t)T * d_in);
+    double *a = (double *)malloc(sizeof(double) * (size_t)T);
+    double *scratch = (double *)malloc(sizeof(double) * (size_t)(3 * m + d_in));
+    oracle_rec(u, k - 1, T, dims, ms, X, idx, alpha, Qs, qs, Ws, ws, h_u);
+    for (int t = 0; t < T; ++t) {
+        oracle_rec(idx[u * T + t], k - 1, T, dims, ms, X, idx, alpha, Qs, qs, Ws, ws,
+                   nbr + (size_t)t * d_in);
+        a[t] = (double)alpha[u * T + t];
+    }
+    oracle_convolve_node(T, d_in, m, d, h_u, nbr, a, Qs[k - 1], qs[k - 1], Ws[k - 1], ws[k - 1],
+                         out, scratch);
+    free(h_u);
+    free(nbr);
+    free(a);
+    free(scratch);
+}
