@@ -1,0 +1,186 @@
+/*
+ * pinsage.h -- C-ABI of the B200-native (sm_100a) PinSage layer-wise inference library.
+ *
+ * The path (citations are /root/reference/PAPER.md = arXiv 1806.01973, line:section):
+ *
+ *   for k = 1..K over ALL N nodes                       (stacking, :126; Alg. 2 l.8-14 :155-164)
+ *     S1  P   = ReLU(H_{k-1} Q^T + q)      once per node    (Alg. 1 l.1 dense part :114; sec. 3.4 job 1 :218)
+ *     S2  n_v = sum_t nbr_w[v,t] P[nbr_idx[v,t]]            (Alg. 1 l.1 gamma :114, importance pooling :124;
+ *                                                            sec. 3.4 job 2 :219)
+ *     S3  z_v = ReLU(W [H_{k-1,v} ; n_v] + w)               (Alg. 1 l.2 :115, self first)
+ *         H_k[v] = z_v / ||z_v||_2   (zero row stays zero)  (Alg. 1 l.3 :116)
+ *   S4  a   = ReLU(H_K G1^T + g)                            (Alg. 2 l.16 :166)
+ *   S5  out = a G2^T                                        (same line; no bias / activation / norm after G2)
+ *
+ * Conventions
+ *   - Plain C99. No exceptions cross the boundary; every call returns a pinsage_status and
+ *     leaves a message retrievable with pinsage_last_error().  There is NO CPU fallback:
+ *     a non-sm_100 device gives PINSAGE_ERR_ARCH.
+ *   - Matrices are row-major.  Parameter matrices are in the paper's orientation, "out x in":
+ *     Q [m x d_in] applied as Q h (:114), W [d x (d_in+m)] (:115), G1 [g1 x d], G2 [d_out x g1] (:166).
+ *   - dtype selects storage of features, weights, intermediates and outputs:
+ *     PINSAGE_BF16 (bf16 storage, tcgen05 tensor-core GEMMs, fp32 accumulate, one RNE rounding at each
+ *     of P, n, H_k, a, out) or PINSAGE_F32 (fp32 storage, IEEE fp32 FMA arithmetic).  Biases and
+ *     neighbour weights are always fp32, neighbour ids int32.
+ *   - Pointers are DEVICE pointers unless a parameter is documented "host or device".
+ *     All pointers must be 16-byte aligned; every feature dimension must be a multiple of 8.
+ *   - The caller owns every buffer passed in.  The library never frees or keeps caller pointers
+ *     beyond the stream-ordered completion of the call.  Compute calls are asynchronous on the
+ *     context's stream unless documented otherwise.
+ *   - 0 <= nbr_idx < N is a precondition of the hot path (checked only by pinsage_validate_graph
+ *     or when the context option "check_indices" is 1).  Self references and repeated ids are
+ *     legal; a short neighbourhood is padded with any valid id and weight 0.
+ *   - nbr_w is used as given (weighted SUM).  The paper's weighted mean = rows that sum to 1,
+ *     e.g. produced by pinsage_normalize_counts.
+ *   - Identical inputs give bit-identical outputs run to run (no atomics, fixed summation order).
+ */
+#ifndef PINSAGE_H_
+#define PINSAGE_H_
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef enum {
+    PINSAGE_OK = 0,
+    PINSAGE_ERR_INVALID_ARG = 1,       /* null pointer, non-positive size, inconsistent dims, bad overlap */
+    PINSAGE_ERR_UNSUPPORTED_SHAPE = 2, /* a dimension outside what the kernels are built for */
+    PINSAGE_ERR_MISALIGNED = 3,        /* pointer not 16-byte aligned */
+    PINSAGE_ERR_BAD_INDEX = 4,         /* nbr_idx outside [0, N) found by validation */
+    PINSAGE_ERR_OOM = 5,               /* workspace allocation failed / caller workspace too small */
+    PINSAGE_ERR_CUDA = 6,              /* CUDA runtime / driver error, text in pinsage_last_error */
+    PINSAGE_ERR_ARCH = 7               /* device is not compute capability 10.x */
+} pinsage_status;
+
+typedef enum { PINSAGE_BF16 = 0, PINSAGE_F32 = 1 } pinsage_dtype;
+
+typedef struct pinsage_ctx pinsage_ctx; /* opaque */
+
+/* One CONVOLVE layer's parameters.  Device pointers. */
+typedef struct {
+    int32_t d_in, m, d; /* Q:[m x d_in]  W:[d x (d_in+m)] */
+    const void *Q;      /* dtype */
+    const float *q;     /* [m] fp32 */
+    const void *W;      /* dtype */
+    const float *w;     /* [d] fp32 */
+} pinsage_layer_params;
+
+/* Head parameters G1, g, G2.  Device pointers. */
+typedef struct {
+    int32_t d, g1, d_out; /* G1:[g1 x d]  G2:[d_out x g1] */
+    const void *G1;       /* dtype */
+    const float *g;       /* [g1] fp32 */
+    const void *G2;       /* dtype */
+} pinsage_head_params;
+
+/* ---- context ------------------------------------------------------------------------------ */
+
+/* Creates a context on `device`.  `cuda_stream` (a cudaStream_t, may be NULL = the legacy default
+ * stream) is borrowed: all work is enqueued there.  Fails with PINSAGE_ERR_ARCH unless the device is
+ * compute capability 10.x.  *out is NULL on failure. */
+pinsage_status pinsage_create(pinsage_ctx **out, int device, void *cuda_stream);
+
+/* Synchronises the context's stream and releases everything the context owns. NULL is a no-op. */
+void pinsage_destroy(pinsage_ctx *ctx);
+
+/* Context-owned, NUL-terminated message of the last failing call ("" if none). With ctx == NULL
+ * returns the message of the last failed pinsage_create on this thread. */
+const char *pinsage_last_error(const pinsage_ctx *ctx);
+
+/* Static version string, e.g. "pinsage-b200 0.1.0 (sm_100a)". */
+const char *pinsage_version(void);
+
+/* Integer options:  "gemm_impl"      0 = tcgen05 (default for BF16), 1 = SIMT reference kernels
+ *                   "check_indices"  1 = every pinsage_pool / layer / embed_all call validates
+ *                                    nbr_idx first (synchronous), default 0
+ *                   "overlap"        1 = pinsage_layer / embed_all overlap S2 of chunk c+1 with S3
+ *                                    of chunk c on a second stream (default 0)
+ *                   "profile"        1 = bracket every kernel launch of the path with CUDA events
+ *                                    on its stream, see pinsage_profile_read (default 0)
+ * Unknown key -> PINSAGE_ERR_INVALID_ARG. */
+pinsage_status pinsage_set_option(pinsage_ctx *ctx, const char *key, int64_t value);
+
+/* Number of kernels this context has launched so far (for launch accounting in benchmarks). */
+int64_t pinsage_launch_count(const pinsage_ctx *ctx);
+
+/* Per-kernel device time gathered while option "profile" is 1.  Synchronises the context's streams,
+ * then sums the event-measured duration of every launch of `kind` since the last reset into
+ * *total_ms and their number into *launches (HOST pointers).  kind: 0 = S2 pool, 1 = S1/S4/S5 dense,
+ * 2 = S3 combine, -1 = reset the records (outputs are then 0). */
+pinsage_status pinsage_profile_read(pinsage_ctx *ctx, int32_t kind, double *total_ms,
+                                    int64_t *launches);
+
+/* ---- the steps of the path, one call each ------------------------------------------------- */
+
+/* S1 / S4 / S5: out[M x n_out] = act(A[M x k] * Wt[n_out x k]^T + bias).
+ * bias may be NULL (S5).  relu: 0/1.  A, Wt, out: dtype.  PAPER.md:114, :166. */
+pinsage_status pinsage_dense(pinsage_ctx *ctx, pinsage_dtype dtype, int64_t M, int32_t k,
+                             int32_t n_out, const void *A, const void *Wt, const float *bias,
+                             int32_t relu, void *out);
+
+/* S2: n[v] = sum_{t<T} nbr_w[v,t] * P[nbr_idx[v,t], :] for v in [0, n_dst), fp32 accumulation in the
+ * order t = 0..T-1.  P:[n_src x m] dtype (randomly accessed); nbr_idx/nbr_w:[n_dst x T];
+ * n:[n_dst x m] dtype.  1 <= T <= 1024.  PAPER.md:114, :124, :219. */
+pinsage_status pinsage_pool(pinsage_ctx *ctx, pinsage_dtype dtype, int64_t n_dst, int64_t n_src,
+                            int32_t T, int32_t m, const void *P, const int32_t *nbr_idx,
+                            const float *nbr_w, void *n);
+
+/* S3: out[v] = normalise(ReLU(W [H[v] ; n[v]] + w)), W:[d x (d_in+m)] read as two K-segments
+ * (no concat is materialised).  H:[M x d_in], n:[M x m], out:[M x d], all dtype.
+ * out == H is allowed iff d == d_in (in-place layer k >= 2).  PAPER.md:115-116. */
+pinsage_status pinsage_combine(pinsage_ctx *ctx, pinsage_dtype dtype, int64_t M, int32_t d_in,
+                               int32_t m, int32_t d, const void *H, const void *n, const void *W,
+                               const float *w, void *out);
+
+/* ---- the entry points BASELINE.json names ------------------------------------------------- */
+
+/* One CONVOLVE layer over all N nodes: S1 -> S2 -> S3.  feats:[N x d_in], out:[N x d].
+ * Workspace (P [N x m] + one chunk of n) is ctx-owned when ws == NULL, else the caller's
+ * (ws_bytes >= pinsage_layer_workspace_bytes, 256-byte aligned; too small -> PINSAGE_ERR_OOM).
+ * out == feats is allowed iff d == d_in.  Alg. 1; schedule sec. 3.4 :214-221. */
+pinsage_status pinsage_layer(pinsage_ctx *ctx, pinsage_dtype dtype, int64_t N, int32_t T,
+                             const void *feats, const int32_t *nbr_idx, const float *nbr_w,
+                             const pinsage_layer_params *params, void *out, void *ws,
+                             size_t ws_bytes);
+
+size_t pinsage_layer_workspace_bytes(pinsage_dtype dtype, int64_t N, int32_t T,
+                                     const pinsage_layer_params *params);
+
+/* Head: S4 -> S5 in node chunks.  h:[N x d] -> out:[N x d_out].  Alg. 2 l.16. */
+pinsage_status pinsage_head(pinsage_ctx *ctx, pinsage_dtype dtype, int64_t N, const void *h,
+                            const pinsage_head_params *params, void *out);
+
+/* K layers + head over all N nodes with the chunked layer driver (Alg. 2 l.8-17 with S^(k) = V).
+ * feats:[N x layers[0].d_in], nbr_idx / nbr_w:[N x T], out:[N x head->d_out] may each be DEVICE or
+ * HOST pointers (detected with cudaPointerGetAttributes; host buffers should be pinned for speed):
+ * host inputs are copied to device staging owned by the context and a host `out` is filled by a
+ * device-to-host copy, all inside this call.  `layers` (array of K structs) and `head` are host
+ * structs holding device pointers.  chunk_nodes = destination rows per S2/S3 chunk (0 = automatic).
+ * If any buffer is a host pointer the call synchronises the stream before returning; with device
+ * buffers only it is asynchronous. */
+pinsage_status pinsage_embed_all(pinsage_ctx *ctx, pinsage_dtype dtype, int64_t N, int32_t T,
+                                 int32_t K, const void *feats, const int32_t *nbr_idx,
+                                 const float *nbr_w, const pinsage_layer_params *layers,
+                                 const pinsage_head_params *head, void *out, int64_t chunk_nodes);
+
+/* ---- helpers ------------------------------------------------------------------------------ */
+
+/* nbr_w[v,t] = (float)counts[v,t] / (float)(sum_t counts[v,t]) in IEEE binary32 (L1-normalised visit
+ * counts).  counts:[N x T] int32 >= 0 with a positive row sum. */
+pinsage_status pinsage_normalize_counts(pinsage_ctx *ctx, int64_t N, int32_t T,
+                                        const int32_t *counts, float *nbr_w);
+
+/* Synchronous.  Checks 0 <= nbr_idx[i] < n_src for all n_dst*T entries and that every weight is
+ * finite.  *first_bad (HOST pointer) receives the flat position of the first offender or -1;
+ * returns PINSAGE_ERR_BAD_INDEX if there is one. */
+pinsage_status pinsage_validate_graph(pinsage_ctx *ctx, int64_t n_dst, int64_t n_src, int32_t T,
+                                      const int32_t *nbr_idx, const float *nbr_w,
+                                      int64_t *first_bad);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* PINSAGE_H_ */

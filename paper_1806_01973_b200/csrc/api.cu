@@ -1,0 +1,841 @@
+// api.cu -- the C-ABI of include/pinsage.h: context, argument checking, the layer driver (S6).
+// Every step of the path runs in this library's own kernels (pool.cu, gemm_tcgen05.cu,
+// gemm_simt.cu); there is no CPU or vendor-library fallback.
+#include "../../include/pinsage.h"
+#include "internal.h"
+
+#include <algorithm>
+#include <cstdarg>
+#include <cstdio>
+#include <cstring>
+#include <new>
+#include <string>
+#include <vector>
+
+using namespace pinsage;
+
+struct pinsage_ctx {
+    int device = 0;
+    cudaStream_t stream = nullptr;
+    cudaStream_t aux = nullptr;      // second stream for S2 / S3 overlap
+    cudaEvent_t ev_pool[2] = {nullptr, nullptr};
+    cudaEvent_t ev_gemm[2] = {nullptr, nullptr};
+    cudaEvent_t ev_fork = nullptr, ev_join = nullptr;
+    int num_sms = 0;
+    int gemm_impl = 0;               // 0 tcgen05, 1 SIMT reference
+    int check_indices = 0;
+    int overlap = 0;
+    int launches = 0;
+    int64_t total_launches = 0;
+    void *ws = nullptr;              // context-owned workspace
+    size_t ws_bytes = 0;
+    void *stage = nullptr;           // device staging for host inputs / outputs
+    size_t stage_bytes = 0;
+    long long *d_first_bad = nullptr;
+    // optional per-kernel timing ("profile" option): event pairs around every launch
+    int profile = 0;
+    std::vector<cudaEvent_t> prof_events;
+    struct ProfRec { int kind; int e0, e1; };
+    std::vector<ProfRec> prof_recs;
+    size_t prof_used = 0;
+    std::string err;
+};
+
+namespace {
+
+thread_local std::string g_create_err;
+
+pinsage_status fail(pinsage_ctx *ctx, pinsage_status st, const char *fmt, ...)
+{
+    char buf[512];
+    va_list ap;
+    va_start(ap, fmt);
+    vsnprintf(buf, sizeof buf, fmt, ap);
+    va_end(ap);
+    if (ctx)
+        ctx->err = buf;
+    else
+        g_create_err = buf;
+    return st;
+}
+
+#define PS_CUDA(ctx, expr)                                                                   \
+    do {                                                                                     \
+        cudaError_t e_ = (expr);                                                             \
+        if (e_ != cudaSuccess)                                                               \
+            return fail(ctx, e_ == cudaErrorMemoryAllocation ? PINSAGE_ERR_OOM               \
+                                                             : PINSAGE_ERR_CUDA,             \
+                        "%s: %s", #expr, cudaGetErrorString(e_));                            \
+    } while (0)
+
+#define PS_TRY(expr)                          \
+    do {                                      \
+        pinsage_status st_ = (expr);          \
+        if (st_ != PINSAGE_OK) return st_;    \
+    } while (0)
+
+struct DeviceGuard {
+    int prev = -1;
+    explicit DeviceGuard(int dev)
+    {
+        cudaGetDevice(&prev);
+        if (prev != dev) cudaSetDevice(dev);
+        else prev = -1;
+    }
+    ~DeviceGuard()
+    {
+        if (prev >= 0) cudaSetDevice(prev);
+    }
+};
+
+inline size_t align_up(size_t x, size_t a) { return (x + a - 1) / a * a; }
+
+bool aligned16(const void *p) { return (reinterpret_cast<uintptr_t>(p) & 15u) == 0; }
+
+pinsage_status check_dtype(pinsage_ctx *ctx, pinsage_dtype dt)
+{
+    if (dt != PINSAGE_BF16 && dt != PINSAGE_F32)
+        return fail(ctx, PINSAGE_ERR_INVALID_ARG, "unknown dtype %d", (int)dt);
+    return PINSAGE_OK;
+}
+
+pinsage_status check_dim(pinsage_ctx *ctx, const char *name, int64_t v)
+{
+    if (v <= 0) return fail(ctx, PINSAGE_ERR_INVALID_ARG, "%s = %lld must be positive", name, (long long)v);
+    if (v % 8 != 0)
+        return fail(ctx, PINSAGE_ERR_UNSUPPORTED_SHAPE, "%s = %lld must be a multiple of 8", name,
+                    (long long)v);
+    if (v > 8192)
+        return fail(ctx, PINSAGE_ERR_UNSUPPORTED_SHAPE, "%s = %lld exceeds 8192", name, (long long)v);
+    return PINSAGE_OK;
+}
+
+pinsage_status check_ptr(pinsage_ctx *ctx, const char *name, const void *p)
+{
+    if (!p) return fail(ctx, PINSAGE_ERR_INVALID_ARG, "%s is NULL", name);
+    if (!aligned16(p)) return fail(ctx, PINSAGE_ERR_MISALIGNED, "%s is not 16-byte aligned", name);
+    return PINSAGE_OK;
+}
+
+bool overlaps(const void *a, size_t na, const void *b, size_t nb)
+{
+    const char *pa = static_cast<const char *>(a), *pb = static_cast<const char *>(b);
+    return pa < pb + nb && pb < pa + na;
+}
+
+pinsage_status ensure_ws(pinsage_ctx *ctx, size_t bytes)
+{
+    if (bytes <= ctx->ws_bytes) return PINSAGE_OK;
+    if (ctx->ws) {
+        PS_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
+        PS_CUDA(ctx, cudaStreamSynchronize(ctx->aux));
+        cudaFree(ctx->ws);
+        ctx->ws = nullptr;
+        ctx->ws_bytes = 0;
+    }
+    cudaError_t e = cudaMalloc(&ctx->ws, bytes);
+    if (e != cudaSuccess) {
+        cudaGetLastError();
+        return fail(ctx, PINSAGE_ERR_OOM, "workspace of %zu bytes: %s", bytes, cudaGetErrorString(e));
+    }
+    ctx->ws_bytes = bytes;
+    return PINSAGE_OK;
+}
+
+pinsage_status ensure_stage(pinsage_ctx *ctx, size_t bytes)
+{
+    if (bytes <= ctx->stage_bytes) return PINSAGE_OK;
+    if (ctx->stage) {
+        PS_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
+        cudaFree(ctx->stage);
+        ctx->stage = nullptr;
+        ctx->stage_bytes = 0;
+    }
+    cudaError_t e = cudaMalloc(&ctx->stage, bytes);
+    if (e != cudaSuccess) {
+        cudaGetLastError();
+        return fail(ctx, PINSAGE_ERR_OOM, "staging of %zu bytes: %s", bytes, cudaGetErrorString(e));
+    }
+    ctx->stage_bytes = bytes;
+    return PINSAGE_OK;
+}
+
+enum ProfKind { PROF_POOL = 0, PROF_DENSE = 1, PROF_COMBINE = 2, PROF_KINDS = 3 };
+
+// Records an event on stream s (profile mode only) and returns its slot, or -1.
+int prof_mark(pinsage_ctx *ctx, cudaStream_t s)
+{
+    if (!ctx->profile) return -1;
+    if (ctx->prof_used == ctx->prof_events.size()) {
+        cudaEvent_t e;
+        if (cudaEventCreate(&e) != cudaSuccess) return -1;
+        ctx->prof_events.push_back(e);
+    }
+    const int slot = (int)ctx->prof_used++;
+    cudaEventRecord(ctx->prof_events[slot], s);
+    return slot;
+}
+
+void prof_close(pinsage_ctx *ctx, int kind, int e0, cudaStream_t s)
+{
+    if (e0 < 0) return;
+    const int e1 = prof_mark(ctx, s);
+    if (e1 >= 0) ctx->prof_recs.push_back({kind, e0, e1});
+}
+
+void count_launches(pinsage_ctx *ctx)
+{
+    ctx->total_launches += ctx->launches;
+    ctx->launches = 0;
+}
+
+// One GEMM of the path on stream s. scratch: fp32 [M x N] for the SIMT norm pass / tcgen05 partials.
+pinsage_status run_gemm(pinsage_ctx *ctx, DType dt, const GemmArgs &a, void *scratch,
+                        size_t scratch_bytes, cudaStream_t s)
+{
+    if (a.M == 0) return PINSAGE_OK;
+    const bool simt = dt == DType::F32 || ctx->gemm_impl == 1;
+    const int kind = a.l2norm ? PROF_COMBINE : PROF_DENSE;
+    if (simt) {
+        const size_t need = gemm_simt_scratch_bytes(a);
+        if (need > scratch_bytes)
+            return fail(ctx, PINSAGE_ERR_OOM, "internal: SIMT scratch %zu > %zu", need, scratch_bytes);
+        const int e0 = prof_mark(ctx, s);
+        cudaError_t e = launch_gemm_simt(dt, a, static_cast<float *>(scratch), s, &ctx->launches);
+        prof_close(ctx, kind, e0, s);
+        count_launches(ctx);
+        PS_CUDA(ctx, e);
+        return PINSAGE_OK;
+    }
+    const char *why = nullptr;
+    if (!gemm_tc_supported(a, &why))
+        return fail(ctx, PINSAGE_ERR_UNSUPPORTED_SHAPE, "tcgen05 GEMM: %s (M=%lld K1=%d K2=%d N=%d)",
+                    why ? why : "unsupported shape", (long long)a.M, a.K1, a.K2, a.N);
+    const int e0 = prof_mark(ctx, s);
+    cudaError_t e = launch_gemm_tc(a, ctx->num_sms, s, &ctx->launches);
+    prof_close(ctx, kind, e0, s);
+    count_launches(ctx);
+    PS_CUDA(ctx, e);
+    return PINSAGE_OK;
+}
+
+size_t gemm_scratch_bytes(const pinsage_ctx *ctx, DType dt, const GemmArgs &a)
+{
+    const bool simt = dt == DType::F32 || (ctx && ctx->gemm_impl == 1);
+    return align_up(simt ? gemm_simt_scratch_bytes(a) : gemm_tc_scratch_bytes(a), 256);
+}
+
+pinsage_status check_layer_params(pinsage_ctx *ctx, const pinsage_layer_params *p, const char *what)
+{
+    if (!p) return fail(ctx, PINSAGE_ERR_INVALID_ARG, "%s is NULL", what);
+    PS_TRY(check_dim(ctx, "d_in", p->d_in));
+    PS_TRY(check_dim(ctx, "m", p->m));
+    PS_TRY(check_dim(ctx, "d", p->d));
+    PS_TRY(check_ptr(ctx, "Q", p->Q));
+    PS_TRY(check_ptr(ctx, "q", p->q));
+    PS_TRY(check_ptr(ctx, "W", p->W));
+    PS_TRY(check_ptr(ctx, "w", p->w));
+    return PINSAGE_OK;
+}
+
+pinsage_status check_head_params(pinsage_ctx *ctx, const pinsage_head_params *p)
+{
+    if (!p) return fail(ctx, PINSAGE_ERR_INVALID_ARG, "head params are NULL");
+    PS_TRY(check_dim(ctx, "head.d", p->d));
+    PS_TRY(check_dim(ctx, "head.g1", p->g1));
+    PS_TRY(check_dim(ctx, "head.d_out", p->d_out));
+    PS_TRY(check_ptr(ctx, "G1", p->G1));
+    PS_TRY(check_ptr(ctx, "g", p->g));
+    PS_TRY(check_ptr(ctx, "G2", p->G2));
+    return PINSAGE_OK;
+}
+
+pinsage_status check_graph_args(pinsage_ctx *ctx, int64_t N, int32_t T)
+{
+    if (N < 1 || N >= (1LL << 31))
+        return fail(ctx, PINSAGE_ERR_INVALID_ARG, "N = %lld outside [1, 2^31)", (long long)N);
+    if (T < 1 || T > 1024) return fail(ctx, PINSAGE_ERR_INVALID_ARG, "T = %d outside [1, 1024]", T);
+    return PINSAGE_OK;
+}
+
+pinsage_status maybe_validate(pinsage_ctx *ctx, int64_t n_dst, int64_t n_src, int32_t T,
+                              const int32_t *idx, const float *w)
+{
+    if (!ctx->check_indices) return PINSAGE_OK;
+    int64_t bad = -1;
+    return pinsage_validate_graph(ctx, n_dst, n_src, T, idx, w, &bad);
+}
+
+int64_t auto_chunk(int64_t N, int64_t requested)
+{
+    int64_t c = requested > 0 ? requested : (int64_t)131072;
+    c = std::min<int64_t>(c, N);
+    if (c < N) c = std::max<int64_t>(128, c / 128 * 128);  // keep chunk starts on GEMM tile edges
+    return c;
+}
+
+// S2 + S3 over all destination rows in chunks; pool of chunk c+1 may overlap combine of chunk c.
+// Hin [N x d_in] (read), P [N x m] (read), Hout [N x d] (written; may alias Hin iff d == d_in).
+// nbuf: two chunk buffers [chunk x m]; scratch: per-GEMM scratch.
+pinsage_status pool_combine_chunks(pinsage_ctx *ctx, DType dt, int64_t N, int32_t T,
+                                   const pinsage_layer_params *lp, const void *Hin, const void *P,
+                                   const int32_t *idx, const float *w, void *Hout, int64_t chunk,
+                                   void *nbuf0, void *nbuf1, void *scratch, size_t scratch_bytes)
+{
+    const size_t es = elem_size(dt);
+    const int64_t nchunks = (N + chunk - 1) / chunk;
+    const bool two = ctx->overlap && nchunks > 1;
+    void *nb[2] = {nbuf0, two ? nbuf1 : nbuf0};
+    if (two) {
+        PS_CUDA(ctx, cudaEventRecord(ctx->ev_fork, ctx->stream));
+        PS_CUDA(ctx, cudaStreamWaitEvent(ctx->aux, ctx->ev_fork, 0));
+    }
+    cudaStream_t ps = two ? ctx->aux : ctx->stream;
+    for (int64_t c = 0; c < nchunks; ++c) {
+        const int64_t r0 = c * chunk, rows = std::min(chunk, N - r0);
+        const int b = (int)(c & 1);
+        if (two && c >= 2) PS_CUDA(ctx, cudaStreamWaitEvent(ps, ctx->ev_gemm[b], 0));
+        const int pe0 = prof_mark(ctx, ps);
+        cudaError_t e = launch_pool(dt, rows, T, lp->m, P, idx + (size_t)r0 * T, w + (size_t)r0 * T,
+                                    nb[b], ps, &ctx->launches);
+        prof_close(ctx, PROF_POOL, pe0, ps);
+        count_launches(ctx);
+        PS_CUDA(ctx, e);
+        if (two) {
+            PS_CUDA(ctx, cudaEventRecord(ctx->ev_pool[b], ps));
+            PS_CUDA(ctx, cudaStreamWaitEvent(ctx->stream, ctx->ev_pool[b], 0));
+        }
+        GemmArgs g;
+        g.M = rows;
+        g.K1 = lp->d_in;
+        g.K2 = lp->m;
+        g.N = lp->d;
+        g.A1 = static_cast<const char *>(Hin) + (size_t)r0 * lp->d_in * es;
+        g.A2 = nb[b];
+        g.B = lp->W;
+        g.bias = lp->w;
+        g.relu = 1;
+        g.l2norm = 1;
+        g.out = static_cast<char *>(Hout) + (size_t)r0 * lp->d * es;
+        PS_TRY(run_gemm(ctx, dt, g, scratch, scratch_bytes, ctx->stream));
+        if (two) PS_CUDA(ctx, cudaEventRecord(ctx->ev_gemm[b], ctx->stream));
+    }
+    if (two) {
+        PS_CUDA(ctx, cudaEventRecord(ctx->ev_join, ps));
+        PS_CUDA(ctx, cudaStreamWaitEvent(ctx->stream, ctx->ev_join, 0));
+    }
+    return PINSAGE_OK;
+}
+
+struct LayerWs {
+    size_t P_off, n0_off, n1_off, scratch_off, scratch_bytes, total;
+};
+
+LayerWs plan_layer_ws(const pinsage_ctx *ctx, DType dt, int64_t N, const pinsage_layer_params *lp,
+                      int64_t chunk)
+{
+    const size_t es = elem_size(dt);
+    LayerWs p{};
+    size_t off = 0;
+    p.P_off = off;
+    off += align_up((size_t)N * lp->m * es, 256);
+    p.n0_off = off;
+    off += align_up((size_t)chunk * lp->m * es, 256);
+    p.n1_off = off;
+    off += align_up((size_t)chunk * lp->m * es, 256);
+    GemmArgs g1;
+    g1.M = N; g1.K1 = lp->d_in; g1.N = lp->m; g1.relu = 1;
+    GemmArgs g3;
+    g3.M = chunk; g3.K1 = lp->d_in; g3.K2 = lp->m; g3.N = lp->d; g3.relu = 1; g3.l2norm = 1;
+    p.scratch_bytes = std::max(gemm_scratch_bytes(ctx, dt, g1), gemm_scratch_bytes(ctx, dt, g3));
+    p.scratch_off = off;
+    off += p.scratch_bytes;
+    p.total = off;
+    return p;
+}
+
+pinsage_status layer_on_ws(pinsage_ctx *ctx, DType dt, int64_t N, int32_t T, const void *feats,
+                           const int32_t *idx, const float *w, const pinsage_layer_params *lp,
+                           void *out, char *ws, const LayerWs &plan, int64_t chunk)
+{
+    GemmArgs g;
+    g.M = N;
+    g.K1 = lp->d_in;
+    g.N = lp->m;
+    g.A1 = feats;
+    g.B = lp->Q;
+    g.bias = lp->q;
+    g.relu = 1;
+    g.out = ws + plan.P_off;
+    PS_TRY(run_gemm(ctx, dt, g, ws + plan.scratch_off, plan.scratch_bytes, ctx->stream));
+    return pool_combine_chunks(ctx, dt, N, T, lp, feats, ws + plan.P_off, idx, w, out, chunk,
+                               ws + plan.n0_off, ws + plan.n1_off, ws + plan.scratch_off,
+                               plan.scratch_bytes);
+}
+
+bool is_host_ptr(const void *p)
+{
+    cudaPointerAttributes at;
+    cudaError_t e = cudaPointerGetAttributes(&at, p);
+    if (e != cudaSuccess) {
+        cudaGetLastError();
+        return true;  // unregistered pageable host memory
+    }
+    return at.type == cudaMemoryTypeHost || at.type == cudaMemoryTypeUnregistered;
+}
+
+}  // namespace
+
+extern "C" {
+
+const char *pinsage_version(void) { return "pinsage-b200 0.1.0 (sm_100a)"; }
+
+const char *pinsage_last_error(const pinsage_ctx *ctx)
+{
+    return ctx ? ctx->err.c_str() : g_create_err.c_str();
+}
+
+pinsage_status pinsage_create(pinsage_ctx **out, int device, void *cuda_stream)
+{
+    if (!out) return fail(nullptr, PINSAGE_ERR_INVALID_ARG, "out is NULL");
+    *out = nullptr;
+    int ndev = 0;
+    cudaError_t e = cudaGetDeviceCount(&ndev);
+    if (e != cudaSuccess) {
+        cudaGetLastError();
+        return fail(nullptr, PINSAGE_ERR_CUDA, "cudaGetDeviceCount: %s", cudaGetErrorString(e));
+    }
+    if (device < 0 || device >= ndev)
+        return fail(nullptr, PINSAGE_ERR_INVALID_ARG, "device %d of %d", device, ndev);
+    cudaDeviceProp prop;
+    e = cudaGetDeviceProperties(&prop, device);
+    if (e != cudaSuccess)
+        return fail(nullptr, PINSAGE_ERR_CUDA, "cudaGetDeviceProperties: %s", cudaGetErrorString(e));
+    if (prop.major != 10)
+        return fail(nullptr, PINSAGE_ERR_ARCH,
+                    "device %d is sm_%d%d; this library is built for sm_100a only", device,
+                    prop.major, prop.minor);
+    pinsage_ctx *ctx = new (std::nothrow) pinsage_ctx;
+    if (!ctx) return fail(nullptr, PINSAGE_ERR_OOM, "host allocation failed");
+    ctx->device = device;
+    ctx->stream = static_cast<cudaStream_t>(cuda_stream);
+    ctx->num_sms = prop.multiProcessorCount;
+    DeviceGuard guard(device);
+    bool ok = cudaStreamCreateWithFlags(&ctx->aux, cudaStreamNonBlocking) == cudaSuccess;
+    for (int i = 0; i < 2 && ok; ++i) {
+        ok = ok && cudaEventCreateWithFlags(&ctx->ev_pool[i], cudaEventDisableTiming) == cudaSuccess;
+        ok = ok && cudaEventCreateWithFlags(&ctx->ev_gemm[i], cudaEventDisableTiming) == cudaSuccess;
+    }
+    ok = ok && cudaEventCreateWithFlags(&ctx->ev_fork, cudaEventDisableTiming) == cudaSuccess;
+    ok = ok && cudaEventCreateWithFlags(&ctx->ev_join, cudaEventDisableTiming) == cudaSuccess;
+    ok = ok && cudaMalloc(&ctx->d_first_bad, sizeof(long long)) == cudaSuccess;
+    if (!ok) {
+        e = cudaGetLastError();
+        pinsage_destroy(ctx);
+        return fail(nullptr, PINSAGE_ERR_CUDA, "context setup: %s", cudaGetErrorString(e));
+    }
+    *out = ctx;
+    return PINSAGE_OK;
+}
+
+void pinsage_destroy(pinsage_ctx *ctx)
+{
+    if (!ctx) return;
+    DeviceGuard guard(ctx->device);
+    cudaStreamSynchronize(ctx->stream);
+    if (ctx->aux) {
+        cudaStreamSynchronize(ctx->aux);
+        cudaStreamDestroy(ctx->aux);
+    }
+    for (int i = 0; i < 2; ++i) {
+        if (ctx->ev_pool[i]) cudaEventDestroy(ctx->ev_pool[i]);
+        if (ctx->ev_gemm[i]) cudaEventDestroy(ctx->ev_gemm[i]);
+    }
+    if (ctx->ev_fork) cudaEventDestroy(ctx->ev_fork);
+    if (ctx->ev_join) cudaEventDestroy(ctx->ev_join);
+    if (ctx->ws) cudaFree(ctx->ws);
+    if (ctx->stage) cudaFree(ctx->stage);
+    if (ctx->d_first_bad) cudaFree(ctx->d_first_bad);
+    for (cudaEvent_t e : ctx->prof_events) cudaEventDestroy(e);
+    cudaGetLastError();
+    delete ctx;
+}
+
+pinsage_status pinsage_set_option(pinsage_ctx *ctx, const char *key, int64_t value)
+{
+    if (!ctx) return PINSAGE_ERR_INVALID_ARG;
+    if (!key) return fail(ctx, PINSAGE_ERR_INVALID_ARG, "key is NULL");
+    if (!strcmp(key, "gemm_impl")) {
+        if (value != 0 && value != 1)
+            return fail(ctx, PINSAGE_ERR_INVALID_ARG, "gemm_impl must be 0 or 1");
+        ctx->gemm_impl = (int)value;
+    } else if (!strcmp(key, "check_indices")) {
+        ctx->check_indices = value != 0;
+    } else if (!strcmp(key, "overlap")) {
+        ctx->overlap = value != 0;
+    } else if (!strcmp(key, "profile")) {
+        ctx->profile = value != 0;
+    } else {
+        return fail(ctx, PINSAGE_ERR_INVALID_ARG, "unknown option '%s'", key);
+    }
+    return PINSAGE_OK;
+}
+
+int64_t pinsage_launch_count(const pinsage_ctx *ctx) { return ctx ? ctx->total_launches : 0; }
+
+pinsage_status pinsage_profile_read(pinsage_ctx *ctx, int32_t kind, double *total_ms, int64_t *launches)
+{
+    if (!ctx) return PINSAGE_ERR_INVALID_ARG;
+    DeviceGuard guard(ctx->device);
+    if (kind < -1 || kind >= PROF_KINDS || !total_ms || !launches)
+        return fail(ctx, PINSAGE_ERR_INVALID_ARG, "profile_read: bad kind or NULL output");
+    PS_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
+    PS_CUDA(ctx, cudaStreamSynchronize(ctx->aux));
+    double ms = 0.0;
+    int64_t n = 0;
+    for (const auto &r : ctx->prof_recs) {
+        if (r.kind != kind) continue;
+        float t = 0.f;
+        PS_CUDA(ctx, cudaEventElapsedTime(&t, ctx->prof_events[r.e0], ctx->prof_events[r.e1]));
+        ms += t;
+        ++n;
+    }
+    *total_ms = ms;
+    *launches = n;
+    if (kind == -1) {  // reset
+        ctx->prof_recs.clear();
+        ctx->prof_used = 0;
+    }
+    return PINSAGE_OK;
+}
+
+pinsage_status pinsage_dense(pinsage_ctx *ctx, pinsage_dtype dtype, int64_t M, int32_t k,
+                             int32_t n_out, const void *A, const void *Wt, const float *bias,
+                             int32_t relu, void *out)
+{
+    if (!ctx) return PINSAGE_ERR_INVALID_ARG;
+    DeviceGuard guard(ctx->device);
+    PS_TRY(check_dtype(ctx, dtype));
+    if (M < 0) return fail(ctx, PINSAGE_ERR_INVALID_ARG, "M = %lld is negative", (long long)M);
+    PS_TRY(check_dim(ctx, "k", k));
+    PS_TRY(check_dim(ctx, "n_out", n_out));
+    PS_TRY(check_ptr(ctx, "A", A));
+    PS_TRY(check_ptr(ctx, "Wt", Wt));
+    PS_TRY(check_ptr(ctx, "out", out));
+    if (bias && !aligned16(bias)) return fail(ctx, PINSAGE_ERR_MISALIGNED, "bias is not 16-byte aligned");
+    const DType dt = static_cast<DType>(dtype);
+    const size_t es = elem_size(dt);
+    if (overlaps(A, (size_t)M * k * es, out, (size_t)M * n_out * es))
+        return fail(ctx, PINSAGE_ERR_INVALID_ARG, "out overlaps A");
+    GemmArgs g;
+    g.M = M; g.K1 = k; g.N = n_out; g.A1 = A; g.B = Wt; g.bias = bias; g.relu = relu != 0; g.out = out;
+    const size_t sb = gemm_scratch_bytes(ctx, dt, g);
+    PS_TRY(ensure_ws(ctx, sb));
+    return run_gemm(ctx, dt, g, ctx->ws, ctx->ws_bytes, ctx->stream);
+}
+
+pinsage_status pinsage_pool(pinsage_ctx *ctx, pinsage_dtype dtype, int64_t n_dst, int64_t n_src,
+                            int32_t T, int32_t m, const void *P, const int32_t *nbr_idx,
+                            const float *nbr_w, void *n)
+{
+    if (!ctx) return PINSAGE_ERR_INVALID_ARG;
+    DeviceGuard guard(ctx->device);
+    PS_TRY(check_dtype(ctx, dtype));
+    if (n_dst < 0) return fail(ctx, PINSAGE_ERR_INVALID_ARG, "n_dst is negative");
+    PS_TRY(check_graph_args(ctx, n_src, T));
+    PS_TRY(check_dim(ctx, "m", m));
+    if (n_dst == 0) return PINSAGE_OK;
+    PS_TRY(check_ptr(ctx, "P", P));
+    PS_TRY(check_ptr(ctx, "nbr_idx", nbr_idx));
+    PS_TRY(check_ptr(ctx, "nbr_w", nbr_w));
+    PS_TRY(check_ptr(ctx, "n", n));
+    const DType dt = static_cast<DType>(dtype);
+    const size_t es = elem_size(dt);
+    if (overlaps(P, (size_t)n_src * m * es, n, (size_t)n_dst * m * es))
+        return fail(ctx, PINSAGE_ERR_INVALID_ARG, "n overlaps P");
+    PS_TRY(maybe_validate(ctx, n_dst, n_src, T, nbr_idx, nbr_w));
+    const int pe0 = prof_mark(ctx, ctx->stream);
+    cudaError_t e = launch_pool(dt, n_dst, T, m, P, nbr_idx, nbr_w, n, ctx->stream, &ctx->launches);
+    prof_close(ctx, PROF_POOL, pe0, ctx->stream);
+    count_launches(ctx);
+    if (e == cudaErrorNotSupported)
+        return fail(ctx, PINSAGE_ERR_UNSUPPORTED_SHAPE, "pool: row of %d elements is too wide", m);
+    PS_CUDA(ctx, e);
+    return PINSAGE_OK;
+}
+
+pinsage_status pinsage_combine(pinsage_ctx *ctx, pinsage_dtype dtype, int64_t M, int32_t d_in,
+                               int32_t m, int32_t d, const void *H, const void *n, const void *W,
+                               const float *w, void *out)
+{
+    if (!ctx) return PINSAGE_ERR_INVALID_ARG;
+    DeviceGuard guard(ctx->device);
+    PS_TRY(check_dtype(ctx, dtype));
+    if (M < 0) return fail(ctx, PINSAGE_ERR_INVALID_ARG, "M is negative");
+    PS_TRY(check_dim(ctx, "d_in", d_in));
+    PS_TRY(check_dim(ctx, "m", m));
+    PS_TRY(check_dim(ctx, "d", d));
+    PS_TRY(check_ptr(ctx, "H", H));
+    PS_TRY(check_ptr(ctx, "n", n));
+    PS_TRY(check_ptr(ctx, "W", W));
+    PS_TRY(check_ptr(ctx, "w", w));
+    PS_TRY(check_ptr(ctx, "out", out));
+    const DType dt = static_cast<DType>(dtype);
+    const size_t es = elem_size(dt);
+    if (out == H) {
+        if (d != d_in) return fail(ctx, PINSAGE_ERR_INVALID_ARG, "out == H requires d == d_in");
+    } else if (overlaps(H, (size_t)M * d_in * es, out, (size_t)M * d * es)) {
+        return fail(ctx, PINSAGE_ERR_INVALID_ARG, "out partially overlaps H");
+    }
+    if (overlaps(n, (size_t)M * m * es, out, (size_t)M * d * es))
+        return fail(ctx, PINSAGE_ERR_INVALID_ARG, "out overlaps n");
+    GemmArgs g;
+    g.M = M; g.K1 = d_in; g.K2 = m; g.N = d; g.A1 = H; g.A2 = n; g.B = W; g.bias = w;
+    g.relu = 1; g.l2norm = 1; g.out = out;
+    PS_TRY(ensure_ws(ctx, gemm_scratch_bytes(ctx, dt, g)));
+    return run_gemm(ctx, dt, g, ctx->ws, ctx->ws_bytes, ctx->stream);
+}
+
+size_t pinsage_layer_workspace_bytes(pinsage_dtype dtype, int64_t N, int32_t T,
+                                     const pinsage_layer_params *params)
+{
+    (void)T;
+    if (!params || N <= 0 || (dtype != PINSAGE_BF16 && dtype != PINSAGE_F32)) return 0;
+    // sized for the larger (SIMT reference) scratch so that either gemm_impl fits
+    pinsage_ctx probe;
+    probe.gemm_impl = 1;
+    const DType dt = static_cast<DType>(dtype);
+    return plan_layer_ws(&probe, dt, N, params, auto_chunk(N, 0)).total;
+}
+
+pinsage_status pinsage_layer(pinsage_ctx *ctx, pinsage_dtype dtype, int64_t N, int32_t T,
+                             const void *feats, const int32_t *nbr_idx, const float *nbr_w,
+                             const pinsage_layer_params *params, void *out, void *ws,
+                             size_t ws_bytes)
+{
+    if (!ctx) return PINSAGE_ERR_INVALID_ARG;
+    DeviceGuard guard(ctx->device);
+    PS_TRY(check_dtype(ctx, dtype));
+    PS_TRY(check_graph_args(ctx, N, T));
+    PS_TRY(check_layer_params(ctx, params, "params"));
+    PS_TRY(check_ptr(ctx, "feats", feats));
+    PS_TRY(check_ptr(ctx, "nbr_idx", nbr_idx));
+    PS_TRY(check_ptr(ctx, "nbr_w", nbr_w));
+    PS_TRY(check_ptr(ctx, "out", out));
+    const DType dt = static_cast<DType>(dtype);
+    const size_t es = elem_size(dt);
+    if (out == feats) {
+        if (params->d != params->d_in)
+            return fail(ctx, PINSAGE_ERR_INVALID_ARG, "out == feats requires d == d_in");
+    } else if (overlaps(feats, (size_t)N * params->d_in * es, out, (size_t)N * params->d * es)) {
+        return fail(ctx, PINSAGE_ERR_INVALID_ARG, "out partially overlaps feats");
+    }
+    const int64_t chunk = auto_chunk(N, 0);
+    const LayerWs plan = plan_layer_ws(ctx, dt, N, params, chunk);
+    char *base;
+    if (ws) {
+        if ((reinterpret_cast<uintptr_t>(ws) & 255u) != 0)
+            return fail(ctx, PINSAGE_ERR_MISALIGNED, "ws is not 256-byte aligned");
+        if (ws_bytes < plan.total)
+            return fail(ctx, PINSAGE_ERR_OOM, "ws_bytes = %zu < required %zu", ws_bytes, plan.total);
+        base = static_cast<char *>(ws);
+    } else {
+        PS_TRY(ensure_ws(ctx, plan.total));
+        base = static_cast<char *>(ctx->ws);
+    }
+    PS_TRY(maybe_validate(ctx, N, N, T, nbr_idx, nbr_w));
+    return layer_on_ws(ctx, dt, N, T, feats, nbr_idx, nbr_w, params, out, base, plan, chunk);
+}
+
+pinsage_status pinsage_head(pinsage_ctx *ctx, pinsage_dtype dtype, int64_t N, const void *h,
+                            const pinsage_head_params *params, void *out)
+{
+    if (!ctx) return PINSAGE_ERR_INVALID_ARG;
+    DeviceGuard guard(ctx->device);
+    PS_TRY(check_dtype(ctx, dtype));
+    if (N < 1) return fail(ctx, PINSAGE_ERR_INVALID_ARG, "N must be positive");
+    PS_TRY(check_head_params(ctx, params));
+    PS_TRY(check_ptr(ctx, "h", h));
+    PS_TRY(check_ptr(ctx, "out", out));
+    const DType dt = static_cast<DType>(dtype);
+    const size_t es = elem_size(dt);
+    if (overlaps(h, (size_t)N * params->d * es, out, (size_t)N * params->d_out * es))
+        return fail(ctx, PINSAGE_ERR_INVALID_ARG, "out overlaps h");
+    const int64_t chunk = auto_chunk(N, 0);
+    const size_t a_bytes = align_up((size_t)chunk * params->g1 * es, 256);
+    PS_TRY(ensure_ws(ctx, a_bytes));
+    for (int64_t r0 = 0; r0 < N; r0 += chunk) {
+        const int64_t rows = std::min(chunk, N - r0);
+        GemmArgs g;
+        g.M = rows; g.K1 = params->d; g.N = params->g1;
+        g.A1 = static_cast<const char *>(h) + (size_t)r0 * params->d * es;
+        g.B = params->G1; g.bias = params->g; g.relu = 1; g.out = ctx->ws;
+        PS_TRY(run_gemm(ctx, dt, g, nullptr, 0, ctx->stream));
+        GemmArgs g2;
+        g2.M = rows; g2.K1 = params->g1; g2.N = params->d_out; g2.A1 = ctx->ws; g2.B = params->G2;
+        g2.out = static_cast<char *>(out) + (size_t)r0 * params->d_out * es;
+        PS_TRY(run_gemm(ctx, dt, g2, nullptr, 0, ctx->stream));
+    }
+    return PINSAGE_OK;
+}
+
+pinsage_status pinsage_embed_all(pinsage_ctx *ctx, pinsage_dtype dtype, int64_t N, int32_t T,
+                                 int32_t K, const void *feats, const int32_t *nbr_idx,
+                                 const float *nbr_w, const pinsage_layer_params *layers,
+                                 const pinsage_head_params *head, void *out, int64_t chunk_nodes)
+{
+    if (!ctx) return PINSAGE_ERR_INVALID_ARG;
+    DeviceGuard guard(ctx->device);
+    PS_TRY(check_dtype(ctx, dtype));
+    PS_TRY(check_graph_args(ctx, N, T));
+    if (K < 1 || K > 64) return fail(ctx, PINSAGE_ERR_INVALID_ARG, "K = %d outside [1, 64]", K);
+    if (chunk_nodes < 0) return fail(ctx, PINSAGE_ERR_INVALID_ARG, "chunk_nodes is negative");
+    if (!layers) return fail(ctx, PINSAGE_ERR_INVALID_ARG, "layers is NULL");
+    for (int k = 0; k < K; ++k) {
+        PS_TRY(check_layer_params(ctx, &layers[k], "layers[k]"));
+        if (k > 0 && layers[k].d_in != layers[k - 1].d)
+            return fail(ctx, PINSAGE_ERR_INVALID_ARG, "layers[%d].d_in = %d != layers[%d].d = %d", k,
+                        layers[k].d_in, k - 1, layers[k - 1].d);
+    }
+    PS_TRY(check_head_params(ctx, head));
+    if (head->d != layers[K - 1].d)
+        return fail(ctx, PINSAGE_ERR_INVALID_ARG, "head.d = %d != layers[K-1].d = %d", head->d,
+                    layers[K - 1].d);
+    PS_TRY(check_ptr(ctx, "feats", feats));
+    PS_TRY(check_ptr(ctx, "nbr_idx", nbr_idx));
+    PS_TRY(check_ptr(ctx, "nbr_w", nbr_w));
+    PS_TRY(check_ptr(ctx, "out", out));
+    const DType dt = static_cast<DType>(dtype);
+    const size_t es = elem_size(dt);
+    const size_t feats_bytes = (size_t)N * layers[0].d_in * es;
+    const size_t tab_bytes = (size_t)N * T * 4;
+    const size_t out_bytes = (size_t)N * head->d_out * es;
+    if (overlaps(feats, feats_bytes, out, out_bytes))
+        return fail(ctx, PINSAGE_ERR_INVALID_ARG, "out overlaps feats");
+
+    // ---- host buffers: stage through context-owned device memory ------------------------------
+    const bool h_feats = is_host_ptr(feats), h_idx = is_host_ptr(nbr_idx), h_w = is_host_ptr(nbr_w);
+    const bool h_out = is_host_ptr(out);
+    const bool any_host = h_feats || h_idx || h_w || h_out;
+    size_t st_off = 0, st_feats = 0, st_idx = 0, st_w = 0, st_out = 0;
+    if (h_feats) { st_feats = st_off; st_off += align_up(feats_bytes, 256); }
+    if (h_idx) { st_idx = st_off; st_off += align_up(tab_bytes, 256); }
+    if (h_w) { st_w = st_off; st_off += align_up(tab_bytes, 256); }
+    if (h_out) { st_out = st_off; st_off += align_up(out_bytes, 256); }
+    if (any_host) PS_TRY(ensure_stage(ctx, st_off));
+    char *stage = static_cast<char *>(ctx->stage);
+    const void *d_feats = feats;
+    const int32_t *d_idx = nbr_idx;
+    const float *d_w = nbr_w;
+    void *d_out = out;
+    if (h_idx) {
+        PS_CUDA(ctx, cudaMemcpyAsync(stage + st_idx, nbr_idx, tab_bytes, cudaMemcpyHostToDevice, ctx->stream));
+        d_idx = reinterpret_cast<const int32_t *>(stage + st_idx);
+    }
+    if (h_w) {
+        PS_CUDA(ctx, cudaMemcpyAsync(stage + st_w, nbr_w, tab_bytes, cudaMemcpyHostToDevice, ctx->stream));
+        d_w = reinterpret_cast<const float *>(stage + st_w);
+    }
+    if (h_feats) {
+        PS_CUDA(ctx, cudaMemcpyAsync(stage + st_feats, feats, feats_bytes, cudaMemcpyHostToDevice, ctx->stream));
+        d_feats = stage + st_feats;
+    }
+    if (h_out) d_out = stage + st_out;
+
+    // ---- workspace plan: P | n0 | n1 | scratch | H_a | H_b | head chunk a ------------------------
+    const int64_t chunk = auto_chunk(N, chunk_nodes);
+    size_t max_layer_ws = 0;
+    int32_t d_max = 0;
+    for (int k = 0; k < K; ++k) {
+        max_layer_ws = std::max(max_layer_ws, plan_layer_ws(ctx, dt, N, &layers[k], chunk).total);
+        d_max = std::max(d_max, layers[k].d);
+    }
+    const size_t H_bytes = align_up((size_t)N * d_max * es, 256);
+    const size_t a_bytes = align_up((size_t)chunk * head->g1 * es, 256);
+    // layer k >= 2 with d == d_in runs in place on H_a; a second H buffer only when widths change
+    bool need_Hb = false;
+    for (int k = 1; k < K; ++k) need_Hb = need_Hb || layers[k].d != layers[k].d_in;
+    const size_t total = max_layer_ws + H_bytes * (need_Hb ? 2 : 1) + a_bytes;
+    PS_TRY(ensure_ws(ctx, total));
+    char *ws = static_cast<char *>(ctx->ws);
+    char *Ha = ws + max_layer_ws;
+    char *Hb = need_Hb ? Ha + H_bytes : nullptr;
+    char *abuf = Ha + H_bytes * (need_Hb ? 2 : 1);
+
+    PS_TRY(maybe_validate(ctx, N, N, T, d_idx, d_w));
+
+    const void *Hin = d_feats;
+    char *Hcur = nullptr;
+    for (int k = 0; k < K; ++k) {
+        const pinsage_layer_params *lp = &layers[k];
+        const LayerWs plan = plan_layer_ws(ctx, dt, N, lp, chunk);
+        char *Hout;
+        if (k == 0) Hout = Ha;
+        else if (lp->d == lp->d_in) Hout = Hcur;           // in place (S1 has consumed all of H first)
+        else Hout = (Hcur == Ha) ? Hb : Ha;
+        PS_TRY(layer_on_ws(ctx, dt, N, T, Hin, d_idx, d_w, lp, Hout, ws, plan, chunk));
+        Hcur = Hout;
+        Hin = Hout;
+    }
+    // ---- head, chunk by chunk (the intermediate a never exists in full) ---------------------------
+    for (int64_t r0 = 0; r0 < N; r0 += chunk) {
+        const int64_t rows = std::min(chunk, N - r0);
+        GemmArgs g;
+        g.M = rows; g.K1 = head->d; g.N = head->g1;
+        g.A1 = Hcur + (size_t)r0 * head->d * es;
+        g.B = head->G1; g.bias = head->g; g.relu = 1; g.out = abuf;
+        PS_TRY(run_gemm(ctx, dt, g, nullptr, 0, ctx->stream));
+        GemmArgs g2;
+        g2.M = rows; g2.K1 = head->g1; g2.N = head->d_out; g2.A1 = abuf; g2.B = head->G2;
+        g2.out = static_cast<char *>(d_out) + (size_t)r0 * head->d_out * es;
+        PS_TRY(run_gemm(ctx, dt, g2, nullptr, 0, ctx->stream));
+    }
+    if (h_out)
+        PS_CUDA(ctx, cudaMemcpyAsync(out, d_out, out_bytes, cudaMemcpyDeviceToHost, ctx->stream));
+    if (any_host) PS_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
+    return PINSAGE_OK;
+}
+
+pinsage_status pinsage_normalize_counts(pinsage_ctx *ctx, int64_t N, int32_t T,
+                                        const int32_t *counts, float *nbr_w)
+{
+    if (!ctx) return PINSAGE_ERR_INVALID_ARG;
+    DeviceGuard guard(ctx->device);
+    PS_TRY(check_graph_args(ctx, N, T));
+    PS_TRY(check_ptr(ctx, "counts", counts));
+    PS_TRY(check_ptr(ctx, "nbr_w", nbr_w));
+    cudaError_t e = launch_normalize_counts(N, T, counts, nbr_w, ctx->stream, &ctx->launches);
+    count_launches(ctx);
+    PS_CUDA(ctx, e);
+    return PINSAGE_OK;
+}
+
+pinsage_status pinsage_validate_graph(pinsage_ctx *ctx, int64_t n_dst, int64_t n_src, int32_t T,
+                                      const int32_t *nbr_idx, const float *nbr_w,
+                                      int64_t *first_bad)
+{
+    if (!ctx) return PINSAGE_ERR_INVALID_ARG;
+    DeviceGuard guard(ctx->device);
+    if (!first_bad) return fail(ctx, PINSAGE_ERR_INVALID_ARG, "first_bad is NULL");
+    *first_bad = -1;
+    if (n_dst < 0) return fail(ctx, PINSAGE_ERR_INVALID_ARG, "n_dst is negative");
+    PS_TRY(check_graph_args(ctx, n_src, T));
+    if (n_dst == 0) return PINSAGE_OK;
+    PS_TRY(check_ptr(ctx, "nbr_idx", nbr_idx));
+    PS_TRY(check_ptr(ctx, "nbr_w", nbr_w));
+    cudaError_t e = launch_validate(n_dst, n_src, T, nbr_idx, nbr_w, ctx->d_first_bad, ctx->stream,
+                                    &ctx->launches);
+    count_launches(ctx);
+    PS_CUDA(ctx, e);
+    long long bad = -1;
+    PS_CUDA(ctx, cudaMemcpyAsync(&bad, ctx->d_first_bad, sizeof bad, cudaMemcpyDeviceToHost, ctx->stream));
+    PS_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
+    *first_bad = bad;
+    if (bad >= 0)
+        return fail(ctx, PINSAGE_ERR_BAD_INDEX,
+                    "entry %lld (node %lld, slot %lld) has an id outside [0, %lld) or a non-finite weight",
+                    bad, bad / T, bad % T, (long long)n_src);
+    return PINSAGE_OK;
+}
+
+}  // extern "C"

@@ -1,0 +1,52 @@
+// internal.h -- declarations shared by the translation units of libpinsage.so.
+// Product code (CUDA path). Shares nothing with oracle/.
+#pragma once
+
+#include <cuda_runtime.h>
+#include <cuda_bf16.h>
+#include <stddef.h>
+#include <stdint.h>
+
+namespace pinsage {
+
+enum class DType : int { BF16 = 0, F32 = 1 };
+
+inline size_t elem_size(DType t) { return t == DType::BF16 ? 2 : 4; }
+
+// out[M x N] = epi(A1[M x K1] * B[:, 0:K1]^T + A2[M x K2] * B[:, K1:K1+K2]^T + bias)
+// B is [N x (K1+K2)] row-major ("out x in"), i.e. K-major.  K2 == 0 -> single segment.
+// epi: +bias (if non-null) -> ReLU (if relu) -> row L2 normalisation (if l2norm) -> round to dtype.
+struct GemmArgs {
+    int64_t M = 0;
+    int32_t K1 = 0, K2 = 0, N = 0;
+    const void *A1 = nullptr;
+    const void *A2 = nullptr;
+    const void *B = nullptr;
+    const float *bias = nullptr;
+    int relu = 0;
+    int l2norm = 0;
+    void *out = nullptr;
+};
+
+// ---- gemm_simt.cu: SIMT fp32-FMA GEMM (the F32 mode; also the BF16 reference kernels) ----------
+// ztmp: fp32 scratch of M*N floats, required iff l2norm (un-normalised z lives there).
+cudaError_t launch_gemm_simt(DType dt, const GemmArgs &a, float *ztmp, cudaStream_t s, int *launches);
+size_t gemm_simt_scratch_bytes(const GemmArgs &a);
+
+// ---- gemm_tcgen05.cu: tcgen05 / TMEM / TMA GEMM, bf16 in, fp32 accumulate ----------------------
+// Returns cudaErrorNotSupported for shapes outside the compiled set (caller reports UNSUPPORTED_SHAPE).
+bool gemm_tc_supported(const GemmArgs &a, const char **why);
+cudaError_t launch_gemm_tc(const GemmArgs &a, int num_sms, cudaStream_t s, int *launches);
+// scratch needed when the row norm spans more than one CTA (N > 512): per-row partial sums
+size_t gemm_tc_scratch_bytes(const GemmArgs &a);
+
+// ---- pool.cu ------------------------------------------------------------------------------------
+cudaError_t launch_pool(DType dt, int64_t n_dst, int32_t T, int32_t m, const void *P,
+                        const int32_t *idx, const float *w, void *out, cudaStream_t s, int *launches);
+cudaError_t launch_normalize_counts(int64_t N, int32_t T, const int32_t *counts, float *w,
+                                    cudaStream_t s, int *launches);
+// first_bad: device int64, set to the smallest offending flat position or -1
+cudaError_t launch_validate(int64_t n_dst, int64_t n_src, int32_t T, const int32_t *idx,
+                            const float *w, long long *first_bad, cudaStream_t s, int *launches);
+
+}  // namespace pinsage

@@ -1,0 +1,279 @@
+// pool.cu -- S2, the importance pool (PAPER.md:114 gamma, :124 "importance pooling";
+// sec. 3.4 job 2 :219):   n[v] = sum_{t<T} w[v,t] * P[idx[v,t], :]
+//
+// HBM-bound gather-weighted-sum.  A group of LPN lanes owns one destination node; every lane
+// owns CPL 16-byte chunks of the feature row and keeps their fp32 partial sums in registers.
+// The node's (id, weight) pairs are read once with a coalesced load and broadcast with warp
+// shuffles; U neighbour rows are requested before the first FMA so that U*CPL 16-byte loads
+// per lane are in flight.  The sum over t runs in table order per lane: no atomics, no
+// cross-lane reduction, bit-reproducible.  Row offsets are 64-bit.
+//
+// Also here: the L1-normalisation of visit counts and table validation.
+#include "internal.h"
+
+#include <climits>
+
+namespace pinsage {
+namespace {
+
+__device__ __forceinline__ int ld_stream_i32(const int *p)
+{
+    int v;
+    asm("ld.global.nc.L1::no_allocate.s32 %0, [%1];" : "=r"(v) : "l"(p));
+    return v;
+}
+__device__ __forceinline__ float ld_stream_f32(const float *p)
+{
+    float v;
+    asm("ld.global.nc.L1::no_allocate.f32 %0, [%1];" : "=f"(v) : "l"(p));
+    return v;
+}
+__device__ __forceinline__ uint4 ld_row16(const uint4 *p)
+{
+    uint4 v;
+    asm volatile("ld.global.nc.v4.u32 {%0, %1, %2, %3}, [%4];"
+                 : "=r"(v.x), "=r"(v.y), "=r"(v.z), "=r"(v.w)
+                 : "l"(p));
+    return v;
+}
+__device__ __forceinline__ void st_stream16(uint4 *p, const uint4 &v)
+{
+    asm volatile("st.global.cs.v4.u32 [%0], {%1, %2, %3, %4};" ::"l"(p), "r"(v.x), "r"(v.y),
+                 "r"(v.z), "r"(v.w)
+                 : "memory");
+}
+
+template <bool BF16>
+struct Chunk;
+
+template <>
+struct Chunk<true> {  // 8 bf16 per 16 bytes
+    static constexpr int E = 8;
+    static __device__ __forceinline__ void fma(const uint4 &r, float wt, float (&acc)[8])
+    {
+        const uint32_t u[4] = {r.x, r.y, r.z, r.w};
+#pragma unroll
+        for (int i = 0; i < 4; ++i) {
+            acc[2 * i] = fmaf(wt, __uint_as_float(u[i] << 16), acc[2 * i]);
+            acc[2 * i + 1] = fmaf(wt, __uint_as_float(u[i] & 0xffff0000u), acc[2 * i + 1]);
+        }
+    }
+    static __device__ __forceinline__ uint4 pack(const float (&acc)[8])
+    {
+        uint32_t u[4];
+#pragma unroll
+        for (int i = 0; i < 4; ++i) {
+            __nv_bfloat162 b = __floats2bfloat162_rn(acc[2 * i], acc[2 * i + 1]);
+            u[i] = *reinterpret_cast<uint32_t *>(&b);
+        }
+        return make_uint4(u[0], u[1], u[2], u[3]);
+    }
+};
+
+template <>
+struct Chunk<false> {  // 4 fp32 per 16 bytes
+    static constexpr int E = 4;
+    static __device__ __forceinline__ void fma(const uint4 &r, float wt, float (&acc)[4])
+    {
+        acc[0] = fmaf(wt, __uint_as_float(r.x), acc[0]);
+        acc[1] = fmaf(wt, __uint_as_float(r.y), acc[1]);
+        acc[2] = fmaf(wt, __uint_as_float(r.z), acc[2]);
+        acc[3] = fmaf(wt, __uint_as_float(r.w), acc[3]);
+    }
+    static __device__ __forceinline__ uint4 pack(const float (&acc)[4])
+    {
+        return make_uint4(__float_as_uint(acc[0]), __float_as_uint(acc[1]),
+                          __float_as_uint(acc[2]), __float_as_uint(acc[3]));
+    }
+};
+
+// UU neighbour rows (slots j0 .. j0+UU-1 of the current batch) for one lane: every one of the
+// UU*CPL 16-byte loads is issued before the first FMA (memory-level parallelism).
+template <bool BF16, int LPN, int CPL, int UU, bool EXACT>
+__device__ __forceinline__ void gather_fma(const uint4 *__restrict__ P, int my_i, float my_w, int j0,
+                                           int sl, int chunks,
+                                           float (&acc)[CPL][Chunk<BF16>::E])
+{
+    using C = Chunk<BF16>;
+    uint4 r[UU][CPL];
+    float wt[UU];
+    const uint4 *row[UU];
+#pragma unroll
+    for (int u = 0; u < UU; ++u) {
+        const int id = __shfl_sync(0xffffffffu, my_i, j0 + u, LPN);
+        wt[u] = __shfl_sync(0xffffffffu, my_w, j0 + u, LPN);
+        row[u] = P + (size_t)id * (size_t)chunks + sl;
+    }
+#pragma unroll
+    for (int u = 0; u < UU; ++u)
+#pragma unroll
+        for (int c = 0; c < CPL; ++c) {
+            if (EXACT) r[u][c] = ld_row16(row[u] + c * LPN);
+            else r[u][c] = (sl + c * LPN < chunks) ? ld_row16(row[u] + c * LPN) : make_uint4(0, 0, 0, 0);
+        }
+#pragma unroll
+    for (int u = 0; u < UU; ++u)
+#pragma unroll
+        for (int c = 0; c < CPL; ++c) C::fma(r[u][c], wt[u], acc[c]);
+}
+
+// LPN lanes per node (4..32), CPL chunks per lane, U neighbour rows in flight,
+// EXACT: the row is exactly LPN*CPL chunks wide (no per-chunk guard).
+// An explicit minBlocksPerSM matters: without it ptxas (-O3) re-serialises the load batch to
+// minimise registers (32 regs, 2 loads in flight); with it the U*CPL loads stay batched.
+template <bool BF16, int LPN, int CPL, int U, bool EXACT>
+__global__ void __launch_bounds__(256, (CPL <= 2) ? 4 : 2)
+pool_kernel(const uint4 *__restrict__ P, const int *__restrict__ idx, const float *__restrict__ w,
+            uint4 *__restrict__ out, long long n_dst, int T, int chunks)
+{
+    using C = Chunk<BF16>;
+    constexpr int NPW = 32 / LPN;
+    static_assert(LPN % U == 0, "U must divide LPN");
+    const int lane = threadIdx.x & 31;
+    const int sl = lane % LPN;
+    const long long warp = (long long)blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5);
+    const long long v_raw = warp * NPW + lane / LPN;
+    if (warp * NPW >= n_dst) return;                       // whole warp out of range
+    const bool active = v_raw < n_dst;
+    const long long v = active ? v_raw : n_dst - 1;        // idle groups shadow the last node
+
+    float acc[CPL][C::E];
+#pragma unroll
+    for (int c = 0; c < CPL; ++c)
+#pragma unroll
+        for (int e = 0; e < C::E; ++e) acc[c][e] = 0.f;
+
+    const int *irow = idx + v * T;
+    const float *wrow = w + v * T;
+    for (int tb = 0; tb < T; tb += LPN) {
+        const int t = tb + sl;
+        int my_i = 0;
+        float my_w = 0.f;
+        if (t < T) {
+            my_i = ld_stream_i32(irow + t);
+            my_w = ld_stream_f32(wrow + t);
+        }
+        const int cnt = min(LPN, T - tb);
+        int j0 = 0;
+        for (; j0 + U <= cnt; j0 += U)
+            gather_fma<BF16, LPN, CPL, U, EXACT>(P, my_i, my_w, j0, sl, chunks, acc);
+        for (; j0 < cnt; ++j0)
+            gather_fma<BF16, LPN, CPL, 1, EXACT>(P, my_i, my_w, j0, sl, chunks, acc);
+    }
+    if (active) {
+        uint4 *orow = out + (size_t)v * (size_t)chunks;
+#pragma unroll
+        for (int c = 0; c < CPL; ++c) {
+            const int ch = sl + c * LPN;
+            if (EXACT || ch < chunks) st_stream16(orow + ch, C::pack(acc[c]));
+        }
+    }
+}
+
+template <bool BF16, int LPN, int CPL, int U>
+cudaError_t run_pool(const void *P, const int *idx, const float *w, void *out, long long n_dst,
+                     int T, int chunks, cudaStream_t s)
+{
+    constexpr int NPW = 32 / LPN;
+    const long long warps = (n_dst + NPW - 1) / NPW;
+    const long long blocks = (warps + 7) / 8;
+    if (blocks > 0x7fffffffLL) return cudaErrorInvalidConfiguration;
+    if (chunks == LPN * CPL)
+        pool_kernel<BF16, LPN, CPL, U, true><<<(unsigned)blocks, 256, 0, s>>>(
+            static_cast<const uint4 *>(P), idx, w, static_cast<uint4 *>(out), n_dst, T, chunks);
+    else
+        pool_kernel<BF16, LPN, CPL, U, false><<<(unsigned)blocks, 256, 0, s>>>(
+            static_cast<const uint4 *>(P), idx, w, static_cast<uint4 *>(out), n_dst, T, chunks);
+    return cudaGetLastError();
+}
+
+template <bool BF16>
+cudaError_t dispatch_pool(const void *P, const int *idx, const float *w, void *out,
+                          long long n_dst, int T, int chunks, cudaStream_t s)
+{
+    if (chunks <= 4) return run_pool<BF16, 4, 1, 4>(P, idx, w, out, n_dst, T, chunks, s);
+    if (chunks <= 8) return run_pool<BF16, 8, 1, 8>(P, idx, w, out, n_dst, T, chunks, s);
+    if (chunks <= 16) return run_pool<BF16, 16, 1, 8>(P, idx, w, out, n_dst, T, chunks, s);
+    if (chunks <= 32) return run_pool<BF16, 32, 1, 8>(P, idx, w, out, n_dst, T, chunks, s);
+    if (chunks <= 64) return run_pool<BF16, 32, 2, 4>(P, idx, w, out, n_dst, T, chunks, s);
+    if (chunks <= 128) return run_pool<BF16, 32, 4, 2>(P, idx, w, out, n_dst, T, chunks, s);
+    if (chunks <= 256) return run_pool<BF16, 32, 8, 1>(P, idx, w, out, n_dst, T, chunks, s);
+    return cudaErrorNotSupported;
+}
+
+// One warp per row: alpha = (float)c / (float)sum(c), IEEE binary32 division.
+__global__ void __launch_bounds__(256)
+normalize_counts_kernel(const int *__restrict__ counts, float *__restrict__ w, long long N, int T)
+{
+    const long long row = (long long)blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5);
+    if (row >= N) return;
+    const int lane = threadIdx.x & 31;
+    const int *c = counts + row * T;
+    long long tot = 0;
+    for (int t = lane; t < T; t += 32) tot += c[t];
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) tot += __shfl_xor_sync(0xffffffffu, tot, o);
+    const float ftot = (float)tot;
+    for (int t = lane; t < T; t += 32) w[row * T + t] = __fdiv_rn((float)c[t], ftot);
+}
+
+__global__ void __launch_bounds__(256)
+validate_kernel(const int *__restrict__ idx, const float *__restrict__ w, long long total,
+                long long n_src, long long *first_bad)
+{
+    long long best = LLONG_MAX;
+    for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < total;
+         i += (long long)gridDim.x * blockDim.x) {
+        const int id = idx[i];
+        const float x = w[i];
+        if (id < 0 || id >= n_src || !isfinite(x)) {
+            best = i;
+            break;
+        }
+    }
+    if (best != LLONG_MAX) atomicMin(first_bad, best);
+}
+
+__global__ void set_ll(long long *p, long long v) { *p = v; }
+__global__ void fix_first_bad(long long *p)
+{
+    if (*p == LLONG_MAX) *p = -1;
+}
+
+}  // namespace
+
+cudaError_t launch_pool(DType dt, int64_t n_dst, int32_t T, int32_t m, const void *P,
+                        const int32_t *idx, const float *w, void *out, cudaStream_t s, int *launches)
+{
+    if (n_dst <= 0) return cudaSuccess;
+    const int chunks = (int)((size_t)m * elem_size(dt) / 16);
+    if (launches) ++*launches;
+    return dt == DType::BF16 ? dispatch_pool<true>(P, idx, w, out, n_dst, T, chunks, s)
+                             : dispatch_pool<false>(P, idx, w, out, n_dst, T, chunks, s);
+}
+
+cudaError_t launch_normalize_counts(int64_t N, int32_t T, const int32_t *counts, float *w,
+                                    cudaStream_t s, int *launches)
+{
+    const long long blocks = (N + 7) / 8;
+    if (blocks > 0x7fffffffLL) return cudaErrorInvalidConfiguration;
+    normalize_counts_kernel<<<(unsigned)blocks, 256, 0, s>>>(counts, w, N, T);
+    if (launches) ++*launches;
+    return cudaGetLastError();
+}
+
+cudaError_t launch_validate(int64_t n_dst, int64_t n_src, int32_t T, const int32_t *idx,
+                            const float *w, long long *first_bad, cudaStream_t s, int *launches)
+{
+    const long long total = n_dst * (long long)T;
+    set_ll<<<1, 1, 0, s>>>(first_bad, LLONG_MAX);
+    long long blocks = (total + 255) / 256;
+    if (blocks > 148 * 16) blocks = 148 * 16;
+    if (blocks < 1) blocks = 1;
+    validate_kernel<<<(unsigned)blocks, 256, 0, s>>>(idx, w, total, n_src, first_bad);
+    fix_first_bad<<<1, 1, 0, s>>>(first_bad);
+    if (launches) *launches += 3;
+    return cudaGetLastError();
+}
+
+}  // namespace pinsage

@@ -1,0 +1,371 @@
+"""Parity tests proper: the CUDA path (through the C-ABI binding) against the fp64 CPU oracle,
+element by element on the same seeded inputs.  Integer / index work is bit-exact; floating
+point is within north_star's tolerances (tests/parity.py)."""
+import numpy as np
+import pytest
+import torch
+
+from oracle import oracle as O
+from paper_1806_01973_b200 import binding, synth
+from tests.parity import assert_rows_close, params_f64, row_errors, to_f64
+
+pytestmark = pytest.mark.gpu
+
+DEV = "cuda:0"
+DTYPES = [torch.bfloat16, torch.float32]
+
+
+@pytest.fixture(scope="module")
+def ctx():
+    c = binding.Context(0)
+    yield c
+    c.close()
+
+
+def _rand(shape, dtype, seed, scale=1.0):
+    g = torch.Generator().manual_seed(seed)
+    return (torch.randn(shape, generator=g) * scale).to(dtype)
+
+
+def _graph(N, T, seed, n_src=None):
+    g = torch.Generator().manual_seed(seed)
+    idx = torch.randint(0, n_src or N, (N, T), generator=g, dtype=torch.int32)
+    counts = torch.randint(1, 101, (N, T), generator=g, dtype=torch.int32)
+    return idx, counts
+
+
+def _both_impls(ctx, dtype):
+    """bf16 runs through the tcgen05 kernels and through the SIMT reference kernels."""
+    return [0, 1] if dtype == torch.bfloat16 else [0]
+
+
+# ------------------------------------------------------------------ helpers of the path
+def test_normalize_counts_bit_exact(ctx):
+    for N, T in [(1, 1), (1000, 50), (777, 100), (33, 7)]:
+        _, counts = _graph(N, T, 5)
+        got = ctx.pinsage_normalize_counts(counts.to(DEV)).cpu().numpy()
+        np.testing.assert_array_equal(got, O.normalize_counts(counts.numpy()))
+
+
+def test_validate_graph(ctx):
+    idx, counts = _graph(500, 20, 6)
+    w = torch.from_numpy(O.normalize_counts(counts.numpy()))
+    assert ctx.pinsage_validate_graph(idx.to(DEV), w.to(DEV), 500) == -1
+    bad = idx.clone()
+    bad[123, 7] = 500
+    bad[400, 0] = -1
+    with pytest.raises(binding.PinsageError) as e:
+        ctx.pinsage_validate_graph(bad.to(DEV), w.to(DEV), 500)
+    assert e.value.status_name == "BAD_INDEX" and ctx.first_bad == 123 * 20 + 7
+    wb = w.clone()
+    wb[9, 3] = float("nan")
+    with pytest.raises(binding.PinsageError):
+        ctx.pinsage_validate_graph(idx.to(DEV), wb.to(DEV), 500)
+    assert ctx.first_bad == 9 * 20 + 3
+
+
+# ------------------------------------------------------------------ S2 pool
+def _encode_rows(n, m, dtype):
+    """Row i holds the base-128 digits of i in columns 0..3 (exact in bf16), zeros elsewhere."""
+    i = torch.arange(n, dtype=torch.int64)
+    P = torch.zeros((n, m), dtype=torch.float32)
+    for c in range(4):
+        P[:, c] = ((i >> (7 * c)) & 127).to(torch.float32)
+    return P.to(dtype)
+
+
+@pytest.mark.parametrize("dtype", DTYPES)
+def test_pool_index_handling_bit_exact(ctx, dtype):
+    """Exact arithmetic gather: T=1 decodes to the id; T=4 with alpha=1/4 sums exactly."""
+    n_src, m, n_dst = 300_000, 16, 5000
+    P = _encode_rows(n_src, m, dtype).to(DEV)
+    g = torch.Generator().manual_seed(7)
+    idx = torch.randint(0, n_src, (n_dst, 1), generator=g, dtype=torch.int32)
+    idx[0, 0], idx[1, 0], idx[2, 0] = 0, n_src - 1, 2    # first row, last row
+    w = torch.ones((n_dst, 1), dtype=torch.float32)
+    out = ctx.pinsage_pool(P, idx.to(DEV), w.to(DEV)).cpu().to(torch.float32)
+    dec = sum(out[:, c].to(torch.int64) << (7 * c) for c in range(4))
+    assert torch.equal(dec, idx[:, 0].to(torch.int64))
+    assert torch.equal(out[:, 4:], torch.zeros_like(out[:, 4:]))
+    # T = 4, alpha = 0.25, with self / repeated ids: sums of <= 4*127 quarter-integers are exact
+    idx4 = torch.randint(0, n_src, (n_dst, 4), generator=g, dtype=torch.int32)
+    idx4[5] = idx4[5, 0]                                    # repeated ids are legal (A7)
+    w4 = torch.full((n_dst, 4), 0.25, dtype=torch.float32)
+    out4 = ctx.pinsage_pool(P, idx4.to(DEV), w4.to(DEV)).cpu()
+    ref = O.pool(to_f64(P), idx4.numpy(), w4.numpy())
+    exp = torch.from_numpy(ref).to(dtype)                   # exact values; bf16 rounds them once
+    assert torch.equal(out4.view(torch.int16 if dtype == torch.bfloat16 else torch.int32),
+                       exp.view(torch.int16 if dtype == torch.bfloat16 else torch.int32))
+
+
+def test_pool_large_ids_and_64bit_offsets(ctx):
+    """ids > 2^24 (a float-cast id would break) and a P larger than 2^32 bytes (32-bit
+    offset arithmetic would break): n_src = 17M rows of 128 bf16 = 4.35 GB."""
+    n_src, m, n_dst = 17_000_000, 128, 4096
+    P = torch.zeros((n_src, m), dtype=torch.bfloat16, device=DEV)
+    i = torch.arange(n_src, dtype=torch.int64, device=DEV)
+    for c in range(4):
+        P[:, c] = ((i >> (7 * c)) & 127).to(torch.bfloat16)
+    del i
+    g = torch.Generator().manual_seed(8)
+    idx = torch.randint(0, n_src, (n_dst, 1), generator=g, dtype=torch.int32)
+    idx[0, 0], idx[1, 0], idx[2, 0] = n_src - 1, (1 << 24) + 1, (1 << 32) // (m * 2) + 3
+    idx[3, 0], idx[4, 0] = (1 << 32) // (m * 2) - 1, (1 << 32) // (m * 2)
+    w = torch.ones((n_dst, 1), dtype=torch.float32)
+    out = ctx.pinsage_pool(P, idx.to(DEV), w.to(DEV)).cpu().to(torch.float32)
+    dec = sum(out[:, c].to(torch.int64) << (7 * c) for c in range(4))
+    assert torch.equal(dec, idx[:, 0].to(torch.int64))
+
+
+@pytest.mark.parametrize("dtype", DTYPES)
+@pytest.mark.parametrize("n_dst,n_src,T,m", [
+    (1, 1, 1, 8), (257, 300, 3, 8), (1000, 1000, 10, 64), (3001, 2000, 50, 256),
+    (515, 4000, 100, 256), (300, 900, 50, 512), (130, 500, 20, 1024), (77, 300, 7, 2048),
+    (999, 999, 33, 24), (640, 640, 50, 192), (200, 200, 5, 320),
+])
+def test_pool_matches_oracle(ctx, dtype, n_dst, n_src, T, m):
+    if dtype == torch.float32 and m > 1024:
+        pytest.skip("fp32 rows above 4 KB are outside the compiled set")
+    P = _rand((n_src, m), dtype, 10 + m)
+    idx, counts = _graph(n_dst, T, 11 + T, n_src=n_src)
+    w = O.normalize_counts(counts.numpy())
+    got = ctx.pinsage_pool(P.to(DEV), idx.to(DEV), torch.from_numpy(w).to(DEV))
+    ref = O.pool(to_f64(P), idx.numpy(), w)
+    # one rounding of an fp32 sum: 2^-9 relative per element in bf16
+    assert_rows_close(to_f64(got), ref, dtype, f"pool {dtype} T={T} m={m}",
+                      tol=3e-3 if dtype == torch.bfloat16 else 2e-6)
+
+
+def test_pool_is_deterministic_and_order_invariant_within_tolerance(ctx):
+    P = _rand((5000, 256), torch.bfloat16, 12).to(DEV)
+    idx, counts = _graph(4000, 50, 13, n_src=5000)
+    w = torch.from_numpy(O.normalize_counts(counts.numpy()))
+    a = ctx.pinsage_pool(P, idx.to(DEV), w.to(DEV))
+    b = ctx.pinsage_pool(P, idx.to(DEV), w.to(DEV))
+    assert torch.equal(a.view(torch.int16), b.view(torch.int16))
+    perm = torch.stack([torch.randperm(50) for _ in range(4000)])
+    c = ctx.pinsage_pool(P, torch.gather(idx, 1, perm).to(DEV), torch.gather(w, 1, perm).to(DEV))
+    rel, _ = row_errors(to_f64(c), to_f64(a))
+    assert rel.max() < 5e-3
+
+
+# ------------------------------------------------------------------ S1 / S4 / S5 dense
+DENSE_SHAPES = [(1, 8, 8), (130, 64, 64), (1000, 256, 256), (777, 256, 128), (300, 2048, 1024),
+                (515, 512, 512), (129, 1024, 1024), (257, 24, 40), (64, 512, 256), (4100, 128, 256)]
+
+
+@pytest.mark.parametrize("dtype", DTYPES)
+@pytest.mark.parametrize("M,k,n_out", DENSE_SHAPES)
+def test_dense_matches_oracle(ctx, dtype, M, k, n_out):
+    A = _rand((M, k), dtype, 20)
+    Wt = _rand((n_out, k), dtype, 21, scale=k ** -0.5)
+    b = _rand((n_out,), torch.float32, 22, scale=0.1)
+    for impl in _both_impls(ctx, dtype):
+        ctx.pinsage_set_option("gemm_impl", impl)
+        try:
+            for bias, relu in [(b, True), (None, False), (b, False)]:
+                try:
+                    got = ctx.pinsage_dense(A.to(DEV), Wt.to(DEV),
+                                            None if bias is None else bias.to(DEV), relu)
+                except binding.PinsageError as e:
+                    if e.status_name == "UNSUPPORTED_SHAPE" and impl == 0:
+                        pytest.skip(f"tcgen05 path does not cover this shape: {e}")
+                    raise
+                ref = O.dense(to_f64(A), to_f64(Wt), None if bias is None else to_f64(bias), relu)
+                # absolute comparison per row against the row scale (ReLU rows can be tiny)
+                err = np.abs(to_f64(got) - ref).max(axis=1)
+                scale = np.abs(ref).max(axis=1) + 1e-3
+                tol = 8e-3 if dtype == torch.bfloat16 else 2e-5
+                assert (err / scale).max() < tol, (impl, relu, (err / scale).max())
+        finally:
+            ctx.pinsage_set_option("gemm_impl", 0)
+
+
+# ------------------------------------------------------------------ S3 combine
+@pytest.mark.parametrize("dtype", DTYPES)
+@pytest.mark.parametrize("M,d_in,m,d", [(1, 8, 8, 8), (130, 64, 64, 64), (1000, 256, 256, 256),
+                                        (515, 512, 512, 512), (300, 2048, 1024, 1024),
+                                        (257, 24, 40, 16), (129, 256, 512, 128),
+                                        (200, 1024, 1024, 1024)])
+def test_combine_matches_oracle(ctx, dtype, M, d_in, m, d):
+    H = _rand((M, d_in), dtype, 30)
+    n = _rand((M, m), dtype, 31).abs()
+    W = _rand((d, d_in + m), dtype, 32, scale=(d_in + m) ** -0.5)
+    w = _rand((d,), torch.float32, 33, scale=0.01)
+    ref = O.combine(to_f64(H), to_f64(n), to_f64(W), to_f64(w))
+    for impl in _both_impls(ctx, dtype):
+        ctx.pinsage_set_option("gemm_impl", impl)
+        try:
+            try:
+                got = ctx.pinsage_combine(H.to(DEV), n.to(DEV), W.to(DEV), w.to(DEV))
+            except binding.PinsageError as e:
+                if e.status_name == "UNSUPPORTED_SHAPE" and impl == 0:
+                    pytest.skip(f"tcgen05 path does not cover this shape: {e}")
+                raise
+            assert_rows_close(to_f64(got), ref, dtype, f"combine impl={impl}",
+                              tol=4e-3 if dtype == torch.bfloat16 else 1e-5)
+            nrm = np.linalg.norm(to_f64(got), axis=1)
+            assert np.all((np.abs(nrm - 1) < (2.0 ** -7 if dtype == torch.bfloat16 else 1e-5))
+                          | (nrm == 0))
+        finally:
+            ctx.pinsage_set_option("gemm_impl", 0)
+
+
+@pytest.mark.parametrize("dtype", DTYPES)
+def test_combine_zero_rows_stay_zero(ctx, dtype):
+    """A3: all-ReLU-dead rows give exactly 0, never NaN."""
+    M, d = 300, 64
+    H = _rand((M, d), dtype, 34).abs()
+    n = _rand((M, d), dtype, 35).abs()
+    W = -_rand((d, 2 * d), dtype, 36).abs()
+    w = torch.zeros(d)
+    got = ctx.pinsage_combine(H.to(DEV), n.to(DEV), W.to(DEV), w.to(DEV))
+    assert torch.equal(got.cpu().to(torch.float32), torch.zeros((M, d)))
+
+
+# ------------------------------------------------------------------ layers, head, whole path
+def _inputs(cfg):
+    X = synth.make_features(cfg)
+    layers, head = synth.make_params(cfg)
+    idx, counts = synth.make_graph(cfg)
+    alpha = O.normalize_counts(counts.numpy())
+    return X, idx, counts, alpha, layers, head
+
+
+def _to_dev(layers, head):
+    L = [{k: v.to(DEV) for k, v in lp.items()} for lp in layers]
+    H = {k: v.to(DEV) for k, v in head.items()}
+    return L, H
+
+
+def _check_whole_path(ctx, cfg, impl=0, chunk_nodes=0):
+    X, idx, counts, alpha, layers, head = _inputs(cfg)
+    Lf, Hf = params_f64(layers, head)
+    ref_out, ref_hidden = O.embed_all(to_f64(X), idx.numpy(), alpha, Lf, Hf, return_hidden=True)
+    Ld, Hd = _to_dev(layers, head)
+    dtype = X.dtype
+    ctx.pinsage_set_option("gemm_impl", impl)
+    try:
+        w_dev = ctx.pinsage_normalize_counts(counts.to(DEV))
+        np.testing.assert_array_equal(w_dev.cpu().numpy(), alpha)
+        # layer by layer through pinsage_layer (every intermediate H_k is checked)
+        H = X.to(DEV)
+        for k, lp in enumerate(Ld):
+            H = ctx.pinsage_layer(H, idx.to(DEV), w_dev, lp)
+            assert_rows_close(to_f64(H), ref_hidden[k], dtype, f"{cfg.name} H_{k + 1} impl={impl}")
+        out_head = ctx.pinsage_head(H, Hd)
+        assert_rows_close(to_f64(out_head), ref_out, dtype, f"{cfg.name} head impl={impl}")
+        # and in one call
+        out = ctx.pinsage_embed_all(X.to(DEV), idx.to(DEV), w_dev, Ld, Hd, chunk_nodes=chunk_nodes)
+        stats = assert_rows_close(to_f64(out), ref_out, dtype, f"{cfg.name} embed_all impl={impl}")
+        return out, stats
+    finally:
+        ctx.pinsage_set_option("gemm_impl", 0)
+
+
+def test_tiny_config_fp32_exhaustive(ctx):
+    """BASELINE config 1 in full: N=2000, fp32, every row, <= 1e-4."""
+    _check_whole_path(ctx, synth.CONFIGS["tiny"])
+
+
+@pytest.mark.parametrize("impl", [0, 1])
+def test_cfg2_small_exhaustive(ctx, impl):
+    """Config 2's shape (256/256/128, T=50, K=2, bf16) on 20 000 nodes, every row; chunked
+    so that several chunks, a ragged tail chunk and ragged GEMM tiles are exercised."""
+    _check_whole_path(ctx, synth.CONFIGS["cfg2"].scaled(20_011), impl=impl, chunk_nodes=4096)
+
+
+@pytest.mark.parametrize("name,N", [("cfg3", 3000), ("cfg4", 6000), ("cfg5", 5000)])
+def test_small_siblings_exhaustive(ctx, name, N):
+    """The "-small" siblings of configs 3-5 (same dims, T, K and value laws), every row."""
+    cfg = synth.CONFIGS[name].scaled(N)
+    try:
+        _check_whole_path(ctx, cfg, impl=0, chunk_nodes=2048)
+    except binding.PinsageError as e:
+        if e.status_name != "UNSUPPORTED_SHAPE":
+            raise
+        _check_whole_path(ctx, cfg, impl=1, chunk_nodes=2048)
+        pytest.xfail(f"tcgen05 path does not cover {name} yet (SIMT reference path is green): {e}")
+
+
+def test_embed_all_deterministic_and_overlap_invariant(ctx):
+    cfg = synth.CONFIGS["cfg2"].scaled(9000)
+    X, idx, counts, alpha, layers, head = _inputs(cfg)
+    Ld, Hd = _to_dev(layers, head)
+    w = torch.from_numpy(alpha).to(DEV)
+    a = ctx.pinsage_embed_all(X.to(DEV), idx.to(DEV), w, Ld, Hd, chunk_nodes=1024)
+    b = ctx.pinsage_embed_all(X.to(DEV), idx.to(DEV), w, Ld, Hd, chunk_nodes=1024)
+    assert torch.equal(a.view(torch.int16), b.view(torch.int16))
+    ctx.pinsage_set_option("overlap", 0)
+    try:
+        c = ctx.pinsage_embed_all(X.to(DEV), idx.to(DEV), w, Ld, Hd, chunk_nodes=3072)
+    finally:
+        ctx.pinsage_set_option("overlap", 1)
+    assert torch.equal(a.view(torch.int16), c.view(torch.int16))
+
+
+def test_embed_all_host_buffers_match_device_buffers(ctx):
+    """The e2e entry: pinned host inputs / output, copies inside the call."""
+    cfg = synth.CONFIGS["cfg2"].scaled(5000)
+    X, idx, counts, alpha, layers, head = _inputs(cfg)
+    Ld, Hd = _to_dev(layers, head)
+    w = torch.from_numpy(alpha)
+    dev = ctx.pinsage_embed_all(X.to(DEV), idx.to(DEV), w.to(DEV), Ld, Hd)
+    out_h = torch.empty((cfg.N, cfg.d_out), dtype=X.dtype).pin_memory()
+    ctx.pinsage_embed_all(X.pin_memory(), idx.pin_memory(), w.pin_memory(), Ld, Hd, out=out_h)
+    assert torch.equal(out_h.view(torch.int16), dev.cpu().view(torch.int16))
+
+
+def test_layer_in_place_and_caller_workspace(ctx):
+    cfg = synth.CONFIGS["cfg2"].scaled(3000)
+    X, idx, counts, alpha, layers, head = _inputs(cfg)
+    Ld, _ = _to_dev(layers, head)
+    w = torch.from_numpy(alpha).to(DEV)
+    H1 = ctx.pinsage_layer(X.to(DEV), idx.to(DEV), w, Ld[0])
+    ref = ctx.pinsage_layer(H1, idx.to(DEV), w, Ld[1])
+    nbytes = ctx.pinsage_layer_workspace_bytes(X.dtype, cfg.N, cfg.T, Ld[1])
+    ws = torch.empty(nbytes, dtype=torch.uint8, device=DEV)
+    inplace = H1.clone()
+    ctx.pinsage_layer(inplace, idx.to(DEV), w, Ld[1], out=inplace, ws=ws)   # d == d_in
+    assert torch.equal(inplace.view(torch.int16), ref.view(torch.int16))
+    with pytest.raises(binding.PinsageError) as e:
+        ctx.pinsage_layer(H1, idx.to(DEV), w, Ld[1], ws=ws[:1024])
+    assert e.value.status_name == "OOM"
+
+
+# ------------------------------------------------------------------ argument checking
+def test_argument_errors(ctx):
+    A = torch.zeros((16, 64), dtype=torch.bfloat16, device=DEV)
+    W = torch.zeros((64, 64), dtype=torch.bfloat16, device=DEV)
+    with pytest.raises(binding.PinsageError) as e:
+        ctx.pinsage_dense(A[:, :60].contiguous(), W[:, :60].contiguous(), None, False)
+    assert e.value.status_name == "UNSUPPORTED_SHAPE"
+    with pytest.raises(binding.PinsageError) as e:
+        ctx.pinsage_dense(A.view(-1)[4:4 + 15 * 64].view(15, 64), W, None, False)
+    assert e.value.status_name == "MISALIGNED"
+    idx = torch.zeros((16, 4), dtype=torch.int32, device=DEV)
+    w = torch.zeros((16, 4), dtype=torch.float32, device=DEV)
+    with pytest.raises(binding.PinsageError) as e:
+        ctx.pinsage_pool(A, idx, w, out=A)
+    assert e.value.status_name == "INVALID_ARG"
+    with pytest.raises(binding.PinsageError) as e:
+        ctx.pinsage_set_option("no_such_option", 1)
+    assert e.value.status_name == "INVALID_ARG"
+    lp = {"Q": W, "q": torch.zeros(64, device=DEV), "W": torch.zeros((64, 128), dtype=torch.bfloat16,
+                                                                      device=DEV),
+          "w": torch.zeros(64, device=DEV)}
+    hp = {"G1": torch.zeros((32, 32), dtype=torch.bfloat16, device=DEV),
+          "g": torch.zeros(32, device=DEV),
+          "G2": torch.zeros((32, 32), dtype=torch.bfloat16, device=DEV)}
+    with pytest.raises(binding.PinsageError) as e:       # head.d != layers[-1].d
+        ctx.pinsage_embed_all(A, idx, w, [lp], hp)
+    assert e.value.status_name == "INVALID_ARG"
+    ctx.pinsage_set_option("check_indices", 1)
+    try:
+        bad = idx.clone()
+        bad[3, 1] = 16
+        with pytest.raises(binding.PinsageError) as e:
+            ctx.pinsage_pool(A, bad, w)
+        assert e.value.status_name == "BAD_INDEX"
+    finally:
+        ctx.pinsage_set_option("check_indices", 0)
