@@ -131,9 +131,10 @@ def test_pool_matches_oracle(ctx, dtype, n_dst, n_src, T, m):
     w = O.normalize_counts(counts.numpy())
     got = ctx.pinsage_pool(P.to(DEV), idx.to(DEV), torch.from_numpy(w).to(DEV))
     ref = O.pool(to_f64(P), idx.numpy(), w)
-    # one rounding of an fp32 sum: 2^-9 relative per element in bf16
+    # one RNE rounding of an fp32 sum: unit roundoff u = 2^-8 per element in bf16 (8-bit
+    # significand), so a row's relative L2 error is at most u = 3.91e-3 (+ fp32 sum error)
     assert_rows_close(to_f64(got), ref, dtype, f"pool {dtype} T={T} m={m}",
-                      tol=3e-3 if dtype == torch.bfloat16 else 2e-6)
+                      tol=4e-3 if dtype == torch.bfloat16 else 2e-6)
 
 
 def test_pool_is_deterministic_and_order_invariant_within_tolerance(ctx):
