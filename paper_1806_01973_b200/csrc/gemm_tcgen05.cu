@@ -1,7 +1,598 @@
-// placeholder: replaced by the tcgen05 kernels
+// gemm_tcgen05.cu -- S1 / S3 / S4 / S5 on the 5th-generation tensor cores (sm_100a).
+//
+//   out[M x N] = epi( A1[M x K1] * B[:, 0:K1]^T  +  A2[M x K2] * B[:, K1:K1+K2]^T  + bias )
+//
+// bf16 operands, fp32 accumulation in TMEM.  B is the paper's "out x in" weight matrix
+// (Q, W, G1, G2 -- PAPER.md:114-115, :166) = a K-major operand as it lies in memory; the
+// concat [h ; n] of Alg. 1 l.2 (:115) is never materialised: its two halves are two K segments
+// that accumulate into the same TMEM tile.  Epilogue, fused, all in fp32 before the single
+// rounding to bf16: + bias -> ReLU -> (S3) row L2 normalisation (Alg. 1 l.3, :116).
+//
+// Structure (one persistent CTA per SM, 256 threads, warp-specialised):
+//   warp 0      TMA producer: 128x64 A tile + (NS x 64) B tile per stage, SWIZZLE_128B, mbarrier ring
+//   warp 1      MMA issuer: one elected thread issues tcgen05.mma (M=128, N=CN<=256, K=16)
+//   warp 2      TMEM allocator
+//   warps 4-7   epilogue: tcgen05.ld (each thread owns one output row) -> bias/ReLU/norm ->
+//               bf16 -> swizzled smem staging -> TMA store (clips the ragged M / N tails)
+// Accumulators are double-buffered in TMEM when a row tile needs <= 256 columns, so the
+// epilogue of tile i overlaps the MMAs of tile i+1.  A thread owns a whole output row, so the
+// row norm needs no cross-thread reduction as long as one CTA holds all N columns (N <= 512);
+// wider rows (N <= 4096) are split over a thread-block cluster along N whose CTAs exchange
+// per-row partial sums of squares through distributed shared memory.
 #include "internal.h"
+
+#include <cuda.h>  // CUtensorMap and enums only; cuTensorMapEncodeTiled is fetched at run time
+
 namespace pinsage {
-bool gemm_tc_supported(const GemmArgs &, const char **why) { if (why) *why = "tcgen05 GEMM not built yet"; return false; }
-cudaError_t launch_gemm_tc(const GemmArgs &, int, cudaStream_t, int *) { return cudaErrorNotSupported; }
-size_t gemm_tc_scratch_bytes(const GemmArgs &) { return 0; }
+namespace {
+
+constexpr int BM = 128;                  // rows per tile = TMEM lanes
+constexpr int BK = 64;                   // K elements per stage: 128 bytes = one SWIZZLE_128B atom
+constexpr int A_BYTES = BM * BK * 2;     // 16 KB
+constexpr int OUT_CHUNK = 64;            // columns per output staging chunk / TMA store box
+constexpr int STG_WARP_BYTES = 32 * OUT_CHUNK * 2;  // 4 KB: 32 rows x 128 B
+constexpr int NUM_THREADS = 256;
+constexpr int MAX_STAGES = 8;
+constexpr int MAX_CLUSTER = 8;
+constexpr int SMEM_LIMIT = 227 * 1024;
+
+struct TcParams {
+    long long M;
+    long long m_blocks;
+    int kb1, kb2;      // 64-wide K blocks in segment 1 / 2
+    int K1;            // column of B where segment 2 starts
+    int N;             // output columns in total
+    int NS;            // output columns owned by one CTA (a slab)
+    int CN;            // N of one tcgen05.mma (multiple of 16, <= 256)
+    int nchunks;       // MMAs side by side per K step: nchunks * CN >= NS
+    int nacc;          // accumulators in TMEM (2 = epilogue overlaps the next tile's MMAs)
+    int acc_cols;      // TMEM columns between accumulators = nchunks * CN rounded up to 64
+    int tmem_cols;     // allocation (power of two >= 32)
+    int stages;
+    int stage_bytes;   // A_BYTES + nchunks * CN * 128
+    int n_slabs;       // slabs along N (= cluster size when l2norm spans several CTAs)
+    int cluster;       // 1, or n_slabs when the row norm is exchanged through DSMEM
+    const float *bias;
+    int relu, l2norm;
+    uint32_t idesc;
+};
+
+// ---- PTX wrappers ------------------------------------------------------------------------------
+__device__ __forceinline__ uint32_t smem_u32(const void *p)
+{
+    return static_cast<uint32_t>(__cvta_generic_to_shared(p));
 }
+__device__ __forceinline__ void mbar_init(uint32_t bar, uint32_t count)
+{
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(bar), "r"(count) : "memory");
+}
+__device__ __forceinline__ void mbar_expect_tx(uint32_t bar, uint32_t bytes)
+{
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes)
+                 : "memory");
+}
+__device__ __forceinline__ void mbar_arrive(uint32_t bar)
+{
+    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(bar) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity)
+{
+    uint32_t done;
+    do {
+        asm volatile(
+            "{\n\t.reg .pred p;\n\t"
+            "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\t"
+            "selp.u32 %0, 1, 0, p;\n\t}"
+            : "=r"(done)
+            : "r"(bar), "r"(parity)
+            : "memory");
+    } while (!done);
+}
+// cluster-scope acquire for the row-norm exchange (peers release with mbar_arrive_remote)
+__device__ __forceinline__ void mbar_wait_cluster(uint32_t bar, uint32_t parity)
+{
+    uint32_t done;
+    do {
+        asm volatile(
+            "{\n\t.reg .pred p;\n\t"
+            "mbarrier.try_wait.parity.acquire.cluster.shared::cta.b64 p, [%1], %2;\n\t"
+            "selp.u32 %0, 1, 0, p;\n\t}"
+            : "=r"(done)
+            : "r"(bar), "r"(parity)
+            : "memory");
+    } while (!done);
+}
+__device__ __forceinline__ uint32_t map_to_cta(uint32_t local_addr, uint32_t cta_rank)
+{
+    uint32_t r;
+    asm volatile("mapa.shared::cluster.u32 %0, %1, %2;" : "=r"(r) : "r"(local_addr), "r"(cta_rank));
+    return r;
+}
+__device__ __forceinline__ void st_cluster_f32(uint32_t cluster_addr, float v)
+{
+    asm volatile("st.shared::cluster.f32 [%0], %1;" ::"r"(cluster_addr), "f"(v) : "memory");
+}
+__device__ __forceinline__ void mbar_arrive_remote(uint32_t cluster_addr)
+{
+    asm volatile("mbarrier.arrive.release.cluster.shared::cluster.b64 _, [%0];" ::"r"(cluster_addr)
+                 : "memory");
+}
+__device__ __forceinline__ uint32_t cluster_ctarank()
+{
+    uint32_t r;
+    asm volatile("mov.u32 %0, %%cluster_ctarank;" : "=r"(r));
+    return r;
+}
+__device__ __forceinline__ void cluster_sync_all()
+{
+    // non-.aligned forms: the role branches leave single lanes diverged from their warps
+    asm volatile("barrier.cluster.arrive.release;\n\tbarrier.cluster.wait.acquire;" ::: "memory");
+}
+
+__device__ __forceinline__ void tma_load_2d(uint32_t dst, const CUtensorMap *map, int c0, int c1,
+                                            uint32_t bar, uint64_t policy)
+{
+    asm volatile(
+        "cp.async.bulk.tensor.2d.shared::cluster.global.tile.mbarrier::complete_tx::bytes.L2::cache_hint"
+        " [%0], [%1, {%2, %3}], [%4], %5;" ::"r"(dst),
+        "l"(map), "r"(c0), "r"(c1), "r"(bar), "l"(policy)
+        : "memory");
+}
+__device__ __forceinline__ void tma_store_2d(const CUtensorMap *map, int c0, int c1, uint32_t src)
+{
+    asm volatile("cp.async.bulk.tensor.2d.global.shared::cta.tile.bulk_group [%0, {%1, %2}], [%3];" ::"l"(map),
+                 "r"(c0), "r"(c1), "r"(src)
+                 : "memory");
+}
+__device__ __forceinline__ void tma_store_commit()
+{
+    asm volatile("cp.async.bulk.commit_group;" ::: "memory");
+}
+template <int N>
+__device__ __forceinline__ void tma_store_wait_read()
+{
+    asm volatile("cp.async.bulk.wait_group.read %0;" ::"n"(N) : "memory");
+}
+__device__ __forceinline__ void tma_store_wait_all()
+{
+    asm volatile("cp.async.bulk.wait_group 0;" ::: "memory");
+}
+__device__ __forceinline__ void fence_proxy_async()
+{
+    asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+}
+__device__ __forceinline__ void tc_fence_before()
+{
+    asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
+}
+__device__ __forceinline__ void tc_fence_after()
+{
+    asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+}
+__device__ __forceinline__ void tc_commit(uint32_t bar)
+{
+    asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" ::"r"(bar)
+                 : "memory");
+}
+__device__ __forceinline__ void tc_mma(uint32_t d_tmem, uint64_t adesc, uint64_t bdesc, uint32_t idesc,
+                                       uint32_t accumulate)
+{
+    asm volatile(
+        "{\n\t.reg .pred p;\n\t"
+        "setp.ne.b32 p, %4, 0;\n\t"
+        "tcgen05.mma.cta_group::1.kind::f16 [%0], %1, %2, %3, p;\n\t}" ::"r"(d_tmem),
+        "l"(adesc), "l"(bdesc), "r"(idesc), "r"(accumulate)
+        : "memory");
+}
+// 32 consecutive fp32 columns of this thread's TMEM lane
+__device__ __forceinline__ void tc_ld32(uint32_t taddr, uint32_t (&v)[32])
+{
+    asm volatile(
+        "tcgen05.ld.sync.aligned.32x32b.x32.b32 "
+        "{%0, %1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15, "
+        "%16, %17, %18, %19, %20, %21, %22, %23, %24, %25, %26, %27, %28, %29, %30, %31}, [%32];"
+        : "=r"(v[0]), "=r"(v[1]), "=r"(v[2]), "=r"(v[3]), "=r"(v[4]), "=r"(v[5]), "=r"(v[6]),
+          "=r"(v[7]), "=r"(v[8]), "=r"(v[9]), "=r"(v[10]), "=r"(v[11]), "=r"(v[12]), "=r"(v[13]),
+          "=r"(v[14]), "=r"(v[15]), "=r"(v[16]), "=r"(v[17]), "=r"(v[18]), "=r"(v[19]), "=r"(v[20]),
+          "=r"(v[21]), "=r"(v[22]), "=r"(v[23]), "=r"(v[24]), "=r"(v[25]), "=r"(v[26]), "=r"(v[27]),
+          "=r"(v[28]), "=r"(v[29]), "=r"(v[30]), "=r"(v[31])
+        : "r"(taddr)
+        : "memory");
+}
+__device__ __forceinline__ void tc_wait_ld()
+{
+    asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
+}
+
+// K-major, SWIZZLE_128B shared-memory matrix descriptor: rows of 128 bytes, 8-row groups 1024 bytes
+// apart (SBO), descriptor version 1 (sm_100), start address in 16-byte units.
+__device__ __forceinline__ uint64_t make_desc(uint32_t saddr)
+{
+    return static_cast<uint64_t>((saddr & 0x3FFFFu) >> 4) | (1ull << 16) | (64ull << 32) |
+           (1ull << 46) | (2ull << 61);
+}
+
+// Shared-memory plan (offsets from the 1024-byte aligned dynamic base):
+//   [0, stages*stage_bytes)   operand ring: per stage A (16 KB) then B (nchunks*CN rows x 128 B)
+//   + 32 KB                   output staging: 4 epilogue warps x 2 buffers x (32 rows x 128 B)
+//   + 2 KB                    bias of this CTA's slab (fp32, zero beyond N)
+//   + 256 B                   mbarriers, TMEM base address
+//   + 8 KB (cluster > 1)      row-norm exchange [2][MAX_CLUSTER][128] fp32
+constexpr int STG_BYTES = 4 * 2 * STG_WARP_BYTES;
+constexpr int BIAS_BYTES = 512 * 4;
+constexpr int BAR_BYTES = 256;
+constexpr int XCHG_BYTES = 2 * MAX_CLUSTER * BM * 4;
+
+__global__ void __launch_bounds__(NUM_THREADS, 1)
+gemm_tc_kernel(const __grid_constant__ CUtensorMap tmA1, const __grid_constant__ CUtensorMap tmA2,
+               const __grid_constant__ CUtensorMap tmB, const __grid_constant__ CUtensorMap tmOut,
+               const TcParams p)
+{
+    extern __shared__ __align__(1024) uint8_t smem[];
+    const uint32_t sbase = smem_u32(smem);
+    if ((sbase & 1023u) != 0) __trap();  // SWIZZLE_128B tiles need 1024-byte alignment
+
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const uint32_t stg_off = (uint32_t)p.stages * p.stage_bytes;
+    const uint32_t bias_off = stg_off + STG_BYTES;
+    const uint32_t bar_off = bias_off + BIAS_BYTES;
+    const uint32_t xchg_off = bar_off + BAR_BYTES;
+    float *sbias = reinterpret_cast<float *>(smem + bias_off);
+    const uint32_t bar_full = sbase + bar_off;                 // [MAX_STAGES]
+    const uint32_t bar_empty = bar_full + 8 * MAX_STAGES;      // [MAX_STAGES]
+    const uint32_t bar_tfull = bar_empty + 8 * MAX_STAGES;     // [2]
+    const uint32_t bar_tempty = bar_tfull + 16;                // [2]
+    const uint32_t bar_xchg = bar_tempty + 16;                 // [2]
+    volatile uint32_t *tmem_slot = reinterpret_cast<volatile uint32_t *>(smem + bar_off + 8 * (2 * MAX_STAGES + 6));
+
+    const int slab = blockIdx.x % p.n_slabs;
+    const long long lane0 = blockIdx.x / p.n_slabs, lanes = gridDim.x / p.n_slabs;
+    const int n0 = slab * p.NS;
+    const int ncols = min(p.NS, p.N - n0);  // valid output columns of this slab
+    const int KB = p.kb1 + p.kb2;
+
+    // ---- one-time setup ---------------------------------------------------------------------
+    if (warp == 0 && lane == 0) {
+        asm volatile("prefetch.tensormap [%0];" ::"l"(&tmA1) : "memory");
+        asm volatile("prefetch.tensormap [%0];" ::"l"(&tmA2) : "memory");
+        asm volatile("prefetch.tensormap [%0];" ::"l"(&tmB) : "memory");
+        asm volatile("prefetch.tensormap [%0];" ::"l"(&tmOut) : "memory");
+    }
+    if (warp == 1 && lane == 0) {
+        for (int s = 0; s < p.stages; ++s) {
+            mbar_init(bar_full + 8 * s, 1);
+            mbar_init(bar_empty + 8 * s, 1);
+        }
+        for (int a = 0; a < 2; ++a) {
+            mbar_init(bar_tfull + 8 * a, 1);
+            mbar_init(bar_tempty + 8 * a, 4);
+            mbar_init(bar_xchg + 8 * a, 128 * (p.cluster > 1 ? p.cluster - 1 : 1));
+        }
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    if (warp == 2) {
+        asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(
+                         smem_u32(const_cast<uint32_t *>(tmem_slot))),
+                     "r"((uint32_t)p.tmem_cols)
+                     : "memory");
+        asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
+    }
+    if (warp >= 4) {
+        for (int c = threadIdx.x - 128; c < 512; c += 128)
+            sbias[c] = (p.bias != nullptr && c < ncols) ? __ldg(p.bias + n0 + c) : 0.f;
+    }
+    tc_fence_before();
+    if (p.cluster > 1) cluster_sync_all();
+    else __syncthreads();
+    tc_fence_after();
+    const uint32_t tmem_base = *tmem_slot;
+
+    if (warp == 0) {
+        // ===== TMA producer =====================================================================
+        if (lane == 0) {
+            uint64_t pol_stream, pol_keep;
+            asm volatile("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(pol_stream));
+            asm volatile("createpolicy.fractional.L2::evict_last.b64 %0, 1.0;" : "=l"(pol_keep));
+            int stage = 0;
+            uint32_t phase = 0;
+            for (long long mb = lane0; mb < p.m_blocks; mb += lanes) {
+                const int m0 = (int)(mb * BM);
+                for (int kb = 0; kb < KB; ++kb) {
+                    const uint32_t full = bar_full + 8 * stage;
+                    mbar_wait(bar_empty + 8 * stage, phase ^ 1);
+                    mbar_expect_tx(full, (uint32_t)p.stage_bytes);
+                    const bool seg2 = kb >= p.kb1;
+                    const int ka = (seg2 ? kb - p.kb1 : kb) * BK;
+                    const uint32_t sA = sbase + (uint32_t)stage * p.stage_bytes;
+                    tma_load_2d(sA, seg2 ? &tmA2 : &tmA1, ka, m0, full, pol_stream);
+                    const int kcol = seg2 ? p.K1 + ka : ka;
+                    for (int j = 0; j < p.nchunks; ++j)
+                        tma_load_2d(sA + A_BYTES + (uint32_t)j * p.CN * 128, &tmB, kcol,
+                                    n0 + j * p.CN, full, pol_keep);
+                    if (++stage == p.stages) {
+                        stage = 0;
+                        phase ^= 1;
+                    }
+                }
+            }
+        }
+    } else if (warp == 1) {
+        // ===== MMA issuer =======================================================================
+        if (lane == 0) {
+            int stage = 0, acc = 0;
+            uint32_t phase = 0, accphase = 0;
+            for (long long mb = lane0; mb < p.m_blocks; mb += lanes) {
+                mbar_wait(bar_tempty + 8 * acc, accphase ^ 1);   // epilogue has drained this accumulator
+                tc_fence_after();
+                const uint32_t d0 = tmem_base + (uint32_t)acc * p.acc_cols;
+                for (int kb = 0; kb < KB; ++kb) {
+                    mbar_wait(bar_full + 8 * stage, phase);      // TMA bytes have landed
+                    tc_fence_after();
+                    const uint32_t sA = sbase + (uint32_t)stage * p.stage_bytes;
+                    const uint64_t ad = make_desc(sA), bd = make_desc(sA + A_BYTES);
+#pragma unroll
+                    for (int k = 0; k < BK / 16; ++k)            // 32 bytes along K per UMMA_K = 16
+                        for (int j = 0; j < p.nchunks; ++j)
+                            tc_mma(d0 + (uint32_t)j * p.CN, ad + 2 * k,
+                                   bd + (uint64_t)((j * p.CN * 128) >> 4) + 2 * k, p.idesc,
+                                   (uint32_t)(kb | k));
+                    tc_commit(bar_empty + 8 * stage);            // frees the stage when the MMAs retire
+                    if (++stage == p.stages) {
+                        stage = 0;
+                        phase ^= 1;
+                    }
+                }
+                tc_commit(bar_tfull + 8 * acc);                  // accumulator complete
+                if (++acc == p.nacc) {
+                    acc = 0;
+                    accphase ^= 1;
+                }
+            }
+        }
+    } else if (warp >= 4) {
+        // ===== epilogue: thread (ew, lane) owns output row m0 + 32*ew + lane =====================
+        const int ew = warp - 4;                                  // == warp % 4: TMEM lanes 32*ew..
+        const int row = ew * 32 + lane;
+        uint8_t *stg = smem + stg_off + ew * 2 * STG_WARP_BYTES;
+        const uint32_t my_rank = p.cluster > 1 ? cluster_ctarank() : 0;
+        float *xbuf = reinterpret_cast<float *>(smem + xchg_off);  // [2][MAX_CLUSTER][BM]
+        int acc = 0, sbuf = 0;
+        uint32_t accphase = 0;
+        long long it = 0;
+        for (long long mb = lane0; mb < p.m_blocks; mb += lanes, ++it) {
+            const long long m0 = mb * BM;
+            mbar_wait(bar_tfull + 8 * acc, accphase);
+            tc_fence_after();
+            const uint32_t t0 = tmem_base + ((uint32_t)(ew * 32) << 16) + (uint32_t)acc * p.acc_cols;
+            float scale = 1.f;
+            if (p.l2norm) {
+                // pass 1: sum of squares of this row's z = act(acc + bias), columns in order
+                float ss = 0.f;
+                for (int c0 = 0; c0 < ncols; c0 += 32) {
+                    uint32_t v[32];
+                    tc_ld32(t0 + c0, v);
+                    tc_wait_ld();
+#pragma unroll
+                    for (int i = 0; i < 32; ++i) {
+                        float z = __uint_as_float(v[i]) + sbias[c0 + i];
+                        z = p.relu ? fmaxf(z, 0.f) : z;
+                        ss = (c0 + i < ncols) ? fmaf(z, z, ss) : ss;
+                    }
+                }
+                if (p.cluster > 1) {
+                    // push my partial to every peer, then wait for theirs (DSMEM + remote mbarrier)
+                    const int par = (int)(it & 1);
+                    const uint32_t my_slot = sbase + xchg_off + ((par * MAX_CLUSTER + my_rank) * BM + row) * 4;
+                    for (uint32_t r = 0; r < (uint32_t)p.cluster; ++r) {
+                        if (r == my_rank) continue;
+                        st_cluster_f32(map_to_cta(my_slot, r), ss);
+                        mbar_arrive_remote(map_to_cta(bar_xchg + 8 * par, r));
+                    }
+                    mbar_wait_cluster(bar_xchg + 8 * par, (uint32_t)((it >> 1) & 1));
+                    float tot = 0.f;
+                    for (uint32_t r = 0; r < (uint32_t)p.cluster; ++r)   // same order in every CTA
+                        tot += (r == my_rank) ? ss : xbuf[(par * MAX_CLUSTER + r) * BM + row];
+                    ss = tot;
+                }
+                scale = ss > 0.f ? rsqrtf(ss) : 0.f;             // zero row stays zero (reading A3)
+            }
+            // pass 2: 64 columns at a time -> bf16 -> swizzled staging -> TMA store
+            for (int c0 = 0; c0 < ncols; c0 += OUT_CHUNK) {
+                uint32_t v[2][32];
+                tc_ld32(t0 + c0, v[0]);
+                tc_ld32(t0 + c0 + 32, v[1]);
+                tc_wait_ld();
+                uint32_t pk[32];
+#pragma unroll
+                for (int h = 0; h < 2; ++h)
+#pragma unroll
+                    for (int i = 0; i < 32; i += 2) {
+                        float z0 = __uint_as_float(v[h][i]) + sbias[c0 + 32 * h + i];
+                        float z1 = __uint_as_float(v[h][i + 1]) + sbias[c0 + 32 * h + i + 1];
+                        if (p.relu) {
+                            z0 = fmaxf(z0, 0.f);
+                            z1 = fmaxf(z1, 0.f);
+                        }
+                        __nv_bfloat162 b = __floats2bfloat162_rn(z0 * scale, z1 * scale);
+                        pk[16 * h + i / 2] = *reinterpret_cast<uint32_t *>(&b);
+                    }
+                if (lane == 0) tma_store_wait_read<1>();          // the buffer used two stores ago is free
+                __syncwarp();
+                uint8_t *buf = stg + sbuf * STG_WARP_BYTES;
+                uint8_t *rowp = buf + lane * 128;
+#pragma unroll
+                for (int q = 0; q < 8; ++q)                       // 16-byte chunk q of the row, XOR-swizzled
+                    *reinterpret_cast<uint4 *>(rowp + ((q ^ (lane & 7)) << 4)) =
+                        make_uint4(pk[4 * q], pk[4 * q + 1], pk[4 * q + 2], pk[4 * q + 3]);
+                fence_proxy_async();
+                __syncwarp();
+                if (lane == 0 && m0 + ew * 32 < p.M) {
+                    tma_store_2d(&tmOut, n0 + c0, (int)(m0 + ew * 32), smem_u32(buf));
+                    tma_store_commit();
+                }
+                sbuf ^= 1;
+            }
+            tc_fence_before();
+            __syncwarp();
+            if (lane == 0) mbar_arrive(bar_tempty + 8 * acc);
+            if (++acc == p.nacc) {
+                acc = 0;
+                accphase ^= 1;
+            }
+        }
+        if (lane == 0) tma_store_wait_all();
+    }
+
+    // ---- teardown ---------------------------------------------------------------------------
+    __syncwarp();
+    tc_fence_before();
+    if (p.cluster > 1) cluster_sync_all();
+    else __syncthreads();
+    if (warp == 2) {
+        tc_fence_after();
+        asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem_base),
+                     "r"((uint32_t)p.tmem_cols)
+                     : "memory");
+    }
+}
+
+// ---- host side ----------------------------------------------------------------------------------
+typedef CUresult (*EncodeTiledFn)(CUtensorMap *, CUtensorMapDataType, cuuint32_t, void *,
+                                  const cuuint64_t *, const cuuint64_t *, const cuuint32_t *,
+                                  const cuuint32_t *, CUtensorMapInterleave, CUtensorMapSwizzle,
+                                  CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+
+EncodeTiledFn encode_fn()
+{
+    static EncodeTiledFn fn = [] {
+        void *sym = nullptr;
+        cudaDriverEntryPointQueryResult q;
+        if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &sym, cudaEnableDefault, &q) != cudaSuccess ||
+            q != cudaDriverEntryPointSuccess)
+            sym = nullptr;
+        return reinterpret_cast<EncodeTiledFn>(sym);
+    }();
+    return fn;
+}
+
+// Row-major bf16 matrix [rows x cols] (cols contiguous), box = box_rows x 64 columns, SWIZZLE_128B.
+// Out-of-bounds parts of a box read as zero and are not written.
+bool make_map(CUtensorMap *map, const void *ptr, long long rows, int cols, int box_rows)
+{
+    EncodeTiledFn fn = encode_fn();
+    if (!fn) return false;
+    const cuuint64_t dims[2] = {(cuuint64_t)cols, (cuuint64_t)rows};
+    const cuuint64_t strides[1] = {(cuuint64_t)cols * 2};
+    const cuuint32_t box[2] = {(cuuint32_t)BK, (cuuint32_t)box_rows};
+    const cuuint32_t estr[2] = {1, 1};
+    return fn(map, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 2, const_cast<void *>(ptr), dims, strides, box,
+              estr, CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B,
+              CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
+}
+
+inline int round_up(int x, int a) { return (x + a - 1) / a * a; }
+
+bool plan(const GemmArgs &a, TcParams &p, int &smem_bytes, const char **why)
+{
+    auto no = [&](const char *msg) {
+        if (why) *why = msg;
+        return false;
+    };
+    if (a.M < 1 || a.M >= (1LL << 31)) return no("M outside [1, 2^31)");
+    if (a.K1 < 8 || a.K1 % 8 || a.K2 < 0 || a.K2 % 8) return no("K1, K2 must be multiples of 8");
+    if (a.N < 8 || a.N % 8) return no("N must be a multiple of 8");
+    p = TcParams{};
+    p.M = a.M;
+    p.m_blocks = (a.M + BM - 1) / BM;
+    p.kb1 = (a.K1 + BK - 1) / BK;
+    p.kb2 = (a.K2 + BK - 1) / BK;
+    p.K1 = a.K1;
+    p.N = a.N;
+    const int slab_max = a.l2norm ? 512 : 256;      // a normalised row must sit in one CTA's TMEM
+    p.n_slabs = (a.N + slab_max - 1) / slab_max;
+    p.NS = p.n_slabs == 1 ? round_up(a.N, 16) : round_up((a.N + p.n_slabs - 1) / p.n_slabs, 64);
+    p.n_slabs = (a.N + p.NS - 1) / p.NS;
+    p.cluster = (a.l2norm && p.n_slabs > 1) ? p.n_slabs : 1;
+    if (p.cluster > MAX_CLUSTER) return no("row norm over more than 4096 columns");
+    p.nchunks = (p.NS + 255) / 256;
+    p.CN = round_up((p.NS + p.nchunks - 1) / p.nchunks, 16);
+    p.acc_cols = round_up(p.nchunks * p.CN, 64);
+    p.nacc = p.acc_cols <= 256 ? 2 : 1;
+    int cols = p.nacc * p.acc_cols;
+    p.tmem_cols = 32;
+    while (p.tmem_cols < cols) p.tmem_cols *= 2;
+    p.stage_bytes = A_BYTES + p.nchunks * p.CN * 128;
+    const int fixed = STG_BYTES + BIAS_BYTES + BAR_BYTES + (p.cluster > 1 ? XCHG_BYTES : 0);
+    p.stages = (SMEM_LIMIT - fixed) / p.stage_bytes;
+    if (p.stages > MAX_STAGES) p.stages = MAX_STAGES;
+    if (p.stages < 2) return no("tile does not fit shared memory");
+    smem_bytes = p.stages * p.stage_bytes + fixed;
+    p.bias = a.bias;
+    p.relu = a.relu;
+    p.l2norm = a.l2norm;
+    // instruction descriptor, kind::f16: D fp32 (bit 4), A and B bf16 (bits 7, 10), both K-major,
+    // N >> 3 at bits [17,23), M >> 4 at bits [24,29)
+    p.idesc = (1u << 4) | (1u << 7) | (1u << 10) | ((uint32_t)(p.CN >> 3) << 17) | ((uint32_t)(BM >> 4) << 24);
+    return true;
+}
+
+}  // namespace
+
+bool gemm_tc_supported(const GemmArgs &a, const char **why)
+{
+    TcParams p;
+    int smem = 0;
+    if (!plan(a, p, smem, why)) return false;
+    if (!encode_fn()) {
+        if (why) *why = "cuTensorMapEncodeTiled is not available from this driver";
+        return false;
+    }
+    return true;
+}
+
+size_t gemm_tc_scratch_bytes(const GemmArgs &) { return 0; }
+
+cudaError_t launch_gemm_tc(const GemmArgs &a, int num_sms, cudaStream_t s, int *launches)
+{
+    TcParams p;
+    int smem = 0;
+    if (!plan(a, p, smem, nullptr)) return cudaErrorNotSupported;
+    CUtensorMap tmA1, tmA2, tmB, tmOut;
+    if (!make_map(&tmA1, a.A1, a.M, a.K1, BM)) return cudaErrorInvalidValue;
+    if (a.K2 > 0) {
+        if (!make_map(&tmA2, a.A2, a.M, a.K2, BM)) return cudaErrorInvalidValue;
+    } else {
+        tmA2 = tmA1;
+    }
+    if (!make_map(&tmB, a.B, a.N, a.K1 + a.K2, p.CN)) return cudaErrorInvalidValue;
+    if (!make_map(&tmOut, a.out, a.M, a.N, 32)) return cudaErrorInvalidValue;
+
+    static bool attr_set = false;
+    if (!attr_set) {
+        cudaError_t e = cudaFuncSetAttribute(gemm_tc_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                             SMEM_LIMIT);
+        if (e != cudaSuccess) return e;
+        attr_set = true;
+    }
+    long long tiles = p.m_blocks * p.n_slabs;
+    long long grid = tiles < num_sms ? tiles : num_sms;
+    grid = grid / p.n_slabs * p.n_slabs;
+    if (grid < p.n_slabs) grid = p.n_slabs;
+
+    cudaLaunchConfig_t cfg{};
+    cfg.gridDim = dim3((unsigned)grid);
+    cfg.blockDim = dim3(NUM_THREADS);
+    cfg.dynamicSmemBytes = (size_t)smem;
+    cfg.stream = s;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeClusterDimension;
+    attr[0].val.clusterDim.x = (unsigned)p.cluster;
+    attr[0].val.clusterDim.y = 1;
+    attr[0].val.clusterDim.z = 1;
+    cfg.attrs = attr;
+    cfg.numAttrs = 1;
+    if (launches) ++*launches;
+    return cudaLaunchKernelEx(&cfg, gemm_tc_kernel, tmA1, tmA2, tmB, tmOut, p);
+}
+
+}  // namespace pinsage
