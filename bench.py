@@ -218,7 +218,9 @@ def run_ours(args, cfg):
     ctx.pinsage_set_option("gemm_impl", args.gemm_impl)
     ctx.pinsage_set_option("overlap", args.overlap)
     alpha = ctx.pinsage_normalize_counts(counts)
+    torch.cuda.synchronize()
     del counts
+    torch.cuda.empty_cache()     # generator temporaries back to the driver: the library cudaMallocs
     out = torch.empty((cfg.N, cfg.d_out), dtype=X.dtype, device=dev)
     e = X.element_size()
 
@@ -300,10 +302,13 @@ def run_ours(args, cfg):
     pool_ms, pool_n = prof["pool"]
     pool_bytes_step = sum(cfg.N * pool_bytes_per_node(cfg.T, m, e) for _, m, _ in cfg.layer_dims())
     pool_gbs = pool_bytes_step * args.steps / (pool_ms * 1e-3) / 1e9 if pool_ms > 0 else 0.0
-    traffic = None
-    tp = os.path.join(ROOT, "profiles", "pool_traffic.json")
+    traffic = None      # DRAM bytes per launch from the committed ncu --set full capture, if any
+    tp = os.path.join(ROOT, "profiles", "pool_traffic.csv")
     if os.path.exists(tp):
-        traffic = json.load(open(tp)).get(cfg.name)
+        for ln in open(tp).read().splitlines()[1:]:
+            f = ln.split(",")
+            if f and f[0] == cfg.name and int(f[1]) == (args.chunk_nodes or 0):
+                traffic = float(f[2])
     kernels = {}
     for name, (kms, kn) in prof.items():
         kernels[name] = {"ms_per_step": kms / args.steps, "launches_per_step": kn / args.steps}
@@ -350,7 +355,7 @@ def main():
     ap.add_argument("--nodes", type=int, default=0, help="override N (a '-small' sibling)")
     ap.add_argument("--chunk-nodes", type=int, default=0)
     ap.add_argument("--gemm-impl", type=int, default=0, help="0 tcgen05, 1 SIMT reference kernels")
-    ap.add_argument("--overlap", type=int, default=1)
+    ap.add_argument("--overlap", type=int, default=0)
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu", action="store_true")
     ap.add_argument("--cpu-seconds", type=float, default=15.0)

@@ -266,9 +266,15 @@ pinsage_status maybe_validate(pinsage_ctx *ctx, int64_t n_dst, int64_t n_src, in
     return pinsage_validate_graph(ctx, n_dst, n_src, T, idx, w, &bad);
 }
 
-int64_t auto_chunk(int64_t N, int64_t requested)
+// Destination rows per S2/S3 chunk.  Automatic: as many rows as keep one chunk buffer (rows x
+// row_bytes) within 1 GiB, at least 131072 -- measured on B200: few
+// large launches beat many small ones (fewer wave tails in the pool, fewer partial waves of
+// 128-row tiles in the persistent GEMM), and chunk buffers of this size cost < 1 % of HBM.
+int64_t auto_chunk(int64_t N, int64_t requested, size_t row_bytes)
 {
-    int64_t c = requested > 0 ? requested : (int64_t)131072;
+    int64_t c = requested > 0
+                    ? requested
+                    : std::max<int64_t>(131072, (int64_t)((size_t(1) << 30) / std::max<size_t>(row_bytes, 1)));
     c = std::min<int64_t>(c, N);
     if (c < N) c = std::max<int64_t>(128, c / 128 * 128);  // keep chunk starts on GEMM tile edges
     return c;
@@ -341,8 +347,11 @@ LayerWs plan_layer_ws(const pinsage_ctx *ctx, DType dt, int64_t N, const pinsage
     off += align_up((size_t)N * lp->m * es, 256);
     p.n0_off = off;
     off += align_up((size_t)chunk * lp->m * es, 256);
-    p.n1_off = off;
-    off += align_up((size_t)chunk * lp->m * es, 256);
+    p.n1_off = p.n0_off;                       // second chunk buffer only for the two-stream schedule
+    if (ctx && ctx->overlap) {
+        p.n1_off = off;
+        off += align_up((size_t)chunk * lp->m * es, 256);
+    }
     GemmArgs g1;
     g1.M = N; g1.K1 = lp->d_in; g1.N = lp->m; g1.relu = 1;
     GemmArgs g3;
@@ -604,8 +613,9 @@ size_t pinsage_layer_workspace_bytes(pinsage_dtype dtype, int64_t N, int32_t T,
     // sized for the larger (SIMT reference) scratch so that either gemm_impl fits
     pinsage_ctx probe;
     probe.gemm_impl = 1;
+    probe.overlap = 1;
     const DType dt = static_cast<DType>(dtype);
-    return plan_layer_ws(&probe, dt, N, params, auto_chunk(N, 0)).total;
+    return plan_layer_ws(&probe, dt, N, params, auto_chunk(N, 0, (size_t)params->m * elem_size(dt))).total;
 }
 
 pinsage_status pinsage_layer(pinsage_ctx *ctx, pinsage_dtype dtype, int64_t N, int32_t T,
@@ -630,7 +640,7 @@ pinsage_status pinsage_layer(pinsage_ctx *ctx, pinsage_dtype dtype, int64_t N, i
     } else if (overlaps(feats, (size_t)N * params->d_in * es, out, (size_t)N * params->d * es)) {
         return fail(ctx, PINSAGE_ERR_INVALID_ARG, "out partially overlaps feats");
     }
-    const int64_t chunk = auto_chunk(N, 0);
+    const int64_t chunk = auto_chunk(N, 0, (size_t)params->m * es);
     const LayerWs plan = plan_layer_ws(ctx, dt, N, params, chunk);
     char *base;
     if (ws) {
@@ -661,7 +671,7 @@ pinsage_status pinsage_head(pinsage_ctx *ctx, pinsage_dtype dtype, int64_t N, co
     const size_t es = elem_size(dt);
     if (overlaps(h, (size_t)N * params->d * es, out, (size_t)N * params->d_out * es))
         return fail(ctx, PINSAGE_ERR_INVALID_ARG, "out overlaps h");
-    const int64_t chunk = auto_chunk(N, 0);
+    const int64_t chunk = auto_chunk(N, 0, (size_t)params->g1 * es);
     const size_t a_bytes = align_up((size_t)chunk * params->g1 * es, 256);
     PS_TRY(ensure_ws(ctx, a_bytes));
     for (int64_t r0 = 0; r0 < N; r0 += chunk) {
@@ -743,7 +753,9 @@ pinsage_status pinsage_embed_all(pinsage_ctx *ctx, pinsage_dtype dtype, int64_t 
     if (h_out) d_out = stage + st_out;
 
     // ---- workspace plan: P | n0 | n1 | scratch | H_a | H_b | head chunk a ------------------------
-    const int64_t chunk = auto_chunk(N, chunk_nodes);
+    int32_t w_max = head->g1;
+    for (int k = 0; k < K; ++k) w_max = std::max(w_max, layers[k].m);
+    const int64_t chunk = auto_chunk(N, chunk_nodes, (size_t)w_max * es);
     size_t max_layer_ws = 0;
     int32_t d_max = 0;
     for (int k = 0; k < K; ++k) {

@@ -297,12 +297,14 @@ def test_embed_all_deterministic_and_overlap_invariant(ctx):
     a = ctx.pinsage_embed_all(X.to(DEV), idx.to(DEV), w, Ld, Hd, chunk_nodes=1024)
     b = ctx.pinsage_embed_all(X.to(DEV), idx.to(DEV), w, Ld, Hd, chunk_nodes=1024)
     assert torch.equal(a.view(torch.int16), b.view(torch.int16))
-    ctx.pinsage_set_option("overlap", 0)
+    ctx.pinsage_set_option("overlap", 1)       # two-stream schedule, different chunking
     try:
         c = ctx.pinsage_embed_all(X.to(DEV), idx.to(DEV), w, Ld, Hd, chunk_nodes=3072)
     finally:
-        ctx.pinsage_set_option("overlap", 1)
+        ctx.pinsage_set_option("overlap", 0)
     assert torch.equal(a.view(torch.int16), c.view(torch.int16))
+    d = ctx.pinsage_embed_all(X.to(DEV), idx.to(DEV), w, Ld, Hd)   # automatic chunk (one chunk)
+    assert torch.equal(a.view(torch.int16), d.view(torch.int16))
 
 
 def test_embed_all_host_buffers_match_device_buffers(ctx):
