@@ -310,3 +310,45 @@ class RecMemo:
     def embed(self, nodes) -> np.ndarray:
         H = self.hidden(nodes, len(self.layers))
         return head(H, self.head_params) if self.head_params is not None else H
+
+
+def minibatch_embed(M, fetch_x, fetch_nbr, layers, head_params=None, return_hidden: bool = False):
+    """Algorithm 2 MINIBATCH for a set M of destination nodes, touching only
+    their K-hop closure -- the full-size parity sampler (rows of X / the tables are read through
+    fetchers, so the arrays may live anywhere).
+
+      lines 1-7 (:147-152)  S^(K) = M;  S^(k-1) = S^(k) U N(u) for u in S^(k)
+      line 8    (:155)      h^(0)_u = x_u for u in S^(0)
+      lines 9-14 (:156-164) h^(k)_u = CONVOLVE^(k)(h^(k-1)_u, {h^(k-1)_v, v in N(u)}), u in S^(k)
+      lines 15-17 (:165-167) z_u = G2 ReLU(G1 h^(K)_u + g), u in M
+
+    CONVOLVE is applied to a whole set at once through the layer-wise steps dense / pool /
+    combine above (each projection computed once per member of S^(k-1)).
+
+    fetch_x(ids int64) -> [len, d_0] float64;  fetch_nbr(ids) -> (idx [len, T], alpha [len, T]).
+    Returns out [len(M), d_out] in the order of M (and the list of h^(k) rows of M if asked).
+    """
+    M = np.asarray(M, dtype=np.int64)
+    K = len(layers)
+    S = [None] * (K + 1)
+    nbr = [None] * (K + 1)
+    S[K] = np.unique(M)
+    for k in range(K, 0, -1):
+        ii, aa = fetch_nbr(S[k])
+        ii = np.asarray(ii, dtype=np.int64)
+        nbr[k] = (ii, np.asarray(aa, dtype=np.float32))
+        S[k - 1] = np.union1d(S[k], ii.ravel())
+    H = np.asarray(fetch_x(S[0]), dtype=np.float64)
+    at_M = []
+    for k in range(1, K + 1):
+        lp = layers[k - 1]
+        ii, aa = nbr[k]
+        P = dense(H, lp["Q"], lp["q"], act=True)                 # every member of S^(k-1), once
+        local = np.searchsorted(S[k - 1], ii).astype(np.int32)   # re-indexed sub-table
+        n = pool(P, local, aa)
+        H = combine(H[np.searchsorted(S[k - 1], S[k])], n, lp["W"], lp["w"])
+        if return_hidden:
+            at_M.append(H[np.searchsorted(S[k], M)])             # M is a subset of every S^(k)
+    HM = H[np.searchsorted(S[K], M)]
+    out = head(HM, head_params) if head_params is not None else HM
+    return (out, at_M) if return_hidden else out

@@ -288,6 +288,42 @@ def test_recursion_equals_literal_equals_layerwise(K, T):
     assert np.all((np.abs(nrm - 1) < 1e-14) | (nrm == 0))
 
 
+@pytest.mark.parametrize("K,T", [(1, 5), (2, 4), (3, 3)])
+def test_minibatch_algorithm2_equals_full_graph_and_brute_force(K, T):
+    """Algorithm 2 on a minibatch M (K-hop sets S^(k), then CONVOLVE per
+    level) gives the rows of the full-graph result and of the brute-force recursion; it is
+    the sampler of the full-size GPU parity tests."""
+    rng = np.random.default_rng(40 + K)
+    N = 80
+    dims = [6, 10, 8, 12][:K + 1]
+    ms = [7, 5, 9][:K]
+    idx, counts = _rand_graph(rng, N, T)
+    alpha = O.normalize_counts(counts)
+    X = rng.normal(size=(N, dims[0]))
+    layers = [_rand_layer(rng, dims[k], ms[k], dims[k + 1], bias=0.05) for k in range(K)]
+    hp = _rand_head(rng, dims[K], 9, 5)
+    full, hid = O.embed_all(X, idx, alpha, layers, hp, mode="literal", return_hidden=True)
+    touched = []
+
+    def fetch_x(ids):
+        touched.append(len(ids))
+        return X[ids]
+
+    M = [7, 0, N - 1, 7, 33]
+    out, hM = O.minibatch_embed(M, fetch_x, lambda ids: (idx[ids], alpha[ids]), layers, hp,
+                                return_hidden=True)
+    np.testing.assert_allclose(out, full[M], rtol=0, atol=1e-15)
+    for a, b in zip(hM, hid):
+        np.testing.assert_allclose(a, b[M], rtol=0, atol=1e-15)
+    for r, u in enumerate(M[:2]):
+        np.testing.assert_allclose(hM[-1][r], O.rec(u, K, X, idx, alpha, layers), atol=1e-15)
+    if K == 1:
+        assert touched == [len(np.union1d(M, idx[M].ravel()))]   # only the closure is read
+    # without a head the last hidden rows come back
+    np.testing.assert_array_equal(
+        O.minibatch_embed(M, fetch_x, lambda ids: (idx[ids], alpha[ids]), layers), hM[-1])
+
+
 def test_neighbour_order_and_relabelling_invariance():
     """gamma is symmetric: permuting (idx, alpha) jointly within a row
     changes nothing; relabelling nodes by pi permutes the outputs by pi."""
