@@ -1,0 +1,214 @@
+"""Full-size parity: BASELINE.json's configs 2-5 at their full N, in the launch configuration
+bench.py times (``pinsage_embed_all`` with the automatic driver chunk), against the fp64 oracle.
+
+Config 2 (the bench workload) is compared on EVERY row.  Configs 3-5 are too large for an
+exhaustive fp64 pass, so they are compared on sampled destinations the oracle computes one
+minibatch at a time (Algorithm 2, ``oracle.minibatch_embed``: only the K-hop closure of the
+sample is read back from the device):
+
+  (a) end to end: out[M] for a fixed list of boundary rows (first / last row, GEMM tile and driver
+      chunk edges, rows either side of every 2^32-byte boundary of P and of the flat tables,
+      destinations that list node 0 / N-1) plus seeded random rows;
+  (b) one layer at a time: layer k of the GPU on the GPU's own stored H_{k-1} (exact inputs by
+      definition) for thousands of destinations per layer;
+  (c) the head on sampled rows, and -- as a whole-array property -- bit equality between the
+      one-call path and the layer-by-layer path on all N rows.
+
+Inputs are generated on the device by the seeded generators of ``synth`` (DESIGN.md "Input
+recipe"); the oracle reads back exactly the rows it needs, so both sides see the same stored values.
+"""
+import time
+
+import numpy as np
+import pytest
+import torch
+
+from oracle import oracle as O
+from paper_1806_01973_b200 import binding, synth
+from tests.parity import assert_rows_close, params_f64, to_f64
+
+pytestmark = pytest.mark.gpu
+
+DEV = "cuda:0"
+
+
+@pytest.fixture()
+def ctx():
+    """One context per test: closing it returns its workspace (tens of GB at these sizes)."""
+    torch.cuda.empty_cache()
+    c = binding.Context(0)
+    yield c
+    c.close()
+    torch.cuda.empty_cache()
+
+
+def _need_memory(gb):
+    free, _ = torch.cuda.mem_get_info(0)
+    if free < gb * 1e9:
+        pytest.skip(f"needs {gb} GB of free HBM, {free / 1e9:.0f} GB available")
+
+
+def _auto_chunk(N, w_max, e):
+    """The driver's automatic chunk rule (api.cu auto_chunk), mirrored to aim samples at its edges."""
+    c = min(N, max(131072, (1 << 30) // (w_max * e)))
+    return c if c == N else max(128, c // 128 * 128)
+
+
+def _boundary_rows(cfg, idx, few=False):
+    """The fixed part of the sample (SURVEY.md 8(c) "which rows to sample").  few=True keeps one
+    representative of each kind (for config 5, where one destination's closure is 10^6 rows)."""
+    N, T, e = cfg.N, cfg.T, 2
+    rows = {0, N - 1, 128} if few else {0, 1, N - 1, N - 2, 127, 128, 129}
+    chunk = _auto_chunk(N, max(cfg.hidden, cfg.g1), e)
+    edges = list(range(chunk, N, chunk))
+    for c in (edges[:1] + edges[-1:] if few else edges):
+        rows.update((c - 1, c))
+    for width_bytes in (cfg.d0 * e, cfg.hidden * e, cfg.d_out * e, 4 * T):
+        b = (1 << 32) // width_bytes          # first row at / after each 2^32-byte boundary
+        for j in range(1, 2 if few else 64):
+            if j * b >= N:
+                break
+            rows.update((j * b - 1, j * b) if few else (j * b - 1, j * b, j * b + 1))
+    # destinations whose neighbour list holds node 0 / node N-1 (searched in the leading rows)
+    lead = idx[: min(N, 4_000_000)]
+    for target in (0, N - 1):
+        hit = (lead == target).any(dim=1).nonzero()
+        if hit.numel():
+            rows.add(int(hit[0]))
+    return sorted(r for r in rows if 0 <= r < N)
+
+
+def _sample(cfg, idx, n_random, seed=12345, few=False):
+    fixed = _boundary_rows(cfg, idx, few)
+    rng = np.random.default_rng(seed)
+    rnd = rng.integers(0, cfg.N, size=n_random)
+    return np.array(fixed + [int(r) for r in rnd], dtype=np.int64)
+
+
+def _fetchers(H, idx, alpha):
+    def fetch_x(ids):
+        t = torch.from_numpy(np.asarray(ids, dtype=np.int64)).to(DEV)
+        return H[t].to(torch.float64).cpu().numpy()
+
+    def fetch_nbr(ids):
+        t = torch.from_numpy(np.asarray(ids, dtype=np.int64)).to(DEV)
+        return idx[t].cpu().numpy(), alpha[t].cpu().numpy()
+
+    return fetch_x, fetch_nbr
+
+
+def _rows(H, ids):
+    return H[torch.from_numpy(np.asarray(ids, dtype=np.int64)).to(DEV)].to(torch.float64).cpu().numpy()
+
+
+def _full_size(ctx, name, n_e2e, e2e_batch, n_layer, few=False, head_block=4_000_000):
+    cfg = synth.CONFIGS[name]
+    dt = synth.torch_dtype(cfg.dtype)
+    t0 = time.time()
+    X = synth.make_features(cfg, device=DEV)
+    layers, head = synth.make_params(cfg, device=DEV)
+    idx, counts = synth.make_graph(cfg, device=DEV)
+    alpha = ctx.pinsage_normalize_counts(counts)
+    probe = _sample(cfg, idx, 2048)
+    np.testing.assert_array_equal(alpha[torch.from_numpy(probe).to(DEV)].cpu().numpy(),
+                                  O.normalize_counts(counts[torch.from_numpy(probe).to(DEV)].cpu().numpy()))
+    assert ctx.pinsage_validate_graph(idx, alpha, cfg.N) == -1
+    del counts
+    torch.cuda.empty_cache()
+    Lf, Hf = params_f64([{k: v.cpu() for k, v in lp.items()} for lp in layers],
+                        {k: v.cpu() for k, v in head.items()})
+    t_gen = time.time() - t0
+
+    # ---- the configuration bench.py times: one call, automatic chunk ---------------------------
+    out = ctx.pinsage_embed_all(X, idx, alpha, layers, head)
+    torch.cuda.synchronize()
+    report = {"config": name, "N": cfg.N, "gen_s": round(t_gen, 1)}
+
+    # ---- (a) end to end on sampled destinations --------------------------------------------------
+    t0 = time.time()
+    fx, fn = _fetchers(X, idx, alpha)
+    M = _sample(cfg, idx, n_e2e, few=few)
+    worst, cmin = 0.0, 1.0
+    for s in range(0, len(M), e2e_batch):
+        Mb = M[s:s + e2e_batch]
+        ref = O.minibatch_embed(Mb, fx, fn, Lf, Hf)
+        rel, cos = assert_rows_close(_rows(out, Mb), ref, dt, f"{name} end-to-end rows {Mb[:4]}..")
+        worst, cmin = max(worst, rel), min(cmin, cos)
+    report.update(e2e_rows=len(M), e2e_max_rel=worst, e2e_min_cos=cmin, e2e_s=round(time.time() - t0, 1))
+    del fx
+
+    # ---- (b) one layer at a time on the GPU's own H_{k-1} -----------------------------------------
+    t0 = time.time()
+    H = X
+    for k, (lp, lpf) in enumerate(zip(layers, Lf), start=1):
+        S = _sample(cfg, idx, n_layer, seed=777 + k)
+        fxk, _ = _fetchers(H, idx, alpha)
+        ref = O.minibatch_embed(S, fxk, fn, [lpf])             # before H is overwritten in place
+        d_in, d = lp["Q"].shape[1], lp["W"].shape[0]
+        if d == d_in:
+            ctx.pinsage_layer(H, idx, alpha, lp, out=H)        # in place (k >= 2 rule, d == d_in)
+        else:
+            Hn = ctx.pinsage_layer(H, idx, alpha, lp)
+            del H
+            if k == 1:
+                del X
+            torch.cuda.empty_cache()
+            H = Hn
+        rel, cos = assert_rows_close(_rows(H, S), ref, dt, f"{name} layer {k}", tol=6e-3)
+        nrm = np.linalg.norm(_rows(H, S), axis=1)
+        assert np.all((np.abs(nrm - 1) < 2.0 ** -7) | (nrm == 0))
+        report[f"layer{k}_rows"] = len(S)
+        report[f"layer{k}_max_rel"] = rel
+    report["layers_s"] = round(time.time() - t0, 1)
+
+    # ---- (c) head on samples; layer-by-layer path == one-call path on all N rows, bit for bit -----
+    S = _sample(cfg, idx, 4096, seed=999)
+    assert_rows_close(_rows(out, S), O.head(_rows(H, S), Hf), dt, f"{name} head", tol=6e-3)
+    for r0 in range(0, cfg.N, head_block):
+        r1 = min(cfg.N, r0 + head_block)
+        blk = ctx.pinsage_head(H[r0:r1], head)
+        assert torch.equal(blk.view(torch.int16), out[r0:r1].view(torch.int16)), \
+            f"{name}: one-call path differs from layer-by-layer path in rows [{r0}, {r1})"
+        del blk
+    print("FULL-SIZE PARITY", report)
+    return report
+
+
+def test_full_cfg2_every_row(ctx):
+    """Config 2 at N = 10^6 -- the workload bench.py times -- against the exhaustive fp64 oracle."""
+    _need_memory(8)
+    cfg = synth.CONFIGS["cfg2"]
+    X = synth.make_features(cfg, device=DEV)
+    layers, head = synth.make_params(cfg, device=DEV)
+    idx, counts = synth.make_graph(cfg, device=DEV)
+    alpha = ctx.pinsage_normalize_counts(counts)
+    ref_alpha = O.normalize_counts(counts.cpu().numpy())
+    np.testing.assert_array_equal(alpha.cpu().numpy(), ref_alpha)
+    out = ctx.pinsage_embed_all(X, idx, alpha, layers, head)
+    torch.cuda.synchronize()
+    Lf, Hf = params_f64([{k: v.cpu() for k, v in lp.items()} for lp in layers],
+                        {k: v.cpu() for k, v in head.items()})
+    ref = O.embed_all(to_f64(X), idx.cpu().numpy(), ref_alpha, Lf, Hf)
+    rel, cos = assert_rows_close(to_f64(out), ref, torch.bfloat16, "cfg2 full, every row")
+    print("FULL-SIZE PARITY", {"config": "cfg2", "N": cfg.N, "rows": cfg.N, "max_rel": rel,
+                               "min_cos": cos})
+
+
+def test_full_cfg2_sampled_and_layerwise(ctx):
+    _need_memory(8)
+    _full_size(ctx, "cfg2", n_e2e=256, e2e_batch=512, n_layer=4096)
+
+
+def test_full_cfg3_paper_shaped(ctx):
+    _need_memory(75)
+    _full_size(ctx, "cfg3", n_e2e=24, e2e_batch=64, n_layer=1024)
+
+
+def test_full_cfg4_power_law(ctx):
+    _need_memory(110)
+    _full_size(ctx, "cfg4", n_e2e=128, e2e_batch=128, n_layer=4096)
+
+
+def test_full_cfg5_deep_wide(ctx):
+    _need_memory(150)
+    _full_size(ctx, "cfg5", n_e2e=2, e2e_batch=2, n_layer=2048, few=True)
