@@ -98,6 +98,10 @@ const char *pinsage_version(void);
  *                                    nbr_idx first (synchronous), default 0
  *                   "overlap"        1 = pinsage_layer / embed_all overlap S2 of chunk c+1 with S3
  *                                    of chunk c on a second stream (default 0)
+ *                   "pool_slab"      column-slab width in bytes of the S2 pool: -1 automatic (default:
+ *                                    128-byte slabs when P exceeds L2 but n_src x 128 bytes fits in
+ *                                    0.7 of it, so that the gathered sub-table stays L2-resident),
+ *                                    0 = always whole rows, 32 / 64 / 128 = forced.  Bit-identical results.
  *                   "profile"        1 = bracket every kernel launch of the path with CUDA events
  *                                    on its stream, see pinsage_profile_read (default 0)
  * Unknown key -> PINSAGE_ERR_INVALID_ARG. */

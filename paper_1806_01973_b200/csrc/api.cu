@@ -25,6 +25,8 @@ struct pinsage_ctx {
     int gemm_impl = 0;               // 0 tcgen05, 1 SIMT reference
     int check_indices = 0;
     int overlap = 0;
+    int pool_slab = -1;              // -1 automatic, 0 off, 32 / 64 / 128 forced slab width in bytes
+    size_t l2_bytes = 0;
     int launches = 0;
     int64_t total_launches = 0;
     void *ws = nullptr;              // context-owned workspace
@@ -158,6 +160,20 @@ pinsage_status ensure_stage(pinsage_ctx *ctx, size_t bytes)
     }
     ctx->stage_bytes = bytes;
     return PINSAGE_OK;
+}
+
+// Column-slab width for the pool (pool.cu): slabs pay off when P does not fit L2 but a 128-byte
+// column slab of it does.  Measured on B200: a slab sub-table of up to ~64 MB
+// is gathered at 14.8 TB/s (whole rows from HBM: 8-9.5 TB/s), the gain fades by ~90 MB, and slabs
+// narrower than the 128-byte L2 line never win (L2 allocates whole lines, requests double).
+int pick_slab(const pinsage_ctx *ctx, DType dt, int64_t n_src, int32_t T, int32_t m)
+{
+    if (ctx->pool_slab == 0) return 0;
+    if (ctx->pool_slab > 0) return pool_slab_ok(dt, T, m, ctx->pool_slab) ? ctx->pool_slab : 0;
+    const size_t row = (size_t)m * elem_size(dt);
+    if ((size_t)n_src * row <= ctx->l2_bytes / 2) return 0;      // whole table is L2-resident anyway
+    if (pool_slab_ok(dt, T, m, 128) && (size_t)n_src * 128 <= ctx->l2_bytes / 10 * 7) return 128;
+    return 0;
 }
 
 enum ProfKind { PROF_POOL = 0, PROF_DENSE = 1, PROF_COMBINE = 2, PROF_KINDS = 3 };
@@ -303,7 +319,7 @@ pinsage_status pool_combine_chunks(pinsage_ctx *ctx, DType dt, int64_t N, int32_
         if (two && c >= 2) PS_CUDA(ctx, cudaStreamWaitEvent(ps, ctx->ev_gemm[b], 0));
         const int pe0 = prof_mark(ctx, ps);
         cudaError_t e = launch_pool(dt, rows, T, lp->m, P, idx + (size_t)r0 * T, w + (size_t)r0 * T,
-                                    nb[b], ps, &ctx->launches);
+                                    nb[b], pick_slab(ctx, dt, N, T, lp->m), ps, &ctx->launches);
         prof_close(ctx, PROF_POOL, pe0, ps);
         count_launches(ctx);
         PS_CUDA(ctx, e);
@@ -429,6 +445,7 @@ pinsage_status pinsage_create(pinsage_ctx **out, int device, void *cuda_stream)
     ctx->device = device;
     ctx->stream = static_cast<cudaStream_t>(cuda_stream);
     ctx->num_sms = prop.multiProcessorCount;
+    ctx->l2_bytes = (size_t)prop.l2CacheSize;
     DeviceGuard guard(device);
     bool ok = cudaStreamCreateWithFlags(&ctx->aux, cudaStreamNonBlocking) == cudaSuccess;
     for (int i = 0; i < 2 && ok; ++i) {
@@ -482,6 +499,10 @@ pinsage_status pinsage_set_option(pinsage_ctx *ctx, const char *key, int64_t val
         ctx->check_indices = value != 0;
     } else if (!strcmp(key, "overlap")) {
         ctx->overlap = value != 0;
+    } else if (!strcmp(key, "pool_slab")) {
+        if (value != -1 && value != 0 && value != 32 && value != 64 && value != 128)
+            return fail(ctx, PINSAGE_ERR_INVALID_ARG, "pool_slab must be -1, 0, 32, 64 or 128");
+        ctx->pool_slab = (int)value;
     } else if (!strcmp(key, "profile")) {
         ctx->profile = value != 0;
     } else {
@@ -564,7 +585,8 @@ pinsage_status pinsage_pool(pinsage_ctx *ctx, pinsage_dtype dtype, int64_t n_dst
         return fail(ctx, PINSAGE_ERR_INVALID_ARG, "n overlaps P");
     PS_TRY(maybe_validate(ctx, n_dst, n_src, T, nbr_idx, nbr_w));
     const int pe0 = prof_mark(ctx, ctx->stream);
-    cudaError_t e = launch_pool(dt, n_dst, T, m, P, nbr_idx, nbr_w, n, ctx->stream, &ctx->launches);
+    cudaError_t e = launch_pool(dt, n_dst, T, m, P, nbr_idx, nbr_w, n, pick_slab(ctx, dt, n_src, T, m),
+                                ctx->stream, &ctx->launches);
     prof_close(ctx, PROF_POOL, pe0, ctx->stream);
     count_launches(ctx);
     if (e == cudaErrorNotSupported)

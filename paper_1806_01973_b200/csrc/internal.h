@@ -41,8 +41,12 @@ cudaError_t launch_gemm_tc(const GemmArgs &a, int num_sms, cudaStream_t s, int *
 size_t gemm_tc_scratch_bytes(const GemmArgs &a);
 
 // ---- pool.cu ------------------------------------------------------------------------------------
+// slab_bytes: 0 = whole rows (one pass); 32 / 64 / 128 = column-slab passes that keep the gathered
+// sub-table L2-resident (ignored when pool_slab_ok is false for the shape).
 cudaError_t launch_pool(DType dt, int64_t n_dst, int32_t T, int32_t m, const void *P,
-                        const int32_t *idx, const float *w, void *out, cudaStream_t s, int *launches);
+                        const int32_t *idx, const float *w, void *out, int slab_bytes, cudaStream_t s,
+                        int *launches);
+bool pool_slab_ok(DType dt, int32_t T, int32_t m, int slab_bytes);
 cudaError_t launch_normalize_counts(int64_t N, int32_t T, const int32_t *counts, float *w,
                                     cudaStream_t s, int *launches);
 // first_bad: device int64, set to the smallest offending flat position or -1

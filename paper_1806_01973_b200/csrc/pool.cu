@@ -36,6 +36,27 @@ __device__ __forceinline__ uint4 ld_row16(const uint4 *p)
                  : "l"(p));
     return v;
 }
+// L2 cache-policy variants: gathered rows are worth keeping (evict_last), tables are read once
+__device__ __forceinline__ uint4 ld_row16_keep(const uint4 *p, uint64_t pol)
+{
+    uint4 v;
+    asm volatile("ld.global.nc.L2::cache_hint.v4.u32 {%0, %1, %2, %3}, [%4], %5;"
+                 : "=r"(v.x), "=r"(v.y), "=r"(v.z), "=r"(v.w)
+                 : "l"(p), "l"(pol));
+    return v;
+}
+__device__ __forceinline__ int ld_once_i32(const int *p, uint64_t pol)
+{
+    int v;
+    asm("ld.global.nc.L1::no_allocate.L2::cache_hint.s32 %0, [%1], %2;" : "=r"(v) : "l"(p), "l"(pol));
+    return v;
+}
+__device__ __forceinline__ float ld_once_f32(const float *p, uint64_t pol)
+{
+    float v;
+    asm("ld.global.nc.L1::no_allocate.L2::cache_hint.f32 %0, [%1], %2;" : "=f"(v) : "l"(p), "l"(pol));
+    return v;
+}
 __device__ __forceinline__ void st_stream16(uint4 *p, const uint4 &v)
 {
     asm volatile("st.global.cs.v4.u32 [%0], {%1, %2, %3, %4};" ::"l"(p), "r"(v.x), "r"(v.y),
@@ -187,6 +208,100 @@ cudaError_t run_pool(const void *P, const int *idx, const float *w, void *out, l
     return cudaGetLastError();
 }
 
+// ---- column-slab variant: keep the gathered table L2-resident -------------------------------------
+// When P is larger than L2 but n_src * SLAB bytes fits in it, the pool runs slab by slab over the
+// feature columns: pass s gathers only bytes [s*SLAB, (s+1)*SLAB) of every row, a strided sub-table
+// of n_src * SLAB bytes that stays in L2 after its first touch, so P crosses HBM about once instead
+// of ~T times.  The price is that the (id, weight) tables are re-read once per slab (they are
+// streamed through shared memory, coalesced).  Slabs are the slow grid dimension: all CTAs of slab
+// s are scheduled before those of slab s+1.  A group of LPN = SLAB/16 lanes owns one node, a warp
+// owns 32/LPN consecutive nodes whose table entries are contiguous in memory.  Per element the
+// sum still runs t = 0..T-1 in fp32: results are bit-identical to pool_kernel.
+template <bool BF16, int LPN, int U>
+__global__ void __launch_bounds__(256, 4)
+pool_slab_kernel(const uint4 *__restrict__ P, const int *__restrict__ idx, const float *__restrict__ w,
+                 uint4 *__restrict__ out, long long n_dst, int T, int chunks, unsigned blocks_per_slab)
+{
+    using C = Chunk<BF16>;
+    constexpr int NPW = 32 / LPN;
+    extern __shared__ __align__(16) unsigned char pool_smem[];
+    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+    const int sl = lane % LPN, grp = lane / LPN;
+    const unsigned slab = blockIdx.x / blocks_per_slab, dblk = blockIdx.x % blocks_per_slab;
+    const long long v0 = ((long long)dblk * 8 + wid) * NPW;     // first node of this warp
+    if (v0 >= n_dst) return;
+    const int nv = (int)min((long long)NPW, n_dst - v0);
+    int *sidx = reinterpret_cast<int *>(pool_smem) + (size_t)wid * NPW * T * 2;
+    float *sw = reinterpret_cast<float *>(sidx + NPW * T);
+    const int *irow = idx + v0 * T;
+    const float *wrow = w + v0 * T;
+    uint64_t pol_keep, pol_once;
+    asm volatile("createpolicy.fractional.L2::evict_last.b64 %0, 1.0;" : "=l"(pol_keep));
+    asm volatile("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(pol_once));
+    for (int i = lane; i < nv * T; i += 32) {
+        sidx[i] = ld_once_i32(irow + i, pol_once);
+        sw[i] = ld_once_f32(wrow + i, pol_once);
+    }
+    __syncwarp();
+    const bool active = grp < nv;
+    const int g = active ? grp : nv - 1;
+    const uint4 *base = P + (size_t)slab * LPN + sl;
+    float acc[C::E];
+#pragma unroll
+    for (int e = 0; e < C::E; ++e) acc[e] = 0.f;
+    const int *gi = sidx + g * T;
+    const float *gw = sw + g * T;
+    int t = 0;
+    for (; t + U <= T; t += U) {
+        uint4 r[U];
+        float wt[U];
+#pragma unroll
+        for (int u = 0; u < U; ++u) {
+            r[u] = ld_row16_keep(base + (size_t)gi[t + u] * (size_t)chunks, pol_keep);
+            wt[u] = gw[t + u];
+        }
+#pragma unroll
+        for (int u = 0; u < U; ++u) C::fma(r[u], wt[u], acc);
+    }
+    for (; t < T; ++t) C::fma(ld_row16_keep(base + (size_t)gi[t] * (size_t)chunks, pol_keep), gw[t], acc);
+    if (active)
+        st_stream16(out + (size_t)(v0 + grp) * (size_t)chunks + (size_t)slab * LPN + sl, C::pack(acc));
+}
+
+template <bool BF16, int LPN>
+cudaError_t run_pool_slab(const void *P, const int *idx, const float *w, void *out, long long n_dst,
+                          int T, int chunks, cudaStream_t s)
+{
+    constexpr int NPW = 32 / LPN;
+    constexpr int U = 10;
+    const long long bps = (n_dst + 8 * NPW - 1) / (8 * NPW);
+    const long long nslabs = chunks / LPN;
+    if (bps * nslabs > 0x7fffffffLL) return cudaErrorInvalidConfiguration;
+    const size_t smem = (size_t)8 * NPW * T * 8;
+    auto kern = pool_slab_kernel<BF16, LPN, U>;
+    if (smem > 48 * 1024) {
+        cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        if (e != cudaSuccess) return e;
+    }
+    kern<<<(unsigned)(bps * nslabs), 256, smem, s>>>(static_cast<const uint4 *>(P), idx, w,
+                                                      static_cast<uint4 *>(out), n_dst, T, chunks,
+                                                      (unsigned)bps);
+    return cudaGetLastError();
+}
+
+// slab_bytes in {32, 64, 128}; requires row bytes % slab_bytes == 0 and the staging to fit smem.
+template <bool BF16>
+cudaError_t dispatch_pool_slab(int slab_bytes, const void *P, const int *idx, const float *w, void *out,
+                               long long n_dst, int T, int chunks, cudaStream_t s)
+{
+    switch (slab_bytes) {
+    case 32: return run_pool_slab<BF16, 2>(P, idx, w, out, n_dst, T, chunks, s);
+    case 64: return run_pool_slab<BF16, 4>(P, idx, w, out, n_dst, T, chunks, s);
+    case 128: return run_pool_slab<BF16, 8>(P, idx, w, out, n_dst, T, chunks, s);
+    }
+    return cudaErrorNotSupported;
+}
+
 template <bool BF16>
 cudaError_t dispatch_pool(const void *P, const int *idx, const float *w, void *out,
                           long long n_dst, int T, int chunks, cudaStream_t s)
@@ -242,12 +357,25 @@ __global__ void fix_first_bad(long long *p)
 
 }  // namespace
 
+bool pool_slab_ok(DType dt, int32_t T, int32_t m, int slab_bytes)
+{
+    if (slab_bytes != 32 && slab_bytes != 64 && slab_bytes != 128) return false;
+    const size_t row = (size_t)m * elem_size(dt);
+    const size_t smem = (size_t)8 * (32 / (slab_bytes / 16)) * T * 8;
+    return row % slab_bytes == 0 && row > (size_t)slab_bytes && smem <= 200 * 1024;
+}
+
 cudaError_t launch_pool(DType dt, int64_t n_dst, int32_t T, int32_t m, const void *P,
-                        const int32_t *idx, const float *w, void *out, cudaStream_t s, int *launches)
+                        const int32_t *idx, const float *w, void *out, int slab_bytes, cudaStream_t s,
+                        int *launches)
 {
     if (n_dst <= 0) return cudaSuccess;
     const int chunks = (int)((size_t)m * elem_size(dt) / 16);
     if (launches) ++*launches;
+    if (slab_bytes > 0 && pool_slab_ok(dt, T, m, slab_bytes))
+        return dt == DType::BF16
+                   ? dispatch_pool_slab<true>(slab_bytes, P, idx, w, out, n_dst, T, chunks, s)
+                   : dispatch_pool_slab<false>(slab_bytes, P, idx, w, out, n_dst, T, chunks, s);
     return dt == DType::BF16 ? dispatch_pool<true>(P, idx, w, out, n_dst, T, chunks, s)
                              : dispatch_pool<false>(P, idx, w, out, n_dst, T, chunks, s);
 }

@@ -137,6 +137,31 @@ def test_pool_matches_oracle(ctx, dtype, n_dst, n_src, T, m):
                       tol=4e-3 if dtype == torch.bfloat16 else 2e-6)
 
 
+@pytest.mark.parametrize("dtype", DTYPES)
+@pytest.mark.parametrize("slab", [32, 64, 128])
+@pytest.mark.parametrize("n_dst,n_src,T,m", [(3001, 2000, 50, 256), (515, 4000, 100, 256),
+                                             (77, 300, 7, 512), (1, 9, 1, 128), (640, 640, 33, 192)])
+def test_pool_column_slab_mode_is_bit_identical(ctx, dtype, slab, n_dst, n_src, T, m):
+    """The L2-resident column-slab schedule (option pool_slab) keeps the per-element summation
+    order t = 0..T-1, so it must reproduce the whole-row kernel bit for bit (and hence the oracle
+    within the same tolerance)."""
+    P = _rand((n_src, m), dtype, 40 + m).to(DEV)
+    idx, counts = _graph(n_dst, T, 41 + T, n_src=n_src)
+    w = torch.from_numpy(O.normalize_counts(counts.numpy())).to(DEV)
+    bits = torch.int16 if dtype == torch.bfloat16 else torch.int32
+    try:
+        ctx.pinsage_set_option("pool_slab", 0)
+        whole = ctx.pinsage_pool(P, idx.to(DEV), w)
+        ctx.pinsage_set_option("pool_slab", slab)
+        slabbed = ctx.pinsage_pool(P, idx.to(DEV), w)
+    finally:
+        ctx.pinsage_set_option("pool_slab", -1)
+    assert torch.equal(whole.view(bits), slabbed.view(bits))
+    ref = O.pool(to_f64(P), idx.numpy(), w.cpu().numpy())
+    assert_rows_close(to_f64(slabbed), ref, dtype, f"slab pool {slab}",
+                      tol=4e-3 if dtype == torch.bfloat16 else 2e-6)
+
+
 def test_pool_is_deterministic_and_order_invariant_within_tolerance(ctx):
     P = _rand((5000, 256), torch.bfloat16, 12).to(DEV)
     idx, counts = _graph(4000, 50, 13, n_src=5000)
