@@ -186,6 +186,27 @@ def workload_config(cfg, args, n_nodes=None):
             "l2": "inputs larger than L2 (features + tables + P exceed 126 MB; no flush needed)"}
 
 
+# ----------------------------------------------------------------------------- multi-rank host logic
+def replica_config(cfg, rank: int):
+    """Replicas only: rank r embeds its own graph, drawn with seed + r."""
+    return cfg if rank == 0 else dataclasses.replace(cfg, seed=cfg.seed + rank)
+
+
+def max_over_ranks(ms: float, world: int, device) -> float:
+    """The step time of the job is the slowest rank's (all-reduce MAX; identity at world 1)."""
+    import torch
+    import torch.distributed as dist
+    t = torch.tensor([ms], dtype=torch.float64, device=device)
+    if world > 1:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def job_throughput(n_per_rank: int, steps: int, world: int, ms_max: float) -> float:
+    """Whole-job nodes/s: every rank embeds n_per_rank nodes per step (weak scaling)."""
+    return n_per_rank * steps * world / (ms_max * 1e-3)
+
+
 # ----------------------------------------------------------------------------- the CUDA arm
 def run_ours(args, cfg):
     import torch
@@ -210,7 +231,7 @@ def run_ours(args, cfg):
         torch.cuda.synchronize()
 
     # ---- seeded synthetic inputs of the workload's shape, generated on the device -------------
-    rcfg = cfg if rank == 0 else dataclasses.replace(cfg, seed=cfg.seed + rank)
+    rcfg = replica_config(cfg, rank)
     X = synth.make_features(rcfg, device=dev)
     layers, head = synth.make_params(rcfg, device=dev)
     idx, counts = synth.make_graph(rcfg, device=dev)
@@ -252,10 +273,7 @@ def run_ours(args, cfg):
     ctx.pinsage_set_option("profile", 0)
     ctx.pinsage_profile_read(-1)
     clocks = sampler.stop() if rank == 0 else None
-    t = torch.tensor([ms], dtype=torch.float64, device=dev)
-    if world > 1:
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-    ms_max = float(t.item())
+    ms_max = max_over_ranks(ms, world, dev)
     assert torch.isfinite(out[:: max(1, cfg.N // 4096)].float()).all()
 
     # ---- e2e: the same public call with pinned HOST buffers, copies inside the timed region ---
@@ -283,12 +301,10 @@ def run_ours(args, cfg):
             step_host()
         e1.record()
         barrier()
-        te = torch.tensor([e0.elapsed_time(e1)], dtype=torch.float64, device=dev)
-        if world > 1:
-            dist.all_reduce(te, op=dist.ReduceOp.MAX)
+        te_max = max_over_ranks(e0.elapsed_time(e1), world, dev)
         assert torch.equal(hO[:1024].view(torch.int16 if e == 2 else torch.int32),
                            out[:1024].cpu().view(torch.int16 if e == 2 else torch.int32))
-        e2e = {"value": cfg.N * nrep * world / (float(te.item()) * 1e-3), "unit": UNIT,
+        e2e = {"value": job_throughput(cfg.N, nrep, world, te_max), "unit": UNIT,
                "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h, "steps": nrep}
         del hX, hI, hW, hO
 
@@ -323,7 +339,7 @@ def run_ours(args, cfg):
     kernels["pool"]["gbs"] = pool_gbs
 
     line = {
-        "metric": METRIC, "value": cfg.N * args.steps * world / (ms_max * 1e-3), "unit": UNIT,
+        "metric": METRIC, "value": job_throughput(cfg.N, args.steps, world, ms_max), "unit": UNIT,
         "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
         "ms_per_step": ms_max / args.steps, "higher_is_better": True, "scaling": "weak",
         "vs_baseline": None, "dtype": "bf16" if cfg.dtype == "bf16" else "f32",
