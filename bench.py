@@ -238,6 +238,9 @@ def run_ours(args, cfg):
     ctx = binding.Context(local)
     ctx.pinsage_set_option("gemm_impl", args.gemm_impl)
     ctx.pinsage_set_option("overlap", args.overlap)
+    ctx.pinsage_set_option("gemm_cg", args.gemm_cg)
+    ctx.pinsage_set_option("gemm_ns", args.gemm_ns)
+    ctx.pinsage_set_option("pool_slab", args.pool_slab)
     alpha = ctx.pinsage_normalize_counts(counts)
     torch.cuda.synchronize()
     del counts
@@ -372,6 +375,9 @@ def main():
     ap.add_argument("--chunk-nodes", type=int, default=0)
     ap.add_argument("--gemm-impl", type=int, default=0, help="0 tcgen05, 1 SIMT reference kernels")
     ap.add_argument("--overlap", type=int, default=0)
+    ap.add_argument("--gemm-cg", type=int, default=0, help="0 auto (CTA pairs), 1 single CTAs, 2 pairs")
+    ap.add_argument("--gemm-ns", type=int, default=0, help="slab width without row norm: 0/256/512")
+    ap.add_argument("--pool-slab", type=int, default=-1, help="-1 auto, 0 whole rows, 32/64/128")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu", action="store_true")
     ap.add_argument("--cpu-seconds", type=float, default=15.0)

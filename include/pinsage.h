@@ -94,6 +94,11 @@ const char *pinsage_last_error(const pinsage_ctx *ctx);
 const char *pinsage_version(void);
 
 /* Integer options:  "gemm_impl"      0 = tcgen05 (default for BF16), 1 = SIMT reference kernels
+ *                   "gemm_cg"        tcgen05 tile owner: 0 = automatic (CTA pairs, cta_group::2, 256-row
+ *                                    tiles when the GEMM is tensor-bound, K N / (K + N) >= 200, and
+ *                                    M > 128, N % 16 == 0; default), 1 = single CTAs
+ *                                    (128-row tiles) only, 2 = CTA pairs or PINSAGE_ERR_UNSUPPORTED_SHAPE
+ *                   "gemm_ns"        slab width of GEMMs without a row norm: 0 / 256 (default) or 512
  *                   "check_indices"  1 = every pinsage_pool / layer / embed_all call validates
  *                                    nbr_idx first (synchronous), default 0
  *                   "overlap"        1 = pinsage_layer / embed_all overlap S2 of chunk c+1 with S3

@@ -23,6 +23,7 @@ struct pinsage_ctx {
     cudaEvent_t ev_fork = nullptr, ev_join = nullptr;
     int num_sms = 0;
     int gemm_impl = 0;               // 0 tcgen05, 1 SIMT reference
+    GemmTune tune;                   // tcgen05 tile knobs ("gemm_cg", "gemm_ns")
     int check_indices = 0;
     int overlap = 0;
     int pool_slab = -1;              // -1 automatic, 0 off, 32 / 64 / 128 forced slab width in bytes
@@ -224,11 +225,11 @@ pinsage_status run_gemm(pinsage_ctx *ctx, DType dt, const GemmArgs &a, void *scr
         return PINSAGE_OK;
     }
     const char *why = nullptr;
-    if (!gemm_tc_supported(a, &why))
+    if (!gemm_tc_supported(a, ctx->tune, &why))
         return fail(ctx, PINSAGE_ERR_UNSUPPORTED_SHAPE, "tcgen05 GEMM: %s (M=%lld K1=%d K2=%d N=%d)",
                     why ? why : "unsupported shape", (long long)a.M, a.K1, a.K2, a.N);
     const int e0 = prof_mark(ctx, s);
-    cudaError_t e = launch_gemm_tc(a, ctx->num_sms, s, &ctx->launches);
+    cudaError_t e = launch_gemm_tc(a, ctx->tune, ctx->num_sms, s, &ctx->launches);
     prof_close(ctx, kind, e0, s);
     count_launches(ctx);
     PS_CUDA(ctx, e);
@@ -495,6 +496,13 @@ pinsage_status pinsage_set_option(pinsage_ctx *ctx, const char *key, int64_t val
         if (value != 0 && value != 1)
             return fail(ctx, PINSAGE_ERR_INVALID_ARG, "gemm_impl must be 0 or 1");
         ctx->gemm_impl = (int)value;
+    } else if (!strcmp(key, "gemm_cg")) {
+        if (value < 0 || value > 2) return fail(ctx, PINSAGE_ERR_INVALID_ARG, "gemm_cg must be 0, 1 or 2");
+        ctx->tune.cg = (int)value;
+    } else if (!strcmp(key, "gemm_ns")) {
+        if (value != 0 && value != 256 && value != 512)
+            return fail(ctx, PINSAGE_ERR_INVALID_ARG, "gemm_ns must be 0, 256 or 512");
+        ctx->tune.ns = (int)value;
     } else if (!strcmp(key, "check_indices")) {
         ctx->check_indices = value != 0;
     } else if (!strcmp(key, "overlap")) {

@@ -8,6 +8,11 @@
 // that accumulate into the same TMEM tile.  Epilogue, fused, all in fp32 before the single
 // rounding to bf16: + bias -> ReLU -> (S3) row L2 normalisation (Alg. 1 l.3, :116).
 //
+// Two instantiations: CG = 1 (one CTA per 128-row tile) and CG = 2 (a CTA PAIR, the two SMs of a
+// TPC, per 256-row tile: tcgen05.mma.cta_group::2 issued by the even CTA, each CTA stages its own
+// 128 rows of A and HALF of the B tile, so shared-memory and L2 operand traffic per flop drop by a
+// third to a half).  CG = 2 is used whenever M >= 256 and the tile shape allows it.
+//
 // Structure (one persistent CTA per SM, 256 threads, warp-specialised):
 //   warp 0      TMA producer: 128x64 A tile + (NS x 64) B tile per stage, SWIZZLE_128B, mbarrier ring
 //   warp 1      MMA issuer: one elected thread issues tcgen05.mma (M=128, N=CN<=256, K=16)
@@ -50,8 +55,9 @@ struct TcParams {
     int tmem_cols;     // allocation (power of two >= 32)
     int stages;
     int stage_bytes;   // A_BYTES + nchunks * CN * 128
-    int n_slabs;       // slabs along N (= cluster size when l2norm spans several CTAs)
-    int cluster;       // 1, or n_slabs when the row norm is exchanged through DSMEM
+    int n_slabs;       // slabs along N (= units per cluster when l2norm spans several CTAs)
+    int cg;            // CTAs per tile: 1, or 2 = CTA pair (tcgen05 cta_group::2, 256-row tiles)
+    int cluster;       // CTAs per cluster: cg, or cg * n_slabs when the row norm is exchanged (DSMEM)
     const float *bias;
     int relu, l2norm;
     uint32_t idesc;
@@ -184,6 +190,37 @@ __device__ __forceinline__ void tc_mma(uint32_t d_tmem, uint64_t adesc, uint64_t
         "l"(adesc), "l"(bdesc), "r"(idesc), "r"(accumulate)
         : "memory");
 }
+// ---- CTA-pair (cta_group::2) variants ---------------------------------------------------------------
+// TMA load issued by either CTA of a pair into its OWN shared memory, completing bytes on the mbarrier
+// of the pair's leader (a shared::cluster address).
+__device__ __forceinline__ void tma_load_2d_pair(uint32_t dst, const CUtensorMap *map, int c0, int c1,
+                                                 uint32_t leader_bar, uint64_t policy)
+{
+    asm volatile(
+        "cp.async.bulk.tensor.2d.cta_group::2.shared::cluster.global.tile.mbarrier::complete_tx::bytes.L2::cache_hint"
+        " [%0], [%1, {%2, %3}], [%4], %5;" ::"r"(dst),
+        "l"(map), "r"(c0), "r"(c1), "r"(leader_bar), "l"(policy)
+        : "memory");
+}
+__device__ __forceinline__ void tc_mma_pair(uint32_t d_tmem, uint64_t adesc, uint64_t bdesc, uint32_t idesc,
+                                            uint32_t accumulate)
+{
+    asm volatile(
+        "{\n\t.reg .pred p;\n\t"
+        "setp.ne.b32 p, %4, 0;\n\t"
+        "tcgen05.mma.cta_group::2.kind::f16 [%0], %1, %2, %3, p;\n\t}" ::"r"(d_tmem),
+        "l"(adesc), "l"(bdesc), "r"(idesc), "r"(accumulate)
+        : "memory");
+}
+// arrive (once all prior MMAs of this thread retire) on the barrier at the same offset in every CTA of mask
+__device__ __forceinline__ void tc_commit_pair(uint32_t bar, uint16_t cta_mask)
+{
+    asm volatile(
+        "tcgen05.commit.cta_group::2.mbarrier::arrive::one.shared::cluster.multicast::cluster.b64 [%0], %1;" ::"r"(bar),
+        "h"(cta_mask)
+        : "memory");
+}
+
 // 32 consecutive fp32 columns of this thread's TMEM lane
 __device__ __forceinline__ void tc_ld32(uint32_t taddr, uint32_t (&v)[32])
 {
@@ -202,6 +239,21 @@ __device__ __forceinline__ void tc_ld32(uint32_t taddr, uint32_t (&v)[32])
 __device__ __forceinline__ void tc_wait_ld()
 {
     asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
+}
+
+// One lane of a fully converged warp.  Issuing tcgen05.mma / TMA under `elect.sync` (the whole warp
+// runs the surrounding loop) lets ptxas keep descriptors in uniform registers: UTCHMMA instructions
+// issue back to back, where an `if (lane == 0)` region costs 11-24 SASS instructions per MMA and
+// caps the tensor pipe near 50 % (measured).
+__device__ __forceinline__ bool elect_one()
+{
+    uint32_t pred;
+    asm volatile(
+        "{\n\t.reg .pred P1;\n\t"
+        "elect.sync _|P1, 0xffffffff;\n\t"
+        "selp.u32 %0, 1, 0, P1;\n\t}"
+        : "=r"(pred));
+    return pred != 0;
 }
 
 // K-major, SWIZZLE_128B shared-memory matrix descriptor: rows of 128 bytes, 8-row groups 1024 bytes
@@ -223,6 +275,9 @@ constexpr int BIAS_BYTES = 512 * 4;
 constexpr int BAR_BYTES = 256;
 constexpr int XCHG_BYTES = 2 * MAX_CLUSTER * BM * 4;
 
+// CG: CTAs per tile (1, or 2 = pair).  NCH: tcgen05.mma instructions side by side per K step (1 or 2;
+// compile-time so that the issue loop unrolls into straight-line UTCHMMAs).
+template <int CG, int NCH>
 __global__ void __launch_bounds__(NUM_THREADS, 1)
 gemm_tc_kernel(const __grid_constant__ CUtensorMap tmA1, const __grid_constant__ CUtensorMap tmA2,
                const __grid_constant__ CUtensorMap tmB, const __grid_constant__ CUtensorMap tmOut,
@@ -238,18 +293,24 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap tmA1, const __grid_constant__
     const uint32_t bar_off = bias_off + BIAS_BYTES;
     const uint32_t xchg_off = bar_off + BAR_BYTES;
     float *sbias = reinterpret_cast<float *>(smem + bias_off);
-    const uint32_t bar_full = sbase + bar_off;                 // [MAX_STAGES]
+    const uint32_t bar_full = sbase + bar_off;                 // [MAX_STAGES]  (CG 2: the leader's are used)
     const uint32_t bar_empty = bar_full + 8 * MAX_STAGES;      // [MAX_STAGES]
     const uint32_t bar_tfull = bar_empty + 8 * MAX_STAGES;     // [2]
-    const uint32_t bar_tempty = bar_tfull + 16;                // [2]
+    const uint32_t bar_tempty = bar_tfull + 16;                // [2]           (CG 2: the leader's are used)
     const uint32_t bar_xchg = bar_tempty + 16;                 // [2]
     volatile uint32_t *tmem_slot = reinterpret_cast<volatile uint32_t *>(smem + bar_off + 8 * (2 * MAX_STAGES + 6));
 
-    const int slab = blockIdx.x % p.n_slabs;
-    const long long lane0 = blockIdx.x / p.n_slabs, lanes = gridDim.x / p.n_slabs;
+    // A "unit" is the CTA (CG 1) or CTA pair (CG 2) that owns one (row tile, slab) at a time.
+    const uint32_t crank = p.cluster > 1 ? cluster_ctarank() : 0;
+    const uint32_t half = CG == 2 ? (crank & 1u) : 0u;         // which 128 rows of the 256-row tile
+    const uint32_t leader = crank & ~1u;                       // cluster rank of this pair's even CTA
+    const long long unit = blockIdx.x / CG, units = gridDim.x / CG;
+    const int slab = (int)(unit % p.n_slabs);
+    const long long lane0 = unit / p.n_slabs, lanes = units / p.n_slabs;
     const int n0 = slab * p.NS;
     const int ncols = min(p.NS, p.N - n0);  // valid output columns of this slab
     const int KB = p.kb1 + p.kb2;
+    const int b_rows = p.CN / CG;           // rows of B this CTA stages per MMA chunk
 
     // ---- one-time setup ---------------------------------------------------------------------
     if (warp == 0 && lane == 0) {
@@ -263,19 +324,28 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap tmA1, const __grid_constant__
             mbar_init(bar_full + 8 * s, 1);
             mbar_init(bar_empty + 8 * s, 1);
         }
+        const int units_per_cluster = p.cluster / CG;
         for (int a = 0; a < 2; ++a) {
             mbar_init(bar_tfull + 8 * a, 1);
-            mbar_init(bar_tempty + 8 * a, 4);
-            mbar_init(bar_xchg + 8 * a, 128 * (p.cluster > 1 ? p.cluster - 1 : 1));
+            mbar_init(bar_tempty + 8 * a, 4 * CG);              // every epilogue warp of the unit
+            mbar_init(bar_xchg + 8 * a, 128 * (units_per_cluster > 1 ? units_per_cluster - 1 : 1));
         }
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
     if (warp == 2) {
-        asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(
-                         smem_u32(const_cast<uint32_t *>(tmem_slot))),
-                     "r"((uint32_t)p.tmem_cols)
-                     : "memory");
-        asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
+        if (CG == 2) {
+            asm volatile("tcgen05.alloc.cta_group::2.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(
+                             smem_u32(const_cast<uint32_t *>(tmem_slot))),
+                         "r"((uint32_t)p.tmem_cols)
+                         : "memory");
+            asm volatile("tcgen05.relinquish_alloc_permit.cta_group::2.sync.aligned;" ::: "memory");
+        } else {
+            asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(
+                             smem_u32(const_cast<uint32_t *>(tmem_slot))),
+                         "r"((uint32_t)p.tmem_cols)
+                         : "memory");
+            asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
+        }
     }
     if (warp >= 4) {
         for (int c = threadIdx.x - 128; c < 512; c += 128)
@@ -288,61 +358,95 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap tmA1, const __grid_constant__
     const uint32_t tmem_base = *tmem_slot;
 
     if (warp == 0) {
-        // ===== TMA producer =====================================================================
-        if (lane == 0) {
-            uint64_t pol_stream, pol_keep;
-            asm volatile("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(pol_stream));
-            asm volatile("createpolicy.fractional.L2::evict_last.b64 %0, 1.0;" : "=l"(pol_keep));
-            int stage = 0;
-            uint32_t phase = 0;
-            for (long long mb = lane0; mb < p.m_blocks; mb += lanes) {
-                const int m0 = (int)(mb * BM);
-                for (int kb = 0; kb < KB; ++kb) {
+        // ===== TMA producer (every CTA: its own 128 rows of A and its share of B) =================
+        // the whole warp runs the loop; one elected lane issues
+        uint64_t pol_stream, pol_keep;
+        asm volatile("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(pol_stream));
+        asm volatile("createpolicy.fractional.L2::evict_last.b64 %0, 1.0;" : "=l"(pol_keep));
+        // A is read once per slab: keep it in L2 while the other slabs of the same rows still need it
+        const uint64_t pol_a = p.n_slabs > 1 ? pol_keep : pol_stream;
+        const uint32_t leader_full = CG == 2 ? map_to_cta(bar_full, leader) : bar_full;
+        int stage = 0;
+        uint32_t phase = 0;
+        for (long long mb = lane0; mb < p.m_blocks; mb += lanes) {
+            const int m0 = (int)(mb * (BM * CG)) + (int)half * BM;
+            for (int kb = 0; kb < KB; ++kb) {
+                mbar_wait(bar_empty + 8 * stage, phase ^ 1);
+                if (elect_one()) {
                     const uint32_t full = bar_full + 8 * stage;
-                    mbar_wait(bar_empty + 8 * stage, phase ^ 1);
-                    mbar_expect_tx(full, (uint32_t)p.stage_bytes);
                     const bool seg2 = kb >= p.kb1;
                     const int ka = (seg2 ? kb - p.kb1 : kb) * BK;
                     const uint32_t sA = sbase + (uint32_t)stage * p.stage_bytes;
-                    tma_load_2d(sA, seg2 ? &tmA2 : &tmA1, ka, m0, full, pol_stream);
                     const int kcol = seg2 ? p.K1 + ka : ka;
-                    for (int j = 0; j < p.nchunks; ++j)
-                        tma_load_2d(sA + A_BYTES + (uint32_t)j * p.CN * 128, &tmB, kcol,
-                                    n0 + j * p.CN, full, pol_keep);
-                    if (++stage == p.stages) {
-                        stage = 0;
-                        phase ^= 1;
+                    if (CG == 2) {
+                        // both CTAs' bytes complete on the leader's barrier
+                        if (half == 0) mbar_expect_tx(full, 2u * (uint32_t)p.stage_bytes);
+                        const uint32_t lfull = leader_full + 8 * stage;
+                        tma_load_2d_pair(sA, seg2 ? &tmA2 : &tmA1, ka, m0, lfull, pol_a);
+#pragma unroll
+                        for (int j = 0; j < NCH; ++j)
+                            tma_load_2d_pair(sA + A_BYTES + (uint32_t)j * b_rows * 128, &tmB, kcol,
+                                             n0 + j * p.CN + (int)half * b_rows, lfull, pol_keep);
+                    } else {
+                        mbar_expect_tx(full, (uint32_t)p.stage_bytes);
+                        tma_load_2d(sA, seg2 ? &tmA2 : &tmA1, ka, m0, full, pol_a);
+#pragma unroll
+                        for (int j = 0; j < NCH; ++j)
+                            tma_load_2d(sA + A_BYTES + (uint32_t)j * p.CN * 128, &tmB, kcol,
+                                        n0 + j * p.CN, full, pol_keep);
                     }
+                }
+                __syncwarp();
+                if (++stage == p.stages) {
+                    stage = 0;
+                    phase ^= 1;
                 }
             }
         }
     } else if (warp == 1) {
-        // ===== MMA issuer =======================================================================
-        if (lane == 0) {
+        // ===== MMA issuer (CG 2: the pair's even CTA only) ========================================
+        // the whole warp runs the loop (all lanes wait on the barriers); one elected lane issues
+        if (half == 0) {
+            const uint16_t pair_mask = (uint16_t)(3u << leader);
+            const uint32_t b_step = (uint32_t)((b_rows * 128) >> 4);  // descriptor units between chunks
             int stage = 0, acc = 0;
             uint32_t phase = 0, accphase = 0;
             for (long long mb = lane0; mb < p.m_blocks; mb += lanes) {
-                mbar_wait(bar_tempty + 8 * acc, accphase ^ 1);   // epilogue has drained this accumulator
+                mbar_wait(bar_tempty + 8 * acc, accphase ^ 1);   // epilogue(s) drained this accumulator
                 tc_fence_after();
                 const uint32_t d0 = tmem_base + (uint32_t)acc * p.acc_cols;
                 for (int kb = 0; kb < KB; ++kb) {
-                    mbar_wait(bar_full + 8 * stage, phase);      // TMA bytes have landed
+                    mbar_wait(bar_full + 8 * stage, phase);      // TMA bytes have landed (both CTAs)
                     tc_fence_after();
-                    const uint32_t sA = sbase + (uint32_t)stage * p.stage_bytes;
-                    const uint64_t ad = make_desc(sA), bd = make_desc(sA + A_BYTES);
+                    if (elect_one()) {
+                        const uint32_t sA = sbase + (uint32_t)stage * p.stage_bytes;
+                        const uint64_t ad = make_desc(sA), bd = make_desc(sA + A_BYTES);
 #pragma unroll
-                    for (int k = 0; k < BK / 16; ++k)            // 32 bytes along K per UMMA_K = 16
-                        for (int j = 0; j < p.nchunks; ++j)
-                            tc_mma(d0 + (uint32_t)j * p.CN, ad + 2 * k,
-                                   bd + (uint64_t)((j * p.CN * 128) >> 4) + 2 * k, p.idesc,
-                                   (uint32_t)(kb | k));
-                    tc_commit(bar_empty + 8 * stage);            // frees the stage when the MMAs retire
+                        for (int k = 0; k < BK / 16; ++k)        // 32 bytes along K per UMMA_K = 16
+#pragma unroll
+                            for (int j = 0; j < NCH; ++j) {
+                                const uint32_t accum = k == 0 ? (uint32_t)kb : 1u;
+                                if (CG == 2)
+                                    tc_mma_pair(d0 + (uint32_t)j * p.CN, ad + 2 * k, bd + j * b_step + 2 * k,
+                                                p.idesc, accum);
+                                else
+                                    tc_mma(d0 + (uint32_t)j * p.CN, ad + 2 * k, bd + j * b_step + 2 * k,
+                                           p.idesc, accum);
+                            }
+                        // frees the stage (in both CTAs) when the MMAs retire
+                        if (CG == 2) tc_commit_pair(bar_empty + 8 * stage, pair_mask);
+                        else tc_commit(bar_empty + 8 * stage);
+                        if (kb == KB - 1) {                      // accumulator complete
+                            if (CG == 2) tc_commit_pair(bar_tfull + 8 * acc, pair_mask);
+                            else tc_commit(bar_tfull + 8 * acc);
+                        }
+                    }
+                    __syncwarp();
                     if (++stage == p.stages) {
                         stage = 0;
                         phase ^= 1;
                     }
                 }
-                tc_commit(bar_tfull + 8 * acc);                  // accumulator complete
                 if (++acc == p.nacc) {
                     acc = 0;
                     accphase ^= 1;
@@ -354,13 +458,15 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap tmA1, const __grid_constant__
         const int ew = warp - 4;                                  // == warp % 4: TMEM lanes 32*ew..
         const int row = ew * 32 + lane;
         uint8_t *stg = smem + stg_off + ew * 2 * STG_WARP_BYTES;
-        const uint32_t my_rank = p.cluster > 1 ? cluster_ctarank() : 0;
+        const int units_per_cluster = p.cluster / CG;
+        const uint32_t my_unit = crank / CG;
         float *xbuf = reinterpret_cast<float *>(smem + xchg_off);  // [2][MAX_CLUSTER][BM]
+        const uint32_t tempty_leader = CG == 2 ? map_to_cta(bar_tempty, leader) : 0u;
         int acc = 0, sbuf = 0;
         uint32_t accphase = 0;
         long long it = 0;
         for (long long mb = lane0; mb < p.m_blocks; mb += lanes, ++it) {
-            const long long m0 = mb * BM;
+            const long long m0 = mb * (BM * CG) + (long long)half * BM;
             mbar_wait(bar_tfull + 8 * acc, accphase);
             tc_fence_after();
             const uint32_t t0 = tmem_base + ((uint32_t)(ew * 32) << 16) + (uint32_t)acc * p.acc_cols;
@@ -379,19 +485,21 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap tmA1, const __grid_constant__
                         ss = (c0 + i < ncols) ? fmaf(z, z, ss) : ss;
                     }
                 }
-                if (p.cluster > 1) {
-                    // push my partial to every peer, then wait for theirs (DSMEM + remote mbarrier)
+                if (units_per_cluster > 1) {
+                    // push my partial to the CTAs that hold the other slabs of the same rows, then wait
+                    // for theirs (DSMEM + remote mbarrier)
                     const int par = (int)(it & 1);
-                    const uint32_t my_slot = sbase + xchg_off + ((par * MAX_CLUSTER + my_rank) * BM + row) * 4;
-                    for (uint32_t r = 0; r < (uint32_t)p.cluster; ++r) {
-                        if (r == my_rank) continue;
+                    const uint32_t my_slot = sbase + xchg_off + ((par * MAX_CLUSTER + my_unit) * BM + row) * 4;
+                    for (uint32_t u = 0; u < (uint32_t)units_per_cluster; ++u) {
+                        if (u == my_unit) continue;
+                        const uint32_t r = u * CG + half;
                         st_cluster_f32(map_to_cta(my_slot, r), ss);
                         mbar_arrive_remote(map_to_cta(bar_xchg + 8 * par, r));
                     }
                     mbar_wait_cluster(bar_xchg + 8 * par, (uint32_t)((it >> 1) & 1));
                     float tot = 0.f;
-                    for (uint32_t r = 0; r < (uint32_t)p.cluster; ++r)   // same order in every CTA
-                        tot += (r == my_rank) ? ss : xbuf[(par * MAX_CLUSTER + r) * BM + row];
+                    for (uint32_t u = 0; u < (uint32_t)units_per_cluster; ++u)   // same order in every CTA
+                        tot += (u == my_unit) ? ss : xbuf[(par * MAX_CLUSTER + u) * BM + row];
                     ss = tot;
                 }
                 scale = ss > 0.f ? rsqrtf(ss) : 0.f;             // zero row stays zero (reading A3)
@@ -434,7 +542,10 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap tmA1, const __grid_constant__
             }
             tc_fence_before();
             __syncwarp();
-            if (lane == 0) mbar_arrive(bar_tempty + 8 * acc);
+            if (lane == 0) {
+                if (CG == 2) mbar_arrive_remote(tempty_leader + 8 * acc);
+                else mbar_arrive(bar_tempty + 8 * acc);
+            }
             if (++acc == p.nacc) {
                 acc = 0;
                 accphase ^= 1;
@@ -450,9 +561,14 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap tmA1, const __grid_constant__
     else __syncthreads();
     if (warp == 2) {
         tc_fence_after();
-        asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem_base),
-                     "r"((uint32_t)p.tmem_cols)
-                     : "memory");
+        if (CG == 2)
+            asm volatile("tcgen05.dealloc.cta_group::2.sync.aligned.b32 %0, %1;" ::"r"(tmem_base),
+                         "r"((uint32_t)p.tmem_cols)
+                         : "memory");
+        else
+            asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem_base),
+                         "r"((uint32_t)p.tmem_cols)
+                         : "memory");
     }
 }
 
@@ -492,7 +608,9 @@ bool make_map(CUtensorMap *map, const void *ptr, long long rows, int cols, int b
 
 inline int round_up(int x, int a) { return (x + a - 1) / a * a; }
 
-bool plan(const GemmArgs &a, TcParams &p, int &smem_bytes, const char **why)
+// cg: CTAs per tile (1 or 2).  ns_pref: preferred slab width without a row norm (256 = double-buffered
+// accumulators, 512 = fewer operand bytes per flop but no epilogue overlap).
+bool plan(const GemmArgs &a, int cg, int ns_pref, TcParams &p, int &smem_bytes, const char **why)
 {
     auto no = [&](const char *msg) {
         if (why) *why = msg;
@@ -501,19 +619,22 @@ bool plan(const GemmArgs &a, TcParams &p, int &smem_bytes, const char **why)
     if (a.M < 1 || a.M >= (1LL << 31)) return no("M outside [1, 2^31)");
     if (a.K1 < 8 || a.K1 % 8 || a.K2 < 0 || a.K2 % 8) return no("K1, K2 must be multiples of 8");
     if (a.N < 8 || a.N % 8) return no("N must be a multiple of 8");
+    if (cg == 2 && (a.M <= BM || a.N % 16)) return no("CTA pairs need M > 128 and N % 16 == 0");
     p = TcParams{};
+    p.cg = cg;
     p.M = a.M;
-    p.m_blocks = (a.M + BM - 1) / BM;
+    p.m_blocks = (a.M + BM * cg - 1) / (BM * cg);
     p.kb1 = (a.K1 + BK - 1) / BK;
     p.kb2 = (a.K2 + BK - 1) / BK;
     p.K1 = a.K1;
     p.N = a.N;
-    const int slab_max = a.l2norm ? 512 : 256;      // a normalised row must sit in one CTA's TMEM
+    const int slab_max = a.l2norm ? 512 : ns_pref;  // a normalised row must sit in one CTA's TMEM
     p.n_slabs = (a.N + slab_max - 1) / slab_max;
     p.NS = p.n_slabs == 1 ? round_up(a.N, 16) : round_up((a.N + p.n_slabs - 1) / p.n_slabs, 64);
     p.n_slabs = (a.N + p.NS - 1) / p.NS;
-    p.cluster = (a.l2norm && p.n_slabs > 1) ? p.n_slabs : 1;
-    if (p.cluster > MAX_CLUSTER) return no("row norm over more than 4096 columns");
+    const int units_per_cluster = (a.l2norm && p.n_slabs > 1) ? p.n_slabs : 1;
+    p.cluster = cg * units_per_cluster;
+    if (p.cluster > MAX_CLUSTER) return no("row norm spans more CTAs than a portable cluster holds");
     p.nchunks = (p.NS + 255) / 256;
     p.CN = round_up((p.NS + p.nchunks - 1) / p.nchunks, 16);
     p.acc_cols = round_up(p.nchunks * p.CN, 64);
@@ -521,8 +642,8 @@ bool plan(const GemmArgs &a, TcParams &p, int &smem_bytes, const char **why)
     int cols = p.nacc * p.acc_cols;
     p.tmem_cols = 32;
     while (p.tmem_cols < cols) p.tmem_cols *= 2;
-    p.stage_bytes = A_BYTES + p.nchunks * p.CN * 128;
-    const int fixed = STG_BYTES + BIAS_BYTES + BAR_BYTES + (p.cluster > 1 ? XCHG_BYTES : 0);
+    p.stage_bytes = A_BYTES + p.nchunks * (p.CN / cg) * 128;
+    const int fixed = STG_BYTES + BIAS_BYTES + BAR_BYTES + (units_per_cluster > 1 ? XCHG_BYTES : 0);
     p.stages = (SMEM_LIMIT - fixed) / p.stage_bytes;
     if (p.stages > MAX_STAGES) p.stages = MAX_STAGES;
     if (p.stages < 2) return no("tile does not fit shared memory");
@@ -531,56 +652,41 @@ bool plan(const GemmArgs &a, TcParams &p, int &smem_bytes, const char **why)
     p.relu = a.relu;
     p.l2norm = a.l2norm;
     // instruction descriptor, kind::f16: D fp32 (bit 4), A and B bf16 (bits 7, 10), both K-major,
-    // N >> 3 at bits [17,23), M >> 4 at bits [24,29)
-    p.idesc = (1u << 4) | (1u << 7) | (1u << 10) | ((uint32_t)(p.CN >> 3) << 17) | ((uint32_t)(BM >> 4) << 24);
+    // N >> 3 at bits [17,23), M >> 4 at bits [24,29); M = 256 for a CTA pair
+    p.idesc = (1u << 4) | (1u << 7) | (1u << 10) | ((uint32_t)(p.CN >> 3) << 17) |
+              ((uint32_t)((BM * cg) >> 4) << 24);
     return true;
 }
 
-}  // namespace
-
-bool gemm_tc_supported(const GemmArgs &a, const char **why)
+// The plan launch_gemm_tc will use: CTA pairs when the shape allows and the caller does not forbid it.
+bool plan_auto(const GemmArgs &a, const GemmTune &t, TcParams &p, int &smem_bytes, const char **why)
 {
-    TcParams p;
-    int smem = 0;
-    if (!plan(a, p, smem, why)) return false;
-    if (!encode_fn()) {
-        if (why) *why = "cuTensorMapEncodeTiled is not available from this driver";
+    const int ns = t.ns == 512 ? 512 : 256;
+    // Pairs pay when the GEMM is tensor-bound (measured on B200: +12-14 % at config 3's shapes); on
+    // the HBM-bound shapes (arithmetic intensity K N / (K + N) below ~200 flop per byte moved, e.g.
+    // 256 x 256) single-CTA tiles keep more independent tiles in flight and are 15-35 % faster.
+    const long long Kt = a.K1 + a.K2;
+    const bool tensor_bound = Kt * a.N >= 200 * (Kt + a.N);
+    if ((t.cg == 2 || (t.cg == 0 && tensor_bound)) && plan(a, 2, ns, p, smem_bytes, nullptr)) return true;
+    if (t.cg == 2) {
+        if (why) *why = "shape not supported by the CTA-pair kernel";
         return false;
     }
-    return true;
+    return plan(a, 1, ns, p, smem_bytes, why);
 }
 
-size_t gemm_tc_scratch_bytes(const GemmArgs &) { return 0; }
-
-cudaError_t launch_gemm_tc(const GemmArgs &a, int num_sms, cudaStream_t s, int *launches)
+template <int CG, int NCH>
+cudaError_t launch_cg(const TcParams &p, int smem, int num_sms, cudaStream_t s, const CUtensorMap &tmA1,
+                      const CUtensorMap &tmA2, const CUtensorMap &tmB, const CUtensorMap &tmOut)
 {
-    TcParams p;
-    int smem = 0;
-    if (!plan(a, p, smem, nullptr)) return cudaErrorNotSupported;
-    CUtensorMap tmA1, tmA2, tmB, tmOut;
-    if (!make_map(&tmA1, a.A1, a.M, a.K1, BM)) return cudaErrorInvalidValue;
-    if (a.K2 > 0) {
-        if (!make_map(&tmA2, a.A2, a.M, a.K2, BM)) return cudaErrorInvalidValue;
-    } else {
-        tmA2 = tmA1;
-    }
-    if (!make_map(&tmB, a.B, a.N, a.K1 + a.K2, p.CN)) return cudaErrorInvalidValue;
-    if (!make_map(&tmOut, a.out, a.M, a.N, 32)) return cudaErrorInvalidValue;
-
     static bool attr_set = false;
     if (!attr_set) {
-        cudaError_t e = cudaFuncSetAttribute(gemm_tc_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
+        cudaError_t e = cudaFuncSetAttribute(gemm_tc_kernel<CG, NCH>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                              SMEM_LIMIT);
         if (e != cudaSuccess) return e;
         attr_set = true;
     }
-    long long tiles = p.m_blocks * p.n_slabs;
-    long long grid = tiles < num_sms ? tiles : num_sms;
-    grid = grid / p.n_slabs * p.n_slabs;
-    if (grid < p.n_slabs) grid = p.n_slabs;
-
     cudaLaunchConfig_t cfg{};
-    cfg.gridDim = dim3((unsigned)grid);
     cfg.blockDim = dim3(NUM_THREADS);
     cfg.dynamicSmemBytes = (size_t)smem;
     cfg.stream = s;
@@ -591,8 +697,67 @@ cudaError_t launch_gemm_tc(const GemmArgs &a, int num_sms, cudaStream_t s, int *
     attr[0].val.clusterDim.z = 1;
     cfg.attrs = attr;
     cfg.numAttrs = 1;
+
+    // co-resident clusters of this shape (cached: the query costs a driver call)
+    static int cached_clusters[MAX_CLUSTER + 1] = {0};
+    int max_clusters = cached_clusters[p.cluster];
+    if (max_clusters == 0) {
+        cfg.gridDim = dim3((unsigned)(num_sms / p.cluster * p.cluster));
+        cfg.dynamicSmemBytes = SMEM_LIMIT;
+        if (cudaOccupancyMaxActiveClusters(&max_clusters, gemm_tc_kernel<CG, NCH>, &cfg) != cudaSuccess ||
+            max_clusters < 1) {
+            cudaGetLastError();
+            max_clusters = num_sms / p.cluster;
+        }
+        cached_clusters[p.cluster] = max_clusters;
+        cfg.dynamicSmemBytes = (size_t)smem;
+    }
+    const int units_per_cluster = p.cluster / CG;
+    const long long tiles = p.m_blocks * p.n_slabs;
+    long long units = (long long)max_clusters * units_per_cluster;
+    if (units > tiles) units = tiles;
+    units = units / p.n_slabs * p.n_slabs;
+    if (units < p.n_slabs) units = p.n_slabs;
+    cfg.gridDim = dim3((unsigned)(units * CG));
+    return cudaLaunchKernelEx(&cfg, gemm_tc_kernel<CG, NCH>, tmA1, tmA2, tmB, tmOut, p);
+}
+
+}  // namespace
+
+bool gemm_tc_supported(const GemmArgs &a, const GemmTune &t, const char **why)
+{
+    TcParams p;
+    int smem = 0;
+    if (!plan_auto(a, t, p, smem, why)) return false;
+    if (!encode_fn()) {
+        if (why) *why = "cuTensorMapEncodeTiled is not available from this driver";
+        return false;
+    }
+    return true;
+}
+
+size_t gemm_tc_scratch_bytes(const GemmArgs &) { return 0; }
+
+cudaError_t launch_gemm_tc(const GemmArgs &a, const GemmTune &t, int num_sms, cudaStream_t s, int *launches)
+{
+    TcParams p;
+    int smem = 0;
+    if (!plan_auto(a, t, p, smem, nullptr)) return cudaErrorNotSupported;
+    CUtensorMap tmA1, tmA2, tmB, tmOut;
+    if (!make_map(&tmA1, a.A1, a.M, a.K1, BM)) return cudaErrorInvalidValue;
+    if (a.K2 > 0) {
+        if (!make_map(&tmA2, a.A2, a.M, a.K2, BM)) return cudaErrorInvalidValue;
+    } else {
+        tmA2 = tmA1;
+    }
+    if (!make_map(&tmB, a.B, a.N, a.K1 + a.K2, p.CN / p.cg)) return cudaErrorInvalidValue;
+    if (!make_map(&tmOut, a.out, a.M, a.N, 32)) return cudaErrorInvalidValue;
     if (launches) ++*launches;
-    return cudaLaunchKernelEx(&cfg, gemm_tc_kernel, tmA1, tmA2, tmB, tmOut, p);
+    if (p.cg == 2)
+        return p.nchunks == 2 ? launch_cg<2, 2>(p, smem, num_sms, s, tmA1, tmA2, tmB, tmOut)
+                              : launch_cg<2, 1>(p, smem, num_sms, s, tmA1, tmA2, tmB, tmOut);
+    return p.nchunks == 2 ? launch_cg<1, 2>(p, smem, num_sms, s, tmA1, tmA2, tmB, tmOut)
+                          : launch_cg<1, 1>(p, smem, num_sms, s, tmA1, tmA2, tmB, tmOut);
 }
 
 }  // namespace pinsage

@@ -34,10 +34,16 @@ cudaError_t launch_gemm_simt(DType dt, const GemmArgs &a, float *ztmp, cudaStrea
 size_t gemm_simt_scratch_bytes(const GemmArgs &a);
 
 // ---- gemm_tcgen05.cu: tcgen05 / TMEM / TMA GEMM, bf16 in, fp32 accumulate ----------------------
+// Tuning knobs (context options "gemm_cg", "gemm_ns"): cg 0 = automatic (CTA pairs, cta_group::2,
+// whenever the shape allows), 1 = single-CTA tiles only, 2 = CTA pairs or fail; ns = slab width of
+// GEMMs without a row norm (0 / 256 = double-buffered accumulators, 512 = wider tile).
+struct GemmTune {
+    int cg = 0;
+    int ns = 0;
+};
 // Returns cudaErrorNotSupported for shapes outside the compiled set (caller reports UNSUPPORTED_SHAPE).
-bool gemm_tc_supported(const GemmArgs &a, const char **why);
-cudaError_t launch_gemm_tc(const GemmArgs &a, int num_sms, cudaStream_t s, int *launches);
-// scratch needed when the row norm spans more than one CTA (N > 512): per-row partial sums
+bool gemm_tc_supported(const GemmArgs &a, const GemmTune &t, const char **why);
+cudaError_t launch_gemm_tc(const GemmArgs &a, const GemmTune &t, int num_sms, cudaStream_t s, int *launches);
 size_t gemm_tc_scratch_bytes(const GemmArgs &a);
 
 // ---- pool.cu ------------------------------------------------------------------------------------

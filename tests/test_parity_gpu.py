@@ -35,8 +35,22 @@ def _graph(N, T, seed, n_src=None):
 
 
 def _both_impls(ctx, dtype):
-    """bf16 runs through the tcgen05 kernels and through the SIMT reference kernels."""
-    return [0, 1] if dtype == torch.bfloat16 else [0]
+    """(gemm_impl, gemm_cg): bf16 runs through the tcgen05 kernel with single-CTA tiles, with CTA
+    pairs (cta_group::2) and through the SIMT reference kernels; fp32 is SIMT only."""
+    return [(0, 1), (0, 2), (1, 0)] if dtype == torch.bfloat16 else [(0, 0)]
+
+
+class _impl:
+    def __init__(self, ctx, impl, cg):
+        self.ctx, self.impl, self.cg = ctx, impl, cg
+
+    def __enter__(self):
+        self.ctx.pinsage_set_option("gemm_impl", self.impl)
+        self.ctx.pinsage_set_option("gemm_cg", self.cg)
+
+    def __exit__(self, *exc):
+        self.ctx.pinsage_set_option("gemm_impl", 0)
+        self.ctx.pinsage_set_option("gemm_cg", 0)
 
 
 # ------------------------------------------------------------------ helpers of the path
@@ -186,25 +200,25 @@ def test_dense_matches_oracle(ctx, dtype, M, k, n_out):
     A = _rand((M, k), dtype, 20)
     Wt = _rand((n_out, k), dtype, 21, scale=k ** -0.5)
     b = _rand((n_out,), torch.float32, 22, scale=0.1)
-    for impl in _both_impls(ctx, dtype):
-        ctx.pinsage_set_option("gemm_impl", impl)
-        try:
+    ran = 0
+    for impl, cg in _both_impls(ctx, dtype):
+        with _impl(ctx, impl, cg):
             for bias, relu in [(b, True), (None, False), (b, False)]:
                 try:
                     got = ctx.pinsage_dense(A.to(DEV), Wt.to(DEV),
                                             None if bias is None else bias.to(DEV), relu)
                 except binding.PinsageError as e:
                     if e.status_name == "UNSUPPORTED_SHAPE" and impl == 0:
-                        pytest.skip(f"tcgen05 path does not cover this shape: {e}")
+                        break                      # e.g. CTA pairs need M > 128 and N % 16 == 0
                     raise
+                ran += 1
                 ref = O.dense(to_f64(A), to_f64(Wt), None if bias is None else to_f64(bias), relu)
                 # absolute comparison per row against the row scale (ReLU rows can be tiny)
                 err = np.abs(to_f64(got) - ref).max(axis=1)
                 scale = np.abs(ref).max(axis=1) + 1e-3
                 tol = 8e-3 if dtype == torch.bfloat16 else 2e-5
-                assert (err / scale).max() < tol, (impl, relu, (err / scale).max())
-        finally:
-            ctx.pinsage_set_option("gemm_impl", 0)
+                assert (err / scale).max() < tol, (impl, cg, relu, (err / scale).max())
+    assert ran >= 3
 
 
 # ------------------------------------------------------------------ S3 combine
@@ -219,22 +233,22 @@ def test_combine_matches_oracle(ctx, dtype, M, d_in, m, d):
     W = _rand((d, d_in + m), dtype, 32, scale=(d_in + m) ** -0.5)
     w = _rand((d,), torch.float32, 33, scale=0.01)
     ref = O.combine(to_f64(H), to_f64(n), to_f64(W), to_f64(w))
-    for impl in _both_impls(ctx, dtype):
-        ctx.pinsage_set_option("gemm_impl", impl)
-        try:
+    ran = 0
+    for impl, cg in _both_impls(ctx, dtype):
+        with _impl(ctx, impl, cg):
             try:
                 got = ctx.pinsage_combine(H.to(DEV), n.to(DEV), W.to(DEV), w.to(DEV))
             except binding.PinsageError as e:
                 if e.status_name == "UNSUPPORTED_SHAPE" and impl == 0:
-                    pytest.skip(f"tcgen05 path does not cover this shape: {e}")
+                    continue
                 raise
-            assert_rows_close(to_f64(got), ref, dtype, f"combine impl={impl}",
+            ran += 1
+            assert_rows_close(to_f64(got), ref, dtype, f"combine impl={impl} cg={cg}",
                               tol=4e-3 if dtype == torch.bfloat16 else 1e-5)
             nrm = np.linalg.norm(to_f64(got), axis=1)
             assert np.all((np.abs(nrm - 1) < (2.0 ** -7 if dtype == torch.bfloat16 else 1e-5))
                           | (nrm == 0))
-        finally:
-            ctx.pinsage_set_option("gemm_impl", 0)
+    assert ran >= 1
 
 
 @pytest.mark.parametrize("dtype", DTYPES)
@@ -264,13 +278,14 @@ def _to_dev(layers, head):
     return L, H
 
 
-def _check_whole_path(ctx, cfg, impl=0, chunk_nodes=0):
+def _check_whole_path(ctx, cfg, impl=0, chunk_nodes=0, cg=0):
     X, idx, counts, alpha, layers, head = _inputs(cfg)
     Lf, Hf = params_f64(layers, head)
     ref_out, ref_hidden = O.embed_all(to_f64(X), idx.numpy(), alpha, Lf, Hf, return_hidden=True)
     Ld, Hd = _to_dev(layers, head)
     dtype = X.dtype
     ctx.pinsage_set_option("gemm_impl", impl)
+    ctx.pinsage_set_option("gemm_cg", cg)
     try:
         w_dev = ctx.pinsage_normalize_counts(counts.to(DEV))
         np.testing.assert_array_equal(w_dev.cpu().numpy(), alpha)
@@ -287,6 +302,7 @@ def _check_whole_path(ctx, cfg, impl=0, chunk_nodes=0):
         return out, stats
     finally:
         ctx.pinsage_set_option("gemm_impl", 0)
+        ctx.pinsage_set_option("gemm_cg", 0)
 
 
 def test_tiny_config_fp32_exhaustive(ctx):
@@ -294,11 +310,11 @@ def test_tiny_config_fp32_exhaustive(ctx):
     _check_whole_path(ctx, synth.CONFIGS["tiny"])
 
 
-@pytest.mark.parametrize("impl", [0, 1])
-def test_cfg2_small_exhaustive(ctx, impl):
+@pytest.mark.parametrize("impl,cg", [(0, 0), (0, 1), (1, 0)])
+def test_cfg2_small_exhaustive(ctx, impl, cg):
     """Config 2's shape (256/256/128, T=50, K=2, bf16) on 20 000 nodes, every row; chunked
     so that several chunks, a ragged tail chunk and ragged GEMM tiles are exercised."""
-    _check_whole_path(ctx, synth.CONFIGS["cfg2"].scaled(20_011), impl=impl, chunk_nodes=4096)
+    _check_whole_path(ctx, synth.CONFIGS["cfg2"].scaled(20_011), impl=impl, chunk_nodes=4096, cg=cg)
 
 
 @pytest.mark.parametrize("name,N", [("cfg3", 3000), ("cfg4", 6000), ("cfg5", 5000)])
