@@ -240,6 +240,7 @@ def run_ours(args, cfg):
     ctx.pinsage_set_option("overlap", args.overlap)
     ctx.pinsage_set_option("gemm_cg", args.gemm_cg)
     ctx.pinsage_set_option("gemm_ns", args.gemm_ns)
+    ctx.pinsage_set_option("gemm_epi", args.gemm_epi)
     ctx.pinsage_set_option("pool_slab", args.pool_slab)
     alpha = ctx.pinsage_normalize_counts(counts)
     torch.cuda.synchronize()
@@ -377,6 +378,7 @@ def main():
     ap.add_argument("--overlap", type=int, default=0)
     ap.add_argument("--gemm-cg", type=int, default=0, help="0 auto (CTA pairs), 1 single CTAs, 2 pairs")
     ap.add_argument("--gemm-ns", type=int, default=0, help="slab width without row norm: 0/256/512")
+    ap.add_argument("--gemm-epi", type=int, default=0, help="0 auto (8 epilogue warps), 1 four")
     ap.add_argument("--pool-slab", type=int, default=-1, help="-1 auto, 0 whole rows, 32/64/128")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu", action="store_true")

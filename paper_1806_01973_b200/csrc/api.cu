@@ -503,6 +503,9 @@ pinsage_status pinsage_set_option(pinsage_ctx *ctx, const char *key, int64_t val
         if (value != 0 && value != 256 && value != 512)
             return fail(ctx, PINSAGE_ERR_INVALID_ARG, "gemm_ns must be 0, 256 or 512");
         ctx->tune.ns = (int)value;
+    } else if (!strcmp(key, "gemm_epi")) {
+        if (value != 0 && value != 1) return fail(ctx, PINSAGE_ERR_INVALID_ARG, "gemm_epi must be 0 or 1");
+        ctx->tune.epi = (int)value;
     } else if (!strcmp(key, "check_indices")) {
         ctx->check_indices = value != 0;
     } else if (!strcmp(key, "overlap")) {

@@ -36,7 +36,7 @@ constexpr int BK = 64;                   // K elements per stage: 128 bytes = on
 constexpr int A_BYTES = BM * BK * 2;     // 16 KB
 constexpr int OUT_CHUNK = 64;            // columns per output staging chunk / TMA store box
 constexpr int STG_WARP_BYTES = 32 * OUT_CHUNK * 2;  // 4 KB: 32 rows x 128 B
-constexpr int NUM_THREADS = 256;
+constexpr int NUM_THREADS = 384;        // 4 role warps + up to 8 epilogue warps
 constexpr int MAX_STAGES = 8;
 constexpr int MAX_CLUSTER = 8;
 constexpr int SMEM_LIMIT = 227 * 1024;
@@ -55,6 +55,10 @@ struct TcParams {
     int tmem_cols;     // allocation (power of two >= 32)
     int stages;
     int stage_bytes;   // A_BYTES + nchunks * CN * 128
+    int epi_halves;    // 1: four epilogue warps own all columns; 2: eight warps, two per row quarter,
+                       // each owning half of the slab's columns
+    int c_split;       // first column of the second half (multiple of 64)
+    int stg_bytes;     // output staging: epi_halves * 4 warps * 2 buffers * 4 KB
     int n_slabs;       // slabs along N (= units per cluster when l2norm spans several CTAs)
     int cg;            // CTAs per tile: 1, or 2 = CTA pair (tcgen05 cta_group::2, 256-row tiles)
     int cluster;       // CTAs per cluster: cg, or cg * n_slabs when the row norm is exchanged (DSMEM)
@@ -266,13 +270,14 @@ __device__ __forceinline__ uint64_t make_desc(uint32_t saddr)
 
 // Shared-memory plan (offsets from the 1024-byte aligned dynamic base):
 //   [0, stages*stage_bytes)   operand ring: per stage A (16 KB) then B (nchunks*CN rows x 128 B)
-//   + 32 KB                   output staging: 4 epilogue warps x 2 buffers x (32 rows x 128 B)
+//   + 32 / 64 KB              output staging: 4 / 8 epilogue warps x 2 buffers x (32 rows x 128 B)
 //   + 2 KB                    bias of this CTA's slab (fp32, zero beyond N)
 //   + 256 B                   mbarriers, TMEM base address
+//   + 2 KB                    row sum-of-squares exchange between the two column halves [2][2][128] fp32
 //   + 8 KB (cluster > 1)      row-norm exchange [2][MAX_CLUSTER][128] fp32
-constexpr int STG_BYTES = 4 * 2 * STG_WARP_BYTES;
 constexpr int BIAS_BYTES = 512 * 4;
 constexpr int BAR_BYTES = 256;
+constexpr int HALF_BYTES = 2 * 2 * BM * 4;
 constexpr int XCHG_BYTES = 2 * MAX_CLUSTER * BM * 4;
 
 // CG: CTAs per tile (1, or 2 = pair).  NCH: tcgen05.mma instructions side by side per K step (1 or 2;
@@ -289,9 +294,10 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap tmA1, const __grid_constant__
 
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const uint32_t stg_off = (uint32_t)p.stages * p.stage_bytes;
-    const uint32_t bias_off = stg_off + STG_BYTES;
+    const uint32_t bias_off = stg_off + (uint32_t)p.stg_bytes;
     const uint32_t bar_off = bias_off + BIAS_BYTES;
-    const uint32_t xchg_off = bar_off + BAR_BYTES;
+    const uint32_t half_off = bar_off + BAR_BYTES;
+    const uint32_t xchg_off = half_off + (p.epi_halves == 2 ? HALF_BYTES : 0);
     float *sbias = reinterpret_cast<float *>(smem + bias_off);
     const uint32_t bar_full = sbase + bar_off;                 // [MAX_STAGES]  (CG 2: the leader's are used)
     const uint32_t bar_empty = bar_full + 8 * MAX_STAGES;      // [MAX_STAGES]
@@ -327,7 +333,7 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap tmA1, const __grid_constant__
         const int units_per_cluster = p.cluster / CG;
         for (int a = 0; a < 2; ++a) {
             mbar_init(bar_tfull + 8 * a, 1);
-            mbar_init(bar_tempty + 8 * a, 4 * CG);              // every epilogue warp of the unit
+            mbar_init(bar_tempty + 8 * a, 4 * CG * p.epi_halves);  // every epilogue warp of the unit
             mbar_init(bar_xchg + 8 * a, 128 * (units_per_cluster > 1 ? units_per_cluster - 1 : 1));
         }
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
@@ -347,7 +353,7 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap tmA1, const __grid_constant__
             asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
         }
     }
-    if (warp >= 4) {
+    if (warp >= 4 && warp < 8) {
         for (int c = threadIdx.x - 128; c < 512; c += 128)
             sbias[c] = (p.bias != nullptr && c < ncols) ? __ldg(p.bias + n0 + c) : 0.f;
     }
@@ -453,14 +459,19 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap tmA1, const __grid_constant__
                 }
             }
         }
-    } else if (warp >= 4) {
-        // ===== epilogue: thread (ew, lane) owns output row m0 + 32*ew + lane =====================
-        const int ew = warp - 4;                                  // == warp % 4: TMEM lanes 32*ew..
+    } else if (warp >= 4 && ((warp - 4) >> 2) < p.epi_halves) {
+        // ===== epilogue: thread (ew, lane) owns output row m0 + 32*ew + lane; with eight warps the two
+        // warps of a row quarter each own one half of the slab's columns =============================
+        const int ew = warp & 3;                                  // == warp % 4: TMEM lanes 32*ew..
+        const int eh = (warp - 4) >> 2;                           // column half
         const int row = ew * 32 + lane;
-        uint8_t *stg = smem + stg_off + ew * 2 * STG_WARP_BYTES;
+        const int c_lo = eh == 0 ? 0 : p.c_split;
+        const int c_hi = (p.epi_halves == 2 && eh == 0) ? min(p.c_split, ncols) : ncols;
+        uint8_t *stg = smem + stg_off + (eh * 4 + ew) * 2 * STG_WARP_BYTES;
         const int units_per_cluster = p.cluster / CG;
         const uint32_t my_unit = crank / CG;
         float *xbuf = reinterpret_cast<float *>(smem + xchg_off);  // [2][MAX_CLUSTER][BM]
+        float *hbuf = reinterpret_cast<float *>(smem + half_off);  // [2][2][BM]
         const uint32_t tempty_leader = CG == 2 ? map_to_cta(bar_tempty, leader) : 0u;
         int acc = 0, sbuf = 0;
         uint32_t accphase = 0;
@@ -472,9 +483,10 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap tmA1, const __grid_constant__
             const uint32_t t0 = tmem_base + ((uint32_t)(ew * 32) << 16) + (uint32_t)acc * p.acc_cols;
             float scale = 1.f;
             if (p.l2norm) {
-                // pass 1: sum of squares of this row's z = act(acc + bias), columns in order
+                // pass 1: sum of squares of this row's z = act(acc + bias) over my columns, in order
+                const int par = (int)(it & 1);
                 float ss = 0.f;
-                for (int c0 = 0; c0 < ncols; c0 += 32) {
+                for (int c0 = c_lo; c0 < c_hi; c0 += 32) {
                     uint32_t v[32];
                     tc_ld32(t0 + c0, v);
                     tc_wait_ld();
@@ -482,19 +494,26 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap tmA1, const __grid_constant__
                     for (int i = 0; i < 32; ++i) {
                         float z = __uint_as_float(v[i]) + sbias[c0 + i];
                         z = p.relu ? fmaxf(z, 0.f) : z;
-                        ss = (c0 + i < ncols) ? fmaf(z, z, ss) : ss;
+                        ss = (c0 + i < c_hi) ? fmaf(z, z, ss) : ss;
                     }
                 }
+                if (p.epi_halves == 2) {
+                    // the two warps of this row quarter add their halves (fixed order: low + high)
+                    hbuf[(par * 2 + eh) * BM + row] = ss;
+                    asm volatile("bar.sync %0, 64;" ::"r"(1 + ew) : "memory");
+                    ss = hbuf[(par * 2 + 0) * BM + row] + hbuf[(par * 2 + 1) * BM + row];
+                }
                 if (units_per_cluster > 1) {
-                    // push my partial to the CTAs that hold the other slabs of the same rows, then wait
-                    // for theirs (DSMEM + remote mbarrier)
-                    const int par = (int)(it & 1);
-                    const uint32_t my_slot = sbase + xchg_off + ((par * MAX_CLUSTER + my_unit) * BM + row) * 4;
-                    for (uint32_t u = 0; u < (uint32_t)units_per_cluster; ++u) {
-                        if (u == my_unit) continue;
-                        const uint32_t r = u * CG + half;
-                        st_cluster_f32(map_to_cta(my_slot, r), ss);
-                        mbar_arrive_remote(map_to_cta(bar_xchg + 8 * par, r));
+                    // push my slab's partial to the CTAs that hold the other slabs of the same rows
+                    // (low-half warps only), then wait for theirs (DSMEM + remote mbarrier)
+                    if (eh == 0) {
+                        const uint32_t my_slot = sbase + xchg_off + ((par * MAX_CLUSTER + my_unit) * BM + row) * 4;
+                        for (uint32_t u = 0; u < (uint32_t)units_per_cluster; ++u) {
+                            if (u == my_unit) continue;
+                            const uint32_t r = u * CG + half;
+                            st_cluster_f32(map_to_cta(my_slot, r), ss);
+                            mbar_arrive_remote(map_to_cta(bar_xchg + 8 * par, r));
+                        }
                     }
                     mbar_wait_cluster(bar_xchg + 8 * par, (uint32_t)((it >> 1) & 1));
                     float tot = 0.f;
@@ -505,7 +524,7 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap tmA1, const __grid_constant__
                 scale = ss > 0.f ? rsqrtf(ss) : 0.f;             // zero row stays zero (reading A3)
             }
             // pass 2: 64 columns at a time -> bf16 -> swizzled staging -> TMA store
-            for (int c0 = 0; c0 < ncols; c0 += OUT_CHUNK) {
+            for (int c0 = c_lo; c0 < c_hi; c0 += OUT_CHUNK) {
                 uint32_t v[2][32];
                 tc_ld32(t0 + c0, v[0]);
                 tc_ld32(t0 + c0 + 32, v[1]);
@@ -610,7 +629,7 @@ inline int round_up(int x, int a) { return (x + a - 1) / a * a; }
 
 // cg: CTAs per tile (1 or 2).  ns_pref: preferred slab width without a row norm (256 = double-buffered
 // accumulators, 512 = fewer operand bytes per flop but no epilogue overlap).
-bool plan(const GemmArgs &a, int cg, int ns_pref, TcParams &p, int &smem_bytes, const char **why)
+bool plan(const GemmArgs &a, int cg, int ns_pref, int epi_pref, TcParams &p, int &smem_bytes, const char **why)
 {
     auto no = [&](const char *msg) {
         if (why) *why = msg;
@@ -643,10 +662,22 @@ bool plan(const GemmArgs &a, int cg, int ns_pref, TcParams &p, int &smem_bytes, 
     p.tmem_cols = 32;
     while (p.tmem_cols < cols) p.tmem_cols *= 2;
     p.stage_bytes = A_BYTES + p.nchunks * (p.CN / cg) * 128;
-    const int fixed = STG_BYTES + BIAS_BYTES + BAR_BYTES + (units_per_cluster > 1 ? XCHG_BYTES : 0);
-    p.stages = (SMEM_LIMIT - fixed) / p.stage_bytes;
-    if (p.stages > MAX_STAGES) p.stages = MAX_STAGES;
+    // Eight epilogue warps (two per row quarter, half of the columns each) halve the two-pass row-norm
+    // epilogue, which is exposed when the accumulator is single-buffered (measured: S3 +3 % at config 3,
+    // +8 % at config 4; the one-pass epilogues lose more from the 32 KB of extra staging than they
+    // gain, and with double-buffered accumulators the epilogue is hidden anyway).  Used for row-norm
+    // GEMMs with a single accumulator when at least three operand stages still fit.
+    int fixed = 0;
+    for (p.epi_halves = (epi_pref == 1 || !a.l2norm || p.nacc == 2) ? 1 : 2; p.epi_halves >= 1; --p.epi_halves) {
+        p.stg_bytes = p.epi_halves * 4 * 2 * STG_WARP_BYTES;
+        fixed = p.stg_bytes + BIAS_BYTES + BAR_BYTES + (p.epi_halves == 2 ? HALF_BYTES : 0) +
+                (units_per_cluster > 1 ? XCHG_BYTES : 0);
+        p.stages = (SMEM_LIMIT - fixed) / p.stage_bytes;
+        if (p.stages > MAX_STAGES) p.stages = MAX_STAGES;
+        if (p.stages >= 3 || p.epi_halves == 1) break;
+    }
     if (p.stages < 2) return no("tile does not fit shared memory");
+    p.c_split = round_up((p.NS + 1) / 2, 64);
     smem_bytes = p.stages * p.stage_bytes + fixed;
     p.bias = a.bias;
     p.relu = a.relu;
@@ -667,12 +698,12 @@ bool plan_auto(const GemmArgs &a, const GemmTune &t, TcParams &p, int &smem_byte
     // 256 x 256) single-CTA tiles keep more independent tiles in flight and are 15-35 % faster.
     const long long Kt = a.K1 + a.K2;
     const bool tensor_bound = Kt * a.N >= 200 * (Kt + a.N);
-    if ((t.cg == 2 || (t.cg == 0 && tensor_bound)) && plan(a, 2, ns, p, smem_bytes, nullptr)) return true;
+    if ((t.cg == 2 || (t.cg == 0 && tensor_bound)) && plan(a, 2, ns, t.epi, p, smem_bytes, nullptr)) return true;
     if (t.cg == 2) {
         if (why) *why = "shape not supported by the CTA-pair kernel";
         return false;
     }
-    return plan(a, 1, ns, p, smem_bytes, why);
+    return plan(a, 1, ns, t.epi, p, smem_bytes, why);
 }
 
 template <int CG, int NCH>

@@ -40,6 +40,7 @@ size_t gemm_simt_scratch_bytes(const GemmArgs &a);
 struct GemmTune {
     int cg = 0;
     int ns = 0;
+    int epi = 0;   // epilogue warps: 0 = automatic (8 when they fit), 1 = always 4
 };
 // Returns cudaErrorNotSupported for shapes outside the compiled set (caller reports UNSUPPORTED_SHAPE).
 bool gemm_tc_supported(const GemmArgs &a, const GemmTune &t, const char **why);
