@@ -18,6 +18,9 @@ struct pinsage_ctx {
     int device = 0;
     cudaStream_t stream = nullptr;
     cudaStream_t aux = nullptr;      // second stream for S2 / S3 overlap
+    cudaStream_t h2d = nullptr;      // copy streams of the host-buffer pipeline (pinsage_embed_all)
+    cudaStream_t d2h = nullptr;
+    std::vector<cudaEvent_t> pipe_events;   // per-chunk "input landed" / "output ready" events
     cudaEvent_t ev_pool[2] = {nullptr, nullptr};
     cudaEvent_t ev_gemm[2] = {nullptr, nullptr};
     cudaEvent_t ev_fork = nullptr, ev_join = nullptr;
@@ -303,7 +306,8 @@ int64_t auto_chunk(int64_t N, int64_t requested, size_t row_bytes)
 pinsage_status pool_combine_chunks(pinsage_ctx *ctx, DType dt, int64_t N, int32_t T,
                                    const pinsage_layer_params *lp, const void *Hin, const void *P,
                                    const int32_t *idx, const float *w, void *Hout, int64_t chunk,
-                                   void *nbuf0, void *nbuf1, void *scratch, size_t scratch_bytes)
+                                   void *nbuf0, void *nbuf1, void *scratch, size_t scratch_bytes,
+                                   const cudaEvent_t *tables_landed = nullptr)
 {
     const size_t es = elem_size(dt);
     const int64_t nchunks = (N + chunk - 1) / chunk;
@@ -318,6 +322,7 @@ pinsage_status pool_combine_chunks(pinsage_ctx *ctx, DType dt, int64_t N, int32_
         const int64_t r0 = c * chunk, rows = std::min(chunk, N - r0);
         const int b = (int)(c & 1);
         if (two && c >= 2) PS_CUDA(ctx, cudaStreamWaitEvent(ps, ctx->ev_gemm[b], 0));
+        if (tables_landed) PS_CUDA(ctx, cudaStreamWaitEvent(ps, tables_landed[c], 0));
         const int pe0 = prof_mark(ctx, ps);
         cudaError_t e = launch_pool(dt, rows, T, lp->m, P, idx + (size_t)r0 * T, w + (size_t)r0 * T,
                                     nb[b], pick_slab(ctx, dt, N, T, lp->m), ps, &ctx->launches);
@@ -380,23 +385,43 @@ LayerWs plan_layer_ws(const pinsage_ctx *ctx, DType dt, int64_t N, const pinsage
     return p;
 }
 
+// feats_landed / tables_landed (host-buffer pipeline of pinsage_embed_all, layer 1 only): per-chunk
+// events recorded on the copy stream.  With feats_landed S1 runs chunk by chunk behind the copies.
 pinsage_status layer_on_ws(pinsage_ctx *ctx, DType dt, int64_t N, int32_t T, const void *feats,
                            const int32_t *idx, const float *w, const pinsage_layer_params *lp,
-                           void *out, char *ws, const LayerWs &plan, int64_t chunk)
+                           void *out, char *ws, const LayerWs &plan, int64_t chunk,
+                           const cudaEvent_t *feats_landed = nullptr,
+                           const cudaEvent_t *tables_landed = nullptr)
 {
-    GemmArgs g;
-    g.M = N;
-    g.K1 = lp->d_in;
-    g.N = lp->m;
-    g.A1 = feats;
-    g.B = lp->Q;
-    g.bias = lp->q;
-    g.relu = 1;
-    g.out = ws + plan.P_off;
-    PS_TRY(run_gemm(ctx, dt, g, ws + plan.scratch_off, plan.scratch_bytes, ctx->stream));
+    const size_t es = elem_size(dt);
+    const int64_t s1_rows = feats_landed ? chunk : N;
+    for (int64_t r0 = 0, c = 0; r0 < N; r0 += s1_rows, ++c) {
+        if (feats_landed) PS_CUDA(ctx, cudaStreamWaitEvent(ctx->stream, feats_landed[c], 0));
+        GemmArgs g;
+        g.M = std::min(s1_rows, N - r0);
+        g.K1 = lp->d_in;
+        g.N = lp->m;
+        g.A1 = static_cast<const char *>(feats) + (size_t)r0 * lp->d_in * es;
+        g.B = lp->Q;
+        g.bias = lp->q;
+        g.relu = 1;
+        g.out = ws + plan.P_off + (size_t)r0 * lp->m * es;
+        PS_TRY(run_gemm(ctx, dt, g, ws + plan.scratch_off, plan.scratch_bytes, ctx->stream));
+    }
     return pool_combine_chunks(ctx, dt, N, T, lp, feats, ws + plan.P_off, idx, w, out, chunk,
                                ws + plan.n0_off, ws + plan.n1_off, ws + plan.scratch_off,
-                               plan.scratch_bytes);
+                               plan.scratch_bytes, tables_landed);
+}
+
+// Grows the per-chunk event pool of the host-buffer pipeline to n events.
+pinsage_status ensure_pipe_events(pinsage_ctx *ctx, size_t n)
+{
+    while (ctx->pipe_events.size() < n) {
+        cudaEvent_t e;
+        PS_CUDA(ctx, cudaEventCreateWithFlags(&e, cudaEventDisableTiming));
+        ctx->pipe_events.push_back(e);
+    }
+    return PINSAGE_OK;
 }
 
 bool is_host_ptr(const void *p)
@@ -449,6 +474,8 @@ pinsage_status pinsage_create(pinsage_ctx **out, int device, void *cuda_stream)
     ctx->l2_bytes = (size_t)prop.l2CacheSize;
     DeviceGuard guard(device);
     bool ok = cudaStreamCreateWithFlags(&ctx->aux, cudaStreamNonBlocking) == cudaSuccess;
+    ok = ok && cudaStreamCreateWithFlags(&ctx->h2d, cudaStreamNonBlocking) == cudaSuccess;
+    ok = ok && cudaStreamCreateWithFlags(&ctx->d2h, cudaStreamNonBlocking) == cudaSuccess;
     for (int i = 0; i < 2 && ok; ++i) {
         ok = ok && cudaEventCreateWithFlags(&ctx->ev_pool[i], cudaEventDisableTiming) == cudaSuccess;
         ok = ok && cudaEventCreateWithFlags(&ctx->ev_gemm[i], cudaEventDisableTiming) == cudaSuccess;
@@ -474,6 +501,12 @@ void pinsage_destroy(pinsage_ctx *ctx)
         cudaStreamSynchronize(ctx->aux);
         cudaStreamDestroy(ctx->aux);
     }
+    for (cudaStream_t st : {ctx->h2d, ctx->d2h})
+        if (st) {
+            cudaStreamSynchronize(st);
+            cudaStreamDestroy(st);
+        }
+    for (cudaEvent_t e : ctx->pipe_events) cudaEventDestroy(e);
     for (int i = 0; i < 2; ++i) {
         if (ctx->ev_pool[i]) cudaEventDestroy(ctx->ev_pool[i]);
         if (ctx->ev_gemm[i]) cudaEventDestroy(ctx->ev_gemm[i]);
@@ -767,28 +800,19 @@ pinsage_status pinsage_embed_all(pinsage_ctx *ctx, pinsage_dtype dtype, int64_t 
     if (h_out) { st_out = st_off; st_off += align_up(out_bytes, 256); }
     if (any_host) PS_TRY(ensure_stage(ctx, st_off));
     char *stage = static_cast<char *>(ctx->stage);
-    const void *d_feats = feats;
-    const int32_t *d_idx = nbr_idx;
-    const float *d_w = nbr_w;
-    void *d_out = out;
-    if (h_idx) {
-        PS_CUDA(ctx, cudaMemcpyAsync(stage + st_idx, nbr_idx, tab_bytes, cudaMemcpyHostToDevice, ctx->stream));
-        d_idx = reinterpret_cast<const int32_t *>(stage + st_idx);
-    }
-    if (h_w) {
-        PS_CUDA(ctx, cudaMemcpyAsync(stage + st_w, nbr_w, tab_bytes, cudaMemcpyHostToDevice, ctx->stream));
-        d_w = reinterpret_cast<const float *>(stage + st_w);
-    }
-    if (h_feats) {
-        PS_CUDA(ctx, cudaMemcpyAsync(stage + st_feats, feats, feats_bytes, cudaMemcpyHostToDevice, ctx->stream));
-        d_feats = stage + st_feats;
-    }
-    if (h_out) d_out = stage + st_out;
+    const void *d_feats = h_feats ? static_cast<const void *>(stage + st_feats) : feats;
+    const int32_t *d_idx = h_idx ? reinterpret_cast<const int32_t *>(stage + st_idx) : nbr_idx;
+    const float *d_w = h_w ? reinterpret_cast<const float *>(stage + st_w) : nbr_w;
+    void *d_out = h_out ? static_cast<void *>(stage + st_out) : out;
 
     // ---- workspace plan: P | n0 | n1 | scratch | H_a | H_b | head chunk a ------------------------
     int32_t w_max = head->g1;
     for (int k = 0; k < K; ++k) w_max = std::max(w_max, layers[k].m);
-    const int64_t chunk = auto_chunk(N, chunk_nodes, (size_t)w_max * es);
+    int64_t chunk = auto_chunk(N, chunk_nodes, (size_t)w_max * es);
+    // host buffers: at least ~8 chunks so that copies and kernels overlap chunk by chunk
+    if (any_host && chunk_nodes == 0)
+        chunk = std::min<int64_t>(chunk, std::max<int64_t>(32768, ((N + 7) / 8 + 127) / 128 * 128));
+    const int64_t nchunks = (N + chunk - 1) / chunk;
     size_t max_layer_ws = 0;
     int32_t d_max = 0;
     for (int k = 0; k < K; ++k) {
@@ -807,6 +831,47 @@ pinsage_status pinsage_embed_all(pinsage_ctx *ctx, pinsage_dtype dtype, int64_t 
     char *Hb = need_Hb ? Ha + H_bytes : nullptr;
     char *abuf = Ha + H_bytes * (need_Hb ? 2 : 1);
 
+    // ---- host inputs: chunked H2D copies on the copy stream, features first, then the tables; the
+    // kernels of layer 1 follow them chunk by chunk (S1 behind the feature chunks, S2/S3 behind the
+    // table chunks), so that PCIe and the SMs work at the same time --------------------------------
+    const cudaEvent_t *feats_landed = nullptr, *tables_landed = nullptr;
+    cudaEvent_t *out_ready = nullptr;
+    if (any_host) {
+        PS_TRY(ensure_pipe_events(ctx, (size_t)3 * nchunks));
+        cudaEvent_t *ev = ctx->pipe_events.data();
+        // the staging buffers may still be read by kernels of an earlier call on the compute stream
+        PS_CUDA(ctx, cudaEventRecord(ctx->ev_fork, ctx->stream));
+        PS_CUDA(ctx, cudaStreamWaitEvent(ctx->h2d, ctx->ev_fork, 0));
+        PS_CUDA(ctx, cudaStreamWaitEvent(ctx->d2h, ctx->ev_fork, 0));
+        if (h_feats) {
+            const size_t rb = (size_t)layers[0].d_in * es;
+            for (int64_t c = 0; c < nchunks; ++c) {
+                const int64_t r0 = c * chunk, rows = std::min(chunk, N - r0);
+                PS_CUDA(ctx, cudaMemcpyAsync(stage + st_feats + r0 * rb, static_cast<const char *>(feats) + r0 * rb,
+                                             rows * rb, cudaMemcpyHostToDevice, ctx->h2d));
+                PS_CUDA(ctx, cudaEventRecord(ev[c], ctx->h2d));
+            }
+            feats_landed = ev;
+        }
+        if (h_idx || h_w) {
+            const size_t rb = (size_t)T * 4;
+            for (int64_t c = 0; c < nchunks; ++c) {
+                const int64_t r0 = c * chunk, rows = std::min(chunk, N - r0);
+                if (h_idx)
+                    PS_CUDA(ctx, cudaMemcpyAsync(stage + st_idx + r0 * rb, reinterpret_cast<const char *>(nbr_idx) + r0 * rb,
+                                                 rows * rb, cudaMemcpyHostToDevice, ctx->h2d));
+                if (h_w)
+                    PS_CUDA(ctx, cudaMemcpyAsync(stage + st_w + r0 * rb, reinterpret_cast<const char *>(nbr_w) + r0 * rb,
+                                                 rows * rb, cudaMemcpyHostToDevice, ctx->h2d));
+                PS_CUDA(ctx, cudaEventRecord(ev[nchunks + c], ctx->h2d));
+            }
+            tables_landed = ev + nchunks;
+        }
+        if (h_out) out_ready = ev + 2 * nchunks;
+        if (ctx->check_indices && tables_landed)     // validation reads whole tables: wait for all of them
+            PS_CUDA(ctx, cudaStreamWaitEvent(ctx->stream, tables_landed[nchunks - 1], 0));
+    }
+
     PS_TRY(maybe_validate(ctx, N, N, T, d_idx, d_w));
 
     const void *Hin = d_feats;
@@ -818,7 +883,8 @@ pinsage_status pinsage_embed_all(pinsage_ctx *ctx, pinsage_dtype dtype, int64_t 
         if (k == 0) Hout = Ha;
         else if (lp->d == lp->d_in) Hout = Hcur;           // in place (S1 has consumed all of H first)
         else Hout = (Hcur == Ha) ? Hb : Ha;
-        PS_TRY(layer_on_ws(ctx, dt, N, T, Hin, d_idx, d_w, lp, Hout, ws, plan, chunk));
+        PS_TRY(layer_on_ws(ctx, dt, N, T, Hin, d_idx, d_w, lp, Hout, ws, plan, chunk,
+                           k == 0 ? feats_landed : nullptr, k == 0 ? tables_landed : nullptr));
         Hcur = Hout;
         Hin = Hout;
     }
@@ -834,10 +900,20 @@ pinsage_status pinsage_embed_all(pinsage_ctx *ctx, pinsage_dtype dtype, int64_t 
         g2.M = rows; g2.K1 = head->g1; g2.N = head->d_out; g2.A1 = abuf; g2.B = head->G2;
         g2.out = static_cast<char *>(d_out) + (size_t)r0 * head->d_out * es;
         PS_TRY(run_gemm(ctx, dt, g2, nullptr, 0, ctx->stream));
+        if (out_ready) {                      // this chunk of out goes home while the next one is computed
+            const int64_t c = r0 / chunk;
+            const size_t rb = (size_t)head->d_out * es;
+            PS_CUDA(ctx, cudaEventRecord(out_ready[c], ctx->stream));
+            PS_CUDA(ctx, cudaStreamWaitEvent(ctx->d2h, out_ready[c], 0));
+            PS_CUDA(ctx, cudaMemcpyAsync(static_cast<char *>(out) + r0 * rb, static_cast<char *>(d_out) + r0 * rb,
+                                         rows * rb, cudaMemcpyDeviceToHost, ctx->d2h));
+        }
     }
-    if (h_out)
-        PS_CUDA(ctx, cudaMemcpyAsync(out, d_out, out_bytes, cudaMemcpyDeviceToHost, ctx->stream));
-    if (any_host) PS_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
+    if (any_host) {
+        PS_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
+        PS_CUDA(ctx, cudaStreamSynchronize(ctx->h2d));
+        PS_CUDA(ctx, cudaStreamSynchronize(ctx->d2h));
+    }
     return PINSAGE_OK;
 }
 

@@ -358,6 +358,20 @@ def test_embed_all_host_buffers_match_device_buffers(ctx):
     out_h = torch.empty((cfg.N, cfg.d_out), dtype=X.dtype).pin_memory()
     ctx.pinsage_embed_all(X.pin_memory(), idx.pin_memory(), w.pin_memory(), Ld, Hd, out=out_h)
     assert torch.equal(out_h.view(torch.int16), dev.cpu().view(torch.int16))
+    # several chunks: the copies are pipelined chunk by chunk with the kernels (ragged last chunk),
+    # pinned and pageable host memory, and a mix of host and device buffers
+    for pin in (True, False):
+        f = (lambda t: t.pin_memory()) if pin else (lambda t: t.clone())
+        out_h.zero_()
+        ctx.pinsage_embed_all(f(X), f(idx), f(w), Ld, Hd, out=out_h, chunk_nodes=1024)
+        assert torch.equal(out_h.view(torch.int16), dev.cpu().view(torch.int16))
+    out_h.zero_()
+    ctx.pinsage_embed_all(X.to(DEV), idx.pin_memory(), w.to(DEV), Ld, Hd, out=out_h, chunk_nodes=640)
+    assert torch.equal(out_h.view(torch.int16), dev.cpu().view(torch.int16))
+    out_d = torch.empty_like(dev)            # host inputs, device output
+    ctx.pinsage_embed_all(X.pin_memory(), idx.to(DEV), w.pin_memory(), Ld, Hd, out=out_d, chunk_nodes=2048)
+    torch.cuda.synchronize()
+    assert torch.equal(out_d.view(torch.int16), dev.view(torch.int16))
 
 
 def test_layer_in_place_and_caller_workspace(ctx):
