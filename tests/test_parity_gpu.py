@@ -427,3 +427,51 @@ def test_argument_errors(ctx):
         assert e.value.status_name == "BAD_INDEX"
     finally:
         ctx.pinsage_set_option("check_indices", 0)
+
+
+# ------------------------------------------------------------------ random shapes (property test)
+def _random_case(rng, narrow_ok):
+    """A random small instance: dims multiples of 8 with m != d != d_in, odd T, K in 1..3, ragged N.
+    narrow_ok=False keeps every normalised / output width >= 32-64: with 8-wide rows ReLU regularly
+    leaves a nearly dead row whose direction is ill-conditioned (a 1e-3 input rounding becomes a 3 %
+    change of z / ||z||), which measures the generator, not the kernels -- those widths are
+    exercised in fp32 mode, where they pass at 1e-4 ("degenerate rows")."""
+    K = int(rng.integers(1, 4))
+    wide = [64, 72, 128, 200, 256, 320]
+    any_w = [8, 24, 40] + wide
+    dims = [int(rng.choice(any_w))] + [int(rng.choice(any_w if narrow_ok else wide)) for _ in range(K)]
+    ms = [int(rng.choice([8, 16, 48, 64, 136, 256, 512])) for _ in range(K)]
+    g1 = int(rng.choice([8, 32, 64, 128, 264] if narrow_ok else [64, 128, 264]))
+    d_out = int(rng.choice([8, 16, 32, 128, 520] if narrow_ok else [32, 128, 520]))
+    N = int(rng.integers(60, 3000))
+    T = int(rng.choice([1, 2, 3, 7, 10, 33, 50]))
+    return N, T, dims, ms, g1, d_out
+
+
+@pytest.mark.parametrize("dtype", DTYPES)
+@pytest.mark.parametrize("seed", range(12))
+def test_random_shapes_whole_path(ctx, dtype, seed):
+    """Random (N, T, K, widths) with m != d != d_in, repeated / self neighbour ids allowed (A7):
+    pinsage_embed_all against the oracle on every row, with the automatic kernel choices."""
+    rng = np.random.default_rng(1000 + seed)
+    N, T, dims, ms, g1, d_out = _random_case(rng, narrow_ok=dtype == torch.float32)
+    g = torch.Generator().manual_seed(2000 + seed)
+
+    def rn(*shape, std=1.0):
+        return torch.randn(shape, generator=g) * std
+
+    X = rn(N, dims[0]).to(dtype)
+    layers = [{"Q": rn(ms[k], dims[k], std=dims[k] ** -0.5).to(dtype), "q": rn(ms[k], std=0.01),
+               "W": rn(dims[k + 1], dims[k] + ms[k], std=(dims[k] + ms[k]) ** -0.5).to(dtype),
+               "w": rn(dims[k + 1], std=0.01)} for k in range(len(ms))]
+    head = {"G1": rn(g1, dims[-1], std=dims[-1] ** -0.5).to(dtype), "g": rn(g1, std=0.01),
+            "G2": rn(d_out, g1, std=g1 ** -0.5).to(dtype)}
+    idx = torch.randint(0, N, (N, T), generator=g, dtype=torch.int32)
+    counts = torch.randint(1, 101, (N, T), generator=g, dtype=torch.int32)
+    alpha = O.normalize_counts(counts.numpy())
+    Lf, Hf = params_f64(layers, head)
+    ref = O.embed_all(to_f64(X), idx.numpy(), alpha, Lf, Hf)
+    Ld, Hd = _to_dev(layers, head)
+    out = ctx.pinsage_embed_all(X.to(DEV), idx.to(DEV), torch.from_numpy(alpha).to(DEV), Ld, Hd,
+                                chunk_nodes=int(rng.choice([0, 128, 1024])))
+    assert_rows_close(to_f64(out), ref, dtype, f"random case {seed}: N={N} T={T} dims={dims} ms={ms}")
