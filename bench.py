@@ -353,7 +353,11 @@ def run_ours(args, cfg):
                      "peak_source": f"{src} (MEASURED_PEAKS.json hbm_gbs)" if src == "measured"
                      else "fallback (B200_PROFILING.md)",
                      "algorithmic_bytes_per_launch": pool_bytes_step * args.steps / max(pool_n, 1),
-                     "avg_launch_ms": pool_ms / max(pool_n, 1), "launches": pool_n},
+                     "avg_launch_ms": pool_ms / max(pool_n, 1), "launches": pool_n,
+                     # the same launch measured in DRAM bytes (ncu traffic / live duration): what is
+                     # above 1.0 in `frac` is gathers served by L2, not work skipped
+                     "dram_gbs": (traffic / (pool_ms / max(pool_n, 1) * 1e-3) / 1e9) if traffic and pool_ms > 0 else None,
+                     "frac_dram": (traffic / (pool_ms / max(pool_n, 1) * 1e-3) / 1e9 / hbm) if traffic and pool_ms > 0 else None},
         "kernels": kernels,
         "e2e": e2e, "gpu_launches": int(launches), "clocks": clocks,
         "gemm_impl": "tcgen05" if args.gemm_impl == 0 and cfg.dtype == "bf16" else "simt",
