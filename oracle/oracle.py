@@ -101,19 +101,27 @@ def dense(H, M, b=None, act=True) -> np.ndarray:
     return out
 
 
-def pool(P, idx, alpha) -> np.ndarray:
+GAMMAS = {"importance": 0, "mean": 1, "max": 2}
+
+
+def pool(P, idx, alpha=None, gamma: str = "importance") -> np.ndarray:
     """n[v] = sum_t alpha[v,t] P[idx[v,t]] (S2).
+    gamma = "mean" / "max": the element-wise ablation aggregators, alpha unused.
     P may have more rows than idx (chunked destinations)."""
     P, Pp = _d(P)
     idx, ip = _i(idx)
-    alpha, ap = _f(alpha)
     N, T = idx.shape
-    assert alpha.shape == (N, T)
     assert idx.min(initial=0) >= 0 and idx.max(initial=0) < P.shape[0]
     m = P.shape[1]
     out = np.empty((N, m), dtype=np.float64)
-    lib().oracle_pool(ctypes.c_int64(N), ctypes.c_int32(T), ctypes.c_int32(m), Pp, ip, ap,
-                      out.ctypes.data_as(_f64p))
+    if gamma == "importance":
+        alpha, ap = _f(alpha)
+        assert alpha.shape == (N, T)
+        lib().oracle_pool(ctypes.c_int64(N), ctypes.c_int32(T), ctypes.c_int32(m), Pp, ip, ap,
+                          out.ctypes.data_as(_f64p))
+    else:
+        lib().oracle_pool_gamma(ctypes.c_int64(N), ctypes.c_int32(T), ctypes.c_int32(m), Pp, ip,
+                                _f32p(), ctypes.c_int32(GAMMAS[gamma]), out.ctypes.data_as(_f64p))
     return out
 
 
@@ -176,8 +184,13 @@ def layer_literal(H, idx, alpha, layer) -> np.ndarray:
     return out
 
 
-def layer_layerwise(H, idx, alpha, layer, return_parts: bool = False):
+def layer_layerwise(H, idx, alpha, layer, return_parts: bool = False, gamma: str = "importance"):
     """Mode B: one layer in the sec. 3.4 schedule (project once, pool, combine)."""
+    if gamma != "importance":
+        P = dense(H, layer["Q"], layer["q"], act=True)
+        n = pool(P, idx, None, gamma)
+        out = combine(H, n, layer["W"], layer["w"])
+        return (out, P, n) if return_parts else out
     H, Hp = _d(H)
     idx, ip = _i(idx)
     alpha, ap = _f(alpha)
@@ -219,15 +232,16 @@ def head(H, hp) -> np.ndarray:
 
 
 def embed_all(X, idx, alpha, layers, head_params=None, mode: str = "layerwise",
-              return_hidden: bool = False):
+              return_hidden: bool = False, gamma: str = "importance"):
     """K stacked layers (Alg. 2 l.8-14) + head (l.16).
 
     mode = "literal" (A) or "layerwise" (B).  Returns out, or (out, [H_1..H_K])."""
     H = np.ascontiguousarray(X, dtype=np.float64)
     hidden = []
     for lp in layers:
+        assert gamma == "importance" or mode == "layerwise"
         H = layer_literal(H, idx, alpha, lp) if mode == "literal" else \
-            layer_layerwise(H, idx, alpha, lp)
+            layer_layerwise(H, idx, alpha, lp, gamma=gamma)
         hidden.append(H)
     out = head(H, head_params) if head_params is not None else H
     return (out, hidden) if return_hidden else out

@@ -185,6 +185,38 @@ void oracle_pool(int64_t N, int32_t T, int32_t m, const double *P,
     }
 }
 
+/* The ablation aggregators of PAPER.md:262-263 (gamma "e.g., a element-wise mean or weighted sum",
+ * :118): gamma = 1 element-wise MEAN of the T projected neighbour rows (weights unused),
+ * gamma = 2 element-wise MAX.  gamma = 0 is importance pooling (oracle_pool).  alpha may be NULL
+ * for gamma != 0.  T >= 1. */
+void oracle_pool_gamma(int64_t N, int32_t T, int32_t m, const double *P, const int32_t *idx,
+                       const float *alpha, int32_t gamma, double *n)
+{
+    if (gamma == 0) {
+        oracle_pool(N, T, m, P, idx, alpha, n);
+        return;
+    }
+#pragma omp parallel for schedule(static)
+    for (int64_t v = 0; v < N; ++v) {
+        double *nv = n + (size_t)v * m;
+        const double *p0 = P + (size_t)idx[v * T] * m;
+        for (int j = 0; j < m; ++j)
+            nv[j] = p0[j];
+        for (int t = 1; t < T; ++t) {
+            const double *pr = P + (size_t)idx[v * T + t] * m;
+            for (int j = 0; j < m; ++j) {
+                if (gamma == 1)
+                    nv[j] += pr[j];
+                else if (pr[j] > nv[j])
+                    nv[j] = pr[j];
+            }
+        }
+        if (gamma == 1)
+            for (int j = 0; j < m; ++j)
+                nv[j] /= (double)T;
+    }
+}
+
 /* S3: out[v] = normalise(ReLU(W concat(H[v], n[v]) + w)). */
 void oracle_combine(int64_t N, int32_t d_in, int32_t m, int32_t d,
                     const double *H, const double *n, const double *W, const double *w,

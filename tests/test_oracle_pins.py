@@ -368,3 +368,45 @@ def test_golden_regression_file():
     from tests.golden.make_golden import compute
     stored = np.loadtxt(os.path.join(GOLDEN, "tiny_rows.txt"))
     np.testing.assert_allclose(compute(), stored, rtol=0, atol=1e-15)
+
+
+# --------------------------------------------------------------------------- ablation aggregators
+@pytest.mark.parametrize("N,T,m", [(50, 1, 8), (64, 7, 12), (200, 50, 16)])
+def test_mean_and_max_pooling_are_numpy_reductions(N, T, m):
+    """gamma = mean / max == numpy mean / max over the gathered rows; mean ==
+    importance pooling with uniform weights; T = 1 returns the row; order does not matter."""
+    rng = np.random.default_rng(50 + T)
+    P = rng.normal(size=(N + 5, m))
+    idx = rng.integers(0, N + 5, size=(N, T)).astype(np.int32)
+    np.testing.assert_allclose(O.pool(P, idx, gamma="mean"), P[idx].mean(axis=1), atol=1e-15)
+    np.testing.assert_array_equal(O.pool(P, idx, gamma="max"), P[idx].max(axis=1))
+    uniform = np.full((N, T), 1.0 / T, dtype=np.float32)
+    np.testing.assert_allclose(O.pool(P, idx, gamma="mean"), O.pool(P, idx, uniform), atol=1e-6)
+    if T == 1:
+        np.testing.assert_array_equal(O.pool(P, idx, gamma="max"), P[idx[:, 0]])
+        np.testing.assert_array_equal(O.pool(P, idx, gamma="mean"), P[idx[:, 0]])
+    perm = np.stack([rng.permutation(T) for _ in range(N)])
+    idx_p = np.take_along_axis(idx, perm, axis=1)
+    np.testing.assert_array_equal(O.pool(P, idx_p, gamma="max"), O.pool(P, idx, gamma="max"))
+    np.testing.assert_allclose(O.pool(P, idx_p, gamma="mean"), O.pool(P, idx, gamma="mean"), atol=1e-14)
+
+
+def test_variant_layers_compose_the_pinned_steps():
+    """A mean / max layer is dense -> variant pool -> combine; with every neighbour id equal to the
+    node itself all three aggregators give the same graph-free MLP (closed form iii)."""
+    rng = np.random.default_rng(60)
+    N, T, d_in, m, d = 30, 4, 6, 10, 8
+    X = rng.normal(size=(N, d_in))
+    lp = _rand_layer(rng, d_in, m, d)
+    idx = np.repeat(np.arange(N, dtype=np.int32)[:, None], T, axis=1)
+    alpha = O.normalize_counts(rng.integers(1, 51, size=(N, T)).astype(np.int32))
+    base = O.layer_layerwise(X, idx, alpha, lp)
+    # (binary32 alpha rows sum to 1 only to ~1e-7, hence the looser match with importance pooling)
+    np.testing.assert_allclose(O.layer_layerwise(X, idx, None, lp, gamma="mean"), base, atol=1e-6)
+    np.testing.assert_allclose(O.layer_layerwise(X, idx, None, lp, gamma="max"),
+                               O.layer_layerwise(X, idx, None, lp, gamma="mean"), atol=1e-14)
+    idx2, _ = _rand_graph(rng, N, T)
+    out = O.embed_all(X, idx2, None, [lp], gamma="max")
+    Pm = np.maximum(X @ lp["Q"].T + lp["q"], 0)[idx2].max(axis=1)
+    Z = np.maximum(X @ lp["W"][:, :d_in].T + Pm @ lp["W"][:, d_in:].T + lp["w"], 0)
+    np.testing.assert_allclose(out, _rownorm(Z), atol=1e-14)
