@@ -104,6 +104,11 @@ const char *pinsage_version(void);
  *                                    nbr_idx first (synchronous), default 0
  *                   "overlap"        1 = pinsage_layer / embed_all overlap S2 of chunk c+1 with S3
  *                                    of chunk c on a second stream (default 0)
+ *                   "pool_mode"      the aggregator gamma of Alg. 1 l.1 used by pinsage_pool / layer /
+ *                                    embed_all: 0 = importance pooling, the weighted sum (default);
+ *                                    1 = element-wise mean, 2 = element-wise max of the T projected
+ *                                    neighbour rows (the paper's ablation variants, PAPER.md:118,
+ *                                    :262-263; nbr_w is not read, but must still be a valid pointer)
  *                   "pool_slab"      column-slab width in bytes of the S2 pool: -1 automatic (default:
  *                                    128-byte slabs when P exceeds L2 but n_src x 128 bytes fits in
  *                                    0.7 of it, so that the gathered sub-table stays L2-resident),

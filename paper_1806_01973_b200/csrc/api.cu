@@ -29,6 +29,7 @@ struct pinsage_ctx {
     GemmTune tune;                   // tcgen05 tile knobs ("gemm_cg", "gemm_ns")
     int check_indices = 0;
     int overlap = 0;
+    int pool_mode = 0;               // aggregator gamma: 0 importance, 1 mean, 2 max
     int pool_slab = -1;              // -1 automatic, 0 off, 32 / 64 / 128 forced slab width in bytes
     size_t l2_bytes = 0;
     int launches = 0;
@@ -324,7 +325,7 @@ pinsage_status pool_combine_chunks(pinsage_ctx *ctx, DType dt, int64_t N, int32_
         if (two && c >= 2) PS_CUDA(ctx, cudaStreamWaitEvent(ps, ctx->ev_gemm[b], 0));
         if (tables_landed) PS_CUDA(ctx, cudaStreamWaitEvent(ps, tables_landed[c], 0));
         const int pe0 = prof_mark(ctx, ps);
-        cudaError_t e = launch_pool(dt, rows, T, lp->m, P, idx + (size_t)r0 * T, w + (size_t)r0 * T,
+        cudaError_t e = launch_pool(dt, ctx->pool_mode, rows, T, lp->m, P, idx + (size_t)r0 * T, w + (size_t)r0 * T,
                                     nb[b], pick_slab(ctx, dt, N, T, lp->m), ps, &ctx->launches);
         prof_close(ctx, PROF_POOL, pe0, ps);
         count_launches(ctx);
@@ -543,6 +544,9 @@ pinsage_status pinsage_set_option(pinsage_ctx *ctx, const char *key, int64_t val
         ctx->check_indices = value != 0;
     } else if (!strcmp(key, "overlap")) {
         ctx->overlap = value != 0;
+    } else if (!strcmp(key, "pool_mode")) {
+        if (value < 0 || value > 2) return fail(ctx, PINSAGE_ERR_INVALID_ARG, "pool_mode must be 0, 1 or 2");
+        ctx->pool_mode = (int)value;
     } else if (!strcmp(key, "pool_slab")) {
         if (value != -1 && value != 0 && value != 32 && value != 64 && value != 128)
             return fail(ctx, PINSAGE_ERR_INVALID_ARG, "pool_slab must be -1, 0, 32, 64 or 128");
@@ -629,7 +633,7 @@ pinsage_status pinsage_pool(pinsage_ctx *ctx, pinsage_dtype dtype, int64_t n_dst
         return fail(ctx, PINSAGE_ERR_INVALID_ARG, "n overlaps P");
     PS_TRY(maybe_validate(ctx, n_dst, n_src, T, nbr_idx, nbr_w));
     const int pe0 = prof_mark(ctx, ctx->stream);
-    cudaError_t e = launch_pool(dt, n_dst, T, m, P, nbr_idx, nbr_w, n, pick_slab(ctx, dt, n_src, T, m),
+    cudaError_t e = launch_pool(dt, ctx->pool_mode, n_dst, T, m, P, nbr_idx, nbr_w, n, pick_slab(ctx, dt, n_src, T, m),
                                 ctx->stream, &ctx->launches);
     prof_close(ctx, PROF_POOL, pe0, ctx->stream);
     count_launches(ctx);

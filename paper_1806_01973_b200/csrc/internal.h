@@ -50,7 +50,8 @@ size_t gemm_tc_scratch_bytes(const GemmArgs &a);
 // ---- pool.cu ------------------------------------------------------------------------------------
 // slab_bytes: 0 = whole rows (one pass); 32 / 64 / 128 = column-slab passes that keep the gathered
 // sub-table L2-resident (ignored when pool_slab_ok is false for the shape).
-cudaError_t launch_pool(DType dt, int64_t n_dst, int32_t T, int32_t m, const void *P,
+// mode: 0 importance (weighted sum), 1 element-wise mean, 2 element-wise max (w unused for 1, 2).
+cudaError_t launch_pool(DType dt, int mode, int64_t n_dst, int32_t T, int32_t m, const void *P,
                         const int32_t *idx, const float *w, void *out, int slab_bytes, cudaStream_t s,
                         int *launches);
 bool pool_slab_ok(DType dt, int32_t T, int32_t m, int slab_bytes);

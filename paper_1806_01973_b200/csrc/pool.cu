@@ -79,6 +79,15 @@ struct Chunk<true> {  // 8 bf16 per 16 bytes
             acc[2 * i + 1] = fmaf(wt, __uint_as_float(u[i] & 0xffff0000u), acc[2 * i + 1]);
         }
     }
+    static __device__ __forceinline__ void vmax(const uint4 &r, float (&acc)[8])
+    {
+        const uint32_t u[4] = {r.x, r.y, r.z, r.w};
+#pragma unroll
+        for (int i = 0; i < 4; ++i) {
+            acc[2 * i] = fmaxf(acc[2 * i], __uint_as_float(u[i] << 16));
+            acc[2 * i + 1] = fmaxf(acc[2 * i + 1], __uint_as_float(u[i] & 0xffff0000u));
+        }
+    }
     static __device__ __forceinline__ uint4 pack(const float (&acc)[8])
     {
         uint32_t u[4];
@@ -101,6 +110,13 @@ struct Chunk<false> {  // 4 fp32 per 16 bytes
         acc[2] = fmaf(wt, __uint_as_float(r.z), acc[2]);
         acc[3] = fmaf(wt, __uint_as_float(r.w), acc[3]);
     }
+    static __device__ __forceinline__ void vmax(const uint4 &r, float (&acc)[4])
+    {
+        acc[0] = fmaxf(acc[0], __uint_as_float(r.x));
+        acc[1] = fmaxf(acc[1], __uint_as_float(r.y));
+        acc[2] = fmaxf(acc[2], __uint_as_float(r.z));
+        acc[3] = fmaxf(acc[3], __uint_as_float(r.w));
+    }
     static __device__ __forceinline__ uint4 pack(const float (&acc)[4])
     {
         return make_uint4(__float_as_uint(acc[0]), __float_as_uint(acc[1]),
@@ -110,7 +126,9 @@ struct Chunk<false> {  // 4 fp32 per 16 bytes
 
 // UU neighbour rows (slots j0 .. j0+UU-1 of the current batch) for one lane: every one of the
 // UU*CPL 16-byte loads is issued before the first FMA (memory-level parallelism).
-template <bool BF16, int LPN, int CPL, int UU, bool EXACT>
+// MODE: 0 importance pooling (weighted sum), 1 element-wise mean (my_w holds 1/T in every lane),
+// 2 element-wise max -- the aggregator variants of PAPER.md:118, :262-263.
+template <bool BF16, int LPN, int CPL, int UU, bool EXACT, int MODE>
 __device__ __forceinline__ void gather_fma(const uint4 *__restrict__ P, int my_i, float my_w, int j0,
                                            int sl, int chunks,
                                            float (&acc)[CPL][Chunk<BF16>::E])
@@ -122,7 +140,7 @@ __device__ __forceinline__ void gather_fma(const uint4 *__restrict__ P, int my_i
 #pragma unroll
     for (int u = 0; u < UU; ++u) {
         const int id = __shfl_sync(0xffffffffu, my_i, j0 + u, LPN);
-        wt[u] = __shfl_sync(0xffffffffu, my_w, j0 + u, LPN);
+        wt[u] = MODE == 0 ? __shfl_sync(0xffffffffu, my_w, j0 + u, LPN) : my_w;
         row[u] = P + (size_t)id * (size_t)chunks + sl;
     }
 #pragma unroll
@@ -135,14 +153,17 @@ __device__ __forceinline__ void gather_fma(const uint4 *__restrict__ P, int my_i
 #pragma unroll
     for (int u = 0; u < UU; ++u)
 #pragma unroll
-        for (int c = 0; c < CPL; ++c) C::fma(r[u][c], wt[u], acc[c]);
+        for (int c = 0; c < CPL; ++c) {
+            if (MODE == 2) C::vmax(r[u][c], acc[c]);
+            else C::fma(r[u][c], wt[u], acc[c]);
+        }
 }
 
 // LPN lanes per node (4..32), CPL chunks per lane, U neighbour rows in flight,
 // EXACT: the row is exactly LPN*CPL chunks wide (no per-chunk guard).
 // An explicit minBlocksPerSM matters: without it ptxas (-O3) re-serialises the load batch to
 // minimise registers (32 regs, 2 loads in flight); with it the U*CPL loads stay batched.
-template <bool BF16, int LPN, int CPL, int U, bool EXACT>
+template <bool BF16, int LPN, int CPL, int U, bool EXACT, int MODE>
 __global__ void __launch_bounds__(256, (CPL <= 2) ? 4 : 2)
 pool_kernel(const uint4 *__restrict__ P, const int *__restrict__ idx, const float *__restrict__ w,
             uint4 *__restrict__ out, long long n_dst, int T, int chunks)
@@ -162,24 +183,24 @@ pool_kernel(const uint4 *__restrict__ P, const int *__restrict__ idx, const floa
 #pragma unroll
     for (int c = 0; c < CPL; ++c)
 #pragma unroll
-        for (int e = 0; e < C::E; ++e) acc[c][e] = 0.f;
+        for (int e = 0; e < C::E; ++e) acc[c][e] = MODE == 2 ? -INFINITY : 0.f;
 
     const int *irow = idx + v * T;
     const float *wrow = w + v * T;
     for (int tb = 0; tb < T; tb += LPN) {
         const int t = tb + sl;
         int my_i = 0;
-        float my_w = 0.f;
+        float my_w = MODE == 1 ? 1.0f / (float)T : 0.f;
         if (t < T) {
             my_i = ld_stream_i32(irow + t);
-            my_w = ld_stream_f32(wrow + t);
+            if (MODE == 0) my_w = ld_stream_f32(wrow + t);
         }
         const int cnt = min(LPN, T - tb);
         int j0 = 0;
         for (; j0 + U <= cnt; j0 += U)
-            gather_fma<BF16, LPN, CPL, U, EXACT>(P, my_i, my_w, j0, sl, chunks, acc);
+            gather_fma<BF16, LPN, CPL, U, EXACT, MODE>(P, my_i, my_w, j0, sl, chunks, acc);
         for (; j0 < cnt; ++j0)
-            gather_fma<BF16, LPN, CPL, 1, EXACT>(P, my_i, my_w, j0, sl, chunks, acc);
+            gather_fma<BF16, LPN, CPL, 1, EXACT, MODE>(P, my_i, my_w, j0, sl, chunks, acc);
     }
     if (active) {
         uint4 *orow = out + (size_t)v * (size_t)chunks;
@@ -191,7 +212,7 @@ pool_kernel(const uint4 *__restrict__ P, const int *__restrict__ idx, const floa
     }
 }
 
-template <bool BF16, int LPN, int CPL, int U>
+template <bool BF16, int LPN, int CPL, int U, int MODE>
 cudaError_t run_pool(const void *P, const int *idx, const float *w, void *out, long long n_dst,
                      int T, int chunks, cudaStream_t s)
 {
@@ -200,10 +221,10 @@ cudaError_t run_pool(const void *P, const int *idx, const float *w, void *out, l
     const long long blocks = (warps + 7) / 8;
     if (blocks > 0x7fffffffLL) return cudaErrorInvalidConfiguration;
     if (chunks == LPN * CPL)
-        pool_kernel<BF16, LPN, CPL, U, true><<<(unsigned)blocks, 256, 0, s>>>(
+        pool_kernel<BF16, LPN, CPL, U, true, MODE><<<(unsigned)blocks, 256, 0, s>>>(
             static_cast<const uint4 *>(P), idx, w, static_cast<uint4 *>(out), n_dst, T, chunks);
     else
-        pool_kernel<BF16, LPN, CPL, U, false><<<(unsigned)blocks, 256, 0, s>>>(
+        pool_kernel<BF16, LPN, CPL, U, false, MODE><<<(unsigned)blocks, 256, 0, s>>>(
             static_cast<const uint4 *>(P), idx, w, static_cast<uint4 *>(out), n_dst, T, chunks);
     return cudaGetLastError();
 }
@@ -302,18 +323,27 @@ cudaError_t dispatch_pool_slab(int slab_bytes, const void *P, const int *idx, co
     return cudaErrorNotSupported;
 }
 
-template <bool BF16>
+template <bool BF16, int MODE>
 cudaError_t dispatch_pool(const void *P, const int *idx, const float *w, void *out,
                           long long n_dst, int T, int chunks, cudaStream_t s)
 {
-    if (chunks <= 4) return run_pool<BF16, 4, 1, 4>(P, idx, w, out, n_dst, T, chunks, s);
-    if (chunks <= 8) return run_pool<BF16, 8, 1, 8>(P, idx, w, out, n_dst, T, chunks, s);
-    if (chunks <= 16) return run_pool<BF16, 16, 1, 8>(P, idx, w, out, n_dst, T, chunks, s);
-    if (chunks <= 32) return run_pool<BF16, 32, 1, 8>(P, idx, w, out, n_dst, T, chunks, s);
-    if (chunks <= 64) return run_pool<BF16, 32, 2, 4>(P, idx, w, out, n_dst, T, chunks, s);
-    if (chunks <= 128) return run_pool<BF16, 32, 4, 2>(P, idx, w, out, n_dst, T, chunks, s);
-    if (chunks <= 256) return run_pool<BF16, 32, 8, 1>(P, idx, w, out, n_dst, T, chunks, s);
+    if (chunks <= 4) return run_pool<BF16, 4, 1, 4, MODE>(P, idx, w, out, n_dst, T, chunks, s);
+    if (chunks <= 8) return run_pool<BF16, 8, 1, 8, MODE>(P, idx, w, out, n_dst, T, chunks, s);
+    if (chunks <= 16) return run_pool<BF16, 16, 1, 8, MODE>(P, idx, w, out, n_dst, T, chunks, s);
+    if (chunks <= 32) return run_pool<BF16, 32, 1, 8, MODE>(P, idx, w, out, n_dst, T, chunks, s);
+    if (chunks <= 64) return run_pool<BF16, 32, 2, 4, MODE>(P, idx, w, out, n_dst, T, chunks, s);
+    if (chunks <= 128) return run_pool<BF16, 32, 4, 2, MODE>(P, idx, w, out, n_dst, T, chunks, s);
+    if (chunks <= 256) return run_pool<BF16, 32, 8, 1, MODE>(P, idx, w, out, n_dst, T, chunks, s);
     return cudaErrorNotSupported;
+}
+
+template <bool BF16>
+cudaError_t dispatch_pool_mode(int mode, const void *P, const int *idx, const float *w, void *out,
+                               long long n_dst, int T, int chunks, cudaStream_t s)
+{
+    if (mode == 1) return dispatch_pool<BF16, 1>(P, idx, w, out, n_dst, T, chunks, s);
+    if (mode == 2) return dispatch_pool<BF16, 2>(P, idx, w, out, n_dst, T, chunks, s);
+    return dispatch_pool<BF16, 0>(P, idx, w, out, n_dst, T, chunks, s);
 }
 
 // One warp per row: alpha = (float)c / (float)sum(c), IEEE binary32 division.
@@ -365,19 +395,22 @@ bool pool_slab_ok(DType dt, int32_t T, int32_t m, int slab_bytes)
     return row % slab_bytes == 0 && row > (size_t)slab_bytes && smem <= 200 * 1024;
 }
 
-cudaError_t launch_pool(DType dt, int64_t n_dst, int32_t T, int32_t m, const void *P,
+cudaError_t launch_pool(DType dt, int mode, int64_t n_dst, int32_t T, int32_t m, const void *P,
                         const int32_t *idx, const float *w, void *out, int slab_bytes, cudaStream_t s,
                         int *launches)
 {
     if (n_dst <= 0) return cudaSuccess;
     const int chunks = (int)((size_t)m * elem_size(dt) / 16);
     if (launches) ++*launches;
+    if (mode != 0)
+        return dt == DType::BF16 ? dispatch_pool_mode<true>(mode, P, idx, w, out, n_dst, T, chunks, s)
+                                 : dispatch_pool_mode<false>(mode, P, idx, w, out, n_dst, T, chunks, s);
     if (slab_bytes > 0 && pool_slab_ok(dt, T, m, slab_bytes))
         return dt == DType::BF16
                    ? dispatch_pool_slab<true>(slab_bytes, P, idx, w, out, n_dst, T, chunks, s)
                    : dispatch_pool_slab<false>(slab_bytes, P, idx, w, out, n_dst, T, chunks, s);
-    return dt == DType::BF16 ? dispatch_pool<true>(P, idx, w, out, n_dst, T, chunks, s)
-                             : dispatch_pool<false>(P, idx, w, out, n_dst, T, chunks, s);
+    return dt == DType::BF16 ? dispatch_pool<true, 0>(P, idx, w, out, n_dst, T, chunks, s)
+                             : dispatch_pool<false, 0>(P, idx, w, out, n_dst, T, chunks, s);
 }
 
 cudaError_t launch_normalize_counts(int64_t N, int32_t T, const int32_t *counts, float *w,

@@ -475,3 +475,47 @@ def test_random_shapes_whole_path(ctx, dtype, seed):
     out = ctx.pinsage_embed_all(X.to(DEV), idx.to(DEV), torch.from_numpy(alpha).to(DEV), Ld, Hd,
                                 chunk_nodes=int(rng.choice([0, 128, 1024])))
     assert_rows_close(to_f64(out), ref, dtype, f"random case {seed}: N={N} T={T} dims={dims} ms={ms}")
+
+
+# ------------------------------------------------------------------ aggregator variants (NEXT #1)
+@pytest.mark.parametrize("dtype", DTYPES)
+@pytest.mark.parametrize("gamma,mode", [("mean", 1), ("max", 2)])
+@pytest.mark.parametrize("n_dst,n_src,T,m", [(1, 1, 1, 8), (3001, 2000, 50, 256), (515, 4000, 100, 256),
+                                             (300, 900, 50, 512), (77, 300, 7, 2048), (999, 999, 33, 24)])
+def test_pool_mean_and_max_variants(ctx, dtype, gamma, mode, n_dst, n_src, T, m):
+    """gamma = mean / max through pinsage_pool with option pool_mode."""
+    if dtype == torch.float32 and m > 1024:
+        pytest.skip("fp32 rows above 4 KB are outside the compiled set")
+    P = _rand((n_src, m), dtype, 50 + m)
+    idx, counts = _graph(n_dst, T, 51 + T, n_src=n_src)
+    w = torch.from_numpy(O.normalize_counts(counts.numpy())).to(DEV)
+    ctx.pinsage_set_option("pool_mode", mode)
+    try:
+        got = ctx.pinsage_pool(P.to(DEV), idx.to(DEV), w)
+    finally:
+        ctx.pinsage_set_option("pool_mode", 0)
+    ref = O.pool(to_f64(P), idx.numpy(), gamma=gamma)
+    if gamma == "max":      # a max of stored values is a stored value: bit-exact
+        exp = torch.from_numpy(ref).to(dtype)
+        bits = torch.int16 if dtype == torch.bfloat16 else torch.int32
+        assert torch.equal(got.cpu().view(bits), exp.view(bits))
+    else:
+        assert_rows_close(to_f64(got), ref, dtype, f"mean pool T={T} m={m}",
+                          tol=4e-3 if dtype == torch.bfloat16 else 2e-6)
+
+
+@pytest.mark.parametrize("gamma,mode", [("mean", 1), ("max", 2)])
+def test_whole_path_with_mean_and_max_pooling(ctx, gamma, mode):
+    """The mean-pooling / max-pooling model variants end to end (config 2's shape, 6 000 nodes)."""
+    cfg = synth.CONFIGS["cfg2"].scaled(6001)
+    X, idx, counts, alpha, layers, head = _inputs(cfg)
+    Lf, Hf = params_f64(layers, head)
+    ref = O.embed_all(to_f64(X), idx.numpy(), None, Lf, Hf, gamma=gamma)
+    Ld, Hd = _to_dev(layers, head)
+    ctx.pinsage_set_option("pool_mode", mode)
+    try:
+        out = ctx.pinsage_embed_all(X.to(DEV), idx.to(DEV), torch.from_numpy(alpha).to(DEV), Ld, Hd,
+                                    chunk_nodes=2048)
+    finally:
+        ctx.pinsage_set_option("pool_mode", 0)
+    assert_rows_close(to_f64(out), ref, X.dtype, f"embed_all gamma={gamma}")
