@@ -242,6 +242,7 @@ def run_ours(args, cfg):
     ctx.pinsage_set_option("gemm_ns", args.gemm_ns)
     ctx.pinsage_set_option("gemm_epi", args.gemm_epi)
     ctx.pinsage_set_option("pool_slab", args.pool_slab)
+    ctx.pinsage_set_option("linear_pool", args.linear_pool)
     alpha = ctx.pinsage_normalize_counts(counts)
     torch.cuda.synchronize()
     del counts
@@ -320,7 +321,10 @@ def run_ours(args, cfg):
     # ---- roofline of the dominant kernel (S2 pool) from the live event records ---------------
     hbm, tflops, src = _peaks()
     pool_ms, pool_n = prof["pool"]
-    pool_bytes_step = sum(cfg.N * pool_bytes_per_node(cfg.T, m, e) for _, m, _ in cfg.layer_dims())
+    # gathered row width: m, or d in the linear-pool schedule (pooling the W2-projection)
+    lin = args.linear_pool
+    pool_bytes_step = sum(cfg.N * pool_bytes_per_node(cfg.T, d if (lin == 1 or (lin == -1 and m > d)) else m, e)
+                          for _, m, d in cfg.layer_dims())
     pool_gbs = pool_bytes_step * args.steps / (pool_ms * 1e-3) / 1e9 if pool_ms > 0 else 0.0
     traffic = None      # DRAM bytes per launch from the committed ncu --set full capture, if any
     tp = os.path.join(ROOT, "profiles", "pool_traffic.csv")
@@ -335,6 +339,10 @@ def run_ours(args, cfg):
     dense_f = sum(2 * d_in * m for d_in, m, _ in cfg.layer_dims()) + 2 * cfg.hidden * cfg.g1 \
         + 2 * cfg.g1 * cfg.d_out
     comb_f = sum(2 * (d_in + m) * d for d_in, m, d in cfg.layer_dims())
+    for d_in, m, d in cfg.layer_dims():          # linear pool: P W2^T is a dense launch, S3 keeps H W1^T
+        if lin == 1 or (lin == -1 and m > d):
+            dense_f += 2 * m * d
+            comb_f -= 2 * m * d
     for name, f in (("dense", dense_f), ("combine", comb_f)):
         kms = prof[name][0]
         if kms > 0:
@@ -383,6 +391,7 @@ def main():
     ap.add_argument("--gemm-cg", type=int, default=0, help="0 auto (CTA pairs), 1 single CTAs, 2 pairs")
     ap.add_argument("--gemm-ns", type=int, default=0, help="slab width without row norm: 0/256/512")
     ap.add_argument("--gemm-epi", type=int, default=0, help="0 auto (8 epilogue warps), 1 four")
+    ap.add_argument("--linear-pool", type=int, default=-1, help="-1 auto (m > d), 0 off, 1 on")
     ap.add_argument("--pool-slab", type=int, default=-1, help="-1 auto, 0 whole rows, 32/64/128")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu", action="store_true")

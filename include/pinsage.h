@@ -109,6 +109,11 @@ const char *pinsage_version(void);
  *                                    1 = element-wise mean, 2 = element-wise max of the T projected
  *                                    neighbour rows (the paper's ablation variants, PAPER.md:118,
  *                                    :262-263; nbr_w is not read, but must still be a valid pointer)
+ *                   "linear_pool"    pinsage_layer / embed_all schedule: pool the W2-projection P W2^T
+ *                                    (width d) and add it to H W1^T in the S3 epilogue, instead of pooling
+ *                                    P (width m) -- the same function in real arithmetic, m / d times
+ *                                    fewer gathered bytes: -1 = when m > d (default), 0 never, 1 always.
+ *                                    Not used with pool_mode 2 (max is not linear).
  *                   "pool_slab"      column-slab width in bytes of the S2 pool: -1 automatic (default:
  *                                    128-byte slabs when P exceeds L2 but n_src x 128 bytes fits in
  *                                    0.7 of it, so that the gathered sub-table stays L2-resident),

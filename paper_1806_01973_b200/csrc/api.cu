@@ -30,6 +30,8 @@ struct pinsage_ctx {
     int check_indices = 0;
     int overlap = 0;
     int pool_mode = 0;               // aggregator gamma: 0 importance, 1 mean, 2 max
+    int linear_pool = -1;            // pool the W2-projection (width d) instead of P (width m):
+                                     // -1 automatic (when m > d), 0 never, 1 always
     int pool_slab = -1;              // -1 automatic, 0 off, 32 / 64 / 128 forced slab width in bytes
     size_t l2_bytes = 0;
     int launches = 0;
@@ -301,9 +303,20 @@ int64_t auto_chunk(int64_t N, int64_t requested, size_t row_bytes)
     return c;
 }
 
+// The linear-pool schedule: W [h ; sum_t a_t p_t] = W1 h + sum_t a_t (W2 p_t), exact in real
+// arithmetic because the pool is linear (not so for the element-wise max).  Pooling the projected
+// rows P' = P W2^T (width d) instead of P (width m) divides the gathered bytes by m / d -- 2x at the
+// paper's own geometry, m = 2048, d = 1024 -- for the same flops.
+bool use_linear_pool(const pinsage_ctx *ctx, const pinsage_layer_params *lp)
+{
+    if (!ctx || ctx->pool_mode == 2 || ctx->linear_pool == 0) return false;
+    return ctx->linear_pool == 1 || lp->m > lp->d;
+}
+
 // S2 + S3 over all destination rows in chunks; pool of chunk c+1 may overlap combine of chunk c.
-// Hin [N x d_in] (read), P [N x m] (read), Hout [N x d] (written; may alias Hin iff d == d_in).
-// nbuf: two chunk buffers [chunk x m]; scratch: per-GEMM scratch.
+// Hin [N x d_in] (read), P [N x pw] (read), Hout [N x d] (written; may alias Hin iff d == d_in).
+// pw = m (P = projections, n is the second K segment of S3) or, in the linear-pool schedule, d
+// (P = projections times W2^T, n is an addend of S3).  nbuf: two chunk buffers [chunk x pw].
 pinsage_status pool_combine_chunks(pinsage_ctx *ctx, DType dt, int64_t N, int32_t T,
                                    const pinsage_layer_params *lp, const void *Hin, const void *P,
                                    const int32_t *idx, const float *w, void *Hout, int64_t chunk,
@@ -311,6 +324,8 @@ pinsage_status pool_combine_chunks(pinsage_ctx *ctx, DType dt, int64_t N, int32_
                                    const cudaEvent_t *tables_landed = nullptr)
 {
     const size_t es = elem_size(dt);
+    const bool linear = use_linear_pool(ctx, lp);
+    const int32_t pw = linear ? lp->d : lp->m;
     const int64_t nchunks = (N + chunk - 1) / chunk;
     const bool two = ctx->overlap && nchunks > 1;
     void *nb[2] = {nbuf0, two ? nbuf1 : nbuf0};
@@ -325,8 +340,8 @@ pinsage_status pool_combine_chunks(pinsage_ctx *ctx, DType dt, int64_t N, int32_
         if (two && c >= 2) PS_CUDA(ctx, cudaStreamWaitEvent(ps, ctx->ev_gemm[b], 0));
         if (tables_landed) PS_CUDA(ctx, cudaStreamWaitEvent(ps, tables_landed[c], 0));
         const int pe0 = prof_mark(ctx, ps);
-        cudaError_t e = launch_pool(dt, ctx->pool_mode, rows, T, lp->m, P, idx + (size_t)r0 * T, w + (size_t)r0 * T,
-                                    nb[b], pick_slab(ctx, dt, N, T, lp->m), ps, &ctx->launches);
+        cudaError_t e = launch_pool(dt, ctx->pool_mode, rows, T, pw, P, idx + (size_t)r0 * T, w + (size_t)r0 * T,
+                                    nb[b], pick_slab(ctx, dt, N, T, pw), ps, &ctx->launches);
         prof_close(ctx, PROF_POOL, pe0, ps);
         count_launches(ctx);
         PS_CUDA(ctx, e);
@@ -337,11 +352,16 @@ pinsage_status pool_combine_chunks(pinsage_ctx *ctx, DType dt, int64_t N, int32_
         GemmArgs g;
         g.M = rows;
         g.K1 = lp->d_in;
-        g.K2 = lp->m;
         g.N = lp->d;
         g.A1 = static_cast<const char *>(Hin) + (size_t)r0 * lp->d_in * es;
-        g.A2 = nb[b];
         g.B = lp->W;
+        if (linear) {                        // z = H W1^T + pooled(P W2^T) + w
+            g.ldb = lp->d_in + lp->m;
+            g.addend = nb[b];
+        } else {                             // z = H W1^T + n W2^T + w: two K segments
+            g.K2 = lp->m;
+            g.A2 = nb[b];
+        }
         g.bias = lp->w;
         g.relu = 1;
         g.l2norm = 1;
@@ -357,28 +377,34 @@ pinsage_status pool_combine_chunks(pinsage_ctx *ctx, DType dt, int64_t N, int32_
 }
 
 struct LayerWs {
-    size_t P_off, n0_off, n1_off, scratch_off, scratch_bytes, total;
+    size_t P_off, Pc_off, n0_off, n1_off, scratch_off, scratch_bytes, total;
 };
 
+// Workspace of one layer.  Standard schedule: P [N x m] | n chunk(s) [chunk x m] | scratch.
+// Linear-pool schedule: P' [N x d] | projection chunk Pc [chunk x m] | n chunk(s) [chunk x d] | scratch.
 LayerWs plan_layer_ws(const pinsage_ctx *ctx, DType dt, int64_t N, const pinsage_layer_params *lp,
                       int64_t chunk)
 {
     const size_t es = elem_size(dt);
+    const bool linear = use_linear_pool(ctx, lp);
+    const int32_t pw = linear ? lp->d : lp->m;
     LayerWs p{};
     size_t off = 0;
     p.P_off = off;
-    off += align_up((size_t)N * lp->m * es, 256);
+    off += align_up((size_t)N * pw * es, 256);
+    p.Pc_off = off;
+    if (linear) off += align_up((size_t)chunk * lp->m * es, 256);
     p.n0_off = off;
-    off += align_up((size_t)chunk * lp->m * es, 256);
+    off += align_up((size_t)chunk * pw * es, 256);
     p.n1_off = p.n0_off;                       // second chunk buffer only for the two-stream schedule
     if (ctx && ctx->overlap) {
         p.n1_off = off;
-        off += align_up((size_t)chunk * lp->m * es, 256);
+        off += align_up((size_t)chunk * pw * es, 256);
     }
     GemmArgs g1;
-    g1.M = N; g1.K1 = lp->d_in; g1.N = lp->m; g1.relu = 1;
+    g1.M = linear ? chunk : N; g1.K1 = lp->d_in; g1.N = lp->m; g1.relu = 1;
     GemmArgs g3;
-    g3.M = chunk; g3.K1 = lp->d_in; g3.K2 = lp->m; g3.N = lp->d; g3.relu = 1; g3.l2norm = 1;
+    g3.M = chunk; g3.K1 = lp->d_in; g3.K2 = linear ? 0 : lp->m; g3.N = lp->d; g3.relu = 1; g3.l2norm = 1;
     p.scratch_bytes = std::max(gemm_scratch_bytes(ctx, dt, g1), gemm_scratch_bytes(ctx, dt, g3));
     p.scratch_off = off;
     off += p.scratch_bytes;
@@ -395,7 +421,8 @@ pinsage_status layer_on_ws(pinsage_ctx *ctx, DType dt, int64_t N, int32_t T, con
                            const cudaEvent_t *tables_landed = nullptr)
 {
     const size_t es = elem_size(dt);
-    const int64_t s1_rows = feats_landed ? chunk : N;
+    const bool linear = use_linear_pool(ctx, lp);
+    const int64_t s1_rows = (feats_landed || linear) ? chunk : N;
     for (int64_t r0 = 0, c = 0; r0 < N; r0 += s1_rows, ++c) {
         if (feats_landed) PS_CUDA(ctx, cudaStreamWaitEvent(ctx->stream, feats_landed[c], 0));
         GemmArgs g;
@@ -406,8 +433,19 @@ pinsage_status layer_on_ws(pinsage_ctx *ctx, DType dt, int64_t N, int32_t T, con
         g.B = lp->Q;
         g.bias = lp->q;
         g.relu = 1;
-        g.out = ws + plan.P_off + (size_t)r0 * lp->m * es;
+        g.out = linear ? ws + plan.Pc_off : ws + plan.P_off + (size_t)r0 * lp->m * es;
         PS_TRY(run_gemm(ctx, dt, g, ws + plan.scratch_off, plan.scratch_bytes, ctx->stream));
+        if (linear) {                          // P'[chunk] = P[chunk] W2^T (W2 = columns d_in.. of W)
+            GemmArgs g2;
+            g2.M = g.M;
+            g2.K1 = lp->m;
+            g2.N = lp->d;
+            g2.A1 = ws + plan.Pc_off;
+            g2.B = static_cast<const char *>(lp->W) + (size_t)lp->d_in * es;
+            g2.ldb = lp->d_in + lp->m;
+            g2.out = ws + plan.P_off + (size_t)r0 * lp->d * es;
+            PS_TRY(run_gemm(ctx, dt, g2, ws + plan.scratch_off, plan.scratch_bytes, ctx->stream));
+        }
     }
     return pool_combine_chunks(ctx, dt, N, T, lp, feats, ws + plan.P_off, idx, w, out, chunk,
                                ws + plan.n0_off, ws + plan.n1_off, ws + plan.scratch_off,
@@ -547,6 +585,9 @@ pinsage_status pinsage_set_option(pinsage_ctx *ctx, const char *key, int64_t val
     } else if (!strcmp(key, "pool_mode")) {
         if (value < 0 || value > 2) return fail(ctx, PINSAGE_ERR_INVALID_ARG, "pool_mode must be 0, 1 or 2");
         ctx->pool_mode = (int)value;
+    } else if (!strcmp(key, "linear_pool")) {
+        if (value < -1 || value > 1) return fail(ctx, PINSAGE_ERR_INVALID_ARG, "linear_pool must be -1, 0 or 1");
+        ctx->linear_pool = (int)value;
     } else if (!strcmp(key, "pool_slab")) {
         if (value != -1 && value != 0 && value != 32 && value != 64 && value != 128)
             return fail(ctx, PINSAGE_ERR_INVALID_ARG, "pool_slab must be -1, 0, 32, 64 or 128");
@@ -685,7 +726,13 @@ size_t pinsage_layer_workspace_bytes(pinsage_dtype dtype, int64_t N, int32_t T,
     probe.gemm_impl = 1;
     probe.overlap = 1;
     const DType dt = static_cast<DType>(dtype);
-    return plan_layer_ws(&probe, dt, N, params, auto_chunk(N, 0, (size_t)params->m * elem_size(dt))).total;
+    const int64_t chunk = auto_chunk(N, 0, (size_t)params->m * elem_size(dt));
+    size_t need = 0;
+    for (int lin = 0; lin <= 1; ++lin) {       // whichever schedule the context options select
+        probe.linear_pool = lin;
+        need = std::max(need, plan_layer_ws(&probe, dt, N, params, chunk).total);
+    }
+    return need;
 }
 
 pinsage_status pinsage_layer(pinsage_ctx *ctx, pinsage_dtype dtype, int64_t N, int32_t T,

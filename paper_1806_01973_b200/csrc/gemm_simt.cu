@@ -29,6 +29,19 @@ __device__ __forceinline__ float2 load2<__nv_bfloat16>(const __nv_bfloat16 *p)
 }
 
 template <typename T>
+__device__ __forceinline__ float load1(const T *p);
+template <>
+__device__ __forceinline__ float load1<float>(const float *p)
+{
+    return *p;
+}
+template <>
+__device__ __forceinline__ float load1<__nv_bfloat16>(const __nv_bfloat16 *p)
+{
+    return __bfloat162float(*p);
+}
+
+template <typename T>
 __device__ __forceinline__ void store1(T *p, float v);
 template <>
 __device__ __forceinline__ void store1<float>(float *p, float v)
@@ -45,8 +58,8 @@ __device__ __forceinline__ void store1<__nv_bfloat16>(__nv_bfloat16 *p, float v)
 template <typename T, typename TOut>
 __global__ void __launch_bounds__(256)
 gemm_simt_kernel(const T *__restrict__ A1, const T *__restrict__ A2, const T *__restrict__ B,
-                 const float *__restrict__ bias, TOut *__restrict__ out, long long M, int K1,
-                 int K2, int N, int relu)
+                 const T *__restrict__ addend, const float *__restrict__ bias, TOut *__restrict__ out,
+                 long long M, int K1, int K2, int N, int ldb, int relu)
 {
     __shared__ float As[BK][BM + 4];
     __shared__ float Bs[BK][BN + 4];
@@ -54,11 +67,11 @@ gemm_simt_kernel(const T *__restrict__ A1, const T *__restrict__ A2, const T *__
     const int tx = tid % 16, ty = tid / 16;
     const long long row0 = (long long)blockIdx.x * BM;
     const int col0 = blockIdx.y * BN;
-    const int ldb = K1 + K2;
+    const int Kt = K1 + K2;
     const int lr = tid / 4;        // 0..63: tile row (A) / tile col (B) this thread loads
     const int lk = (tid % 4) * 2;  // 0,2,4,6
     float acc[4][4] = {};
-    for (int k0 = 0; k0 < ldb; k0 += BK) {
+    for (int k0 = 0; k0 < Kt; k0 += BK) {
         // K1 and K2 are multiples of 8 = BK, so a K tile never straddles the two segments
         const bool seg2 = k0 >= K1;
         const T *A = seg2 ? A2 : A1;
@@ -95,6 +108,7 @@ gemm_simt_kernel(const T *__restrict__ A1, const T *__restrict__ A2, const T *__
             const int c = col0 + tx * 4 + j;
             if (c >= N) continue;
             float v = acc[i][j];
+            if (addend) v += load1<T>(addend + (size_t)r * N + c);
             if (bias) v += bias[c];
             if (relu) v = fmaxf(v, 0.f);
             store1<TOut>(out + (size_t)r * N + c, v);
@@ -127,16 +141,18 @@ cudaError_t run(const GemmArgs &a, float *ztmp, cudaStream_t s, int *launches)
     dim3 grid((unsigned)mb, (unsigned)((a.N + BN - 1) / BN));
     const T *A1 = static_cast<const T *>(a.A1), *A2 = static_cast<const T *>(a.A2);
     const T *B = static_cast<const T *>(a.B);
+    const T *add = static_cast<const T *>(a.addend);
+    const int ldb = a.ldb > 0 ? a.ldb : a.K1 + a.K2;
     if (a.l2norm) {
         if (!ztmp) return cudaErrorInvalidValue;
-        gemm_simt_kernel<T, float><<<grid, 256, 0, s>>>(A1, A2, B, a.bias, ztmp, a.M, a.K1, a.K2,
-                                                        a.N, a.relu);
+        gemm_simt_kernel<T, float><<<grid, 256, 0, s>>>(A1, A2, B, add, a.bias, ztmp, a.M, a.K1, a.K2,
+                                                        a.N, ldb, a.relu);
         const long long rb = (a.M + 7) / 8;
         rownorm_kernel<T><<<(unsigned)rb, 256, 0, s>>>(ztmp, static_cast<T *>(a.out), a.M, a.N);
         if (launches) *launches += 2;
     } else {
-        gemm_simt_kernel<T, T><<<grid, 256, 0, s>>>(A1, A2, B, a.bias, static_cast<T *>(a.out),
-                                                    a.M, a.K1, a.K2, a.N, a.relu);
+        gemm_simt_kernel<T, T><<<grid, 256, 0, s>>>(A1, A2, B, add, a.bias, static_cast<T *>(a.out),
+                                                    a.M, a.K1, a.K2, a.N, ldb, a.relu);
         if (launches) *launches += 1;
     }
     return cudaGetLastError();

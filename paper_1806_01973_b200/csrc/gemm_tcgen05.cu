@@ -63,6 +63,7 @@ struct TcParams {
     int cg;            // CTAs per tile: 1, or 2 = CTA pair (tcgen05 cta_group::2, 256-row tiles)
     int cluster;       // CTAs per cluster: cg, or cg * n_slabs when the row norm is exchanged (DSMEM)
     const float *bias;
+    const uint4 *addend;   // optional [M x N] bf16 added to the accumulator (row stride N), or null
     int relu, l2norm;
     uint32_t idesc;
 };
@@ -243,6 +244,23 @@ __device__ __forceinline__ void tc_ld32(uint32_t taddr, uint32_t (&v)[32])
 __device__ __forceinline__ void tc_wait_ld()
 {
     asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
+}
+
+// 32 addend values (bf16, columns c .. c+31 of one row) as four 16-byte words; chunks at or beyond
+// c_hi are not touched and read as zero.
+__device__ __forceinline__ void load_addend32(const uint4 *arow, int c, int c_hi, uint4 (&ad)[4])
+{
+#pragma unroll
+    for (int q = 0; q < 4; ++q) {
+        ad[q] = make_uint4(0, 0, 0, 0);
+        if (arow != nullptr && c + 8 * q < c_hi) ad[q] = __ldg(arow + (c >> 3) + q);
+    }
+}
+__device__ __forceinline__ uint32_t addend_pair(const uint4 (&ad)[4], int i)   // elements i, i+1 (i even)
+{
+    const uint4 &w = ad[i >> 3];
+    const int k = (i & 7) >> 1;
+    return k == 0 ? w.x : k == 1 ? w.y : k == 2 ? w.z : w.w;
 }
 
 // One lane of a fully converged warp.  Issuing tcgen05.mma / TMA under `elect.sync` (the whole warp
@@ -481,20 +499,30 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap tmA1, const __grid_constant__
             mbar_wait(bar_tfull + 8 * acc, accphase);
             tc_fence_after();
             const uint32_t t0 = tmem_base + ((uint32_t)(ew * 32) << 16) + (uint32_t)acc * p.acc_cols;
+            // this row's slice of the addend (slab column 0), null if there is none or the row is past M
+            const uint4 *arow = (p.addend != nullptr && m0 + row < p.M)
+                                    ? p.addend + (((size_t)(m0 + row) * (size_t)p.N + (size_t)n0) >> 3)
+                                    : nullptr;
             float scale = 1.f;
             if (p.l2norm) {
-                // pass 1: sum of squares of this row's z = act(acc + bias) over my columns, in order
+                // pass 1: sum of squares of this row's z = act(acc + addend + bias) over my columns
                 const int par = (int)(it & 1);
                 float ss = 0.f;
                 for (int c0 = c_lo; c0 < c_hi; c0 += 32) {
                     uint32_t v[32];
+                    uint4 ad[4];
                     tc_ld32(t0 + c0, v);
+                    load_addend32(arow, c0, c_hi, ad);
                     tc_wait_ld();
 #pragma unroll
-                    for (int i = 0; i < 32; ++i) {
-                        float z = __uint_as_float(v[i]) + sbias[c0 + i];
-                        z = p.relu ? fmaxf(z, 0.f) : z;
-                        ss = (c0 + i < c_hi) ? fmaf(z, z, ss) : ss;
+                    for (int i = 0; i < 32; i += 2) {
+                        const uint32_t aw = addend_pair(ad, i);
+                        float z0 = __uint_as_float(v[i]) + __uint_as_float(aw << 16) + sbias[c0 + i];
+                        float z1 = __uint_as_float(v[i + 1]) + __uint_as_float(aw & 0xffff0000u) + sbias[c0 + i + 1];
+                        z0 = p.relu ? fmaxf(z0, 0.f) : z0;
+                        z1 = p.relu ? fmaxf(z1, 0.f) : z1;
+                        ss = (c0 + i < c_hi) ? fmaf(z0, z0, ss) : ss;
+                        ss = (c0 + i + 1 < c_hi) ? fmaf(z1, z1, ss) : ss;
                     }
                 }
                 if (p.epi_halves == 2) {
@@ -531,11 +559,15 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap tmA1, const __grid_constant__
                 tc_wait_ld();
                 uint32_t pk[32];
 #pragma unroll
-                for (int h = 0; h < 2; ++h)
+                for (int h = 0; h < 2; ++h) {
+                    uint4 ad[4];
+                    load_addend32(arow, c0 + 32 * h, c_hi, ad);
 #pragma unroll
                     for (int i = 0; i < 32; i += 2) {
-                        float z0 = __uint_as_float(v[h][i]) + sbias[c0 + 32 * h + i];
-                        float z1 = __uint_as_float(v[h][i + 1]) + sbias[c0 + 32 * h + i + 1];
+                        const uint32_t aw = addend_pair(ad, i);
+                        float z0 = __uint_as_float(v[h][i]) + __uint_as_float(aw << 16) + sbias[c0 + 32 * h + i];
+                        float z1 = __uint_as_float(v[h][i + 1]) + __uint_as_float(aw & 0xffff0000u) +
+                                   sbias[c0 + 32 * h + i + 1];
                         if (p.relu) {
                             z0 = fmaxf(z0, 0.f);
                             z1 = fmaxf(z1, 0.f);
@@ -543,6 +575,7 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap tmA1, const __grid_constant__
                         __nv_bfloat162 b = __floats2bfloat162_rn(z0 * scale, z1 * scale);
                         pk[16 * h + i / 2] = *reinterpret_cast<uint32_t *>(&b);
                     }
+                }
                 if (lane == 0) tma_store_wait_read<1>();          // the buffer used two stores ago is free
                 __syncwarp();
                 uint8_t *buf = stg + sbuf * STG_WARP_BYTES;
@@ -612,12 +645,12 @@ EncodeTiledFn encode_fn()
 
 // Row-major bf16 matrix [rows x cols] (cols contiguous), box = box_rows x 64 columns, SWIZZLE_128B.
 // Out-of-bounds parts of a box read as zero and are not written.
-bool make_map(CUtensorMap *map, const void *ptr, long long rows, int cols, int box_rows)
+bool make_map(CUtensorMap *map, const void *ptr, long long rows, int cols, int box_rows, int ld = 0)
 {
     EncodeTiledFn fn = encode_fn();
     if (!fn) return false;
     const cuuint64_t dims[2] = {(cuuint64_t)cols, (cuuint64_t)rows};
-    const cuuint64_t strides[1] = {(cuuint64_t)cols * 2};
+    const cuuint64_t strides[1] = {(cuuint64_t)(ld > 0 ? ld : cols) * 2};
     const cuuint32_t box[2] = {(cuuint32_t)BK, (cuuint32_t)box_rows};
     const cuuint32_t estr[2] = {1, 1};
     return fn(map, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 2, const_cast<void *>(ptr), dims, strides, box,
@@ -638,6 +671,7 @@ bool plan(const GemmArgs &a, int cg, int ns_pref, int epi_pref, TcParams &p, int
     if (a.M < 1 || a.M >= (1LL << 31)) return no("M outside [1, 2^31)");
     if (a.K1 < 8 || a.K1 % 8 || a.K2 < 0 || a.K2 % 8) return no("K1, K2 must be multiples of 8");
     if (a.N < 8 || a.N % 8) return no("N must be a multiple of 8");
+    if (a.ldb % 8 || (a.ldb > 0 && a.ldb < a.K1 + a.K2)) return no("ldb must be a multiple of 8, >= K1 + K2");
     if (cg == 2 && (a.M <= BM || a.N % 16)) return no("CTA pairs need M > 128 and N % 16 == 0");
     p = TcParams{};
     p.cg = cg;
@@ -680,6 +714,7 @@ bool plan(const GemmArgs &a, int cg, int ns_pref, int epi_pref, TcParams &p, int
     p.c_split = round_up((p.NS + 1) / 2, 64);
     smem_bytes = p.stages * p.stage_bytes + fixed;
     p.bias = a.bias;
+    p.addend = static_cast<const uint4 *>(a.addend);
     p.relu = a.relu;
     p.l2norm = a.l2norm;
     // instruction descriptor, kind::f16: D fp32 (bit 4), A and B bf16 (bits 7, 10), both K-major,
@@ -781,7 +816,7 @@ cudaError_t launch_gemm_tc(const GemmArgs &a, const GemmTune &t, int num_sms, cu
     } else {
         tmA2 = tmA1;
     }
-    if (!make_map(&tmB, a.B, a.N, a.K1 + a.K2, p.CN / p.cg)) return cudaErrorInvalidValue;
+    if (!make_map(&tmB, a.B, a.N, a.K1 + a.K2, p.CN / p.cg, a.ldb)) return cudaErrorInvalidValue;
     if (!make_map(&tmOut, a.out, a.M, a.N, 32)) return cudaErrorInvalidValue;
     if (launches) ++*launches;
     if (p.cg == 2)

@@ -15,13 +15,18 @@ inline size_t elem_size(DType t) { return t == DType::BF16 ? 2 : 4; }
 
 // out[M x N] = epi(A1[M x K1] * B[:, 0:K1]^T + A2[M x K2] * B[:, K1:K1+K2]^T + bias)
 // B is [N x (K1+K2)] row-major ("out x in"), i.e. K-major.  K2 == 0 -> single segment.
-// epi: +bias (if non-null) -> ReLU (if relu) -> row L2 normalisation (if l2norm) -> round to dtype.
+// epi: +addend (if non-null) -> +bias (if non-null) -> ReLU (if relu) -> row L2 normalisation (if l2norm) -> round to dtype.
 struct GemmArgs {
     int64_t M = 0;
     int32_t K1 = 0, K2 = 0, N = 0;
     const void *A1 = nullptr;
     const void *A2 = nullptr;
     const void *B = nullptr;
+    int32_t ldb = 0;                // row stride of B in elements; 0 = K1 + K2 (B may be a column
+                                    // block of a wider matrix, e.g. W1 / W2 inside W)
+    const void *addend = nullptr;   // optional [M x N] (dtype, row stride N) added to the product in
+                                    // fp32 before bias / ReLU: the pooled W2-projection of the
+                                    // linear-pool schedule
     const float *bias = nullptr;
     int relu = 0;
     int l2norm = 0;

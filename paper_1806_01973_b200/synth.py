@@ -39,6 +39,7 @@ class Config:
     zipf_s: float = 0.0
     unit_rows: bool = False   # config 3: features row-L2-normalised before rounding
     seed: int = 0
+    m_proj: int = 0      # projection width m when it differs from d (0: m = hidden)
 
     def scaled(self, N: int, name: Optional[str] = None) -> "Config":
         """The "-small" sibling: same dims, T, K and value laws, fewer nodes."""
@@ -48,7 +49,7 @@ class Config:
         """[(d_in, m, d)] per layer."""
         out, d_in = [], self.d0
         for _ in range(self.K):
-            out.append((d_in, self.hidden, self.hidden))
+            out.append((d_in, self.m_proj or self.hidden, self.hidden))
             d_in = self.hidden
         return out
 
@@ -63,6 +64,10 @@ CONFIGS: Dict[str, Config] = {
                    "multinomial_ids", walks=200, zipf_s=1.2),
     "cfg5": Config("cfg5", 50_000_000, 256, 100, 3, 256, 256, 256, "bf16", "uniform",
                    "zipf_shape"),
+    # not a BASELINE config: the paper's own geometry: d0 = 4096 + 256 + 1 padded
+    # to 4360, m = 2048, d = 1024, T = 50, K = 2 -- exercises m > d (the linear-pool schedule)
+    "paper": Config("paper", 2_000_000, 4360, 50, 2, 1024, 1024, 1024, "bf16", "uniform",
+                    "multinomial_pool", walks=500, zipf_s=1.1, unit_rows=True, m_proj=2048),
 }
 
 _TAG_X, _TAG_IDX, _TAG_CNT, _TAG_LAYER, _TAG_HEAD = 1, 2, 3, 10, 99
