@@ -212,3 +212,10 @@ def test_full_cfg4_power_law(ctx):
 def test_full_cfg5_deep_wide(ctx):
     _need_memory(150)
     _full_size(ctx, "cfg5", n_e2e=2, e2e_batch=2, n_layer=2048, few=True)
+
+
+def test_full_paper_geometry_linear_pool(ctx):
+    """Not a BASELINE config: the paper's own widths (d0 = 4096 + 256 + 1 -> 4360, m = 2048,
+    d = 1024) on 2 000 000 nodes, which runs the linear-pool schedule (m > d)."""
+    _need_memory(70)
+    _full_size(ctx, "paper", n_e2e=8, e2e_batch=32, n_layer=512, few=True)
