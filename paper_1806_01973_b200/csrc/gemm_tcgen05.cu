@@ -263,6 +263,19 @@ __device__ __forceinline__ uint32_t addend_pair(const uint4 (&ad)[4], int i)   /
     return k == 0 ? w.x : k == 1 ? w.y : k == 2 ? w.z : w.w;
 }
 
+// v[0..31] (fp32 bit patterns of accumulator columns c..c+31) += addend columns, in place
+__device__ __forceinline__ void add_addend32(const uint4 *arow, int c, int c_hi, uint32_t (&v)[32])
+{
+    uint4 ad[4];
+    load_addend32(arow, c, c_hi, ad);
+#pragma unroll
+    for (int i = 0; i < 32; i += 2) {
+        const uint32_t aw = addend_pair(ad, i);
+        v[i] = __float_as_uint(__uint_as_float(v[i]) + __uint_as_float(aw << 16));
+        v[i + 1] = __float_as_uint(__uint_as_float(v[i + 1]) + __uint_as_float(aw & 0xffff0000u));
+    }
+}
+
 // One lane of a fully converged warp.  Issuing tcgen05.mma / TMA under `elect.sync` (the whole warp
 // runs the surrounding loop) lets ptxas keep descriptors in uniform registers: UTCHMMA instructions
 // issue back to back, where an `if (lane == 0)` region costs 11-24 SASS instructions per MMA and
@@ -510,19 +523,14 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap tmA1, const __grid_constant__
                 float ss = 0.f;
                 for (int c0 = c_lo; c0 < c_hi; c0 += 32) {
                     uint32_t v[32];
-                    uint4 ad[4];
                     tc_ld32(t0 + c0, v);
-                    load_addend32(arow, c0, c_hi, ad);
                     tc_wait_ld();
+                    if (p.addend != nullptr) add_addend32(arow, c0, c_hi, v);   // uniform branch
 #pragma unroll
-                    for (int i = 0; i < 32; i += 2) {
-                        const uint32_t aw = addend_pair(ad, i);
-                        float z0 = __uint_as_float(v[i]) + __uint_as_float(aw << 16) + sbias[c0 + i];
-                        float z1 = __uint_as_float(v[i + 1]) + __uint_as_float(aw & 0xffff0000u) + sbias[c0 + i + 1];
-                        z0 = p.relu ? fmaxf(z0, 0.f) : z0;
-                        z1 = p.relu ? fmaxf(z1, 0.f) : z1;
-                        ss = (c0 + i < c_hi) ? fmaf(z0, z0, ss) : ss;
-                        ss = (c0 + i + 1 < c_hi) ? fmaf(z1, z1, ss) : ss;
+                    for (int i = 0; i < 32; ++i) {
+                        float z = __uint_as_float(v[i]) + sbias[c0 + i];
+                        z = p.relu ? fmaxf(z, 0.f) : z;
+                        ss = (c0 + i < c_hi) ? fmaf(z, z, ss) : ss;
                     }
                 }
                 if (p.epi_halves == 2) {
@@ -557,17 +565,17 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap tmA1, const __grid_constant__
                 tc_ld32(t0 + c0, v[0]);
                 tc_ld32(t0 + c0 + 32, v[1]);
                 tc_wait_ld();
+                if (p.addend != nullptr) {                        // uniform branch
+                    add_addend32(arow, c0, c_hi, v[0]);
+                    add_addend32(arow, c0 + 32, c_hi, v[1]);
+                }
                 uint32_t pk[32];
 #pragma unroll
                 for (int h = 0; h < 2; ++h) {
-                    uint4 ad[4];
-                    load_addend32(arow, c0 + 32 * h, c_hi, ad);
 #pragma unroll
                     for (int i = 0; i < 32; i += 2) {
-                        const uint32_t aw = addend_pair(ad, i);
-                        float z0 = __uint_as_float(v[h][i]) + __uint_as_float(aw << 16) + sbias[c0 + 32 * h + i];
-                        float z1 = __uint_as_float(v[h][i + 1]) + __uint_as_float(aw & 0xffff0000u) +
-                                   sbias[c0 + 32 * h + i + 1];
+                        float z0 = __uint_as_float(v[h][i]) + sbias[c0 + 32 * h + i];
+                        float z1 = __uint_as_float(v[h][i + 1]) + sbias[c0 + 32 * h + i + 1];
                         if (p.relu) {
                             z0 = fmaxf(z0, 0.f);
                             z1 = fmaxf(z1, 0.f);
