@@ -366,3 +366,21 @@ def minibatch_embed(M, fetch_x, fetch_nbr, layers, head_params=None, return_hidd
     HM = H[np.searchsorted(S[K], M)]
     out = head(HM, head_params) if head_params is not None else HM
     return (out, at_M) if return_hidden else out
+
+
+def walk_neighbourhoods(row_ptr, col_idx, n_walks: int, walk_len: int, T: int, seed: int = 0):
+    """Importance-based neighbourhoods by simulated random walks (readings
+    B1-B5): returns (nbr_idx [N, T] int32, counts [N, T] int32), top-T by (count desc, id asc)."""
+    row_ptr = np.ascontiguousarray(row_ptr, dtype=np.int64)
+    col_idx = np.ascontiguousarray(col_idx, dtype=np.int32)
+    N = row_ptr.shape[0] - 1
+    assert row_ptr[0] == 0 and row_ptr[-1] == col_idx.shape[0] and np.all(np.diff(row_ptr) >= 0)
+    assert col_idx.size == 0 or (col_idx.min() >= 0 and col_idx.max() < N)
+    idx = np.empty((N, T), dtype=np.int32)
+    cnt = np.empty((N, T), dtype=np.int32)
+    lib().oracle_walk_neighbourhoods(
+        ctypes.c_int64(N), row_ptr.ctypes.data_as(ctypes.POINTER(ctypes.c_int64)),
+        col_idx.ctypes.data_as(_i32p), ctypes.c_int32(n_walks), ctypes.c_int32(walk_len),
+        ctypes.c_int32(T), ctypes.c_uint64(seed), idx.ctypes.data_as(_i32p),
+        cnt.ctypes.data_as(_i32p))
+    return idx, cnt

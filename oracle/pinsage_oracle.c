@@ -83,8 +83,8 @@ void oracle_normalize_counts(int64_t N, int32_t T, const int32_t *counts, float 
         for (int t = 0; t < T; ++t)
             tot += counts[v * T + t];
         float ftot = (float)tot;
-        for (int t = 0; t < T; ++t)
-            alpha[v * T + t] = (float)counts[v * T + t] / ftot;
+        for (int t = 0; t < T; ++t)   /* a node that visited nobody (reading B4) has all-zero weights */
+            alpha[v * T + t] = tot > 0 ? (float)counts[v * T + t] / ftot : 0.0f;
     }
 }
 
@@ -307,4 +307,87 @@ void oracle_rec(int64_t u, int32_t k, int32_t T, const int32_t *dims, const int3
     free(nbr);
     free(a);
     free(scratch);
+}
+
+/* ---------------------------------------------------------------------------------------------
+ * Importance-based neighbourhoods: "we simulate random walks starting from
+ * node u and compute the L1-normalized visit count of nodes visited by the random walk.  The
+ * neighborhood of u is then defined as the top T nodes with the highest normalized visit counts".
+ * The paper gives no walk parameters (it cites Pixie [14]); readings B1-B5 of DESIGN.md:
+ *   B1 the graph is a CSR adjacency (row_ptr [N+1] int64, col_idx [E] int32), any ids in [0, N);
+ *   B2 n_walks walks per node, each restarting at u and taking walk_len steps to a uniformly
+ *      chosen out-neighbour of the current node; a node without out-neighbours ends the walk;
+ *   B3 every arrival at a node v != u is one visit (u is never its own neighbour);
+ *   B4 keep the T most visited, ties to the smaller id, in that order; fewer than T distinct
+ *      visited nodes: pad with id u and count 0 (weight 0, reading A7);
+ *   B5 randomness is counter-based, a function of (seed, u, walk, step) only:
+ *      key = mix(seed + 0x100000001B3 * u), x = mix(key ^ (walk << 32 | step)), mix = the
+ *      splitmix64 finaliser; choice = ((x >> 32) * degree) >> 32.
+ * counts are the raw integer visit counts; the L1 normalisation is oracle_normalize_counts.
+ * -------------------------------------------------------------------------------------------- */
+static uint64_t walk_mix(uint64_t z)
+{
+    z += 0x9E3779B97F4A7C15ULL;
+    z = (z ^ (z >> 30)) * 0xBF58476D1CE4E5B9ULL;
+    z = (z ^ (z >> 27)) * 0x94D049BB133111EBULL;
+    return z ^ (z >> 31);
+}
+
+static int cmp_i32(const void *a, const void *b)
+{
+    int32_t x = *(const int32_t *)a, y = *(const int32_t *)b;
+    return (x > y) - (x < y);
+}
+
+typedef struct { int32_t id, count; } visit_t;
+
+static int cmp_visit(const void *a, const void *b)   /* count descending, then id ascending */
+{
+    const visit_t *x = (const visit_t *)a, *y = (const visit_t *)b;
+    if (x->count != y->count) return (x->count < y->count) - (x->count > y->count);
+    return (x->id > y->id) - (x->id < y->id);
+}
+
+void oracle_walk_neighbourhoods(int64_t N, const int64_t *row_ptr, const int32_t *col_idx,
+                                int32_t n_walks, int32_t walk_len, int32_t T, uint64_t seed,
+                                int32_t *nbr_idx, int32_t *counts)
+{
+#pragma omp parallel
+    {
+        int32_t *seen = (int32_t *)malloc(sizeof(int32_t) * (size_t)n_walks * walk_len + 4);
+        visit_t *vis = (visit_t *)malloc(sizeof(visit_t) * ((size_t)n_walks * walk_len + 1));
+#pragma omp for schedule(dynamic, 64)
+        for (int64_t u = 0; u < N; ++u) {
+            const uint64_t key = walk_mix(seed + 0x100000001B3ULL * (uint64_t)u);
+            size_t ns = 0;
+            for (int32_t r = 0; r < n_walks; ++r) {
+                int64_t cur = u;
+                for (int32_t s = 0; s < walk_len; ++s) {
+                    const int64_t beg = row_ptr[cur], deg = row_ptr[cur + 1] - beg;
+                    if (deg <= 0) break;                                         /* B2 */
+                    const uint64_t x = walk_mix(key ^ (((uint64_t)r << 32) | (uint64_t)s));
+                    const uint64_t pick = ((x >> 32) * (uint64_t)deg) >> 32;     /* B5 */
+                    cur = col_idx[beg + (int64_t)pick];
+                    if (cur != u) seen[ns++] = (int32_t)cur;                     /* B3 */
+                }
+            }
+            qsort(seen, ns, sizeof(int32_t), cmp_i32);
+            size_t nv = 0;
+            for (size_t i = 0; i < ns;) {
+                size_t j = i;
+                while (j < ns && seen[j] == seen[i]) ++j;
+                vis[nv].id = seen[i];
+                vis[nv].count = (int32_t)(j - i);
+                ++nv;
+                i = j;
+            }
+            qsort(vis, nv, sizeof(visit_t), cmp_visit);                          /* B4 */
+            for (int32_t t = 0; t < T; ++t) {
+                nbr_idx[u * T + t] = (size_t)t < nv ? vis[t].id : (int32_t)u;
+                counts[u * T + t] = (size_t)t < nv ? vis[t].count : 0;
+            }
+        }
+        free(seen);
+        free(vis);
+    }
 }

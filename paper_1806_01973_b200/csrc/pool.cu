@@ -359,7 +359,8 @@ normalize_counts_kernel(const int *__restrict__ counts, float *__restrict__ w, l
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) tot += __shfl_xor_sync(0xffffffffu, tot, o);
     const float ftot = (float)tot;
-    for (int t = lane; t < T; t += 32) w[row * T + t] = __fdiv_rn((float)c[t], ftot);
+    // a row without any visit (an isolated node of the neighbourhood builder) gets all-zero weights
+    for (int t = lane; t < T; t += 32) w[row * T + t] = tot > 0 ? __fdiv_rn((float)c[t], ftot) : 0.f;
 }
 
 __global__ void __launch_bounds__(256)

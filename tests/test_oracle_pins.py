@@ -410,3 +410,79 @@ def test_variant_layers_compose_the_pinned_steps():
     Pm = np.maximum(X @ lp["Q"].T + lp["q"], 0)[idx2].max(axis=1)
     Z = np.maximum(X @ lp["W"][:, :d_in].T + Pm @ lp["W"][:, d_in:].T + lp["w"], 0)
     np.testing.assert_allclose(out, _rownorm(Z), atol=1e-14)
+
+
+# --------------------------------------------------------------------------- importance neighbourhoods
+def _csr(adj):
+    row_ptr = np.zeros(len(adj) + 1, dtype=np.int64)
+    row_ptr[1:] = np.cumsum([len(a) for a in adj])
+    col = np.array([v for a in adj for v in a], dtype=np.int32)
+    return row_ptr, col
+
+
+def test_walks_on_a_directed_cycle_are_deterministic():
+    """Out-degree 1 leaves nothing to chance: R walks of L steps from u visit u+1..u+L, R times
+    each (readings B2-B4: ties to the smaller id, padding = (u, 0))."""
+    N, R, L, T = 20, 7, 4, 6
+    rp, ci = _csr([[(u + 1) % N] for u in range(N)])
+    idx, cnt = O.walk_neighbourhoods(rp, ci, R, L, T, seed=3)
+    for u in range(N):
+        ids = sorted((u + s) % N for s in range(1, L + 1))
+        assert list(idx[u]) == ids + [u] * (T - L)
+        assert list(cnt[u]) == [R] * L + [0] * (T - L)
+    # a cycle shorter than the walk returns to u: arrivals at u are not counted (B3)
+    rp, ci = _csr([[1], [2], [0]])
+    idx, cnt = O.walk_neighbourhoods(rp, ci, 5, 6, 2, seed=0)
+    assert list(idx[0]) == [1, 2] and list(cnt[0]) == [10, 10]
+
+
+def test_walk_visit_frequencies_match_the_markov_chain():
+    """Expected visits of v != u per walk = sum_{s=1..L} (e_u P^s)_v with P the uniform
+    out-neighbour transition matrix (and, as L grows, Personalized PageRank -- PAPER.md fn. 2):
+    pins the uniform choice, the restart at u, the step count and the exclusion of u."""
+    rng = np.random.default_rng(70)
+    N, R, L = 12, 60000, 4
+    adj = [list(rng.choice(np.delete(np.arange(N), u), size=rng.integers(1, 5), replace=False))
+           for u in range(N)]
+    adj[5] = []                                   # a dead end (B2): walks stop there
+    rp, ci = _csr(adj)
+    P = np.zeros((N, N))
+    for u, a in enumerate(adj):
+        for v in a:
+            P[u, v] += 1.0 / len(a)
+    idx, cnt = O.walk_neighbourhoods(rp, ci, R, L, N, seed=11)   # T = N: nothing truncated
+    for u in (0, 3, 7):
+        e = np.zeros(N)
+        e[u] = 1.0
+        expect = np.zeros(N)
+        for _ in range(L):
+            e = e @ P
+            expect += e
+        expect[u] = 0.0
+        got = np.zeros(N)
+        got[idx[u]] += cnt[u] / R
+        np.testing.assert_allclose(got, expect, atol=5 * np.sqrt(L / R) + 1e-12)
+        assert cnt[u].sum() <= R * L
+    assert np.all(cnt[5] == 0) and np.all(idx[5] == 5)          # isolated start: all padding
+    assert np.all(O.normalize_counts(cnt[5:6]) == 0)             # and all-zero weights, not NaN
+
+
+def test_walk_neighbourhoods_ranking_and_counter_based_rng():
+    rng = np.random.default_rng(71)
+    N = 40
+    adj = [list(rng.integers(0, N, size=rng.integers(1, 8))) for _ in range(N)]   # repeats, self loops
+    rp, ci = _csr(adj)
+    full_i, full_c = O.walk_neighbourhoods(rp, ci, 50, 3, N, seed=5)
+    top_i, top_c = O.walk_neighbourhoods(rp, ci, 50, 3, 6, seed=5)
+    np.testing.assert_array_equal(top_i, full_i[:, :6])          # top-T is a prefix of the ranking
+    np.testing.assert_array_equal(top_c, full_c[:, :6])
+    for u in range(N):
+        keys = [(-int(c), int(i)) for i, c in zip(full_i[u], full_c[u]) if c > 0]
+        assert keys == sorted(keys) and len({k[1] for k in keys}) == len(keys)   # count desc, id asc
+        assert u not in {k[1] for k in keys}
+        assert full_c[u].sum() <= 50 * 3
+    # counter-based: a node's walks depend on (seed, u) and the graph only -- appending an
+    # unreachable node changes no existing row; another seed changes the draws
+    rp2, ci2 = _csr(adj + [[0]])
+    np.testing.assert_array_equal(O.walk_neighbourhoods(rp2, ci2, 50, 3, 6, seed=5)[0][:N], top_i)
+    assert not np.array_equal(O.walk_neighbourhoods(rp, ci, 50, 3, 6, seed=6)[1], top_c)
