@@ -193,6 +193,19 @@ pinsage_status pinsage_embed_all(pinsage_ctx *ctx, pinsage_dtype dtype, int64_t 
 pinsage_status pinsage_normalize_counts(pinsage_ctx *ctx, int64_t N, int32_t T,
                                         const int32_t *counts, float *nbr_w);
 
+/* Importance-based neighbourhoods: for every node u simulate n_walks random walks
+ * that start at u and take walk_len steps to a uniformly chosen out-neighbour (a node without
+ * out-neighbours ends the walk), count the arrivals at every node v != u, and keep the T most visited
+ * nodes (ties to the smaller id) in that order; a node with fewer than T distinct visited nodes is
+ * padded with (id u, count 0).  The graph is a CSR adjacency: row_ptr [N+1] int64 (row_ptr[0] = 0,
+ * non-decreasing), col_idx [row_ptr[N]] int32 in [0, N) -- device pointers, as are the outputs
+ * nbr_idx / counts [N x T] int32.  Draws are a counter-based function of (seed, u, walk, step), so the
+ * result does not depend on scheduling (readings B1-B5).  counts feeds
+ * pinsage_normalize_counts.  1 <= n_walks * walk_len <= 2048 (else PINSAGE_ERR_UNSUPPORTED_SHAPE). */
+pinsage_status pinsage_build_neighbourhoods(pinsage_ctx *ctx, int64_t N, const int64_t *row_ptr,
+                                            const int32_t *col_idx, int32_t n_walks, int32_t walk_len,
+                                            int32_t T, uint64_t seed, int32_t *nbr_idx, int32_t *counts);
+
 /* Synchronous.  Checks 0 <= nbr_idx[i] < n_src for all n_dst*T entries and that every weight is
  * finite.  *first_bad (HOST pointer) receives the flat position of the first offender or -1;
  * returns PINSAGE_ERR_BAD_INDEX if there is one. */

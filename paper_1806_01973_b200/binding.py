@@ -26,6 +26,7 @@ SYMBOLS = [
     "pinsage_set_option", "pinsage_launch_count", "pinsage_profile_read", "pinsage_dense", "pinsage_pool",
     "pinsage_combine", "pinsage_layer", "pinsage_layer_workspace_bytes", "pinsage_head",
     "pinsage_embed_all", "pinsage_normalize_counts", "pinsage_validate_graph",
+    "pinsage_build_neighbourhoods",
 ]
 
 
@@ -96,6 +97,8 @@ def load_library() -> ctypes.CDLL:
     lib.pinsage_embed_all.restype = ctypes.c_int
     lib.pinsage_normalize_counts.argtypes = [vp, i64, i32, vp, vp]
     lib.pinsage_normalize_counts.restype = ctypes.c_int
+    lib.pinsage_build_neighbourhoods.argtypes = [vp, i64, vp, vp, i32, i32, i32, ctypes.c_uint64, vp, vp]
+    lib.pinsage_build_neighbourhoods.restype = ctypes.c_int
     lib.pinsage_validate_graph.argtypes = [vp, i64, i64, i32, vp, vp, ctypes.POINTER(i64)]
     lib.pinsage_validate_graph.restype = ctypes.c_int
     _lib = lib
@@ -272,6 +275,18 @@ class Context:
             out = torch.empty((N, T), dtype=torch.float32, device=counts.device)
         self._check(self.lib.pinsage_normalize_counts(self.handle, N, T, _ptr(counts), _ptr(out)))
         return out
+
+    def pinsage_build_neighbourhoods(self, row_ptr, col_idx, n_walks: int, walk_len: int, T: int,
+                                     seed: int = 0):
+        """(nbr_idx, counts) [N, T] int32 from a CSR graph (row_ptr int64 [N+1], col_idx int32)."""
+        assert row_ptr.dtype == torch.int64 and col_idx.dtype == torch.int32
+        N = row_ptr.shape[0] - 1
+        idx = torch.empty((N, T), dtype=torch.int32, device=row_ptr.device)
+        cnt = torch.empty((N, T), dtype=torch.int32, device=row_ptr.device)
+        self._check(self.lib.pinsage_build_neighbourhoods(
+            self.handle, N, _ptr(row_ptr), _ptr(col_idx), int(n_walks), int(walk_len), int(T),
+            ctypes.c_uint64(seed), _ptr(idx), _ptr(cnt)))
+        return idx, cnt
 
     def pinsage_validate_graph(self, nbr_idx, nbr_w, n_src: int) -> int:
         """Returns -1 if the tables are valid, else raises PinsageError(BAD_INDEX)."""

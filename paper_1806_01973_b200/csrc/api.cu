@@ -982,6 +982,29 @@ pinsage_status pinsage_normalize_counts(pinsage_ctx *ctx, int64_t N, int32_t T,
     return PINSAGE_OK;
 }
 
+pinsage_status pinsage_build_neighbourhoods(pinsage_ctx *ctx, int64_t N, const int64_t *row_ptr,
+                                            const int32_t *col_idx, int32_t n_walks, int32_t walk_len,
+                                            int32_t T, uint64_t seed, int32_t *nbr_idx, int32_t *counts)
+{
+    if (!ctx) return PINSAGE_ERR_INVALID_ARG;
+    DeviceGuard guard(ctx->device);
+    PS_TRY(check_graph_args(ctx, N, T));
+    if (n_walks < 1 || walk_len < 1)
+        return fail(ctx, PINSAGE_ERR_INVALID_ARG, "n_walks = %d and walk_len = %d must be positive", n_walks, walk_len);
+    if (walk_slots(n_walks, walk_len) == 0)
+        return fail(ctx, PINSAGE_ERR_UNSUPPORTED_SHAPE, "n_walks * walk_len = %lld exceeds 2048",
+                    (long long)n_walks * walk_len);
+    PS_TRY(check_ptr(ctx, "row_ptr", row_ptr));
+    PS_TRY(check_ptr(ctx, "nbr_idx", nbr_idx));
+    PS_TRY(check_ptr(ctx, "counts", counts));
+    // col_idx may be NULL for a graph without edges (it is then never dereferenced)
+    cudaError_t e = launch_walk_neighbourhoods(N, row_ptr, col_idx, n_walks, walk_len, T, seed, nbr_idx,
+                                               counts, ctx->stream, &ctx->launches);
+    count_launches(ctx);
+    PS_CUDA(ctx, e);
+    return PINSAGE_OK;
+}
+
 pinsage_status pinsage_validate_graph(pinsage_ctx *ctx, int64_t n_dst, int64_t n_src, int32_t T,
                                       const int32_t *nbr_idx, const float *nbr_w,
                                       int64_t *first_bad)

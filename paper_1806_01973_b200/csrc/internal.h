@@ -66,4 +66,11 @@ cudaError_t launch_normalize_counts(int64_t N, int32_t T, const int32_t *counts,
 cudaError_t launch_validate(int64_t n_dst, int64_t n_src, int32_t T, const int32_t *idx,
                             const float *w, long long *first_bad, cudaStream_t s, int *launches);
 
+// ---- walks.cu: importance-based neighbourhoods by simulated random walks ------------------------
+// walk_slots: shared-memory key slots per node (0 = n_walks * walk_len outside [1, 2048]).
+int walk_slots(int32_t n_walks, int32_t walk_len);
+cudaError_t launch_walk_neighbourhoods(int64_t N, const int64_t *row_ptr, const int32_t *col_idx,
+                                       int32_t n_walks, int32_t walk_len, int32_t T, uint64_t seed,
+                                       int32_t *nbr_idx, int32_t *counts, cudaStream_t s, int *launches);
+
 }  // namespace pinsage

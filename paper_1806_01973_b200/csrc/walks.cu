@@ -1,0 +1,171 @@
+// walks.cu -- importance-based neighbourhoods by simulated random walks:
+// "we simulate random walks starting from node u and compute the L1-normalized visit count of
+// nodes visited by the random walk ... the top T nodes with the highest normalized visit counts".
+// This is the step that PRODUCES the (nbr_idx, counts) tables the pool consumes.
+//
+// The paper gives no walk parameters; readings B1-B5: CSR graph; n_walks walks per node,
+// each restarting at u and taking walk_len uniform out-neighbour steps (a dead end stops the walk);
+// every arrival at v != u is a visit; keep the T most visited (ties to the smaller id), pad with
+// (u, 0); draws are a counter-based function of (seed, u, walk, step) -- splitmix64 finaliser.
+//
+// One warp per node.  Lane l simulates walks l, l+32, ... (a latency-bound pointer chase, hidden by
+// many resident warps) and drops every arrival into slot walk*walk_len + step of a shared-memory
+// array of 64-bit keys (empty = all ones).  The warp then (1) bitonic-sorts the keys, (2) run-length
+// encodes them in place into keys (~count << 32 | id), (3) bitonic-sorts those -- ascending order is
+// (count descending, id ascending) -- and (4) writes the first T.  Integer work only: bit-exact and
+// independent of scheduling.
+#include "internal.h"
+
+namespace pinsage {
+namespace {
+
+constexpr int WARPS_PER_CTA = 4;
+constexpr unsigned long long EMPTY = ~0ull;
+
+__device__ __forceinline__ unsigned long long mix64(unsigned long long z)
+{
+    z += 0x9E3779B97F4A7C15ull;
+    z = (z ^ (z >> 30)) * 0xBF58476D1CE4E5B9ull;
+    z = (z ^ (z >> 27)) * 0x94D049BB133111EBull;
+    return z ^ (z >> 31);
+}
+
+// ascending bitonic sort of s[0 .. n), n a power of two >= 32, by one warp
+__device__ __forceinline__ void warp_bitonic_sort(unsigned long long *s, int n, int lane)
+{
+    for (int k = 2; k <= n; k <<= 1) {
+        for (int j = k >> 1; j > 0; j >>= 1) {
+            for (int i = lane; i < n; i += 32) {
+                const int ixj = i ^ j;
+                if (ixj > i) {
+                    const unsigned long long a = s[i], b = s[ixj];
+                    const bool up = (i & k) == 0;
+                    if ((a > b) == up) {
+                        s[i] = b;
+                        s[ixj] = a;
+                    }
+                }
+            }
+            __syncwarp();
+        }
+    }
+}
+
+__global__ void __launch_bounds__(WARPS_PER_CTA * 32)
+walk_neighbourhoods_kernel(const long long *__restrict__ row_ptr, const int *__restrict__ col_idx,
+                           long long N, int n_walks, int walk_len, int T, unsigned long long seed,
+                           int slots /* power of two >= max(32, n_walks * walk_len) */,
+                           int *__restrict__ nbr_idx, int *__restrict__ counts)
+{
+    extern __shared__ __align__(16) unsigned long long walk_smem[];
+    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+    const long long u = (long long)blockIdx.x * WARPS_PER_CTA + wid;
+    if (u >= N) return;
+    unsigned long long *s = walk_smem + (size_t)wid * slots;
+    for (int i = lane; i < slots; i += 32) s[i] = EMPTY;
+    __syncwarp();
+
+    // ---- the walks (B2, B3, B5) -----------------------------------------------------------------
+    const unsigned long long key = mix64(seed + 0x100000001B3ull * (unsigned long long)u);
+    for (int r = lane; r < n_walks; r += 32) {
+        long long cur = u;
+        for (int st = 0; st < walk_len; ++st) {
+            const long long beg = __ldg(row_ptr + cur);
+            const long long deg = __ldg(row_ptr + cur + 1) - beg;
+            if (deg <= 0) break;
+            const unsigned long long x = mix64(key ^ (((unsigned long long)r << 32) | (unsigned long long)st));
+            const unsigned long long pick = ((x >> 32) * (unsigned long long)deg) >> 32;
+            cur = __ldg(col_idx + beg + (long long)pick);
+            if (cur != u) s[r * walk_len + st] = (unsigned long long)(unsigned)cur;
+        }
+    }
+    __syncwarp();
+
+    // ---- (1) sort the arrivals; (2) run-length encode in place -----------------------------------
+    warp_bitonic_sort(s, slots, lane);
+    int ns = 0;
+    for (int base = 0; base < slots; base += 32)
+        ns += __popc(__ballot_sync(0xffffffffu, s[base + lane] != EMPTY));
+    int nv = 0;                              // distinct ids written so far
+    unsigned long long carry_prev = EMPTY;   // last id of the previous chunk
+    int carry_start = 0;                     // start index of the run that enters this chunk
+    for (int base = 0; base < ns; base += 32) {
+        const int i = base + lane;
+        const bool valid = i < ns;
+        const unsigned long long a = valid ? s[i] : EMPTY;
+        const unsigned long long nxt = (i + 1 < ns) ? s[i + 1] : EMPTY;
+        unsigned long long prev = __shfl_up_sync(0xffffffffu, a, 1);
+        if (lane == 0) prev = carry_prev;
+        const bool is_start = valid && (i == 0 || a != prev);
+        const bool is_end = valid && a != nxt;
+        int start = is_start ? i : -1;       // inclusive max-scan: start index of my run
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) {
+            const int t = __shfl_up_sync(0xffffffffu, start, o);
+            if (lane >= o) start = max(start, t);
+        }
+        if (start < 0) start = carry_start;
+        const unsigned ends = __ballot_sync(0xffffffffu, is_end);
+        const int pos = nv + __popc(ends & ((1u << lane) - 1u));
+        const unsigned count = (unsigned)(i - start + 1);
+        __syncwarp();                        // every read of this chunk is done before any write
+        if (is_end) s[pos] = ((unsigned long long)(0xFFFFFFFFu - count) << 32) | a;
+        carry_prev = __shfl_sync(0xffffffffu, a, 31);
+        carry_start = __shfl_sync(0xffffffffu, start, 31);
+        nv += __popc(ends);
+        __syncwarp();
+    }
+
+    // ---- (3) rank: ascending (~count, id) = count descending, id ascending (B4) -------------------
+    int n2 = 32;
+    while (n2 < nv) n2 <<= 1;
+    for (int i = nv + lane; i < n2; i += 32) s[i] = EMPTY;
+    __syncwarp();
+    warp_bitonic_sort(s, n2, lane);
+
+    // ---- (4) the top T, padded with (u, 0) ------------------------------------------------------------
+    for (int t = lane; t < T; t += 32) {
+        int id = (int)u, c = 0;
+        if (t < nv) {
+            const unsigned long long k = s[t];
+            id = (int)(unsigned)(k & 0xFFFFFFFFull);
+            c = (int)(0xFFFFFFFFu - (unsigned)(k >> 32));
+        }
+        nbr_idx[u * T + t] = id;
+        counts[u * T + t] = c;
+    }
+}
+
+}  // namespace
+
+int walk_slots(int32_t n_walks, int32_t walk_len)
+{
+    const long long need = (long long)n_walks * walk_len;
+    if (n_walks < 1 || walk_len < 1 || need > 2048) return 0;
+    int s = 32;
+    while (s < need) s <<= 1;
+    return s;
+}
+
+cudaError_t launch_walk_neighbourhoods(int64_t N, const int64_t *row_ptr, const int32_t *col_idx,
+                                       int32_t n_walks, int32_t walk_len, int32_t T, uint64_t seed,
+                                       int32_t *nbr_idx, int32_t *counts, cudaStream_t s, int *launches)
+{
+    const int slots = walk_slots(n_walks, walk_len);
+    if (slots == 0) return cudaErrorNotSupported;
+    const long long blocks = (N + WARPS_PER_CTA - 1) / WARPS_PER_CTA;
+    if (blocks > 0x7fffffffLL) return cudaErrorInvalidConfiguration;
+    const size_t smem = (size_t)WARPS_PER_CTA * slots * sizeof(unsigned long long);
+    if (smem > 48 * 1024) {
+        cudaError_t e = cudaFuncSetAttribute(walk_neighbourhoods_kernel,
+                                             cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        if (e != cudaSuccess) return e;
+    }
+    walk_neighbourhoods_kernel<<<(unsigned)blocks, WARPS_PER_CTA * 32, smem, s>>>(
+        reinterpret_cast<const long long *>(row_ptr), col_idx, N, n_walks, walk_len, T,
+        (unsigned long long)seed, slots, nbr_idx, counts);
+    if (launches) ++*launches;
+    return cudaGetLastError();
+}
+
+}  // namespace pinsage

@@ -256,3 +256,23 @@ def make_graph(cfg: Config, device="cpu", row_chunk: int = 1 << 20):
         else:
             raise ValueError(cfg.count_law)
     return idx, cnt
+
+
+def make_csr(N: int, deg_lo: int, deg_hi: int, law: str = "uniform", zipf_s: float = 1.2,
+             seed: int = 0, device="cpu"):
+    """A synthetic directed graph in CSR form for the neighbourhood builder: out-degrees iid uniform
+    on [deg_lo, deg_hi] (deg_lo = 0 gives dead ends), targets iid uniform over node ids or
+    Zipf(zipf_s) over ids (hub-heavy, as in a user-curated graph -- PAPER.md:58); repeated edges
+    and self loops may occur.  Returns (row_ptr [N+1] int64, col_idx [E] int32)."""
+    g = _gen(seed, 4, device)
+    deg = torch.randint(deg_lo, deg_hi + 1, (N,), generator=g, device=device, dtype=torch.int64)
+    row_ptr = torch.zeros(N + 1, dtype=torch.int64, device=device)
+    row_ptr[1:] = torch.cumsum(deg, 0)
+    E = int(row_ptr[-1])
+    if law == "uniform":
+        col = torch.randint(0, N, (E,), generator=g, device=device, dtype=torch.int64)
+    elif law == "zipf":
+        col = _zipf(torch.rand((E,), generator=g, device=device, dtype=torch.float64), N, zipf_s)
+    else:
+        raise ValueError(law)
+    return row_ptr, col.to(torch.int32)
