@@ -186,6 +186,20 @@ pinsage_status pinsage_embed_all(pinsage_ctx *ctx, pinsage_dtype dtype, int64_t 
                                  const float *nbr_w, const pinsage_layer_params *layers,
                                  const pinsage_head_params *head, void *out, int64_t chunk_nodes);
 
+/* Targeted / incremental inference = Algorithm 2 on a minibatch: embeds only the M
+ * nodes listed in `targets` (device int32 [M], ids in [0, N), repeats allowed) by building their K-hop
+ * sets S^(K) = targets, S^(k-1) = S^(k) U N(S^(k)) (l.1-7), re-indexing the sub-tables (:182) and running
+ * the same S1-S5 kernels on the closure only.  All pointers are DEVICE pointers; feats / nbr_idx / nbr_w
+ * describe the whole graph as in pinsage_embed_all; out:[M x head->d_out], row j = embedding of
+ * targets[j], bit-identical to row targets[j] of pinsage_embed_all.  The call synchronises the stream
+ * K + 1 times (set sizes are read back); scratch is context-owned.  A target outside [0, N) gives
+ * PINSAGE_ERR_BAD_INDEX. */
+pinsage_status pinsage_embed_nodes(pinsage_ctx *ctx, pinsage_dtype dtype, int64_t N, int32_t T,
+                                   int32_t K, const void *feats, const int32_t *nbr_idx,
+                                   const float *nbr_w, const pinsage_layer_params *layers,
+                                   const pinsage_head_params *head, int64_t M, const int32_t *targets,
+                                   void *out);
+
 /* ---- helpers ------------------------------------------------------------------------------ */
 
 /* nbr_w[v,t] = (float)counts[v,t] / (float)(sum_t counts[v,t]) in IEEE binary32 (L1-normalised visit

@@ -26,7 +26,7 @@ SYMBOLS = [
     "pinsage_set_option", "pinsage_launch_count", "pinsage_profile_read", "pinsage_dense", "pinsage_pool",
     "pinsage_combine", "pinsage_layer", "pinsage_layer_workspace_bytes", "pinsage_head",
     "pinsage_embed_all", "pinsage_normalize_counts", "pinsage_validate_graph",
-    "pinsage_build_neighbourhoods",
+    "pinsage_build_neighbourhoods", "pinsage_embed_nodes",
 ]
 
 
@@ -97,6 +97,10 @@ def load_library() -> ctypes.CDLL:
     lib.pinsage_embed_all.restype = ctypes.c_int
     lib.pinsage_normalize_counts.argtypes = [vp, i64, i32, vp, vp]
     lib.pinsage_normalize_counts.restype = ctypes.c_int
+    lib.pinsage_embed_nodes.argtypes = [vp, ctypes.c_int, i64, i32, i32, vp, vp, vp,
+                                        ctypes.POINTER(LayerParams), ctypes.POINTER(HeadParams),
+                                        i64, vp, vp]
+    lib.pinsage_embed_nodes.restype = ctypes.c_int
     lib.pinsage_build_neighbourhoods.argtypes = [vp, i64, vp, vp, i32, i32, i32, ctypes.c_uint64, vp, vp]
     lib.pinsage_build_neighbourhoods.restype = ctypes.c_int
     lib.pinsage_validate_graph.argtypes = [vp, i64, i64, i32, vp, vp, ctypes.POINTER(i64)]
@@ -274,6 +278,23 @@ class Context:
         if out is None:
             out = torch.empty((N, T), dtype=torch.float32, device=counts.device)
         self._check(self.lib.pinsage_normalize_counts(self.handle, N, T, _ptr(counts), _ptr(out)))
+        return out
+
+    def pinsage_embed_nodes(self, feats, nbr_idx, nbr_w, layers: Sequence[dict], head: dict, targets,
+                            out=None):
+        """Embeddings of the nodes in `targets` (int32 CUDA tensor) only, via their K-hop closure."""
+        N, d0 = feats.shape
+        T = nbr_idx.shape[1]
+        K = len(layers)
+        arr = (LayerParams * K)(*[_layer_struct(lp) for lp in layers])
+        hs = _head_struct(head)
+        assert arr[0].d_in == d0 and targets.dtype == torch.int32 and targets.dim() == 1
+        M = targets.shape[0]
+        if out is None:
+            out = torch.empty((M, hs.d_out), dtype=feats.dtype, device=feats.device)
+        self._check(self.lib.pinsage_embed_nodes(
+            self.handle, dtype_code(feats.dtype), N, T, K, _ptr(feats), _ptr(nbr_idx), _ptr(nbr_w), arr,
+            ctypes.byref(hs), M, _ptr(targets), _ptr(out)))
         return out
 
     def pinsage_build_neighbourhoods(self, row_ptr, col_idx, n_walks: int, walk_len: int, T: int,

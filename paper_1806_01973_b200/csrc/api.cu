@@ -41,6 +41,8 @@ struct pinsage_ctx {
     void *stage = nullptr;           // device staging for host inputs / outputs
     size_t stage_bytes = 0;
     long long *d_first_bad = nullptr;
+    void *subA = nullptr, *subB = nullptr;   // scratch of pinsage_embed_nodes (sets / compact tensors)
+    size_t subA_bytes = 0, subB_bytes = 0;
     // optional per-kernel timing ("profile" option): event pairs around every launch
     int profile = 0;
     std::vector<cudaEvent_t> prof_events;
@@ -183,6 +185,24 @@ int pick_slab(const pinsage_ctx *ctx, DType dt, int64_t n_src, int32_t T, int32_
     return 0;
 }
 
+pinsage_status ensure_buf(pinsage_ctx *ctx, void **buf, size_t *cap, size_t bytes, const char *what)
+{
+    if (bytes <= *cap) return PINSAGE_OK;
+    if (*buf) {
+        PS_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
+        cudaFree(*buf);
+        *buf = nullptr;
+        *cap = 0;
+    }
+    cudaError_t e = cudaMalloc(buf, bytes);
+    if (e != cudaSuccess) {
+        cudaGetLastError();
+        return fail(ctx, PINSAGE_ERR_OOM, "%s of %zu bytes: %s", what, bytes, cudaGetErrorString(e));
+    }
+    *cap = bytes;
+    return PINSAGE_OK;
+}
+
 enum ProfKind { PROF_POOL = 0, PROF_DENSE = 1, PROF_COMBINE = 2, PROF_KINDS = 3 };
 
 // Records an event on stream s (profile mode only) and returns its slot, or -1.
@@ -321,8 +341,9 @@ pinsage_status pool_combine_chunks(pinsage_ctx *ctx, DType dt, int64_t N, int32_
                                    const pinsage_layer_params *lp, const void *Hin, const void *P,
                                    const int32_t *idx, const float *w, void *Hout, int64_t chunk,
                                    void *nbuf0, void *nbuf1, void *scratch, size_t scratch_bytes,
-                                   const cudaEvent_t *tables_landed = nullptr)
+                                   const cudaEvent_t *tables_landed = nullptr, int64_t n_src = -1)
 {
+    if (n_src < 0) n_src = N;                // rows of P; N = destination rows
     const size_t es = elem_size(dt);
     const bool linear = use_linear_pool(ctx, lp);
     const int32_t pw = linear ? lp->d : lp->m;
@@ -341,7 +362,7 @@ pinsage_status pool_combine_chunks(pinsage_ctx *ctx, DType dt, int64_t N, int32_
         if (tables_landed) PS_CUDA(ctx, cudaStreamWaitEvent(ps, tables_landed[c], 0));
         const int pe0 = prof_mark(ctx, ps);
         cudaError_t e = launch_pool(dt, ctx->pool_mode, rows, T, pw, P, idx + (size_t)r0 * T, w + (size_t)r0 * T,
-                                    nb[b], pick_slab(ctx, dt, N, T, pw), ps, &ctx->launches);
+                                    nb[b], pick_slab(ctx, dt, n_src, T, pw), ps, &ctx->launches);
         prof_close(ctx, PROF_POOL, pe0, ps);
         count_launches(ctx);
         PS_CUDA(ctx, e);
@@ -418,18 +439,25 @@ pinsage_status layer_on_ws(pinsage_ctx *ctx, DType dt, int64_t N, int32_t T, con
                            const int32_t *idx, const float *w, const pinsage_layer_params *lp,
                            void *out, char *ws, const LayerWs &plan, int64_t chunk,
                            const cudaEvent_t *feats_landed = nullptr,
-                           const cudaEvent_t *tables_landed = nullptr)
+                           const cudaEvent_t *tables_landed = nullptr, int64_t n_src = -1,
+                           const void *src_feats = nullptr)
 {
+    // n_src / src_feats (targeted inference): the source rows S1 projects differ from the N
+    // destination rows, whose own previous representations are `feats`
     const size_t es = elem_size(dt);
     const bool linear = use_linear_pool(ctx, lp);
-    const int64_t s1_rows = (feats_landed || linear) ? chunk : N;
-    for (int64_t r0 = 0, c = 0; r0 < N; r0 += s1_rows, ++c) {
+    if (n_src < 0) {
+        n_src = N;
+        src_feats = feats;
+    }
+    const int64_t s1_rows = (feats_landed || linear) ? chunk : n_src;
+    for (int64_t r0 = 0, c = 0; r0 < n_src; r0 += s1_rows, ++c) {
         if (feats_landed) PS_CUDA(ctx, cudaStreamWaitEvent(ctx->stream, feats_landed[c], 0));
         GemmArgs g;
-        g.M = std::min(s1_rows, N - r0);
+        g.M = std::min(s1_rows, n_src - r0);
         g.K1 = lp->d_in;
         g.N = lp->m;
-        g.A1 = static_cast<const char *>(feats) + (size_t)r0 * lp->d_in * es;
+        g.A1 = static_cast<const char *>(src_feats) + (size_t)r0 * lp->d_in * es;
         g.B = lp->Q;
         g.bias = lp->q;
         g.relu = 1;
@@ -449,7 +477,7 @@ pinsage_status layer_on_ws(pinsage_ctx *ctx, DType dt, int64_t N, int32_t T, con
     }
     return pool_combine_chunks(ctx, dt, N, T, lp, feats, ws + plan.P_off, idx, w, out, chunk,
                                ws + plan.n0_off, ws + plan.n1_off, ws + plan.scratch_off,
-                               plan.scratch_bytes, tables_landed);
+                               plan.scratch_bytes, tables_landed, n_src);
 }
 
 // Grows the per-chunk event pool of the host-buffer pipeline to n events.
@@ -555,6 +583,8 @@ void pinsage_destroy(pinsage_ctx *ctx)
     if (ctx->ws) cudaFree(ctx->ws);
     if (ctx->stage) cudaFree(ctx->stage);
     if (ctx->d_first_bad) cudaFree(ctx->d_first_bad);
+    if (ctx->subA) cudaFree(ctx->subA);
+    if (ctx->subB) cudaFree(ctx->subB);
     for (cudaEvent_t e : ctx->prof_events) cudaEventDestroy(e);
     cudaGetLastError();
     delete ctx;
@@ -965,6 +995,119 @@ pinsage_status pinsage_embed_all(pinsage_ctx *ctx, pinsage_dtype dtype, int64_t 
         PS_CUDA(ctx, cudaStreamSynchronize(ctx->h2d));
         PS_CUDA(ctx, cudaStreamSynchronize(ctx->d2h));
     }
+    return PINSAGE_OK;
+}
+
+pinsage_status pinsage_embed_nodes(pinsage_ctx *ctx, pinsage_dtype dtype, int64_t N, int32_t T,
+                                   int32_t K, const void *feats, const int32_t *nbr_idx,
+                                   const float *nbr_w, const pinsage_layer_params *layers,
+                                   const pinsage_head_params *head, int64_t M, const int32_t *targets,
+                                   void *out)
+{
+    if (!ctx) return PINSAGE_ERR_INVALID_ARG;
+    DeviceGuard guard(ctx->device);
+    PS_TRY(check_dtype(ctx, dtype));
+    PS_TRY(check_graph_args(ctx, N, T));
+    if (K < 1 || K > 64) return fail(ctx, PINSAGE_ERR_INVALID_ARG, "K = %d outside [1, 64]", K);
+    if (M < 1 || M >= (1LL << 31)) return fail(ctx, PINSAGE_ERR_INVALID_ARG, "M = %lld outside [1, 2^31)", (long long)M);
+    if (!layers) return fail(ctx, PINSAGE_ERR_INVALID_ARG, "layers is NULL");
+    for (int k = 0; k < K; ++k) {
+        PS_TRY(check_layer_params(ctx, &layers[k], "layers[k]"));
+        if (k > 0 && layers[k].d_in != layers[k - 1].d)
+            return fail(ctx, PINSAGE_ERR_INVALID_ARG, "layers[%d].d_in != layers[%d].d", k, k - 1);
+    }
+    PS_TRY(check_head_params(ctx, head));
+    if (head->d != layers[K - 1].d) return fail(ctx, PINSAGE_ERR_INVALID_ARG, "head.d != layers[K-1].d");
+    PS_TRY(check_ptr(ctx, "feats", feats));
+    PS_TRY(check_ptr(ctx, "nbr_idx", nbr_idx));
+    PS_TRY(check_ptr(ctx, "nbr_w", nbr_w));
+    PS_TRY(check_ptr(ctx, "targets", targets));
+    PS_TRY(check_ptr(ctx, "out", out));
+    const DType dt = static_cast<DType>(dtype);
+    const size_t es = elem_size(dt);
+    cudaStream_t st = ctx->stream;
+    PS_TRY(maybe_validate(ctx, N, N, T, nbr_idx, nbr_w));
+
+    // ---- phase A: the sets S^(K) = targets, S^(k-1) = S^(k) U N(S^(k))  (Alg. 2 l.1-7) ---------------
+    const long long nb = subset_blocks(N);
+    const size_t markB = align_up((size_t)N, 256), i32B = align_up((size_t)N * 4, 256);
+    const size_t cntB = align_up((size_t)(nb + 1) * 8, 256);
+    PS_TRY(ensure_buf(ctx, &ctx->subA, &ctx->subA_bytes, (size_t)(K + 1) * (markB + 2 * i32B) + cntB,
+                      "embed_nodes set storage"));
+    char *A = static_cast<char *>(ctx->subA);
+    auto mark = [&](int k) { return reinterpret_cast<unsigned char *>(A + (size_t)k * markB); };
+    auto list = [&](int k) { return reinterpret_cast<int32_t *>(A + (size_t)(K + 1) * markB + (size_t)k * i32B); };
+    auto pos = [&](int k) { return reinterpret_cast<int32_t *>(A + (size_t)(K + 1) * (markB + i32B) + (size_t)k * i32B); };
+    long long *counts = reinterpret_cast<long long *>(A + (size_t)(K + 1) * (markB + 2 * i32B));
+    PS_CUDA(ctx, cudaMemsetAsync(A, 0, (size_t)(K + 1) * markB, st));
+    PS_CUDA(ctx, subset_mark_targets(targets, M, N, mark(K), ctx->d_first_bad, st, &ctx->launches));
+    std::vector<int64_t> n(K + 1, 0);
+    for (int k = K; k >= 0; --k) {
+        PS_CUDA(ctx, subset_compact(mark(k), N, counts, nullptr, nullptr, false, st, &ctx->launches));
+        long long host[2] = {0, 0};
+        PS_CUDA(ctx, cudaMemcpyAsync(&host[0], counts + nb, 8, cudaMemcpyDeviceToHost, st));
+        PS_CUDA(ctx, cudaMemcpyAsync(&host[1], ctx->d_first_bad, 8, cudaMemcpyDeviceToHost, st));
+        PS_CUDA(ctx, cudaStreamSynchronize(st));
+        if (k == K && host[1] != 0x7fffffffffffffffLL) {
+            count_launches(ctx);
+            return fail(ctx, PINSAGE_ERR_BAD_INDEX, "targets[%lld] is outside [0, %lld)", host[1], (long long)N);
+        }
+        n[k] = host[0];
+        PS_CUDA(ctx, subset_compact(mark(k), N, counts, list(k), pos(k), true, st, &ctx->launches));
+        if (k > 0) PS_CUDA(ctx, subset_expand(list(k), n[k], nbr_idx, T, mark(k - 1), st, &ctx->launches));
+    }
+    count_launches(ctx);
+
+    // ---- phase B: compact tensors, sized from the set sizes ----------------------------------------------
+    size_t Hmax = (size_t)n[0] * layers[0].d_in * es, selfmax = 0, tabmax = 0, wsmax = 0;
+    std::vector<int64_t> chunk(K + 1, 0);
+    for (int k = 1; k <= K; ++k) {
+        const pinsage_layer_params *lp = &layers[k - 1];
+        Hmax = std::max(Hmax, (size_t)n[k] * lp->d * es);
+        selfmax = std::max(selfmax, (size_t)n[k] * lp->d_in * es);
+        tabmax = std::max(tabmax, (size_t)n[k] * T * 4);
+        chunk[k] = auto_chunk(n[k], 0, (size_t)std::max(lp->m, lp->d) * es);
+        wsmax = std::max(wsmax, plan_layer_ws(ctx, dt, n[k - 1], lp, chunk[k]).total);
+    }
+    const size_t aB = align_up((size_t)n[K] * head->g1 * es, 256), oB = align_up((size_t)n[K] * head->d_out * es, 256);
+    Hmax = align_up(Hmax, 256); selfmax = align_up(selfmax, 256); tabmax = align_up(tabmax, 256);
+    wsmax = align_up(wsmax, 256);
+    PS_TRY(ensure_buf(ctx, &ctx->subB, &ctx->subB_bytes, 2 * Hmax + selfmax + 2 * tabmax + wsmax + aB + oB,
+                      "embed_nodes compact tensors"));
+    char *B = static_cast<char *>(ctx->subB);
+    char *Hbuf[2] = {B, B + Hmax};
+    char *Hself = B + 2 * Hmax;
+    int32_t *idx_loc = reinterpret_cast<int32_t *>(Hself + selfmax);
+    float *w_loc = reinterpret_cast<float *>(Hself + selfmax + tabmax);
+    char *lws = Hself + selfmax + 2 * tabmax;
+    char *abuf = lws + wsmax, *obuf = abuf + aB;
+
+    // h^(0) = x on S^(0)  (Alg. 2 l.8), then CONVOLVE level by level on the re-indexed sub-graph (l.9-14)
+    PS_CUDA(ctx, subset_gather_rows(feats, list(0), nullptr, n[0], (size_t)layers[0].d_in * es, Hbuf[0], st,
+                                    &ctx->launches));
+    int cur = 0;
+    for (int k = 1; k <= K; ++k) {
+        const pinsage_layer_params *lp = &layers[k - 1];
+        PS_CUDA(ctx, subset_remap_tables(list(k), n[k], nbr_idx, nbr_w, T, pos(k - 1), idx_loc, w_loc, st,
+                                         &ctx->launches));
+        PS_CUDA(ctx, subset_gather_rows(Hbuf[cur], list(k), pos(k - 1), n[k], (size_t)lp->d_in * es, Hself, st,
+                                        &ctx->launches));
+        count_launches(ctx);
+        const LayerWs plan = plan_layer_ws(ctx, dt, n[k - 1], lp, chunk[k]);
+        PS_TRY(layer_on_ws(ctx, dt, n[k], T, Hself, idx_loc, w_loc, lp, Hbuf[cur ^ 1], lws, plan, chunk[k],
+                           nullptr, nullptr, n[k - 1], Hbuf[cur]));
+        cur ^= 1;
+    }
+    // head on S^(K) (l.15-17), then one row per requested target, in the caller's order
+    GemmArgs g;
+    g.M = n[K]; g.K1 = head->d; g.N = head->g1; g.A1 = Hbuf[cur]; g.B = head->G1; g.bias = head->g;
+    g.relu = 1; g.out = abuf;
+    PS_TRY(run_gemm(ctx, dt, g, nullptr, 0, st));
+    GemmArgs g2;
+    g2.M = n[K]; g2.K1 = head->g1; g2.N = head->d_out; g2.A1 = abuf; g2.B = head->G2; g2.out = obuf;
+    PS_TRY(run_gemm(ctx, dt, g2, nullptr, 0, st));
+    PS_CUDA(ctx, subset_gather_rows(obuf, targets, pos(K), M, (size_t)head->d_out * es, out, st, &ctx->launches));
+    count_launches(ctx);
     return PINSAGE_OK;
 }
 

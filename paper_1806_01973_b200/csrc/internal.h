@@ -73,4 +73,18 @@ cudaError_t launch_walk_neighbourhoods(int64_t N, const int64_t *row_ptr, const 
                                        int32_t n_walks, int32_t walk_len, int32_t T, uint64_t seed,
                                        int32_t *nbr_idx, int32_t *counts, cudaStream_t s, int *launches);
 
+// ---- subset.cu: K-hop sets of a minibatch and re-indexed sub-tables (Algorithm 2 l.1-7) ----------
+long long subset_blocks(int64_t N);
+cudaError_t subset_mark_targets(const int32_t *targets, int64_t M, int64_t N, unsigned char *mark,
+                                long long *first_bad, cudaStream_t s, int *launches);
+cudaError_t subset_expand(const int32_t *list, int64_t n, const int32_t *idx, int32_t T,
+                          unsigned char *mark_prev, cudaStream_t s, int *launches);
+cudaError_t subset_compact(const unsigned char *mark, int64_t N, long long *counts, int32_t *list,
+                           int32_t *pos, bool scatter, cudaStream_t s, int *launches);
+cudaError_t subset_gather_rows(const void *src, const int32_t *ids, const int32_t *map, int64_t n,
+                               size_t row_bytes, void *dst, cudaStream_t s, int *launches);
+cudaError_t subset_remap_tables(const int32_t *list, int64_t n, const int32_t *idx, const float *w,
+                                int32_t T, const int32_t *pos_prev, int32_t *idx_loc, float *w_loc,
+                                cudaStream_t s, int *launches);
+
 }  // namespace pinsage
