@@ -137,6 +137,16 @@ def _full_size(ctx, name, n_e2e, e2e_batch, n_layer, few=False, head_block=4_000
     report.update(e2e_rows=len(M), e2e_max_rel=worst, e2e_min_cos=cmin, e2e_s=round(time.time() - t0, 1))
     del fx
 
+    # ---- (a') targeted inference (Algorithm 2 on the GPU) reproduces the same rows bit for bit --------
+    Mt = M[:4] if few else M
+    tg = torch.from_numpy(Mt).to(DEV).to(torch.int32)
+    sub = ctx.pinsage_embed_nodes(X, idx, alpha, layers, head, tg)
+    torch.cuda.synchronize()
+    assert torch.equal(sub.view(torch.int16), out[tg.long()].view(torch.int16)), \
+        f"{name}: pinsage_embed_nodes differs from pinsage_embed_all on the sampled rows"
+    report["embed_nodes_rows"] = len(Mt)
+    del sub
+
     # ---- (b) one layer at a time on the GPU's own H_{k-1} -----------------------------------------
     t0 = time.time()
     H = X
