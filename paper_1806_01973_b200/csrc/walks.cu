@@ -10,9 +10,9 @@
 //
 // One warp per node.  Lane l simulates walks l, l+32, ... (a latency-bound pointer chase, hidden by
 // many resident warps) and drops every arrival into slot walk*walk_len + step of a shared-memory
-// array of 64-bit keys (empty = all ones).  The warp then (1) bitonic-sorts the keys, (2) run-length
-// encodes them in place into keys (~count << 32 | id), (3) bitonic-sorts those -- ascending order is
-// (count descending, id ascending) -- and (4) writes the first T.  Integer work only: bit-exact and
+// array of 64-bit keys (empty = all ones).  The warp then (1) bitonic-sorts the keys in registers,
+// (2) run-length encodes them in place (shared memory) into keys (~count << 32 | id), (3) bitonic-sorts
+// those in registers -- ascending order is (count descending, id ascending) -- and (4) writes the first T.  Integer work only: bit-exact and
 // independent of scheduling.
 #include "internal.h"
 
@@ -30,33 +30,68 @@ __device__ __forceinline__ unsigned long long mix64(unsigned long long z)
     return z ^ (z >> 31);
 }
 
-// ascending bitonic sort of s[0 .. n), n a power of two >= 32, by one warp
-__device__ __forceinline__ void warp_bitonic_sort(unsigned long long *s, int n, int lane)
+// ---- register-resident bitonic sort ------------------------------------------------------------------
+// A warp sorts 32 * R keys held R per lane: key i lives in register i / 32 of lane i % 32.  Partners at
+// distance j < 32 are in another lane (one shuffle), at distance j >= 32 in another register of the same
+// lane (register indices are compile-time through the JR template).  No shared-memory traffic: the
+// shared-memory version of these sorts ran at 78 % of the shared pipe and bounded the kernel.
+template <int R, int JR>
+__device__ __forceinline__ void cmpex_regs(unsigned long long (&v)[R], int k, int lane)
 {
-    for (int k = 2; k <= n; k <<= 1) {
-        for (int j = k >> 1; j > 0; j >>= 1) {
-            for (int i = lane; i < n; i += 32) {
-                const int ixj = i ^ j;
-                if (ixj > i) {
-                    const unsigned long long a = s[i], b = s[ixj];
-                    const bool up = (i & k) == 0;
-                    if ((a > b) == up) {
-                        s[i] = b;
-                        s[ixj] = a;
-                    }
-                }
-            }
-            __syncwarp();
+#pragma unroll
+    for (int r = 0; r < R; ++r) {
+        const int rr = r ^ JR;
+        if (rr > r) {
+            const bool up = (((r << 5) | lane) & k) == 0;
+            const unsigned long long a = v[r], b = v[rr];
+            const bool sw = (a > b) == up;
+            v[r] = sw ? b : a;
+            v[rr] = sw ? a : b;
         }
     }
 }
+template <int R>
+__device__ __forceinline__ void stage_regs(unsigned long long (&v)[R], int jr, int k, int lane)
+{
+    switch (jr) {
+    case 1: if constexpr (R > 1) cmpex_regs<R, 1>(v, k, lane); break;
+    case 2: if constexpr (R > 2) cmpex_regs<R, 2>(v, k, lane); break;
+    case 4: if constexpr (R > 4) cmpex_regs<R, 4>(v, k, lane); break;
+    case 8: if constexpr (R > 8) cmpex_regs<R, 8>(v, k, lane); break;
+    case 16: if constexpr (R > 16) cmpex_regs<R, 16>(v, k, lane); break;
+    case 32: if constexpr (R > 32) cmpex_regs<R, 32>(v, k, lane); break;
+    }
+}
+template <int R>
+__device__ __forceinline__ void stage_shfl(unsigned long long (&v)[R], int j, int k, int lane)
+{
+    const bool lower = (lane & j) == 0;
+#pragma unroll
+    for (int r = 0; r < R; ++r) {
+        const bool up = (((r << 5) | lane) & k) == 0;
+        const unsigned long long a = v[r], b = __shfl_xor_sync(0xffffffffu, a, j);
+        v[r] = (lower == up) ? (a < b ? a : b) : (a > b ? a : b);
+    }
+}
+// ascending sort of the first n keys' worth of stages (n a power of two, 32 <= n <= 32 * R; keys at
+// index >= n must be EMPTY so that they stay in place)
+template <int R>
+__device__ __forceinline__ void warp_sort_regs(unsigned long long (&v)[R], int n, int lane)
+{
+    for (int k = 2; k <= n; k <<= 1)
+        for (int j = k >> 1; j > 0; j >>= 1) {
+            if (j >= 32) stage_regs<R>(v, j >> 5, k, lane);
+            else stage_shfl<R>(v, j, k, lane);
+        }
+}
 
+template <int R>
 __global__ void __launch_bounds__(WARPS_PER_CTA * 32)
 walk_neighbourhoods_kernel(const long long *__restrict__ row_ptr, const int *__restrict__ col_idx,
                            long long N, int n_walks, int walk_len, int T, unsigned long long seed,
-                           int slots /* power of two >= max(32, n_walks * walk_len) */,
                            int *__restrict__ nbr_idx, int *__restrict__ counts)
 {
+    constexpr int slots = 32 * R;            // power of two >= max(32, n_walks * walk_len)
     extern __shared__ __align__(16) unsigned long long walk_smem[];
     const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
     const long long u = (long long)blockIdx.x * WARPS_PER_CTA + wid;
@@ -81,8 +116,14 @@ walk_neighbourhoods_kernel(const long long *__restrict__ row_ptr, const int *__r
     }
     __syncwarp();
 
-    // ---- (1) sort the arrivals; (2) run-length encode in place -----------------------------------
-    warp_bitonic_sort(s, slots, lane);
+    // ---- (1) sort the arrivals (in registers); (2) run-length encode in place ----------------------
+    unsigned long long v[R];
+#pragma unroll
+    for (int r = 0; r < R; ++r) v[r] = s[r * 32 + lane];
+    warp_sort_regs<R>(v, slots, lane);
+#pragma unroll
+    for (int r = 0; r < R; ++r) s[r * 32 + lane] = v[r];
+    __syncwarp();
     int ns = 0;
     for (int base = 0; base < slots; base += 32)
         ns += __popc(__ballot_sync(0xffffffffu, s[base + lane] != EMPTY));
@@ -119,9 +160,13 @@ walk_neighbourhoods_kernel(const long long *__restrict__ row_ptr, const int *__r
     // ---- (3) rank: ascending (~count, id) = count descending, id ascending (B4) -------------------
     int n2 = 32;
     while (n2 < nv) n2 <<= 1;
-    for (int i = nv + lane; i < n2; i += 32) s[i] = EMPTY;
+#pragma unroll
+    for (int r = 0; r < R; ++r) v[r] = (r * 32 + lane < nv) ? s[r * 32 + lane] : EMPTY;
+    warp_sort_regs<R>(v, n2, lane);          // only the stages the nv distinct keys need
     __syncwarp();
-    warp_bitonic_sort(s, n2, lane);
+#pragma unroll
+    for (int r = 0; r < R; ++r) s[r * 32 + lane] = v[r];
+    __syncwarp();
 
     // ---- (4) the top T, padded with (u, 0) ------------------------------------------------------------
     for (int t = lane; t < T; t += 32) {
@@ -156,14 +201,27 @@ cudaError_t launch_walk_neighbourhoods(int64_t N, const int64_t *row_ptr, const 
     const long long blocks = (N + WARPS_PER_CTA - 1) / WARPS_PER_CTA;
     if (blocks > 0x7fffffffLL) return cudaErrorInvalidConfiguration;
     const size_t smem = (size_t)WARPS_PER_CTA * slots * sizeof(unsigned long long);
-    if (smem > 48 * 1024) {
-        cudaError_t e = cudaFuncSetAttribute(walk_neighbourhoods_kernel,
-                                             cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-        if (e != cudaSuccess) return e;
+    auto go = [&](auto kern) -> cudaError_t {
+        if (smem > 48 * 1024) {
+            cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+            if (e != cudaSuccess) return e;
+        }
+        kern<<<(unsigned)blocks, WARPS_PER_CTA * 32, smem, s>>>(
+            reinterpret_cast<const long long *>(row_ptr), col_idx, N, n_walks, walk_len, T,
+            (unsigned long long)seed, nbr_idx, counts);
+        return cudaSuccess;
+    };
+    cudaError_t e = cudaErrorNotSupported;
+    switch (slots / 32) {
+    case 1: e = go(walk_neighbourhoods_kernel<1>); break;
+    case 2: e = go(walk_neighbourhoods_kernel<2>); break;
+    case 4: e = go(walk_neighbourhoods_kernel<4>); break;
+    case 8: e = go(walk_neighbourhoods_kernel<8>); break;
+    case 16: e = go(walk_neighbourhoods_kernel<16>); break;
+    case 32: e = go(walk_neighbourhoods_kernel<32>); break;
+    case 64: e = go(walk_neighbourhoods_kernel<64>); break;
     }
-    walk_neighbourhoods_kernel<<<(unsigned)blocks, WARPS_PER_CTA * 32, smem, s>>>(
-        reinterpret_cast<const long long *>(row_ptr), col_idx, N, n_walks, walk_len, T,
-        (unsigned long long)seed, slots, nbr_idx, counts);
+    if (e != cudaSuccess) return e;
     if (launches) ++*launches;
     return cudaGetLastError();
 }
