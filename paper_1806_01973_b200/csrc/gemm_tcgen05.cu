@@ -241,6 +241,24 @@ __device__ __forceinline__ void tc_ld32(uint32_t taddr, uint32_t (&v)[32])
         : "r"(taddr)
         : "memory");
 }
+// write 32 consecutive fp32 columns of this thread's TMEM lane back (the epilogue parks z = act(acc +
+// bias) there between the norm pass and the store pass)
+__device__ __forceinline__ void tc_st32(uint32_t taddr, const uint32_t (&v)[32])
+{
+    asm volatile(
+        "tcgen05.st.sync.aligned.32x32b.x32.b32 [%0], "
+        "{%1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15, %16, "
+        "%17, %18, %19, %20, %21, %22, %23, %24, %25, %26, %27, %28, %29, %30, %31, %32};" ::"r"(taddr),
+        "r"(v[0]), "r"(v[1]), "r"(v[2]), "r"(v[3]), "r"(v[4]), "r"(v[5]), "r"(v[6]), "r"(v[7]), "r"(v[8]),
+        "r"(v[9]), "r"(v[10]), "r"(v[11]), "r"(v[12]), "r"(v[13]), "r"(v[14]), "r"(v[15]), "r"(v[16]),
+        "r"(v[17]), "r"(v[18]), "r"(v[19]), "r"(v[20]), "r"(v[21]), "r"(v[22]), "r"(v[23]), "r"(v[24]),
+        "r"(v[25]), "r"(v[26]), "r"(v[27]), "r"(v[28]), "r"(v[29]), "r"(v[30]), "r"(v[31])
+        : "memory");
+}
+__device__ __forceinline__ void tc_wait_st()
+{
+    asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory");
+}
 __device__ __forceinline__ void tc_wait_ld()
 {
     asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
@@ -520,19 +538,30 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap tmA1, const __grid_constant__
             if (p.l2norm) {
                 // pass 1: sum of squares of this row's z = act(acc + addend + bias) over my columns
                 const int par = (int)(it & 1);
-                float ss = 0.f;
+                float2 ss2 = make_float2(0.f, 0.f);       // sums of squares of the even / odd columns
                 for (int c0 = c_lo; c0 < c_hi; c0 += 32) {
                     uint32_t v[32];
                     tc_ld32(t0 + c0, v);
                     tc_wait_ld();
                     if (p.addend != nullptr) add_addend32(arow, c0, c_hi, v);   // uniform branch
+                    // packed fp32x2 adds / fmas (sm_100): half the issue slots of the scalar forms; z is
+                    // parked back in TMEM so that the store pass only scales and rounds
 #pragma unroll
-                    for (int i = 0; i < 32; ++i) {
-                        float z = __uint_as_float(v[i]) + sbias[c0 + i];
-                        z = p.relu ? fmaxf(z, 0.f) : z;
-                        ss = (c0 + i < c_hi) ? fmaf(z, z, ss) : ss;
+                    for (int i = 0; i < 32; i += 2) {
+                        const float2 b2 = *reinterpret_cast<const float2 *>(sbias + c0 + i);
+                        float2 z2 = __fadd2_rn(make_float2(__uint_as_float(v[i]), __uint_as_float(v[i + 1])), b2);
+                        if (p.relu) {
+                            z2.x = fmaxf(z2.x, 0.f);
+                            z2.y = fmaxf(z2.y, 0.f);
+                        }
+                        if (c0 + i < c_hi) ss2 = __ffma2_rn(z2, z2, ss2);   // N % 8 == 0: pairs never straddle
+                        v[i] = __float_as_uint(z2.x);
+                        v[i + 1] = __float_as_uint(z2.y);
                     }
+                    tc_st32(t0 + c0, v);
                 }
+                tc_wait_st();
+                float ss = ss2.x + ss2.y;
                 if (p.epi_halves == 2) {
                     // the two warps of this row quarter add their halves (fixed order: low + high)
                     hbuf[(par * 2 + eh) * BM + row] = ss;
@@ -565,24 +594,37 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap tmA1, const __grid_constant__
                 tc_ld32(t0 + c0, v[0]);
                 tc_ld32(t0 + c0 + 32, v[1]);
                 tc_wait_ld();
-                if (p.addend != nullptr) {                        // uniform branch
-                    add_addend32(arow, c0, c_hi, v[0]);
-                    add_addend32(arow, c0 + 32, c_hi, v[1]);
-                }
                 uint32_t pk[32];
+                if (p.l2norm) {                                   // TMEM already holds z: scale and round
+                    const float2 sc2 = make_float2(scale, scale);
 #pragma unroll
-                for (int h = 0; h < 2; ++h) {
+                    for (int h = 0; h < 2; ++h)
 #pragma unroll
-                    for (int i = 0; i < 32; i += 2) {
-                        float z0 = __uint_as_float(v[h][i]) + sbias[c0 + 32 * h + i];
-                        float z1 = __uint_as_float(v[h][i + 1]) + sbias[c0 + 32 * h + i + 1];
-                        if (p.relu) {
-                            z0 = fmaxf(z0, 0.f);
-                            z1 = fmaxf(z1, 0.f);
+                        for (int i = 0; i < 32; i += 2) {
+                            const float2 z2 = __fmul2_rn(
+                                make_float2(__uint_as_float(v[h][i]), __uint_as_float(v[h][i + 1])), sc2);
+                            __nv_bfloat162 b = __floats2bfloat162_rn(z2.x, z2.y);
+                            pk[16 * h + i / 2] = *reinterpret_cast<uint32_t *>(&b);
                         }
-                        __nv_bfloat162 b = __floats2bfloat162_rn(z0 * scale, z1 * scale);
-                        pk[16 * h + i / 2] = *reinterpret_cast<uint32_t *>(&b);
+                } else {
+                    if (p.addend != nullptr) {                    // uniform branch
+                        add_addend32(arow, c0, c_hi, v[0]);
+                        add_addend32(arow, c0 + 32, c_hi, v[1]);
                     }
+#pragma unroll
+                    for (int h = 0; h < 2; ++h)
+#pragma unroll
+                        for (int i = 0; i < 32; i += 2) {
+                            const float2 b2 = *reinterpret_cast<const float2 *>(sbias + c0 + 32 * h + i);
+                            float2 z2 = __fadd2_rn(
+                                make_float2(__uint_as_float(v[h][i]), __uint_as_float(v[h][i + 1])), b2);
+                            if (p.relu) {
+                                z2.x = fmaxf(z2.x, 0.f);
+                                z2.y = fmaxf(z2.y, 0.f);
+                            }
+                            __nv_bfloat162 b = __floats2bfloat162_rn(z2.x, z2.y);
+                            pk[16 * h + i / 2] = *reinterpret_cast<uint32_t *>(&b);
+                        }
                 }
                 if (lane == 0) tma_store_wait_read<1>();          // the buffer used two stores ago is free
                 __syncwarp();
