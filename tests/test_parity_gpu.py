@@ -135,7 +135,7 @@ def test_pool_large_ids_and_64bit_offsets(ctx):
 @pytest.mark.parametrize("n_dst,n_src,T,m", [
     (1, 1, 1, 8), (257, 300, 3, 8), (1000, 1000, 10, 64), (3001, 2000, 50, 256),
     (515, 4000, 100, 256), (300, 900, 50, 512), (130, 500, 20, 1024), (77, 300, 7, 2048),
-    (999, 999, 33, 24), (640, 640, 50, 192), (200, 200, 5, 320),
+    (999, 999, 33, 24), (640, 640, 50, 192), (200, 200, 5, 320), (50, 3000, 1024, 64),
 ])
 def test_pool_matches_oracle(ctx, dtype, n_dst, n_src, T, m):
     if dtype == torch.float32 and m > 1024:
