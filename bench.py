@@ -332,7 +332,9 @@ def run_ours(args, cfg):
         for ln in open(tp).read().splitlines()[1:]:
             f = ln.split(",")
             if f and f[0] == cfg.name and int(f[1]) == (args.chunk_nodes or 0):
-                traffic = float(f[2])
+                # the capture is one full driver chunk: scale to the average launch of this run
+                per_node = float(f[2]) / float(f[3])
+                traffic = per_node * cfg.N * len(cfg.layer_dims()) * args.steps / max(pool_n, 1)
     kernels = {}
     for name, (kms, kn) in prof.items():
         kernels[name] = {"ms_per_step": kms / args.steps, "launches_per_step": kn / args.steps}
