@@ -150,7 +150,10 @@ pinsage_status pinsage_pool(pinsage_ctx *ctx, pinsage_dtype dtype, int64_t n_dst
 
 /* S3: out[v] = normalise(ReLU(W [H[v] ; n[v]] + w)), W:[d x (d_in+m)] read as two K-segments
  * (no concat is materialised).  H:[M x d_in], n:[M x m], out:[M x d], all dtype.
- * out == H is allowed iff d == d_in (in-place layer k >= 2).  PAPER.md:115-116. */
+ * out == H is allowed iff d == d_in (in-place layer k >= 2).  PAPER.md:115-116.
+ * H == NULL with d_in == 0 drops the self segment (W:[d x m]): a destination type without a
+ * representation of its own, as the boards of the paper's bipartite pin-board graph (:216-221);
+ * with pinsage_dense and pinsage_pool (n_dst != n_src) this composes the alternating layers. */
 pinsage_status pinsage_combine(pinsage_ctx *ctx, pinsage_dtype dtype, int64_t M, int32_t d_in,
                                int32_t m, int32_t d, const void *H, const void *n, const void *W,
                                const float *w, void *out);

@@ -217,13 +217,14 @@ class Context:
         return out
 
     def pinsage_combine(self, H, n, W, w, out=None):
-        M, d_in = H.shape
-        m = n.shape[1]
+        """H may be None: no self segment (W is then [d x m])."""
+        M, m = n.shape
+        d_in = 0 if H is None else H.shape[1]
         d = W.shape[0]
-        assert W.shape[1] == d_in + m and n.shape[0] == M
+        assert W.shape[1] == d_in + m and (H is None or H.shape[0] == M)
         if out is None:
-            out = torch.empty((M, d), dtype=H.dtype, device=H.device)
-        self._check(self.lib.pinsage_combine(self.handle, dtype_code(H.dtype), M, d_in, m, d,
+            out = torch.empty((M, d), dtype=n.dtype, device=n.device)
+        self._check(self.lib.pinsage_combine(self.handle, dtype_code(n.dtype), M, d_in, m, d,
                                              _ptr(H), _ptr(n), _ptr(W), _ptr(w), _ptr(out)))
         return out
 

@@ -722,17 +722,23 @@ pinsage_status pinsage_combine(pinsage_ctx *ctx, pinsage_dtype dtype, int64_t M,
     DeviceGuard guard(ctx->device);
     PS_TRY(check_dtype(ctx, dtype));
     if (M < 0) return fail(ctx, PINSAGE_ERR_INVALID_ARG, "M is negative");
-    PS_TRY(check_dim(ctx, "d_in", d_in));
+    // d_in == 0 with H == NULL: a destination without a representation of its own (a feature-less
+    // node type of a bipartite graph): z = ReLU(W n + w), W:[d x m]
+    const bool no_self = d_in == 0 && H == nullptr;
+    if (!no_self) {
+        PS_TRY(check_dim(ctx, "d_in", d_in));
+        PS_TRY(check_ptr(ctx, "H", H));
+    }
     PS_TRY(check_dim(ctx, "m", m));
     PS_TRY(check_dim(ctx, "d", d));
-    PS_TRY(check_ptr(ctx, "H", H));
     PS_TRY(check_ptr(ctx, "n", n));
     PS_TRY(check_ptr(ctx, "W", W));
     PS_TRY(check_ptr(ctx, "w", w));
     PS_TRY(check_ptr(ctx, "out", out));
     const DType dt = static_cast<DType>(dtype);
     const size_t es = elem_size(dt);
-    if (out == H) {
+    if (no_self) {
+    } else if (out == H) {
         if (d != d_in) return fail(ctx, PINSAGE_ERR_INVALID_ARG, "out == H requires d == d_in");
     } else if (overlaps(H, (size_t)M * d_in * es, out, (size_t)M * d * es)) {
         return fail(ctx, PINSAGE_ERR_INVALID_ARG, "out partially overlaps H");
@@ -740,8 +746,13 @@ pinsage_status pinsage_combine(pinsage_ctx *ctx, pinsage_dtype dtype, int64_t M,
     if (overlaps(n, (size_t)M * m * es, out, (size_t)M * d * es))
         return fail(ctx, PINSAGE_ERR_INVALID_ARG, "out overlaps n");
     GemmArgs g;
-    g.M = M; g.K1 = d_in; g.K2 = m; g.N = d; g.A1 = H; g.A2 = n; g.B = W; g.bias = w;
+    g.M = M; g.N = d; g.B = W; g.bias = w;
     g.relu = 1; g.l2norm = 1; g.out = out;
+    if (no_self) {
+        g.K1 = m; g.A1 = n;
+    } else {
+        g.K1 = d_in; g.K2 = m; g.A1 = H; g.A2 = n;
+    }
     PS_TRY(ensure_ws(ctx, gemm_scratch_bytes(ctx, dt, g)));
     return run_gemm(ctx, dt, g, ctx->ws, ctx->ws_bytes, ctx->stream);
 }

@@ -558,3 +558,44 @@ def test_linear_pool_schedule_matches_oracle(ctx, dtype, d0, m, d, N, T):
                 ctx.pinsage_set_option("pool_mode", 0)
             assert_rows_close(to_f64(got), ref, dtype, f"layer linear_pool={lin} gamma={gamma}",
                               tol=6e-3 if dtype == torch.bfloat16 else 2e-5)
+
+
+# ------------------------------------------------------------------ bipartite alternation (NEXT #1)
+@pytest.mark.parametrize("dtype", DTYPES)
+def test_bipartite_layers_compose_from_the_step_calls(ctx, dtype):
+    """The paper's production graph is bipartite (pins with features, feature-less boards) and its
+    layers alternate pins -> boards -> pins.  Reading A8: a board has no
+    representation of its own, so its layer drops the self segment.  Composed from pinsage_dense /
+    pinsage_pool (n_dst != n_src) / pinsage_combine (H = NULL), against the same composition of the
+    oracle's steps."""
+    n_pin, n_board, T, d0, m, d = 3000, 700, 20, 64, 128, 64
+    g = torch.Generator().manual_seed(90)
+
+    def rn(*shape, std=1.0):
+        return torch.randn(shape, generator=g) * std
+
+    X = rn(n_pin, d0).to(dtype)
+    Q1, q1 = rn(m, d0, std=d0 ** -0.5).to(dtype), rn(m, std=0.01)
+    W1, w1 = rn(d, m, std=m ** -0.5).to(dtype), rn(d, std=0.01)             # boards: no self segment
+    Q2, q2 = rn(m, d, std=d ** -0.5).to(dtype), rn(m, std=0.01)
+    W2, w2 = rn(d, d0 + m, std=(d0 + m) ** -0.5).to(dtype), rn(d, std=0.01)  # pins: self = features
+    idx_b = torch.randint(0, n_pin, (n_board, T), generator=g, dtype=torch.int32)    # board <- pins
+    idx_p = torch.randint(0, n_board, (n_pin, T), generator=g, dtype=torch.int32)    # pin <- boards
+    a_b = O.normalize_counts(torch.randint(1, 50, (n_board, T), generator=g, dtype=torch.int32).numpy())
+    a_p = O.normalize_counts(torch.randint(1, 50, (n_pin, T), generator=g, dtype=torch.int32).numpy())
+    D = lambda t: t.to(DEV)
+    # GPU
+    P1 = ctx.pinsage_dense(D(X), D(Q1), D(q1), True)
+    nb = ctx.pinsage_pool(P1, D(idx_b), D(torch.from_numpy(a_b)))
+    hb = ctx.pinsage_combine(None, nb, D(W1), D(w1))
+    P2 = ctx.pinsage_dense(hb, D(Q2), D(q2), True)
+    np_ = ctx.pinsage_pool(P2, D(idx_p), D(torch.from_numpy(a_p)))
+    hp = ctx.pinsage_combine(D(X), np_, D(W2), D(w2))
+    # oracle
+    f = to_f64
+    oP1 = O.dense(f(X), f(Q1), f(q1), True)
+    ohb = O.combine(np.zeros((n_board, 0)), O.pool(oP1, idx_b.numpy(), a_b), f(W1), f(w1))
+    oP2 = O.dense(ohb, f(Q2), f(q2), True)
+    ohp = O.combine(f(X), O.pool(oP2, idx_p.numpy(), a_p), f(W2), f(w2))
+    assert_rows_close(to_f64(hb), ohb, dtype, "board layer", tol=6e-3 if dtype == torch.bfloat16 else 2e-5)
+    assert_rows_close(to_f64(hp), ohp, dtype, "pin layer")
