@@ -384,3 +384,18 @@ def walk_neighbourhoods(row_ptr, col_idx, n_walks: int, walk_len: int, T: int, s
         ctypes.c_int32(T), ctypes.c_uint64(seed), idx.ctypes.data_as(_i32p),
         cnt.ctypes.data_as(_i32p))
     return idx, cnt
+
+
+def topk(Q, Z, k: int):
+    """Exact K-nearest-neighbour lookup in the embedding space (PAPER.md:225 sec. 3.5; :289 "top K
+    nearest neighbors ... from a sample of 5 million test pins", K = 500) -- the exact form of what the
+    paper serves approximately with LSH.  Reading C1: "nearest" = largest inner product
+    z_q . z_i, the score the training loss ranks by (Eq. 1, :172-176); ties go to the smaller id; the
+    query itself is not excluded.  Q [nq, d], Z [N, d] -> (idx [nq, k] int32, score [nq, k] float64),
+    each row ordered by (score descending, id ascending).  The matmul and the sort are numpy's."""
+    Q = np.asarray(Q, dtype=np.float64)
+    Z = np.asarray(Z, dtype=np.float64)
+    S = Q @ Z.T
+    ids = np.broadcast_to(np.arange(Z.shape[0]), S.shape)
+    order = np.lexsort((ids, -S), axis=1)[:, :k]           # primary key -S, secondary key id
+    return order.astype(np.int32), np.take_along_axis(S, order, axis=1)

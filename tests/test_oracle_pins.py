@@ -486,3 +486,29 @@ def test_walk_neighbourhoods_ranking_and_counter_based_rng():
     rp2, ci2 = _csr(adj + [[0]])
     np.testing.assert_array_equal(O.walk_neighbourhoods(rp2, ci2, 50, 3, 6, seed=5)[0][:N], top_i)
     assert not np.array_equal(O.walk_neighbourhoods(rp, ci, 50, 3, 6, seed=6)[1], top_c)
+
+
+# --------------------------------------------------------------------------- exact top-K lookup
+def test_topk_against_brute_force_and_special_cases():
+    """K nearest neighbours by inner product (reading C1), ties to the smaller id."""
+    rng = np.random.default_rng(80)
+    Z = rng.normal(size=(37, 6))
+    Q = rng.normal(size=(5, 6))
+    idx, sc = O.topk(Q, Z, 7)
+    for q in range(5):                                      # brute force, one pair at a time
+        pairs = sorted(((-sum(Q[q, j] * Z[i, j] for j in range(6)), i) for i in range(37)))[:7]
+        assert [p[1] for p in pairs] == list(idx[q])
+        np.testing.assert_allclose([-p[0] for p in pairs], sc[q], atol=1e-14)
+    # orthonormal candidates: the score of candidate i is the i-th coordinate of the query
+    E = np.eye(6)
+    q = np.array([[0.3, 0.9, -0.2, 0.9, 0.1, 0.5]])
+    idx, sc = O.topk(q, E, 4)
+    assert list(idx[0]) == [1, 3, 5, 0] and list(sc[0]) == [0.9, 0.9, 0.5, 0.3]   # tie 1 < 3
+    assert O.topk(Q, Z, 1)[0][:, 0].tolist() == (Q @ Z.T).argmax(axis=1).tolist()
+    # relabelling the candidates relabels the answer (no ties here)
+    perm = rng.permutation(37)
+    idx_p, sc_p = O.topk(Q, Z[perm], 7)
+    np.testing.assert_array_equal(perm[idx_p], O.topk(Q, Z, 7)[0])
+    # a unit-norm query among unit-norm candidates finds itself first
+    U = Z / np.linalg.norm(Z, axis=1, keepdims=True)
+    assert O.topk(U[[4, 9]], U, 3)[0][:, 0].tolist() == [4, 9]
