@@ -203,6 +203,16 @@ pinsage_status pinsage_embed_nodes(pinsage_ctx *ctx, pinsage_dtype dtype, int64_
                                    const pinsage_head_params *head, int64_t M, const int32_t *targets,
                                    void *out);
 
+/* Exact K-nearest-neighbour lookup in the embedding space (PAPER.md:225 sec. 3.5; :289: top K = 500
+ * neighbours of a query among 5 million candidates) -- the exact form of what the paper serves
+ * approximately with LSH.  "Nearest" = largest inner product z_q . z_i, the score the loss ranks by
+ * (Eq. 1); ties go to the smaller id; the query is not excluded.  Q:[nq x d], Z:[N x d] dtype (device);
+ * out_idx:[nq x k] int32, out_score:[nq x k] fp32 (device), each row ordered by (score descending, id
+ * ascending).  Scores are fp32 accumulations of the exact bf16 / fp32 products (tcgen05 GEMM in BF16
+ * mode), compared as IEEE values.  1 <= k <= min(N, 1024).  Asynchronous on the context's stream. */
+pinsage_status pinsage_topk(pinsage_ctx *ctx, pinsage_dtype dtype, int64_t nq, int64_t N, int32_t d,
+                            const void *Q, const void *Z, int32_t k, int32_t *out_idx, float *out_score);
+
 /* ---- helpers ------------------------------------------------------------------------------ */
 
 /* nbr_w[v,t] = (float)counts[v,t] / (float)(sum_t counts[v,t]) in IEEE binary32 (L1-normalised visit

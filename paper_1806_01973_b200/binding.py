@@ -26,7 +26,7 @@ SYMBOLS = [
     "pinsage_set_option", "pinsage_launch_count", "pinsage_profile_read", "pinsage_dense", "pinsage_pool",
     "pinsage_combine", "pinsage_layer", "pinsage_layer_workspace_bytes", "pinsage_head",
     "pinsage_embed_all", "pinsage_normalize_counts", "pinsage_validate_graph",
-    "pinsage_build_neighbourhoods", "pinsage_embed_nodes",
+    "pinsage_build_neighbourhoods", "pinsage_embed_nodes", "pinsage_topk",
 ]
 
 
@@ -101,6 +101,8 @@ def load_library() -> ctypes.CDLL:
                                         ctypes.POINTER(LayerParams), ctypes.POINTER(HeadParams),
                                         i64, vp, vp]
     lib.pinsage_embed_nodes.restype = ctypes.c_int
+    lib.pinsage_topk.argtypes = [vp, ctypes.c_int, i64, i64, i32, vp, vp, i32, vp, vp]
+    lib.pinsage_topk.restype = ctypes.c_int
     lib.pinsage_build_neighbourhoods.argtypes = [vp, i64, vp, vp, i32, i32, i32, ctypes.c_uint64, vp, vp]
     lib.pinsage_build_neighbourhoods.restype = ctypes.c_int
     lib.pinsage_validate_graph.argtypes = [vp, i64, i64, i32, vp, vp, ctypes.POINTER(i64)]
@@ -297,6 +299,17 @@ class Context:
             self.handle, dtype_code(feats.dtype), N, T, K, _ptr(feats), _ptr(nbr_idx), _ptr(nbr_w), arr,
             ctypes.byref(hs), M, _ptr(targets), _ptr(out)))
         return out
+
+    def pinsage_topk(self, Q, Z, k: int):
+        """(idx [nq, k] int32, score [nq, k] fp32): the k candidates of Z with the largest Q . Z."""
+        nq, d = Q.shape
+        N = Z.shape[0]
+        assert Z.shape[1] == d and Z.dtype == Q.dtype
+        idx = torch.empty((nq, k), dtype=torch.int32, device=Q.device)
+        score = torch.empty((nq, k), dtype=torch.float32, device=Q.device)
+        self._check(self.lib.pinsage_topk(self.handle, dtype_code(Q.dtype), nq, N, d, _ptr(Q), _ptr(Z),
+                                          int(k), _ptr(idx), _ptr(score)))
+        return idx, score
 
     def pinsage_build_neighbourhoods(self, row_ptr, col_idx, n_walks: int, walk_len: int, T: int,
                                      seed: int = 0):

@@ -1122,6 +1122,54 @@ pinsage_status pinsage_embed_nodes(pinsage_ctx *ctx, pinsage_dtype dtype, int64_
     return PINSAGE_OK;
 }
 
+pinsage_status pinsage_topk(pinsage_ctx *ctx, pinsage_dtype dtype, int64_t nq, int64_t N, int32_t d,
+                            const void *Q, const void *Z, int32_t k, int32_t *out_idx, float *out_score)
+{
+    if (!ctx) return PINSAGE_ERR_INVALID_ARG;
+    DeviceGuard guard(ctx->device);
+    PS_TRY(check_dtype(ctx, dtype));
+    if (nq < 1 || nq >= (1LL << 31)) return fail(ctx, PINSAGE_ERR_INVALID_ARG, "nq = %lld outside [1, 2^31)", (long long)nq);
+    if (N < 1 || N >= (1LL << 31)) return fail(ctx, PINSAGE_ERR_INVALID_ARG, "N = %lld outside [1, 2^31)", (long long)N);
+    if (k < 1 || k > N) return fail(ctx, PINSAGE_ERR_INVALID_ARG, "k = %d outside [1, N]", k);
+    if (k > 1024) return fail(ctx, PINSAGE_ERR_UNSUPPORTED_SHAPE, "k = %d exceeds 1024", k);
+    PS_TRY(check_dim(ctx, "d", d));
+    PS_TRY(check_ptr(ctx, "Q", Q));
+    PS_TRY(check_ptr(ctx, "Z", Z));
+    PS_TRY(check_ptr(ctx, "out_idx", out_idx));
+    PS_TRY(check_ptr(ctx, "out_score", out_score));
+    const DType dt = static_cast<DType>(dtype);
+    const size_t es = elem_size(dt);
+    // candidate block: as wide as keeps the fp32 score block within 1 GiB, a multiple of 256, <= 65536
+    int64_t NB = std::min<int64_t>(65536, std::max<int64_t>(256, ((int64_t)1 << 28) / nq / 256 * 256));
+    NB = std::min<int64_t>(NB, (N + 7) / 8 * 8);
+    const size_t score_bytes = align_up((size_t)nq * NB * 4, 256), key_bytes = align_up(topk_state_bytes(nq), 256);
+    GemmArgs probe;
+    probe.M = nq; probe.K1 = d; probe.N = (int32_t)NB; probe.out_f32 = 1;
+    const size_t scratch = gemm_scratch_bytes(ctx, dt, probe);
+    PS_TRY(ensure_ws(ctx, score_bytes + key_bytes + scratch));
+    char *ws = static_cast<char *>(ctx->ws);
+    float *scores = reinterpret_cast<float *>(ws);
+    void *keys = ws + score_bytes;
+    PS_CUDA(ctx, cudaMemsetAsync(keys, 0, topk_state_bytes(nq), ctx->stream));
+    for (int64_t c0 = 0; c0 < N; c0 += NB) {
+        const int64_t nb = std::min(NB, N - c0), nb_pad = (nb + 7) / 8 * 8;
+        GemmArgs g;                                   // scores[nq x nb_pad] = Q Z[c0 .. c0+nb)^T, fp32
+        g.M = nq; g.K1 = d; g.N = (int32_t)nb_pad; g.A1 = Q;
+        g.B = static_cast<const char *>(Z) + (size_t)c0 * d * es;
+        g.b_rows = nb;
+        g.out = scores;
+        g.out_f32 = 1;
+        PS_TRY(run_gemm(ctx, dt, g, ws + score_bytes + key_bytes, scratch, ctx->stream));
+        cudaError_t e = launch_topk_merge(scores, nq, nb_pad, (int32_t)nb, c0, k, keys, ctx->stream, &ctx->launches);
+        count_launches(ctx);
+        PS_CUDA(ctx, e);
+    }
+    cudaError_t e = launch_topk_finish(keys, nq, k, out_idx, out_score, ctx->stream, &ctx->launches);
+    count_launches(ctx);
+    PS_CUDA(ctx, e);
+    return PINSAGE_OK;
+}
+
 pinsage_status pinsage_normalize_counts(pinsage_ctx *ctx, int64_t N, int32_t T,
                                         const int32_t *counts, float *nbr_w)
 {

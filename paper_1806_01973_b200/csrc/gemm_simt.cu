@@ -59,7 +59,7 @@ template <typename T, typename TOut>
 __global__ void __launch_bounds__(256)
 gemm_simt_kernel(const T *__restrict__ A1, const T *__restrict__ A2, const T *__restrict__ B,
                  const T *__restrict__ addend, const float *__restrict__ bias, TOut *__restrict__ out,
-                 long long M, int K1, int K2, int N, int ldb, int relu)
+                 long long M, int K1, int K2, int N, int ldb, int relu, int Nb)
 {
     __shared__ float As[BK][BM + 4];
     __shared__ float Bs[BK][BN + 4];
@@ -79,7 +79,7 @@ gemm_simt_kernel(const T *__restrict__ A1, const T *__restrict__ A2, const T *__
         const int ka = seg2 ? k0 - K1 : k0;
         float2 a = make_float2(0.f, 0.f), b = make_float2(0.f, 0.f);
         if (row0 + lr < M) a = load2<T>(A + (size_t)(row0 + lr) * lda + ka + lk);
-        if (col0 + lr < N) b = load2<T>(B + (size_t)(col0 + lr) * ldb + k0 + lk);
+        if (col0 + lr < Nb) b = load2<T>(B + (size_t)(col0 + lr) * ldb + k0 + lk);   // Nb = rows of B that exist
         As[lk][lr] = a.x;
         As[lk + 1][lr] = a.y;
         Bs[lk][lr] = b.x;
@@ -143,16 +143,21 @@ cudaError_t run(const GemmArgs &a, float *ztmp, cudaStream_t s, int *launches)
     const T *B = static_cast<const T *>(a.B);
     const T *add = static_cast<const T *>(a.addend);
     const int ldb = a.ldb > 0 ? a.ldb : a.K1 + a.K2;
+    const int Nb = a.b_rows > 0 ? (int)a.b_rows : a.N;
     if (a.l2norm) {
         if (!ztmp) return cudaErrorInvalidValue;
         gemm_simt_kernel<T, float><<<grid, 256, 0, s>>>(A1, A2, B, add, a.bias, ztmp, a.M, a.K1, a.K2,
-                                                        a.N, ldb, a.relu);
+                                                        a.N, ldb, a.relu, Nb);
         const long long rb = (a.M + 7) / 8;
         rownorm_kernel<T><<<(unsigned)rb, 256, 0, s>>>(ztmp, static_cast<T *>(a.out), a.M, a.N);
         if (launches) *launches += 2;
+    } else if (a.out_f32) {
+        gemm_simt_kernel<T, float><<<grid, 256, 0, s>>>(A1, A2, B, add, a.bias, static_cast<float *>(a.out),
+                                                        a.M, a.K1, a.K2, a.N, ldb, a.relu, Nb);
+        if (launches) *launches += 1;
     } else {
         gemm_simt_kernel<T, T><<<grid, 256, 0, s>>>(A1, A2, B, add, a.bias, static_cast<T *>(a.out),
-                                                    a.M, a.K1, a.K2, a.N, ldb, a.relu);
+                                                    a.M, a.K1, a.K2, a.N, ldb, a.relu, Nb);
         if (launches) *launches += 1;
     }
     return cudaGetLastError();

@@ -65,6 +65,7 @@ struct TcParams {
     const float *bias;
     const uint4 *addend;   // optional [M x N] bf16 added to the accumulator (row stride N), or null
     int relu, l2norm;
+    int out_f32;           // store fp32 (32-column TMA boxes) instead of bf16 (64-column boxes)
     uint32_t idesc;
 };
 
@@ -626,6 +627,36 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap tmA1, const __grid_constant__
                             pk[16 * h + i / 2] = *reinterpret_cast<uint32_t *>(&b);
                         }
                 }
+                if (p.out_f32) {
+                    // fp32 result: each 32-column half is one 32 x 128-byte box of raw accumulator values
+                    // (after bias / ReLU), same XOR swizzle, one TMA store per half
+#pragma unroll
+                    for (int h = 0; h < 2; ++h) {
+                        if (c0 + 32 * h >= c_hi) break;
+                        uint32_t z[32];
+#pragma unroll
+                        for (int i = 0; i < 32; ++i) {
+                            float x = __uint_as_float(v[h][i]) + sbias[c0 + 32 * h + i];
+                            z[i] = __float_as_uint(p.relu ? fmaxf(x, 0.f) : x);
+                        }
+                        if (lane == 0) tma_store_wait_read<1>();
+                        __syncwarp();
+                        uint8_t *fbuf = stg + sbuf * STG_WARP_BYTES;
+                        uint8_t *frow = fbuf + lane * 128;
+#pragma unroll
+                        for (int q = 0; q < 8; ++q)
+                            *reinterpret_cast<uint4 *>(frow + ((q ^ (lane & 7)) << 4)) =
+                                make_uint4(z[4 * q], z[4 * q + 1], z[4 * q + 2], z[4 * q + 3]);
+                        fence_proxy_async();
+                        __syncwarp();
+                        if (lane == 0 && m0 + ew * 32 < p.M) {
+                            tma_store_2d(&tmOut, n0 + c0 + 32 * h, (int)(m0 + ew * 32), smem_u32(fbuf));
+                            tma_store_commit();
+                        }
+                        sbuf ^= 1;
+                    }
+                    continue;
+                }
                 if (lane == 0) tma_store_wait_read<1>();          // the buffer used two stores ago is free
                 __syncwarp();
                 uint8_t *buf = stg + sbuf * STG_WARP_BYTES;
@@ -695,15 +726,18 @@ EncodeTiledFn encode_fn()
 
 // Row-major bf16 matrix [rows x cols] (cols contiguous), box = box_rows x 64 columns, SWIZZLE_128B.
 // Out-of-bounds parts of a box read as zero and are not written.
-bool make_map(CUtensorMap *map, const void *ptr, long long rows, int cols, int box_rows, int ld = 0)
+bool make_map(CUtensorMap *map, const void *ptr, long long rows, int cols, int box_rows, int ld = 0,
+              bool f32 = false)
 {
     EncodeTiledFn fn = encode_fn();
     if (!fn) return false;
+    const int es = f32 ? 4 : 2;
     const cuuint64_t dims[2] = {(cuuint64_t)cols, (cuuint64_t)rows};
-    const cuuint64_t strides[1] = {(cuuint64_t)(ld > 0 ? ld : cols) * 2};
-    const cuuint32_t box[2] = {(cuuint32_t)BK, (cuuint32_t)box_rows};
+    const cuuint64_t strides[1] = {(cuuint64_t)(ld > 0 ? ld : cols) * es};
+    const cuuint32_t box[2] = {(cuuint32_t)(128 / es), (cuuint32_t)box_rows};   // 128-byte rows
     const cuuint32_t estr[2] = {1, 1};
-    return fn(map, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 2, const_cast<void *>(ptr), dims, strides, box,
+    return fn(map, f32 ? CU_TENSOR_MAP_DATA_TYPE_FLOAT32 : CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 2,
+              const_cast<void *>(ptr), dims, strides, box,
               estr, CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B,
               CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
 }
@@ -723,6 +757,7 @@ bool plan(const GemmArgs &a, int cg, int ns_pref, int epi_pref, TcParams &p, int
     if (a.N < 8 || a.N % 8) return no("N must be a multiple of 8");
     if (a.ldb % 8 || (a.ldb > 0 && a.ldb < a.K1 + a.K2)) return no("ldb must be a multiple of 8, >= K1 + K2");
     if (cg == 2 && (a.M <= BM || a.N % 16)) return no("CTA pairs need M > 128 and N % 16 == 0");
+    if (a.out_f32 && (a.l2norm || a.addend)) return no("fp32 output is for plain products only");
     p = TcParams{};
     p.cg = cg;
     p.M = a.M;
@@ -765,6 +800,7 @@ bool plan(const GemmArgs &a, int cg, int ns_pref, int epi_pref, TcParams &p, int
     smem_bytes = p.stages * p.stage_bytes + fixed;
     p.bias = a.bias;
     p.addend = static_cast<const uint4 *>(a.addend);
+    p.out_f32 = a.out_f32;
     p.relu = a.relu;
     p.l2norm = a.l2norm;
     // instruction descriptor, kind::f16: D fp32 (bit 4), A and B bf16 (bits 7, 10), both K-major,
@@ -866,8 +902,9 @@ cudaError_t launch_gemm_tc(const GemmArgs &a, const GemmTune &t, int num_sms, cu
     } else {
         tmA2 = tmA1;
     }
-    if (!make_map(&tmB, a.B, a.N, a.K1 + a.K2, p.CN / p.cg, a.ldb)) return cudaErrorInvalidValue;
-    if (!make_map(&tmOut, a.out, a.M, a.N, 32)) return cudaErrorInvalidValue;
+    if (!make_map(&tmB, a.B, a.b_rows > 0 ? a.b_rows : a.N, a.K1 + a.K2, p.CN / p.cg, a.ldb))
+        return cudaErrorInvalidValue;
+    if (!make_map(&tmOut, a.out, a.M, a.N, 32, 0, a.out_f32 != 0)) return cudaErrorInvalidValue;
     if (launches) ++*launches;
     if (p.cg == 2)
         return p.nchunks == 2 ? launch_cg<2, 2>(p, smem, num_sms, s, tmA1, tmA2, tmB, tmOut)

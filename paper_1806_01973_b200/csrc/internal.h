@@ -22,6 +22,7 @@ struct GemmArgs {
     const void *A1 = nullptr;
     const void *A2 = nullptr;
     const void *B = nullptr;
+    int64_t b_rows = 0;             // rows of B that exist (0 = N); rows b_rows .. N-1 read as zero
     int32_t ldb = 0;                // row stride of B in elements; 0 = K1 + K2 (B may be a column
                                     // block of a wider matrix, e.g. W1 / W2 inside W)
     const void *addend = nullptr;   // optional [M x N] (dtype, row stride N) added to the product in
@@ -30,6 +31,7 @@ struct GemmArgs {
     const float *bias = nullptr;
     int relu = 0;
     int l2norm = 0;
+    int out_f32 = 0;                // BF16 mode only: store the result as fp32 (the scores of the top-K lookup)
     void *out = nullptr;
 };
 
@@ -86,5 +88,12 @@ cudaError_t subset_gather_rows(const void *src, const int32_t *ids, const int32_
 cudaError_t subset_remap_tables(const int32_t *list, int64_t n, const int32_t *idx, const float *w,
                                 int32_t T, const int32_t *pos_prev, int32_t *idx_loc, float *w_loc,
                                 cudaStream_t s, int *launches);
+
+// ---- topk.cu: running top-k lists for the exact nearest-neighbour lookup ---------------------------
+size_t topk_state_bytes(int64_t nq);   // per-query running lists + buffers; zero it before the first block
+cudaError_t launch_topk_merge(const float *scores, int64_t nq, int64_t ld, int32_t nb, int64_t id0,
+                              int32_t k, void *state, cudaStream_t s, int *launches);
+cudaError_t launch_topk_finish(const void *state, int64_t nq, int32_t k, int32_t *idx, float *score,
+                               cudaStream_t s, int *launches);
 
 }  // namespace pinsage

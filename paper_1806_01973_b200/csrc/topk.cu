@@ -1,0 +1,192 @@
+// topk.cu -- exact K-nearest-neighbour lookup in the embedding space (PAPER.md:225 sec. 3.5; :289:
+// "top K nearest neighbors ... from a sample of 5 million test pins", K = 500): the exact form of
+// what the paper serves approximately with LSH + Weak-AND.  Reading C1: nearest = largest inner
+// product z_q . z_i (the score of Eq. 1), ties to the smaller id.
+//
+// The scores of a block of candidates come from the tcgen05 GEMM (fp32 output).  This file keeps, per
+// query, a running list of the k best (score, id) pairs as 64-bit keys
+//     key = orderable(score) << 32 | (0xFFFFFFFF - id)        (larger key = better)
+// and merges a block of scores into it: one CTA per query scans the block (coalesced), appends what
+// beats the current k-th key to a 1024-entry buffer, and only when the buffer could overflow
+// bitonic-sorts list + buffer (2048 keys) and keeps the top k.  The result is the exact top k under a
+// total order, so it does not depend on the order in which candidates were buffered.
+#include "internal.h"
+
+namespace pinsage {
+namespace {
+
+constexpr int TK_THREADS = 256;
+constexpr int TK_LIST = 1024;              // k <= TK_LIST
+constexpr int TK_TOTAL = 2 * TK_LIST;      // running list + candidate buffer
+
+__device__ __forceinline__ unsigned ord_f32(float x)       // order-preserving map fp32 -> uint32
+{
+    const unsigned u = __float_as_uint(x);
+    return (u & 0x80000000u) ? ~u : (u | 0x80000000u);
+}
+__device__ __forceinline__ float unord_f32(unsigned o)
+{
+    return __uint_as_float((o & 0x80000000u) ? (o & 0x7fffffffu) : ~o);
+}
+
+// descending bitonic sort of s[0 .. TK_TOTAL) by the whole CTA
+__device__ void cta_sort_desc(unsigned long long *s)
+{
+    for (int k = 2; k <= TK_TOTAL; k <<= 1)
+        for (int j = k >> 1; j > 0; j >>= 1) {
+            for (int i = threadIdx.x; i < TK_TOTAL; i += TK_THREADS) {
+                const int ixj = i ^ j;
+                if (ixj > i) {
+                    const unsigned long long a = s[i], b = s[ixj];
+                    const bool down = (i & k) == 0;
+                    if ((a < b) == down) {
+                        s[i] = b;
+                        s[ixj] = a;
+                    }
+                }
+            }
+            __syncthreads();
+        }
+}
+
+__device__ __forceinline__ unsigned long long make_key(float score, long long id)
+{
+    return ((unsigned long long)ord_f32(score) << 32) | (unsigned long long)(0xFFFFFFFFu - (unsigned)id);
+}
+
+// sort list + buffer, keep the best k, empty the buffer; returns the new k-th best key
+__device__ unsigned long long merge_buffer(unsigned long long *s, int *cnt, int k)
+{
+    __syncthreads();
+    cta_sort_desc(s);
+    for (int i = k + threadIdx.x; i < TK_TOTAL; i += TK_THREADS) s[i] = 0ull;
+    if (threadIdx.x == 0) *cnt = 0;
+    __syncthreads();
+    return s[k - 1];
+}
+
+// Per-query state in global memory: state[q] = TK_TOTAL keys (running list, sorted descending, in
+// [0, k); zeros up to TK_LIST; candidate buffer in [TK_LIST, TK_LIST + cnt[q])), cnt[q] buffered keys.
+// scores [nq x ld] fp32 (ld % 4 == 0, rows 16-byte aligned), columns [0, nb) valid = candidates id0 ...
+// One CTA per query scans its row, TK_BLOCK scores per iteration (four float4 per thread up front),
+// and appends what beats the current k-th key straight to the global buffer -- in steady state a
+// handful of keys per block of scores.  Only when the buffer could overflow (the first blocks of a
+// fresh list) does the CTA pull the state into shared memory, merge (bitonic sort of 2048 keys, keep
+// k) and continue there in 256-key steps.  No sort and no state traffic otherwise.
+constexpr int TK_BLOCK = 16 * TK_THREADS;
+__global__ void __launch_bounds__(TK_THREADS)
+topk_scan_kernel(const float *__restrict__ scores, long long ld, int nb, long long id0, int k,
+                 unsigned long long *__restrict__ state, int *__restrict__ cnts)
+{
+    __shared__ unsigned long long s[TK_TOTAL];
+    __shared__ int cnt, blk;
+    const long long q = blockIdx.x;
+    const float *row = scores + q * ld;
+    unsigned long long *st = state + q * TK_TOTAL;
+    int have = cnts[q];
+    unsigned long long tau = st[k - 1];                        // current k-th best (0 while not full)
+    if (threadIdx.x == 0) blk = 0;
+    __syncthreads();
+    for (int base = 0; base < nb; base += TK_BLOCK) {
+        float4 v[4];
+#pragma unroll
+        for (int i = 0; i < 4; ++i) {                          // columns base + (i*256 + t)*4 .. +3
+            const int j = base + (i * TK_THREADS + threadIdx.x) * 4;
+            v[i] = j < nb ? __ldcs(reinterpret_cast<const float4 *>(row + j))   // (ld is padded past nb)
+                          : make_float4(0.f, 0.f, 0.f, 0.f);
+        }
+        unsigned long long key[16];
+        int mine = 0;
+#pragma unroll
+        for (int i = 0; i < 4; ++i) {
+            const int j = base + (i * TK_THREADS + threadIdx.x) * 4;
+            const float x[4] = {v[i].x, v[i].y, v[i].z, v[i].w};
+#pragma unroll
+            for (int e = 0; e < 4; ++e) {
+                key[4 * i + e] = j + e < nb ? make_key(x[e], id0 + j + e) : 0ull;
+                mine += key[4 * i + e] > tau;
+            }
+        }
+        int at = 0;
+        if (mine) at = atomicAdd(&blk, mine);                  // my offset among this block's keepers
+        __syncthreads();
+        const int total = blk;
+        __syncthreads();
+        if (threadIdx.x == 0) blk = 0;
+        if (total == 0) continue;
+        if (have + total <= TK_LIST) {                         // fits: append to the global buffer
+            if (mine) {
+                at += TK_LIST + have;
+#pragma unroll
+                for (int e = 0; e < 16; ++e)
+                    if (key[e] > tau) st[at++] = key[e];
+            }
+            have += total;
+        } else {                                               // could overflow: merge in shared memory
+            __syncthreads();
+            for (int i = threadIdx.x; i < TK_TOTAL; i += TK_THREADS)
+                s[i] = (i < TK_LIST || i < TK_LIST + have) ? st[i] : 0ull;
+            if (threadIdx.x == 0) cnt = have;
+            __syncthreads();
+#pragma unroll 1
+            for (int e = 0; e < 16; ++e) {
+                if (cnt + TK_THREADS > TK_LIST) tau = merge_buffer(s, &cnt, k);
+                if (key[e] > tau) s[TK_LIST + atomicAdd(&cnt, 1)] = key[e];
+                __syncthreads();
+            }
+            tau = merge_buffer(s, &cnt, k);
+            for (int i = threadIdx.x; i < TK_LIST; i += TK_THREADS) st[i] = s[i];
+            have = 0;
+            __syncthreads();
+        }
+    }
+    if (threadIdx.x == 0) cnts[q] = have;
+}
+
+// final merge of list + buffer and decoding: idx / score [nq x k]
+__global__ void __launch_bounds__(TK_THREADS)
+topk_finish_kernel(const unsigned long long *__restrict__ state, const int *__restrict__ cnts, int k,
+                   int *__restrict__ idx, float *__restrict__ score)
+{
+    __shared__ unsigned long long s[TK_TOTAL];
+    const long long q = blockIdx.x;
+    const unsigned long long *st = state + q * TK_TOTAL;
+    const int have = cnts[q];
+    for (int i = threadIdx.x; i < TK_TOTAL; i += TK_THREADS)
+        s[i] = (i < TK_LIST || i < TK_LIST + have) ? st[i] : 0ull;
+    __syncthreads();
+    cta_sort_desc(s);
+    for (int i = threadIdx.x; i < k; i += TK_THREADS) {
+        const unsigned long long key = s[i];
+        idx[q * k + i] = key ? (int)(0xFFFFFFFFu - (unsigned)(key & 0xFFFFFFFFull)) : -1;
+        score[q * k + i] = key ? unord_f32((unsigned)(key >> 32)) : -INFINITY;
+    }
+}
+
+}  // namespace
+
+size_t topk_state_bytes(int64_t nq) { return (size_t)nq * TK_TOTAL * 8 + (size_t)nq * 4; }
+
+// state: topk_state_bytes(nq) zeroed bytes (keys, then the counters) before the first block of scores
+cudaError_t launch_topk_merge(const float *scores, int64_t nq, int64_t ld, int32_t nb, int64_t id0,
+                              int32_t k, void *state, cudaStream_t s, int *launches)
+{
+    if (k < 1 || k > TK_LIST) return cudaErrorNotSupported;
+    unsigned long long *keys = static_cast<unsigned long long *>(state);
+    int *cnts = reinterpret_cast<int *>(keys + (size_t)nq * TK_TOTAL);
+    topk_scan_kernel<<<(unsigned)nq, TK_THREADS, 0, s>>>(scores, ld, nb, id0, k, keys, cnts);
+    if (launches) ++*launches;
+    return cudaGetLastError();
+}
+
+cudaError_t launch_topk_finish(const void *state, int64_t nq, int32_t k, int32_t *idx, float *score,
+                               cudaStream_t s, int *launches)
+{
+    const unsigned long long *keys = static_cast<const unsigned long long *>(state);
+    const int *cnts = reinterpret_cast<const int *>(keys + (size_t)nq * TK_TOTAL);
+    topk_finish_kernel<<<(unsigned)nq, TK_THREADS, 0, s>>>(keys, cnts, k, idx, score);
+    if (launches) ++*launches;
+    return cudaGetLastError();
+}
+
+}  // namespace pinsage

@@ -1,0 +1,82 @@
+"""Parity of the exact top-K lookup (pinsage_topk) with the oracle.
+
+Index work is compared bit for bit where floating point cannot interfere: with small-integer
+embeddings every inner product is exact in fp32, so ids, order and tie-breaks must equal the oracle's.
+With Gaussian embeddings the GPU's fp32 accumulation can swap candidates whose fp64 scores differ by
+less than its rounding error: there the unique part is compared (everything clearly above the k-th
+score is present, nothing clearly below it is) and the returned scores must match."""
+import numpy as np
+import pytest
+import torch
+
+from oracle import oracle as O
+from paper_1806_01973_b200 import binding
+from tests.parity import to_f64
+
+pytestmark = pytest.mark.gpu
+DEV = "cuda:0"
+DTYPES = [torch.bfloat16, torch.float32]
+
+
+@pytest.fixture(scope="module")
+def ctx():
+    c = binding.Context(0)
+    yield c
+    c.close()
+
+
+@pytest.mark.parametrize("dtype", DTYPES)
+@pytest.mark.parametrize("nq,N,d,k", [(1, 1, 8, 1), (5, 37, 8, 7), (130, 5000, 64, 50), (300, 70001, 32, 500),
+                                      (7, 3000, 256, 1024), (257, 66000, 128, 10)])
+def test_topk_exact_on_integer_embeddings(ctx, dtype, nq, N, d, k):
+    """Entries in {-2..2}: products and sums are exact, ties are everywhere -> ids must be identical."""
+    k = min(k, N)
+    g = torch.Generator().manual_seed(nq + N)
+    Q = torch.randint(-2, 3, (nq, d), generator=g).to(dtype)
+    Z = torch.randint(-2, 3, (N, d), generator=g).to(dtype)
+    for cg in ([1, 0] if dtype == torch.bfloat16 else [0]):
+        ctx.pinsage_set_option("gemm_cg", cg)
+        try:
+            idx, score = ctx.pinsage_topk(Q.to(DEV), Z.to(DEV), k)
+        finally:
+            ctx.pinsage_set_option("gemm_cg", 0)
+        ref_idx, ref_score = O.topk(to_f64(Q), to_f64(Z), k)
+        np.testing.assert_array_equal(idx.cpu().numpy(), ref_idx)
+        np.testing.assert_array_equal(score.cpu().numpy().astype(np.float64), ref_score)
+
+
+@pytest.mark.parametrize("dtype", DTYPES)
+def test_topk_on_unit_embeddings(ctx, dtype):
+    """Row-normalised Gaussian embeddings (what the path produces), K = 500 as in the paper's evaluation."""
+    nq, N, d, k = 200, 100_003, 128, 500
+    g = torch.Generator().manual_seed(5)
+    Z = torch.randn((N, d), generator=g)
+    Z = (Z / Z.norm(dim=1, keepdim=True)).to(dtype)
+    Q = Z[torch.randint(0, N, (nq,), generator=g)].clone()
+    idx, score = ctx.pinsage_topk(Q.to(DEV), Z.to(DEV), k)
+    idx, score = idx.cpu().numpy(), score.cpu().numpy().astype(np.float64)
+    S = to_f64(Q) @ to_f64(Z).T
+    tol = 2e-6                                           # fp32 accumulation of d = 128 products of size <= 1
+    for q in range(nq):
+        np.testing.assert_allclose(score[q], S[q, idx[q]], atol=tol)         # returned scores are the scores
+        assert len(set(idx[q])) == k
+        assert np.all(np.diff(score[q]) <= 0)                                # descending
+        kth = np.sort(S[q])[-k]
+        assert np.all(S[q, idx[q]] >= kth - tol)                             # nothing clearly below the k-th
+        must = np.nonzero(S[q] > kth + tol)[0]
+        assert np.isin(must, idx[q]).all()                                   # everything clearly above it
+    ref_idx, _ = O.topk(to_f64(Q), to_f64(Z), k)
+    assert (idx[:, 0] == ref_idx[:, 0]).all()            # the query itself (score 1) comes first
+
+
+def test_topk_argument_errors(ctx):
+    Q = torch.zeros((4, 16), dtype=torch.bfloat16, device=DEV)
+    Z = torch.zeros((100, 16), dtype=torch.bfloat16, device=DEV)
+    for k, name in ((0, "INVALID_ARG"), (101, "INVALID_ARG")):
+        with pytest.raises(binding.PinsageError) as e:
+            ctx.pinsage_topk(Q, Z, k)
+        assert e.value.status_name == name
+    Zb = torch.zeros((5000, 16), dtype=torch.bfloat16, device=DEV)
+    with pytest.raises(binding.PinsageError) as e:
+        ctx.pinsage_topk(Q, Zb, 2000)
+    assert e.value.status_name == "UNSUPPORTED_SHAPE"
