@@ -95,7 +95,7 @@ const char *pinsage_version(void);
 
 /* Integer options:  "gemm_impl"      0 = tcgen05 (default for BF16), 1 = SIMT reference kernels
  *                   "gemm_cg"        tcgen05 tile owner: 0 = automatic (CTA pairs, cta_group::2, 256-row
- *                                    tiles when the GEMM is tensor-bound, K N / (K + N) >= 200, and
+ *                                    tiles when the GEMM is tensor-bound, K N / (K + N) >= 160, and
  *                                    M > 128, N % 16 == 0; default), 1 = single CTAs
  *                                    (128-row tiles) only, 2 = CTA pairs or PINSAGE_ERR_UNSUPPORTED_SHAPE
  *                   "gemm_ns"        slab width of GEMMs without a row norm: 0 / 256 (default) or 512

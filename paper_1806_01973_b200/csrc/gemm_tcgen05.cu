@@ -129,6 +129,15 @@ __device__ __forceinline__ void mbar_arrive_remote(uint32_t cluster_addr)
     asm volatile("mbarrier.arrive.release.cluster.shared::cluster.b64 _, [%0];" ::"r"(cluster_addr)
                  : "memory");
 }
+// The "accumulator drained" signal carries no memory data (the TMEM reads are ordered by
+// tcgen05.wait::ld + tcgen05.fence::before_thread_sync), so it needs no release fence: a
+// release.cluster arrive compiles to MEMBAR.ALL.GPU, which cost each epilogue warp of a CTA pair
+// ~1-2 us per tile and made short-K pair tiles epilogue-bound (measured, profiles/r01_gemm_cfg4.md).
+__device__ __forceinline__ void mbar_arrive_remote_relaxed(uint32_t cluster_addr)
+{
+    asm volatile("mbarrier.arrive.relaxed.cluster.shared::cluster.b64 _, [%0];" ::"r"(cluster_addr)
+                 : "memory");
+}
 __device__ __forceinline__ uint32_t cluster_ctarank()
 {
     uint32_t r;
@@ -676,7 +685,7 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap tmA1, const __grid_constant__
             tc_fence_before();
             __syncwarp();
             if (lane == 0) {
-                if (CG == 2) mbar_arrive_remote(tempty_leader + 8 * acc);
+                if (CG == 2) mbar_arrive_remote_relaxed(tempty_leader + 8 * acc);
                 else mbar_arrive(bar_tempty + 8 * acc);
             }
             if (++acc == p.nacc) {
@@ -815,10 +824,10 @@ bool plan_auto(const GemmArgs &a, const GemmTune &t, TcParams &p, int &smem_byte
 {
     const int ns = t.ns == 512 ? 512 : 256;
     // Pairs pay when the GEMM is tensor-bound (measured on B200: +12-14 % at config 3's shapes); on
-    // the HBM-bound shapes (arithmetic intensity K N / (K + N) below ~200 flop per byte moved, e.g.
+    // the HBM-bound shapes (arithmetic intensity K N / (K + N) below ~160 flop per byte moved, e.g.
     // 256 x 256) single-CTA tiles keep more independent tiles in flight and are 15-35 % faster.
     const long long Kt = a.K1 + a.K2;
-    const bool tensor_bound = Kt * a.N >= 200 * (Kt + a.N);
+    const bool tensor_bound = Kt * a.N >= 160 * (Kt + a.N);
     if ((t.cg == 2 || (t.cg == 0 && tensor_bound)) && plan(a, 2, ns, t.epi, p, smem_bytes, nullptr)) return true;
     if (t.cg == 2) {
         if (why) *why = "shape not supported by the CTA-pair kernel";
