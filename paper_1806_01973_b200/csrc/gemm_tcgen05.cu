@@ -124,6 +124,16 @@ __device__ __forceinline__ void st_cluster_f32(uint32_t cluster_addr, float v)
 {
     asm volatile("st.shared::cluster.f32 [%0], %1;" ::"r"(cluster_addr), "f"(v) : "memory");
 }
+// One fp32 to a peer CTA's shared memory, completing 4 bytes of the transaction count of a barrier in
+// that CTA: data and signal travel together, so the sender needs no release fence (a st.shared::cluster
+// followed by a release.cluster arrive costs a MEMBAR.ALL.GPU per thread and tile).
+__device__ __forceinline__ void st_async_f32(uint32_t cluster_addr, float v, uint32_t cluster_bar)
+{
+    asm volatile("st.async.weak.shared::cluster.mbarrier::complete_tx::bytes.b32 [%0], %1, [%2];" ::"r"(
+                     cluster_addr),
+                 "r"(__float_as_uint(v)), "r"(cluster_bar)
+                 : "memory");
+}
 __device__ __forceinline__ void mbar_arrive_remote(uint32_t cluster_addr)
 {
     asm volatile("mbarrier.arrive.release.cluster.shared::cluster.b64 _, [%0];" ::"r"(cluster_addr)
@@ -393,7 +403,7 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap tmA1, const __grid_constant__
         for (int a = 0; a < 2; ++a) {
             mbar_init(bar_tfull + 8 * a, 1);
             mbar_init(bar_tempty + 8 * a, 4 * CG * p.epi_halves);  // every epilogue warp of the unit
-            mbar_init(bar_xchg + 8 * a, 128 * (units_per_cluster > 1 ? units_per_cluster - 1 : 1));
+            mbar_init(bar_xchg + 8 * a, 1);                         // armed per tile with the expected bytes
         }
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
@@ -580,14 +590,17 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap tmA1, const __grid_constant__
                 }
                 if (units_per_cluster > 1) {
                     // push my slab's partial to the CTAs that hold the other slabs of the same rows
-                    // (low-half warps only), then wait for theirs (DSMEM + remote mbarrier)
+                    // (low-half warps only; st.async: DSMEM store + transaction count of the peer's
+                    // barrier in one operation), then wait for theirs
                     if (eh == 0) {
+                        // one thread arms this tile's phase: 128 rows x 4 bytes from each other slab
+                        if (ew == 0 && lane == 0)
+                            mbar_expect_tx(bar_xchg + 8 * par, (uint32_t)(BM * 4 * (units_per_cluster - 1)));
                         const uint32_t my_slot = sbase + xchg_off + ((par * MAX_CLUSTER + my_unit) * BM + row) * 4;
                         for (uint32_t u = 0; u < (uint32_t)units_per_cluster; ++u) {
                             if (u == my_unit) continue;
                             const uint32_t r = u * CG + half;
-                            st_cluster_f32(map_to_cta(my_slot, r), ss);
-                            mbar_arrive_remote(map_to_cta(bar_xchg + 8 * par, r));
+                            st_async_f32(map_to_cta(my_slot, r), ss, map_to_cta(bar_xchg + 8 * par, r));
                         }
                     }
                     mbar_wait_cluster(bar_xchg + 8 * par, (uint32_t)((it >> 1) & 1));
