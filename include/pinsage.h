@@ -99,7 +99,8 @@ const char *pinsage_version(void);
  *                                    M > 128, N % 16 == 0; default), 1 = single CTAs
  *                                    (128-row tiles) only, 2 = CTA pairs or PINSAGE_ERR_UNSUPPORTED_SHAPE
  *                   "gemm_ns"        slab width of GEMMs without a row norm: 0 / 256 (default) or 512
- *                   "gemm_epi"       epilogue warps: 0 = eight when shared memory allows (default), 1 = four
+ *                   "gemm_epi"       epilogue warps: 0 = eight for single-accumulator row-norm tiles (default),
+ *                                    1 = always four, 2 = eight wherever they fit (measured slower)
  *                   "check_indices"  1 = every pinsage_pool / layer / embed_all call validates
  *                                    nbr_idx first (synchronous), default 0
  *                   "overlap"        1 = pinsage_layer / embed_all overlap S2 of chunk c+1 with S3

@@ -606,7 +606,7 @@ pinsage_status pinsage_set_option(pinsage_ctx *ctx, const char *key, int64_t val
             return fail(ctx, PINSAGE_ERR_INVALID_ARG, "gemm_ns must be 0, 256 or 512");
         ctx->tune.ns = (int)value;
     } else if (!strcmp(key, "gemm_epi")) {
-        if (value != 0 && value != 1) return fail(ctx, PINSAGE_ERR_INVALID_ARG, "gemm_epi must be 0 or 1");
+        if (value < 0 || value > 2) return fail(ctx, PINSAGE_ERR_INVALID_ARG, "gemm_epi must be 0, 1 or 2");
         ctx->tune.epi = (int)value;
     } else if (!strcmp(key, "check_indices")) {
         ctx->check_indices = value != 0;

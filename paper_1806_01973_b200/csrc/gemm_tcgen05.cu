@@ -809,7 +809,7 @@ bool plan(const GemmArgs &a, int cg, int ns_pref, int epi_pref, TcParams &p, int
     // gain, and with double-buffered accumulators the epilogue is hidden anyway).  Used for row-norm
     // GEMMs with a single accumulator when at least three operand stages still fit.
     int fixed = 0;
-    for (p.epi_halves = (epi_pref == 1 || !a.l2norm || p.nacc == 2) ? 1 : 2; p.epi_halves >= 1; --p.epi_halves) {
+    for (p.epi_halves = (epi_pref == 2 && p.NS > 64) ? 2 : (epi_pref == 1 || !a.l2norm || p.nacc == 2) ? 1 : 2; p.epi_halves >= 1; --p.epi_halves) {
         p.stg_bytes = p.epi_halves * 4 * 2 * STG_WARP_BYTES;
         fixed = p.stg_bytes + BIAS_BYTES + BAR_BYTES + (p.epi_halves == 2 ? HALF_BYTES : 0) +
                 (units_per_cluster > 1 ? XCHG_BYTES : 0);
