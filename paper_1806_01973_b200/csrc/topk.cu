@@ -95,6 +95,9 @@ topk_scan_kernel(const float *__restrict__ scores, long long ld, int nb, long lo
             v[i] = j < nb ? __ldcs(reinterpret_cast<const float4 *>(row + j))   // (ld is padded past nb)
                           : make_float4(0.f, 0.f, 0.f, 0.f);
         }
+        // cheap float pre-filter (a score below the k-th best score can never enter); keys are built
+        // only for the few survivors -- an un-built key is 0 and loses every comparison
+        const float tau_f = tau ? unord_f32((unsigned)(tau >> 32)) : -INFINITY;
         unsigned long long key[16];
         int mine = 0;
 #pragma unroll
@@ -103,8 +106,11 @@ topk_scan_kernel(const float *__restrict__ scores, long long ld, int nb, long lo
             const float x[4] = {v[i].x, v[i].y, v[i].z, v[i].w};
 #pragma unroll
             for (int e = 0; e < 4; ++e) {
-                key[4 * i + e] = j + e < nb ? make_key(x[e], id0 + j + e) : 0ull;
-                mine += key[4 * i + e] > tau;
+                key[4 * i + e] = 0ull;
+                if (x[e] >= tau_f && j + e < nb) {
+                    key[4 * i + e] = make_key(x[e], id0 + j + e);
+                    mine += key[4 * i + e] > tau;
+                }
             }
         }
         int at = 0;
