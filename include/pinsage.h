@@ -33,6 +33,8 @@
  *   - nbr_w is used as given (weighted SUM).  The paper's weighted mean = rows that sum to 1,
  *     e.g. produced by pinsage_normalize_counts.
  *   - Identical inputs give bit-identical outputs run to run (no atomics, fixed summation order).
+ *   - A context is not thread-safe: calls on one context must be serialised by the caller; different
+ *     contexts (one per device or stream) may be used from different threads.
  */
 #ifndef PINSAGE_H_
 #define PINSAGE_H_

@@ -853,12 +853,17 @@ template <int CG, int NCH>
 cudaError_t launch_cg(const TcParams &p, int smem, int num_sms, cudaStream_t s, const CUtensorMap &tmA1,
                       const CUtensorMap &tmA2, const CUtensorMap &tmB, const CUtensorMap &tmOut)
 {
-    static bool attr_set = false;
-    if (!attr_set) {
+    // per-device function attribute and cluster-occupancy cache (a process may drive several devices)
+    static int attr_dev = -1;
+    static int cached_clusters[MAX_CLUSTER + 1] = {0};
+    int dev = 0;
+    cudaGetDevice(&dev);
+    if (attr_dev != dev) {
         cudaError_t e = cudaFuncSetAttribute(gemm_tc_kernel<CG, NCH>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                              SMEM_LIMIT);
         if (e != cudaSuccess) return e;
-        attr_set = true;
+        attr_dev = dev;
+        for (int &c : cached_clusters) c = 0;
     }
     cudaLaunchConfig_t cfg{};
     cfg.blockDim = dim3(NUM_THREADS);
@@ -873,7 +878,6 @@ cudaError_t launch_cg(const TcParams &p, int smem, int num_sms, cudaStream_t s, 
     cfg.numAttrs = 1;
 
     // co-resident clusters of this shape (cached: the query costs a driver call)
-    static int cached_clusters[MAX_CLUSTER + 1] = {0};
     int max_clusters = cached_clusters[p.cluster];
     if (max_clusters == 0) {
         cfg.gridDim = dim3((unsigned)(num_sms / p.cluster * p.cluster));
