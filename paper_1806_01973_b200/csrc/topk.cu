@@ -113,13 +113,13 @@ topk_scan_kernel(const float *__restrict__ scores, long long ld, int nb, long lo
                 }
             }
         }
+        if (!__syncthreads_or(mine)) continue;                 // steady state: nothing beats the k-th key
         int at = 0;
         if (mine) at = atomicAdd(&blk, mine);                  // my offset among this block's keepers
         __syncthreads();
         const int total = blk;
         __syncthreads();
         if (threadIdx.x == 0) blk = 0;
-        if (total == 0) continue;
         if (have + total <= TK_LIST) {                         // fits: append to the global buffer
             if (mine) {
                 at += TK_LIST + have;
