@@ -55,7 +55,7 @@ __device__ __forceinline__ unsigned long long make_key(float score, long long id
 }
 
 // sort list + buffer, keep the best k, empty the buffer; returns the new k-th best key
-__device__ unsigned long long merge_buffer(unsigned long long *s, int *cnt, int k)
+__device__ __noinline__ unsigned long long merge_buffer(unsigned long long *s, int *cnt, int k)
 {
     __syncthreads();
     cta_sort_desc(s);
@@ -134,8 +134,8 @@ topk_scan_kernel(const float *__restrict__ scores, long long ld, int nb, long lo
                 s[i] = (i < TK_LIST || i < TK_LIST + have) ? st[i] : 0ull;
             if (threadIdx.x == 0) cnt = have;
             __syncthreads();
-#pragma unroll 1
-            for (int e = 0; e < 16; ++e) {
+#pragma unroll                                             // (a rolled loop would index key[] dynamically
+            for (int e = 0; e < 16; ++e) {                      //  and push the whole array to local memory)
                 if (cnt + TK_THREADS > TK_LIST) tau = merge_buffer(s, &cnt, k);
                 if (key[e] > tau) s[TK_LIST + atomicAdd(&cnt, 1)] = key[e];
                 __syncthreads();
