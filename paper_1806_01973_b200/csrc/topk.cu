@@ -87,14 +87,22 @@ topk_scan_kernel(const float *__restrict__ scores, long long ld, int nb, long lo
     unsigned long long tau = st[k - 1];                        // current k-th best (0 while not full)
     if (threadIdx.x == 0) blk = 0;
     __syncthreads();
-    for (int base = 0; base < nb; base += TK_BLOCK) {
-        float4 v[4];
+    // software pipeline: the loads of block b+1 are in flight while block b is tested
+    auto load_block = [&](int base, float4 (&dst)[4]) {
 #pragma unroll
         for (int i = 0; i < 4; ++i) {                          // columns base + (i*256 + t)*4 .. +3
             const int j = base + (i * TK_THREADS + threadIdx.x) * 4;
-            v[i] = j < nb ? __ldcs(reinterpret_cast<const float4 *>(row + j))   // (ld is padded past nb)
-                          : make_float4(0.f, 0.f, 0.f, 0.f);
+            dst[i] = j < nb ? __ldcs(reinterpret_cast<const float4 *>(row + j))   // (ld is padded past nb)
+                            : make_float4(0.f, 0.f, 0.f, 0.f);
         }
+    };
+    float4 nxt[4];
+    load_block(0, nxt);
+    for (int base = 0; base < nb; base += TK_BLOCK) {
+        float4 v[4];
+#pragma unroll
+        for (int i = 0; i < 4; ++i) v[i] = nxt[i];
+        load_block(base + TK_BLOCK, nxt);                      // (past the end: zeros, no loads)
         // cheap float pre-filter (a score below the k-th best score can never enter); keys are built
         // only for the few survivors -- an un-built key is 0 and loses every comparison
         const float tau_f = tau ? unord_f32((unsigned)(tau >> 32)) : -INFINITY;
