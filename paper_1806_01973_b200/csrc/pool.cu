@@ -332,7 +332,7 @@ cudaError_t dispatch_pool(const void *P, const int *idx, const float *w, void *o
     if (chunks <= 16) return run_pool<BF16, 16, 1, 8, MODE>(P, idx, w, out, n_dst, T, chunks, s);
     if (chunks <= 32) return run_pool<BF16, 32, 1, 8, MODE>(P, idx, w, out, n_dst, T, chunks, s);
     if (chunks <= 64) return run_pool<BF16, 32, 2, 4, MODE>(P, idx, w, out, n_dst, T, chunks, s);
-    if (chunks <= 128) return run_pool<BF16, 32, 4, 2, MODE>(P, idx, w, out, n_dst, T, chunks, s);
+    if (chunks <= 128) return run_pool<BF16, 32, 4, 4, MODE>(P, idx, w, out, n_dst, T, chunks, s);
     if (chunks <= 256) return run_pool<BF16, 32, 8, 1, MODE>(P, idx, w, out, n_dst, T, chunks, s);
     return cudaErrorNotSupported;
 }
