@@ -140,12 +140,14 @@ __device__ __forceinline__ void mbar_arrive_remote(uint32_t cluster_addr)
                  : "memory");
 }
 // The "accumulator drained" signal carries no memory data (the TMEM reads are ordered by
-// tcgen05.wait::ld + tcgen05.fence::before_thread_sync), so it needs no release fence: a
+// tcgen05.wait::ld + tcgen05.fence::before_thread_sync), so it needs no cluster-scope release: a
 // release.cluster arrive compiles to MEMBAR.ALL.GPU, which cost each epilogue warp of a CTA pair
 // ~1-2 us per tile and made short-K pair tiles epilogue-bound (measured, profiles/r01_gemm_cfg4.md).
+// The default form (release at CTA scope, no GPU-wide membar) is enough and measures the same as
+// a fully relaxed arrive.
 __device__ __forceinline__ void mbar_arrive_remote_relaxed(uint32_t cluster_addr)
 {
-    asm volatile("mbarrier.arrive.relaxed.cluster.shared::cluster.b64 _, [%0];" ::"r"(cluster_addr)
+    asm volatile("mbarrier.arrive.shared::cluster.b64 _, [%0];" ::"r"(cluster_addr)
                  : "memory");
 }
 __device__ __forceinline__ uint32_t cluster_ctarank()
