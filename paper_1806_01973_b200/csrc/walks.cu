@@ -35,53 +35,53 @@ __device__ __forceinline__ unsigned long long mix64(unsigned long long z)
 // distance j < 32 are in another lane (one shuffle), at distance j >= 32 in another register of the same
 // lane (register indices are compile-time through the JR template).  No shared-memory traffic: the
 // shared-memory version of these sorts ran at 78 % of the shared pipe and bounded the kernel.
-template <int R, int JR>
-__device__ __forceinline__ void cmpex_regs(unsigned long long (&v)[R], int k, int lane)
+template <typename K, int R, int JR>
+__device__ __forceinline__ void cmpex_regs(K (&v)[R], int k, int lane)
 {
 #pragma unroll
     for (int r = 0; r < R; ++r) {
         const int rr = r ^ JR;
         if (rr > r) {
             const bool up = (((r << 5) | lane) & k) == 0;
-            const unsigned long long a = v[r], b = v[rr];
+            const K a = v[r], b = v[rr];
             const bool sw = (a > b) == up;
             v[r] = sw ? b : a;
             v[rr] = sw ? a : b;
         }
     }
 }
-template <int R>
-__device__ __forceinline__ void stage_regs(unsigned long long (&v)[R], int jr, int k, int lane)
+template <typename K, int R>
+__device__ __forceinline__ void stage_regs(K (&v)[R], int jr, int k, int lane)
 {
     switch (jr) {
-    case 1: if constexpr (R > 1) cmpex_regs<R, 1>(v, k, lane); break;
-    case 2: if constexpr (R > 2) cmpex_regs<R, 2>(v, k, lane); break;
-    case 4: if constexpr (R > 4) cmpex_regs<R, 4>(v, k, lane); break;
-    case 8: if constexpr (R > 8) cmpex_regs<R, 8>(v, k, lane); break;
-    case 16: if constexpr (R > 16) cmpex_regs<R, 16>(v, k, lane); break;
-    case 32: if constexpr (R > 32) cmpex_regs<R, 32>(v, k, lane); break;
+    case 1: if constexpr (R > 1) cmpex_regs<K, R, 1>(v, k, lane); break;
+    case 2: if constexpr (R > 2) cmpex_regs<K, R, 2>(v, k, lane); break;
+    case 4: if constexpr (R > 4) cmpex_regs<K, R, 4>(v, k, lane); break;
+    case 8: if constexpr (R > 8) cmpex_regs<K, R, 8>(v, k, lane); break;
+    case 16: if constexpr (R > 16) cmpex_regs<K, R, 16>(v, k, lane); break;
+    case 32: if constexpr (R > 32) cmpex_regs<K, R, 32>(v, k, lane); break;
     }
 }
-template <int R>
-__device__ __forceinline__ void stage_shfl(unsigned long long (&v)[R], int j, int k, int lane)
+template <typename K, int R>
+__device__ __forceinline__ void stage_shfl(K (&v)[R], int j, int k, int lane)
 {
     const bool lower = (lane & j) == 0;
 #pragma unroll
     for (int r = 0; r < R; ++r) {
         const bool up = (((r << 5) | lane) & k) == 0;
-        const unsigned long long a = v[r], b = __shfl_xor_sync(0xffffffffu, a, j);
+        const K a = v[r], b = __shfl_xor_sync(0xffffffffu, a, j);
         v[r] = (lower == up) ? (a < b ? a : b) : (a > b ? a : b);
     }
 }
 // ascending sort of the first n keys' worth of stages (n a power of two, 32 <= n <= 32 * R; keys at
 // index >= n must be EMPTY so that they stay in place)
-template <int R>
-__device__ __forceinline__ void warp_sort_regs(unsigned long long (&v)[R], int n, int lane)
+template <typename K, int R>
+__device__ __forceinline__ void warp_sort_regs(K (&v)[R], int n, int lane)
 {
     for (int k = 2; k <= n; k <<= 1)
         for (int j = k >> 1; j > 0; j >>= 1) {
-            if (j >= 32) stage_regs<R>(v, j >> 5, k, lane);
-            else stage_shfl<R>(v, j, k, lane);
+            if (j >= 32) stage_regs<K, R>(v, j >> 5, k, lane);
+            else stage_shfl<K, R>(v, j, k, lane);
         }
 }
 
@@ -117,13 +117,16 @@ walk_neighbourhoods_kernel(const long long *__restrict__ row_ptr, const int *__r
     __syncwarp();
 
     // ---- (1) sort the arrivals (in registers); (2) run-length encode in place ----------------------
-    unsigned long long v[R];
+    {   // ids fit 31 bits: the first sort runs on 32-bit keys (half the registers, shuffles and ALU work)
+        unsigned v1[R];
 #pragma unroll
-    for (int r = 0; r < R; ++r) v[r] = s[r * 32 + lane];
-    warp_sort_regs<R>(v, slots, lane);
+        for (int r = 0; r < R; ++r) v1[r] = (unsigned)s[r * 32 + lane];          // EMPTY -> 0xFFFFFFFF
+        warp_sort_regs<unsigned, R>(v1, slots, lane);
 #pragma unroll
-    for (int r = 0; r < R; ++r) s[r * 32 + lane] = v[r];
+        for (int r = 0; r < R; ++r) s[r * 32 + lane] = v1[r] == 0xFFFFFFFFu ? EMPTY : (unsigned long long)v1[r];
+    }
     __syncwarp();
+    unsigned long long v[R];
     int ns = 0;
     for (int base = 0; base < slots; base += 32)
         ns += __popc(__ballot_sync(0xffffffffu, s[base + lane] != EMPTY));
@@ -162,7 +165,7 @@ walk_neighbourhoods_kernel(const long long *__restrict__ row_ptr, const int *__r
     while (n2 < nv) n2 <<= 1;
 #pragma unroll
     for (int r = 0; r < R; ++r) v[r] = (r * 32 + lane < nv) ? s[r * 32 + lane] : EMPTY;
-    warp_sort_regs<R>(v, n2, lane);          // only the stages the nv distinct keys need
+    warp_sort_regs<unsigned long long, R>(v, n2, lane);   // only the stages the nv distinct keys need
     __syncwarp();
 #pragma unroll
     for (int r = 0; r < R; ++r) s[r * 32 + lane] = v[r];
