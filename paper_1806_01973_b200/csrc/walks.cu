@@ -10,9 +10,10 @@
 //
 // One warp per node.  Lane l simulates walks l, l+32, ... (a latency-bound pointer chase, hidden by
 // many resident warps) and drops every arrival into slot walk*walk_len + step of a shared-memory
-// array of 64-bit keys (empty = all ones).  The warp then (1) bitonic-sorts the keys in registers,
-// (2) run-length encodes them in place (shared memory) into keys (~count << 32 | id), (3) bitonic-sorts
-// those in registers -- ascending order is (count descending, id ascending) -- and (4) writes the first T.  Integer work only: bit-exact and
+// array of 64-bit keys (empty = all ones).  The warp then (1) bitonic-sorts the ids in registers (32-bit
+// keys), (2) run-length encodes them in place (shared memory) into (~count << 32 | id) entries ordered by
+// id, (3) bitonic-sorts 32-bit rank keys (2048 - count) << 11 | position in registers -- ascending order
+// is (count descending, id ascending) -- and (4) writes the first T.  Integer work only: bit-exact and
 // independent of scheduling.
 #include "internal.h"
 
@@ -126,7 +127,6 @@ walk_neighbourhoods_kernel(const long long *__restrict__ row_ptr, const int *__r
         for (int r = 0; r < R; ++r) s[r * 32 + lane] = v1[r] == 0xFFFFFFFFu ? EMPTY : (unsigned long long)v1[r];
     }
     __syncwarp();
-    unsigned long long v[R];
     int ns = 0;
     for (int base = 0; base < slots; base += 32)
         ns += __popc(__ballot_sync(0xffffffffu, s[base + lane] != EMPTY));
@@ -160,27 +160,40 @@ walk_neighbourhoods_kernel(const long long *__restrict__ row_ptr, const int *__r
         __syncwarp();
     }
 
-    // ---- (3) rank: ascending (~count, id) = count descending, id ascending (B4) -------------------
+    // ---- (3) rank (B4).  The run-length output s[0 .. nv) is ordered by id, so a 32-bit key
+    // (2048 - count) << 11 | position sorts ascending into (count descending, id ascending) --------
     int n2 = 32;
     while (n2 < nv) n2 <<= 1;
+    unsigned v2[R];
 #pragma unroll
-    for (int r = 0; r < R; ++r) v[r] = (r * 32 + lane < nv) ? s[r * 32 + lane] : EMPTY;
-    warp_sort_regs<unsigned long long, R>(v, n2, lane);   // only the stages the nv distinct keys need
-    __syncwarp();
-#pragma unroll
-    for (int r = 0; r < R; ++r) s[r * 32 + lane] = v[r];
-    __syncwarp();
-
-    // ---- (4) the top T, padded with (u, 0) ------------------------------------------------------------
-    for (int t = lane; t < T; t += 32) {
-        int id = (int)u, c = 0;
-        if (t < nv) {
-            const unsigned long long k = s[t];
-            id = (int)(unsigned)(k & 0xFFFFFFFFull);
-            c = (int)(0xFFFFFFFFu - (unsigned)(k >> 32));
+    for (int r = 0; r < R; ++r) {
+        const int i = r * 32 + lane;
+        v2[r] = 0xFFFFFFFFu;
+        if (i < nv) {
+            const unsigned count = 0xFFFFFFFFu - (unsigned)(s[i] >> 32);
+            v2[r] = ((2048u - count) << 11) | (unsigned)i;
         }
-        nbr_idx[u * T + t] = id;
-        counts[u * T + t] = c;
+    }
+    warp_sort_regs<unsigned, R>(v2, n2, lane);   // only the stages the nv distinct keys need
+
+    // ---- (4) the top T, padded with (u, 0): rank t sits in register t / 32 of lane t % 32 -------------
+#pragma unroll
+    for (int r = 0; r < R; ++r) {
+        const int t = r * 32 + lane;
+        if (t < T && t < slots) {
+            int id = (int)u, c = 0;
+            if (t < nv) {
+                const unsigned long long e = s[v2[r] & 0x7FFu];
+                id = (int)(unsigned)(e & 0xFFFFFFFFull);
+                c = (int)(0xFFFFFFFFu - (unsigned)(e >> 32));
+            }
+            nbr_idx[u * T + t] = id;
+            counts[u * T + t] = c;
+        }
+    }
+    for (int t = slots + lane; t < T; t += 32) {         // T beyond the slot count: padding only
+        nbr_idx[u * T + t] = (int)u;
+        counts[u * T + t] = 0;
     }
 }
 
