@@ -95,7 +95,15 @@ const char *pinsage_last_error(const pinsage_ctx *ctx);
 /* Static version string, e.g. "pinsage-b200 0.1.0 (sm_100a)". */
 const char *pinsage_version(void);
 
-/* Integer options:  "gemm_impl"      0 = tcgen05 (default for BF16), 1 = SIMT reference kernels
+/* Integer options:  "gemm_impl"      0 = tcgen05 (default), 1 = SIMT reference kernels
+ *                   "f32_split"      PINSAGE_F32 GEMMs on the tensor cores: both operands split into
+ *                                    three bf16 planes (x = x0 + x1 + x2 exactly), the six products with
+ *                                    i + j <= 2 summed by one tcgen05 GEMM over a six times longer K
+ *                                    (fp32 accumulate, error ~1e-6 relative; 5-7 x the SIMT kernel):
+ *                                    -1 = when M N K >= 2^28 and the shape is covered (default),
+ *                                    0 = never (SIMT fp32 FMA kernels), 1 = always, a GEMM the split
+ *                                    path does not cover (K % 4 != 0, the linear-pool addend) is then
+ *                                    PINSAGE_ERR_UNSUPPORTED_SHAPE.  Ignored when gemm_impl = 1.
  *                   "gemm_cg"        tcgen05 tile owner: 0 = automatic (CTA pairs, cta_group::2, 256-row
  *                                    tiles when the GEMM is tensor-bound, K N / (K + N) >= 160, and
  *                                    M > 128, N % 16 == 0; default), 1 = single CTAs

@@ -41,6 +41,9 @@ struct pinsage_ctx {
     void *stage = nullptr;           // device staging for host inputs / outputs
     size_t stage_bytes = 0;
     long long *d_first_bad = nullptr;
+    int f32_split = -1;              // fp32 GEMMs on the tensor cores by bf16 splitting: -1 automatic, 0 never, 1 always
+    void *split_buf = nullptr;       // bf16 planes of the operands of a split fp32 GEMM (grown on demand)
+    size_t split_bytes = 0;
     void *subA = nullptr, *subB = nullptr;   // scratch of pinsage_embed_nodes (sets / compact tensors)
     size_t subA_bytes = 0, subB_bytes = 0;
     // optional per-kernel timing ("profile" option): event pairs around every launch
@@ -232,6 +235,72 @@ void count_launches(pinsage_ctx *ctx)
     ctx->launches = 0;
 }
 
+// The fp32 GEMM on the tensor cores (split_f32.cu): both operands as K-concatenated bf16 planes in a
+// context-owned buffer, A in row blocks so that the buffer stays bounded, one tcgen05 GEMM with fp32
+// output per block.  *done = false when the shape is outside what the split path covers (the caller
+// falls back to the SIMT kernel).
+constexpr size_t SPLIT_A_BYTES = 256u << 20;    // planes of one row block of A
+
+pinsage_status run_gemm_split(pinsage_ctx *ctx, const GemmArgs &a, cudaStream_t s, bool *done)
+{
+    *done = false;
+    const int kt = a.K1 + a.K2;
+    const int ldb = a.ldb ? a.ldb : kt;
+    if (a.addend || a.K1 % 4 || a.K2 % 4 || ldb % 4 || !aligned16(a.A1) || !aligned16(a.B) ||
+        (a.K2 && !aligned16(a.A2)) || (long long)kt * 6 > 0x7fffffffLL || s != ctx->stream)
+        return PINSAGE_OK;
+    const int64_t b_rows = a.b_rows ? a.b_rows : a.N;
+    const size_t row_bytes = (size_t)kt * 6 * 2;
+    int64_t blk = (int64_t)(SPLIT_A_BYTES / row_bytes) / 256 * 256;
+    blk = std::min<int64_t>(std::max<int64_t>(blk, 256), a.M);
+    GemmArgs g;
+    g.M = blk;
+    g.K1 = kt * 6;
+    g.N = a.N;
+    g.b_rows = b_rows;
+    g.bias = a.bias;
+    g.relu = a.relu;
+    g.l2norm = a.l2norm;
+    g.out_f32 = 1;
+    g.A1 = g.B = g.out = reinterpret_cast<void *>(16);          // (shape check only)
+    GemmArgs tail = g;
+    tail.M = a.M % blk ? a.M % blk : blk;
+    if (!gemm_tc_supported(g, ctx->tune, nullptr) || !gemm_tc_supported(tail, ctx->tune, nullptr))
+        return PINSAGE_OK;
+    const size_t b_bytes = align_up((size_t)b_rows * row_bytes, 256);
+    const size_t need = b_bytes + (size_t)blk * row_bytes;
+    if (need > ctx->split_bytes) {
+        PS_CUDA(ctx, cudaStreamSynchronize(s));
+        if (ctx->split_buf) cudaFree(ctx->split_buf);
+        ctx->split_buf = nullptr;
+        ctx->split_bytes = 0;
+        PS_CUDA(ctx, cudaMalloc(&ctx->split_buf, need));
+        ctx->split_bytes = need;
+    }
+    char *Bp = static_cast<char *>(ctx->split_buf), *Ap = Bp + b_bytes;
+    const int kind = a.l2norm ? PROF_COMBINE : PROF_DENSE;
+    const int e0 = prof_mark(ctx, s);
+    cudaError_t e = launch_split3(true, static_cast<const float *>(a.B), kt, ldb, nullptr, 0, 0, b_rows, Bp, s,
+                                  &ctx->launches);
+    for (int64_t r0 = 0; r0 < a.M && e == cudaSuccess; r0 += blk) {
+        const int64_t rows = std::min<int64_t>(blk, a.M - r0);
+        e = launch_split3(false, static_cast<const float *>(a.A1) + r0 * a.K1, a.K1, a.K1,
+                          a.K2 ? static_cast<const float *>(a.A2) + r0 * a.K2 : nullptr, a.K2, a.K2, rows, Ap, s,
+                          &ctx->launches);
+        if (e != cudaSuccess) break;
+        g.M = rows;
+        g.A1 = Ap;
+        g.B = Bp;
+        g.out = static_cast<float *>(a.out) + r0 * a.N;
+        e = launch_gemm_tc(g, ctx->tune, ctx->num_sms, s, &ctx->launches);
+    }
+    prof_close(ctx, kind, e0, s);
+    count_launches(ctx);
+    PS_CUDA(ctx, e);
+    *done = true;
+    return PINSAGE_OK;
+}
+
 // One GEMM of the path on stream s. scratch: fp32 [M x N] for the SIMT norm pass / tcgen05 partials.
 pinsage_status run_gemm(pinsage_ctx *ctx, DType dt, const GemmArgs &a, void *scratch,
                         size_t scratch_bytes, cudaStream_t s)
@@ -239,6 +308,16 @@ pinsage_status run_gemm(pinsage_ctx *ctx, DType dt, const GemmArgs &a, void *scr
     if (a.M == 0) return PINSAGE_OK;
     const bool simt = dt == DType::F32 || ctx->gemm_impl == 1;
     const int kind = a.l2norm ? PROF_COMBINE : PROF_DENSE;
+    if (dt == DType::F32 && ctx->gemm_impl == 0 &&
+        (ctx->f32_split == 1 || (ctx->f32_split == -1 && (double)a.M * a.N * (a.K1 + a.K2) >= (double)(1 << 28)))) {
+        bool done = false;
+        PS_TRY(run_gemm_split(ctx, a, s, &done));
+        if (done) return PINSAGE_OK;
+        if (ctx->f32_split == 1)
+            return fail(ctx, PINSAGE_ERR_UNSUPPORTED_SHAPE,
+                        "f32_split = 1: shape outside the split fp32 GEMM (M=%lld K1=%d K2=%d N=%d)",
+                        (long long)a.M, a.K1, a.K2, a.N);
+    }
     if (simt) {
         const size_t need = gemm_simt_scratch_bytes(a);
         if (need > scratch_bytes)
@@ -583,6 +662,7 @@ void pinsage_destroy(pinsage_ctx *ctx)
     if (ctx->ws) cudaFree(ctx->ws);
     if (ctx->stage) cudaFree(ctx->stage);
     if (ctx->d_first_bad) cudaFree(ctx->d_first_bad);
+    if (ctx->split_buf) cudaFree(ctx->split_buf);
     if (ctx->subA) cudaFree(ctx->subA);
     if (ctx->subB) cudaFree(ctx->subB);
     for (cudaEvent_t e : ctx->prof_events) cudaEventDestroy(e);
@@ -622,6 +702,9 @@ pinsage_status pinsage_set_option(pinsage_ctx *ctx, const char *key, int64_t val
         if (value != -1 && value != 0 && value != 32 && value != 64 && value != 128)
             return fail(ctx, PINSAGE_ERR_INVALID_ARG, "pool_slab must be -1, 0, 32, 64 or 128");
         ctx->pool_slab = (int)value;
+    } else if (!strcmp(key, "f32_split")) {
+        if (value < -1 || value > 1) return fail(ctx, PINSAGE_ERR_INVALID_ARG, "f32_split must be -1, 0 or 1");
+        ctx->f32_split = (int)value;
     } else if (!strcmp(key, "profile")) {
         ctx->profile = value != 0;
     } else {

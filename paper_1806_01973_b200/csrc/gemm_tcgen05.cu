@@ -660,8 +660,14 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap tmA1, const __grid_constant__
                         uint32_t z[32];
 #pragma unroll
                         for (int i = 0; i < 32; ++i) {
-                            float x = __uint_as_float(v[h][i]) + sbias[c0 + 32 * h + i];
-                            z[i] = __float_as_uint(p.relu ? fmaxf(x, 0.f) : x);
+                            float x = __uint_as_float(v[h][i]);
+                            if (p.l2norm) {                       // TMEM already holds z
+                                x *= scale;
+                            } else {
+                                x += sbias[c0 + 32 * h + i];
+                                x = p.relu ? fmaxf(x, 0.f) : x;
+                            }
+                            z[i] = __float_as_uint(x);
                         }
                         if (lane == 0) tma_store_wait_read<1>();
                         __syncwarp();
@@ -781,7 +787,7 @@ bool plan(const GemmArgs &a, int cg, int ns_pref, int epi_pref, TcParams &p, int
     if (a.N < 8 || a.N % 8) return no("N must be a multiple of 8");
     if (a.ldb % 8 || (a.ldb > 0 && a.ldb < a.K1 + a.K2)) return no("ldb must be a multiple of 8, >= K1 + K2");
     if (cg == 2 && (a.M <= BM || a.N % 16)) return no("CTA pairs need M > 128 and N % 16 == 0");
-    if (a.out_f32 && (a.l2norm || a.addend)) return no("fp32 output is for plain products only");
+    if (a.out_f32 && a.addend) return no("fp32 output takes no addend");
     p = TcParams{};
     p.cg = cg;
     p.M = a.M;

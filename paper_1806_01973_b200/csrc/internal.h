@@ -31,7 +31,7 @@ struct GemmArgs {
     const float *bias = nullptr;
     int relu = 0;
     int l2norm = 0;
-    int out_f32 = 0;                // BF16 mode only: store the result as fp32 (the scores of the top-K lookup)
+    int out_f32 = 0;                // tcgen05 kernel only: store the result as fp32 (top-K scores; split fp32 mode)
     void *out = nullptr;
 };
 
@@ -53,6 +53,12 @@ struct GemmTune {
 bool gemm_tc_supported(const GemmArgs &a, const GemmTune &t, const char **why);
 cudaError_t launch_gemm_tc(const GemmArgs &a, const GemmTune &t, int num_sms, cudaStream_t s, int *launches);
 size_t gemm_tc_scratch_bytes(const GemmArgs &a);
+
+// ---- split_f32.cu: fp32 operands as K-concatenated bf16 planes (fp32 mode on the tensor cores) ----
+// out [rows x 6 (K1 + K2)] bf16 from [S1 | S2] (fp32, row strides ld1 / ld2; all multiples of 4).
+// is_b selects the plane order of the B operand, so that A' . B'^T sums the six leading terms.
+cudaError_t launch_split3(bool is_b, const float *S1, int32_t K1, int64_t ld1, const float *S2, int32_t K2,
+                          int64_t ld2, int64_t rows, void *out, cudaStream_t s, int *launches);
 
 // ---- pool.cu ------------------------------------------------------------------------------------
 // slab_bytes: 0 = whole rows (one pass); 32 / 64 / 128 = column-slab passes that keep the gathered

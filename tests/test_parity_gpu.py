@@ -36,7 +36,8 @@ def _graph(N, T, seed, n_src=None):
 
 def _both_impls(ctx, dtype):
     """(gemm_impl, gemm_cg): bf16 runs through the tcgen05 kernel with single-CTA tiles, with CTA
-    pairs (cta_group::2) and through the SIMT reference kernels; fp32 is SIMT only."""
+    pairs (cta_group::2) and through the SIMT reference kernels; fp32 takes the automatic choice here
+    (SIMT at these sizes; the split tensor-core path has its own file, test_f32_split_gpu.py)."""
     return [(0, 1), (0, 2), (1, 0)] if dtype == torch.bfloat16 else [(0, 0)]
 
 
