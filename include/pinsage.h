@@ -129,6 +129,10 @@ const char *pinsage_version(void);
  *                                    128-byte slabs when P exceeds L2 but n_src x 128 bytes fits in
  *                                    0.7 of it, so that the gathered sub-table stays L2-resident),
  *                                    0 = always whole rows, 32 / 64 / 128 = forced.  Bit-identical results.
+ *                   "topk_fused"     pinsage_topk: 1 (default) = once every running list is full, scores
+ *                                    are tested against the query's k-th score in the GEMM's epilogue and
+ *                                    only the keepers leave the SM (no fp32 score matrix in HBM); 0 = every
+ *                                    block of scores is stored and scanned by a second kernel.  Same result.
  *                   "profile"        1 = bracket every kernel launch of the path with CUDA events
  *                                    on its stream, see pinsage_profile_read (default 0)
  * Unknown key -> PINSAGE_ERR_INVALID_ARG. */
@@ -220,7 +224,10 @@ pinsage_status pinsage_embed_nodes(pinsage_ctx *ctx, pinsage_dtype dtype, int64_
  * (Eq. 1); ties go to the smaller id; the query is not excluded.  Q:[nq x d], Z:[N x d] dtype (device);
  * out_idx:[nq x k] int32, out_score:[nq x k] fp32 (device), each row ordered by (score descending, id
  * ascending).  Scores are fp32 accumulations of the exact bf16 / fp32 products (tcgen05 GEMM in BF16
- * mode), compared as IEEE values.  1 <= k <= min(N, 1024).  Asynchronous on the context's stream. */
+ * mode; the split tcgen05 GEMM or the SIMT kernel in F32 mode, option "f32_split"), compared as IEEE
+ * values.  1 <= k <= min(N, 1024).  With N beyond one candidate block (up to 65 536) and option
+ * "topk_fused" on, the call synchronises the context's stream once before it returns (it reads back
+ * which blocks, if any, overflowed a candidate buffer and must be redone); otherwise asynchronous. */
 pinsage_status pinsage_topk(pinsage_ctx *ctx, pinsage_dtype dtype, int64_t nq, int64_t N, int32_t d,
                             const void *Q, const void *Z, int32_t k, int32_t *out_idx, float *out_score);
 

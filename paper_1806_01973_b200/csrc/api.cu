@@ -41,6 +41,7 @@ struct pinsage_ctx {
     void *stage = nullptr;           // device staging for host inputs / outputs
     size_t stage_bytes = 0;
     long long *d_first_bad = nullptr;
+    int topk_fused = 1;              // pinsage_topk: select in the GEMM epilogue (1) or in a second pass over stored scores (0)
     int f32_split = -1;              // fp32 GEMMs on the tensor cores by bf16 splitting: -1 automatic, 0 never, 1 always
     void *split_buf = nullptr;       // bf16 planes of the operands of a split fp32 GEMM (grown on demand)
     size_t split_bytes = 0;
@@ -241,32 +242,54 @@ void count_launches(pinsage_ctx *ctx)
 // falls back to the SIMT kernel).
 constexpr size_t SPLIT_A_BYTES = 256u << 20;    // planes of one row block of A
 
-pinsage_status run_gemm_split(pinsage_ctx *ctx, const GemmArgs &a, cudaStream_t s, bool *done)
+// Whether the split path takes this GEMM; fills the bf16 GEMM of one row block (pointers unset).
+bool split_covers(const pinsage_ctx *ctx, const GemmArgs &a, cudaStream_t s, GemmArgs &g, int64_t &blk)
 {
-    *done = false;
     const int kt = a.K1 + a.K2;
     const int ldb = a.ldb ? a.ldb : kt;
     if (a.addend || a.K1 % 4 || a.K2 % 4 || ldb % 4 || !aligned16(a.A1) || !aligned16(a.B) ||
         (a.K2 && !aligned16(a.A2)) || (long long)kt * 6 > 0x7fffffffLL || s != ctx->stream)
-        return PINSAGE_OK;
-    const int64_t b_rows = a.b_rows ? a.b_rows : a.N;
+        return false;
     const size_t row_bytes = (size_t)kt * 6 * 2;
-    int64_t blk = (int64_t)(SPLIT_A_BYTES / row_bytes) / 256 * 256;
+    blk = (int64_t)(SPLIT_A_BYTES / row_bytes) / 256 * 256;
     blk = std::min<int64_t>(std::max<int64_t>(blk, 256), a.M);
-    GemmArgs g;
+    if (a.sel_state && blk < a.M) return false;                 // (the selection epilogue numbers rows from 0)
+    g = GemmArgs{};
     g.M = blk;
     g.K1 = kt * 6;
     g.N = a.N;
-    g.b_rows = b_rows;
+    g.b_rows = a.b_rows ? a.b_rows : a.N;
     g.bias = a.bias;
     g.relu = a.relu;
     g.l2norm = a.l2norm;
     g.out_f32 = 1;
+    g.sel_state = a.sel_state;
+    g.sel_cnt = a.sel_cnt;
+    g.sel_k = a.sel_k;
+    g.sel_id0 = a.sel_id0;
     g.A1 = g.B = g.out = reinterpret_cast<void *>(16);          // (shape check only)
     GemmArgs tail = g;
     tail.M = a.M % blk ? a.M % blk : blk;
-    if (!gemm_tc_supported(g, ctx->tune, nullptr) || !gemm_tc_supported(tail, ctx->tune, nullptr))
-        return PINSAGE_OK;
+    return gemm_tc_supported(g, ctx->tune, nullptr) && gemm_tc_supported(tail, ctx->tune, nullptr);
+}
+
+bool split_wanted(const pinsage_ctx *ctx, DType dt, const GemmArgs &a)
+{
+    return dt == DType::F32 && ctx->gemm_impl == 0 &&
+           (ctx->f32_split == 1 ||
+            (ctx->f32_split == -1 && (double)a.M * a.N * (a.K1 + a.K2) >= (double)(1 << 28)));
+}
+
+pinsage_status run_gemm_split(pinsage_ctx *ctx, const GemmArgs &a, cudaStream_t s, bool *done)
+{
+    *done = false;
+    GemmArgs g;
+    int64_t blk = 0;
+    if (!split_covers(ctx, a, s, g, blk)) return PINSAGE_OK;
+    const int kt = a.K1 + a.K2;
+    const int ldb = a.ldb ? a.ldb : kt;
+    const int64_t b_rows = g.b_rows;
+    const size_t row_bytes = (size_t)kt * 6 * 2;
     const size_t b_bytes = align_up((size_t)b_rows * row_bytes, 256);
     const size_t need = b_bytes + (size_t)blk * row_bytes;
     if (need > ctx->split_bytes) {
@@ -308,8 +331,7 @@ pinsage_status run_gemm(pinsage_ctx *ctx, DType dt, const GemmArgs &a, void *scr
     if (a.M == 0) return PINSAGE_OK;
     const bool simt = dt == DType::F32 || ctx->gemm_impl == 1;
     const int kind = a.l2norm ? PROF_COMBINE : PROF_DENSE;
-    if (dt == DType::F32 && ctx->gemm_impl == 0 &&
-        (ctx->f32_split == 1 || (ctx->f32_split == -1 && (double)a.M * a.N * (a.K1 + a.K2) >= (double)(1 << 28)))) {
+    if (split_wanted(ctx, dt, a)) {
         bool done = false;
         PS_TRY(run_gemm_split(ctx, a, s, &done));
         if (done) return PINSAGE_OK;
@@ -319,6 +341,7 @@ pinsage_status run_gemm(pinsage_ctx *ctx, DType dt, const GemmArgs &a, void *scr
                         (long long)a.M, a.K1, a.K2, a.N);
     }
     if (simt) {
+        if (a.sel_state) return fail(ctx, PINSAGE_ERR_CUDA, "internal: selection epilogue on the SIMT path");
         const size_t need = gemm_simt_scratch_bytes(a);
         if (need > scratch_bytes)
             return fail(ctx, PINSAGE_ERR_OOM, "internal: SIMT scratch %zu > %zu", need, scratch_bytes);
@@ -702,6 +725,8 @@ pinsage_status pinsage_set_option(pinsage_ctx *ctx, const char *key, int64_t val
         if (value != -1 && value != 0 && value != 32 && value != 64 && value != 128)
             return fail(ctx, PINSAGE_ERR_INVALID_ARG, "pool_slab must be -1, 0, 32, 64 or 128");
         ctx->pool_slab = (int)value;
+    } else if (!strcmp(key, "topk_fused")) {
+        ctx->topk_fused = value != 0;
     } else if (!strcmp(key, "f32_split")) {
         if (value < -1 || value > 1) return fail(ctx, PINSAGE_ERR_INVALID_ARG, "f32_split must be -1, 0 or 1");
         ctx->f32_split = (int)value;
@@ -1224,28 +1249,103 @@ pinsage_status pinsage_topk(pinsage_ctx *ctx, pinsage_dtype dtype, int64_t nq, i
     const size_t es = elem_size(dt);
     // candidate block: as wide as keeps the fp32 score block within 1 GiB, a multiple of 256, <= 65536
     int64_t NB = std::min<int64_t>(65536, std::max<int64_t>(256, ((int64_t)1 << 28) / nq / 256 * 256));
+    // (whole waves: a CTA pair owns one 256-candidate slab for all queries, num_sms / 2 pairs run at a time)
+    const int64_t wave = (int64_t)(ctx->num_sms / 2) * 256;
+    if (NB >= wave) NB = NB / wave * wave;
     NB = std::min<int64_t>(NB, (N + 7) / 8 * 8);
+    const int64_t n_blocks = (N + NB - 1) / NB;
     const size_t score_bytes = align_up((size_t)nq * NB * 4, 256), key_bytes = align_up(topk_state_bytes(nq), 256);
+    const size_t prev_bytes = align_up((size_t)nq * 4, 256), any_bytes = align_up((size_t)n_blocks * 4, 256);
+    const size_t ovf_bytes = align_up((size_t)n_blocks * nq, 256);
     GemmArgs probe;
     probe.M = nq; probe.K1 = d; probe.N = (int32_t)NB; probe.out_f32 = 1;
+    probe.A1 = Q; probe.B = Z;
     const size_t scratch = gemm_scratch_bytes(ctx, dt, probe);
-    PS_TRY(ensure_ws(ctx, score_bytes + key_bytes + scratch));
+    PS_TRY(ensure_ws(ctx, score_bytes + key_bytes + prev_bytes + any_bytes + ovf_bytes + scratch));
     char *ws = static_cast<char *>(ctx->ws);
     float *scores = reinterpret_cast<float *>(ws);
     void *keys = ws + score_bytes;
+    int *cnts = reinterpret_cast<int *>(static_cast<unsigned long long *>(keys) + (size_t)nq * TK_TOTAL);
+    int *cnt_prev = reinterpret_cast<int *>(ws + score_bytes + key_bytes);
+    int *any = reinterpret_cast<int *>(ws + score_bytes + key_bytes + prev_bytes);
+    unsigned char *ovf = reinterpret_cast<unsigned char *>(ws + score_bytes + key_bytes + prev_bytes + any_bytes);
+    char *gscratch = ws + score_bytes + key_bytes + prev_bytes + any_bytes + ovf_bytes;
+    // Selection in the GEMM epilogue (no score round trip through HBM) once every list is full and its
+    // k-th score is a useful threshold: after the first block (two for k > 512; a block then adds about
+    // k / blocks-seen keys per query to a 1024-key buffer).  A buffer that overflows anyway is detected
+    // on the device and that (block, query) is redone from stored scores after the pass.
+    probe.sel_state = static_cast<unsigned long long *>(keys);
+    probe.sel_cnt = cnts;
+    probe.sel_k = k;
+    bool fused = ctx->topk_fused && ctx->gemm_impl == 0;
+    if (fused && dt == DType::BF16) fused = gemm_tc_supported(probe, ctx->tune, nullptr);
+    if (fused && dt == DType::F32) {
+        GemmArgs g6;
+        int64_t blk = 0;
+        fused = split_wanted(ctx, dt, probe) && split_covers(ctx, probe, ctx->stream, g6, blk);
+    }
+    const int64_t warm = k <= TK_LIST / 2 ? 1 : 2;
     PS_CUDA(ctx, cudaMemsetAsync(keys, 0, topk_state_bytes(nq), ctx->stream));
-    for (int64_t c0 = 0; c0 < N; c0 += NB) {
-        const int64_t nb = std::min(NB, N - c0), nb_pad = (nb + 7) / 8 * 8;
+    PS_CUDA(ctx, cudaMemsetAsync(any, 0, (size_t)n_blocks * 4, ctx->stream));
+    auto block_args = [&](int64_t b, int64_t &nb, int64_t &nb_pad) {
+        const int64_t c0 = b * NB;
+        nb = std::min(NB, N - c0);
+        nb_pad = (nb + 7) / 8 * 8;
         GemmArgs g;                                   // scores[nq x nb_pad] = Q Z[c0 .. c0+nb)^T, fp32
         g.M = nq; g.K1 = d; g.N = (int32_t)nb_pad; g.A1 = Q;
         g.B = static_cast<const char *>(Z) + (size_t)c0 * d * es;
         g.b_rows = nb;
         g.out = scores;
         g.out_f32 = 1;
-        PS_TRY(run_gemm(ctx, dt, g, ws + score_bytes + key_bytes, scratch, ctx->stream));
-        cudaError_t e = launch_topk_merge(scores, nq, nb_pad, (int32_t)nb, c0, k, keys, ctx->stream, &ctx->launches);
+        return g;
+    };
+    for (int64_t b = 0; b < n_blocks; ++b) {
+        int64_t nb = 0, nb_pad = 0;
+        GemmArgs g = block_args(b, nb, nb_pad);
+        cudaError_t e;
+        bool fb = fused && b >= warm;
+        if (fb) {
+            g.sel_state = static_cast<unsigned long long *>(keys);
+            g.sel_cnt = cnts;
+            g.sel_k = k;
+            g.sel_id0 = b * NB;
+            GemmArgs g6;
+            int64_t blk = 0;
+            fb = dt == DType::BF16 ? gemm_tc_supported(g, ctx->tune, nullptr)      // (a ragged last block)
+                                   : split_wanted(ctx, dt, g) && split_covers(ctx, g, ctx->stream, g6, blk);
+            if (!fb) g.sel_state = nullptr;
+        }
+        if (fb) {
+            PS_TRY(run_gemm(ctx, dt, g, gscratch, scratch, ctx->stream));
+            e = launch_topk_maintain(keys, nq, k, 3 * TK_LIST / 8, cnt_prev, ovf + (size_t)b * nq, any + b,
+                                     ctx->stream, &ctx->launches);
+        } else {
+            PS_TRY(run_gemm(ctx, dt, g, gscratch, scratch, ctx->stream));
+            e = launch_topk_merge(scores, nq, nb_pad, (int32_t)nb, b * NB, k, keys, nullptr, ctx->stream,
+                                  &ctx->launches);
+            // before a block that selects in the epilogue: merge every buffer, so that the k-th key is
+            // that of everything seen so far (the scan leaves it as of its last in-kernel merge)
+            if (e == cudaSuccess && fused && b + 1 >= warm && b + 1 < n_blocks)
+                e = launch_topk_maintain(keys, nq, k, 0, cnt_prev, ovf + (size_t)b * nq, any + b, ctx->stream,
+                                         &ctx->launches);
+        }
         count_launches(ctx);
         PS_CUDA(ctx, e);
+    }
+    if (fused && n_blocks > warm) {                   // redo what overflowed (normally nothing)
+        std::vector<int> any_h((size_t)n_blocks);
+        PS_CUDA(ctx, cudaMemcpyAsync(any_h.data(), any, (size_t)n_blocks * 4, cudaMemcpyDeviceToHost, ctx->stream));
+        PS_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
+        for (int64_t b = warm; b < n_blocks; ++b) {
+            if (!any_h[(size_t)b]) continue;
+            int64_t nb = 0, nb_pad = 0;
+            GemmArgs g = block_args(b, nb, nb_pad);
+            PS_TRY(run_gemm(ctx, dt, g, gscratch, scratch, ctx->stream));
+            cudaError_t e = launch_topk_merge(scores, nq, nb_pad, (int32_t)nb, b * NB, k, keys,
+                                              ovf + (size_t)b * nq, ctx->stream, &ctx->launches);
+            count_launches(ctx);
+            PS_CUDA(ctx, e);
+        }
     }
     cudaError_t e = launch_topk_finish(keys, nq, k, out_idx, out_score, ctx->stream, &ctx->launches);
     count_launches(ctx);

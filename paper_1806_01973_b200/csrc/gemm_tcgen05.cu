@@ -66,6 +66,12 @@ struct TcParams {
     const uint4 *addend;   // optional [M x N] bf16 added to the accumulator (row stride N), or null
     int relu, l2norm;
     int out_f32;           // store fp32 (32-column TMA boxes) instead of bf16 (64-column boxes)
+    // top-K selection epilogue (internal.h): no output matrix; scores that beat row q's k-th key are
+    // appended to q's candidate buffer.  sel_nb = valid columns (candidates sel_id0 + column).
+    unsigned long long *sel_state;
+    int *sel_cnt;
+    int sel_k, sel_nb;
+    long long sel_id0;
     uint32_t idesc;
 };
 
@@ -346,6 +352,7 @@ __device__ __forceinline__ uint64_t make_desc(uint32_t saddr)
 //   + 256 B                   mbarriers, TMEM base address
 //   + 2 KB                    row sum-of-squares exchange between the two column halves [2][2][128] fp32
 //   + 8 KB (cluster > 1)      row-norm exchange [2][MAX_CLUSTER][128] fp32
+constexpr int SEL_Q = 8;                 // selection epilogue: queue slots per row and warp (2 KB per warp)
 constexpr int BIAS_BYTES = 512 * 4;
 constexpr int BAR_BYTES = 256;
 constexpr int HALF_BYTES = 2 * 2 * BM * 4;
@@ -613,6 +620,80 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap tmA1, const __grid_constant__
                 }
                 scale = ss > 0.f ? rsqrtf(ss) : 0.f;             // zero row stays zero (reading A3)
             }
+            if (p.sel_state != nullptr) {
+                // selection epilogue of the top-K lookup: one max per score against the row's current
+                // k-th score; the (rare) survivors become keys in the row's candidate buffer
+                const long long q = m0 + row;
+                const bool live = q < p.M;
+                unsigned long long *st = p.sel_state + (size_t)(live ? q : 0) * TK_TOTAL;
+                const unsigned long long tau = live ? st[p.sel_k - 1] : ~0ull;
+                const float tau_f = !live ? INFINITY : tau ? unord_f32((unsigned)(tau >> 32)) : -INFINITY;
+                // A score is kept when it reaches the k-th score (ties with it included: a key that
+                // does not beat tau is dropped by the next merge, so a superset is harmless).  One pass
+                // over the accumulator; the rare keepers become keys in this row's queue in the warp's
+                // staging memory.  The accumulator is released before the queue goes to global memory,
+                // so the one atomicAdd per row that reserves the slots is off the MMA's critical path.
+                const int lim = min(c_hi, p.sel_nb - n0);         // valid columns of this slab
+                unsigned long long *sq = reinterpret_cast<unsigned long long *>(
+                    smem + stg_off + (eh * 4 + ew) * (SEL_Q * 32 * 8));                  // [SEL_Q][32 lanes]
+                int nl = 0;
+                for (int c0 = c_lo; c0 < c_hi; c0 += OUT_CHUNK) {
+                    uint32_t v[2][32];
+                    tc_ld32(t0 + c0, v[0]);                       // (warp-collective: never under a lane's branch)
+                    tc_ld32(t0 + c0 + 32, v[1]);
+                    tc_wait_ld();
+                    if (c0 + OUT_CHUNK > lim) {                   // ragged end (uniform): columns past it lose
+#pragma unroll
+                        for (int i = 0; i < 64; ++i)
+                            if (c0 + i >= lim) v[i >> 5][i & 31] = 0xff800000u;   // -inf
+                    }
+                    // eight columns at a time: one max tree and one warp vote; only a group in which some
+                    // row has a keeper is looked at column by column, again under warp-uniform branches
+#pragma unroll
+                    for (int g8 = 0; g8 < 8; ++g8) {
+                        const uint32_t *w = &v[g8 >> 2][(g8 & 3) * 8];
+                        const float mx = fmaxf(
+                            fmaxf(fmaxf(__uint_as_float(w[0]), __uint_as_float(w[1])),
+                                  fmaxf(__uint_as_float(w[2]), __uint_as_float(w[3]))),
+                            fmaxf(fmaxf(__uint_as_float(w[4]), __uint_as_float(w[5])),
+                                  fmaxf(__uint_as_float(w[6]), __uint_as_float(w[7]))));
+                        if (!__any_sync(0xffffffffu, mx >= tau_f)) continue;
+#pragma unroll
+                        for (int j = 0; j < 8; ++j) {
+                            const float x = __uint_as_float(w[j]);
+                            const bool hit = x >= tau_f;
+                            if (!__any_sync(0xffffffffu, hit)) continue;
+                            if (hit) {
+                                const unsigned long long key = make_key(x, p.sel_id0 + n0 + c0 + g8 * 8 + j);
+                                if (nl < SEL_Q) {
+                                    sq[nl * 32 + lane] = key;
+                                } else {                          // queue full (a very loose tau): one by one
+                                    const int slot = atomicAdd(p.sel_cnt + q, 1);
+                                    if (slot < TK_LIST) st[TK_LIST + slot] = key;
+                                }
+                                ++nl;
+                            }
+                        }
+                    }
+                }
+                tc_fence_before();
+                __syncwarp();
+                if (lane == 0) {
+                    if (CG == 2) mbar_arrive_remote_relaxed(tempty_leader + 8 * acc);
+                    else mbar_arrive(bar_tempty + 8 * acc);
+                }
+                nl = min(nl, SEL_Q);
+                if (nl) {
+                    const int at = atomicAdd(p.sel_cnt + q, nl);
+                    for (int j = 0; j < nl && at + j < TK_LIST; ++j) st[TK_LIST + at + j] = sq[j * 32 + lane];
+                }
+                __syncwarp();
+                if (++acc == p.nacc) {
+                    acc = 0;
+                    accphase ^= 1;
+                }
+                continue;
+            } else
             // pass 2: 64 columns at a time -> bf16 -> swizzled staging -> TMA store
             for (int c0 = c_lo; c0 < c_hi; c0 += OUT_CHUNK) {
                 uint32_t v[2][32];
@@ -788,6 +869,8 @@ bool plan(const GemmArgs &a, int cg, int ns_pref, int epi_pref, TcParams &p, int
     if (a.ldb % 8 || (a.ldb > 0 && a.ldb < a.K1 + a.K2)) return no("ldb must be a multiple of 8, >= K1 + K2");
     if (cg == 2 && (a.M <= BM || a.N % 16)) return no("CTA pairs need M > 128 and N % 16 == 0");
     if (a.out_f32 && a.addend) return no("fp32 output takes no addend");
+    if (a.sel_state && (a.l2norm || a.addend || a.bias || a.relu || a.sel_k < 1 || a.sel_k > TK_LIST))
+        return no("the selection epilogue takes plain products and 1 <= k <= 1024");
     p = TcParams{};
     p.cg = cg;
     p.M = a.M;
@@ -817,8 +900,11 @@ bool plan(const GemmArgs &a, int cg, int ns_pref, int epi_pref, TcParams &p, int
     // gain, and with double-buffered accumulators the epilogue is hidden anyway).  Used for row-norm
     // GEMMs with a single accumulator when at least three operand stages still fit.
     int fixed = 0;
-    for (p.epi_halves = (epi_pref == 2 && p.NS > 64) ? 2 : (epi_pref == 1 || !a.l2norm || p.nacc == 2) ? 1 : 2; p.epi_halves >= 1; --p.epi_halves) {
-        p.stg_bytes = p.epi_halves * 4 * 2 * STG_WARP_BYTES;
+    // (the selection epilogue is ALU work per score, not stores: eight warps there as well)
+    const bool want8 = (a.sel_state && p.NS > 64 && epi_pref != 1) || (epi_pref == 2 && p.NS > 64) ||
+                       (epi_pref != 1 && a.l2norm && p.nacc != 2);
+    for (p.epi_halves = want8 ? 2 : 1; p.epi_halves >= 1; --p.epi_halves) {
+        p.stg_bytes = a.sel_state ? p.epi_halves * 4 * (SEL_Q * 32 * 8) : p.epi_halves * 4 * 2 * STG_WARP_BYTES;
         fixed = p.stg_bytes + BIAS_BYTES + BAR_BYTES + (p.epi_halves == 2 ? HALF_BYTES : 0) +
                 (units_per_cluster > 1 ? XCHG_BYTES : 0);
         p.stages = (SMEM_LIMIT - fixed) / p.stage_bytes;
@@ -831,6 +917,11 @@ bool plan(const GemmArgs &a, int cg, int ns_pref, int epi_pref, TcParams &p, int
     p.bias = a.bias;
     p.addend = static_cast<const uint4 *>(a.addend);
     p.out_f32 = a.out_f32;
+    p.sel_state = a.sel_state;
+    p.sel_cnt = a.sel_cnt;
+    p.sel_k = a.sel_k;
+    p.sel_nb = (int)(a.b_rows ? a.b_rows : a.N);
+    p.sel_id0 = a.sel_id0;
     p.relu = a.relu;
     p.l2norm = a.l2norm;
     // instruction descriptor, kind::f16: D fp32 (bit 4), A and B bf16 (bits 7, 10), both K-major,

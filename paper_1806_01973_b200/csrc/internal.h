@@ -31,6 +31,13 @@ struct GemmArgs {
     const float *bias = nullptr;
     int relu = 0;
     int l2norm = 0;
+    // top-K selection epilogue (tcgen05 kernel only, see topk.cu): instead of storing the product,
+    // every score that beats row q's current k-th key is appended to q's candidate buffer.  Columns are
+    // candidates sel_id0 + [0, b_rows).  out is not written.
+    unsigned long long *sel_state = nullptr;
+    int *sel_cnt = nullptr;
+    int32_t sel_k = 0;
+    int64_t sel_id0 = 0;
     int out_f32 = 0;                // tcgen05 kernel only: store the result as fp32 (top-K scores; split fp32 mode)
     void *out = nullptr;
 };
@@ -95,10 +102,41 @@ cudaError_t subset_remap_tables(const int32_t *list, int64_t n, const int32_t *i
                                 int32_t T, const int32_t *pos_prev, int32_t *idx_loc, float *w_loc,
                                 cudaStream_t s, int *launches);
 
+// ---- keys of the top-K lookup (shared by topk.cu and the selection epilogue of the tcgen05 GEMM) ----
+//     key = orderable(score) << 32 | (0xFFFFFFFF - id)        (larger key = better: score desc, id asc)
+// Per-query state: TK_TOTAL keys -- the running list (sorted descending at its last merge) in [0, k),
+// zeros up to TK_LIST, the candidate buffer in [TK_LIST, TK_LIST + cnt[q]).
+constexpr int TK_LIST = 1024;              // k <= TK_LIST
+constexpr int TK_TOTAL = 2 * TK_LIST;      // running list + candidate buffer
+#ifdef __CUDACC__
+__device__ __forceinline__ unsigned ord_f32(float x)       // order-preserving map fp32 -> uint32
+{
+    const unsigned u = __float_as_uint(x);
+    return (u & 0x80000000u) ? ~u : (u | 0x80000000u);
+}
+__device__ __forceinline__ float unord_f32(unsigned o)
+{
+    return __uint_as_float((o & 0x80000000u) ? (o & 0x7fffffffu) : ~o);
+}
+__device__ __forceinline__ unsigned long long make_key(float score, long long id)
+{
+    return ((unsigned long long)ord_f32(score) << 32) | (unsigned long long)(0xFFFFFFFFu - (unsigned)id);
+}
+#endif
+
 // ---- topk.cu: running top-k lists for the exact nearest-neighbour lookup ---------------------------
 size_t topk_state_bytes(int64_t nq);   // per-query running lists + buffers; zero it before the first block
+// only: optional byte mask [nq]; queries with only[q] == 0 are skipped (the redo of overflowed blocks)
 cudaError_t launch_topk_merge(const float *scores, int64_t nq, int64_t ld, int32_t nb, int64_t id0,
-                              int32_t k, void *state, cudaStream_t s, int *launches);
+                              int32_t k, void *state, const unsigned char *only, cudaStream_t s,
+                              int *launches);
+// After a block of candidates went through the selection epilogue: per query, if its buffer
+// overflowed (cnt > TK_LIST) the block's entries are dropped (cnt restored from cnt_prev), ovf[q] = 1
+// and *any = 1 -- the caller redoes that block for those queries from stored scores; otherwise
+// ovf[q] = 0 and a buffer at least merge_at full is merged into the list (new k-th key).
+// cnt_prev [nq] ints (device), equal to the counters before the block; updated for the next block.
+cudaError_t launch_topk_maintain(void *state, int64_t nq, int32_t k, int32_t merge_at, int *cnt_prev,
+                                 unsigned char *ovf, int *any, cudaStream_t s, int *launches);
 cudaError_t launch_topk_finish(const void *state, int64_t nq, int32_t k, int32_t *idx, float *score,
                                cudaStream_t s, int *launches);
 

@@ -3,55 +3,70 @@
 // what the paper serves approximately with LSH + Weak-AND.  Reading C1: nearest = largest inner
 // product z_q . z_i (the score of Eq. 1), ties to the smaller id.
 //
-// The scores of a block of candidates come from the tcgen05 GEMM (fp32 output).  This file keeps, per
-// query, a running list of the k best (score, id) pairs as 64-bit keys
+// The scores of a block of candidates come from the tcgen05 GEMM.  This file keeps, per query, a
+// running list of the k best (score, id) pairs as 64-bit keys
 //     key = orderable(score) << 32 | (0xFFFFFFFF - id)        (larger key = better)
-// and merges a block of scores into it: one CTA per query scans the block (coalesced), appends what
-// beats the current k-th key to a 1024-entry buffer, and only when the buffer could overflow
-// bitonic-sorts list + buffer (2048 keys) and keeps the top k.  The result is the exact top k under a
-// total order, so it does not depend on the order in which candidates were buffered.
+// plus a 1024-key candidate buffer.  Two ways in:
+//  * two-pass (the first block(s), option topk_fused = 0, redone blocks): the GEMM stores fp32 scores,
+//    topk_scan_kernel (one CTA per query) scans them coalesced and appends what beats the current k-th
+//    key to the buffer; only when the buffer could overflow does it merge (sort buffer, bitonic-merge
+//    with the list, keep k);
+//  * fused (every later block): the GEMM's selection epilogue (gemm_tcgen05.cu) appends the keepers
+//    itself -- no score matrix in HBM -- and topk_maintain_kernel merges buffers that are filling up
+//    and flags the (block, query) pairs whose buffer overflowed, which the caller redoes two-pass.
+// The result is the exact top k under a total order, so it does not depend on the order in which
+// candidates were buffered, merged or redone.
 #include "internal.h"
 
 namespace pinsage {
 namespace {
 
 constexpr int TK_THREADS = 256;
-constexpr int TK_LIST = 1024;              // k <= TK_LIST
-constexpr int TK_TOTAL = 2 * TK_LIST;      // running list + candidate buffer
+static_assert(TK_THREADS == 256 && TK_LIST == 1024, "cta_sort_desc maps 8 warps onto 1024 + 2048 keys");
 
-__device__ __forceinline__ unsigned ord_f32(float x)       // order-preserving map fp32 -> uint32
-{
-    const unsigned u = __float_as_uint(x);
-    return (u & 0x80000000u) ? ~u : (u | 0x80000000u);
-}
-__device__ __forceinline__ float unord_f32(unsigned o)
-{
-    return __uint_as_float((o & 0x80000000u) ? (o & 0x7fffffffu) : ~o);
-}
-
-// descending bitonic sort of s[0 .. TK_TOTAL) by the whole CTA
+// s[0 .. TK_LIST) is the running list, sorted descending (zeros at its end); s[TK_LIST .. TK_TOTAL) is the
+// buffer in any order.  Sorts the buffer ascending (bitonic network on 1024 keys) -- list + buffer is
+// then one bitonic sequence -- and finishes with a bitonic merge of all 2048 keys, descending: 38
+// stage-equivalents instead of the 66 of a full sort.  Each warp owns a contiguous run of keys, so
+// every stage whose partner distance stays inside the run needs a __syncwarp only (10 CTA-wide
+// barriers in all instead of 66).
 __device__ void cta_sort_desc(unsigned long long *s)
 {
-    for (int k = 2; k <= TK_TOTAL; k <<= 1)
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    unsigned long long *b = s + TK_LIST;
+    for (int k = 2; k <= TK_LIST; k <<= 1)
         for (int j = k >> 1; j > 0; j >>= 1) {
-            for (int i = threadIdx.x; i < TK_TOTAL; i += TK_THREADS) {
-                const int ixj = i ^ j;
-                if (ixj > i) {
-                    const unsigned long long a = s[i], b = s[ixj];
-                    const bool down = (i & k) == 0;
-                    if ((a < b) == down) {
-                        s[i] = b;
-                        s[ixj] = a;
-                    }
+            if (j >= 128) __syncthreads();
+#pragma unroll
+            for (int r = 0; r < 2; ++r) {                      // warp w: pairs inside b[128 w, 128 w + 128) for j <= 64
+                const int p = warp * 64 + r * 32 + lane;
+                const int i = ((p & ~(j - 1)) << 1) | (p & (j - 1)), l = i | j;
+                const unsigned long long a = b[i], c = b[l];
+                if ((a > c) == ((i & k) == 0)) {
+                    b[i] = c;
+                    b[l] = a;
                 }
             }
-            __syncthreads();
+            if (j >= 128) __syncthreads();
+            else __syncwarp();
         }
-}
-
-__device__ __forceinline__ unsigned long long make_key(float score, long long id)
-{
-    return ((unsigned long long)ord_f32(score) << 32) | (unsigned long long)(0xFFFFFFFFu - (unsigned)id);
+    __syncthreads();
+    for (int j = TK_LIST; j > 0; j >>= 1) {
+        if (j >= 256) __syncthreads();
+#pragma unroll
+        for (int r = 0; r < 4; ++r) {                          // warp w: pairs inside s[256 w, 256 w + 256) for j <= 128
+            const int p = warp * 128 + r * 32 + lane;
+            const int i = ((p & ~(j - 1)) << 1) | (p & (j - 1)), l = i | j;
+            const unsigned long long a = s[i], c = s[l];
+            if (a < c) {
+                s[i] = c;
+                s[l] = a;
+            }
+        }
+        if (j >= 256) __syncthreads();
+        else __syncwarp();
+    }
+    __syncthreads();
 }
 
 // sort list + buffer, keep the best k, empty the buffer; returns the new k-th best key
@@ -76,11 +91,13 @@ __device__ __noinline__ unsigned long long merge_buffer(unsigned long long *s, i
 constexpr int TK_BLOCK = 16 * TK_THREADS;
 __global__ void __launch_bounds__(TK_THREADS)
 topk_scan_kernel(const float *__restrict__ scores, long long ld, int nb, long long id0, int k,
-                 unsigned long long *__restrict__ state, int *__restrict__ cnts)
+                 unsigned long long *__restrict__ state, int *__restrict__ cnts,
+                 const unsigned char *__restrict__ only)
 {
     __shared__ unsigned long long s[TK_TOTAL];
     __shared__ int cnt, blk;
     const long long q = blockIdx.x;
+    if (only != nullptr && only[q] == 0) return;
     const float *row = scores + q * ld;
     unsigned long long *st = state + q * TK_TOTAL;
     int have = cnts[q];
@@ -157,6 +174,35 @@ topk_scan_kernel(const float *__restrict__ scores, long long ld, int nb, long lo
     if (threadIdx.x == 0) cnts[q] = have;
 }
 
+// bookkeeping after a block that went through the GEMM's selection epilogue (see internal.h)
+__global__ void __launch_bounds__(TK_THREADS)
+topk_maintain_kernel(unsigned long long *__restrict__ state, int *__restrict__ cnts, int k, int merge_at,
+                     int *__restrict__ cnt_prev, unsigned char *__restrict__ ovf, int *__restrict__ any)
+{
+    __shared__ unsigned long long s[TK_TOTAL];
+    const long long q = blockIdx.x;
+    const int have = cnts[q];
+    if (have > TK_LIST) {                                      // some of this block's keepers were dropped
+        if (threadIdx.x == 0) {
+            cnts[q] = cnt_prev[q];
+            ovf[q] = 1;
+            *any = 1;
+        }
+        return;
+    }
+    if (threadIdx.x == 0) ovf[q] = 0;
+    if (have < merge_at) {
+        if (threadIdx.x == 0) cnt_prev[q] = have;
+        return;
+    }
+    unsigned long long *st = state + q * TK_TOTAL;
+    for (int i = threadIdx.x; i < TK_TOTAL; i += TK_THREADS) s[i] = i < TK_LIST + have ? st[i] : 0ull;
+    __syncthreads();
+    cta_sort_desc(s);
+    for (int i = threadIdx.x; i < TK_LIST; i += TK_THREADS) st[i] = i < k ? s[i] : 0ull;
+    if (threadIdx.x == 0) cnts[q] = cnt_prev[q] = 0;
+}
+
 // final merge of list + buffer and decoding: idx / score [nq x k]
 __global__ void __launch_bounds__(TK_THREADS)
 topk_finish_kernel(const unsigned long long *__restrict__ state, const int *__restrict__ cnts, int k,
@@ -183,12 +229,23 @@ size_t topk_state_bytes(int64_t nq) { return (size_t)nq * TK_TOTAL * 8 + (size_t
 
 // state: topk_state_bytes(nq) zeroed bytes (keys, then the counters) before the first block of scores
 cudaError_t launch_topk_merge(const float *scores, int64_t nq, int64_t ld, int32_t nb, int64_t id0,
-                              int32_t k, void *state, cudaStream_t s, int *launches)
+                              int32_t k, void *state, const unsigned char *only, cudaStream_t s,
+                              int *launches)
 {
     if (k < 1 || k > TK_LIST) return cudaErrorNotSupported;
     unsigned long long *keys = static_cast<unsigned long long *>(state);
     int *cnts = reinterpret_cast<int *>(keys + (size_t)nq * TK_TOTAL);
-    topk_scan_kernel<<<(unsigned)nq, TK_THREADS, 0, s>>>(scores, ld, nb, id0, k, keys, cnts);
+    topk_scan_kernel<<<(unsigned)nq, TK_THREADS, 0, s>>>(scores, ld, nb, id0, k, keys, cnts, only);
+    if (launches) ++*launches;
+    return cudaGetLastError();
+}
+
+cudaError_t launch_topk_maintain(void *state, int64_t nq, int32_t k, int32_t merge_at, int *cnt_prev,
+                                 unsigned char *ovf, int *any, cudaStream_t s, int *launches)
+{
+    unsigned long long *keys = static_cast<unsigned long long *>(state);
+    int *cnts = reinterpret_cast<int *>(keys + (size_t)nq * TK_TOTAL);
+    topk_maintain_kernel<<<(unsigned)nq, TK_THREADS, 0, s>>>(keys, cnts, k, merge_at, cnt_prev, ovf, any);
     if (launches) ++*launches;
     return cudaGetLastError();
 }

@@ -34,15 +34,57 @@ def test_topk_exact_on_integer_embeddings(ctx, dtype, nq, N, d, k):
     g = torch.Generator().manual_seed(nq + N)
     Q = torch.randint(-2, 3, (nq, d), generator=g).to(dtype)
     Z = torch.randint(-2, 3, (N, d), generator=g).to(dtype)
-    for cg in ([1, 0] if dtype == torch.bfloat16 else [0]):
+    ref_idx, ref_score = O.topk(to_f64(Q), to_f64(Z), k)
+    for cg, fused in ([(1, 1), (0, 1), (0, 0)] if dtype == torch.bfloat16 else [(0, 1)]):
         ctx.pinsage_set_option("gemm_cg", cg)
+        ctx.pinsage_set_option("topk_fused", fused)
         try:
             idx, score = ctx.pinsage_topk(Q.to(DEV), Z.to(DEV), k)
         finally:
             ctx.pinsage_set_option("gemm_cg", 0)
-        ref_idx, ref_score = O.topk(to_f64(Q), to_f64(Z), k)
+            ctx.pinsage_set_option("topk_fused", 1)
         np.testing.assert_array_equal(idx.cpu().numpy(), ref_idx)
         np.testing.assert_array_equal(score.cpu().numpy().astype(np.float64), ref_score)
+
+
+@pytest.mark.parametrize("k", [100, 1024])
+def test_topk_many_blocks_fused_selection(ctx, k):
+    """Several candidate blocks, so that most of them go through the GEMM's selection epilogue (only the
+    first one or two are scanned from stored scores); integer embeddings -> identical to the oracle, and
+    identical to the two-pass form."""
+    nq, N, d = 50, 400_003, 32
+    g = torch.Generator().manual_seed(11)
+    Q = torch.randint(-2, 3, (nq, d), generator=g).to(torch.bfloat16)
+    Z = torch.randint(-2, 3, (N, d), generator=g).to(torch.bfloat16)
+    ref_idx, ref_score = O.topk(to_f64(Q), to_f64(Z), k)
+    for fused in (1, 0):
+        ctx.pinsage_set_option("topk_fused", fused)
+        try:
+            idx, score = ctx.pinsage_topk(Q.to(DEV), Z.to(DEV), k)
+        finally:
+            ctx.pinsage_set_option("topk_fused", 1)
+        np.testing.assert_array_equal(idx.cpu().numpy(), ref_idx)
+        np.testing.assert_array_equal(score.cpu().numpy().astype(np.float64), ref_score)
+
+
+def test_topk_fused_selection_overflow_is_redone(ctx):
+    """Adversarial order: candidate scores ascend with the id (ties of 32), so for the "ascending"
+    queries EVERY score of every later block beats the running k-th score, the 1024-key buffers of the
+    selection epilogue overflow in every block, and those (block, query) pairs must be redone from
+    stored scores -- while the "descending" queries of the same blocks keep nothing.  Exact products."""
+    N, d, k = 250_000, 16, 500
+    t = torch.arange(N) // 32
+    Z = torch.zeros((N, d))
+    Z[:, 0], Z[:, 1] = (t // 64).float(), (t % 64).float()      # 64 * Z0 + Z1 = t, all exact in bf16
+    Q = torch.zeros((6, d))
+    Q[0::2, 0], Q[0::2, 1] = 64.0, 1.0                          # score = t: ascending
+    Q[1::2, 0], Q[1::2, 1] = -64.0, -1.0                        # score = -t: descending
+    Q, Z = Q.to(torch.bfloat16), Z.to(torch.bfloat16)
+    ref_idx, ref_score = O.topk(to_f64(Q), to_f64(Z), k)
+    assert ref_idx[0, 0] == N - N % 32 - (32 if N % 32 == 0 else 0) or ref_idx[0, 0] >= N - 32
+    idx, score = ctx.pinsage_topk(Q.to(DEV), Z.to(DEV), k)
+    np.testing.assert_array_equal(idx.cpu().numpy(), ref_idx)
+    np.testing.assert_array_equal(score.cpu().numpy().astype(np.float64), ref_score)
 
 
 @pytest.mark.parametrize("dtype", DTYPES)
