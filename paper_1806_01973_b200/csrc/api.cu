@@ -5,6 +5,7 @@
 #include "internal.h"
 
 #include <algorithm>
+#include <functional>
 #include <cstdarg>
 #include <cstdio>
 #include <cstring>
@@ -435,6 +436,9 @@ bool use_linear_pool(const pinsage_ctx *ctx, const pinsage_layer_params *lp)
     return ctx->linear_pool == 1 || lp->m > lp->d;
 }
 
+// Called on the compute stream's timeline right after rows [r0, r0 + rows) of a layer's output exist.
+using ChunkHook = std::function<pinsage_status(int64_t r0, int64_t rows)>;
+
 // S2 + S3 over all destination rows in chunks; pool of chunk c+1 may overlap combine of chunk c.
 // Hin [N x d_in] (read), P [N x pw] (read), Hout [N x d] (written; may alias Hin iff d == d_in).
 // pw = m (P = projections, n is the second K segment of S3) or, in the linear-pool schedule, d
@@ -443,7 +447,8 @@ pinsage_status pool_combine_chunks(pinsage_ctx *ctx, DType dt, int64_t N, int32_
                                    const pinsage_layer_params *lp, const void *Hin, const void *P,
                                    const int32_t *idx, const float *w, void *Hout, int64_t chunk,
                                    void *nbuf0, void *nbuf1, void *scratch, size_t scratch_bytes,
-                                   const cudaEvent_t *tables_landed = nullptr, int64_t n_src = -1)
+                                   const cudaEvent_t *tables_landed = nullptr, int64_t n_src = -1,
+                                   const ChunkHook &after_chunk = nullptr)
 {
     if (n_src < 0) n_src = N;                // rows of P; N = destination rows
     const size_t es = elem_size(dt);
@@ -491,6 +496,7 @@ pinsage_status pool_combine_chunks(pinsage_ctx *ctx, DType dt, int64_t N, int32_
         g.out = static_cast<char *>(Hout) + (size_t)r0 * lp->d * es;
         PS_TRY(run_gemm(ctx, dt, g, scratch, scratch_bytes, ctx->stream));
         if (two) PS_CUDA(ctx, cudaEventRecord(ctx->ev_gemm[b], ctx->stream));
+        if (after_chunk) PS_TRY(after_chunk(r0, rows));
     }
     if (two) {
         PS_CUDA(ctx, cudaEventRecord(ctx->ev_join, ps));
@@ -542,7 +548,7 @@ pinsage_status layer_on_ws(pinsage_ctx *ctx, DType dt, int64_t N, int32_t T, con
                            void *out, char *ws, const LayerWs &plan, int64_t chunk,
                            const cudaEvent_t *feats_landed = nullptr,
                            const cudaEvent_t *tables_landed = nullptr, int64_t n_src = -1,
-                           const void *src_feats = nullptr)
+                           const void *src_feats = nullptr, const ChunkHook &after_chunk = nullptr)
 {
     // n_src / src_feats (targeted inference): the source rows S1 projects differ from the N
     // destination rows, whose own previous representations are `feats`
@@ -579,7 +585,7 @@ pinsage_status layer_on_ws(pinsage_ctx *ctx, DType dt, int64_t N, int32_t T, con
     }
     return pool_combine_chunks(ctx, dt, N, T, lp, feats, ws + plan.P_off, idx, w, out, chunk,
                                ws + plan.n0_off, ws + plan.n1_off, ws + plan.scratch_off,
-                               plan.scratch_bytes, tables_landed, n_src);
+                               plan.scratch_bytes, tables_landed, n_src, after_chunk);
 }
 
 // Grows the per-chunk event pool of the host-buffer pipeline to n events.
@@ -1076,24 +1082,12 @@ pinsage_status pinsage_embed_all(pinsage_ctx *ctx, pinsage_dtype dtype, int64_t 
 
     const void *Hin = d_feats;
     char *Hcur = nullptr;
-    for (int k = 0; k < K; ++k) {
-        const pinsage_layer_params *lp = &layers[k];
-        const LayerWs plan = plan_layer_ws(ctx, dt, N, lp, chunk);
-        char *Hout;
-        if (k == 0) Hout = Ha;
-        else if (lp->d == lp->d_in) Hout = Hcur;           // in place (S1 has consumed all of H first)
-        else Hout = (Hcur == Ha) ? Hb : Ha;
-        PS_TRY(layer_on_ws(ctx, dt, N, T, Hin, d_idx, d_w, lp, Hout, ws, plan, chunk,
-                           k == 0 ? feats_landed : nullptr, k == 0 ? tables_landed : nullptr));
-        Hcur = Hout;
-        Hin = Hout;
-    }
-    // ---- head, chunk by chunk (the intermediate a never exists in full) ---------------------------
-    for (int64_t r0 = 0; r0 < N; r0 += chunk) {
-        const int64_t rows = std::min(chunk, N - r0);
+    // ---- head of rows [r0, r0 + rows) (the intermediate a never exists in full) -------------------
+    const char *Hlast = nullptr;              // the last layer's output buffer (set when the loop reaches it)
+    ChunkHook head_chunk = [&](int64_t r0, int64_t rows) -> pinsage_status {
         GemmArgs g;
         g.M = rows; g.K1 = head->d; g.N = head->g1;
-        g.A1 = Hcur + (size_t)r0 * head->d * es;
+        g.A1 = Hlast + (size_t)r0 * head->d * es;
         g.B = head->G1; g.bias = head->g; g.relu = 1; g.out = abuf;
         PS_TRY(run_gemm(ctx, dt, g, nullptr, 0, ctx->stream));
         GemmArgs g2;
@@ -1108,7 +1102,26 @@ pinsage_status pinsage_embed_all(pinsage_ctx *ctx, pinsage_dtype dtype, int64_t 
             PS_CUDA(ctx, cudaMemcpyAsync(static_cast<char *>(out) + r0 * rb, static_cast<char *>(d_out) + r0 * rb,
                                          rows * rb, cudaMemcpyDeviceToHost, ctx->d2h));
         }
+        return PINSAGE_OK;
+    };
+    for (int k = 0; k < K; ++k) {
+        const pinsage_layer_params *lp = &layers[k];
+        const LayerWs plan = plan_layer_ws(ctx, dt, N, lp, chunk);
+        char *Hout;
+        if (k == 0) Hout = Ha;
+        else if (lp->d == lp->d_in) Hout = Hcur;           // in place (S1 has consumed all of H first)
+        else Hout = (Hcur == Ha) ? Hb : Ha;
+        if (k == K - 1) Hlast = Hout;
+        // host output: the head of a chunk follows its last S3 directly, so that finished chunks of
+        // `out` travel home while the rest of the last layer is still being computed
+        PS_TRY(layer_on_ws(ctx, dt, N, T, Hin, d_idx, d_w, lp, Hout, ws, plan, chunk,
+                           k == 0 ? feats_landed : nullptr, k == 0 ? tables_landed : nullptr, -1, nullptr,
+                           (k == K - 1 && out_ready) ? head_chunk : ChunkHook()));
+        Hcur = Hout;
+        Hin = Hout;
     }
+    if (!out_ready)
+        for (int64_t r0 = 0; r0 < N; r0 += chunk) PS_TRY(head_chunk(r0, std::min(chunk, N - r0)));
     if (any_host) {
         PS_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
         PS_CUDA(ctx, cudaStreamSynchronize(ctx->h2d));
