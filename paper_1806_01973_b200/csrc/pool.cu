@@ -74,9 +74,12 @@ struct Chunk<true> {  // 8 bf16 per 16 bytes
     {
         const uint32_t u[4] = {r.x, r.y, r.z, r.w};
 #pragma unroll
-        for (int i = 0; i < 4; ++i) {
-            acc[2 * i] = fmaf(wt, __uint_as_float(u[i] << 16), acc[2 * i]);
-            acc[2 * i + 1] = fmaf(wt, __uint_as_float(u[i] & 0xffff0000u), acc[2 * i + 1]);
+        for (int i = 0; i < 4; ++i) {                      // packed fp32x2 FMA (sm_100): same two IEEE fmas, one issue slot
+            const float2 z = __ffma2_rn(make_float2(wt, wt),
+                                        make_float2(__uint_as_float(u[i] << 16), __uint_as_float(u[i] & 0xffff0000u)),
+                                        make_float2(acc[2 * i], acc[2 * i + 1]));
+            acc[2 * i] = z.x;
+            acc[2 * i + 1] = z.y;
         }
     }
     static __device__ __forceinline__ void vmax(const uint4 &r, float (&acc)[8])
