@@ -42,6 +42,17 @@ struct pinsage_ctx {
     void *stage = nullptr;           // device staging for host inputs / outputs
     size_t stage_bytes = 0;
     long long *d_first_bad = nullptr;
+    int pool_hubs = 0;               // hub-split pool (hubs.cu): 0 off, -1 automatic, H = 64..512 forced
+    struct HubState {                // valid during one pinsage_embed_all call
+        int H = 0;
+        const int32_t *src_idx = nullptr;   // the caller's table the remapped one stands for
+        const int32_t *idxm = nullptr;      // remapped table: hub entries are -(rank + 1)
+        const int32_t *hub_ids = nullptr;
+        void *A = nullptr;                  // [chunk x 2H] bf16
+        void *BT = nullptr;                 // [pw x 2H] bf16
+    } hub;
+    void *hub_buf = nullptr;
+    size_t hub_bytes = 0;
     int topk_fused = 1;              // pinsage_topk: select in the GEMM epilogue (1) or in a second pass over stored scores (0)
     int f32_split = -1;              // fp32 GEMMs on the tensor cores by bf16 splitting: -1 automatic, 0 never, 1 always
     void *split_buf = nullptr;       // bf16 planes of the operands of a split fp32 GEMM (grown on demand)
@@ -296,6 +307,7 @@ pinsage_status run_gemm_split(pinsage_ctx *ctx, const GemmArgs &a, cudaStream_t 
     if (need > ctx->split_bytes) {
         PS_CUDA(ctx, cudaStreamSynchronize(s));
         if (ctx->split_buf) cudaFree(ctx->split_buf);
+    if (ctx->hub_buf) cudaFree(ctx->hub_buf);
         ctx->split_buf = nullptr;
         ctx->split_bytes = 0;
         PS_CUDA(ctx, cudaMalloc(&ctx->split_buf, need));
@@ -327,11 +339,11 @@ pinsage_status run_gemm_split(pinsage_ctx *ctx, const GemmArgs &a, cudaStream_t 
 
 // One GEMM of the path on stream s. scratch: fp32 [M x N] for the SIMT norm pass / tcgen05 partials.
 pinsage_status run_gemm(pinsage_ctx *ctx, DType dt, const GemmArgs &a, void *scratch,
-                        size_t scratch_bytes, cudaStream_t s)
+                        size_t scratch_bytes, cudaStream_t s, int prof_kind = -1)
 {
     if (a.M == 0) return PINSAGE_OK;
     const bool simt = dt == DType::F32 || ctx->gemm_impl == 1;
-    const int kind = a.l2norm ? PROF_COMBINE : PROF_DENSE;
+    const int kind = prof_kind >= 0 ? prof_kind : a.l2norm ? PROF_COMBINE : PROF_DENSE;
     if (split_wanted(ctx, dt, a)) {
         bool done = false;
         PS_TRY(run_gemm_split(ctx, a, s, &done));
@@ -462,17 +474,44 @@ pinsage_status pool_combine_chunks(pinsage_ctx *ctx, DType dt, int64_t N, int32_
         PS_CUDA(ctx, cudaStreamWaitEvent(ctx->aux, ctx->ev_fork, 0));
     }
     cudaStream_t ps = two ? ctx->aux : ctx->stream;
+    // hub-split pool (hubs.cu): the gather skips the hub entries, the hub part is a GEMM on the chunk
+    const bool hubs = ctx->hub.H > 0 && idx == ctx->hub.src_idx && !two && dt == DType::BF16 &&
+                      ctx->pool_mode == 0;
+    if (hubs) {
+        cudaError_t e = launch_hub_rows(P, ctx->hub.hub_ids, ctx->hub.H, pw, ctx->hub.BT, ps, &ctx->launches);
+        count_launches(ctx);
+        PS_CUDA(ctx, e);
+    }
     for (int64_t c = 0; c < nchunks; ++c) {
         const int64_t r0 = c * chunk, rows = std::min(chunk, N - r0);
         const int b = (int)(c & 1);
         if (two && c >= 2) PS_CUDA(ctx, cudaStreamWaitEvent(ps, ctx->ev_gemm[b], 0));
         if (tables_landed) PS_CUDA(ctx, cudaStreamWaitEvent(ps, tables_landed[c], 0));
         const int pe0 = prof_mark(ctx, ps);
-        cudaError_t e = launch_pool(dt, ctx->pool_mode, rows, T, pw, P, idx + (size_t)r0 * T, w + (size_t)r0 * T,
-                                    nb[b], pick_slab(ctx, dt, n_src, T, pw), ps, &ctx->launches);
+        cudaError_t e;
+        if (hubs) {
+            const int32_t *im = ctx->hub.idxm + (size_t)r0 * T;
+            e = launch_pool(dt, 0, rows, T, pw, P, im, w + (size_t)r0 * T, nb[b], 0, ps, &ctx->launches, 1);
+            if (e == cudaSuccess)
+                e = launch_hub_matrix(im, w + (size_t)r0 * T, rows, T, ctx->hub.H, 0, ctx->hub.A, ps, &ctx->launches);
+        } else {
+            e = launch_pool(dt, ctx->pool_mode, rows, T, pw, P, idx + (size_t)r0 * T, w + (size_t)r0 * T,
+                            nb[b], pick_slab(ctx, dt, n_src, T, pw), ps, &ctx->launches);
+        }
         prof_close(ctx, PROF_POOL, pe0, ps);
         count_launches(ctx);
         PS_CUDA(ctx, e);
+        if (hubs) {                              // n[chunk] += A_hub P_hub  (added in the GEMM's epilogue, in place)
+            GemmArgs gh;
+            gh.M = rows;
+            gh.K1 = 2 * ctx->hub.H;
+            gh.N = pw;
+            gh.A1 = ctx->hub.A;
+            gh.B = ctx->hub.BT;
+            gh.addend = nb[b];
+            gh.out = nb[b];
+            PS_TRY(run_gemm(ctx, dt, gh, nullptr, 0, ps, PROF_POOL));
+        }
         if (two) {
             PS_CUDA(ctx, cudaEventRecord(ctx->ev_pool[b], ps));
             PS_CUDA(ctx, cudaStreamWaitEvent(ctx->stream, ctx->ev_pool[b], 0));
@@ -731,6 +770,10 @@ pinsage_status pinsage_set_option(pinsage_ctx *ctx, const char *key, int64_t val
         if (value != -1 && value != 0 && value != 32 && value != 64 && value != 128)
             return fail(ctx, PINSAGE_ERR_INVALID_ARG, "pool_slab must be -1, 0, 32, 64 or 128");
         ctx->pool_slab = (int)value;
+    } else if (!strcmp(key, "pool_hubs")) {
+        if (value != -1 && value != 0 && (value < 64 || value > 512 || value % 64))
+            return fail(ctx, PINSAGE_ERR_INVALID_ARG, "pool_hubs must be -1, 0 or a multiple of 64 in [64, 512]");
+        ctx->pool_hubs = (int)value;
     } else if (!strcmp(key, "topk_fused")) {
         ctx->topk_fused = value != 0;
     } else if (!strcmp(key, "f32_split")) {
@@ -1079,6 +1122,52 @@ pinsage_status pinsage_embed_all(pinsage_ctx *ctx, pinsage_dtype dtype, int64_t 
     }
 
     PS_TRY(maybe_validate(ctx, N, N, T, d_idx, d_w));
+
+    // ---- hub-split pool (skewed graphs; hubs.cu): pick the hubs from a sample of the lists, remap ----
+    struct HubReset {
+        pinsage_ctx *c;
+        ~HubReset() { c->hub.H = 0; }
+    } hub_reset{ctx};
+    if (ctx->pool_hubs != 0 && dt == DType::BF16 && ctx->pool_mode == 0 && ctx->gemm_impl == 0 && !ctx->overlap &&
+        !h_idx && !h_w && N * (int64_t)T >= (1 << 22)) {
+        const int H = ctx->pool_hubs > 0 ? ctx->pool_hubs : 128;
+        int32_t pw_max = 0;
+        for (int k = 0; k < K; ++k) pw_max = std::max(pw_max, use_linear_pool(ctx, &layers[k]) ? layers[k].d : layers[k].m);
+        const size_t nB = align_up((size_t)N * 4, 256), candB = align_up(hub_cand_bytes(), 256);
+        const size_t idsB = align_up((size_t)H * 4, 256), tabB = align_up((size_t)N * T * 4, 256);
+        const size_t AB = align_up((size_t)chunk * 2 * H * 2, 256), BTB = align_up((size_t)pw_max * 2 * H * 2, 256);
+        PS_TRY(ensure_buf(ctx, &ctx->hub_buf, &ctx->hub_bytes, 2 * nB + candB + idsB + 256 + tabB + AB + BTB,
+                          "hub-split pool storage"));
+        char *hb = static_cast<char *>(ctx->hub_buf);
+        int32_t *counts = reinterpret_cast<int32_t *>(hb), *rank = reinterpret_cast<int32_t *>(hb + nB);
+        void *cand = hb + 2 * nB;
+        int32_t *hub_ids = reinterpret_cast<int32_t *>(hb + 2 * nB + candB);
+        long long *info = reinterpret_cast<long long *>(hb + 2 * nB + candB + idsB);
+        int32_t *idxm = reinterpret_cast<int32_t *>(hb + 2 * nB + candB + idsB + 256);
+        int64_t sampled = 0;
+        cudaError_t e = launch_hub_select(d_idx, N, T, N, H, counts, rank, cand, hub_ids, info, &sampled,
+                                          ctx->stream, &ctx->launches);
+        count_launches(ctx);
+        PS_CUDA(ctx, e);
+        bool use = true;
+        if (ctx->pool_hubs < 0) {              // automatic: worth it when the hubs hold a third of the entries
+            long long info_h[2] = {0, 0};
+            PS_CUDA(ctx, cudaMemcpyAsync(info_h, info, 16, cudaMemcpyDeviceToHost, ctx->stream));
+            PS_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
+            use = info_h[0] > 0 && 3 * info_h[1] >= sampled;
+        }
+        if (use) {
+            e = launch_hub_remap(d_idx, rank, N * (int64_t)T, idxm, ctx->stream, &ctx->launches);
+            count_launches(ctx);
+            PS_CUDA(ctx, e);
+            ctx->hub.H = H;
+            ctx->hub.src_idx = d_idx;
+            ctx->hub.idxm = idxm;
+            ctx->hub.hub_ids = hub_ids;
+            ctx->hub.A = reinterpret_cast<char *>(idxm) + tabB;
+            ctx->hub.BT = reinterpret_cast<char *>(idxm) + tabB + AB;
+        }
+    }
 
     const void *Hin = d_feats;
     char *Hcur = nullptr;

@@ -1,0 +1,215 @@
+// hubs.cu -- the hub part of the S2 pool on skewed graphs as a dense contraction.
+//
+// N(u) = the T nodes with the highest visit counts of random walks from u.  On a
+// graph with a power-law degree distribution (BASELINE config 4) a few hundred "hub" nodes sit in
+// almost every neighbourhood: the pool n_u = sum_t alpha_ut P[idx_ut] (Alg. 1 l.1) then spends most of
+// its gathers on the same few rows, and is bound by the SM's L1 / issue rate instead of by HBM
+// (profiles/r01_pool_cfg4.md).  Splitting the sum over the neighbour's kind,
+//     n_u = sum_{t: idx_ut not a hub} alpha_ut P[idx_ut]  +  sum_h A[u, h] P[hub_h],
+//     A[u, h] = sum_{t: idx_ut = hub_h} alpha_ut,
+// the second term is a GEMM  A [n x H] . P_hub [H x m]  for the tensor cores and the first a gather
+// over what is left of the lists.  The weights are kept to 16 significand bits (A = A_hi + A_lo in
+// bf16, K = 2H), the products are exact and the sum is fp32; the gathered part is added in the GEMM's
+// epilogue, where the result is rounded to bf16 once more.  Which nodes are hubs is a choice, not
+// part of the result: any set gives the same sum in real arithmetic.
+//
+// Kernels: sampled visit histogram -> candidates -> top-H selection (one CTA) and rank table ->
+// remapped index table (hub entries become -(rank + 1), which the pool kernel skips) -> per chunk the
+// matrix A, per layer the operand P_hub^T.
+#include "internal.h"
+
+#include <algorithm>
+
+namespace pinsage {
+namespace {
+
+constexpr int HUB_CAND = 2048;   // candidate ids whose sampled count can reach the threshold (see hub_cmin)
+
+__global__ void __launch_bounds__(256)
+hub_count_kernel(const int *__restrict__ idx, long long rows, long long row_stride, int T, int *__restrict__ counts)
+{
+    const long long total = rows * T;
+    for (long long e = (long long)blockIdx.x * blockDim.x + threadIdx.x; e < total;
+         e += (long long)gridDim.x * blockDim.x) {
+        const long long r = e / T;
+        const int t = (int)(e - r * T);
+        atomicAdd(counts + idx[r * row_stride * T + t], 1);
+    }
+}
+
+// ids with counts[i] >= cmin: at most sum(counts) / cmin of them, HUB_CAND by the choice of cmin
+__global__ void __launch_bounds__(256)
+hub_candidates_kernel(const int *__restrict__ counts, long long n, int cmin, unsigned long long *__restrict__ cand,
+                      int *__restrict__ n_cand)
+{
+    for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < n;
+         i += (long long)gridDim.x * blockDim.x) {
+        const int c = counts[i];
+        if (c >= cmin) {
+            const int slot = atomicAdd(n_cand, 1);
+            if (slot < HUB_CAND) cand[slot] = ((unsigned long long)(unsigned)c << 32) | (0xFFFFFFFFu - (unsigned)i);
+        }
+    }
+}
+
+// one CTA: sort the candidates (count descending, id ascending), keep H, write hub_ids [H] (-1 beyond
+// the number found), rank[id] = position, info = {hubs found, sampled entries they cover}
+__global__ void __launch_bounds__(1024)
+hub_select_kernel(const unsigned long long *__restrict__ cand, const int *__restrict__ n_cand, int H,
+                  int *__restrict__ hub_ids, int *__restrict__ rank, long long *__restrict__ info)
+{
+    __shared__ unsigned long long s[HUB_CAND];
+    __shared__ long long cover;
+    const int nc = min(*n_cand, HUB_CAND);
+    for (int i = threadIdx.x; i < HUB_CAND; i += blockDim.x) s[i] = i < nc ? cand[i] : 0ull;
+    if (threadIdx.x == 0) cover = 0;
+    __syncthreads();
+    for (int k = 2; k <= HUB_CAND; k <<= 1)
+        for (int j = k >> 1; j > 0; j >>= 1) {
+            for (int i = threadIdx.x; i < HUB_CAND; i += blockDim.x) {
+                const int l = i ^ j;
+                if (l > i) {
+                    const unsigned long long a = s[i], b = s[l];
+                    if ((a < b) == ((i & k) == 0)) {
+                        s[i] = b;
+                        s[l] = a;
+                    }
+                }
+            }
+            __syncthreads();
+        }
+    const int found = min(H, nc);
+    long long mine = 0;
+    for (int r = threadIdx.x; r < H; r += blockDim.x) {
+        int id = -1;
+        if (r < found) {
+            id = (int)(0xFFFFFFFFu - (unsigned)(s[r] & 0xFFFFFFFFull));
+            rank[id] = r;
+            mine += (long long)(s[r] >> 32);
+        }
+        hub_ids[r] = id;
+    }
+    atomicAdd(reinterpret_cast<unsigned long long *>(&cover), (unsigned long long)mine);
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        info[0] = found;
+        info[1] = cover;
+    }
+}
+
+__global__ void __launch_bounds__(256)
+hub_remap_kernel(const int *__restrict__ idx, const int *__restrict__ rank, long long total, int *__restrict__ out)
+{
+    for (long long e = (long long)blockIdx.x * blockDim.x + threadIdx.x; e < total;
+         e += (long long)gridDim.x * blockDim.x) {
+        const int id = idx[e];
+        const int r = rank[id];
+        out[e] = r >= 0 ? -(r + 1) : id;
+    }
+}
+
+// A [rows x 2H] bf16 = [hi | lo] planes of A[u, h] = sum of the weights of u's entries that point at
+// hub h (mean aggregator: 1/T each).  One warp per node, the row is summed in shared memory.
+__global__ void __launch_bounds__(256)
+hub_matrix_kernel(const int *__restrict__ idxm, const float *__restrict__ w, long long rows, int T, int H, int mean,
+                  __nv_bfloat16 *__restrict__ A)
+{
+    extern __shared__ float hub_smem[];
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    float *buf = hub_smem + (size_t)warp * H;
+    const long long v = (long long)blockIdx.x * 8 + warp;
+    if (v >= rows) return;
+    for (int h = lane; h < H; h += 32) buf[h] = 0.f;
+    __syncwarp();
+    const float wmean = 1.0f / (float)T;
+    for (int t = lane; t < T; t += 32) {
+        const int i = idxm[v * T + t];
+        if (i < 0) atomicAdd(buf - (i + 1), mean ? wmean : w[v * T + t]);   // (a list may name a hub twice)
+    }
+    __syncwarp();
+    __nv_bfloat16 *row = A + v * 2 * H;
+    for (int h = lane; h < H; h += 32) {
+        const float a = buf[h];
+        const __nv_bfloat16 hi = __float2bfloat16_rn(a);
+        row[h] = hi;
+        row[H + h] = __float2bfloat16_rn(a - __bfloat162float(hi));
+    }
+}
+
+// BT [pw x 2H] bf16, BT[n, k] = P[hub_ids[k mod H], n] (zero for an unused hub slot): the K-major B
+// operand of the hub GEMM
+__global__ void __launch_bounds__(256)
+hub_rows_kernel(const __nv_bfloat16 *__restrict__ P, const int *__restrict__ hub_ids, int H, int pw,
+                __nv_bfloat16 *__restrict__ BT)
+{
+    const int total = pw * 2 * H;
+    for (int e = blockIdx.x * blockDim.x + threadIdx.x; e < total; e += gridDim.x * blockDim.x) {
+        const int n = e / (2 * H), k = e - n * 2 * H;
+        const int id = hub_ids[k % H];
+        BT[e] = id >= 0 ? P[(size_t)id * pw + n] : __float2bfloat16_rn(0.f);
+    }
+}
+
+inline unsigned grid_for(long long total)
+{
+    return (unsigned)std::max<long long>(1, std::min<long long>((total + 255) / 256, 148LL * 16));
+}
+
+}  // namespace
+
+// Sampled histogram of the neighbour ids (every row_stride-th row of idx [N x T]), the H most frequent
+// ids and their rank table.  counts / rank: device int32 [n_src] (rank is filled with -1 here); cand:
+// device scratch of 2048 keys + one int; hub_ids: device int32 [H]; info: device int64 [2] = {hubs
+// found, sampled entries they cover}.  Returns the number of sampled entries in *sampled.
+cudaError_t launch_hub_select(const int32_t *idx, int64_t N, int32_t T, int64_t n_src, int32_t H,
+                              int32_t *counts, int32_t *rank, void *cand, int32_t *hub_ids, long long *info,
+                              int64_t *sampled, cudaStream_t s, int *launches)
+{
+    const int64_t rows = std::min<int64_t>(N, 16384), stride = N / rows;
+    const int64_t entries = rows * T;
+    *sampled = entries;
+    unsigned long long *keys = static_cast<unsigned long long *>(cand);
+    int *n_cand = reinterpret_cast<int *>(keys + HUB_CAND);
+    cudaError_t e = cudaMemsetAsync(counts, 0, (size_t)n_src * 4, s);
+    if (e == cudaSuccess) e = cudaMemsetAsync(rank, 0xFF, (size_t)n_src * 4, s);
+    if (e == cudaSuccess) e = cudaMemsetAsync(n_cand, 0, 4, s);
+    if (e != cudaSuccess) return e;
+    hub_count_kernel<<<grid_for(entries), 256, 0, s>>>(idx, rows, stride, T, counts);
+    // an id needs cmin hits to be a candidate; at most entries / cmin <= HUB_CAND ids can have them
+    const int cmin = (int)std::max<int64_t>(2, (entries + HUB_CAND - 1) / HUB_CAND);
+    hub_candidates_kernel<<<grid_for(n_src), 256, 0, s>>>(counts, n_src, cmin, keys, n_cand);
+    hub_select_kernel<<<1, 1024, 0, s>>>(keys, n_cand, H, hub_ids, rank, info);
+    if (launches) *launches += 3;
+    return cudaGetLastError();
+}
+
+size_t hub_cand_bytes() { return (size_t)HUB_CAND * 8 + 256; }
+
+cudaError_t launch_hub_remap(const int32_t *idx, const int32_t *rank, int64_t total, int32_t *out,
+                             cudaStream_t s, int *launches)
+{
+    hub_remap_kernel<<<grid_for(total), 256, 0, s>>>(idx, rank, total, out);
+    if (launches) ++*launches;
+    return cudaGetLastError();
+}
+
+cudaError_t launch_hub_matrix(const int32_t *idxm, const float *w, int64_t rows, int32_t T, int32_t H,
+                              int mean, void *A, cudaStream_t s, int *launches)
+{
+    if (rows <= 0) return cudaSuccess;
+    hub_matrix_kernel<<<(unsigned)((rows + 7) / 8), 256, (size_t)8 * H * 4, s>>>(
+        idxm, w, rows, T, H, mean, static_cast<__nv_bfloat16 *>(A));
+    if (launches) ++*launches;
+    return cudaGetLastError();
+}
+
+cudaError_t launch_hub_rows(const void *P, const int32_t *hub_ids, int32_t H, int32_t pw, void *BT,
+                            cudaStream_t s, int *launches)
+{
+    hub_rows_kernel<<<grid_for((long long)pw * 2 * H), 256, 0, s>>>(static_cast<const __nv_bfloat16 *>(P), hub_ids,
+                                                                    H, pw, static_cast<__nv_bfloat16 *>(BT));
+    if (launches) ++*launches;
+    return cudaGetLastError();
+}
+
+}  // namespace pinsage

@@ -73,13 +73,25 @@ cudaError_t launch_split3(bool is_b, const float *S1, int32_t K1, int64_t ld1, c
 // mode: 0 importance (weighted sum), 1 element-wise mean, 2 element-wise max (w unused for 1, 2).
 cudaError_t launch_pool(DType dt, int mode, int64_t n_dst, int32_t T, int32_t m, const void *P,
                         const int32_t *idx, const float *w, void *out, int slab_bytes, cudaStream_t s,
-                        int *launches);
+                        int *launches, int skip_neg = 0);   // skip_neg: entries with idx < 0 are not gathered
 bool pool_slab_ok(DType dt, int32_t T, int32_t m, int slab_bytes);
 cudaError_t launch_normalize_counts(int64_t N, int32_t T, const int32_t *counts, float *w,
                                     cudaStream_t s, int *launches);
 // first_bad: device int64, set to the smallest offending flat position or -1
 cudaError_t launch_validate(int64_t n_dst, int64_t n_src, int32_t T, const int32_t *idx,
                             const float *w, long long *first_bad, cudaStream_t s, int *launches);
+
+// ---- hubs.cu: the hub part of the pool on skewed graphs as a GEMM (see the file header) ----------
+cudaError_t launch_hub_select(const int32_t *idx, int64_t N, int32_t T, int64_t n_src, int32_t H,
+                              int32_t *counts, int32_t *rank, void *cand, int32_t *hub_ids, long long *info,
+                              int64_t *sampled, cudaStream_t s, int *launches);
+size_t hub_cand_bytes();
+cudaError_t launch_hub_remap(const int32_t *idx, const int32_t *rank, int64_t total, int32_t *out,
+                             cudaStream_t s, int *launches);
+cudaError_t launch_hub_matrix(const int32_t *idxm, const float *w, int64_t rows, int32_t T, int32_t H,
+                              int mean, void *A, cudaStream_t s, int *launches);
+cudaError_t launch_hub_rows(const void *P, const int32_t *hub_ids, int32_t H, int32_t pw, void *BT,
+                            cudaStream_t s, int *launches);
 
 // ---- walks.cu: importance-based neighbourhoods by simulated random walks ------------------------
 // walk_slots: shared-memory key slots per node (0 = n_walks * walk_len outside [1, 2048]).

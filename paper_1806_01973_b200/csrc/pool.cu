@@ -169,7 +169,7 @@ __device__ __forceinline__ void gather_fma(const uint4 *__restrict__ P, int my_i
 template <bool BF16, int LPN, int CPL, int U, bool EXACT, int MODE>
 __global__ void __launch_bounds__(256, (CPL <= 2) ? 4 : 2)
 pool_kernel(const uint4 *__restrict__ P, const int *__restrict__ idx, const float *__restrict__ w,
-            uint4 *__restrict__ out, long long n_dst, int T, int chunks)
+            uint4 *__restrict__ out, long long n_dst, int T, int chunks, int skip_neg)
 {
     using C = Chunk<BF16>;
     constexpr int NPW = 32 / LPN;
@@ -198,7 +198,21 @@ pool_kernel(const uint4 *__restrict__ P, const int *__restrict__ idx, const floa
             my_i = ld_stream_i32(irow + t);
             if (MODE == 0) my_w = ld_stream_f32(wrow + t);
         }
-        const int cnt = min(LPN, T - tb);
+        int cnt = min(LPN, T - tb);
+        if (skip_neg) {
+            // entries with a negative id (hub neighbours, summed by the hub GEMM: hubs.cu) are squeezed
+            // out of this batch: lane k of a node's group takes the k-th remaining entry.  Groups of
+            // one warp run the same number of steps (the shuffles below are warp-wide); a group that
+            // has fewer entries pads with weight 0 on row 0.
+            const unsigned live = __ballot_sync(0xffffffffu, t < T && my_i >= 0);
+            const unsigned gm = LPN == 32 ? live : (live >> (lane / LPN * LPN)) & ((1u << (LPN & 31)) - 1u);
+            const unsigned src = __fns(gm, 0, sl + 1);             // position of the (sl+1)-th live entry
+            const int ci = __shfl_sync(0xffffffffu, my_i, src & (LPN - 1), LPN);
+            const float cw = __shfl_sync(0xffffffffu, my_w, src & (LPN - 1), LPN);
+            my_i = src != 0xffffffffu ? ci : 0;
+            my_w = src != 0xffffffffu ? cw : 0.f;
+            cnt = __reduce_max_sync(0xffffffffu, __popc(gm));
+        }
         int j0 = 0;
         for (; j0 + U <= cnt; j0 += U)
             gather_fma<BF16, LPN, CPL, U, EXACT, MODE>(P, my_i, my_w, j0, sl, chunks, acc);
@@ -217,7 +231,7 @@ pool_kernel(const uint4 *__restrict__ P, const int *__restrict__ idx, const floa
 
 template <bool BF16, int LPN, int CPL, int U, int MODE>
 cudaError_t run_pool(const void *P, const int *idx, const float *w, void *out, long long n_dst,
-                     int T, int chunks, cudaStream_t s)
+                     int T, int chunks, cudaStream_t s, int skip_neg = 0)
 {
     constexpr int NPW = 32 / LPN;
     const long long warps = (n_dst + NPW - 1) / NPW;
@@ -225,10 +239,10 @@ cudaError_t run_pool(const void *P, const int *idx, const float *w, void *out, l
     if (blocks > 0x7fffffffLL) return cudaErrorInvalidConfiguration;
     if (chunks == LPN * CPL)
         pool_kernel<BF16, LPN, CPL, U, true, MODE><<<(unsigned)blocks, 256, 0, s>>>(
-            static_cast<const uint4 *>(P), idx, w, static_cast<uint4 *>(out), n_dst, T, chunks);
+            static_cast<const uint4 *>(P), idx, w, static_cast<uint4 *>(out), n_dst, T, chunks, skip_neg);
     else
         pool_kernel<BF16, LPN, CPL, U, false, MODE><<<(unsigned)blocks, 256, 0, s>>>(
-            static_cast<const uint4 *>(P), idx, w, static_cast<uint4 *>(out), n_dst, T, chunks);
+            static_cast<const uint4 *>(P), idx, w, static_cast<uint4 *>(out), n_dst, T, chunks, skip_neg);
     return cudaGetLastError();
 }
 
@@ -328,15 +342,15 @@ cudaError_t dispatch_pool_slab(int slab_bytes, const void *P, const int *idx, co
 
 template <bool BF16, int MODE>
 cudaError_t dispatch_pool(const void *P, const int *idx, const float *w, void *out,
-                          long long n_dst, int T, int chunks, cudaStream_t s)
+                          long long n_dst, int T, int chunks, cudaStream_t s, int skip_neg = 0)
 {
-    if (chunks <= 4) return run_pool<BF16, 4, 1, 4, MODE>(P, idx, w, out, n_dst, T, chunks, s);
-    if (chunks <= 8) return run_pool<BF16, 8, 1, 8, MODE>(P, idx, w, out, n_dst, T, chunks, s);
-    if (chunks <= 16) return run_pool<BF16, 16, 1, 8, MODE>(P, idx, w, out, n_dst, T, chunks, s);
-    if (chunks <= 32) return run_pool<BF16, 32, 1, 8, MODE>(P, idx, w, out, n_dst, T, chunks, s);
-    if (chunks <= 64) return run_pool<BF16, 32, 2, 4, MODE>(P, idx, w, out, n_dst, T, chunks, s);
-    if (chunks <= 128) return run_pool<BF16, 32, 4, 4, MODE>(P, idx, w, out, n_dst, T, chunks, s);
-    if (chunks <= 256) return run_pool<BF16, 32, 8, 1, MODE>(P, idx, w, out, n_dst, T, chunks, s);
+    if (chunks <= 4) return run_pool<BF16, 4, 1, 4, MODE>(P, idx, w, out, n_dst, T, chunks, s, skip_neg);
+    if (chunks <= 8) return run_pool<BF16, 8, 1, 8, MODE>(P, idx, w, out, n_dst, T, chunks, s, skip_neg);
+    if (chunks <= 16) return run_pool<BF16, 16, 1, 8, MODE>(P, idx, w, out, n_dst, T, chunks, s, skip_neg);
+    if (chunks <= 32) return run_pool<BF16, 32, 1, 8, MODE>(P, idx, w, out, n_dst, T, chunks, s, skip_neg);
+    if (chunks <= 64) return run_pool<BF16, 32, 2, 4, MODE>(P, idx, w, out, n_dst, T, chunks, s, skip_neg);
+    if (chunks <= 128) return run_pool<BF16, 32, 4, 4, MODE>(P, idx, w, out, n_dst, T, chunks, s, skip_neg);
+    if (chunks <= 256) return run_pool<BF16, 32, 8, 1, MODE>(P, idx, w, out, n_dst, T, chunks, s, skip_neg);
     return cudaErrorNotSupported;
 }
 
@@ -401,11 +415,16 @@ bool pool_slab_ok(DType dt, int32_t T, int32_t m, int slab_bytes)
 
 cudaError_t launch_pool(DType dt, int mode, int64_t n_dst, int32_t T, int32_t m, const void *P,
                         const int32_t *idx, const float *w, void *out, int slab_bytes, cudaStream_t s,
-                        int *launches)
+                        int *launches, int skip_neg)
 {
     if (n_dst <= 0) return cudaSuccess;
     const int chunks = (int)((size_t)m * elem_size(dt) / 16);
     if (launches) ++*launches;
+    if (skip_neg) {                            // hub-split pool: importance pooling, whole rows
+        if (mode != 0) return cudaErrorNotSupported;
+        return dt == DType::BF16 ? dispatch_pool<true, 0>(P, idx, w, out, n_dst, T, chunks, s, 1)
+                                 : dispatch_pool<false, 0>(P, idx, w, out, n_dst, T, chunks, s, 1);
+    }
     if (mode != 0)
         return dt == DType::BF16 ? dispatch_pool_mode<true>(mode, P, idx, w, out, n_dst, T, chunks, s)
                                  : dispatch_pool_mode<false>(mode, P, idx, w, out, n_dst, T, chunks, s);

@@ -1,0 +1,104 @@
+"""Parity of the hub-split pool (option ``pool_hubs``; hubs.cu): on a power-law graph the entries of the
+neighbour lists that point at the few hundred most listed nodes are summed by a tensor-core GEMM, the
+rest by the gather kernel.  Same function as Algorithm 1 line 1 in real arithmetic;
+checked against the fp64 oracle on sampled destinations (Algorithm 2 on their K-hop closure) and against
+the plain pool on every row."""
+import numpy as np
+import pytest
+import torch
+
+from oracle import oracle as O
+from paper_1806_01973_b200 import binding, synth
+from tests.parity import assert_rows_close, params_f64, row_errors, to_f64
+
+pytestmark = pytest.mark.gpu
+DEV = "cuda:0"
+
+
+@pytest.fixture(scope="module")
+def ctx():
+    c = binding.Context(0)
+    yield c
+    c.close()
+
+
+def _setup(cfg):
+    X = synth.make_features(cfg, device=DEV)
+    layers, head = synth.make_params(cfg, device=DEV)
+    idx, counts = synth.make_graph(cfg, device=DEV)
+    return X, layers, head, idx, counts
+
+
+def _oracle_rows(X, idx, alpha, layers, head, rows):
+    Lf, Hf = params_f64([{k: v.cpu() for k, v in lp.items()} for lp in layers], {k: v.cpu() for k, v in head.items()})
+
+    def fetch_x(ids):
+        t = torch.from_numpy(np.asarray(ids, dtype=np.int64)).to(DEV)
+        return X[t].to(torch.float64).cpu().numpy()
+
+    def fetch_nbr(ids):
+        t = torch.from_numpy(np.asarray(ids, dtype=np.int64)).to(DEV)
+        return idx[t].cpu().numpy(), alpha[t].cpu().numpy()
+
+    return O.minibatch_embed(rows, fetch_x, fetch_nbr, Lf, Hf)
+
+
+@pytest.mark.parametrize("hubs", [256, 64, -1])
+def test_power_law_graph_with_hub_split_pool(ctx, hubs):
+    cfg = synth.CONFIGS["cfg4"].scaled(150_000)
+    X, layers, head, idx, counts = _setup(cfg)
+    alpha = ctx.pinsage_normalize_counts(counts)
+    plain = ctx.pinsage_embed_all(X, idx, alpha, layers, head, chunk_nodes=65536)
+    l0 = ctx.pinsage_launch_count()
+    ctx.pinsage_embed_all(X, idx, alpha, layers, head, chunk_nodes=65536)
+    plain_launches = ctx.pinsage_launch_count() - l0
+    ctx.pinsage_set_option("pool_hubs", hubs)
+    try:
+        l0 = ctx.pinsage_launch_count()
+        out = ctx.pinsage_embed_all(X, idx, alpha, layers, head, chunk_nodes=65536)
+        hub_launches = ctx.pinsage_launch_count() - l0
+    finally:
+        ctx.pinsage_set_option("pool_hubs", 0)
+    torch.cuda.synchronize()
+    assert hub_launches > plain_launches + 4, "the hub path did not run"
+    # the lists really are dominated by a few ids (what the path is for)
+    share = float((idx < 256).float().mean())
+    assert share > 0.3, share
+    rows = np.concatenate([[0, 1, 255, 256, cfg.N - 1], np.random.default_rng(3).integers(0, cfg.N, 123)])
+    ref = _oracle_rows(X, idx, alpha, layers, head, rows)
+    t = torch.from_numpy(rows).to(DEV)
+    assert_rows_close(to_f64(out[t]), ref, torch.bfloat16, f"hub-split pool H={hubs} vs oracle")
+    assert_rows_close(to_f64(plain[t]), ref, torch.bfloat16, "plain pool vs oracle")
+    rel, cos = row_errors(to_f64(out), to_f64(plain))
+    assert rel.max() <= 1e-2 and cos.min() >= 0.999, (rel.max(), cos.min())
+
+
+def test_uniform_graph_finds_no_hubs(ctx):
+    """No id reaches the candidate threshold on a uniform graph: forced on, the remapped table equals the
+    original and the hub GEMM adds zero -> bit-identical output; automatic -> the path is not taken."""
+    cfg = synth.CONFIGS["cfg2"].scaled(120_000)
+    X, layers, head, idx, counts = _setup(cfg)
+    alpha = ctx.pinsage_normalize_counts(counts)
+    plain = ctx.pinsage_embed_all(X, idx, alpha, layers, head)
+    l0 = ctx.pinsage_launch_count()
+    ctx.pinsage_embed_all(X, idx, alpha, layers, head)
+    plain_launches = ctx.pinsage_launch_count() - l0
+    for hubs in (128, -1):
+        ctx.pinsage_set_option("pool_hubs", hubs)
+        try:
+            l0 = ctx.pinsage_launch_count()
+            out = ctx.pinsage_embed_all(X, idx, alpha, layers, head)
+            n = ctx.pinsage_launch_count() - l0
+        finally:
+            ctx.pinsage_set_option("pool_hubs", 0)
+        assert torch.equal(out.view(torch.int16), plain.view(torch.int16))
+        if hubs == -1:
+            assert n == plain_launches + 3          # histogram, candidates, selection -- and nothing else
+        else:
+            assert n > plain_launches + 4
+
+
+def test_pool_hubs_option_values(ctx):
+    for bad in (1, 63, 576, -2):
+        with pytest.raises(binding.PinsageError):
+            ctx.pinsage_set_option("pool_hubs", bad)
