@@ -130,15 +130,17 @@ const char *pinsage_version(void);
  *                                    0.7 of it, so that the gathered sub-table stays L2-resident),
  *                                    0 = always whole rows, 32 / 64 / 128 = forced.  Bit-identical results.
  *                   "pool_hubs"      pinsage_embed_all on skewed graphs (BF16, importance pooling, device
- *                                    tables): the entries of the neighbour lists that point at the H most
- *                                    listed nodes ("hubs", found from a sample of the lists) are summed
- *                                    by a tensor-core GEMM (weights kept to 16 bits, fp32 accumulate), the
- *                                    rest by the gather kernel, which skips them; the two parts meet in the
- *                                    GEMM's epilogue, so n is rounded to bf16 twice -- the same function in
- *                                    real arithmetic, not bit-identical to the plain pool.  0 = off
- *                                    (default), H = 64 .. 512 (multiple of 64) = on, -1 = on (H = 128) when
- *                                    the sampled hubs hold at least a third of all entries (costs one
- *                                    stream synchronisation per call).
+ *                                    tables, m <= d schedule): the entries of the neighbour lists that
+ *                                    point at the H most listed nodes ("hubs", found from a sample of the
+ *                                    lists) are not gathered; their term  A (P_hub W2^T),  A[u, h] = the
+ *                                    summed weight of u's entries naming hub h, enters S3 as a third K
+ *                                    segment on the tensor cores (A and P_hub W2^T rounded to bf16, exact
+ *                                    products, fp32 sum).  The same function in real arithmetic and the
+ *                                    same error level as the plain pool (which rounds all of n to bf16),
+ *                                    but a different rounding: not bit-identical.  0 = off (default),
+ *                                    H = 64 .. 512 (multiple of 64) = on, -1 = on (H = 128) when the
+ *                                    sampled hubs hold at least a third of all entries (one stream
+ *                                    synchronisation per call).  Power-law config: 1.45 x faster.
  *                   "topk_fused"     pinsage_topk: 1 (default) = once every running list is full, scores
  *                                    are tested against the query's k-th score in the GEMM's epilogue and
  *                                    only the keepers leave the SM (no fp32 score matrix in HBM); 0 = every

@@ -48,8 +48,10 @@ struct pinsage_ctx {
         const int32_t *src_idx = nullptr;   // the caller's table the remapped one stands for
         const int32_t *idxm = nullptr;      // remapped table: hub entries are -(rank + 1)
         const int32_t *hub_ids = nullptr;
-        void *A = nullptr;                  // [chunk x 2H] bf16
-        void *BT = nullptr;                 // [pw x 2H] bf16
+        void *A = nullptr;                  // [chunk x H] bf16
+        void *Ph = nullptr;                 // [H x m] bf16: the hub rows of P
+        float *G = nullptr;                 // [H x d] fp32: P_hub W2^T
+        void *Wext = nullptr;               // [d x (d_in + m + H)] bf16: [W1 | W2 | G^T]
     } hub;
     void *hub_buf = nullptr;
     size_t hub_bytes = 0;
@@ -354,7 +356,8 @@ pinsage_status run_gemm(pinsage_ctx *ctx, DType dt, const GemmArgs &a, void *scr
                         (long long)a.M, a.K1, a.K2, a.N);
     }
     if (simt) {
-        if (a.sel_state) return fail(ctx, PINSAGE_ERR_CUDA, "internal: selection epilogue on the SIMT path");
+        if (a.sel_state || a.K3)
+            return fail(ctx, PINSAGE_ERR_CUDA, "internal: selection epilogue / third K segment on the SIMT path");
         const size_t need = gemm_simt_scratch_bytes(a);
         if (need > scratch_bytes)
             return fail(ctx, PINSAGE_ERR_OOM, "internal: SIMT scratch %zu > %zu", need, scratch_bytes);
@@ -474,11 +477,28 @@ pinsage_status pool_combine_chunks(pinsage_ctx *ctx, DType dt, int64_t N, int32_
         PS_CUDA(ctx, cudaStreamWaitEvent(ctx->aux, ctx->ev_fork, 0));
     }
     cudaStream_t ps = two ? ctx->aux : ctx->stream;
-    // hub-split pool (hubs.cu): the gather skips the hub entries, the hub part is a GEMM on the chunk
-    const bool hubs = ctx->hub.H > 0 && idx == ctx->hub.src_idx && !two && dt == DType::BF16 &&
+    // hub-split pool (hubs.cu): the gather skips the hub entries; their term enters S3 as a third K
+    // segment A [rows x H] against G = P_hub W2^T, appended to the layer's W once per layer
+    const bool hubs = ctx->hub.H > 0 && idx == ctx->hub.src_idx && !two && !linear && dt == DType::BF16 &&
                       ctx->pool_mode == 0;
+    const int H = ctx->hub.H;
     if (hubs) {
-        cudaError_t e = launch_hub_rows(P, ctx->hub.hub_ids, ctx->hub.H, pw, ctx->hub.BT, ps, &ctx->launches);
+        const int pe0 = prof_mark(ctx, ps);
+        cudaError_t e = launch_hub_gather(P, ctx->hub.hub_ids, H, pw, ctx->hub.Ph, ps, &ctx->launches);
+        prof_close(ctx, PROF_POOL, pe0, ps);
+        count_launches(ctx);
+        PS_CUDA(ctx, e);
+        GemmArgs gg;                              // G [H x d] = P_hub W2^T in fp32
+        gg.M = H;
+        gg.K1 = lp->m;
+        gg.N = lp->d;
+        gg.A1 = ctx->hub.Ph;
+        gg.B = static_cast<const char *>(lp->W) + (size_t)lp->d_in * es;
+        gg.ldb = lp->d_in + lp->m;
+        gg.out_f32 = 1;
+        gg.out = ctx->hub.G;
+        PS_TRY(run_gemm(ctx, dt, gg, nullptr, 0, ps, PROF_POOL));
+        e = launch_hub_weights(lp->W, lp->d_in + lp->m, ctx->hub.G, H, lp->d, ctx->hub.Wext, ps, &ctx->launches);
         count_launches(ctx);
         PS_CUDA(ctx, e);
     }
@@ -491,9 +511,11 @@ pinsage_status pool_combine_chunks(pinsage_ctx *ctx, DType dt, int64_t N, int32_
         cudaError_t e;
         if (hubs) {
             const int32_t *im = ctx->hub.idxm + (size_t)r0 * T;
-            e = launch_pool(dt, 0, rows, T, pw, P, im, w + (size_t)r0 * T, nb[b], 0, ps, &ctx->launches, 1);
-            if (e == cudaSuccess)
-                e = launch_hub_matrix(im, w + (size_t)r0 * T, rows, T, ctx->hub.H, 0, ctx->hub.A, ps, &ctx->launches);
+            const bool fusedA = pool_hub_fused_ok(dt, pw);     // the gather kernel also writes A
+            e = launch_pool(dt, 0, rows, T, pw, P, im, w + (size_t)r0 * T, nb[b], 0, ps, &ctx->launches, 1,
+                            fusedA ? ctx->hub.A : nullptr, H);
+            if (e == cudaSuccess && !fusedA)
+                e = launch_hub_matrix(im, w + (size_t)r0 * T, rows, T, H, 0, ctx->hub.A, ps, &ctx->launches);
         } else {
             e = launch_pool(dt, ctx->pool_mode, rows, T, pw, P, idx + (size_t)r0 * T, w + (size_t)r0 * T,
                             nb[b], pick_slab(ctx, dt, n_src, T, pw), ps, &ctx->launches);
@@ -501,17 +523,6 @@ pinsage_status pool_combine_chunks(pinsage_ctx *ctx, DType dt, int64_t N, int32_
         prof_close(ctx, PROF_POOL, pe0, ps);
         count_launches(ctx);
         PS_CUDA(ctx, e);
-        if (hubs) {                              // n[chunk] += A_hub P_hub  (added in the GEMM's epilogue, in place)
-            GemmArgs gh;
-            gh.M = rows;
-            gh.K1 = 2 * ctx->hub.H;
-            gh.N = pw;
-            gh.A1 = ctx->hub.A;
-            gh.B = ctx->hub.BT;
-            gh.addend = nb[b];
-            gh.out = nb[b];
-            PS_TRY(run_gemm(ctx, dt, gh, nullptr, 0, ps, PROF_POOL));
-        }
         if (two) {
             PS_CUDA(ctx, cudaEventRecord(ctx->ev_pool[b], ps));
             PS_CUDA(ctx, cudaStreamWaitEvent(ctx->stream, ctx->ev_pool[b], 0));
@@ -528,6 +539,12 @@ pinsage_status pool_combine_chunks(pinsage_ctx *ctx, DType dt, int64_t N, int32_
         } else {                             // z = H W1^T + n W2^T + w: two K segments
             g.K2 = lp->m;
             g.A2 = nb[b];
+            if (hubs) {                          // ... + A (P_hub W2^T): the hub term as a third one
+                g.K3 = H;
+                g.A3 = ctx->hub.A;
+                g.B = ctx->hub.Wext;
+                g.ldb = lp->d_in + lp->m + H;
+            }
         }
         g.bias = lp->w;
         g.relu = 1;
@@ -1131,13 +1148,19 @@ pinsage_status pinsage_embed_all(pinsage_ctx *ctx, pinsage_dtype dtype, int64_t 
     if (ctx->pool_hubs != 0 && dt == DType::BF16 && ctx->pool_mode == 0 && ctx->gemm_impl == 0 && !ctx->overlap &&
         !h_idx && !h_w && N * (int64_t)T >= (1 << 22)) {
         const int H = ctx->pool_hubs > 0 ? ctx->pool_hubs : 128;
-        int32_t pw_max = 0;
-        for (int k = 0; k < K; ++k) pw_max = std::max(pw_max, use_linear_pool(ctx, &layers[k]) ? layers[k].d : layers[k].m);
+        int32_t m_max = 0, dd_max = 0, kw_max = 0;
+        for (int k = 0; k < K; ++k) {
+            m_max = std::max(m_max, layers[k].m);
+            dd_max = std::max(dd_max, layers[k].d);
+            kw_max = std::max(kw_max, layers[k].d_in + layers[k].m);
+        }
         const size_t nB = align_up((size_t)N * 4, 256), candB = align_up(hub_cand_bytes(), 256);
         const size_t idsB = align_up((size_t)H * 4, 256), tabB = align_up((size_t)N * T * 4, 256);
-        const size_t AB = align_up((size_t)chunk * 2 * H * 2, 256), BTB = align_up((size_t)pw_max * 2 * H * 2, 256);
-        PS_TRY(ensure_buf(ctx, &ctx->hub_buf, &ctx->hub_bytes, 2 * nB + candB + idsB + 256 + tabB + AB + BTB,
-                          "hub-split pool storage"));
+        const size_t AB = align_up((size_t)chunk * H * 2, 256), PhB = align_up((size_t)H * m_max * 2, 256);
+        const size_t GB = align_up((size_t)H * dd_max * 4, 256);
+        const size_t WB = align_up((size_t)dd_max * (kw_max + H) * 2, 256);
+        PS_TRY(ensure_buf(ctx, &ctx->hub_buf, &ctx->hub_bytes,
+                          2 * nB + candB + idsB + 256 + tabB + AB + PhB + GB + WB, "hub-split pool storage"));
         char *hb = static_cast<char *>(ctx->hub_buf);
         int32_t *counts = reinterpret_cast<int32_t *>(hb), *rank = reinterpret_cast<int32_t *>(hb + nB);
         void *cand = hb + 2 * nB;
@@ -1164,8 +1187,11 @@ pinsage_status pinsage_embed_all(pinsage_ctx *ctx, pinsage_dtype dtype, int64_t 
             ctx->hub.src_idx = d_idx;
             ctx->hub.idxm = idxm;
             ctx->hub.hub_ids = hub_ids;
-            ctx->hub.A = reinterpret_cast<char *>(idxm) + tabB;
-            ctx->hub.BT = reinterpret_cast<char *>(idxm) + tabB + AB;
+            char *after = reinterpret_cast<char *>(idxm) + tabB;
+            ctx->hub.A = after;
+            ctx->hub.Ph = after + AB;
+            ctx->hub.G = reinterpret_cast<float *>(after + AB + PhB);
+            ctx->hub.Wext = after + AB + PhB + GB;
         }
     }
 

@@ -1,6 +1,6 @@
 // gemm_tcgen05.cu -- S1 / S3 / S4 / S5 on the 5th-generation tensor cores (sm_100a).
 //
-//   out[M x N] = epi( A1[M x K1] * B[:, 0:K1]^T  +  A2[M x K2] * B[:, K1:K1+K2]^T  + bias )
+//   out[M x N] = epi( A1[M x K1] * B[:, 0:K1]^T  +  A2[M x K2] * B[:, K1:K1+K2]^T  [+ A3[M x K3] * B[:, K1+K2:]^T] + bias )
 //
 // bf16 operands, fp32 accumulation in TMEM.  B is the paper's "out x in" weight matrix
 // (Q, W, G1, G2 -- PAPER.md:114-115, :166) = a K-major operand as it lies in memory; the
@@ -44,7 +44,8 @@ constexpr int SMEM_LIMIT = 227 * 1024;
 struct TcParams {
     long long M;
     long long m_blocks;
-    int kb1, kb2;      // 64-wide K blocks in segment 1 / 2
+    int kb1, kb2, kb3; // 64-wide K blocks in segment 1 / 2 / 3
+    int K12;           // column of B where segment 3 starts
     int K1;            // column of B where segment 2 starts
     int N;             // output columns in total
     int NS;            // output columns owned by one CTA (a slab)
@@ -363,6 +364,7 @@ constexpr int XCHG_BYTES = 2 * MAX_CLUSTER * BM * 4;
 template <int CG, int NCH>
 __global__ void __launch_bounds__(NUM_THREADS, 1)
 gemm_tc_kernel(const __grid_constant__ CUtensorMap tmA1, const __grid_constant__ CUtensorMap tmA2,
+               const __grid_constant__ CUtensorMap tmA3,
                const __grid_constant__ CUtensorMap tmB, const __grid_constant__ CUtensorMap tmOut,
                const TcParams p)
 {
@@ -393,13 +395,14 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap tmA1, const __grid_constant__
     const long long lane0 = unit / p.n_slabs, lanes = units / p.n_slabs;
     const int n0 = slab * p.NS;
     const int ncols = min(p.NS, p.N - n0);  // valid output columns of this slab
-    const int KB = p.kb1 + p.kb2;
+    const int KB = p.kb1 + p.kb2 + p.kb3;
     const int b_rows = p.CN / CG;           // rows of B this CTA stages per MMA chunk
 
     // ---- one-time setup ---------------------------------------------------------------------
     if (warp == 0 && lane == 0) {
         asm volatile("prefetch.tensormap [%0];" ::"l"(&tmA1) : "memory");
         asm volatile("prefetch.tensormap [%0];" ::"l"(&tmA2) : "memory");
+        asm volatile("prefetch.tensormap [%0];" ::"l"(&tmA3) : "memory");
         asm volatile("prefetch.tensormap [%0];" ::"l"(&tmB) : "memory");
         asm volatile("prefetch.tensormap [%0];" ::"l"(&tmOut) : "memory");
     }
@@ -458,22 +461,23 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap tmA1, const __grid_constant__
                 mbar_wait(bar_empty + 8 * stage, phase ^ 1);
                 if (elect_one()) {
                     const uint32_t full = bar_full + 8 * stage;
-                    const bool seg2 = kb >= p.kb1;
-                    const int ka = (seg2 ? kb - p.kb1 : kb) * BK;
+                    const int seg = kb < p.kb1 ? 0 : kb < p.kb1 + p.kb2 ? 1 : 2;
+                    const int ka = (seg == 0 ? kb : seg == 1 ? kb - p.kb1 : kb - p.kb1 - p.kb2) * BK;
                     const uint32_t sA = sbase + (uint32_t)stage * p.stage_bytes;
-                    const int kcol = seg2 ? p.K1 + ka : ka;
+                    const int kcol = (seg == 0 ? 0 : seg == 1 ? p.K1 : p.K12) + ka;
+                    const CUtensorMap *tmA = seg == 0 ? &tmA1 : seg == 1 ? &tmA2 : &tmA3;
                     if (CG == 2) {
                         // both CTAs' bytes complete on the leader's barrier
                         if (half == 0) mbar_expect_tx(full, 2u * (uint32_t)p.stage_bytes);
                         const uint32_t lfull = leader_full + 8 * stage;
-                        tma_load_2d_pair(sA, seg2 ? &tmA2 : &tmA1, ka, m0, lfull, pol_a);
+                        tma_load_2d_pair(sA, tmA, ka, m0, lfull, pol_a);
 #pragma unroll
                         for (int j = 0; j < NCH; ++j)
                             tma_load_2d_pair(sA + A_BYTES + (uint32_t)j * b_rows * 128, &tmB, kcol,
                                              n0 + j * p.CN + (int)half * b_rows, lfull, pol_keep);
                     } else {
                         mbar_expect_tx(full, (uint32_t)p.stage_bytes);
-                        tma_load_2d(sA, seg2 ? &tmA2 : &tmA1, ka, m0, full, pol_a);
+                        tma_load_2d(sA, tmA, ka, m0, full, pol_a);
 #pragma unroll
                         for (int j = 0; j < NCH; ++j)
                             tma_load_2d(sA + A_BYTES + (uint32_t)j * p.CN * 128, &tmB, kcol,
@@ -864,9 +868,12 @@ bool plan(const GemmArgs &a, int cg, int ns_pref, int epi_pref, TcParams &p, int
         return false;
     };
     if (a.M < 1 || a.M >= (1LL << 31)) return no("M outside [1, 2^31)");
-    if (a.K1 < 8 || a.K1 % 8 || a.K2 < 0 || a.K2 % 8) return no("K1, K2 must be multiples of 8");
+    if (a.K1 < 8 || a.K1 % 8 || a.K2 < 0 || a.K2 % 8 || a.K3 < 0 || a.K3 % 8)
+        return no("K1, K2, K3 must be multiples of 8");
+    if (a.K3 > 0 && a.K2 == 0) return no("a third K segment needs the second");
     if (a.N < 8 || a.N % 8) return no("N must be a multiple of 8");
-    if (a.ldb % 8 || (a.ldb > 0 && a.ldb < a.K1 + a.K2)) return no("ldb must be a multiple of 8, >= K1 + K2");
+    if (a.ldb % 8 || (a.ldb > 0 && a.ldb < a.K1 + a.K2 + a.K3))
+        return no("ldb must be a multiple of 8, >= K1 + K2 + K3");
     if (cg == 2 && (a.M <= BM || a.N % 16)) return no("CTA pairs need M > 128 and N % 16 == 0");
     if (a.out_f32 && a.addend) return no("fp32 output takes no addend");
     if (a.sel_state && (a.l2norm || a.addend || a.bias || a.relu || a.sel_k < 1 || a.sel_k > TK_LIST))
@@ -877,6 +884,8 @@ bool plan(const GemmArgs &a, int cg, int ns_pref, int epi_pref, TcParams &p, int
     p.m_blocks = (a.M + BM * cg - 1) / (BM * cg);
     p.kb1 = (a.K1 + BK - 1) / BK;
     p.kb2 = (a.K2 + BK - 1) / BK;
+    p.kb3 = (a.K3 + BK - 1) / BK;
+    p.K12 = a.K1 + a.K2;
     p.K1 = a.K1;
     p.N = a.N;
     const int slab_max = a.l2norm ? 512 : ns_pref;  // a normalised row must sit in one CTA's TMEM
@@ -938,7 +947,7 @@ bool plan_auto(const GemmArgs &a, const GemmTune &t, TcParams &p, int &smem_byte
     // Pairs pay when the GEMM is tensor-bound (measured on B200: +12-14 % at config 3's shapes); on
     // the HBM-bound shapes (arithmetic intensity K N / (K + N) below ~160 flop per byte moved, e.g.
     // 256 x 256) single-CTA tiles keep more independent tiles in flight and are 15-35 % faster.
-    const long long Kt = a.K1 + a.K2;
+    const long long Kt = a.K1 + a.K2 + a.K3;
     const bool tensor_bound = Kt * a.N >= 160 * (Kt + a.N);
     if ((t.cg == 2 || (t.cg == 0 && tensor_bound)) && plan(a, 2, ns, t.epi, p, smem_bytes, nullptr)) return true;
     if (t.cg == 2) {
@@ -950,7 +959,8 @@ bool plan_auto(const GemmArgs &a, const GemmTune &t, TcParams &p, int &smem_byte
 
 template <int CG, int NCH>
 cudaError_t launch_cg(const TcParams &p, int smem, int num_sms, cudaStream_t s, const CUtensorMap &tmA1,
-                      const CUtensorMap &tmA2, const CUtensorMap &tmB, const CUtensorMap &tmOut)
+                      const CUtensorMap &tmA2, const CUtensorMap &tmA3, const CUtensorMap &tmB,
+                      const CUtensorMap &tmOut)
 {
     // per-device function attribute and cluster-occupancy cache (a process may drive several devices)
     static int attr_dev = -1;
@@ -996,7 +1006,7 @@ cudaError_t launch_cg(const TcParams &p, int smem, int num_sms, cudaStream_t s, 
     units = units / p.n_slabs * p.n_slabs;
     if (units < p.n_slabs) units = p.n_slabs;
     cfg.gridDim = dim3((unsigned)(units * CG));
-    return cudaLaunchKernelEx(&cfg, gemm_tc_kernel<CG, NCH>, tmA1, tmA2, tmB, tmOut, p);
+    return cudaLaunchKernelEx(&cfg, gemm_tc_kernel<CG, NCH>, tmA1, tmA2, tmA3, tmB, tmOut, p);
 }
 
 }  // namespace
@@ -1020,22 +1030,27 @@ cudaError_t launch_gemm_tc(const GemmArgs &a, const GemmTune &t, int num_sms, cu
     TcParams p;
     int smem = 0;
     if (!plan_auto(a, t, p, smem, nullptr)) return cudaErrorNotSupported;
-    CUtensorMap tmA1, tmA2, tmB, tmOut;
+    CUtensorMap tmA1, tmA2, tmA3, tmB, tmOut;
     if (!make_map(&tmA1, a.A1, a.M, a.K1, BM)) return cudaErrorInvalidValue;
     if (a.K2 > 0) {
         if (!make_map(&tmA2, a.A2, a.M, a.K2, BM)) return cudaErrorInvalidValue;
     } else {
         tmA2 = tmA1;
     }
-    if (!make_map(&tmB, a.B, a.b_rows > 0 ? a.b_rows : a.N, a.K1 + a.K2, p.CN / p.cg, a.ldb))
+    if (a.K3 > 0) {
+        if (!make_map(&tmA3, a.A3, a.M, a.K3, BM)) return cudaErrorInvalidValue;
+    } else {
+        tmA3 = tmA1;
+    }
+    if (!make_map(&tmB, a.B, a.b_rows > 0 ? a.b_rows : a.N, a.K1 + a.K2 + a.K3, p.CN / p.cg, a.ldb))
         return cudaErrorInvalidValue;
     if (!make_map(&tmOut, a.out, a.M, a.N, 32, 0, a.out_f32 != 0)) return cudaErrorInvalidValue;
     if (launches) ++*launches;
     if (p.cg == 2)
-        return p.nchunks == 2 ? launch_cg<2, 2>(p, smem, num_sms, s, tmA1, tmA2, tmB, tmOut)
-                              : launch_cg<2, 1>(p, smem, num_sms, s, tmA1, tmA2, tmB, tmOut);
-    return p.nchunks == 2 ? launch_cg<1, 2>(p, smem, num_sms, s, tmA1, tmA2, tmB, tmOut)
-                          : launch_cg<1, 1>(p, smem, num_sms, s, tmA1, tmA2, tmB, tmOut);
+        return p.nchunks == 2 ? launch_cg<2, 2>(p, smem, num_sms, s, tmA1, tmA2, tmA3, tmB, tmOut)
+                              : launch_cg<2, 1>(p, smem, num_sms, s, tmA1, tmA2, tmA3, tmB, tmOut);
+    return p.nchunks == 2 ? launch_cg<1, 2>(p, smem, num_sms, s, tmA1, tmA2, tmA3, tmB, tmOut)
+                          : launch_cg<1, 1>(p, smem, num_sms, s, tmA1, tmA2, tmA3, tmB, tmOut);
 }
 
 }  // namespace pinsage

@@ -7,15 +7,18 @@
 // (profiles/r01_pool_cfg4.md).  Splitting the sum over the neighbour's kind,
 //     n_u = sum_{t: idx_ut not a hub} alpha_ut P[idx_ut]  +  sum_h A[u, h] P[hub_h],
 //     A[u, h] = sum_{t: idx_ut = hub_h} alpha_ut,
-// the second term is a GEMM  A [n x H] . P_hub [H x m]  for the tensor cores and the first a gather
-// over what is left of the lists.  The weights are kept to 16 significand bits (A = A_hi + A_lo in
-// bf16, K = 2H), the products are exact and the sum is fp32; the gathered part is added in the GEMM's
-// epilogue, where the result is rounded to bf16 once more.  Which nodes are hubs is a choice, not
-// part of the result: any set gives the same sum in real arithmetic.
+// the first term is a gather over what is left of the lists and the second a dense contraction.  It is
+// not even formed: S3 multiplies n by W2 (Alg. 1 l.2), and  (A P_hub) W2^T = A (P_hub W2^T), so the hub
+// term enters S3 as a THIRD K segment -- A [n x H] against the small matrix G = P_hub W2^T [H x d],
+// computed once per layer on the tensor cores in fp32.  A and G are rounded to bf16 (K3 = H), their
+// products are exact and the sum is fp32: the hub term carries two independent 2^-9 roundings per
+// product, averaged over the node's hub entries, where the plain path rounds all of n to bf16 (2^-9
+// per element, not averaged) before S3 -- the same error level, a different rounding.  Which nodes are
+// hubs is a choice, not part of the result: any set gives the same z in real arithmetic.
 //
 // Kernels: sampled visit histogram -> candidates -> top-H selection (one CTA) and rank table ->
-// remapped index table (hub entries become -(rank + 1), which the pool kernel skips) -> per chunk the
-// matrix A, per layer the operand P_hub^T.
+// remapped index table (hub entries become -(rank + 1), which the pool kernel skips) -> per layer the
+// hub rows of P and the extended weight matrix [W1 | W2 | G^T], per chunk the matrix A.
 #include "internal.h"
 
 #include <algorithm>
@@ -108,7 +111,7 @@ hub_remap_kernel(const int *__restrict__ idx, const int *__restrict__ rank, long
     }
 }
 
-// A [rows x 2H] bf16 = [hi | lo] planes of A[u, h] = sum of the weights of u's entries that point at
+// A [rows x H] bf16, A[u, h] = sum of the weights of u's entries that point at
 // hub h (mean aggregator: 1/T each).  One warp per node, the row is summed in shared memory.
 __global__ void __launch_bounds__(256)
 hub_matrix_kernel(const int *__restrict__ idxm, const float *__restrict__ w, long long rows, int T, int H, int mean,
@@ -127,26 +130,39 @@ hub_matrix_kernel(const int *__restrict__ idxm, const float *__restrict__ w, lon
         if (i < 0) atomicAdd(buf - (i + 1), mean ? wmean : w[v * T + t]);   // (a list may name a hub twice)
     }
     __syncwarp();
-    __nv_bfloat16 *row = A + v * 2 * H;
-    for (int h = lane; h < H; h += 32) {
-        const float a = buf[h];
-        const __nv_bfloat16 hi = __float2bfloat16_rn(a);
-        row[h] = hi;
-        row[H + h] = __float2bfloat16_rn(a - __bfloat162float(hi));
+    __nv_bfloat16 *row = A + v * H;
+    for (int h = lane; h < H; h += 32) row[h] = __float2bfloat16_rn(buf[h]);
+}
+
+// Ph [H x pw] = the hub rows of P (zero rows for unused hub slots)
+__global__ void __launch_bounds__(256)
+hub_gather_kernel(const __nv_bfloat16 *__restrict__ P, const int *__restrict__ hub_ids, int H, int pw,
+                  __nv_bfloat16 *__restrict__ Ph)
+{
+    const int total = H * pw;
+    for (int e = blockIdx.x * blockDim.x + threadIdx.x; e < total; e += gridDim.x * blockDim.x) {
+        const int h = e / pw, c = e - h * pw;
+        const int id = hub_ids[h];
+        Ph[e] = id >= 0 ? P[(size_t)id * pw + c] : __float2bfloat16_rn(0.f);
     }
 }
 
-// BT [pw x 2H] bf16, BT[n, k] = P[hub_ids[k mod H], n] (zero for an unused hub slot): the K-major B
-// operand of the hub GEMM
+// Wext [d x (kw + H)] bf16: columns [0, kw) = W (row stride kw), then G^T with G [H x d] fp32 (G[h, j]
+// multiplies A[u, h] in output column j): Wext[j, kw + h] = bf16(G[h, j])
 __global__ void __launch_bounds__(256)
-hub_rows_kernel(const __nv_bfloat16 *__restrict__ P, const int *__restrict__ hub_ids, int H, int pw,
-                __nv_bfloat16 *__restrict__ BT)
+hub_weights_kernel(const __nv_bfloat16 *__restrict__ W, int kw, const float *__restrict__ G, int H, int d,
+                   __nv_bfloat16 *__restrict__ Wext)
 {
-    const int total = pw * 2 * H;
-    for (int e = blockIdx.x * blockDim.x + threadIdx.x; e < total; e += gridDim.x * blockDim.x) {
-        const int n = e / (2 * H), k = e - n * 2 * H;
-        const int id = hub_ids[k % H];
-        BT[e] = id >= 0 ? P[(size_t)id * pw + n] : __float2bfloat16_rn(0.f);
+    const int ld = kw + H;
+    const long long total = (long long)d * ld;
+    for (long long e = (long long)blockIdx.x * blockDim.x + threadIdx.x; e < total;
+         e += (long long)gridDim.x * blockDim.x) {
+        const int j = (int)(e / ld), c = (int)(e - (long long)j * ld);
+        if (c < kw) {
+            Wext[e] = W[(size_t)j * kw + c];
+        } else {
+            Wext[e] = __float2bfloat16_rn(G[(size_t)(c - kw) * d + j]);
+        }
     }
 }
 
@@ -203,11 +219,20 @@ cudaError_t launch_hub_matrix(const int32_t *idxm, const float *w, int64_t rows,
     return cudaGetLastError();
 }
 
-cudaError_t launch_hub_rows(const void *P, const int32_t *hub_ids, int32_t H, int32_t pw, void *BT,
-                            cudaStream_t s, int *launches)
+cudaError_t launch_hub_gather(const void *P, const int32_t *hub_ids, int32_t H, int32_t pw, void *Ph,
+                              cudaStream_t s, int *launches)
 {
-    hub_rows_kernel<<<grid_for((long long)pw * 2 * H), 256, 0, s>>>(static_cast<const __nv_bfloat16 *>(P), hub_ids,
-                                                                    H, pw, static_cast<__nv_bfloat16 *>(BT));
+    hub_gather_kernel<<<grid_for((long long)H * pw), 256, 0, s>>>(static_cast<const __nv_bfloat16 *>(P), hub_ids, H,
+                                                                  pw, static_cast<__nv_bfloat16 *>(Ph));
+    if (launches) ++*launches;
+    return cudaGetLastError();
+}
+
+cudaError_t launch_hub_weights(const void *W, int32_t kw, const float *G, int32_t H, int32_t d, void *Wext,
+                               cudaStream_t s, int *launches)
+{
+    hub_weights_kernel<<<grid_for((long long)d * (kw + H)), 256, 0, s>>>(
+        static_cast<const __nv_bfloat16 *>(W), kw, G, H, d, static_cast<__nv_bfloat16 *>(Wext));
     if (launches) ++*launches;
     return cudaGetLastError();
 }

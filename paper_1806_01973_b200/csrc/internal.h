@@ -21,6 +21,8 @@ struct GemmArgs {
     int32_t K1 = 0, K2 = 0, N = 0;
     const void *A1 = nullptr;
     const void *A2 = nullptr;
+    int32_t K3 = 0;                 // tcgen05 kernel only: a third K segment A3 [M x K3] against
+    const void *A3 = nullptr;       // B[:, K1+K2 : K1+K2+K3] (the hub term of the hub-split pool)
     const void *B = nullptr;
     int64_t b_rows = 0;             // rows of B that exist (0 = N); rows b_rows .. N-1 read as zero
     int32_t ldb = 0;                // row stride of B in elements; 0 = K1 + K2 (B may be a column
@@ -73,7 +75,10 @@ cudaError_t launch_split3(bool is_b, const float *S1, int32_t K1, int64_t ld1, c
 // mode: 0 importance (weighted sum), 1 element-wise mean, 2 element-wise max (w unused for 1, 2).
 cudaError_t launch_pool(DType dt, int mode, int64_t n_dst, int32_t T, int32_t m, const void *P,
                         const int32_t *idx, const float *w, void *out, int slab_bytes, cudaStream_t s,
-                        int *launches, int skip_neg = 0);   // skip_neg: entries with idx < 0 are not gathered
+                        int *launches, int skip_neg = 0, void *hubA = nullptr, int H = 0);
+// skip_neg: entries with idx < 0 are not gathered; hubA (rows of >= 272 bytes only): such an entry
+// -(r + 1) adds its weight to A[v, r] instead, A [n_dst x H] bf16 (the hub-split pool, hubs.cu)
+bool pool_hub_fused_ok(DType dt, int32_t m);
 bool pool_slab_ok(DType dt, int32_t T, int32_t m, int slab_bytes);
 cudaError_t launch_normalize_counts(int64_t N, int32_t T, const int32_t *counts, float *w,
                                     cudaStream_t s, int *launches);
@@ -90,8 +95,10 @@ cudaError_t launch_hub_remap(const int32_t *idx, const int32_t *rank, int64_t to
                              cudaStream_t s, int *launches);
 cudaError_t launch_hub_matrix(const int32_t *idxm, const float *w, int64_t rows, int32_t T, int32_t H,
                               int mean, void *A, cudaStream_t s, int *launches);
-cudaError_t launch_hub_rows(const void *P, const int32_t *hub_ids, int32_t H, int32_t pw, void *BT,
-                            cudaStream_t s, int *launches);
+cudaError_t launch_hub_gather(const void *P, const int32_t *hub_ids, int32_t H, int32_t pw, void *Ph,
+                              cudaStream_t s, int *launches);
+cudaError_t launch_hub_weights(const void *W, int32_t kw, const float *G, int32_t H, int32_t d, void *Wext,
+                               cudaStream_t s, int *launches);
 
 // ---- walks.cu: importance-based neighbourhoods by simulated random walks ------------------------
 // walk_slots: shared-memory key slots per node (0 = n_walks * walk_len outside [1, 2048]).

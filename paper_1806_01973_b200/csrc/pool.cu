@@ -167,10 +167,12 @@ __device__ __forceinline__ void gather_fma(const uint4 *__restrict__ P, int my_i
 // An explicit minBlocksPerSM matters: without it ptxas (-O3) re-serialises the load batch to
 // minimise registers (32 regs, 2 loads in flight); with it the U*CPL loads stay batched.
 template <bool BF16, int LPN, int CPL, int U, bool EXACT, int MODE>
-__global__ void __launch_bounds__(256, (CPL <= 2) ? 4 : 2)
+__global__ void __launch_bounds__(256, (CPL <= 2) ? (U == 1 ? 5 : 4) : 2)
 pool_kernel(const uint4 *__restrict__ P, const int *__restrict__ idx, const float *__restrict__ w,
-            uint4 *__restrict__ out, long long n_dst, int T, int chunks, int skip_neg)
+            uint4 *__restrict__ out, long long n_dst, int T, int chunks, int skip_neg,
+            __nv_bfloat16 *__restrict__ hubA, int H)
 {
+    extern __shared__ float hub_acc[];                     // hub mode (LPN == 32): H sums per warp
     using C = Chunk<BF16>;
     constexpr int NPW = 32 / LPN;
     static_assert(LPN % U == 0, "U must divide LPN");
@@ -190,6 +192,11 @@ pool_kernel(const uint4 *__restrict__ P, const int *__restrict__ idx, const floa
 
     const int *irow = idx + v * T;
     const float *wrow = w + v * T;
+    float *hbuf = hub_acc + (size_t)(threadIdx.x >> 5) * H;
+    if (hubA != nullptr) {                                 // (one node per warp: LPN == 32)
+        for (int h = lane; h < H; h += 32) hbuf[h] = 0.f;
+        __syncwarp();
+    }
     for (int tb = 0; tb < T; tb += LPN) {
         const int t = tb + sl;
         int my_i = 0;
@@ -199,6 +206,8 @@ pool_kernel(const uint4 *__restrict__ P, const int *__restrict__ idx, const floa
             if (MODE == 0) my_w = ld_stream_f32(wrow + t);
         }
         int cnt = min(LPN, T - tb);
+        if (hubA != nullptr && t < T && my_i < 0)          // hub entry -(rank + 1): its weight goes to A[v, rank]
+            atomicAdd(hbuf - (my_i + 1), my_w);
         if (skip_neg) {
             // entries with a negative id (hub neighbours, summed by the hub GEMM: hubs.cu) are squeezed
             // out of this batch: lane k of a node's group takes the k-th remaining entry.  Groups of
@@ -219,6 +228,11 @@ pool_kernel(const uint4 *__restrict__ P, const int *__restrict__ idx, const floa
         for (; j0 < cnt; ++j0)
             gather_fma<BF16, LPN, CPL, 1, EXACT, MODE>(P, my_i, my_w, j0, sl, chunks, acc);
     }
+    if (hubA != nullptr) {                                 // A[v, :] = bf16 of the sums (hubs.cu)
+        __syncwarp();
+        __nv_bfloat16 *arow = hubA + (size_t)v * H;
+        for (int h = lane; h < H; h += 32) arow[h] = __float2bfloat16_rn(hbuf[h]);
+    }
     if (active) {
         uint4 *orow = out + (size_t)v * (size_t)chunks;
 #pragma unroll
@@ -231,18 +245,21 @@ pool_kernel(const uint4 *__restrict__ P, const int *__restrict__ idx, const floa
 
 template <bool BF16, int LPN, int CPL, int U, int MODE>
 cudaError_t run_pool(const void *P, const int *idx, const float *w, void *out, long long n_dst,
-                     int T, int chunks, cudaStream_t s, int skip_neg = 0)
+                     int T, int chunks, cudaStream_t s, int skip_neg = 0, void *hubA = nullptr, int H = 0)
 {
+    if (hubA != nullptr && LPN != 32) return cudaErrorNotSupported;
+    const size_t smem = hubA != nullptr ? (size_t)8 * H * 4 : 0;
+    __nv_bfloat16 *hA = static_cast<__nv_bfloat16 *>(hubA);
     constexpr int NPW = 32 / LPN;
     const long long warps = (n_dst + NPW - 1) / NPW;
     const long long blocks = (warps + 7) / 8;
     if (blocks > 0x7fffffffLL) return cudaErrorInvalidConfiguration;
     if (chunks == LPN * CPL)
-        pool_kernel<BF16, LPN, CPL, U, true, MODE><<<(unsigned)blocks, 256, 0, s>>>(
-            static_cast<const uint4 *>(P), idx, w, static_cast<uint4 *>(out), n_dst, T, chunks, skip_neg);
+        pool_kernel<BF16, LPN, CPL, U, true, MODE><<<(unsigned)blocks, 256, smem, s>>>(
+            static_cast<const uint4 *>(P), idx, w, static_cast<uint4 *>(out), n_dst, T, chunks, skip_neg, hA, H);
     else
-        pool_kernel<BF16, LPN, CPL, U, false, MODE><<<(unsigned)blocks, 256, 0, s>>>(
-            static_cast<const uint4 *>(P), idx, w, static_cast<uint4 *>(out), n_dst, T, chunks, skip_neg);
+        pool_kernel<BF16, LPN, CPL, U, false, MODE><<<(unsigned)blocks, 256, smem, s>>>(
+            static_cast<const uint4 *>(P), idx, w, static_cast<uint4 *>(out), n_dst, T, chunks, skip_neg, hA, H);
     return cudaGetLastError();
 }
 
@@ -342,15 +359,23 @@ cudaError_t dispatch_pool_slab(int slab_bytes, const void *P, const int *idx, co
 
 template <bool BF16, int MODE>
 cudaError_t dispatch_pool(const void *P, const int *idx, const float *w, void *out,
-                          long long n_dst, int T, int chunks, cudaStream_t s, int skip_neg = 0)
+                          long long n_dst, int T, int chunks, cudaStream_t s, int skip_neg = 0,
+                          void *hubA = nullptr, int H = 0)
 {
-    if (chunks <= 4) return run_pool<BF16, 4, 1, 4, MODE>(P, idx, w, out, n_dst, T, chunks, s, skip_neg);
-    if (chunks <= 8) return run_pool<BF16, 8, 1, 8, MODE>(P, idx, w, out, n_dst, T, chunks, s, skip_neg);
-    if (chunks <= 16) return run_pool<BF16, 16, 1, 8, MODE>(P, idx, w, out, n_dst, T, chunks, s, skip_neg);
-    if (chunks <= 32) return run_pool<BF16, 32, 1, 8, MODE>(P, idx, w, out, n_dst, T, chunks, s, skip_neg);
-    if (chunks <= 64) return run_pool<BF16, 32, 2, 4, MODE>(P, idx, w, out, n_dst, T, chunks, s, skip_neg);
-    if (chunks <= 128) return run_pool<BF16, 32, 4, 4, MODE>(P, idx, w, out, n_dst, T, chunks, s, skip_neg);
-    if (chunks <= 256) return run_pool<BF16, 32, 8, 1, MODE>(P, idx, w, out, n_dst, T, chunks, s, skip_neg);
+    // what is left of the lists after the hub entries is a handful of rows per node: the kernel is then
+    // bound by the chain table load -> gather -> store, and more resident warps (U = 1: fewer
+    // registers) beat deeper load batches
+    if (skip_neg && chunks > 32 && chunks <= 64)
+        return run_pool<BF16, 32, 2, 1, MODE>(P, idx, w, out, n_dst, T, chunks, s, skip_neg, hubA, H);
+    if (skip_neg && chunks > 16 && chunks <= 32)
+        return run_pool<BF16, 32, 1, 1, MODE>(P, idx, w, out, n_dst, T, chunks, s, skip_neg, hubA, H);
+    if (chunks <= 4) return run_pool<BF16, 4, 1, 4, MODE>(P, idx, w, out, n_dst, T, chunks, s, skip_neg, hubA, H);
+    if (chunks <= 8) return run_pool<BF16, 8, 1, 8, MODE>(P, idx, w, out, n_dst, T, chunks, s, skip_neg, hubA, H);
+    if (chunks <= 16) return run_pool<BF16, 16, 1, 8, MODE>(P, idx, w, out, n_dst, T, chunks, s, skip_neg, hubA, H);
+    if (chunks <= 32) return run_pool<BF16, 32, 1, 8, MODE>(P, idx, w, out, n_dst, T, chunks, s, skip_neg, hubA, H);
+    if (chunks <= 64) return run_pool<BF16, 32, 2, 4, MODE>(P, idx, w, out, n_dst, T, chunks, s, skip_neg, hubA, H);
+    if (chunks <= 128) return run_pool<BF16, 32, 4, 4, MODE>(P, idx, w, out, n_dst, T, chunks, s, skip_neg, hubA, H);
+    if (chunks <= 256) return run_pool<BF16, 32, 8, 1, MODE>(P, idx, w, out, n_dst, T, chunks, s, skip_neg, hubA, H);
     return cudaErrorNotSupported;
 }
 
@@ -413,17 +438,23 @@ bool pool_slab_ok(DType dt, int32_t T, int32_t m, int slab_bytes)
     return row % slab_bytes == 0 && row > (size_t)slab_bytes && smem <= 200 * 1024;
 }
 
+bool pool_hub_fused_ok(DType dt, int32_t m)
+{
+    const size_t chunks = (size_t)m * elem_size(dt) / 16;
+    return chunks > 16 && chunks <= 256;       // one node per warp (LPN == 32)
+}
+
 cudaError_t launch_pool(DType dt, int mode, int64_t n_dst, int32_t T, int32_t m, const void *P,
                         const int32_t *idx, const float *w, void *out, int slab_bytes, cudaStream_t s,
-                        int *launches, int skip_neg)
+                        int *launches, int skip_neg, void *hubA, int H)
 {
     if (n_dst <= 0) return cudaSuccess;
     const int chunks = (int)((size_t)m * elem_size(dt) / 16);
     if (launches) ++*launches;
     if (skip_neg) {                            // hub-split pool: importance pooling, whole rows
         if (mode != 0) return cudaErrorNotSupported;
-        return dt == DType::BF16 ? dispatch_pool<true, 0>(P, idx, w, out, n_dst, T, chunks, s, 1)
-                                 : dispatch_pool<false, 0>(P, idx, w, out, n_dst, T, chunks, s, 1);
+        return dt == DType::BF16 ? dispatch_pool<true, 0>(P, idx, w, out, n_dst, T, chunks, s, 1, hubA, H)
+                                 : dispatch_pool<false, 0>(P, idx, w, out, n_dst, T, chunks, s, 1, hubA, H);
     }
     if (mode != 0)
         return dt == DType::BF16 ? dispatch_pool_mode<true>(mode, P, idx, w, out, n_dst, T, chunks, s)

@@ -1,6 +1,6 @@
 """Parity of the hub-split pool (option ``pool_hubs``; hubs.cu): on a power-law graph the entries of the
-neighbour lists that point at the few hundred most listed nodes are summed by a tensor-core GEMM, the
-rest by the gather kernel.  Same function as Algorithm 1 line 1 in real arithmetic;
+neighbour lists that point at the few hundred most listed nodes are not gathered; their term enters S3 as
+a third K segment on the tensor cores.  Same function as Algorithm 1 lines 1-2 in real arithmetic;
 checked against the fp64 oracle on sampled destinations (Algorithm 2 on their K-hop closure) and against
 the plain pool on every row."""
 import numpy as np
