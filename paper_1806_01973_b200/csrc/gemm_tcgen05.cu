@@ -127,10 +127,6 @@ __device__ __forceinline__ uint32_t map_to_cta(uint32_t local_addr, uint32_t cta
     asm volatile("mapa.shared::cluster.u32 %0, %1, %2;" : "=r"(r) : "r"(local_addr), "r"(cta_rank));
     return r;
 }
-__device__ __forceinline__ void st_cluster_f32(uint32_t cluster_addr, float v)
-{
-    asm volatile("st.shared::cluster.f32 [%0], %1;" ::"r"(cluster_addr), "f"(v) : "memory");
-}
 // One fp32 to a peer CTA's shared memory, completing 4 bytes of the transaction count of a barrier in
 // that CTA: data and signal travel together, so the sender needs no release fence (a st.shared::cluster
 // followed by a release.cluster arrive costs a MEMBAR.ALL.GPU per thread and tile).
@@ -139,11 +135,6 @@ __device__ __forceinline__ void st_async_f32(uint32_t cluster_addr, float v, uin
     asm volatile("st.async.weak.shared::cluster.mbarrier::complete_tx::bytes.b32 [%0], %1, [%2];" ::"r"(
                      cluster_addr),
                  "r"(__float_as_uint(v)), "r"(cluster_bar)
-                 : "memory");
-}
-__device__ __forceinline__ void mbar_arrive_remote(uint32_t cluster_addr)
-{
-    asm volatile("mbarrier.arrive.release.cluster.shared::cluster.b64 _, [%0];" ::"r"(cluster_addr)
                  : "memory");
 }
 // The "accumulator drained" signal carries no memory data (the TMEM reads are ordered by
@@ -411,7 +402,6 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap tmA1, const __grid_constant__
             mbar_init(bar_full + 8 * s, 1);
             mbar_init(bar_empty + 8 * s, 1);
         }
-        const int units_per_cluster = p.cluster / CG;
         for (int a = 0; a < 2; ++a) {
             mbar_init(bar_tfull + 8 * a, 1);
             mbar_init(bar_tempty + 8 * a, 4 * CG * p.epi_halves);  // every epilogue warp of the unit

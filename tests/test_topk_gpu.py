@@ -122,3 +122,41 @@ def test_topk_argument_errors(ctx):
     with pytest.raises(binding.PinsageError) as e:
         ctx.pinsage_topk(Q, Zb, 2000)
     assert e.value.status_name == "UNSUPPORTED_SHAPE"
+
+
+def test_topk_full_size_sampled(ctx):
+    """The shape topk_bench times (K = 500 among 5 million candidates; 4 096 queries,
+    d = 1024, bf16), in the launch configuration it times (88 candidate blocks, 87 of them through the
+    GEMM's selection epilogue).  Sampled queries are checked against fp64 scores computed on the host
+    from the stored bf16 values, block of candidates by block of candidates (numpy), then ordered as
+    the oracle orders (score descending, id ascending)."""
+    free, _ = torch.cuda.mem_get_info(0)
+    if free < 30e9:
+        pytest.skip("needs 30 GB of free HBM")
+    nq, N, d, k = 4096, 5_000_000, 1024, 500
+    g = torch.Generator(device=DEV).manual_seed(0)
+    Z = torch.empty((N, d), dtype=torch.bfloat16, device=DEV)
+    for s in range(0, N, 1 << 20):
+        e = min(N, s + (1 << 20))
+        z = torch.randn((e - s, d), generator=g, device=DEV)
+        Z[s:e] = (z / z.norm(dim=1, keepdim=True)).to(torch.bfloat16)
+    Q = Z[torch.randint(0, N, (nq,), generator=g, device=DEV)].clone()
+    idx, score = ctx.pinsage_topk(Q, Z, k)
+    torch.cuda.synchronize()
+    sample = [0, 1, 777, 2048, 4095]
+    Qs = to_f64(Q[sample])
+    S = np.empty((len(sample), N))
+    for s in range(0, N, 500_000):
+        e = min(N, s + 500_000)
+        S[:, s:e] = Qs @ to_f64(Z[s:e]).T
+    idx, score = idx[sample].cpu().numpy(), score[sample].cpu().numpy().astype(np.float64)
+    tol = 4e-6                                           # fp32 accumulation of d = 1024 products, |score| <= 1
+    for q in range(len(sample)):
+        np.testing.assert_allclose(score[q], S[q, idx[q]], atol=tol)
+        assert len(set(idx[q])) == k and np.all(np.diff(score[q]) <= 0)
+        order = np.lexsort((np.arange(N), -S[q]))[:k + 50]            # the oracle's order
+        kth = S[q, order[k - 1]]
+        assert np.all(S[q, idx[q]] >= kth - tol)
+        must = order[:k][S[q, order[:k]] > kth + tol]
+        assert np.isin(must, idx[q]).all()
+        assert idx[q, 0] == order[0]
