@@ -109,6 +109,10 @@ const char *pinsage_version(void);
  *                                    M > 128, N % 16 == 0; default), 1 = single CTAs
  *                                    (128-row tiles) only, 2 = CTA pairs or PINSAGE_ERR_UNSUPPORTED_SHAPE
  *                   "gemm_ns"        slab width of GEMMs without a row norm: 0 / 256 (default) or 512
+ *                   "gemm_nl"        slab width of the row-norm GEMM (S3): 0 / 512 (default) = one TMEM
+ *                                    accumulator per CTA, 256 = two (the epilogue overlaps the next tile's
+ *                                    MMAs; clusters twice as large).  Measured: S3 -9 % at d = 512, no
+ *                                    change at d = 1024 (8-CTA clusters fill only 128 of the 148 SMs).
  *                   "gemm_epi"       epilogue warps: 0 = eight for single-accumulator row-norm tiles (default),
  *                                    1 = always four, 2 = eight wherever they fit (measured slower)
  *                   "check_indices"  1 = every pinsage_pool / layer / embed_all call validates

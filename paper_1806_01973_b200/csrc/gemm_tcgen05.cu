@@ -851,7 +851,8 @@ inline int round_up(int x, int a) { return (x + a - 1) / a * a; }
 
 // cg: CTAs per tile (1 or 2).  ns_pref: preferred slab width without a row norm (256 = double-buffered
 // accumulators, 512 = fewer operand bytes per flop but no epilogue overlap).
-bool plan(const GemmArgs &a, int cg, int ns_pref, int epi_pref, TcParams &p, int &smem_bytes, const char **why)
+bool plan(const GemmArgs &a, int cg, int ns_pref, int epi_pref, int nl_pref, TcParams &p, int &smem_bytes,
+          const char **why)
 {
     auto no = [&](const char *msg) {
         if (why) *why = msg;
@@ -878,7 +879,9 @@ bool plan(const GemmArgs &a, int cg, int ns_pref, int epi_pref, TcParams &p, int
     p.K12 = a.K1 + a.K2;
     p.K1 = a.K1;
     p.N = a.N;
-    const int slab_max = a.l2norm ? 512 : ns_pref;  // a normalised row must sit in one CTA's TMEM
+    // a normalised row sits in the TMEM of one cluster: slabs of 512 columns (one accumulator), or of 256
+    // (two accumulators: the epilogue overlaps the next tile, at the price of a larger cluster)
+    const int slab_max = a.l2norm ? (nl_pref == 256 ? 256 : 512) : ns_pref;
     p.n_slabs = (a.N + slab_max - 1) / slab_max;
     p.NS = p.n_slabs == 1 ? round_up(a.N, 16) : round_up((a.N + p.n_slabs - 1) / p.n_slabs, 64);
     p.n_slabs = (a.N + p.NS - 1) / p.NS;
@@ -939,12 +942,12 @@ bool plan_auto(const GemmArgs &a, const GemmTune &t, TcParams &p, int &smem_byte
     // 256 x 256) single-CTA tiles keep more independent tiles in flight and are 15-35 % faster.
     const long long Kt = a.K1 + a.K2 + a.K3;
     const bool tensor_bound = Kt * a.N >= 160 * (Kt + a.N);
-    if ((t.cg == 2 || (t.cg == 0 && tensor_bound)) && plan(a, 2, ns, t.epi, p, smem_bytes, nullptr)) return true;
+    if ((t.cg == 2 || (t.cg == 0 && tensor_bound)) && plan(a, 2, ns, t.epi, t.nl, p, smem_bytes, nullptr)) return true;
     if (t.cg == 2) {
         if (why) *why = "shape not supported by the CTA-pair kernel";
         return false;
     }
-    return plan(a, 1, ns, t.epi, p, smem_bytes, why);
+    return plan(a, 1, ns, t.epi, t.nl, p, smem_bytes, why);
 }
 
 template <int CG, int NCH>

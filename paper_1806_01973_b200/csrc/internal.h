@@ -57,6 +57,7 @@ struct GemmTune {
     int cg = 0;
     int ns = 0;
     int epi = 0;   // epilogue warps: 0 = automatic (8 when they fit), 1 = always 4
+    int nl = 0;    // slab width of row-norm GEMMs: 0 / 512 = one accumulator per CTA, 256 = two
 };
 // Returns cudaErrorNotSupported for shapes outside the compiled set (caller reports UNSUPPORTED_SHAPE).
 bool gemm_tc_supported(const GemmArgs &a, const GemmTune &t, const char **why);
