@@ -1377,6 +1377,18 @@ pinsage_status pinsage_topk(pinsage_ctx *ctx, pinsage_dtype dtype, int64_t nq, i
     PS_TRY(check_ptr(ctx, "Z", Z));
     PS_TRY(check_ptr(ctx, "out_idx", out_idx));
     PS_TRY(check_ptr(ctx, "out_score", out_score));
+    // many queries: groups of 16 384, so that the candidate blocks stay wide (>= 16 384 candidates
+    // per GEMM) and the per-block bookkeeping small; the groups are independent lookups
+    constexpr int64_t Q_GROUP = 16384;
+    if (nq > Q_GROUP) {
+        const size_t esz = elem_size(static_cast<DType>(dtype));
+        for (int64_t q0 = 0; q0 < nq; q0 += Q_GROUP) {
+            const int64_t n = std::min(Q_GROUP, nq - q0);
+            PS_TRY(pinsage_topk(ctx, dtype, n, N, d, static_cast<const char *>(Q) + (size_t)q0 * d * esz, Z, k,
+                                out_idx + (size_t)q0 * k, out_score + (size_t)q0 * k));
+        }
+        return PINSAGE_OK;
+    }
     const DType dt = static_cast<DType>(dtype);
     const size_t es = elem_size(dt);
     // candidate block: as wide as keeps the fp32 score block within 1 GiB, a multiple of 256, <= 65536

@@ -160,3 +160,16 @@ def test_topk_full_size_sampled(ctx):
         must = order[:k][S[q, order[:k]] > kth + tol]
         assert np.isin(must, idx[q]).all()
         assert idx[q, 0] == order[0]
+
+
+def test_topk_many_queries_in_groups(ctx):
+    """More queries than one group (16 384): the groups are independent lookups with the same result."""
+    nq, N, d, k = 40_000, 30_011, 16, 20
+    g = torch.Generator().manual_seed(9)
+    Q = torch.randint(-2, 3, (nq, d), generator=g).to(torch.bfloat16)
+    Z = torch.randint(-2, 3, (N, d), generator=g).to(torch.bfloat16)
+    idx, score = ctx.pinsage_topk(Q.to(DEV), Z.to(DEV), k)
+    pick = np.r_[0, 16383, 16384, 32767, 32768, nq - 1, np.random.default_rng(1).integers(0, nq, 200)]
+    ref_idx, ref_score = O.topk(to_f64(Q[pick]), to_f64(Z), k)
+    np.testing.assert_array_equal(idx.cpu().numpy()[pick], ref_idx)
+    np.testing.assert_array_equal(score.cpu().numpy().astype(np.float64)[pick], ref_score)
