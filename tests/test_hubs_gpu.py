@@ -102,3 +102,29 @@ def test_pool_hubs_option_values(ctx):
     for bad in (1, 63, 576, -2):
         with pytest.raises(binding.PinsageError):
             ctx.pinsage_set_option("pool_hubs", bad)
+
+
+@pytest.mark.parametrize("d0,hidden,T,hubs,chunk", [(264, 264, 37, 64, 30_000), (136, 520, 50, 512, 0),
+                                                     (512, 128, 64, 128, 50_048)])
+def test_hub_split_pool_odd_shapes(ctx, d0, hidden, T, hubs, chunk):
+    """Widths that are not multiples of 64 (ragged K blocks in all three S3 segments, inexact row
+    chunks in the gather), a row narrow enough for two nodes per warp (hidden = 128: the separate
+    matrix kernel), T beyond one 32-entry batch, ragged driver chunks."""
+    import dataclasses
+    cfg = dataclasses.replace(synth.CONFIGS["cfg4"].scaled(130_003), d0=d0, hidden=hidden, g1=hidden, d_out=64, T=T)
+    X, layers, head, idx, counts = _setup(cfg)
+    alpha = ctx.pinsage_normalize_counts(counts)
+    plain = ctx.pinsage_embed_all(X, idx, alpha, layers, head, chunk_nodes=chunk)
+    ctx.pinsage_set_option("pool_hubs", hubs)
+    try:
+        out = ctx.pinsage_embed_all(X, idx, alpha, layers, head, chunk_nodes=chunk)
+    finally:
+        ctx.pinsage_set_option("pool_hubs", 0)
+    torch.cuda.synchronize()
+    rows = np.concatenate([[0, 1, hubs - 1, hubs, cfg.N - 1], np.random.default_rng(5).integers(0, cfg.N, 59)])
+    ref = _oracle_rows(X, idx, alpha, layers, head, rows)
+    t = torch.from_numpy(rows).to(DEV)
+    assert_rows_close(to_f64(out[t]), ref, torch.bfloat16, "hub-split pool vs oracle")
+    rel, cos = row_errors(to_f64(out), to_f64(plain))
+    assert rel.max() <= 1e-2 and cos.min() >= 0.999, (rel.max(), cos.min())
+    assert not torch.equal(out.view(torch.int16), plain.view(torch.int16)), "the hub path did not run"
