@@ -71,6 +71,7 @@ struct TcParams {
     // appended to q's candidate buffer.  sel_nb = valid columns (candidates sel_id0 + column).
     unsigned long long *sel_state;
     int *sel_cnt;
+    int tile_major;        // see the unit decode in the kernel
     int sel_k, sel_nb;
     long long sel_id0;
     uint32_t idesc;
@@ -382,8 +383,13 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap tmA1, const __grid_constant__
     const uint32_t half = CG == 2 ? (crank & 1u) : 0u;         // which 128 rows of the 256-row tile
     const uint32_t leader = crank & ~1u;                       // cluster rank of this pair's even CTA
     const long long unit = blockIdx.x / CG, units = gridDim.x / CG;
-    const int slab = (int)(unit % p.n_slabs);
-    const long long lane0 = unit / p.n_slabs, lanes = units / p.n_slabs;
+    // Persistent schedule: a unit keeps its slab and walks the row tiles lane0, lane0 + lanes, ...
+    // Tile-major schedule (p.tile_major; one tile per unit, row tile fastest): the units resident at
+    // one time then share a few slabs of B instead of holding one each -- for long K with many slabs,
+    // where the slabs in flight would not fit L2 and each would be re-read from HBM per row tile.
+    const int slab = p.tile_major ? (int)(unit / p.m_blocks) : (int)(unit % p.n_slabs);
+    const long long lane0 = p.tile_major ? unit % p.m_blocks : unit / p.n_slabs;
+    const long long lanes = p.tile_major ? p.m_blocks : units / p.n_slabs;
     const int n0 = slab * p.NS;
     const int ncols = min(p.NS, p.N - n0);  // valid output columns of this slab
     const int KB = p.kb1 + p.kb2 + p.kb3;
@@ -924,6 +930,10 @@ bool plan(const GemmArgs &a, int cg, int ns_pref, int epi_pref, int nl_pref, TcP
     p.sel_k = a.sel_k;
     p.sel_nb = (int)(a.b_rows ? a.b_rows : a.N);
     p.sel_id0 = a.sel_id0;
+    // slabs in flight (one per resident unit) against half of L2; only without per-slab state (bias,
+    // row-norm exchange), i.e. the top-K lookup's products
+    p.tile_major = !a.l2norm && !a.bias && p.n_slabs > 148 / cg && p.m_blocks > 1 &&
+                   (long long)(148 / cg) * p.NS * (a.K1 + a.K2 + a.K3) * 2 > (48LL << 20);
     p.relu = a.relu;
     p.l2norm = a.l2norm;
     // instruction descriptor, kind::f16: D fp32 (bit 4), A and B bf16 (bits 7, 10), both K-major,
@@ -998,6 +1008,7 @@ cudaError_t launch_cg(const TcParams &p, int smem, int num_sms, cudaStream_t s, 
     if (units > tiles) units = tiles;
     units = units / p.n_slabs * p.n_slabs;
     if (units < p.n_slabs) units = p.n_slabs;
+    if (p.tile_major) units = tiles;
     cfg.gridDim = dim3((unsigned)(units * CG));
     return cudaLaunchKernelEx(&cfg, gemm_tc_kernel<CG, NCH>, tmA1, tmA2, tmA3, tmB, tmOut, p);
 }
