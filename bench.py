@@ -243,6 +243,7 @@ def run_ours(args, cfg):
     ctx.pinsage_set_option("gemm_epi", args.gemm_epi)
     ctx.pinsage_set_option("pool_slab", args.pool_slab)
     ctx.pinsage_set_option("gemm_nl", args.gemm_nl)
+    ctx.pinsage_set_option("gemm_gx", args.gemm_gx)
     if args.pool_hubs is not None:
         ctx.pinsage_set_option("pool_hubs", args.pool_hubs)
     ctx.pinsage_set_option("linear_pool", args.linear_pool)
@@ -398,6 +399,7 @@ def main():
     ap.add_argument("--gemm-epi", type=int, default=0, help="0 auto (8 epilogue warps), 1 four")
     ap.add_argument("--linear-pool", type=int, default=-1, help="-1 auto (m > d), 0 off, 1 on")
     ap.add_argument("--pool-slab", type=int, default=-1, help="-1 auto, 0 whole rows, 32/64/128")
+    ap.add_argument("--gemm-gx", type=int, default=1, help="0: row norms of wide S3 exchanged inside a cluster")
     ap.add_argument("--gemm-nl", type=int, default=0, help="row-norm GEMM slab width: 0/512 or 256")
     ap.add_argument("--pool-hubs", type=int, default=None,
                     help="hub-split pool: 0 off, -1 automatic, 64..512 forced (default: the library's)")

@@ -109,6 +109,13 @@ const char *pinsage_version(void);
  *                                    M > 128, N % 16 == 0; default), 1 = single CTAs
  *                                    (128-row tiles) only, 2 = CTA pairs or PINSAGE_ERR_UNSUPPORTED_SHAPE
  *                   "gemm_ns"        slab width of GEMMs without a row norm: 0 / 256 (default) or 512
+ *                   "gemm_gx"        row-norm GEMM (S3) wider than 512 columns: 1 (default) = 256-column
+ *                                    slabs with two TMEM accumulators each, the CTA pairs that hold the
+ *                                    slabs of one row tile exchange their partial row norms through global
+ *                                    memory (cooperative launch: the grid is co-resident by construction),
+ *                                    so the epilogue hides behind the next tile's MMAs and 144 of 148 SMs
+ *                                    work; 0 = 512-column slabs exchanged inside a 4-CTA cluster (132 SMs,
+ *                                    exposed epilogue).  S3 at d = 1024: 1.21-1.25 -> 1.45-1.50 PFLOP/s.
  *                   "gemm_nl"        slab width of the row-norm GEMM (S3): 0 / 512 (default) = one TMEM
  *                                    accumulator per CTA, 256 = two (the epilogue overlaps the next tile's
  *                                    MMAs; clusters twice as large).  Measured: S3 -9 % at d = 512, no

@@ -26,6 +26,9 @@
 // per-row partial sums of squares through distributed shared memory.
 #include "internal.h"
 
+#include <mutex>
+#include <vector>
+
 #include <cuda.h>  // CUtensorMap and enums only; cuTensorMapEncodeTiled is fetched at run time
 
 namespace pinsage {
@@ -72,6 +75,11 @@ struct TcParams {
     unsigned long long *sel_state;
     int *sel_cnt;
     int tile_major;        // see the unit decode in the kernel
+    // row-norm exchange through global memory between the CTA pairs that hold the slabs of one row
+    // tile (gx = 1; they are co-resident: the grid is persistent, one CTA per SM): no cluster needed
+    int gx;
+    float *gx_buf;         // [2 parities][lanes][n_slabs][BM * cg] partial sums of squares
+    unsigned *gx_cnt;      // [2 parities][lanes][cg][4 row quarters] arrivals (zeroed before the launch)
     int sel_k, sel_nb;
     long long sel_id0;
     uint32_t idesc;
@@ -618,6 +626,32 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap tmA1, const __grid_constant__
                         tot += (u == my_unit) ? ss : xbuf[(par * MAX_CLUSTER + u) * BM + row];
                     ss = tot;
                 }
+                if (p.gx) {
+                    // same exchange through global memory: publish my slab's partial, count the
+                    // arrival of my 32 rows, wait until all slabs of this row quarter have arrived
+                    const int rows_u = BM * CG;
+                    float *slot = p.gx_buf + ((size_t)par * lanes + lane0) * p.n_slabs * rows_u + half * BM + row;
+                    unsigned *cnt = p.gx_cnt + (((size_t)par * lanes + lane0) * CG + half) * 4 + ew;
+                    if (eh == 0) {
+                        __stcg(slot + (size_t)slab * rows_u, ss);
+                        __threadfence();
+                        __syncwarp();
+                        if (lane == 0) atomicAdd(cnt, 1u);
+                    }
+                    const unsigned target = (unsigned)((it >> 1) + 1) * (unsigned)p.n_slabs;
+                    if (lane == 0) {
+                        unsigned seen;
+                        do {
+                            asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(seen) : "l"(cnt) : "memory");
+                        } while (seen < target);
+                    }
+                    __syncwarp();
+                    __threadfence();
+                    float tot = 0.f;
+                    for (int u = 0; u < p.n_slabs; ++u)           // same order in every CTA
+                        tot += (u == slab) ? ss : __ldcg(slot + (size_t)u * rows_u);
+                    ss = tot;
+                }
                 scale = ss > 0.f ? rsqrtf(ss) : 0.f;             // zero row stays zero (reading A3)
             }
             if (p.sel_state != nullptr) {
@@ -857,8 +891,8 @@ inline int round_up(int x, int a) { return (x + a - 1) / a * a; }
 
 // cg: CTAs per tile (1 or 2).  ns_pref: preferred slab width without a row norm (256 = double-buffered
 // accumulators, 512 = fewer operand bytes per flop but no epilogue overlap).
-bool plan(const GemmArgs &a, int cg, int ns_pref, int epi_pref, int nl_pref, TcParams &p, int &smem_bytes,
-          const char **why)
+bool plan(const GemmArgs &a, int cg, int ns_pref, int epi_pref, int nl_pref, int gx_pref, TcParams &p,
+          int &smem_bytes, const char **why)
 {
     auto no = [&](const char *msg) {
         if (why) *why = msg;
@@ -887,12 +921,14 @@ bool plan(const GemmArgs &a, int cg, int ns_pref, int epi_pref, int nl_pref, TcP
     p.N = a.N;
     // a normalised row sits in the TMEM of one cluster: slabs of 512 columns (one accumulator), or of 256
     // (two accumulators: the epilogue overlaps the next tile, at the price of a larger cluster)
-    const int slab_max = a.l2norm ? (nl_pref == 256 ? 256 : 512) : ns_pref;
+    const bool gx = a.l2norm && gx_pref && a.N > 512 && a.N <= 2048;   // 256-column slabs, exchange through global memory
+    const int slab_max = a.l2norm ? ((nl_pref == 256 || gx) ? 256 : 512) : ns_pref;
     p.n_slabs = (a.N + slab_max - 1) / slab_max;
     p.NS = p.n_slabs == 1 ? round_up(a.N, 16) : round_up((a.N + p.n_slabs - 1) / p.n_slabs, 64);
     p.n_slabs = (a.N + p.NS - 1) / p.NS;
-    const int units_per_cluster = (a.l2norm && p.n_slabs > 1) ? p.n_slabs : 1;
+    const int units_per_cluster = (a.l2norm && p.n_slabs > 1 && !gx) ? p.n_slabs : 1;
     p.cluster = cg * units_per_cluster;
+    p.gx = gx && p.n_slabs > 1;
     if (p.cluster > MAX_CLUSTER) return no("row norm spans more CTAs than a portable cluster holds");
     p.nchunks = (p.NS + 255) / 256;
     p.CN = round_up((p.NS + p.nchunks - 1) / p.nchunks, 16);
@@ -952,12 +988,12 @@ bool plan_auto(const GemmArgs &a, const GemmTune &t, TcParams &p, int &smem_byte
     // 256 x 256) single-CTA tiles keep more independent tiles in flight and are 15-35 % faster.
     const long long Kt = a.K1 + a.K2 + a.K3;
     const bool tensor_bound = Kt * a.N >= 160 * (Kt + a.N);
-    if ((t.cg == 2 || (t.cg == 0 && tensor_bound)) && plan(a, 2, ns, t.epi, t.nl, p, smem_bytes, nullptr)) return true;
+    if ((t.cg == 2 || (t.cg == 0 && tensor_bound)) && plan(a, 2, ns, t.epi, t.nl, t.gx, p, smem_bytes, nullptr)) return true;
     if (t.cg == 2) {
         if (why) *why = "shape not supported by the CTA-pair kernel";
         return false;
     }
-    return plan(a, 1, ns, t.epi, t.nl, p, smem_bytes, why);
+    return plan(a, 1, ns, t.epi, t.nl, t.gx, p, smem_bytes, why);
 }
 
 template <int CG, int NCH>
@@ -981,13 +1017,17 @@ cudaError_t launch_cg(const TcParams &p, int smem, int num_sms, cudaStream_t s, 
     cfg.blockDim = dim3(NUM_THREADS);
     cfg.dynamicSmemBytes = (size_t)smem;
     cfg.stream = s;
-    cudaLaunchAttribute attr[1];
+    cudaLaunchAttribute attr[2];
     attr[0].id = cudaLaunchAttributeClusterDimension;
     attr[0].val.clusterDim.x = (unsigned)p.cluster;
     attr[0].val.clusterDim.y = 1;
     attr[0].val.clusterDim.z = 1;
+    // grid-wide norm exchange: the CTAs wait on each other, so the whole grid must be co-resident --
+    // a cooperative launch makes that a guarantee (it does not start until every CTA has an SM)
+    attr[1].id = cudaLaunchAttributeCooperative;
+    attr[1].val.cooperative = 1;
     cfg.attrs = attr;
-    cfg.numAttrs = 1;
+    cfg.numAttrs = p.gx ? 2 : 1;
 
     // co-resident clusters of this shape (cached: the query costs a driver call)
     int max_clusters = cached_clusters[p.cluster];
@@ -1050,6 +1090,32 @@ cudaError_t launch_gemm_tc(const GemmArgs &a, const GemmTune &t, int num_sms, cu
         return cudaErrorInvalidValue;
     if (!make_map(&tmOut, a.out, a.M, a.N, 32, 0, a.out_f32 != 0)) return cudaErrorInvalidValue;
     if (launches) ++*launches;
+    if (p.gx) {
+        // exchange buffers of the grid-wide row-norm exchange: one allocation per device, arrival
+        // counters zeroed before every launch (stream order)
+        constexpr size_t BUF = (size_t)2 * 148 * 8 * 256 * 4, CNT = (size_t)2 * 148 * 2 * 4 * 4;
+        // one buffer per (device, stream): launches on different streams may overlap in time
+        struct GxSlot { int dev; cudaStream_t s; void *mem; };
+        static std::mutex gx_mutex;
+        static std::vector<GxSlot> gx_slots;
+        int dev = 0;
+        cudaGetDevice(&dev);
+        void *mem = nullptr;
+        {
+            std::lock_guard<std::mutex> lock(gx_mutex);
+            for (const GxSlot &g : gx_slots)
+                if (g.dev == dev && g.s == s) mem = g.mem;
+            if (!mem) {
+                cudaError_t e = cudaMalloc(&mem, BUF + CNT);
+                if (e != cudaSuccess) return e;
+                gx_slots.push_back({dev, s, mem});
+            }
+        }
+        p.gx_buf = static_cast<float *>(mem);
+        p.gx_cnt = reinterpret_cast<unsigned *>(static_cast<char *>(mem) + BUF);
+        cudaError_t e = cudaMemsetAsync(p.gx_cnt, 0, CNT, s);
+        if (e != cudaSuccess) return e;
+    }
     if (p.cg == 2)
         return p.nchunks == 2 ? launch_cg<2, 2>(p, smem, num_sms, s, tmA1, tmA2, tmA3, tmB, tmOut)
                               : launch_cg<2, 1>(p, smem, num_sms, s, tmA1, tmA2, tmA3, tmB, tmOut);
