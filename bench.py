@@ -399,7 +399,8 @@ def main():
     ap.add_argument("--gemm-epi", type=int, default=0, help="0 auto (8 epilogue warps), 1 four")
     ap.add_argument("--linear-pool", type=int, default=-1, help="-1 auto (m > d), 0 off, 1 on")
     ap.add_argument("--pool-slab", type=int, default=-1, help="-1 auto, 0 whole rows, 32/64/128")
-    ap.add_argument("--gemm-gx", type=int, default=1, help="0: row norms of wide S3 exchanged inside a cluster")
+    ap.add_argument("--gemm-gx", type=int, default=1, help="wide S3 row norms: 1 global-memory exchange (cooperative launch), 2 same with a plain "
+                         "launch (for ncu), 0 cluster exchange")
     ap.add_argument("--gemm-nl", type=int, default=0, help="row-norm GEMM slab width: 0/512 or 256")
     ap.add_argument("--pool-hubs", type=int, default=None,
                     help="hub-split pool: 0 off, -1 automatic, 64..512 forced (default: the library's)")

@@ -114,8 +114,12 @@ const char *pinsage_version(void);
  *                                    slabs of one row tile exchange their partial row norms through global
  *                                    memory (cooperative launch: the grid is co-resident by construction),
  *                                    so the epilogue hides behind the next tile's MMAs and 144 of 148 SMs
- *                                    work; 0 = 512-column slabs exchanged inside a 4-CTA cluster (132 SMs,
- *                                    exposed epilogue).  S3 at d = 1024: 1.21-1.25 -> 1.45-1.50 PFLOP/s.
+ *                                    work; 2 = the same with a plain launch (Nsight Compute cannot replay
+ *                                    the cooperative one; co-residency then rests on the persistent grid
+ *                                    having the device to itself, which holds under a profiler, where
+ *                                    kernels are serialised); 0 = 512-column slabs exchanged inside a
+ *                                    4-CTA cluster (132 SMs, exposed epilogue).  S3 at d = 1024:
+ *                                    1.21-1.25 -> 1.45-1.50 PFLOP/s.
  *                   "gemm_nl"        slab width of the row-norm GEMM (S3): 0 / 512 (default) = one TMEM
  *                                    accumulator per CTA, 256 = two (the epilogue overlaps the next tile's
  *                                    MMAs; clusters twice as large).  Measured: S3 -9 % at d = 512, no

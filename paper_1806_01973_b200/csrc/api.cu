@@ -771,7 +771,8 @@ pinsage_status pinsage_set_option(pinsage_ctx *ctx, const char *key, int64_t val
             return fail(ctx, PINSAGE_ERR_INVALID_ARG, "gemm_ns must be 0, 256 or 512");
         ctx->tune.ns = (int)value;
     } else if (!strcmp(key, "gemm_gx")) {
-        ctx->tune.gx = value != 0;
+        if (value < 0 || value > 2) return fail(ctx, PINSAGE_ERR_INVALID_ARG, "gemm_gx must be 0, 1 or 2");
+        ctx->tune.gx = (int)value;
     } else if (!strcmp(key, "gemm_nl")) {
         if (value != 0 && value != 256 && value != 512)
             return fail(ctx, PINSAGE_ERR_INVALID_ARG, "gemm_nl must be 0, 256 or 512");

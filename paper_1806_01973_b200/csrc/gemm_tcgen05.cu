@@ -928,7 +928,7 @@ bool plan(const GemmArgs &a, int cg, int ns_pref, int epi_pref, int nl_pref, int
     p.n_slabs = (a.N + p.NS - 1) / p.NS;
     const int units_per_cluster = (a.l2norm && p.n_slabs > 1 && !gx) ? p.n_slabs : 1;
     p.cluster = cg * units_per_cluster;
-    p.gx = gx && p.n_slabs > 1;
+    p.gx = (gx && p.n_slabs > 1) ? (gx_pref == 2 ? 2 : 1) : 0;
     if (p.cluster > MAX_CLUSTER) return no("row norm spans more CTAs than a portable cluster holds");
     p.nchunks = (p.NS + 255) / 256;
     p.CN = round_up((p.NS + p.nchunks - 1) / p.nchunks, 16);
@@ -1027,7 +1027,7 @@ cudaError_t launch_cg(const TcParams &p, int smem, int num_sms, cudaStream_t s, 
     attr[1].id = cudaLaunchAttributeCooperative;
     attr[1].val.cooperative = 1;
     cfg.attrs = attr;
-    cfg.numAttrs = p.gx ? 2 : 1;
+    cfg.numAttrs = p.gx == 1 ? 2 : 1;            // (gx == 2: plain launch, for profilers that cannot replay a cooperative one)
 
     // co-resident clusters of this shape (cached: the query costs a driver call)
     int max_clusters = cached_clusters[p.cluster];

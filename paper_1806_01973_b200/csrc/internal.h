@@ -59,7 +59,8 @@ struct GemmTune {
     int epi = 0;   // epilogue warps: 0 = automatic (8 when they fit), 1 = always 4
     int nl = 0;    // slab width of row-norm GEMMs: 0 / 512 = one accumulator per CTA, 256 = two
     int gx = 1;    // 1: row-norm GEMMs wider than 512 use 256-column slabs and exchange the norms through
-                   // global memory between co-resident CTA pairs (no cluster: all SMs, hidden epilogue)
+                   // global memory between co-resident CTA pairs (no cluster: all SMs, hidden epilogue),
+                   // cooperative launch; 2: the same with a plain launch (profilers); 0: cluster exchange
 };
 // Returns cudaErrorNotSupported for shapes outside the compiled set (caller reports UNSUPPORTED_SHAPE).
 bool gemm_tc_supported(const GemmArgs &a, const GemmTune &t, const char **why);
