@@ -227,7 +227,8 @@ def test_dense_matches_oracle(ctx, dtype, M, k, n_out):
 @pytest.mark.parametrize("M,d_in,m,d", [(1, 8, 8, 8), (130, 64, 64, 64), (1000, 256, 256, 256),
                                         (515, 512, 512, 512), (300, 2048, 1024, 1024),
                                         (257, 24, 40, 16), (129, 256, 512, 128),
-                                        (200, 1024, 1024, 1024)])
+                                        (200, 1024, 1024, 1024), (5000, 256, 256, 768),
+                                        (1500, 512, 512, 2048)])
 def test_combine_matches_oracle(ctx, dtype, M, d_in, m, d):
     H = _rand((M, d_in), dtype, 30)
     n = _rand((M, m), dtype, 31).abs()
@@ -235,16 +236,24 @@ def test_combine_matches_oracle(ctx, dtype, M, d_in, m, d):
     w = _rand((d,), torch.float32, 33, scale=0.01)
     ref = O.combine(to_f64(H), to_f64(n), to_f64(W), to_f64(w))
     ran = 0
+    # rows wider than 512 columns: the slabs of a row exchange their partial norms through global
+    # memory (gemm_gx 1: cooperative launch, 2: plain launch) or inside a cluster (0)
+    gxs = (1, 0, 2) if (dtype == torch.bfloat16 and d > 512) else (1,)
     for impl, cg in _both_impls(ctx, dtype):
-        with _impl(ctx, impl, cg):
+        for gx in (gxs if impl == 0 else (1,)):
+            ctx.pinsage_set_option("gemm_gx", gx)
             try:
-                got = ctx.pinsage_combine(H.to(DEV), n.to(DEV), W.to(DEV), w.to(DEV))
-            except binding.PinsageError as e:
-                if e.status_name == "UNSUPPORTED_SHAPE" and impl == 0:
-                    continue
-                raise
+                with _impl(ctx, impl, cg):
+                    try:
+                        got = ctx.pinsage_combine(H.to(DEV), n.to(DEV), W.to(DEV), w.to(DEV))
+                    except binding.PinsageError as e:
+                        if e.status_name == "UNSUPPORTED_SHAPE" and impl == 0:
+                            continue
+                        raise
+            finally:
+                ctx.pinsage_set_option("gemm_gx", 1)
             ran += 1
-            assert_rows_close(to_f64(got), ref, dtype, f"combine impl={impl} cg={cg}",
+            assert_rows_close(to_f64(got), ref, dtype, f"combine impl={impl} cg={cg} gx={gx}",
                               tol=4e-3 if dtype == torch.bfloat16 else 1e-5)
             nrm = np.linalg.norm(to_f64(got), axis=1)
             assert np.all((np.abs(nrm - 1) < (2.0 ** -7 if dtype == torch.bfloat16 else 1e-5))
