@@ -103,16 +103,55 @@ walk_neighbourhoods_kernel(const long long *__restrict__ row_ptr, const int *__r
 
     // ---- the walks (B2, B3, B5) -----------------------------------------------------------------
     const unsigned long long key = mix64(seed + 0x100000001B3ull * (unsigned long long)u);
-    for (int r = lane; r < n_walks; r += 32) {
-        long long cur = u;
+    // A walk is a chain of dependent loads (row_ptr, then col_idx, per step): a lane advances all of its
+    // walks (up to WPL = 8, i.e. n_walks <= 256) one step at a time, so that their loads are in flight
+    // together.  Same draws, same arrivals, same slots as walking them one after the other.
+    constexpr int WPL = 8;
+    if (n_walks <= 32 * WPL) {
+        long long cur[WPL];
+        bool alive[WPL];
+#pragma unroll
+        for (int w = 0; w < WPL; ++w) {
+            cur[w] = u;
+            alive[w] = lane + 32 * w < n_walks;
+        }
         for (int st = 0; st < walk_len; ++st) {
-            const long long beg = __ldg(row_ptr + cur);
-            const long long deg = __ldg(row_ptr + cur + 1) - beg;
-            if (deg <= 0) break;
-            const unsigned long long x = mix64(key ^ (((unsigned long long)r << 32) | (unsigned long long)st));
-            const unsigned long long pick = ((x >> 32) * (unsigned long long)deg) >> 32;
-            cur = __ldg(col_idx + beg + (long long)pick);
-            if (cur != u) s[r * walk_len + st] = (unsigned long long)(unsigned)cur;
+            long long beg[WPL], end[WPL];
+#pragma unroll
+            for (int w = 0; w < WPL; ++w)
+                if (alive[w]) {
+                    beg[w] = __ldg(row_ptr + cur[w]);
+                    end[w] = __ldg(row_ptr + cur[w] + 1);
+                }
+#pragma unroll
+            for (int w = 0; w < WPL; ++w)
+                if (alive[w]) {
+                    const long long deg = end[w] - beg[w];
+                    if (deg <= 0) {
+                        alive[w] = false;                     // dead end: the walk stops (B3)
+                    } else {
+                        const unsigned long long r = (unsigned long long)(lane + 32 * w);
+                        const unsigned long long x = mix64(key ^ ((r << 32) | (unsigned long long)st));
+                        const unsigned long long pick = ((x >> 32) * (unsigned long long)deg) >> 32;
+                        cur[w] = __ldg(col_idx + beg[w] + (long long)pick);
+                    }
+                }
+#pragma unroll
+            for (int w = 0; w < WPL; ++w)
+                if (alive[w] && cur[w] != u) s[(lane + 32 * w) * walk_len + st] = (unsigned long long)(unsigned)cur[w];
+        }
+    } else {
+        for (int r = lane; r < n_walks; r += 32) {
+            long long cur = u;
+            for (int st = 0; st < walk_len; ++st) {
+                const long long beg = __ldg(row_ptr + cur);
+                const long long deg = __ldg(row_ptr + cur + 1) - beg;
+                if (deg <= 0) break;
+                const unsigned long long x = mix64(key ^ (((unsigned long long)r << 32) | (unsigned long long)st));
+                const unsigned long long pick = ((x >> 32) * (unsigned long long)deg) >> 32;
+                cur = __ldg(col_idx + beg + (long long)pick);
+                if (cur != u) s[r * walk_len + st] = (unsigned long long)(unsigned)cur;
+            }
         }
     }
     __syncwarp();
@@ -162,19 +201,73 @@ walk_neighbourhoods_kernel(const long long *__restrict__ row_ptr, const int *__r
 
     // ---- (3) rank (B4).  The run-length output s[0 .. nv) is ordered by id, so a 32-bit key
     // (2048 - count) << 11 | position sorts ascending into (count descending, id ascending) --------
-    int n2 = 32;
-    while (n2 < nv) n2 <<= 1;
     unsigned v2[R];
+    __shared__ unsigned sel_keys[WARPS_PER_CTA][128];
+    if (R > 4 && T <= 128 && nv > 128) {
+        // Only the top T <= 128 of (typically ~1000) distinct ids are wanted: instead of sorting them all,
+        // find the count c* of the T-th best (binary search on the count, entries in registers), take
+        // every id with a larger count and, of those with exactly c*, the smallest ids -- which are the
+        // first in s, already ordered by id -- and sort just these T keys.
+        unsigned cnt[R];
 #pragma unroll
-    for (int r = 0; r < R; ++r) {
-        const int i = r * 32 + lane;
-        v2[r] = 0xFFFFFFFFu;
-        if (i < nv) {
-            const unsigned count = 0xFFFFFFFFu - (unsigned)(s[i] >> 32);
-            v2[r] = ((2048u - count) << 11) | (unsigned)i;
+        for (int r = 0; r < R; ++r) {
+            const int i = r * 32 + lane;
+            cnt[r] = i < nv ? 0xFFFFFFFFu - (unsigned)(s[i] >> 32) : 0u;
         }
+        auto count_ge = [&](unsigned c) {
+            int n = 0;
+#pragma unroll
+            for (int r = 0; r < R; ++r) n += cnt[r] >= c ? 1 : 0;
+            return __reduce_add_sync(0xffffffffu, n);
+        };
+        int lo = 1, hi = 2048;                   // invariant: #(count >= lo) >= T  (nv > 128 >= T)
+        while (lo < hi) {
+            const int mid = (lo + hi + 1) >> 1;
+            if (count_ge((unsigned)mid) >= T) lo = mid;
+            else hi = mid - 1;
+        }
+        const unsigned cstar = (unsigned)lo;
+        const int quota = T - count_ge(cstar + 1);
+        const unsigned lt = (1u << lane) - 1u;
+        int taken_eq = 0, npos = 0;
+#pragma unroll
+        for (int r = 0; r < R; ++r) {
+            const bool eq = cnt[r] == cstar;
+            const unsigned beq = __ballot_sync(0xffffffffu, eq);
+            const bool take = cnt[r] > cstar || (eq && taken_eq + __popc(beq & lt) < quota);
+            const unsigned bt = __ballot_sync(0xffffffffu, take);
+            if (take) sel_keys[wid][npos + __popc(bt & lt)] = ((2048u - cnt[r]) << 11) | (unsigned)(r * 32 + lane);
+            taken_eq += __popc(beq);
+            npos += __popc(bt);
+        }
+        __syncwarp();
+        unsigned w2[4];
+#pragma unroll
+        for (int r = 0; r < 4; ++r) w2[r] = r * 32 + lane < npos ? sel_keys[wid][r * 32 + lane] : 0xFFFFFFFFu;
+        if (npos <= 64) {                        // (warp-uniform) two registers per lane are enough
+            unsigned w1[2] = {w2[0], w2[1]};
+            warp_sort_regs<unsigned, 2>(w1, 64, lane);
+            w2[0] = w1[0];
+            w2[1] = w1[1];
+        } else {
+            warp_sort_regs<unsigned, 4>(w2, 128, lane);
+        }
+#pragma unroll
+        for (int r = 0; r < R; ++r) v2[r] = r < 4 ? w2[r < 4 ? r : 0] : 0xFFFFFFFFu;
+    } else {
+        int n2 = 32;
+        while (n2 < nv) n2 <<= 1;
+#pragma unroll
+        for (int r = 0; r < R; ++r) {
+            const int i = r * 32 + lane;
+            v2[r] = 0xFFFFFFFFu;
+            if (i < nv) {
+                const unsigned count = 0xFFFFFFFFu - (unsigned)(s[i] >> 32);
+                v2[r] = ((2048u - count) << 11) | (unsigned)i;
+            }
+        }
+        warp_sort_regs<unsigned, R>(v2, n2, lane);   // only the stages the nv distinct keys need
     }
-    warp_sort_regs<unsigned, R>(v2, n2, lane);   // only the stages the nv distinct keys need
 
     // ---- (4) the top T, padded with (u, 0): rank t sits in register t / 32 of lane t % 32 -------------
 #pragma unroll

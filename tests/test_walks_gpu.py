@@ -29,7 +29,8 @@ def _both(ctx, row_ptr, col, R, L, T, seed):
 
 @pytest.mark.parametrize("law", ["uniform", "zipf"])
 @pytest.mark.parametrize("R,L,T", [(1, 1, 1), (50, 3, 10), (200, 5, 50), (64, 32, 100), (33, 7, 20),
-                                   (2048, 1, 8), (3, 300, 40)])
+                                   (2048, 1, 8), (3, 300, 40), (200, 5, 128), (200, 5, 65), (256, 4, 64),
+                                   (200, 5, 129), (300, 5, 50)])
 def test_walk_neighbourhoods_bit_exact(ctx, law, R, L, T):
     """Random graphs with dead ends, self loops and repeated edges; ragged N (not a multiple of the
     warps per CTA); slot counts from 32 to the 2048 maximum."""
