@@ -117,7 +117,8 @@ const char *pinsage_version(void);
  *                                    work; 2 = the same with a plain launch (Nsight Compute cannot replay
  *                                    the cooperative one; co-residency then rests on the persistent grid
  *                                    having the device to itself, which holds under a profiler, where
- *                                    kernels are serialised); 0 = 512-column slabs exchanged inside a
+ *                                    kernels are serialised -- under ncu, recognised by its environment
+ *                                    variable NV_COMPUTE_PROFILER_PERFWORKS_DIR, 1 behaves like 2); 0 = 512-column slabs exchanged inside a
  *                                    4-CTA cluster (132 SMs, exposed epilogue).  S3 at d = 1024:
  *                                    1.21-1.25 -> 1.45-1.50 PFLOP/s.
  *                   "gemm_nl"        slab width of the row-norm GEMM (S3): 0 / 512 (default) = one TMEM

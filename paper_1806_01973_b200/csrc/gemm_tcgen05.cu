@@ -26,6 +26,7 @@
 // per-row partial sums of squares through distributed shared memory.
 #include "internal.h"
 
+#include <cstdlib>
 #include <mutex>
 #include <vector>
 
@@ -1027,7 +1028,11 @@ cudaError_t launch_cg(const TcParams &p, int smem, int num_sms, cudaStream_t s, 
     attr[1].id = cudaLaunchAttributeCooperative;
     attr[1].val.cooperative = 1;
     cfg.attrs = attr;
-    cfg.numAttrs = p.gx == 1 ? 2 : 1;            // (gx == 2: plain launch, for profilers that cannot replay a cooperative one)
+    // gx == 2: plain launch, for profilers that cannot replay a cooperative one.  Nsight Compute is
+    // recognised by the variable it sets in the target process and gets the plain launch by itself
+    // (it serialises kernels, so the persistent grid has the device to itself).
+    static const bool profiled = getenv("NV_COMPUTE_PROFILER_PERFWORKS_DIR") != nullptr;
+    cfg.numAttrs = (p.gx == 1 && !profiled) ? 2 : 1;
 
     // co-resident clusters of this shape (cached: the query costs a driver call)
     int max_clusters = cached_clusters[p.cluster];
