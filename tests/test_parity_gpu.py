@@ -609,3 +609,31 @@ def test_bipartite_layers_compose_from_the_step_calls(ctx, dtype):
     ohp = O.combine(f(X), O.pool(oP2, idx_p.numpy(), a_p), f(W2), f(w2))
     assert_rows_close(to_f64(hb), ohb, dtype, "board layer", tol=6e-3 if dtype == torch.bfloat16 else 2e-5)
     assert_rows_close(to_f64(hp), ohp, dtype, "pin layer")
+
+
+def test_grid_exchange_from_two_streams():
+    """S3 wider than 512 columns exchanges row norms between CTA pairs of ONE launch through global
+    memory: the pairs wait on each other, so the launch is cooperative (all of its CTAs get an SM before
+    it starts).  Two contexts on two streams launching such GEMMs at the same time must neither block
+    each other for good nor disturb each other's exchange buffers (one per stream): same bits as alone."""
+    M, d_in, m, d = 30_000, 512, 512, 1024
+    H = _rand((M, d_in), torch.bfloat16, 40).to(DEV)
+    n = _rand((M, m), torch.bfloat16, 41).abs().to(DEV)
+    W = _rand((d, d_in + m), torch.bfloat16, 42, scale=(d_in + m) ** -0.5).to(DEV)
+    w = _rand((d,), torch.float32, 43, scale=0.01).to(DEV)
+    s2 = torch.cuda.Stream()
+    c1 = binding.Context(0)
+    c2 = binding.Context(0, stream=s2.cuda_stream)
+    try:
+        ref = c1.pinsage_combine(H, n, W, w).clone()
+        o1, o2 = torch.empty_like(ref), torch.empty_like(ref)
+        torch.cuda.synchronize()
+        for _ in range(300):
+            c1.pinsage_combine(H, n, W, w, out=o1)
+            c2.pinsage_combine(H, n, W, w, out=o2)
+        torch.cuda.synchronize()
+        assert torch.equal(o1.view(torch.int16), ref.view(torch.int16))
+        assert torch.equal(o2.view(torch.int16), ref.view(torch.int16))
+    finally:
+        c1.close()
+        c2.close()
