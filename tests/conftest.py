@@ -14,6 +14,13 @@ if ROOT not in sys.path:
 
 def pytest_configure(config):
     config.addinivalue_line("markers", "gpu: needs a CUDA device (B200, sm_100a)")
+    # a fresh checkout has no libpinsage.so (it is git-ignored): build it once, as
+    # `__graft_entry__.build()` does (nvcc cross-compiles without a GPU; no-op when it is up to date)
+    try:
+        from paper_1806_01973_b200 import build as _build
+        _build.build()
+    except Exception as e:  # pragma: no cover -- the tests that need the library then fail loudly
+        print(f"conftest: could not build libpinsage.so: {e}", file=sys.stderr)
 
 
 def pytest_collection_modifyitems(config, items):
