@@ -1,19 +1,30 @@
 #!/usr/bin/env python
 """bench.py -- node embeddings / s of K-layer PinSage inference (BASELINE.json's metric).
 
-    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload cfg2] [--impl ours|reference]
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload all|cfg2|cfg3|cfg4|cfg5|tiny]
+                    [--impl ours|reference]
 
 A step = one pass of the whole hot path (S1..S6 of include/pinsage.h: K layers + head over all
 N nodes of the workload) = one ``pinsage_embed_all`` call.  One JSON line is printed by rank 0.
 
-  value      nodes embedded per second, inputs already resident in HBM, CUDA-event timed on the
-             context's stream, max over ranks.
-  e2e        the same call with HOST (pinned) features / tables / output: H2D and D2H copies are
-             inside the timed region.
-  roofline   the dominant kernel (S2 pool): algorithmic bytes per launch / event-measured launch
-             duration inside the timed region, against MEASURED_PEAKS.json's HBM figure.
-  cpu_baseline  the fp64 oracle (oracle/, as it stands) on this box's host cores on a bounded
-             sample of the same workload.  A reported baseline, not the target.
+The default run (``--workload all``) times BASELINE.json's largest single-GPU configuration, config 5
+(N = 5e7, T = 100, K = 3; BASELINE.json's ``metric`` names no configuration), as the headline and carries
+configs 2, 3 and 4 in ``per_config`` (fewer steps each, same timing rules), so that every roofline claim
+is measured by the same command:
+
+  value        nodes embedded per second, inputs already resident in HBM, CUDA-event timed on the
+               context's stream, max over ranks.
+  e2e          the same call with HOST (pinned) features / tables / output: H2D and D2H copies are
+               inside the timed region.
+  roofline     the dominant kernel (S2 pool): algorithmic bytes per launch / event-measured launch
+               duration inside the timed region, against MEASURED_PEAKS.json's HBM figure; next to it the
+               calibration ceilings measured in this very run (``calib``: m1 read-only stream, m2 random-row
+               gather from HBM, m3 random-row gather from L2 -- SURVEY.md 8(d)).
+  roofline_gemm  S1 and S3 at the paper-shaped config 3, the one place the GEMMs are tensor-bound.
+  per_config[*].gemm  per GEMM kind: TFLOP/s, its own bound min(sustained bf16 peak, AI x HBM GB/s) and
+               the fraction of that bound.
+  cpu_baseline the fp64 oracle (oracle/, as it stands) on this box's host cores on a bounded
+               sample of the headline workload.  A reported baseline, not the target.
 
 N > 1 (torchrun): the path does not shard in this library (replicas only),
 so every rank embeds its own replica of the workload; scaling is "weak".
@@ -23,6 +34,7 @@ from __future__ import annotations
 
 import argparse
 import dataclasses
+import gc
 import json
 import os
 import subprocess
@@ -36,15 +48,18 @@ if ROOT not in sys.path:
 
 METRIC = "node embeddings/sec for K-layer inference"
 UNIT = "nodes/s"
+HEADLINE = "cfg5"                      # the largest single-GPU configuration of BASELINE.json
+SIDE_CONFIGS = ("cfg2", "cfg3", "cfg4")
 
 
 def _peaks():
-    """(hbm GB/s, bf16 TFLOP/s sustained, source)."""
+    """(hbm GB/s, bf16 TFLOP/s burst, bf16 TFLOP/s sustained, source)."""
     p = os.path.join(ROOT, "MEASURED_PEAKS.json")
     if os.path.exists(p):
         d = json.load(open(p))
-        return float(d["hbm_gbs"]), float(d.get("bf16_tflops_sustained", d["bf16_tflops"])), "measured"
-    return 6650.0, 1400.0, "fallback"   # B200_PROFILING.md fallback figures
+        burst = float(d["bf16_tflops"])
+        return float(d["hbm_gbs"]), burst, float(d.get("bf16_tflops_sustained", burst)), "measured"
+    return 6650.0, 1590.0, 1400.0, "fallback"   # B200_PROFILING.md fallback figures
 
 
 class ClockSampler:
@@ -112,6 +127,27 @@ def gemm_flops_per_node(cfg):
         f += 2 * d_in * m + 2 * (d_in + m) * d
     f += 2 * cfg.hidden * cfg.g1 + 2 * cfg.g1 * cfg.d_out
     return f
+
+
+def gemm_kinds(cfg, linear_pool: int):
+    """The GEMMs of one step as (name, profile kind, layer, flops per node, HBM bytes per node): what the
+    method must compute and move per node (weights amortise to zero; e = 2 bytes).  In the linear-pool
+    schedule (m > d) S3 keeps only H W1^T and the projection P W2^T is its own launch."""
+    e = 2 if cfg.dtype == "bf16" else 4
+    out = []
+    dims = cfg.layer_dims()
+    for k, (d_in, m, d) in enumerate(dims, start=1):
+        lin = linear_pool == 1 or (linear_pool == -1 and m > d)
+        out.append((f"S1 layer {k}", 1, k, 2 * d_in * m, (d_in + m) * e))
+        if lin:
+            out.append((f"P W2^T layer {k}", 5, k, 2 * m * d, (m + d) * e))
+            out.append((f"S3 layer {k}", 2, k, 2 * d_in * d, (d_in + 2 * d) * e))
+        else:
+            out.append((f"S3 layer {k}", 2, k, 2 * (d_in + m) * d, (d_in + m + d) * e))
+    K = len(dims)
+    out.append(("S4 head", 3, K, 2 * cfg.hidden * cfg.g1, (cfg.hidden + cfg.g1) * e))
+    out.append(("S5 head", 4, K, 2 * cfg.g1 * cfg.d_out, (cfg.g1 + cfg.d_out) * e))
+    return out
 
 
 # ----------------------------------------------------------------------------- oracle legs
@@ -207,8 +243,211 @@ def job_throughput(n_per_rank: int, steps: int, world: int, ms_max: float) -> fl
     return n_per_rank * steps * world / (ms_max * 1e-3)
 
 
+def e2e_nodes(cfg, world: int, avail_bytes: int) -> int:
+    """Nodes of the e2e leg: the whole workload when its pinned host buffers (features, both tables,
+    output) fit 60 % of this rank's share of the available host memory, else the largest sibling that does
+    (a multiple of 10^6 nodes; the copy volume per node is the same)."""
+    e = 2 if cfg.dtype == "bf16" else 4
+    per_node = cfg.d0 * e + 8 * cfg.T + cfg.d_out * e
+    fit = int(0.6 * avail_bytes / max(world, 1) / per_node)
+    if fit >= cfg.N:
+        return cfg.N
+    return max(min(cfg.N, 1_000_000), fit // 1_000_000 * 1_000_000)
+
+
 # ----------------------------------------------------------------------------- the CUDA arm
-def run_ours(args, cfg):
+def calibrate(ctx, dev):
+    """Calibration kernels m1 / m2 / m3 (include/pinsage.h pinsage_calibrate): the read,
+    random-row-gather (HBM) and random-row-gather (L2) ceilings of this device, in GB/s of gathered +
+    written bytes, measured in this run."""
+    import torch
+    T = 50
+    sms = torch.cuda.get_device_properties(dev).multi_processor_count
+    table = torch.zeros(10 << 30, dtype=torch.uint8, device=dev)          # 10 GiB >> L2
+    sink = torch.empty(sms * 8 * 256 * 16, dtype=torch.uint8, device=dev)
+    res = {"how": f"pinsage_calibrate, 5 launches each after one warm-up; m1 streams a 10 GiB buffer; m2 gathers "
+                  f"T = {T} hashed rows per destination from a 10 GiB table, m3 from a 32 MiB one; GB/s of "
+                  f"gathered + written bytes"}
+    ms = ctx.pinsage_calibrate(0, table, 0, 0, 0, sink, reps=5)
+    res["m1_stream_read_gbs"] = table.numel() / (ms * 1e-3) / 1e9
+    res["m2_gather_hbm_gbs"], res["m3_gather_l2_gbs"] = {}, {}
+    small = table[: 32 << 20]
+    for row in (256, 512, 1024, 2048):
+        n_dst = int(16e9 / (T * row))
+        out = torch.empty(n_dst * row, dtype=torch.uint8, device=dev)
+        moved = n_dst * (T * row + row)
+        for name, tab in (("m2_gather_hbm_gbs", table), ("m3_gather_l2_gbs", small)):
+            ms = ctx.pinsage_calibrate(1, tab, row, n_dst, T, out, reps=5)
+            res[name][str(row)] = moved / (ms * 1e-3) / 1e9
+        del out
+    del table, sink, small
+    torch.cuda.empty_cache()
+    return res
+
+
+def _pool_traffic(cfg_name):
+    """DRAM bytes per destination node of the pool from the committed ncu --set full capture of this
+    config (profiles/pool_traffic.csv: name, chunk_nodes, dram_bytes, nodes, source), or None."""
+    tp = os.path.join(ROOT, "profiles", "pool_traffic.csv")
+    if not os.path.exists(tp):
+        return None, None
+    for ln in open(tp).read().splitlines()[1:]:
+        f = [x.strip() for x in ln.split(",")]
+        if len(f) >= 4 and f[0] == cfg_name:
+            return float(f[2]) / float(f[3]), (f[4] if len(f) > 4 else "profiles/pool_traffic.csv")
+    return None, None
+
+
+def run_config(cfg, args, steps, warmup, env, with_clocks=False, e2e_steps=0):
+    """Times `steps` calls of pinsage_embed_all on cfg (device-resident inputs) after `warmup` calls, reads
+    the per-kernel event records, optionally runs the host-buffer (e2e) leg, and frees everything."""
+    import psutil
+    import torch
+    from paper_1806_01973_b200 import binding, synth
+    rank, world, local, dev, barrier = env
+    hbm, burst, sustained, src = _peaks()
+
+    t_gen = time.time()
+    rcfg = replica_config(cfg, rank)
+    X = synth.make_features(rcfg, device=dev)
+    layers, head = synth.make_params(rcfg, device=dev)
+    idx, counts = synth.make_graph(rcfg, device=dev)
+    ctx = binding.Context(local)
+    ctx.pinsage_set_option("gemm_impl", args.gemm_impl)
+    ctx.pinsage_set_option("overlap", args.overlap)
+    ctx.pinsage_set_option("gemm_cg", args.gemm_cg)
+    ctx.pinsage_set_option("pool_slab", args.pool_slab)
+    ctx.pinsage_set_option("gemm_gx", args.gemm_gx)
+    if args.pool_hubs is not None:
+        ctx.pinsage_set_option("pool_hubs", args.pool_hubs)
+    ctx.pinsage_set_option("linear_pool", args.linear_pool)
+    alpha = ctx.pinsage_normalize_counts(counts)
+    torch.cuda.synchronize()
+    del counts
+    torch.cuda.empty_cache()     # generator temporaries back to the driver: the library cudaMallocs
+    out = torch.empty((cfg.N, cfg.d_out), dtype=X.dtype, device=dev)
+    e = X.element_size()
+    t_gen = time.time() - t_gen
+
+    def step():
+        ctx.pinsage_embed_all(X, idx, alpha, layers, head, out=out, chunk_nodes=args.chunk_nodes)
+
+    for _ in range(warmup):
+        step()
+    barrier()
+
+    # ---- timed region: CUDA events on the context's stream (= torch's current stream) -------------
+    sampler = ClockSampler(local) if (with_clocks and rank == 0) else None
+    if sampler:
+        sampler.start()
+    ctx.pinsage_set_option("profile", 1)
+    ctx.pinsage_profile_read(-1)
+    l0 = ctx.pinsage_launch_count()
+    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    barrier()
+    ev0.record()
+    for _ in range(steps):
+        step()
+    ev1.record()
+    barrier()
+    ms = ev0.elapsed_time(ev1)
+    launches = ctx.pinsage_launch_count() - l0
+    kinds = gemm_kinds(cfg, args.linear_pool)
+    pool_ms, pool_n = ctx.pinsage_profile_read(0)
+    gemm_ms = {name: ctx.pinsage_profile_read(kind, layer) for name, kind, layer, _, _ in kinds}
+    ctx.pinsage_set_option("profile", 0)
+    ctx.pinsage_profile_read(-1)
+    clocks = sampler.stop() if sampler else None
+    ms_max = max_over_ranks(ms, world, dev)
+    assert torch.isfinite(out[:: max(1, cfg.N // 4096)].float()).all()
+
+    # ---- roofline of the dominant kernel (S2 pool) from the live event records --------------------
+    lin = args.linear_pool
+    pool_bytes_step = sum(cfg.N * pool_bytes_per_node(cfg.T, d if (lin == 1 or (lin == -1 and m > d)) else m, e)
+                          for _, m, d in cfg.layer_dims())
+    pool_gbs = pool_bytes_step * steps / (pool_ms * 1e-3) / 1e9 if pool_ms > 0 else 0.0
+    per_node, tsrc = _pool_traffic(cfg.name)
+    n_layers = len(cfg.layer_dims())
+    traffic = per_node * cfg.N * n_layers * steps / max(pool_n, 1) if per_node else None
+    roof = {"bound": "hbm", "kernel": "pool_kernel (S2)", "achieved": pool_gbs, "peak": hbm, "unit": "GB/s",
+            "frac": pool_gbs / hbm, "traffic": traffic, "traffic_from": tsrc,
+            "peak_source": f"{src} (MEASURED_PEAKS.json hbm_gbs: a copy, half reads half writes)"
+            if src == "measured" else "fallback (B200_PROFILING.md)",
+            "algorithmic_bytes_per_launch": pool_bytes_step * steps / max(pool_n, 1),
+            "avg_launch_ms": pool_ms / max(pool_n, 1), "launches": pool_n,
+            "ms_per_step": pool_ms / steps,
+            "traffic_over_algorithmic": (traffic / (pool_bytes_step * steps / max(pool_n, 1))) if traffic else None}
+    gemm = {}
+    for name, kind, layer, flops, nbytes in kinds:
+        kms, kn = gemm_ms[name]
+        if kms <= 0:
+            continue
+        tf = flops * cfg.N * steps / (kms * 1e-3) / 1e12
+        ai = flops / nbytes
+        bound = min(sustained, ai * hbm / 1e3)
+        gemm[name] = {"ms_per_step": kms / steps, "launches_per_step": kn / steps, "tflops": tf,
+                      "ai_flop_per_byte": ai, "bound_tflops": bound,
+                      "bound": "tensor" if bound == sustained else "hbm", "frac_of_bound": tf / bound,
+                      "frac_of_nominal_2250": tf / 2250.0}
+    rec = {"workload": workload_config(cfg, args)["workload"], "steps": steps, "warmup": warmup,
+           "ms_per_step": ms_max / steps, "value": job_throughput(cfg.N, steps, world, ms_max), "unit": UNIT,
+           "roofline": roof, "gemm": gemm, "gpu_launches": int(launches), "gen_s": round(t_gen, 1)}
+    if clocks is not None:
+        rec["clocks"] = clocks
+
+    # ---- e2e: the same public call with pinned HOST buffers, copies inside the timed region -------
+    if e2e_steps > 0:
+        n_e = e2e_nodes(cfg, world, psutil.virtual_memory().available)
+        ref_rows = out[:1024].cpu()
+        bits = torch.int16 if e == 2 else torch.int32
+        try:
+            hX = torch.empty((n_e, cfg.d0), dtype=X.dtype, pin_memory=True)
+            hX.copy_(X[:n_e])
+            del X
+            hI = torch.empty((n_e, cfg.T), dtype=idx.dtype, pin_memory=True)
+            hI.copy_(idx[:n_e])
+            if n_e < cfg.N:                      # a sibling: ids must stay inside it
+                hI.remainder_(n_e)
+            del idx
+            hW = torch.empty((n_e, cfg.T), dtype=alpha.dtype, pin_memory=True)
+            hW.copy_(alpha[:n_e])
+            del alpha, out
+            torch.cuda.empty_cache()
+            hO = torch.empty((n_e, cfg.d_out), dtype=hX.dtype, pin_memory=True)
+            h2d = hX.numel() * e + hI.numel() * 4 + hW.numel() * 4
+            d2h = hO.numel() * e
+
+            def step_host():
+                ctx.pinsage_embed_all(hX, hI, hW, layers, head, out=hO, chunk_nodes=args.chunk_nodes)
+
+            step_host()
+            barrier()
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record()
+            for _ in range(e2e_steps):
+                step_host()
+            e1.record()
+            barrier()
+            te_max = max_over_ranks(e0.elapsed_time(e1), world, dev)
+            if n_e == cfg.N:
+                assert torch.equal(hO[:1024].view(bits), ref_rows.view(bits)), "e2e output differs"
+            rec["e2e"] = {"value": job_throughput(n_e, e2e_steps, world, te_max), "unit": UNIT,
+                          "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h, "steps": e2e_steps,
+                          "ms_per_step": te_max / e2e_steps, "nodes": n_e,
+                          "workload": "the headline workload" if n_e == cfg.N else
+                          f"{n_e}-node sibling (pinned host buffers of the full workload exceed this host's memory)"}
+            del hX, hI, hW, hO
+        except RuntimeError as ex:           # pinned allocation refused
+            rec["e2e"] = {"value": None, "unit": UNIT, "error": str(ex)[:200]}
+    ctx.close()
+    del ctx
+    X = idx = alpha = out = layers = head = None
+    gc.collect()
+    torch.cuda.empty_cache()
+    return rec
+
+
+def run_ours(args):
     import torch
     import torch.distributed as dist
     from paper_1806_01973_b200 import binding, synth
@@ -230,154 +469,78 @@ def run_ours(args, cfg):
             dist.barrier()
         torch.cuda.synchronize()
 
-    # ---- seeded synthetic inputs of the workload's shape, generated on the device -------------
-    rcfg = replica_config(cfg, rank)
-    X = synth.make_features(rcfg, device=dev)
-    layers, head = synth.make_params(rcfg, device=dev)
-    idx, counts = synth.make_graph(rcfg, device=dev)
-    ctx = binding.Context(local)
-    ctx.pinsage_set_option("gemm_impl", args.gemm_impl)
-    ctx.pinsage_set_option("overlap", args.overlap)
-    ctx.pinsage_set_option("gemm_cg", args.gemm_cg)
-    ctx.pinsage_set_option("gemm_ns", args.gemm_ns)
-    ctx.pinsage_set_option("gemm_epi", args.gemm_epi)
-    ctx.pinsage_set_option("pool_slab", args.pool_slab)
-    ctx.pinsage_set_option("gemm_nl", args.gemm_nl)
-    ctx.pinsage_set_option("gemm_gx", args.gemm_gx)
-    if args.pool_hubs is not None:
-        ctx.pinsage_set_option("pool_hubs", args.pool_hubs)
-    ctx.pinsage_set_option("linear_pool", args.linear_pool)
-    alpha = ctx.pinsage_normalize_counts(counts)
-    torch.cuda.synchronize()
-    del counts
-    torch.cuda.empty_cache()     # generator temporaries back to the driver: the library cudaMallocs
-    out = torch.empty((cfg.N, cfg.d_out), dtype=X.dtype, device=dev)
-    e = X.element_size()
+    env = (rank, world, local, dev, barrier)
+    everything = args.workload == "all"
+    head_cfg = synth.CONFIGS[HEADLINE if everything else args.workload]
+    if args.nodes:
+        head_cfg = head_cfg.scaled(args.nodes)
 
-    def step():
-        ctx.pinsage_embed_all(X, idx, alpha, layers, head, out=out, chunk_nodes=args.chunk_nodes)
-
-    for _ in range(args.warmup):
-        step()
-    barrier()
-
-    # ---- timed region: K steps, CUDA events on the context's stream (= torch's current) -------
-    sampler = ClockSampler(local)
-    if rank == 0:
-        sampler.start()
-    ctx.pinsage_set_option("profile", 1)
-    ctx.pinsage_profile_read(-1)
-    l0 = ctx.pinsage_launch_count()
-    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    barrier()
-    ev0.record()
-    for _ in range(args.steps):
-        step()
-    ev1.record()
-    barrier()
-    ms = ev0.elapsed_time(ev1)
-    launches = ctx.pinsage_launch_count() - l0
-    prof = {name: ctx.pinsage_profile_read(kind) for kind, name in
-            ((0, "pool"), (1, "dense"), (2, "combine"))}
-    ctx.pinsage_set_option("profile", 0)
-    ctx.pinsage_profile_read(-1)
-    clocks = sampler.stop() if rank == 0 else None
-    ms_max = max_over_ranks(ms, world, dev)
-    assert torch.isfinite(out[:: max(1, cfg.N // 4096)].float()).all()
-
-    # ---- e2e: the same public call with pinned HOST buffers, copies inside the timed region ---
-    e2e = None
-    if not args.no_e2e:
-        hX = torch.empty(X.shape, dtype=X.dtype).pin_memory()
-        hX.copy_(X)
-        hI = torch.empty(idx.shape, dtype=idx.dtype).pin_memory()
-        hI.copy_(idx)
-        hW = torch.empty(alpha.shape, dtype=alpha.dtype).pin_memory()
-        hW.copy_(alpha)
-        hO = torch.empty(out.shape, dtype=out.dtype).pin_memory()
-        h2d = hX.numel() * e + hI.numel() * 4 + hW.numel() * 4
-        d2h = hO.numel() * e
-
-        def step_host():
-            ctx.pinsage_embed_all(hX, hI, hW, layers, head, out=hO, chunk_nodes=args.chunk_nodes)
-
-        step_host()
+    # ---- calibration ceilings of the day (rank 0's device; a few seconds) -------------------------
+    calib = None
+    if (everything or args.calib) and not args.no_calib:
+        c = binding.Context(local)
+        try:
+            calib = calibrate(c, dev)
+        finally:
+            c.close()
         barrier()
-        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-        e0.record()
-        nrep = max(1, min(args.steps, 5))
-        for _ in range(nrep):
-            step_host()
-        e1.record()
-        barrier()
-        te_max = max_over_ranks(e0.elapsed_time(e1), world, dev)
-        assert torch.equal(hO[:1024].view(torch.int16 if e == 2 else torch.int32),
-                           out[:1024].cpu().view(torch.int16 if e == 2 else torch.int32))
-        e2e = {"value": job_throughput(cfg.N, nrep, world, te_max), "unit": UNIT,
-               "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h, "steps": nrep}
-        del hX, hI, hW, hO
+
+    # ---- the headline workload, then the other BASELINE configs -----------------------------------
+    e2e_steps = 0 if args.no_e2e else max(1, min(args.steps, 3))
+    head = run_config(head_cfg, args, args.steps, args.warmup, env, with_clocks=True, e2e_steps=e2e_steps)
+    per_config = []
+    if everything:
+        for name in SIDE_CONFIGS:
+            rec = run_config(synth.CONFIGS[name], args, args.side_steps, max(3, min(args.warmup, 3)), env)
+            rec["config"] = name
+            per_config.append(rec)
 
     if rank != 0:
         if world > 1:
             dist.destroy_process_group()
         return
 
-    # ---- roofline of the dominant kernel (S2 pool) from the live event records ---------------
-    hbm, tflops, src = _peaks()
-    pool_ms, pool_n = prof["pool"]
-    # gathered row width: m, or d in the linear-pool schedule (pooling the W2-projection)
-    lin = args.linear_pool
-    pool_bytes_step = sum(cfg.N * pool_bytes_per_node(cfg.T, d if (lin == 1 or (lin == -1 and m > d)) else m, e)
-                          for _, m, d in cfg.layer_dims())
-    pool_gbs = pool_bytes_step * args.steps / (pool_ms * 1e-3) / 1e9 if pool_ms > 0 else 0.0
-    traffic = None      # DRAM bytes per launch from the committed ncu --set full capture, if any
-    tp = os.path.join(ROOT, "profiles", "pool_traffic.csv")
-    if os.path.exists(tp):
-        for ln in open(tp).read().splitlines()[1:]:
-            f = ln.split(",")
-            if f and f[0] == cfg.name and int(f[1]) == (args.chunk_nodes or 0):
-                # the capture is one full driver chunk: scale to the average launch of this run
-                per_node = float(f[2]) / float(f[3])
-                traffic = per_node * cfg.N * len(cfg.layer_dims()) * args.steps / max(pool_n, 1)
-    kernels = {}
-    for name, (kms, kn) in prof.items():
-        kernels[name] = {"ms_per_step": kms / args.steps, "launches_per_step": kn / args.steps}
-    dense_f = sum(2 * d_in * m for d_in, m, _ in cfg.layer_dims()) + 2 * cfg.hidden * cfg.g1 \
-        + 2 * cfg.g1 * cfg.d_out
-    comb_f = sum(2 * (d_in + m) * d for d_in, m, d in cfg.layer_dims())
-    for d_in, m, d in cfg.layer_dims():          # linear pool: P W2^T is a dense launch, S3 keeps H W1^T
-        if lin == 1 or (lin == -1 and m > d):
-            dense_f += 2 * m * d
-            comb_f -= 2 * m * d
-    for name, f in (("dense", dense_f), ("combine", comb_f)):
-        kms = prof[name][0]
-        if kms > 0:
-            kernels[name]["tflops"] = f * cfg.N * args.steps / (kms * 1e-3) / 1e12
-            kernels[name]["frac_of_bf16_peak"] = kernels[name]["tflops"] / tflops
-    kernels["pool"]["gbs"] = pool_gbs
+    hbm, burst, sustained, src = _peaks()
+
+    def against_calib(roof, cfg):
+        """The pool against the ceilings measured in this run: m2 at its own row width (HBM-bound
+        configs), m3 (the power-law config, whose gathers hit L2-resident hub rows), m1."""
+        if not calib:
+            return
+        row = str(min(2048, max(256, cfg.hidden * 2)))
+        roof["calib"] = {"row_bytes": int(row), "frac_of_m1_stream_read": roof["achieved"] / calib["m1_stream_read_gbs"],
+                         "frac_of_m2_gather_hbm": roof["achieved"] / calib["m2_gather_hbm_gbs"][row],
+                         "frac_of_m3_gather_l2": roof["achieved"] / calib["m3_gather_l2_gbs"][row]}
+
+    against_calib(head["roofline"], head_cfg)
+    for rec in per_config:
+        against_calib(rec["roofline"], synth.CONFIGS[rec["config"]])
 
     line = {
-        "metric": METRIC, "value": job_throughput(cfg.N, args.steps, world, ms_max), "unit": UNIT,
+        "metric": METRIC, "value": head["value"], "unit": UNIT,
         "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
-        "ms_per_step": ms_max / args.steps, "higher_is_better": True, "scaling": "weak",
-        "vs_baseline": None, "dtype": "bf16" if cfg.dtype == "bf16" else "f32",
-        "data": "synthetic", "config": workload_config(cfg, args),
-        "roofline": {"bound": "hbm", "kernel": "pool_kernel (S2)", "achieved": pool_gbs,
-                     "peak": hbm, "unit": "GB/s", "frac": pool_gbs / hbm, "traffic": traffic,
-                     "peak_source": f"{src} (MEASURED_PEAKS.json hbm_gbs)" if src == "measured"
-                     else "fallback (B200_PROFILING.md)",
-                     "algorithmic_bytes_per_launch": pool_bytes_step * args.steps / max(pool_n, 1),
-                     "avg_launch_ms": pool_ms / max(pool_n, 1), "launches": pool_n,
-                     # the same launch measured in DRAM bytes (ncu traffic / live duration): what is
-                     # above 1.0 in `frac` is gathers served by L2, not work skipped
-                     "dram_gbs": (traffic / (pool_ms / max(pool_n, 1) * 1e-3) / 1e9) if traffic and pool_ms > 0 else None,
-                     "frac_dram": (traffic / (pool_ms / max(pool_n, 1) * 1e-3) / 1e9 / hbm) if traffic and pool_ms > 0 else None},
-        "kernels": kernels,
-        "e2e": e2e, "gpu_launches": int(launches), "clocks": clocks,
-        "gemm_impl": "tcgen05" if args.gemm_impl == 0 and cfg.dtype == "bf16" else "simt",
+        "ms_per_step": head["ms_per_step"], "higher_is_better": True, "scaling": "weak",
+        "vs_baseline": None, "dtype": "bf16" if head_cfg.dtype == "bf16" else "f32",
+        "data": "synthetic", "config": workload_config(head_cfg, args),
+        "roofline": head["roofline"], "gemm": head["gemm"],
+        "e2e": head.get("e2e"), "gpu_launches": head["gpu_launches"], "clocks": head.get("clocks"),
+        "gemm_impl": "tcgen05" if args.gemm_impl == 0 and head_cfg.dtype == "bf16" else "simt",
+        "peaks": {"hbm_gbs": hbm, "bf16_tflops_burst": burst, "bf16_tflops_sustained": sustained, "source": src},
     }
+    if calib:
+        line["calib"] = calib
+    if per_config:
+        line["per_config"] = per_config
+        c3 = next((r for r in per_config if r["config"] == "cfg3"), None)
+        if c3:      # the GEMM roofline where the GEMMs are tensor-bound: the paper-shaped config
+            line["roofline_gemm"] = {
+                "workload": c3["workload"], "bound": "tensor", "unit": "TFLOP/s", "peak": sustained,
+                "peak_source": f"{src} (MEASURED_PEAKS.json bf16_tflops_sustained: the kernels are timed inside a long step)",
+                "kernels": {k: {"achieved": v["tflops"], "frac": v["tflops"] / sustained,
+                                "frac_of_nominal_2250": v["frac_of_nominal_2250"], "ms_per_step": v["ms_per_step"]}
+                            for k, v in c3["gemm"].items()}}
     if not args.no_cpu and world == 1:
-        line["cpu_baseline"], _ = cpu_baseline(cfg, args.cpu_seconds)
+        line["cpu_baseline"], _ = cpu_baseline(head_cfg, args.cpu_seconds)
     print(json.dumps(line))
     if world > 1:
         dist.destroy_process_group()
@@ -389,35 +552,38 @@ def main():
     ap.add_argument("--steps", type=int, default=10)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--workload", default="cfg2", help="tiny | cfg2 | cfg3 | cfg4 | cfg5 (full N)")
+    ap.add_argument("--workload", default="all",
+                    help="all (default: cfg5 headline + cfg2-4 in per_config + calibration) | tiny | cfg2 | cfg3 | "
+                         "cfg4 | cfg5 | paper (one workload at full N)")
+    ap.add_argument("--side-steps", type=int, default=5, help="timed steps of each per_config entry")
     ap.add_argument("--nodes", type=int, default=0, help="override N (a '-small' sibling)")
     ap.add_argument("--chunk-nodes", type=int, default=0)
     ap.add_argument("--gemm-impl", type=int, default=0, help="0 tcgen05, 1 SIMT reference kernels")
     ap.add_argument("--overlap", type=int, default=0)
     ap.add_argument("--gemm-cg", type=int, default=0, help="0 auto (CTA pairs), 1 single CTAs, 2 pairs")
-    ap.add_argument("--gemm-ns", type=int, default=0, help="slab width without row norm: 0/256/512")
-    ap.add_argument("--gemm-epi", type=int, default=0, help="0 auto (8 epilogue warps), 1 four")
     ap.add_argument("--linear-pool", type=int, default=-1, help="-1 auto (m > d), 0 off, 1 on")
     ap.add_argument("--pool-slab", type=int, default=-1, help="-1 auto, 0 whole rows, 32/64/128")
-    ap.add_argument("--gemm-gx", type=int, default=1, help="wide S3 row norms: 1 global-memory exchange (cooperative launch), 2 same with a plain "
-                         "launch (for ncu), 0 cluster exchange")
-    ap.add_argument("--gemm-nl", type=int, default=0, help="row-norm GEMM slab width: 0/512 or 256")
+    ap.add_argument("--gemm-gx", type=int, default=1,
+                    help="wide S3 row norms: 1 global-memory exchange (cooperative launch), 2 the same with a plain "
+                         "launch (for ncu, which cannot replay a cooperative one), 0 cluster exchange")
     ap.add_argument("--pool-hubs", type=int, default=None,
                     help="hub-split pool: 0 off, -1 automatic, 64..512 forced (default: the library's)")
+    ap.add_argument("--calib", action="store_true", help="run the calibration kernels with a single workload too")
+    ap.add_argument("--no-calib", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu", action="store_true")
     ap.add_argument("--cpu-seconds", type=float, default=15.0)
     args = ap.parse_args()
     if args.warmup < 3 and args.impl == "ours":
         args.warmup = 3          # timing rule: at least 3 warm-up steps
-    from paper_1806_01973_b200 import synth
-    cfg = synth.CONFIGS[args.workload]
-    if args.nodes:
-        cfg = cfg.scaled(args.nodes)
     if args.impl == "reference":
+        from paper_1806_01973_b200 import synth
+        cfg = synth.CONFIGS[HEADLINE if args.workload == "all" else args.workload]
+        if args.nodes:
+            cfg = cfg.scaled(args.nodes)
         run_reference(args, cfg)
     else:
-        run_ours(args, cfg)
+        run_ours(args)
 
 
 if __name__ == "__main__":

@@ -95,85 +95,66 @@ const char *pinsage_last_error(const pinsage_ctx *ctx);
 /* Static version string, e.g. "pinsage-b200 0.1.0 (sm_100a)". */
 const char *pinsage_version(void);
 
-/* Integer options:  "gemm_impl"      0 = tcgen05 (default), 1 = SIMT reference kernels
- *                   "f32_split"      PINSAGE_F32 GEMMs on the tensor cores: both operands split into
- *                                    three bf16 planes (x = x0 + x1 + x2 exactly), the six products with
- *                                    i + j <= 2 summed by one tcgen05 GEMM over a six times longer K
- *                                    (fp32 accumulate, error ~1e-6 relative; 5-7 x the SIMT kernel):
- *                                    -1 = when M N K >= 2^28 and the shape is covered (default),
- *                                    0 = never (SIMT fp32 FMA kernels), 1 = always, a GEMM the split
- *                                    path does not cover (K % 4 != 0, the linear-pool addend) is then
- *                                    PINSAGE_ERR_UNSUPPORTED_SHAPE.  Ignored when gemm_impl = 1.
- *                   "gemm_cg"        tcgen05 tile owner: 0 = automatic (CTA pairs, cta_group::2, 256-row
- *                                    tiles when the GEMM is tensor-bound, K N / (K + N) >= 160, and
- *                                    M > 128, N % 16 == 0; default), 1 = single CTAs
- *                                    (128-row tiles) only, 2 = CTA pairs or PINSAGE_ERR_UNSUPPORTED_SHAPE
- *                   "gemm_ns"        slab width of GEMMs without a row norm: 0 / 256 (default) or 512
- *                   "gemm_gx"        row-norm GEMM (S3) wider than 512 columns: 1 (default) = 256-column
- *                                    slabs with two TMEM accumulators each, the CTA pairs that hold the
- *                                    slabs of one row tile exchange their partial row norms through global
- *                                    memory (cooperative launch: the grid is co-resident by construction),
- *                                    so the epilogue hides behind the next tile's MMAs and 144 of 148 SMs
- *                                    work; 2 = the same with a plain launch (Nsight Compute cannot replay
- *                                    the cooperative one; co-residency then rests on the persistent grid
- *                                    having the device to itself, which holds under a profiler, where
- *                                    kernels are serialised -- under ncu, recognised by its environment
- *                                    variable NV_COMPUTE_PROFILER_PERFWORKS_DIR, 1 behaves like 2); 0 = 512-column slabs exchanged inside a
- *                                    4-CTA cluster (132 SMs, exposed epilogue).  S3 at d = 1024:
- *                                    1.21-1.25 -> 1.45-1.50 PFLOP/s.
- *                   "gemm_nl"        slab width of the row-norm GEMM (S3): 0 / 512 (default) = one TMEM
- *                                    accumulator per CTA, 256 = two (the epilogue overlaps the next tile's
- *                                    MMAs; clusters twice as large).  Measured: S3 -9 % at d = 512, no
- *                                    change at d = 1024 (8-CTA clusters fill only 128 of the 148 SMs).
- *                   "gemm_epi"       epilogue warps: 0 = eight for single-accumulator row-norm tiles (default),
- *                                    1 = always four, 2 = eight wherever they fit (measured slower)
- *                   "check_indices"  1 = every pinsage_pool / layer / embed_all call validates
- *                                    nbr_idx first (synchronous), default 0
- *                   "overlap"        1 = pinsage_layer / embed_all overlap S2 of chunk c+1 with S3
- *                                    of chunk c on a second stream (default 0)
- *                   "pool_mode"      the aggregator gamma of Alg. 1 l.1 used by pinsage_pool / layer /
- *                                    embed_all: 0 = importance pooling, the weighted sum (default);
- *                                    1 = element-wise mean, 2 = element-wise max of the T projected
- *                                    neighbour rows (the paper's ablation variants, PAPER.md:118,
- *                                    :262-263; nbr_w is not read, but must still be a valid pointer)
- *                   "linear_pool"    pinsage_layer / embed_all schedule: pool the W2-projection P W2^T
- *                                    (width d) and add it to H W1^T in the S3 epilogue, instead of pooling
- *                                    P (width m) -- the same function in real arithmetic, m / d times
- *                                    fewer gathered bytes: -1 = when m > d (default), 0 never, 1 always.
- *                                    Not used with pool_mode 2 (max is not linear).
- *                   "pool_slab"      column-slab width in bytes of the S2 pool: -1 automatic (default:
- *                                    128-byte slabs when P exceeds L2 but n_src x 128 bytes fits in
- *                                    0.7 of it, so that the gathered sub-table stays L2-resident),
- *                                    0 = always whole rows, 32 / 64 / 128 = forced.  Bit-identical results.
- *                   "pool_hubs"      pinsage_embed_all on skewed graphs (BF16, importance pooling, device
- *                                    tables, m <= d schedule): the entries of the neighbour lists that
- *                                    point at the H most listed nodes ("hubs", found from a sample of the
- *                                    lists) are not gathered; their term  A (P_hub W2^T),  A[u, h] = the
- *                                    summed weight of u's entries naming hub h, enters S3 as a third K
- *                                    segment on the tensor cores (A and P_hub W2^T rounded to bf16, exact
- *                                    products, fp32 sum).  The same function in real arithmetic and the
- *                                    same error level as the plain pool (which rounds all of n to bf16),
- *                                    but a different rounding: not bit-identical.  0 = off (default),
- *                                    H = 64 .. 512 (multiple of 64) = on, -1 = on (H = 128) when the
- *                                    sampled hubs hold at least a third of all entries (one stream
- *                                    synchronisation per call).  Power-law config: 1.45 x faster.
- *                   "topk_fused"     pinsage_topk: 1 (default) = once every running list is full, scores
- *                                    are tested against the query's k-th score in the GEMM's epilogue and
- *                                    only the keepers leave the SM (no fp32 score matrix in HBM); 0 = every
- *                                    block of scores is stored and scanned by a second kernel.  Same result.
- *                   "profile"        1 = bracket every kernel launch of the path with CUDA events
- *                                    on its stream, see pinsage_profile_read (default 0)
- * Unknown key -> PINSAGE_ERR_INVALID_ARG. */
+/* Integer options (key, value).  Unknown key or value out of range -> PINSAGE_ERR_INVALID_ARG.
+ *
+ *   "gemm_impl"      0 = tcgen05 tensor-core GEMMs (default), 1 = SIMT reference kernels
+ *   "f32_split"      PINSAGE_F32 GEMMs on the tensor cores: both operands split into three bf16 planes
+ *                    (x = x0 + x1 + x2 exactly), the six products with i + j <= 2 summed by one tcgen05 GEMM
+ *                    over a six times longer K (fp32 accumulate, error ~1e-6 relative; 5-7 x the SIMT
+ *                    kernel): -1 = when rows x N x K >= 2^28 and the shape is covered (default; "rows" are
+ *                    those of the whole call -- N nodes -- not of a chunk or of a sub-graph, so every
+ *                    chunking and pinsage_embed_nodes make the same choice), 0 = never (SIMT fp32 FMA
+ *                    kernels), 1 = always; a GEMM the split path does not cover (K % 4 != 0, the
+ *                    linear-pool addend) is then PINSAGE_ERR_UNSUPPORTED_SHAPE.  Ignored when gemm_impl = 1.
+ *   "check_indices"  1 = every pinsage_pool / layer / embed_all / embed_nodes call validates nbr_idx
+ *                    first (synchronous), default 0
+ *   "overlap"        1 = pinsage_layer / embed_all run S2 of chunk c+1 and S3 of chunk c on two streams
+ *                    (default 0: measured no faster on B200, the pool's CTAs fill the device first)
+ *   "pool_mode"      the aggregator gamma of Alg. 1 l.1 used by pinsage_pool / layer / embed_all /
+ *                    embed_nodes: 0 = importance pooling, the weighted sum (default); 1 = element-wise
+ *                    mean, 2 = element-wise max of the T projected neighbour rows (the paper's ablation
+ *                    variants; nbr_w is not read, but must still be a valid pointer)
+ *   "linear_pool"    pinsage_layer / embed_all / embed_nodes schedule: pool the W2-projection P W2^T
+ *                    (width d) and add it to H W1^T in the S3 epilogue, instead of pooling P (width m) --
+ *                    the same function in real arithmetic, m / d times fewer gathered bytes: -1 = when
+ *                    m > d (default), 0 never, 1 always.  Not used with pool_mode 2 (max is not linear).
+ *   "pool_hubs"      skewed graphs (BF16, importance pooling, m <= d schedule): the entries of the neighbour
+ *                    lists that point at the H most listed nodes ("hubs", found from a sample of the lists)
+ *                    are not gathered; their term  A (P_hub W2^T),  A[u, h] = the summed weight of u's
+ *                    entries naming hub h (summed in table order), enters S3 as a third K segment on the
+ *                    tensor cores (A and P_hub W2^T rounded to bf16, exact products, fp32 sum).  The same
+ *                    function in real arithmetic and the same error level as the plain pool (which rounds
+ *                    all of n to bf16), but a different rounding.  0 = off, H = 64 .. 512 (multiple of 64)
+ *                    = on, -1 = on (H = 128) when the sampled hubs hold at least a third of all entries
+ *                    (one stream synchronisation per call).  Power-law config: 1.45 x faster.
+ *   "topk_fused"     pinsage_topk: 1 (default) = once every running list is full, scores are tested against
+ *                    the query's k-th score in the GEMM's epilogue and only the keepers leave the SM (no
+ *                    fp32 score matrix in HBM); 0 = every block of scores is stored and scanned by a
+ *                    second kernel.  Same result.
+ *   "profile"        1 = bracket every kernel launch of the path with CUDA events on its stream, see
+ *                    pinsage_profile_read (default 0)
+ *
+ * Diagnostic keys (tests and profiling; not part of the stable interface, results are unchanged):
+ *   "gemm_cg"        tcgen05 tile owner: 0 = automatic (CTA pairs, cta_group::2, 256-row tiles, when the
+ *                    GEMM is tensor-bound), 1 = single CTAs only, 2 = CTA pairs or UNSUPPORTED_SHAPE
+ *   "gemm_gx"        row norms of S3 wider than 512 columns: 1 (default) = exchanged through global memory
+ *                    between the co-resident CTA pairs of a cooperative launch; 2 = the same with a plain
+ *                    launch (Nsight Compute cannot replay a cooperative one; a wait longer than ~2 s traps);
+ *                    0 = exchanged inside a thread-block cluster (512-column slabs)
+ *   "pool_slab"      column-slab width in bytes of the S2 pool: -1 automatic (default: 128-byte slabs when
+ *                    P exceeds L2 but n_src x 128 bytes fits in 0.7 of it), 0 = whole rows, 32 / 64 / 128 */
 pinsage_status pinsage_set_option(pinsage_ctx *ctx, const char *key, int64_t value);
 
 /* Number of kernels this context has launched so far (for launch accounting in benchmarks). */
 int64_t pinsage_launch_count(const pinsage_ctx *ctx);
 
 /* Per-kernel device time gathered while option "profile" is 1.  Synchronises the context's streams,
- * then sums the event-measured duration of every launch of `kind` since the last reset into
- * *total_ms and their number into *launches (HOST pointers).  kind: 0 = S2 pool, 1 = S1/S4/S5 dense,
- * 2 = S3 combine, -1 = reset the records (outputs are then 0). */
-pinsage_status pinsage_profile_read(pinsage_ctx *ctx, int32_t kind, double *total_ms,
+ * then sums the event-measured duration of every launch of `kind` (in layer `layer`, 1-based; 0 = all
+ * layers; the head carries the last layer's number) since the last reset into *total_ms and their number
+ * into *launches (HOST pointers).  kind: 0 = S2 pool (with the hub preparation of "pool_hubs"), 1 = S1
+ * (also pinsage_dense and the score GEMMs of pinsage_topk), 2 = S3, 3 = S4, 4 = S5, 5 = the P W2^T
+ * projection of the linear-pool schedule, -1 = reset the records (outputs are then 0). */
+pinsage_status pinsage_profile_read(pinsage_ctx *ctx, int32_t kind, int32_t layer, double *total_ms,
                                     int64_t *launches);
 
 /* ---- the steps of the path, one call each ------------------------------------------------- */
@@ -285,6 +266,21 @@ pinsage_status pinsage_build_neighbourhoods(pinsage_ctx *ctx, int64_t N, const i
 pinsage_status pinsage_validate_graph(pinsage_ctx *ctx, int64_t n_dst, int64_t n_src, int32_t T,
                                       const int32_t *nbr_idx, const float *nbr_w,
                                       int64_t *first_bad);
+
+/* Measurement aid, not a step of the path ("how to report the pool honestly"): what
+ * this device delivers to the access patterns of the S2 pool, so that the pool can be
+ * reported against physical ceilings of the day instead of a copy rate.
+ *   kind 0 (m1): read-only streaming reduction over table_bytes bytes of `table`; `out` needs
+ *                num_sms x 8 x 256 x 16 bytes (303 104 x 16 on a 148-SM part).
+ *   kind 1 (m2 / m3): un-weighted random-row gather: for each of n_dst destinations, T rows of row_bytes
+ *                (256, 512, 1024 or 2048) bytes at hashed positions of `table` (table_bytes / row_bytes rows)
+ *                are XOR-summed into out [n_dst x row_bytes].  A table far larger than L2 gives the random-row
+ *                ceiling from HBM (m2), a table that fits L2 the L2 / LSU ceiling (m3).
+ * Device pointers, 16-byte aligned.  Synchronous: one warm-up launch, then `reps` launches between two CUDA
+ * events on the context's stream; *ms (HOST pointer) = average milliseconds per launch. */
+pinsage_status pinsage_calibrate(pinsage_ctx *ctx, int32_t kind, const void *table, size_t table_bytes,
+                                 int32_t row_bytes, int64_t n_dst, int32_t T, void *out, size_t out_bytes,
+                                 int32_t reps, double *ms);
 
 #ifdef __cplusplus
 }

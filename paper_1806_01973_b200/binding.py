@@ -26,7 +26,7 @@ SYMBOLS = [
     "pinsage_set_option", "pinsage_launch_count", "pinsage_profile_read", "pinsage_dense", "pinsage_pool",
     "pinsage_combine", "pinsage_layer", "pinsage_layer_workspace_bytes", "pinsage_head",
     "pinsage_embed_all", "pinsage_normalize_counts", "pinsage_validate_graph",
-    "pinsage_build_neighbourhoods", "pinsage_embed_nodes", "pinsage_topk",
+    "pinsage_build_neighbourhoods", "pinsage_embed_nodes", "pinsage_topk", "pinsage_calibrate",
 ]
 
 
@@ -74,7 +74,7 @@ def load_library() -> ctypes.CDLL:
     lib.pinsage_set_option.restype = ctypes.c_int
     lib.pinsage_launch_count.argtypes = [vp]
     lib.pinsage_launch_count.restype = i64
-    lib.pinsage_profile_read.argtypes = [vp, i32, ctypes.POINTER(ctypes.c_double),
+    lib.pinsage_profile_read.argtypes = [vp, i32, i32, ctypes.POINTER(ctypes.c_double),
                                          ctypes.POINTER(i64)]
     lib.pinsage_profile_read.restype = ctypes.c_int
     lib.pinsage_dense.argtypes = [vp, ctypes.c_int, i64, i32, i32, vp, vp, vp, i32, vp]
@@ -105,6 +105,9 @@ def load_library() -> ctypes.CDLL:
     lib.pinsage_topk.restype = ctypes.c_int
     lib.pinsage_build_neighbourhoods.argtypes = [vp, i64, vp, vp, i32, i32, i32, ctypes.c_uint64, vp, vp]
     lib.pinsage_build_neighbourhoods.restype = ctypes.c_int
+    lib.pinsage_calibrate.argtypes = [vp, i32, vp, sz, i32, i64, i32, vp, sz, i32,
+                                      ctypes.POINTER(ctypes.c_double)]
+    lib.pinsage_calibrate.restype = ctypes.c_int
     lib.pinsage_validate_graph.argtypes = [vp, i64, i64, i32, vp, vp, ctypes.POINTER(i64)]
     lib.pinsage_validate_graph.restype = ctypes.c_int
     _lib = lib
@@ -190,10 +193,11 @@ class Context:
     def pinsage_launch_count(self) -> int:
         return int(self.lib.pinsage_launch_count(self.handle))
 
-    def pinsage_profile_read(self, kind: int):
-        """(total_ms, launches) of kernel kind 0 pool / 1 dense / 2 combine; kind -1 resets."""
+    def pinsage_profile_read(self, kind: int, layer: int = 0):
+        """(total_ms, launches) of kind 0 S2 / 1 S1 / 2 S3 / 3 S4 / 4 S5 / 5 linear-pool projection in
+        `layer` (0 = all layers); kind -1 resets."""
         ms, n = ctypes.c_double(0.0), ctypes.c_int64(0)
-        self._check(self.lib.pinsage_profile_read(self.handle, kind, ctypes.byref(ms),
+        self._check(self.lib.pinsage_profile_read(self.handle, kind, layer, ctypes.byref(ms),
                                                   ctypes.byref(n)))
         return float(ms.value), int(n.value)
 
@@ -322,6 +326,14 @@ class Context:
             self.handle, N, _ptr(row_ptr), _ptr(col_idx), int(n_walks), int(walk_len), int(T),
             ctypes.c_uint64(seed), _ptr(idx), _ptr(cnt)))
         return idx, cnt
+
+    def pinsage_calibrate(self, kind: int, table, row_bytes: int, n_dst: int, T: int, out, reps: int = 5):
+        """Milliseconds per launch of calibration kernel `kind` (0 stream, 1 random-row gather)."""
+        ms = ctypes.c_double(0.0)
+        self._check(self.lib.pinsage_calibrate(
+            self.handle, int(kind), _ptr(table), table.numel() * table.element_size(), int(row_bytes),
+            int(n_dst), int(T), _ptr(out), out.numel() * out.element_size(), int(reps), ctypes.byref(ms)))
+        return float(ms.value)
 
     def pinsage_validate_graph(self, nbr_idx, nbr_w, n_src: int) -> int:
         """Returns -1 if the tables are valid, else raises PinsageError(BAD_INDEX)."""

@@ -13,6 +13,8 @@
 #include <string>
 #include <vector>
 
+#include <nvtx3/nvToolsExt.h>   // header-only; ranges cost a pointer test when no tool is attached
+
 using namespace pinsage;
 
 struct pinsage_ctx {
@@ -27,7 +29,11 @@ struct pinsage_ctx {
     cudaEvent_t ev_fork = nullptr, ev_join = nullptr;
     int num_sms = 0;
     int gemm_impl = 0;               // 0 tcgen05, 1 SIMT reference
-    GemmTune tune;                   // tcgen05 tile knobs ("gemm_cg", "gemm_ns")
+    GemmTune tune;                   // tcgen05 diagnostic knobs ("gemm_cg", "gemm_gx")
+    GemmTcState *tc = nullptr;       // launcher state: function attributes, exchange buffers, tensor maps
+    int cur_layer = 0;               // 1-based layer of the running call (NVTX range names only)
+    int64_t m_hint = 0;              // rows the GEMMs of the running call would have on the whole graph
+                                     // (pinsage_embed_nodes: same kernel choice as pinsage_embed_all)
     int check_indices = 0;
     int overlap = 0;
     int pool_mode = 0;               // aggregator gamma: 0 importance, 1 mean, 2 max
@@ -64,7 +70,7 @@ struct pinsage_ctx {
     // optional per-kernel timing ("profile" option): event pairs around every launch
     int profile = 0;
     std::vector<cudaEvent_t> prof_events;
-    struct ProfRec { int kind; int e0, e1; };
+    struct ProfRec { int kind, layer; int e0, e1; };
     std::vector<ProfRec> prof_recs;
     size_t prof_used = 0;
     std::string err;
@@ -117,7 +123,35 @@ struct DeviceGuard {
     }
 };
 
+// NVTX range "S<step> <what>" around the launches of one step: makes an nsys / ncu
+// capture self-describing.  No tool attached: nvtxRangePush is a null-pointer test.
+struct StepRange {
+    StepRange(const char *fmt, ...)
+    {
+        char buf[96];
+        va_list ap;
+        va_start(ap, fmt);
+        vsnprintf(buf, sizeof buf, fmt, ap);
+        va_end(ap);
+        nvtxRangePushA(buf);
+    }
+    ~StepRange() { nvtxRangePop(); }
+};
+
+// Kernel choices that depend on the problem size (the fp32 GEMM: split tensor-core path or SIMT) are
+// taken from the rows of the CALL, not of the chunk or sub-graph a launch happens to cover, so that
+// every chunking and pinsage_embed_nodes (hint = the whole graph's N) give the same bits.
+struct HintGuard {
+    pinsage_ctx *c;
+    int64_t prev;
+    HintGuard(pinsage_ctx *ctx, int64_t rows);
+    ~HintGuard();
+};
+
 inline size_t align_up(size_t x, size_t a) { return (x + a - 1) / a * a; }
+
+HintGuard::HintGuard(pinsage_ctx *ctx, int64_t rows) : c(ctx), prev(ctx->m_hint) { ctx->m_hint = std::max(prev, rows); }
+HintGuard::~HintGuard() { c->m_hint = prev; }
 
 bool aligned16(const void *p) { return (reinterpret_cast<uintptr_t>(p) & 15u) == 0; }
 
@@ -221,7 +255,10 @@ pinsage_status ensure_buf(pinsage_ctx *ctx, void **buf, size_t *cap, size_t byte
     return PINSAGE_OK;
 }
 
-enum ProfKind { PROF_POOL = 0, PROF_DENSE = 1, PROF_COMBINE = 2, PROF_KINDS = 3 };
+// kinds of pinsage_profile_read: the steps of the path; PROF_DENSE also takes pinsage_dense and the score
+// GEMMs of pinsage_topk, PROF_AUX the P W2^T projection of the linear-pool schedule
+enum ProfKind { PROF_POOL = 0, PROF_DENSE = 1, PROF_COMBINE = 2, PROF_HEAD1 = 3, PROF_HEAD2 = 4, PROF_AUX = 5,
+                PROF_KINDS = 6 };
 
 // Records an event on stream s (profile mode only) and returns its slot, or -1.
 int prof_mark(pinsage_ctx *ctx, cudaStream_t s)
@@ -241,7 +278,7 @@ void prof_close(pinsage_ctx *ctx, int kind, int e0, cudaStream_t s)
 {
     if (e0 < 0) return;
     const int e1 = prof_mark(ctx, s);
-    if (e1 >= 0) ctx->prof_recs.push_back({kind, e0, e1});
+    if (e1 >= 0) ctx->prof_recs.push_back({kind, ctx->cur_layer, e0, e1});
 }
 
 void count_launches(pinsage_ctx *ctx)
@@ -291,10 +328,11 @@ bool split_wanted(const pinsage_ctx *ctx, DType dt, const GemmArgs &a)
 {
     return dt == DType::F32 && ctx->gemm_impl == 0 &&
            (ctx->f32_split == 1 ||
-            (ctx->f32_split == -1 && (double)a.M * a.N * (a.K1 + a.K2) >= (double)(1 << 28)));
+            (ctx->f32_split == -1 &&
+             (double)std::max<int64_t>(a.M, ctx->m_hint) * a.N * (a.K1 + a.K2) >= (double)(1 << 28)));
 }
 
-pinsage_status run_gemm_split(pinsage_ctx *ctx, const GemmArgs &a, cudaStream_t s, bool *done)
+pinsage_status run_gemm_split(pinsage_ctx *ctx, const GemmArgs &a, cudaStream_t s, int kind, bool *done)
 {
     *done = false;
     GemmArgs g;
@@ -309,14 +347,12 @@ pinsage_status run_gemm_split(pinsage_ctx *ctx, const GemmArgs &a, cudaStream_t 
     if (need > ctx->split_bytes) {
         PS_CUDA(ctx, cudaStreamSynchronize(s));
         if (ctx->split_buf) cudaFree(ctx->split_buf);
-    if (ctx->hub_buf) cudaFree(ctx->hub_buf);
         ctx->split_buf = nullptr;
         ctx->split_bytes = 0;
         PS_CUDA(ctx, cudaMalloc(&ctx->split_buf, need));
         ctx->split_bytes = need;
     }
     char *Bp = static_cast<char *>(ctx->split_buf), *Ap = Bp + b_bytes;
-    const int kind = a.l2norm ? PROF_COMBINE : PROF_DENSE;
     const int e0 = prof_mark(ctx, s);
     cudaError_t e = launch_split3(true, static_cast<const float *>(a.B), kt, ldb, nullptr, 0, 0, b_rows, Bp, s,
                                   &ctx->launches);
@@ -330,7 +366,7 @@ pinsage_status run_gemm_split(pinsage_ctx *ctx, const GemmArgs &a, cudaStream_t 
         g.A1 = Ap;
         g.B = Bp;
         g.out = static_cast<float *>(a.out) + r0 * a.N;
-        e = launch_gemm_tc(g, ctx->tune, ctx->num_sms, s, &ctx->launches);
+        e = launch_gemm_tc(g, ctx->tune, ctx->tc, s, &ctx->launches);
     }
     prof_close(ctx, kind, e0, s);
     count_launches(ctx);
@@ -348,7 +384,7 @@ pinsage_status run_gemm(pinsage_ctx *ctx, DType dt, const GemmArgs &a, void *scr
     const int kind = prof_kind >= 0 ? prof_kind : a.l2norm ? PROF_COMBINE : PROF_DENSE;
     if (split_wanted(ctx, dt, a)) {
         bool done = false;
-        PS_TRY(run_gemm_split(ctx, a, s, &done));
+        PS_TRY(run_gemm_split(ctx, a, s, kind, &done));
         if (done) return PINSAGE_OK;
         if (ctx->f32_split == 1)
             return fail(ctx, PINSAGE_ERR_UNSUPPORTED_SHAPE,
@@ -373,7 +409,7 @@ pinsage_status run_gemm(pinsage_ctx *ctx, DType dt, const GemmArgs &a, void *scr
         return fail(ctx, PINSAGE_ERR_UNSUPPORTED_SHAPE, "tcgen05 GEMM: %s (M=%lld K1=%d K2=%d N=%d)",
                     why ? why : "unsupported shape", (long long)a.M, a.K1, a.K2, a.N);
     const int e0 = prof_mark(ctx, s);
-    cudaError_t e = launch_gemm_tc(a, ctx->tune, ctx->num_sms, s, &ctx->launches);
+    cudaError_t e = launch_gemm_tc(a, ctx->tune, ctx->tc, s, &ctx->launches);
     prof_close(ctx, kind, e0, s);
     count_launches(ctx);
     PS_CUDA(ctx, e);
@@ -383,7 +419,7 @@ pinsage_status run_gemm(pinsage_ctx *ctx, DType dt, const GemmArgs &a, void *scr
 size_t gemm_scratch_bytes(const pinsage_ctx *ctx, DType dt, const GemmArgs &a)
 {
     const bool simt = dt == DType::F32 || (ctx && ctx->gemm_impl == 1);
-    return align_up(simt ? gemm_simt_scratch_bytes(a) : gemm_tc_scratch_bytes(a), 256);
+    return simt ? align_up(gemm_simt_scratch_bytes(a), 256) : 0;   // (the tcgen05 kernel needs none)
 }
 
 pinsage_status check_layer_params(pinsage_ctx *ctx, const pinsage_layer_params *p, const char *what)
@@ -451,6 +487,18 @@ bool use_linear_pool(const pinsage_ctx *ctx, const pinsage_layer_params *lp)
     return ctx->linear_pool == 1 || lp->m > lp->d;
 }
 
+// The pool kernels cover rows of at most 256 16-byte chunks (4096 bytes: 2048 bf16 / 1024 fp32 values).
+// Checked before anything is enqueued, for the row width the chosen schedule pools.
+pinsage_status check_pool_width(pinsage_ctx *ctx, DType dt, const pinsage_layer_params *lp)
+{
+    const int32_t pw = use_linear_pool(ctx, lp) ? lp->d : lp->m;
+    if ((size_t)pw * elem_size(dt) > 4096)
+        return fail(ctx, PINSAGE_ERR_UNSUPPORTED_SHAPE,
+                    "pooled rows of %d %s values exceed 4096 bytes (m = %d, d = %d)", pw,
+                    dt == DType::BF16 ? "bf16" : "fp32", lp->m, lp->d);
+    return PINSAGE_OK;
+}
+
 // Called on the compute stream's timeline right after rows [r0, r0 + rows) of a layer's output exist.
 using ChunkHook = std::function<pinsage_status(int64_t r0, int64_t rows)>;
 
@@ -507,6 +555,7 @@ pinsage_status pool_combine_chunks(pinsage_ctx *ctx, DType dt, int64_t N, int32_
         const int b = (int)(c & 1);
         if (two && c >= 2) PS_CUDA(ctx, cudaStreamWaitEvent(ps, ctx->ev_gemm[b], 0));
         if (tables_landed) PS_CUDA(ctx, cudaStreamWaitEvent(ps, tables_landed[c], 0));
+        StepRange r2("S2 pool k=%d rows %lld+%lld", ctx->cur_layer, (long long)r0, (long long)rows);
         const int pe0 = prof_mark(ctx, ps);
         cudaError_t e;
         if (hubs) {
@@ -550,7 +599,10 @@ pinsage_status pool_combine_chunks(pinsage_ctx *ctx, DType dt, int64_t N, int32_
         g.relu = 1;
         g.l2norm = 1;
         g.out = static_cast<char *>(Hout) + (size_t)r0 * lp->d * es;
-        PS_TRY(run_gemm(ctx, dt, g, scratch, scratch_bytes, ctx->stream));
+        {
+            StepRange r3("S3 combine k=%d rows %lld+%lld", ctx->cur_layer, (long long)r0, (long long)rows);
+            PS_TRY(run_gemm(ctx, dt, g, scratch, scratch_bytes, ctx->stream));
+        }
         if (two) PS_CUDA(ctx, cudaEventRecord(ctx->ev_gemm[b], ctx->stream));
         if (after_chunk) PS_TRY(after_chunk(r0, rows));
     }
@@ -626,6 +678,7 @@ pinsage_status layer_on_ws(pinsage_ctx *ctx, DType dt, int64_t N, int32_t T, con
         g.bias = lp->q;
         g.relu = 1;
         g.out = linear ? ws + plan.Pc_off : ws + plan.P_off + (size_t)r0 * lp->m * es;
+        StepRange r1("S1 project k=%d rows %lld+%lld", ctx->cur_layer, (long long)r0, (long long)g.M);
         PS_TRY(run_gemm(ctx, dt, g, ws + plan.scratch_off, plan.scratch_bytes, ctx->stream));
         if (linear) {                          // P'[chunk] = P[chunk] W2^T (W2 = columns d_in.. of W)
             GemmArgs g2;
@@ -636,7 +689,7 @@ pinsage_status layer_on_ws(pinsage_ctx *ctx, DType dt, int64_t N, int32_t T, con
             g2.B = static_cast<const char *>(lp->W) + (size_t)lp->d_in * es;
             g2.ldb = lp->d_in + lp->m;
             g2.out = ws + plan.P_off + (size_t)r0 * lp->d * es;
-            PS_TRY(run_gemm(ctx, dt, g2, ws + plan.scratch_off, plan.scratch_bytes, ctx->stream));
+            PS_TRY(run_gemm(ctx, dt, g2, ws + plan.scratch_off, plan.scratch_bytes, ctx->stream, PROF_AUX));
         }
     }
     return pool_combine_chunks(ctx, dt, N, T, lp, feats, ws + plan.P_off, idx, w, out, chunk,
@@ -714,6 +767,7 @@ pinsage_status pinsage_create(pinsage_ctx **out, int device, void *cuda_stream)
     ok = ok && cudaEventCreateWithFlags(&ctx->ev_fork, cudaEventDisableTiming) == cudaSuccess;
     ok = ok && cudaEventCreateWithFlags(&ctx->ev_join, cudaEventDisableTiming) == cudaSuccess;
     ok = ok && cudaMalloc(&ctx->d_first_bad, sizeof(long long)) == cudaSuccess;
+    ok = ok && (ctx->tc = gemm_tc_state_create(ctx->num_sms)) != nullptr;
     if (!ok) {
         e = cudaGetLastError();
         pinsage_destroy(ctx);
@@ -748,6 +802,8 @@ void pinsage_destroy(pinsage_ctx *ctx)
     if (ctx->stage) cudaFree(ctx->stage);
     if (ctx->d_first_bad) cudaFree(ctx->d_first_bad);
     if (ctx->split_buf) cudaFree(ctx->split_buf);
+    if (ctx->hub_buf) cudaFree(ctx->hub_buf);
+    gemm_tc_state_destroy(ctx->tc);
     if (ctx->subA) cudaFree(ctx->subA);
     if (ctx->subB) cudaFree(ctx->subB);
     for (cudaEvent_t e : ctx->prof_events) cudaEventDestroy(e);
@@ -766,20 +822,9 @@ pinsage_status pinsage_set_option(pinsage_ctx *ctx, const char *key, int64_t val
     } else if (!strcmp(key, "gemm_cg")) {
         if (value < 0 || value > 2) return fail(ctx, PINSAGE_ERR_INVALID_ARG, "gemm_cg must be 0, 1 or 2");
         ctx->tune.cg = (int)value;
-    } else if (!strcmp(key, "gemm_ns")) {
-        if (value != 0 && value != 256 && value != 512)
-            return fail(ctx, PINSAGE_ERR_INVALID_ARG, "gemm_ns must be 0, 256 or 512");
-        ctx->tune.ns = (int)value;
     } else if (!strcmp(key, "gemm_gx")) {
         if (value < 0 || value > 2) return fail(ctx, PINSAGE_ERR_INVALID_ARG, "gemm_gx must be 0, 1 or 2");
         ctx->tune.gx = (int)value;
-    } else if (!strcmp(key, "gemm_nl")) {
-        if (value != 0 && value != 256 && value != 512)
-            return fail(ctx, PINSAGE_ERR_INVALID_ARG, "gemm_nl must be 0, 256 or 512");
-        ctx->tune.nl = (int)value;
-    } else if (!strcmp(key, "gemm_epi")) {
-        if (value < 0 || value > 2) return fail(ctx, PINSAGE_ERR_INVALID_ARG, "gemm_epi must be 0, 1 or 2");
-        ctx->tune.epi = (int)value;
     } else if (!strcmp(key, "check_indices")) {
         ctx->check_indices = value != 0;
     } else if (!strcmp(key, "overlap")) {
@@ -813,7 +858,8 @@ pinsage_status pinsage_set_option(pinsage_ctx *ctx, const char *key, int64_t val
 
 int64_t pinsage_launch_count(const pinsage_ctx *ctx) { return ctx ? ctx->total_launches : 0; }
 
-pinsage_status pinsage_profile_read(pinsage_ctx *ctx, int32_t kind, double *total_ms, int64_t *launches)
+pinsage_status pinsage_profile_read(pinsage_ctx *ctx, int32_t kind, int32_t layer, double *total_ms,
+                                    int64_t *launches)
 {
     if (!ctx) return PINSAGE_ERR_INVALID_ARG;
     DeviceGuard guard(ctx->device);
@@ -824,7 +870,7 @@ pinsage_status pinsage_profile_read(pinsage_ctx *ctx, int32_t kind, double *tota
     double ms = 0.0;
     int64_t n = 0;
     for (const auto &r : ctx->prof_recs) {
-        if (r.kind != kind) continue;
+        if (r.kind != kind || (layer > 0 && r.layer != layer)) continue;
         float t = 0.f;
         PS_CUDA(ctx, cudaEventElapsedTime(&t, ctx->prof_events[r.e0], ctx->prof_events[r.e1]));
         ms += t;
@@ -874,6 +920,8 @@ pinsage_status pinsage_pool(pinsage_ctx *ctx, pinsage_dtype dtype, int64_t n_dst
     if (n_dst < 0) return fail(ctx, PINSAGE_ERR_INVALID_ARG, "n_dst is negative");
     PS_TRY(check_graph_args(ctx, n_src, T));
     PS_TRY(check_dim(ctx, "m", m));
+    if ((size_t)m * elem_size(static_cast<DType>(dtype)) > 4096)
+        return fail(ctx, PINSAGE_ERR_UNSUPPORTED_SHAPE, "pool: rows of %d values exceed 4096 bytes", m);
     if (n_dst == 0) return PINSAGE_OK;
     PS_TRY(check_ptr(ctx, "P", P));
     PS_TRY(check_ptr(ctx, "nbr_idx", nbr_idx));
@@ -973,6 +1021,7 @@ pinsage_status pinsage_layer(pinsage_ctx *ctx, pinsage_dtype dtype, int64_t N, i
     PS_TRY(check_ptr(ctx, "out", out));
     const DType dt = static_cast<DType>(dtype);
     const size_t es = elem_size(dt);
+    PS_TRY(check_pool_width(ctx, dt, params));
     if (out == feats) {
         if (params->d != params->d_in)
             return fail(ctx, PINSAGE_ERR_INVALID_ARG, "out == feats requires d == d_in");
@@ -993,6 +1042,8 @@ pinsage_status pinsage_layer(pinsage_ctx *ctx, pinsage_dtype dtype, int64_t N, i
         base = static_cast<char *>(ctx->ws);
     }
     PS_TRY(maybe_validate(ctx, N, N, T, nbr_idx, nbr_w));
+    HintGuard hint(ctx, N);
+    ctx->cur_layer = 1;
     return layer_on_ws(ctx, dt, N, T, feats, nbr_idx, nbr_w, params, out, base, plan, chunk);
 }
 
@@ -1013,17 +1064,19 @@ pinsage_status pinsage_head(pinsage_ctx *ctx, pinsage_dtype dtype, int64_t N, co
     const int64_t chunk = auto_chunk(N, 0, (size_t)params->g1 * es);
     const size_t a_bytes = align_up((size_t)chunk * params->g1 * es, 256);
     PS_TRY(ensure_ws(ctx, a_bytes));
+    HintGuard hint(ctx, N);
     for (int64_t r0 = 0; r0 < N; r0 += chunk) {
         const int64_t rows = std::min(chunk, N - r0);
         GemmArgs g;
         g.M = rows; g.K1 = params->d; g.N = params->g1;
         g.A1 = static_cast<const char *>(h) + (size_t)r0 * params->d * es;
         g.B = params->G1; g.bias = params->g; g.relu = 1; g.out = ctx->ws;
-        PS_TRY(run_gemm(ctx, dt, g, nullptr, 0, ctx->stream));
+        StepRange r45("S4+S5 head rows %lld+%lld", (long long)r0, (long long)rows);
+        PS_TRY(run_gemm(ctx, dt, g, nullptr, 0, ctx->stream, PROF_HEAD1));
         GemmArgs g2;
         g2.M = rows; g2.K1 = params->g1; g2.N = params->d_out; g2.A1 = ctx->ws; g2.B = params->G2;
         g2.out = static_cast<char *>(out) + (size_t)r0 * params->d_out * es;
-        PS_TRY(run_gemm(ctx, dt, g2, nullptr, 0, ctx->stream));
+        PS_TRY(run_gemm(ctx, dt, g2, nullptr, 0, ctx->stream, PROF_HEAD2));
     }
     return PINSAGE_OK;
 }
@@ -1056,6 +1109,8 @@ pinsage_status pinsage_embed_all(pinsage_ctx *ctx, pinsage_dtype dtype, int64_t 
     PS_TRY(check_ptr(ctx, "out", out));
     const DType dt = static_cast<DType>(dtype);
     const size_t es = elem_size(dt);
+    for (int k = 0; k < K; ++k) PS_TRY(check_pool_width(ctx, dt, &layers[k]));
+    HintGuard hint(ctx, N);
     const size_t feats_bytes = (size_t)N * layers[0].d_in * es;
     const size_t tab_bytes = (size_t)N * T * 4;
     const size_t out_bytes = (size_t)N * head->d_out * es;
@@ -1211,11 +1266,12 @@ pinsage_status pinsage_embed_all(pinsage_ctx *ctx, pinsage_dtype dtype, int64_t 
         g.M = rows; g.K1 = head->d; g.N = head->g1;
         g.A1 = Hlast + (size_t)r0 * head->d * es;
         g.B = head->G1; g.bias = head->g; g.relu = 1; g.out = abuf;
-        PS_TRY(run_gemm(ctx, dt, g, nullptr, 0, ctx->stream));
+        StepRange r45("S4+S5 head rows %lld+%lld", (long long)r0, (long long)rows);
+        PS_TRY(run_gemm(ctx, dt, g, nullptr, 0, ctx->stream, PROF_HEAD1));
         GemmArgs g2;
         g2.M = rows; g2.K1 = head->g1; g2.N = head->d_out; g2.A1 = abuf; g2.B = head->G2;
         g2.out = static_cast<char *>(d_out) + (size_t)r0 * head->d_out * es;
-        PS_TRY(run_gemm(ctx, dt, g2, nullptr, 0, ctx->stream));
+        PS_TRY(run_gemm(ctx, dt, g2, nullptr, 0, ctx->stream, PROF_HEAD2));
         if (out_ready) {                      // this chunk of out goes home while the next one is computed
             const int64_t c = r0 / chunk;
             const size_t rb = (size_t)head->d_out * es;
@@ -1229,6 +1285,7 @@ pinsage_status pinsage_embed_all(pinsage_ctx *ctx, pinsage_dtype dtype, int64_t 
     for (int k = 0; k < K; ++k) {
         const pinsage_layer_params *lp = &layers[k];
         const LayerWs plan = plan_layer_ws(ctx, dt, N, lp, chunk);
+        ctx->cur_layer = k + 1;
         char *Hout;
         if (k == 0) Hout = Ha;
         else if (lp->d == lp->d_in) Hout = Hcur;           // in place (S1 has consumed all of H first)
@@ -1279,6 +1336,8 @@ pinsage_status pinsage_embed_nodes(pinsage_ctx *ctx, pinsage_dtype dtype, int64_
     PS_TRY(check_ptr(ctx, "out", out));
     const DType dt = static_cast<DType>(dtype);
     const size_t es = elem_size(dt);
+    for (int k = 0; k < K; ++k) PS_TRY(check_pool_width(ctx, dt, &layers[k]));
+    HintGuard hint(ctx, N);
     cudaStream_t st = ctx->stream;
     PS_TRY(maybe_validate(ctx, N, N, T, nbr_idx, nbr_w));
 
@@ -1348,6 +1407,7 @@ pinsage_status pinsage_embed_nodes(pinsage_ctx *ctx, pinsage_dtype dtype, int64_
                                         &ctx->launches));
         count_launches(ctx);
         const LayerWs plan = plan_layer_ws(ctx, dt, n[k - 1], lp, chunk[k]);
+        ctx->cur_layer = k;
         PS_TRY(layer_on_ws(ctx, dt, n[k], T, Hself, idx_loc, w_loc, lp, Hbuf[cur ^ 1], lws, plan, chunk[k],
                            nullptr, nullptr, n[k - 1], Hbuf[cur]));
         cur ^= 1;
@@ -1356,10 +1416,10 @@ pinsage_status pinsage_embed_nodes(pinsage_ctx *ctx, pinsage_dtype dtype, int64_
     GemmArgs g;
     g.M = n[K]; g.K1 = head->d; g.N = head->g1; g.A1 = Hbuf[cur]; g.B = head->G1; g.bias = head->g;
     g.relu = 1; g.out = abuf;
-    PS_TRY(run_gemm(ctx, dt, g, nullptr, 0, st));
+    PS_TRY(run_gemm(ctx, dt, g, nullptr, 0, st, PROF_HEAD1));
     GemmArgs g2;
     g2.M = n[K]; g2.K1 = head->g1; g2.N = head->d_out; g2.A1 = abuf; g2.B = head->G2; g2.out = obuf;
-    PS_TRY(run_gemm(ctx, dt, g2, nullptr, 0, st));
+    PS_TRY(run_gemm(ctx, dt, g2, nullptr, 0, st, PROF_HEAD2));
     PS_CUDA(ctx, subset_gather_rows(obuf, targets, pos(K), M, (size_t)head->d_out * es, out, st, &ctx->launches));
     count_launches(ctx);
     return PINSAGE_OK;
@@ -1534,6 +1594,55 @@ pinsage_status pinsage_build_neighbourhoods(pinsage_ctx *ctx, int64_t N, const i
                                                counts, ctx->stream, &ctx->launches);
     count_launches(ctx);
     PS_CUDA(ctx, e);
+    return PINSAGE_OK;
+}
+
+pinsage_status pinsage_calibrate(pinsage_ctx *ctx, int32_t kind, const void *table, size_t table_bytes,
+                                 int32_t row_bytes, int64_t n_dst, int32_t T, void *out, size_t out_bytes,
+                                 int32_t reps, double *ms)
+{
+    if (!ctx) return PINSAGE_ERR_INVALID_ARG;
+    DeviceGuard guard(ctx->device);
+    if (!ms) return fail(ctx, PINSAGE_ERR_INVALID_ARG, "ms is NULL");
+    *ms = 0.0;
+    PS_TRY(check_ptr(ctx, "table", table));
+    PS_TRY(check_ptr(ctx, "out", out));
+    if (reps < 1 || reps > 1000) return fail(ctx, PINSAGE_ERR_INVALID_ARG, "reps = %d outside [1, 1000]", reps);
+    int64_t n_src = 0;
+    if (kind == 0) {
+        if (table_bytes < 16 || out_bytes < (size_t)ctx->num_sms * 8 * 256 * 16)
+            return fail(ctx, PINSAGE_ERR_INVALID_ARG, "calibrate m1: out needs %zu bytes",
+                        (size_t)ctx->num_sms * 8 * 256 * 16);
+    } else if (kind == 1) {
+        if (row_bytes != 256 && row_bytes != 512 && row_bytes != 1024 && row_bytes != 2048)
+            return fail(ctx, PINSAGE_ERR_UNSUPPORTED_SHAPE, "calibrate: row_bytes must be 256, 512, 1024 or 2048");
+        n_src = (int64_t)(table_bytes / (size_t)row_bytes);
+        if (n_src < 1 || n_src >= (1LL << 31) || n_dst < 1 || T < 1 || T > 1024)
+            return fail(ctx, PINSAGE_ERR_INVALID_ARG, "calibrate: bad table size, n_dst or T");
+        if (out_bytes < (size_t)n_dst * row_bytes)
+            return fail(ctx, PINSAGE_ERR_INVALID_ARG, "calibrate: out needs n_dst x row_bytes bytes");
+    } else {
+        return fail(ctx, PINSAGE_ERR_INVALID_ARG, "calibrate: kind must be 0 (stream) or 1 (gather)");
+    }
+    cudaEvent_t e0, e1;
+    PS_CUDA(ctx, cudaEventCreate(&e0));
+    PS_CUDA(ctx, cudaEventCreate(&e1));
+    cudaError_t e = cudaSuccess;
+    for (int r = -1; r < reps && e == cudaSuccess; ++r) {          // one untimed warm-up launch
+        if (r == 0) e = cudaEventRecord(e0, ctx->stream);
+        if (e == cudaSuccess)
+            e = launch_calib(kind, table, table_bytes, row_bytes, n_src, n_dst, T, out, ctx->num_sms, ctx->stream,
+                             &ctx->launches);
+    }
+    if (e == cudaSuccess) e = cudaEventRecord(e1, ctx->stream);
+    if (e == cudaSuccess) e = cudaEventSynchronize(e1);
+    float t = 0.f;
+    if (e == cudaSuccess) e = cudaEventElapsedTime(&t, e0, e1);
+    cudaEventDestroy(e0);
+    cudaEventDestroy(e1);
+    count_launches(ctx);
+    PS_CUDA(ctx, e);
+    *ms = (double)t / reps;
     return PINSAGE_OK;
 }
 

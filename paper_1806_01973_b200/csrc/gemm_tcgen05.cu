@@ -26,8 +26,7 @@
 // per-row partial sums of squares through distributed shared memory.
 #include "internal.h"
 
-#include <cstdlib>
-#include <mutex>
+#include <new>
 #include <vector>
 
 #include <cuda.h>  // CUtensorMap and enums only; cuTensorMapEncodeTiled is fetched at run time
@@ -641,9 +640,13 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap tmA1, const __grid_constant__
                     }
                     const unsigned target = (unsigned)((it >> 1) + 1) * (unsigned)p.n_slabs;
                     if (lane == 0) {
-                        unsigned seen;
+                        // plain launch (gx 2): nothing but the idle device makes the peers co-resident,
+                        // so a wait that outlasts ~2^32 cycles traps (a loud error, not a hang)
+                        const long long t_start = p.gx == 2 ? clock64() : 0;
+                        unsigned seen, polls = 0;
                         do {
                             asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(seen) : "l"(cnt) : "memory");
+                            if (p.gx == 2 && (++polls & 0xfffu) == 0 && clock64() - t_start > (1LL << 32)) __trap();
                         } while (seen < target);
                     }
                     __syncwarp();
@@ -859,7 +862,7 @@ typedef CUresult (*EncodeTiledFn)(CUtensorMap *, CUtensorMapDataType, cuuint32_t
 
 EncodeTiledFn encode_fn()
 {
-    static EncodeTiledFn fn = [] {
+    static EncodeTiledFn fn = [] {          // (thread-safe: a C++11 function-local static)
         void *sym = nullptr;
         cudaDriverEntryPointQueryResult q;
         if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &sym, cudaEnableDefault, &q) != cudaSuccess ||
@@ -870,30 +873,101 @@ EncodeTiledFn encode_fn()
     return fn;
 }
 
-// Row-major bf16 matrix [rows x cols] (cols contiguous), box = box_rows x 64 columns, SWIZZLE_128B.
-// Out-of-bounds parts of a box read as zero and are not written.
-bool make_map(CUtensorMap *map, const void *ptr, long long rows, int cols, int box_rows, int ld = 0,
-              bool f32 = false)
+inline int round_up(int x, int a) { return (x + a - 1) / a * a; }
+
+}  // namespace
+
+// Everything the launcher remembers between calls lives here, one per context (internal.h).
+struct GemmTcState {
+    int num_sms = 0;
+    bool attr_set[2][2] = {{false, false}, {false, false}};            // [CG - 1][NCH - 1]
+    int clusters[2][2][MAX_CLUSTER + 1] = {};                          // co-resident clusters, 0 = not asked yet
+    struct GxSlot { cudaStream_t s; void *mem; };
+    std::vector<GxSlot> gx;                                            // exchange buffers, one per stream used
+    size_t gx_buf_bytes = 0, gx_cnt_bytes = 0;
+    // tensor maps by (pointer, shape): encoding one is a driver call, and a chunked layer reuses the
+    // same few dozen descriptors call after call
+    struct MapKey {
+        const void *ptr; long long rows; int cols, box_rows, ld, f32;
+        bool operator==(const MapKey &o) const
+        {
+            return ptr == o.ptr && rows == o.rows && cols == o.cols && box_rows == o.box_rows && ld == o.ld &&
+                   f32 == o.f32;
+        }
+    };
+    static constexpr int MAP_SLOTS = 512, MAP_WAYS = 4;
+    struct MapEntry { MapKey key; CUtensorMap map; bool used; };
+    std::vector<MapEntry> maps;
+    unsigned map_clock = 0;
+    long long map_hits = 0, map_misses = 0;
+};
+
+GemmTcState *gemm_tc_state_create(int num_sms)
+{
+    GemmTcState *st = new (std::nothrow) GemmTcState;
+    if (!st) return nullptr;
+    st->num_sms = num_sms;
+    // [2 parities][lanes][n_slabs][BM * cg] floats with lanes * n_slabs * cg <= num_sms CTAs, and
+    // [2][lanes][cg][4] arrival counters
+    st->gx_buf_bytes = (size_t)2 * num_sms * BM * sizeof(float);
+    st->gx_cnt_bytes = (size_t)2 * num_sms * 4 * sizeof(unsigned);
+    st->maps.resize(GemmTcState::MAP_SLOTS);
+    for (auto &m : st->maps) m.used = false;
+    return st;
+}
+
+void gemm_tc_state_destroy(GemmTcState *st)
+{
+    if (!st) return;
+    for (const auto &g : st->gx) cudaFree(g.mem);
+    delete st;
+}
+
+namespace {
+
+// Row-major matrix [rows x cols] (cols contiguous, bf16 or fp32), box = box_rows x 128 bytes,
+// SWIZZLE_128B.  Out-of-bounds parts of a box read as zero and are not written.
+const CUtensorMap *get_map(GemmTcState *st, const void *ptr, long long rows, int cols, int box_rows, int ld = 0,
+                           bool f32 = false)
 {
     EncodeTiledFn fn = encode_fn();
-    if (!fn) return false;
+    if (!fn) return nullptr;
+    const GemmTcState::MapKey key{ptr, rows, cols, box_rows, ld, f32 ? 1 : 0};
+    size_t h = reinterpret_cast<uintptr_t>(ptr) >> 4;
+    h = (h ^ (h >> 17) ^ (size_t)rows * 0x9E3779B1u ^ (size_t)cols * 0x85EBCA77u ^ (size_t)box_rows * 0xC2B2AE3Du ^
+         (size_t)ld * 0x27D4EB2Fu ^ (size_t)key.f32) & (GemmTcState::MAP_SLOTS / GemmTcState::MAP_WAYS - 1);
+    GemmTcState::MapEntry *set = st->maps.data() + h * GemmTcState::MAP_WAYS;
+    for (int w = 0; w < GemmTcState::MAP_WAYS; ++w)
+        if (set[w].used && set[w].key == key) {
+            ++st->map_hits;
+            return &set[w].map;
+        }
+    ++st->map_misses;
+    GemmTcState::MapEntry *e = &set[st->map_clock++ % GemmTcState::MAP_WAYS];
+    for (int w = 0; w < GemmTcState::MAP_WAYS; ++w)
+        if (!set[w].used) {
+            e = &set[w];
+            break;
+        }
     const int es = f32 ? 4 : 2;
     const cuuint64_t dims[2] = {(cuuint64_t)cols, (cuuint64_t)rows};
     const cuuint64_t strides[1] = {(cuuint64_t)(ld > 0 ? ld : cols) * es};
     const cuuint32_t box[2] = {(cuuint32_t)(128 / es), (cuuint32_t)box_rows};   // 128-byte rows
     const cuuint32_t estr[2] = {1, 1};
-    return fn(map, f32 ? CU_TENSOR_MAP_DATA_TYPE_FLOAT32 : CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 2,
-              const_cast<void *>(ptr), dims, strides, box,
-              estr, CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B,
-              CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
+    e->used = false;
+    if (fn(&e->map, f32 ? CU_TENSOR_MAP_DATA_TYPE_FLOAT32 : CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 2,
+           const_cast<void *>(ptr), dims, strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
+           CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+           CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) != CUDA_SUCCESS)
+        return nullptr;
+    e->key = key;
+    e->used = true;
+    return &e->map;
 }
 
-inline int round_up(int x, int a) { return (x + a - 1) / a * a; }
-
-// cg: CTAs per tile (1 or 2).  ns_pref: preferred slab width without a row norm (256 = double-buffered
-// accumulators, 512 = fewer operand bytes per flop but no epilogue overlap).
-bool plan(const GemmArgs &a, int cg, int ns_pref, int epi_pref, int nl_pref, int gx_pref, TcParams &p,
-          int &smem_bytes, const char **why)
+// cg: CTAs per tile (1 or 2).  Slabs without a row norm are 256 columns wide (double-buffered
+// accumulators: the epilogue of tile i overlaps the MMAs of tile i+1).
+bool plan(const GemmArgs &a, int cg, int gx_pref, TcParams &p, int &smem_bytes, const char **why)
 {
     auto no = [&](const char *msg) {
         if (why) *why = msg;
@@ -920,10 +994,11 @@ bool plan(const GemmArgs &a, int cg, int ns_pref, int epi_pref, int nl_pref, int
     p.K12 = a.K1 + a.K2;
     p.K1 = a.K1;
     p.N = a.N;
-    // a normalised row sits in the TMEM of one cluster: slabs of 512 columns (one accumulator), or of 256
-    // (two accumulators: the epilogue overlaps the next tile, at the price of a larger cluster)
-    const bool gx = a.l2norm && gx_pref && a.N > 512 && a.N <= 2048;   // 256-column slabs, exchange through global memory
-    const int slab_max = a.l2norm ? ((nl_pref == 256 || gx) ? 256 : 512) : ns_pref;
+    // a normalised row of up to 512 columns sits in the TMEM of one CTA (one accumulator); a wider one
+    // is cut into 256-column slabs (two accumulators each) whose partial norms are exchanged through
+    // global memory, or -- gx 0, and rows beyond 2048 columns -- into 512-column slabs inside a cluster
+    const bool gx = a.l2norm && gx_pref && a.N > 512 && a.N <= 2048;
+    const int slab_max = a.l2norm ? (gx ? 256 : 512) : 256;
     p.n_slabs = (a.N + slab_max - 1) / slab_max;
     p.NS = p.n_slabs == 1 ? round_up(a.N, 16) : round_up((a.N + p.n_slabs - 1) / p.n_slabs, 64);
     p.n_slabs = (a.N + p.NS - 1) / p.NS;
@@ -943,11 +1018,10 @@ bool plan(const GemmArgs &a, int cg, int ns_pref, int epi_pref, int nl_pref, int
     // epilogue, which is exposed when the accumulator is single-buffered (measured: S3 +3 % at config 3,
     // +8 % at config 4; the one-pass epilogues lose more from the 32 KB of extra staging than they
     // gain, and with double-buffered accumulators the epilogue is hidden anyway).  Used for row-norm
-    // GEMMs with a single accumulator when at least three operand stages still fit.
+    // GEMMs with a single accumulator when at least three operand stages still fit, and for the
+    // selection epilogue (ALU work per score, not stores).
     int fixed = 0;
-    // (the selection epilogue is ALU work per score, not stores: eight warps there as well)
-    const bool want8 = (a.sel_state && p.NS > 64 && epi_pref != 1) || (epi_pref == 2 && p.NS > 64) ||
-                       (epi_pref != 1 && a.l2norm && p.nacc != 2);
+    const bool want8 = (a.sel_state && p.NS > 64) || (a.l2norm && p.nacc != 2);
     for (p.epi_halves = want8 ? 2 : 1; p.epi_halves >= 1; --p.epi_halves) {
         p.stg_bytes = a.sel_state ? p.epi_halves * 4 * (SEL_Q * 32 * 8) : p.epi_halves * 4 * 2 * STG_WARP_BYTES;
         fixed = p.stg_bytes + BIAS_BYTES + BAR_BYTES + (p.epi_halves == 2 ? HALF_BYTES : 0) +
@@ -983,36 +1057,29 @@ bool plan(const GemmArgs &a, int cg, int ns_pref, int epi_pref, int nl_pref, int
 // The plan launch_gemm_tc will use: CTA pairs when the shape allows and the caller does not forbid it.
 bool plan_auto(const GemmArgs &a, const GemmTune &t, TcParams &p, int &smem_bytes, const char **why)
 {
-    const int ns = t.ns == 512 ? 512 : 256;
     // Pairs pay when the GEMM is tensor-bound (measured on B200: +12-14 % at config 3's shapes); on
     // the HBM-bound shapes (arithmetic intensity K N / (K + N) below ~160 flop per byte moved, e.g.
     // 256 x 256) single-CTA tiles keep more independent tiles in flight and are 15-35 % faster.
     const long long Kt = a.K1 + a.K2 + a.K3;
     const bool tensor_bound = Kt * a.N >= 160 * (Kt + a.N);
-    if ((t.cg == 2 || (t.cg == 0 && tensor_bound)) && plan(a, 2, ns, t.epi, t.nl, t.gx, p, smem_bytes, nullptr)) return true;
+    if ((t.cg == 2 || (t.cg == 0 && tensor_bound)) && plan(a, 2, t.gx, p, smem_bytes, nullptr)) return true;
     if (t.cg == 2) {
         if (why) *why = "shape not supported by the CTA-pair kernel";
         return false;
     }
-    return plan(a, 1, ns, t.epi, t.nl, t.gx, p, smem_bytes, why);
+    return plan(a, 1, t.gx, p, smem_bytes, why);
 }
 
 template <int CG, int NCH>
-cudaError_t launch_cg(const TcParams &p, int smem, int num_sms, cudaStream_t s, const CUtensorMap &tmA1,
+cudaError_t launch_cg(GemmTcState *st, const TcParams &p, int smem, cudaStream_t s, const CUtensorMap &tmA1,
                       const CUtensorMap &tmA2, const CUtensorMap &tmA3, const CUtensorMap &tmB,
                       const CUtensorMap &tmOut)
 {
-    // per-device function attribute and cluster-occupancy cache (a process may drive several devices)
-    static int attr_dev = -1;
-    static int cached_clusters[MAX_CLUSTER + 1] = {0};
-    int dev = 0;
-    cudaGetDevice(&dev);
-    if (attr_dev != dev) {
+    if (!st->attr_set[CG - 1][NCH - 1]) {
         cudaError_t e = cudaFuncSetAttribute(gemm_tc_kernel<CG, NCH>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                              SMEM_LIMIT);
         if (e != cudaSuccess) return e;
-        attr_dev = dev;
-        for (int &c : cached_clusters) c = 0;
+        st->attr_set[CG - 1][NCH - 1] = true;
     }
     cudaLaunchConfig_t cfg{};
     cfg.blockDim = dim3(NUM_THREADS);
@@ -1024,27 +1091,25 @@ cudaError_t launch_cg(const TcParams &p, int smem, int num_sms, cudaStream_t s, 
     attr[0].val.clusterDim.y = 1;
     attr[0].val.clusterDim.z = 1;
     // grid-wide norm exchange: the CTAs wait on each other, so the whole grid must be co-resident --
-    // a cooperative launch makes that a guarantee (it does not start until every CTA has an SM)
+    // a cooperative launch makes that a guarantee (it does not start until every CTA has an SM).
+    // gx == 2 asks for a plain launch (profilers that cannot replay a cooperative one): co-residency then
+    // rests on the persistent grid having the device to itself, and a wait that outlasts ~2 s traps.
     attr[1].id = cudaLaunchAttributeCooperative;
     attr[1].val.cooperative = 1;
     cfg.attrs = attr;
-    // gx == 2: plain launch, for profilers that cannot replay a cooperative one.  Nsight Compute is
-    // recognised by the variable it sets in the target process and gets the plain launch by itself
-    // (it serialises kernels, so the persistent grid has the device to itself).
-    static const bool profiled = getenv("NV_COMPUTE_PROFILER_PERFWORKS_DIR") != nullptr;
-    cfg.numAttrs = (p.gx == 1 && !profiled) ? 2 : 1;
+    cfg.numAttrs = p.gx == 1 ? 2 : 1;
 
     // co-resident clusters of this shape (cached: the query costs a driver call)
-    int max_clusters = cached_clusters[p.cluster];
+    int max_clusters = st->clusters[CG - 1][NCH - 1][p.cluster];
     if (max_clusters == 0) {
-        cfg.gridDim = dim3((unsigned)(num_sms / p.cluster * p.cluster));
+        cfg.gridDim = dim3((unsigned)(st->num_sms / p.cluster * p.cluster));
         cfg.dynamicSmemBytes = SMEM_LIMIT;
         if (cudaOccupancyMaxActiveClusters(&max_clusters, gemm_tc_kernel<CG, NCH>, &cfg) != cudaSuccess ||
             max_clusters < 1) {
             cudaGetLastError();
-            max_clusters = num_sms / p.cluster;
+            max_clusters = st->num_sms / p.cluster;
         }
-        cached_clusters[p.cluster] = max_clusters;
+        st->clusters[CG - 1][NCH - 1][p.cluster] = max_clusters;
         cfg.dynamicSmemBytes = (size_t)smem;
     }
     const int units_per_cluster = p.cluster / CG;
@@ -1053,6 +1118,7 @@ cudaError_t launch_cg(const TcParams &p, int smem, int num_sms, cudaStream_t s, 
     if (units > tiles) units = tiles;
     units = units / p.n_slabs * p.n_slabs;
     if (units < p.n_slabs) units = p.n_slabs;
+    if (p.gx && units * CG > st->num_sms) return cudaErrorLaunchOutOfResources;   // (never: one CTA per SM)
     if (p.tile_major) units = tiles;
     cfg.gridDim = dim3((unsigned)(units * CG));
     return cudaLaunchKernelEx(&cfg, gemm_tc_kernel<CG, NCH>, tmA1, tmA2, tmA3, tmB, tmOut, p);
@@ -1072,60 +1138,57 @@ bool gemm_tc_supported(const GemmArgs &a, const GemmTune &t, const char **why)
     return true;
 }
 
-size_t gemm_tc_scratch_bytes(const GemmArgs &) { return 0; }
-
-cudaError_t launch_gemm_tc(const GemmArgs &a, const GemmTune &t, int num_sms, cudaStream_t s, int *launches)
+cudaError_t launch_gemm_tc(const GemmArgs &a, const GemmTune &t, GemmTcState *st, cudaStream_t s, int *launches)
 {
     TcParams p;
     int smem = 0;
+    if (!st) return cudaErrorInvalidValue;
     if (!plan_auto(a, t, p, smem, nullptr)) return cudaErrorNotSupported;
-    CUtensorMap tmA1, tmA2, tmA3, tmB, tmOut;
-    if (!make_map(&tmA1, a.A1, a.M, a.K1, BM)) return cudaErrorInvalidValue;
+    // (maps are copied out of the cache: a later get_map may evict the entry a pointer refers to)
+    const CUtensorMap *m = get_map(st, a.A1, a.M, a.K1, BM);
+    if (!m) return cudaErrorInvalidValue;
+    const CUtensorMap tmA1 = *m;
+    CUtensorMap tmA2 = tmA1, tmA3 = tmA1;
     if (a.K2 > 0) {
-        if (!make_map(&tmA2, a.A2, a.M, a.K2, BM)) return cudaErrorInvalidValue;
-    } else {
-        tmA2 = tmA1;
+        if (!(m = get_map(st, a.A2, a.M, a.K2, BM))) return cudaErrorInvalidValue;
+        tmA2 = *m;
     }
     if (a.K3 > 0) {
-        if (!make_map(&tmA3, a.A3, a.M, a.K3, BM)) return cudaErrorInvalidValue;
-    } else {
-        tmA3 = tmA1;
+        if (!(m = get_map(st, a.A3, a.M, a.K3, BM))) return cudaErrorInvalidValue;
+        tmA3 = *m;
     }
-    if (!make_map(&tmB, a.B, a.b_rows > 0 ? a.b_rows : a.N, a.K1 + a.K2 + a.K3, p.CN / p.cg, a.ldb))
+    if (!(m = get_map(st, a.B, a.b_rows > 0 ? a.b_rows : a.N, a.K1 + a.K2 + a.K3, p.CN / p.cg, a.ldb)))
         return cudaErrorInvalidValue;
-    if (!make_map(&tmOut, a.out, a.M, a.N, 32, 0, a.out_f32 != 0)) return cudaErrorInvalidValue;
+    const CUtensorMap tmB = *m;
+    // (the selection epilogue stores nothing: its output map is never used)
+    CUtensorMap tmOut = tmA1;
+    if (!a.sel_state) {
+        if (!(m = get_map(st, a.out, a.M, a.N, 32, 0, a.out_f32 != 0))) return cudaErrorInvalidValue;
+        tmOut = *m;
+    }
     if (launches) ++*launches;
     if (p.gx) {
-        // exchange buffers of the grid-wide row-norm exchange: one allocation per device, arrival
-        // counters zeroed before every launch (stream order)
-        constexpr size_t BUF = (size_t)2 * 148 * 8 * 256 * 4, CNT = (size_t)2 * 148 * 2 * 4 * 4;
-        // one buffer per (device, stream): launches on different streams may overlap in time
-        struct GxSlot { int dev; cudaStream_t s; void *mem; };
-        static std::mutex gx_mutex;
-        static std::vector<GxSlot> gx_slots;
-        int dev = 0;
-        cudaGetDevice(&dev);
+        // exchange buffers of the grid-wide row-norm exchange: one per stream this context has used
+        // (launches on different streams may overlap in time); arrival counters are zeroed before
+        // every launch, in stream order
         void *mem = nullptr;
-        {
-            std::lock_guard<std::mutex> lock(gx_mutex);
-            for (const GxSlot &g : gx_slots)
-                if (g.dev == dev && g.s == s) mem = g.mem;
-            if (!mem) {
-                cudaError_t e = cudaMalloc(&mem, BUF + CNT);
-                if (e != cudaSuccess) return e;
-                gx_slots.push_back({dev, s, mem});
-            }
+        for (const auto &g : st->gx)
+            if (g.s == s) mem = g.mem;
+        if (!mem) {
+            cudaError_t e = cudaMalloc(&mem, st->gx_buf_bytes + st->gx_cnt_bytes);
+            if (e != cudaSuccess) return e;
+            st->gx.push_back({s, mem});
         }
         p.gx_buf = static_cast<float *>(mem);
-        p.gx_cnt = reinterpret_cast<unsigned *>(static_cast<char *>(mem) + BUF);
-        cudaError_t e = cudaMemsetAsync(p.gx_cnt, 0, CNT, s);
+        p.gx_cnt = reinterpret_cast<unsigned *>(static_cast<char *>(mem) + st->gx_buf_bytes);
+        cudaError_t e = cudaMemsetAsync(p.gx_cnt, 0, st->gx_cnt_bytes, s);
         if (e != cudaSuccess) return e;
     }
     if (p.cg == 2)
-        return p.nchunks == 2 ? launch_cg<2, 2>(p, smem, num_sms, s, tmA1, tmA2, tmA3, tmB, tmOut)
-                              : launch_cg<2, 1>(p, smem, num_sms, s, tmA1, tmA2, tmA3, tmB, tmOut);
-    return p.nchunks == 2 ? launch_cg<1, 2>(p, smem, num_sms, s, tmA1, tmA2, tmA3, tmB, tmOut)
-                          : launch_cg<1, 1>(p, smem, num_sms, s, tmA1, tmA2, tmA3, tmB, tmOut);
+        return p.nchunks == 2 ? launch_cg<2, 2>(st, p, smem, s, tmA1, tmA2, tmA3, tmB, tmOut)
+                              : launch_cg<2, 1>(st, p, smem, s, tmA1, tmA2, tmA3, tmB, tmOut);
+    return p.nchunks == 2 ? launch_cg<1, 2>(st, p, smem, s, tmA1, tmA2, tmA3, tmB, tmOut)
+                          : launch_cg<1, 1>(st, p, smem, s, tmA1, tmA2, tmA3, tmB, tmOut);
 }
 
 }  // namespace pinsage

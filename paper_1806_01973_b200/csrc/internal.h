@@ -50,22 +50,25 @@ cudaError_t launch_gemm_simt(DType dt, const GemmArgs &a, float *ztmp, cudaStrea
 size_t gemm_simt_scratch_bytes(const GemmArgs &a);
 
 // ---- gemm_tcgen05.cu: tcgen05 / TMEM / TMA GEMM, bf16 in, fp32 accumulate ----------------------
-// Tuning knobs (context options "gemm_cg", "gemm_ns"): cg 0 = automatic (CTA pairs, cta_group::2,
-// whenever the shape allows), 1 = single-CTA tiles only, 2 = CTA pairs or fail; ns = slab width of
-// GEMMs without a row norm (0 / 256 = double-buffered accumulators, 512 = wider tile).
+// Diagnostic knobs (context options "gemm_cg", "gemm_gx"; tests and profiling only).
 struct GemmTune {
-    int cg = 0;
-    int ns = 0;
-    int epi = 0;   // epilogue warps: 0 = automatic (8 when they fit), 1 = always 4
-    int nl = 0;    // slab width of row-norm GEMMs: 0 / 512 = one accumulator per CTA, 256 = two
-    int gx = 1;    // 1: row-norm GEMMs wider than 512 use 256-column slabs and exchange the norms through
-                   // global memory between co-resident CTA pairs (no cluster: all SMs, hidden epilogue),
-                   // cooperative launch; 2: the same with a plain launch (profilers); 0: cluster exchange
+    int cg = 0;    // 0 = automatic (CTA pairs, cta_group::2, when the GEMM is tensor-bound), 1 = single-CTA
+                   // tiles only, 2 = CTA pairs or fail
+    int gx = 1;    // row-norm GEMMs wider than 512 columns: 1 = 256-column slabs, the norms exchanged through
+                   // global memory between co-resident CTA pairs, cooperative launch; 2 = the same with a
+                   // plain launch (Nsight Compute cannot replay a cooperative one; a wait that outlasts
+                   // ~2 s traps instead of hanging); 0 = 512-column slabs exchanged inside a cluster
 };
-// Returns cudaErrorNotSupported for shapes outside the compiled set (caller reports UNSUPPORTED_SHAPE).
+// Per-context state of the launcher: function attributes already set, co-resident cluster counts, the
+// exchange buffers of the grid-wide row-norm exchange (one per stream used, sized from the SM count),
+// cached tensor maps.  Owned by the pinsage_ctx, freed with it; not thread-safe (neither is a context).
+struct GemmTcState;
+GemmTcState *gemm_tc_state_create(int num_sms);
+void gemm_tc_state_destroy(GemmTcState *st);
+// Shapes outside the compiled set: gemm_tc_supported is false / launch returns cudaErrorNotSupported
+// (the caller reports PINSAGE_ERR_UNSUPPORTED_SHAPE).
 bool gemm_tc_supported(const GemmArgs &a, const GemmTune &t, const char **why);
-cudaError_t launch_gemm_tc(const GemmArgs &a, const GemmTune &t, int num_sms, cudaStream_t s, int *launches);
-size_t gemm_tc_scratch_bytes(const GemmArgs &a);
+cudaError_t launch_gemm_tc(const GemmArgs &a, const GemmTune &t, GemmTcState *st, cudaStream_t s, int *launches);
 
 // ---- split_f32.cu: fp32 operands as K-concatenated bf16 planes (fp32 mode on the tensor cores) ----
 // out [rows x 6 (K1 + K2)] bf16 from [S1 | S2] (fp32, row strides ld1 / ld2; all multiples of 4).
@@ -89,6 +92,10 @@ cudaError_t launch_normalize_counts(int64_t N, int32_t T, const int32_t *counts,
 // first_bad: device int64, set to the smallest offending flat position or -1
 cudaError_t launch_validate(int64_t n_dst, int64_t n_src, int32_t T, const int32_t *idx,
                             const float *w, long long *first_bad, cudaStream_t s, int *launches);
+
+// ---- calib.cu: calibration kernels of the roofline report (not on the product path) ---------------
+cudaError_t launch_calib(int kind, const void *buf, size_t bytes, int row_bytes, long long n_src, long long n_dst,
+                         int T, void *out, int num_sms, cudaStream_t s, int *launches);
 
 // ---- hubs.cu: the hub part of the pool on skewed graphs as a GEMM (see the file header) ----------
 cudaError_t launch_hub_select(const int32_t *idx, int64_t N, int32_t T, int64_t n_src, int32_t H,
