@@ -110,6 +110,12 @@ const char *pinsage_version(void);
  *                    first (synchronous), default 0
  *   "overlap"        1 = pinsage_layer / embed_all run S2 of chunk c+1 and S3 of chunk c on two streams
  *                    (default 0: measured no faster on B200, the pool's CTAs fill the device first)
+ *   "mem_limit_mb"   bytes (in MiB) of device memory pinsage_embed_all may plan with for its workspace and
+ *                    staging; 0 (default) = what cudaMemGetInfo reports free at the call, less a margin.
+ *                    The plan keeps P and one H resident (none when a device `out` as wide as every layer
+ *                    can serve as H), stages host inputs whole when that fits and streams them through
+ *                    rings of chunk slots otherwise, and halves the chunk (down to 16384 rows) before it
+ *                    gives up with PINSAGE_ERR_OOM.
  *   "pool_mode"      the aggregator gamma of Alg. 1 l.1 used by pinsage_pool / layer / embed_all /
  *                    embed_nodes: 0 = importance pooling, the weighted sum (default); 1 = element-wise
  *                    mean, 2 = element-wise max of the T projected neighbour rows (the paper's ablation
@@ -135,6 +141,9 @@ const char *pinsage_version(void);
  *                    pinsage_profile_read (default 0)
  *
  * Diagnostic keys (tests and profiling; not part of the stable interface, results are unchanged):
+ *   "debug_poison"   1 = pinsage_embed_all fills every buffer with NaN patterns the moment the plan says it
+ *                    is dead (P after a layer's last pool, the pooled and head chunks after their consumer,
+ *                    a replaced H, ring slots): a read that the aliasing rules forbid shows in the output
  *   "gemm_cg"        tcgen05 tile owner: 0 = automatic (CTA pairs, cta_group::2, 256-row tiles, when the
  *                    GEMM is tensor-bound), 1 = single CTAs only, 2 = CTA pairs or UNSUPPORTED_SHAPE
  *   "gemm_gx"        row norms of S3 wider than 512 columns: 1 (default) = exchanged through global memory
@@ -147,6 +156,11 @@ pinsage_status pinsage_set_option(pinsage_ctx *ctx, const char *key, int64_t val
 
 /* Number of kernels this context has launched so far (for launch accounting in benchmarks). */
 int64_t pinsage_launch_count(const pinsage_ctx *ctx);
+
+/* Context-owned description of the memory plan the last pinsage_embed_all call chose, e.g.
+ * "chunk=1048576 chunks=48 H=out feats=staged tables=ring out=ring workspace=... staging=..." ("" before
+ * the first call).  Valid until the next pinsage_embed_all on this context. */
+const char *pinsage_last_plan(const pinsage_ctx *ctx);
 
 /* Per-kernel device time gathered while option "profile" is 1.  Synchronises the context's streams,
  * then sums the event-measured duration of every launch of `kind` (in layer `layer`, 1-based; 0 = all

@@ -23,7 +23,7 @@ STATUS = {0: "OK", 1: "INVALID_ARG", 2: "UNSUPPORTED_SHAPE", 3: "MISALIGNED", 4:
 # every symbol include/pinsage.h declares
 SYMBOLS = [
     "pinsage_create", "pinsage_destroy", "pinsage_last_error", "pinsage_version",
-    "pinsage_set_option", "pinsage_launch_count", "pinsage_profile_read", "pinsage_dense", "pinsage_pool",
+    "pinsage_set_option", "pinsage_launch_count", "pinsage_last_plan", "pinsage_profile_read", "pinsage_dense", "pinsage_pool",
     "pinsage_combine", "pinsage_layer", "pinsage_layer_workspace_bytes", "pinsage_head",
     "pinsage_embed_all", "pinsage_normalize_counts", "pinsage_validate_graph",
     "pinsage_build_neighbourhoods", "pinsage_embed_nodes", "pinsage_topk", "pinsage_calibrate",
@@ -74,6 +74,8 @@ def load_library() -> ctypes.CDLL:
     lib.pinsage_set_option.restype = ctypes.c_int
     lib.pinsage_launch_count.argtypes = [vp]
     lib.pinsage_launch_count.restype = i64
+    lib.pinsage_last_plan.argtypes = [vp]
+    lib.pinsage_last_plan.restype = ctypes.c_char_p
     lib.pinsage_profile_read.argtypes = [vp, i32, i32, ctypes.POINTER(ctypes.c_double),
                                          ctypes.POINTER(i64)]
     lib.pinsage_profile_read.restype = ctypes.c_int
@@ -192,6 +194,9 @@ class Context:
 
     def pinsage_launch_count(self) -> int:
         return int(self.lib.pinsage_launch_count(self.handle))
+
+    def pinsage_last_plan(self) -> str:
+        return self.lib.pinsage_last_plan(self.handle).decode()
 
     def pinsage_profile_read(self, kind: int, layer: int = 0):
         """(total_ms, launches) of kind 0 S2 / 1 S1 / 2 S3 / 3 S4 / 4 S5 / 5 linear-pool projection in

@@ -36,6 +36,8 @@ struct pinsage_ctx {
                                      // (pinsage_embed_nodes: same kernel choice as pinsage_embed_all)
     int check_indices = 0;
     int overlap = 0;
+    int poison = 0;                  // debug: buffers are filled with NaN patterns the moment they are dead
+    int64_t mem_limit = 0;           // bytes the context may own for one call (0 = what the device has free)
     int pool_mode = 0;               // aggregator gamma: 0 importance, 1 mean, 2 max
     int linear_pool = -1;            // pool the W2-projection (width d) instead of P (width m):
                                      // -1 automatic (when m > d), 0 never, 1 always
@@ -48,7 +50,7 @@ struct pinsage_ctx {
     void *stage = nullptr;           // device staging for host inputs / outputs
     size_t stage_bytes = 0;
     long long *d_first_bad = nullptr;
-    int pool_hubs = 0;               // hub-split pool (hubs.cu): 0 off, -1 automatic, H = 64..512 forced
+    int pool_hubs = -1;              // hub-split pool (hubs.cu): 0 off, -1 automatic (default), H = 64..512 forced
     struct HubState {                // valid during one pinsage_embed_all call
         int H = 0;
         const int32_t *src_idx = nullptr;   // the caller's table the remapped one stands for
@@ -59,8 +61,12 @@ struct pinsage_ctx {
         float *G = nullptr;                 // [H x d] fp32: P_hub W2^T
         void *Wext = nullptr;               // [d x (d_in + m + H)] bf16: [W1 | W2 | G^T]
     } hub;
-    void *hub_buf = nullptr;
-    size_t hub_bytes = 0;
+    void *hub_buf = nullptr, *hub_tab = nullptr;   // selection scratch; remapped table + per-layer matrices
+    size_t hub_bytes = 0, hub_tab_bytes = 0;
+    void *hub_sample = nullptr;      // sampled rows of a host table
+    size_t hub_sample_bytes = 0;
+    long long *hub_info_h = nullptr; // pinned: {hubs found, sampled entries they hold}
+    cudaEvent_t ev_hub = nullptr;
     int topk_fused = 1;              // pinsage_topk: select in the GEMM epilogue (1) or in a second pass over stored scores (0)
     int f32_split = -1;              // fp32 GEMMs on the tensor cores by bf16 splitting: -1 automatic, 0 never, 1 always
     void *split_buf = nullptr;       // bf16 planes of the operands of a split fp32 GEMM (grown on demand)
@@ -74,6 +80,7 @@ struct pinsage_ctx {
     std::vector<ProfRec> prof_recs;
     size_t prof_used = 0;
     std::string err;
+    std::string plan;                // description of the last pinsage_embed_all memory plan
 };
 
 namespace {
@@ -499,8 +506,24 @@ pinsage_status check_pool_width(pinsage_ctx *ctx, DType dt, const pinsage_layer_
     return PINSAGE_OK;
 }
 
-// Called on the compute stream's timeline right after rows [r0, r0 + rows) of a layer's output exist.
-using ChunkHook = std::function<pinsage_status(int64_t r0, int64_t rows)>;
+// Where the chunk loops of a layer get a chunk's inputs from and what happens around its steps.  Every
+// member may be empty: the arrays are then device arrays addressed by row offset.  pinsage_embed_all
+// fills them in when inputs arrive from the host (staged whole, or streamed through a ring of chunk
+// slots), and to run the head of a chunk right after its last S3.
+struct ChunkIO {
+    // before / after S1 of source chunk c (layer 1 of a host-feature call): the chunk's rows
+    std::function<pinsage_status(int64_t c, const void **src)> s1_in;
+    std::function<pinsage_status(int64_t c)> s1_done;
+    // before / after S2 of chunk c, on the pool's stream: the chunk's (id, weight) rows -- ids already
+    // remapped when hub_remapped (the hub-split pool on tables that came from the host)
+    std::function<pinsage_status(int64_t c, cudaStream_t ps, const int32_t **idx, const float **w)> tables_in;
+    std::function<pinsage_status(int64_t c, cudaStream_t ps)> tables_done;
+    bool hub_remapped = false;
+    // before S3 of chunk c: the chunk's own previous representations (the self segment)
+    std::function<pinsage_status(int64_t c, const void **self)> self_in;
+    // after S3 of chunk c: its self rows are consumed, its output rows exist
+    std::function<pinsage_status(int64_t c, int64_t r0, int64_t rows)> after_chunk;
+};
 
 // S2 + S3 over all destination rows in chunks; pool of chunk c+1 may overlap combine of chunk c.
 // Hin [N x d_in] (read), P [N x pw] (read), Hout [N x d] (written; may alias Hin iff d == d_in).
@@ -510,8 +533,7 @@ pinsage_status pool_combine_chunks(pinsage_ctx *ctx, DType dt, int64_t N, int32_
                                    const pinsage_layer_params *lp, const void *Hin, const void *P,
                                    const int32_t *idx, const float *w, void *Hout, int64_t chunk,
                                    void *nbuf0, void *nbuf1, void *scratch, size_t scratch_bytes,
-                                   const cudaEvent_t *tables_landed = nullptr, int64_t n_src = -1,
-                                   const ChunkHook &after_chunk = nullptr)
+                                   int64_t n_src, const ChunkIO &io)
 {
     if (n_src < 0) n_src = N;                // rows of P; N = destination rows
     const size_t es = elem_size(dt);
@@ -527,8 +549,8 @@ pinsage_status pool_combine_chunks(pinsage_ctx *ctx, DType dt, int64_t N, int32_
     cudaStream_t ps = two ? ctx->aux : ctx->stream;
     // hub-split pool (hubs.cu): the gather skips the hub entries; their term enters S3 as a third K
     // segment A [rows x H] against G = P_hub W2^T, appended to the layer's W once per layer
-    const bool hubs = ctx->hub.H > 0 && idx == ctx->hub.src_idx && !two && !linear && dt == DType::BF16 &&
-                      ctx->pool_mode == 0;
+    const bool hubs = ctx->hub.H > 0 && (io.hub_remapped || idx == ctx->hub.src_idx) && !two && !linear &&
+                      dt == DType::BF16 && ctx->pool_mode == 0;
     const int H = ctx->hub.H;
     if (hubs) {
         const int pe0 = prof_mark(ctx, ps);
@@ -554,33 +576,39 @@ pinsage_status pool_combine_chunks(pinsage_ctx *ctx, DType dt, int64_t N, int32_
         const int64_t r0 = c * chunk, rows = std::min(chunk, N - r0);
         const int b = (int)(c & 1);
         if (two && c >= 2) PS_CUDA(ctx, cudaStreamWaitEvent(ps, ctx->ev_gemm[b], 0));
-        if (tables_landed) PS_CUDA(ctx, cudaStreamWaitEvent(ps, tables_landed[c], 0));
-        StepRange r2("S2 pool k=%d rows %lld+%lld", ctx->cur_layer, (long long)r0, (long long)rows);
-        const int pe0 = prof_mark(ctx, ps);
-        cudaError_t e;
-        if (hubs) {
-            const int32_t *im = ctx->hub.idxm + (size_t)r0 * T;
-            const bool fusedA = pool_hub_fused_ok(dt, pw);     // the gather kernel also writes A
-            e = launch_pool(dt, 0, rows, T, pw, P, im, w + (size_t)r0 * T, nb[b], 0, ps, &ctx->launches, 1,
-                            fusedA ? ctx->hub.A : nullptr, H);
-            if (e == cudaSuccess && !fusedA)
-                e = launch_hub_matrix(im, w + (size_t)r0 * T, rows, T, H, 0, ctx->hub.A, ps, &ctx->launches);
-        } else {
-            e = launch_pool(dt, ctx->pool_mode, rows, T, pw, P, idx + (size_t)r0 * T, w + (size_t)r0 * T,
-                            nb[b], pick_slab(ctx, dt, n_src, T, pw), ps, &ctx->launches);
+        const int32_t *ic = hubs && !io.hub_remapped ? ctx->hub.idxm + (size_t)r0 * T : idx + (size_t)r0 * T;
+        const float *wc = w + (size_t)r0 * T;
+        if (io.tables_in) PS_TRY(io.tables_in(c, ps, &ic, &wc));
+        {
+            StepRange r2("S2 pool k=%d rows %lld+%lld", ctx->cur_layer, (long long)r0, (long long)rows);
+            const int pe0 = prof_mark(ctx, ps);
+            cudaError_t e;
+            if (hubs) {
+                const bool fusedA = pool_hub_fused_ok(dt, pw);     // the gather kernel also writes A
+                e = launch_pool(dt, 0, rows, T, pw, P, ic, wc, nb[b], 0, ps, &ctx->launches, 1,
+                                fusedA ? ctx->hub.A : nullptr, H);
+                if (e == cudaSuccess && !fusedA)
+                    e = launch_hub_matrix(ic, wc, rows, T, H, 0, ctx->hub.A, ps, &ctx->launches);
+            } else {
+                e = launch_pool(dt, ctx->pool_mode, rows, T, pw, P, ic, wc, nb[b], pick_slab(ctx, dt, n_src, T, pw), ps,
+                                &ctx->launches);
+            }
+            prof_close(ctx, PROF_POOL, pe0, ps);
+            count_launches(ctx);
+            PS_CUDA(ctx, e);
         }
-        prof_close(ctx, PROF_POOL, pe0, ps);
-        count_launches(ctx);
-        PS_CUDA(ctx, e);
+        if (io.tables_done) PS_TRY(io.tables_done(c, ps));
         if (two) {
             PS_CUDA(ctx, cudaEventRecord(ctx->ev_pool[b], ps));
             PS_CUDA(ctx, cudaStreamWaitEvent(ctx->stream, ctx->ev_pool[b], 0));
         }
+        const void *self = static_cast<const char *>(Hin) + (size_t)r0 * lp->d_in * es;
+        if (io.self_in) PS_TRY(io.self_in(c, &self));
         GemmArgs g;
         g.M = rows;
         g.K1 = lp->d_in;
         g.N = lp->d;
-        g.A1 = static_cast<const char *>(Hin) + (size_t)r0 * lp->d_in * es;
+        g.A1 = self;
         g.B = lp->W;
         if (linear) {                        // z = H W1^T + pooled(P W2^T) + w
             g.ldb = lp->d_in + lp->m;
@@ -604,12 +632,16 @@ pinsage_status pool_combine_chunks(pinsage_ctx *ctx, DType dt, int64_t N, int32_
             PS_TRY(run_gemm(ctx, dt, g, scratch, scratch_bytes, ctx->stream));
         }
         if (two) PS_CUDA(ctx, cudaEventRecord(ctx->ev_gemm[b], ctx->stream));
-        if (after_chunk) PS_TRY(after_chunk(r0, rows));
+        if (ctx->poison)                     // the pooled chunk is dead once S3 has consumed it
+            PS_CUDA(ctx, cudaMemsetAsync(nb[b], 0xFF, (size_t)rows * pw * es, ctx->stream));
+        if (io.after_chunk) PS_TRY(io.after_chunk(c, r0, rows));
     }
     if (two) {
         PS_CUDA(ctx, cudaEventRecord(ctx->ev_join, ps));
         PS_CUDA(ctx, cudaStreamWaitEvent(ctx->stream, ctx->ev_join, 0));
     }
+    if (ctx->poison)                         // P is dead once the layer's last pool has run
+        PS_CUDA(ctx, cudaMemsetAsync(const_cast<void *>(P), 0xFF, (size_t)n_src * pw * es, ctx->stream));
     return PINSAGE_OK;
 }
 
@@ -649,37 +681,31 @@ LayerWs plan_layer_ws(const pinsage_ctx *ctx, DType dt, int64_t N, const pinsage
     return p;
 }
 
-// feats_landed / tables_landed (host-buffer pipeline of pinsage_embed_all, layer 1 only): per-chunk
-// events recorded on the copy stream.  With feats_landed S1 runs chunk by chunk behind the copies.
-pinsage_status layer_on_ws(pinsage_ctx *ctx, DType dt, int64_t N, int32_t T, const void *feats,
-                           const int32_t *idx, const float *w, const pinsage_layer_params *lp,
-                           void *out, char *ws, const LayerWs &plan, int64_t chunk,
-                           const cudaEvent_t *feats_landed = nullptr,
-                           const cudaEvent_t *tables_landed = nullptr, int64_t n_src = -1,
-                           const void *src_feats = nullptr, const ChunkHook &after_chunk = nullptr)
+// S1 of one layer on a planned workspace: P = ReLU(src Q^T + q) over the n_src source rows -- in one
+// launch, or chunk by chunk when the features arrive from the host (io.s1_in) or the linear-pool
+// schedule projects P W2^T per chunk.
+pinsage_status project_chunks(pinsage_ctx *ctx, DType dt, int64_t n_src, const pinsage_layer_params *lp,
+                              const void *src_feats, char *ws, const LayerWs &plan, int64_t chunk,
+                              const ChunkIO &io)
 {
-    // n_src / src_feats (targeted inference): the source rows S1 projects differ from the N
-    // destination rows, whose own previous representations are `feats`
     const size_t es = elem_size(dt);
     const bool linear = use_linear_pool(ctx, lp);
-    if (n_src < 0) {
-        n_src = N;
-        src_feats = feats;
-    }
-    const int64_t s1_rows = (feats_landed || linear) ? chunk : n_src;
+    const int64_t s1_rows = (io.s1_in || linear) ? chunk : n_src;
     for (int64_t r0 = 0, c = 0; r0 < n_src; r0 += s1_rows, ++c) {
-        if (feats_landed) PS_CUDA(ctx, cudaStreamWaitEvent(ctx->stream, feats_landed[c], 0));
+        const void *src = static_cast<const char *>(src_feats) + (size_t)r0 * lp->d_in * es;
+        if (io.s1_in) PS_TRY(io.s1_in(c, &src));
         GemmArgs g;
         g.M = std::min(s1_rows, n_src - r0);
         g.K1 = lp->d_in;
         g.N = lp->m;
-        g.A1 = static_cast<const char *>(src_feats) + (size_t)r0 * lp->d_in * es;
+        g.A1 = src;
         g.B = lp->Q;
         g.bias = lp->q;
         g.relu = 1;
         g.out = linear ? ws + plan.Pc_off : ws + plan.P_off + (size_t)r0 * lp->m * es;
         StepRange r1("S1 project k=%d rows %lld+%lld", ctx->cur_layer, (long long)r0, (long long)g.M);
         PS_TRY(run_gemm(ctx, dt, g, ws + plan.scratch_off, plan.scratch_bytes, ctx->stream));
+        if (io.s1_done) PS_TRY(io.s1_done(c));
         if (linear) {                          // P'[chunk] = P[chunk] W2^T (W2 = columns d_in.. of W)
             GemmArgs g2;
             g2.M = g.M;
@@ -692,9 +718,25 @@ pinsage_status layer_on_ws(pinsage_ctx *ctx, DType dt, int64_t N, int32_t T, con
             PS_TRY(run_gemm(ctx, dt, g2, ws + plan.scratch_off, plan.scratch_bytes, ctx->stream, PROF_AUX));
         }
     }
+    return PINSAGE_OK;
+}
+
+// One layer: S1 over the source rows, then the S2 / S3 chunk loop over the N destination rows.
+// n_src / src_feats (targeted inference): the source rows S1 projects differ from the destination rows,
+// whose own previous representations are `feats`.
+pinsage_status layer_on_ws(pinsage_ctx *ctx, DType dt, int64_t N, int32_t T, const void *feats,
+                           const int32_t *idx, const float *w, const pinsage_layer_params *lp,
+                           void *out, char *ws, const LayerWs &plan, int64_t chunk, int64_t n_src = -1,
+                           const void *src_feats = nullptr, const ChunkIO &io = ChunkIO())
+{
+    if (n_src < 0) {
+        n_src = N;
+        src_feats = feats;
+    }
+    PS_TRY(project_chunks(ctx, dt, n_src, lp, src_feats, ws, plan, chunk, io));
     return pool_combine_chunks(ctx, dt, N, T, lp, feats, ws + plan.P_off, idx, w, out, chunk,
                                ws + plan.n0_off, ws + plan.n1_off, ws + plan.scratch_off,
-                               plan.scratch_bytes, tables_landed, n_src, after_chunk);
+                               plan.scratch_bytes, n_src, io);
 }
 
 // Grows the per-chunk event pool of the host-buffer pipeline to n events.
@@ -705,6 +747,339 @@ pinsage_status ensure_pipe_events(pinsage_ctx *ctx, size_t n)
         PS_CUDA(ctx, cudaEventCreateWithFlags(&e, cudaEventDisableTiming));
         ctx->pipe_events.push_back(e);
     }
+    return PINSAGE_OK;
+}
+
+// ---- host buffers of pinsage_embed_all ---------------------------------------------------------------
+// An input [N x row_bytes] that lives in host memory reaches the kernels chunk by chunk through device
+// slots: `depth` = number of chunks (the array is staged whole: copied once, valid for the rest of the
+// call) or a small ring that every pass over the chunks re-fills.  Copies run on the context's h2d stream;
+// `landed[slot]` orders a chunk's consumer behind its copy, `freed[slot]` the next copy into a slot
+// behind the slot's last consumer.  (cudaStreamWaitEvent looks at the LAST record of an event, so a
+// slot's `freed` is always recorded before the copy that waits for it is enqueued.)
+struct HostSrc {
+    const char *host = nullptr;
+    char *dev = nullptr;
+    size_t row_bytes = 0;
+    int64_t N = 0, chunk = 0, nchunks = 0;
+    int depth = 0;
+    bool whole = false, loaded = false;
+    cudaEvent_t *landed = nullptr, *freed = nullptr;
+    std::vector<char> used;                     // slot has had a consumer whose `freed` was recorded
+
+    bool active() const { return host != nullptr; }
+    int slot(int64_t c) const { return (int)(c % depth); }
+    char *ptr(int64_t c) const { return dev + (size_t)slot(c) * chunk * row_bytes; }
+
+    pinsage_status copy(pinsage_ctx *ctx, int64_t c)
+    {
+        const int sl = slot(c);
+        const int64_t r0 = c * chunk, rows = std::min(chunk, N - r0);
+        if (used[sl]) PS_CUDA(ctx, cudaStreamWaitEvent(ctx->h2d, freed[sl], 0));
+        PS_CUDA(ctx, cudaMemcpyAsync(ptr(c), host + (size_t)r0 * row_bytes, (size_t)rows * row_bytes,
+                                     cudaMemcpyHostToDevice, ctx->h2d));
+        PS_CUDA(ctx, cudaEventRecord(landed[sl], ctx->h2d));
+        return PINSAGE_OK;
+    }
+    // start of a pass over the chunks 0 .. nchunks-1: the first `depth` copies
+    pinsage_status begin_pass(pinsage_ctx *ctx)
+    {
+        if (!active() || loaded) return PINSAGE_OK;
+        for (int64_t c = 0; c < std::min<int64_t>(depth, nchunks); ++c) PS_TRY(copy(ctx, c));
+        return PINSAGE_OK;
+    }
+    // consumer side, on stream s: chunk c's rows
+    pinsage_status acquire(pinsage_ctx *ctx, int64_t c, cudaStream_t s, const void **p)
+    {
+        if (!loaded) PS_CUDA(ctx, cudaStreamWaitEvent(s, landed[slot(c)], 0));
+        *p = ptr(c);
+        return PINSAGE_OK;
+    }
+    // the consumer of chunk c has been enqueued on s: a ring slot may take chunk c + depth
+    pinsage_status release(pinsage_ctx *ctx, int64_t c, cudaStream_t s)
+    {
+        if (whole) {
+            if (c == nchunks - 1) loaded = true;
+            return PINSAGE_OK;
+        }
+        const int sl = slot(c);
+        if (ctx->poison) PS_CUDA(ctx, cudaMemsetAsync(ptr(c), 0xFF, (size_t)chunk * row_bytes, s));
+        PS_CUDA(ctx, cudaEventRecord(freed[sl], s));
+        used[sl] = 1;
+        if (c + depth < nchunks) PS_TRY(copy(ctx, c + depth));
+        return PINSAGE_OK;
+    }
+};
+
+// The output [N x row_bytes] of a call whose `out` is host memory: two chunk slots on the device, each
+// copied home on the d2h stream while the next chunk is computed into the other.
+struct HostSink {
+    char *host = nullptr, *dev = nullptr;
+    size_t row_bytes = 0;
+    int64_t chunk = 0;
+    cudaEvent_t ready[2] = {nullptr, nullptr}, copied[2] = {nullptr, nullptr};
+    bool used[2] = {false, false};
+
+    bool active() const { return host != nullptr; }
+    char *ptr(int64_t c) const { return dev + (size_t)(c & 1) * chunk * row_bytes; }
+    pinsage_status acquire(pinsage_ctx *ctx, int64_t c, cudaStream_t s)
+    {
+        if (used[c & 1]) PS_CUDA(ctx, cudaStreamWaitEvent(s, copied[c & 1], 0));
+        return PINSAGE_OK;
+    }
+    pinsage_status release(pinsage_ctx *ctx, int64_t c, int64_t r0, int64_t rows, cudaStream_t s)
+    {
+        const int sl = (int)(c & 1);
+        PS_CUDA(ctx, cudaEventRecord(ready[sl], s));
+        PS_CUDA(ctx, cudaStreamWaitEvent(ctx->d2h, ready[sl], 0));
+        PS_CUDA(ctx, cudaMemcpyAsync(host + (size_t)r0 * row_bytes, ptr(c), (size_t)rows * row_bytes,
+                                     cudaMemcpyDeviceToHost, ctx->d2h));
+        PS_CUDA(ctx, cudaEventRecord(copied[sl], ctx->d2h));
+        used[sl] = true;
+        return PINSAGE_OK;
+    }
+};
+
+// ---- memory plan of pinsage_embed_all -------------------------------------------
+// Resident by necessity: P (the one randomly accessed array) and one H buffer -- none when the caller's
+// device `out` can serve as H (every layer as wide as the output: same row stride, and a chunk's out rows
+// are written after its H rows were consumed) -- plus a second H only when layer widths change.
+// Everything else is per chunk.  Host inputs are staged whole when that fits (tables first: every layer
+// reads them; then the features: layer 1 reads them twice), else streamed through rings of RING chunk
+// slots per pass; a host output always leaves through two chunk slots.  When the plan does not fit the
+// budget (free device memory, or the "mem_limit_mb" option) the chunk is halved, down to 16384 rows.
+constexpr int RING = 3;
+
+struct EmbedPlan {
+    int64_t chunk = 0, nchunks = 0;
+    bool H_is_out = false, need_Hb = false, feats_whole = false, tabs_whole = false;
+    size_t max_layer_ws = 0, H_bytes = 0, a_bytes = 0, ws_total = 0;
+    size_t feats_off = 0, idx_off = 0, w_off = 0, out_off = 0, stage_total = 0;
+};
+
+pinsage_status plan_embed(pinsage_ctx *ctx, DType dt, int64_t N, int32_t T, int32_t K,
+                          const pinsage_layer_params *layers, const pinsage_head_params *head, int64_t chunk_nodes,
+                          bool h_feats, bool h_idx, bool h_w, bool h_out, EmbedPlan &pl)
+{
+    const size_t es = elem_size(dt);
+    const bool any_host = h_feats || h_idx || h_w || h_out;
+    // what this call may own: the device's free memory plus what the context already holds for it
+    size_t free_b = 0, total_b = 0;
+    PS_CUDA(ctx, cudaMemGetInfo(&free_b, &total_b));
+    size_t budget = free_b + ctx->ws_bytes + ctx->stage_bytes;
+    budget -= std::min(budget, std::max<size_t>(budget / 64, (size_t)128 << 20));     // allocator slack
+    if (ctx->mem_limit > 0) budget = std::min(budget, (size_t)ctx->mem_limit);
+    int32_t w_max = head->g1, d_max = 0;
+    pl.H_is_out = !h_out;
+    for (int k = 0; k < K; ++k) {
+        w_max = std::max(w_max, layers[k].m);
+        d_max = std::max(d_max, layers[k].d);
+        pl.H_is_out = pl.H_is_out && layers[k].d == head->d_out;
+        if (k > 0) pl.need_Hb = pl.need_Hb || layers[k].d != layers[k].d_in;
+    }
+    pl.H_bytes = align_up((size_t)N * d_max * es, 256);
+    int64_t chunk = auto_chunk(N, chunk_nodes, (size_t)w_max * es);
+    // host buffers: at least ~8 chunks so that copies and kernels overlap chunk by chunk
+    if (any_host && chunk_nodes == 0)
+        chunk = std::min<int64_t>(chunk, std::max<int64_t>(32768, ((N + 7) / 8 + 127) / 128 * 128));
+    size_t least = 0;
+    for (;;) {
+        pl.chunk = chunk;
+        pl.nchunks = (N + chunk - 1) / chunk;
+        pl.max_layer_ws = 0;
+        for (int k = 0; k < K; ++k)
+            pl.max_layer_ws = std::max(pl.max_layer_ws, plan_layer_ws(ctx, dt, N, &layers[k], chunk).total);
+        pl.a_bytes = align_up((size_t)chunk * head->g1 * es, 256);
+        pl.ws_total = pl.max_layer_ws + pl.H_bytes * ((pl.H_is_out ? 0 : 1) + (pl.need_Hb ? 1 : 0)) + pl.a_bytes;
+        const size_t feats_row = (size_t)layers[0].d_in * es, tab_row = (size_t)T * 4, out_row = (size_t)head->d_out * es;
+        auto bytes = [&](bool on, bool whole, size_t row) -> size_t {
+            if (!on) return 0;
+            return align_up(whole ? (size_t)N * row : (size_t)std::min<int64_t>(RING, pl.nchunks) * chunk * row, 256);
+        };
+        // whole staging where it fits: the tables first (read by every layer), then the features
+        for (int mode = 0; mode < 3; ++mode) {
+            pl.tabs_whole = mode < 2;
+            pl.feats_whole = mode < 1;
+            size_t off = 0;
+            pl.feats_off = off; off += bytes(h_feats, pl.feats_whole, feats_row);
+            pl.idx_off = off;   off += bytes(h_idx, pl.tabs_whole, tab_row);
+            pl.w_off = off;     off += bytes(h_w, pl.tabs_whole, tab_row);
+            pl.out_off = off;   off += h_out ? align_up((size_t)2 * chunk * out_row, 256) : 0;
+            pl.stage_total = off;
+            if (pl.ws_total + pl.stage_total <= budget) return PINSAGE_OK;
+            least = pl.ws_total + pl.stage_total;
+        }
+        if (chunk_nodes > 0) break;                        // the caller fixed the chunk
+        const int64_t smaller = std::max<int64_t>(16384, chunk / 2 / 128 * 128);
+        if (smaller >= chunk) break;
+        chunk = smaller;
+    }
+    return fail(ctx, PINSAGE_ERR_OOM,
+                "embed_all needs at least %zu bytes of device memory (P [N x m] and H [N x d] must be resident; "
+                "chunk of %lld rows) but only %zu are available%s",
+                least, (long long)chunk, budget, ctx->mem_limit > 0 ? " (option mem_limit_mb)" : "");
+}
+
+// The context's workspace and staging allocations at the planned sizes.  When one of them has to grow,
+// an oversized other one is released first, so that the pair never holds more than the plan.
+pinsage_status fit_buffers(pinsage_ctx *ctx, size_t ws_need, size_t stage_need)
+{
+    const bool grow = ws_need > ctx->ws_bytes || stage_need > ctx->stage_bytes;
+    if (grow) {
+        PS_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
+        PS_CUDA(ctx, cudaStreamSynchronize(ctx->aux));
+        if (ctx->ws && ctx->ws_bytes != ws_need) {
+            cudaFree(ctx->ws);
+            ctx->ws = nullptr;
+            ctx->ws_bytes = 0;
+        }
+        if (ctx->stage && ctx->stage_bytes != stage_need) {
+            cudaFree(ctx->stage);
+            ctx->stage = nullptr;
+            ctx->stage_bytes = 0;
+        }
+    }
+    PS_TRY(ensure_ws(ctx, ws_need));
+    if (stage_need) PS_TRY(ensure_stage(ctx, stage_need));
+    return PINSAGE_OK;
+}
+
+// ---- hub-split pool: shared by pinsage_layer, pinsage_embed_all and pinsage_embed_nodes, which must
+// take the same decision and pick the same hubs for their results to agree bit for bit ------------------
+struct HubPlan {                 // layout of ctx->hub_buf for one call
+    int H = 0;
+    int32_t *counts = nullptr, *rank = nullptr, *hub_ids = nullptr, *hub_loc = nullptr, *idxm = nullptr;
+    void *cand = nullptr;
+    long long *info = nullptr;
+    void *A = nullptr, *Ph = nullptr, *Wext = nullptr;
+    float *G = nullptr;
+    int64_t sampled = 0;         // entries of the sample
+};
+
+struct HubReset {                // the hub state is valid during one call only
+    pinsage_ctx *c;
+    ~HubReset() { c->hub = pinsage_ctx::HubState{}; }
+};
+
+// Whether the hub-split pool can apply to a call at all: the option, BF16 importance pooling on the
+// tcgen05 path, one stream, at least one layer on the m <= d schedule, a table of at least 2^22 entries.
+// Depends on the whole graph and the options only, never on chunks or on which nodes are embedded.
+bool hub_eligible(const pinsage_ctx *ctx, DType dt, int64_t N, int32_t T, int32_t K, const pinsage_layer_params *layers)
+{
+    if (ctx->pool_hubs == 0 || dt != DType::BF16 || ctx->pool_mode != 0 || ctx->gemm_impl != 0 || ctx->overlap ||
+        N * (int64_t)T < (1 << 22))
+        return false;
+    for (int k = 0; k < K; ++k)
+        if (!use_linear_pool(ctx, &layers[k])) return true;
+    return false;
+}
+
+// Picks the hubs of the whole graph's table for a call that runs `layers`, in two steps so that the one
+// read-back of the automatic mode hides behind work enqueued in between (S1 of the first layer):
+//   hub_select_begin   histogram of a sample of the lists (every (N / 16384)-th row: `sample` is the
+//                      device table itself with sample_n = N, or the gathered sample rows with sample_n =
+//                      their number), candidates, the H most listed ids and their ranks; asynchronous
+//   hub_select_finish  *use = the split is taken: forced, or -- automatic mode -- the sampled hubs hold a
+//                      third of the sampled entries (waits for the selection only, not for the stream);
+//                      then the storage of the split: [the remapped whole table,] A, P_hub, G, [W | G^T]
+// a_rows: rows of the per-chunk matrix A.  want_table: room for the remapped whole table (device tables).
+pinsage_status hub_select_begin(pinsage_ctx *ctx, DType dt, int64_t N, int32_t T, int32_t K,
+                                const pinsage_layer_params *layers, const int32_t *sample, int64_t sample_n, HubPlan &hp)
+{
+    hp = HubPlan{};
+    if (!hub_eligible(ctx, dt, N, T, K, layers)) return PINSAGE_OK;
+    const int H = ctx->pool_hubs > 0 ? ctx->pool_hubs : 128;
+    const size_t nB = align_up((size_t)N * 4, 256), candB = align_up(hub_cand_bytes(), 256);
+    const size_t idsB = align_up((size_t)H * 4, 256);
+    PS_TRY(ensure_buf(ctx, &ctx->hub_buf, &ctx->hub_bytes, 2 * nB + candB + 2 * idsB + 256, "hub selection scratch"));
+    if (!ctx->hub_info_h) {
+        PS_CUDA(ctx, cudaMallocHost(reinterpret_cast<void **>(&ctx->hub_info_h), 16));
+        PS_CUDA(ctx, cudaEventCreateWithFlags(&ctx->ev_hub, cudaEventDisableTiming));
+    }
+    char *hb = static_cast<char *>(ctx->hub_buf);
+    hp.H = H;
+    hp.counts = reinterpret_cast<int32_t *>(hb);
+    hp.rank = reinterpret_cast<int32_t *>(hb + nB);
+    hp.cand = hb + 2 * nB;
+    hp.hub_ids = reinterpret_cast<int32_t *>(hb + 2 * nB + candB);
+    hp.hub_loc = reinterpret_cast<int32_t *>(hb + 2 * nB + candB + idsB);
+    hp.info = reinterpret_cast<long long *>(hb + 2 * nB + candB + 2 * idsB);
+    StepRange r("hub selection");
+    cudaError_t e = launch_hub_select(sample, sample_n, T, N, H, hp.counts, hp.rank, hp.cand, hp.hub_ids, hp.info,
+                                      &hp.sampled, ctx->stream, &ctx->launches);
+    count_launches(ctx);
+    PS_CUDA(ctx, e);
+    if (ctx->pool_hubs < 0) {
+        PS_CUDA(ctx, cudaMemcpyAsync(ctx->hub_info_h, hp.info, 16, cudaMemcpyDeviceToHost, ctx->stream));
+        PS_CUDA(ctx, cudaEventRecord(ctx->ev_hub, ctx->stream));
+    }
+    return PINSAGE_OK;
+}
+
+pinsage_status hub_select_finish(pinsage_ctx *ctx, int64_t N, int32_t T, int32_t K, const pinsage_layer_params *layers,
+                                 int64_t a_rows, bool want_table, HubPlan &hp, bool *use)
+{
+    *use = false;
+    if (hp.H == 0) return PINSAGE_OK;
+    *use = true;
+    if (ctx->pool_hubs < 0) {              // automatic: worth it when the hubs hold a third of the entries
+        PS_CUDA(ctx, cudaEventSynchronize(ctx->ev_hub));
+        *use = ctx->hub_info_h[0] > 0 && 3 * ctx->hub_info_h[1] >= hp.sampled;
+    }
+    if (!*use) return PINSAGE_OK;
+    int32_t m_max = 0, dd_max = 0, kw_max = 0;
+    for (int k = 0; k < K; ++k) {
+        if (use_linear_pool(ctx, &layers[k])) continue;
+        m_max = std::max(m_max, layers[k].m);
+        dd_max = std::max(dd_max, layers[k].d);
+        kw_max = std::max(kw_max, layers[k].d_in + layers[k].m);
+    }
+    const int H = hp.H;
+    const size_t tabB = want_table ? align_up((size_t)N * T * 4, 256) : 0;
+    const size_t AB = align_up((size_t)a_rows * H * 2, 256), PhB = align_up((size_t)H * m_max * 2, 256);
+    const size_t GB = align_up((size_t)H * dd_max * 4, 256);
+    const size_t WB = align_up((size_t)dd_max * (kw_max + H) * 2, 256);
+    const size_t need = tabB + AB + PhB + GB + WB;
+    if (need > ctx->hub_tab_bytes) {       // no room left for the split's storage: the plain pool (a different
+        size_t free_b = 0, total_b = 0;    // rounding of the same function) instead of PINSAGE_ERR_OOM
+        if (cudaMemGetInfo(&free_b, &total_b) != cudaSuccess || need > free_b + ctx->hub_tab_bytes ||
+            (ctx->mem_limit > 0 && need > (size_t)ctx->mem_limit)) {
+            cudaGetLastError();
+            *use = false;
+            return PINSAGE_OK;
+        }
+    }
+    PS_TRY(ensure_buf(ctx, &ctx->hub_tab, &ctx->hub_tab_bytes, need, "hub-split pool storage"));
+    char *after = static_cast<char *>(ctx->hub_tab);
+    hp.idxm = reinterpret_cast<int32_t *>(after);
+    after += tabB;
+    hp.A = after;
+    hp.Ph = after + AB;
+    hp.G = reinterpret_cast<float *>(after + AB + PhB);
+    hp.Wext = after + AB + PhB + GB;
+    return PINSAGE_OK;
+}
+
+void hub_activate(pinsage_ctx *ctx, const HubPlan &hp, const int32_t *src_idx, const int32_t *idxm,
+                  const int32_t *hub_ids)
+{
+    ctx->hub.H = hp.H;
+    ctx->hub.src_idx = src_idx;
+    ctx->hub.idxm = idxm;
+    ctx->hub.hub_ids = hub_ids;
+    ctx->hub.A = hp.A;
+    ctx->hub.Ph = hp.Ph;
+    ctx->hub.G = hp.G;
+    ctx->hub.Wext = hp.Wext;
+}
+
+// whole-graph calls: hub entries of the table become -(rank + 1) in a remapped copy
+pinsage_status hub_remap_whole(pinsage_ctx *ctx, const HubPlan &hp, const int32_t *idx, int64_t N, int32_t T)
+{
+    cudaError_t e = launch_hub_remap(idx, hp.rank, N * (int64_t)T, hp.idxm, ctx->stream, &ctx->launches);
+    count_launches(ctx);
+    PS_CUDA(ctx, e);
+    hub_activate(ctx, hp, idx, hp.idxm, hp.hub_ids);
     return PINSAGE_OK;
 }
 
@@ -803,6 +1178,10 @@ void pinsage_destroy(pinsage_ctx *ctx)
     if (ctx->d_first_bad) cudaFree(ctx->d_first_bad);
     if (ctx->split_buf) cudaFree(ctx->split_buf);
     if (ctx->hub_buf) cudaFree(ctx->hub_buf);
+    if (ctx->hub_tab) cudaFree(ctx->hub_tab);
+    if (ctx->hub_sample) cudaFree(ctx->hub_sample);
+    if (ctx->hub_info_h) cudaFreeHost(ctx->hub_info_h);
+    if (ctx->ev_hub) cudaEventDestroy(ctx->ev_hub);
     gemm_tc_state_destroy(ctx->tc);
     if (ctx->subA) cudaFree(ctx->subA);
     if (ctx->subB) cudaFree(ctx->subB);
@@ -829,6 +1208,11 @@ pinsage_status pinsage_set_option(pinsage_ctx *ctx, const char *key, int64_t val
         ctx->check_indices = value != 0;
     } else if (!strcmp(key, "overlap")) {
         ctx->overlap = value != 0;
+    } else if (!strcmp(key, "debug_poison")) {
+        ctx->poison = value != 0;
+    } else if (!strcmp(key, "mem_limit_mb")) {
+        if (value < 0) return fail(ctx, PINSAGE_ERR_INVALID_ARG, "mem_limit_mb must be >= 0");
+        ctx->mem_limit = value << 20;
     } else if (!strcmp(key, "pool_mode")) {
         if (value < 0 || value > 2) return fail(ctx, PINSAGE_ERR_INVALID_ARG, "pool_mode must be 0, 1 or 2");
         ctx->pool_mode = (int)value;
@@ -857,6 +1241,8 @@ pinsage_status pinsage_set_option(pinsage_ctx *ctx, const char *key, int64_t val
 }
 
 int64_t pinsage_launch_count(const pinsage_ctx *ctx) { return ctx ? ctx->total_launches : 0; }
+
+const char *pinsage_last_plan(const pinsage_ctx *ctx) { return ctx ? ctx->plan.c_str() : ""; }
 
 pinsage_status pinsage_profile_read(pinsage_ctx *ctx, int32_t kind, int32_t layer, double *total_ms,
                                     int64_t *launches)
@@ -1044,7 +1430,16 @@ pinsage_status pinsage_layer(pinsage_ctx *ctx, pinsage_dtype dtype, int64_t N, i
     PS_TRY(maybe_validate(ctx, N, N, T, nbr_idx, nbr_w));
     HintGuard hint(ctx, N);
     ctx->cur_layer = 1;
-    return layer_on_ws(ctx, dt, N, T, feats, nbr_idx, nbr_w, params, out, base, plan, chunk);
+    HubReset hub_reset{ctx};
+    HubPlan hp;
+    bool use = false;
+    PS_TRY(hub_select_begin(ctx, dt, N, T, 1, params, nbr_idx, N, hp));
+    PS_TRY(project_chunks(ctx, dt, N, params, feats, base, plan, chunk, ChunkIO()));   // (hides the read-back)
+    PS_TRY(hub_select_finish(ctx, N, T, 1, params, chunk, true, hp, &use));
+    if (use) PS_TRY(hub_remap_whole(ctx, hp, nbr_idx, N, T));
+    return pool_combine_chunks(ctx, dt, N, T, params, feats, base + plan.P_off, nbr_idx, nbr_w, out, chunk,
+                               base + plan.n0_off, base + plan.n1_off, base + plan.scratch_off, plan.scratch_bytes, N,
+                               ChunkIO());
 }
 
 pinsage_status pinsage_head(pinsage_ctx *ctx, pinsage_dtype dtype, int64_t N, const void *h,
@@ -1117,190 +1512,214 @@ pinsage_status pinsage_embed_all(pinsage_ctx *ctx, pinsage_dtype dtype, int64_t 
     if (overlaps(feats, feats_bytes, out, out_bytes))
         return fail(ctx, PINSAGE_ERR_INVALID_ARG, "out overlaps feats");
 
-    // ---- host buffers: stage through context-owned device memory ------------------------------
+    // ---- where the arrays live, and the memory plan -------------------------------------------------
     const bool h_feats = is_host_ptr(feats), h_idx = is_host_ptr(nbr_idx), h_w = is_host_ptr(nbr_w);
     const bool h_out = is_host_ptr(out);
     const bool any_host = h_feats || h_idx || h_w || h_out;
-    size_t st_off = 0, st_feats = 0, st_idx = 0, st_w = 0, st_out = 0;
-    if (h_feats) { st_feats = st_off; st_off += align_up(feats_bytes, 256); }
-    if (h_idx) { st_idx = st_off; st_off += align_up(tab_bytes, 256); }
-    if (h_w) { st_w = st_off; st_off += align_up(tab_bytes, 256); }
-    if (h_out) { st_out = st_off; st_off += align_up(out_bytes, 256); }
-    if (any_host) PS_TRY(ensure_stage(ctx, st_off));
-    char *stage = static_cast<char *>(ctx->stage);
-    const void *d_feats = h_feats ? static_cast<const void *>(stage + st_feats) : feats;
-    const int32_t *d_idx = h_idx ? reinterpret_cast<const int32_t *>(stage + st_idx) : nbr_idx;
-    const float *d_w = h_w ? reinterpret_cast<const float *>(stage + st_w) : nbr_w;
-    void *d_out = h_out ? static_cast<void *>(stage + st_out) : out;
-
-    // ---- workspace plan: P | n0 | n1 | scratch | H_a | H_b | head chunk a ------------------------
-    int32_t w_max = head->g1;
-    for (int k = 0; k < K; ++k) w_max = std::max(w_max, layers[k].m);
-    int64_t chunk = auto_chunk(N, chunk_nodes, (size_t)w_max * es);
-    // host buffers: at least ~8 chunks so that copies and kernels overlap chunk by chunk
-    if (any_host && chunk_nodes == 0)
-        chunk = std::min<int64_t>(chunk, std::max<int64_t>(32768, ((N + 7) / 8 + 127) / 128 * 128));
-    const int64_t nchunks = (N + chunk - 1) / chunk;
-    size_t max_layer_ws = 0;
-    int32_t d_max = 0;
-    for (int k = 0; k < K; ++k) {
-        max_layer_ws = std::max(max_layer_ws, plan_layer_ws(ctx, dt, N, &layers[k], chunk).total);
-        d_max = std::max(d_max, layers[k].d);
+    EmbedPlan pl;
+    PS_TRY(plan_embed(ctx, dt, N, T, K, layers, head, chunk_nodes, h_feats, h_idx, h_w, h_out, pl));
+    const int64_t chunk = pl.chunk, nchunks = pl.nchunks;
+    {
+        char buf[256];
+        snprintf(buf, sizeof buf, "chunk=%lld chunks=%lld H=%s%s feats=%s tables=%s out=%s workspace=%zu staging=%zu",
+                 (long long)chunk, (long long)nchunks, pl.H_is_out ? "out" : "workspace", pl.need_Hb ? "+second" : "",
+                 !h_feats ? "device" : pl.feats_whole ? "staged" : "ring", !(h_idx || h_w) ? "device" : pl.tabs_whole ? "staged" : "ring",
+                 h_out ? "ring" : "device", pl.ws_total, pl.stage_total);
+        ctx->plan = buf;
     }
-    const size_t H_bytes = align_up((size_t)N * d_max * es, 256);
-    const size_t a_bytes = align_up((size_t)chunk * head->g1 * es, 256);
-    // layer k >= 2 with d == d_in runs in place on H_a; a second H buffer only when widths change
-    bool need_Hb = false;
-    for (int k = 1; k < K; ++k) need_Hb = need_Hb || layers[k].d != layers[k].d_in;
-    const size_t total = max_layer_ws + H_bytes * (need_Hb ? 2 : 1) + a_bytes;
-    PS_TRY(ensure_ws(ctx, total));
+    PS_TRY(fit_buffers(ctx, pl.ws_total, pl.stage_total));
     char *ws = static_cast<char *>(ctx->ws);
-    char *Ha = ws + max_layer_ws;
-    char *Hb = need_Hb ? Ha + H_bytes : nullptr;
-    char *abuf = Ha + H_bytes * (need_Hb ? 2 : 1);
+    char *stage = static_cast<char *>(ctx->stage);
+    char *Ha = pl.H_is_out ? static_cast<char *>(out) : ws + pl.max_layer_ws;
+    char *Hb = pl.need_Hb ? ws + pl.max_layer_ws + (pl.H_is_out ? 0 : pl.H_bytes) : nullptr;
+    char *abuf = ws + pl.max_layer_ws + pl.H_bytes * ((pl.H_is_out ? 0 : 1) + (pl.need_Hb ? 1 : 0));
 
-    // ---- host inputs: chunked H2D copies on the copy stream, features first, then the tables; the
-    // kernels of layer 1 follow them chunk by chunk (S1 behind the feature chunks, S2/S3 behind the
-    // table chunks), so that PCIe and the SMs work at the same time --------------------------------
-    const cudaEvent_t *feats_landed = nullptr, *tables_landed = nullptr;
-    cudaEvent_t *out_ready = nullptr;
+    // ---- host inputs / output: slots, events, the first copies (features first, then the tables: layer
+    // 1's S1 launches chase the feature chunks, its S2 / S3 the table chunks) --------------------------
+    HostSrc sF, sI, sW;
+    HostSink sO;
     if (any_host) {
-        PS_TRY(ensure_pipe_events(ctx, (size_t)3 * nchunks));
+        auto setup = [&](HostSrc &h, const void *p, size_t row_bytes, bool whole, size_t off) {
+            h.host = static_cast<const char *>(p);
+            h.dev = stage + off;
+            h.row_bytes = row_bytes;
+            h.N = N;
+            h.chunk = chunk;
+            h.nchunks = nchunks;
+            h.whole = whole;
+            h.depth = whole ? (int)nchunks : (int)std::min<int64_t>(RING, nchunks);
+            h.used.assign((size_t)h.depth, 0);
+        };
+        if (h_feats) setup(sF, feats, (size_t)layers[0].d_in * es, pl.feats_whole, pl.feats_off);
+        if (h_idx) setup(sI, nbr_idx, (size_t)T * 4, pl.tabs_whole, pl.idx_off);
+        if (h_w) setup(sW, nbr_w, (size_t)T * 4, pl.tabs_whole, pl.w_off);
+        size_t n_ev = 4;
+        for (HostSrc *h : {&sF, &sI, &sW}) n_ev += h->active() ? 2 * (size_t)h->depth : 0;
+        PS_TRY(ensure_pipe_events(ctx, n_ev));
         cudaEvent_t *ev = ctx->pipe_events.data();
-        // the staging buffers may still be read by kernels of an earlier call on the compute stream
+        for (HostSrc *h : {&sF, &sI, &sW})
+            if (h->active()) {
+                h->landed = ev;
+                h->freed = ev + h->depth;
+                ev += 2 * h->depth;
+            }
+        if (h_out) {
+            sO.host = static_cast<char *>(out);
+            sO.dev = stage + pl.out_off;
+            sO.row_bytes = (size_t)head->d_out * es;
+            sO.chunk = chunk;
+            sO.ready[0] = ev[0]; sO.ready[1] = ev[1]; sO.copied[0] = ev[2]; sO.copied[1] = ev[3];
+        }
+        // the staging slots may still be read by kernels of an earlier call on the compute stream
         PS_CUDA(ctx, cudaEventRecord(ctx->ev_fork, ctx->stream));
         PS_CUDA(ctx, cudaStreamWaitEvent(ctx->h2d, ctx->ev_fork, 0));
         PS_CUDA(ctx, cudaStreamWaitEvent(ctx->d2h, ctx->ev_fork, 0));
-        if (h_feats) {
-            const size_t rb = (size_t)layers[0].d_in * es;
-            for (int64_t c = 0; c < nchunks; ++c) {
-                const int64_t r0 = c * chunk, rows = std::min(chunk, N - r0);
-                PS_CUDA(ctx, cudaMemcpyAsync(stage + st_feats + r0 * rb, static_cast<const char *>(feats) + r0 * rb,
-                                             rows * rb, cudaMemcpyHostToDevice, ctx->h2d));
-                PS_CUDA(ctx, cudaEventRecord(ev[c], ctx->h2d));
-            }
-            feats_landed = ev;
-        }
-        if (h_idx || h_w) {
-            const size_t rb = (size_t)T * 4;
-            for (int64_t c = 0; c < nchunks; ++c) {
-                const int64_t r0 = c * chunk, rows = std::min(chunk, N - r0);
-                if (h_idx)
-                    PS_CUDA(ctx, cudaMemcpyAsync(stage + st_idx + r0 * rb, reinterpret_cast<const char *>(nbr_idx) + r0 * rb,
-                                                 rows * rb, cudaMemcpyHostToDevice, ctx->h2d));
-                if (h_w)
-                    PS_CUDA(ctx, cudaMemcpyAsync(stage + st_w + r0 * rb, reinterpret_cast<const char *>(nbr_w) + r0 * rb,
-                                                 rows * rb, cudaMemcpyHostToDevice, ctx->h2d));
-                PS_CUDA(ctx, cudaEventRecord(ev[nchunks + c], ctx->h2d));
-            }
-            tables_landed = ev + nchunks;
-        }
-        if (h_out) out_ready = ev + 2 * nchunks;
-        if (ctx->check_indices && tables_landed)     // validation reads whole tables: wait for all of them
-            PS_CUDA(ctx, cudaStreamWaitEvent(ctx->stream, tables_landed[nchunks - 1], 0));
     }
 
-    PS_TRY(maybe_validate(ctx, N, N, T, d_idx, d_w));
+    // ---- validation on request (whole tables: host tables are checked chunk by chunk as they land) ----
+    if (ctx->check_indices && !h_idx && !h_w) PS_TRY(maybe_validate(ctx, N, N, T, nbr_idx, nbr_w));
 
-    // ---- hub-split pool (skewed graphs; hubs.cu): pick the hubs from a sample of the lists, remap ----
-    struct HubReset {
-        pinsage_ctx *c;
-        ~HubReset() { c->hub.H = 0; }
-    } hub_reset{ctx};
-    if (ctx->pool_hubs != 0 && dt == DType::BF16 && ctx->pool_mode == 0 && ctx->gemm_impl == 0 && !ctx->overlap &&
-        !h_idx && !h_w && N * (int64_t)T >= (1 << 22)) {
-        const int H = ctx->pool_hubs > 0 ? ctx->pool_hubs : 128;
-        int32_t m_max = 0, dd_max = 0, kw_max = 0;
-        for (int k = 0; k < K; ++k) {
-            m_max = std::max(m_max, layers[k].m);
-            dd_max = std::max(dd_max, layers[k].d);
-            kw_max = std::max(kw_max, layers[k].d_in + layers[k].m);
+    // ---- hub-split pool (skewed graphs; hubs.cu): pick the hubs from a sample of the lists.  Device
+    // tables are remapped into a copy; tables from the host are remapped in their staging slots. -------
+    HubReset hub_reset{ctx};
+    bool hubs_on = false;
+    HubPlan hp;
+    {
+        const int64_t rows_s = std::min<int64_t>(N, 16384), stride = N / rows_s;
+        const int32_t *sample = nbr_idx;
+        int64_t sample_n = N;
+        if (h_idx && hub_eligible(ctx, dt, N, T, K, layers)) {
+            // every stride-th row of the host table, as the device path samples it: one strided copy
+            PS_TRY(ensure_buf(ctx, &ctx->hub_sample, &ctx->hub_sample_bytes, (size_t)rows_s * T * 4, "hub sample"));
+            PS_CUDA(ctx, cudaMemcpy2DAsync(ctx->hub_sample, (size_t)T * 4, nbr_idx, (size_t)stride * T * 4,
+                                           (size_t)T * 4, (size_t)rows_s, cudaMemcpyHostToDevice, ctx->stream));
+            sample = static_cast<const int32_t *>(ctx->hub_sample);
+            sample_n = rows_s;
         }
-        const size_t nB = align_up((size_t)N * 4, 256), candB = align_up(hub_cand_bytes(), 256);
-        const size_t idsB = align_up((size_t)H * 4, 256), tabB = align_up((size_t)N * T * 4, 256);
-        const size_t AB = align_up((size_t)chunk * H * 2, 256), PhB = align_up((size_t)H * m_max * 2, 256);
-        const size_t GB = align_up((size_t)H * dd_max * 4, 256);
-        const size_t WB = align_up((size_t)dd_max * (kw_max + H) * 2, 256);
-        PS_TRY(ensure_buf(ctx, &ctx->hub_buf, &ctx->hub_bytes,
-                          2 * nB + candB + idsB + 256 + tabB + AB + PhB + GB + WB, "hub-split pool storage"));
-        char *hb = static_cast<char *>(ctx->hub_buf);
-        int32_t *counts = reinterpret_cast<int32_t *>(hb), *rank = reinterpret_cast<int32_t *>(hb + nB);
-        void *cand = hb + 2 * nB;
-        int32_t *hub_ids = reinterpret_cast<int32_t *>(hb + 2 * nB + candB);
-        long long *info = reinterpret_cast<long long *>(hb + 2 * nB + candB + idsB);
-        int32_t *idxm = reinterpret_cast<int32_t *>(hb + 2 * nB + candB + idsB + 256);
-        int64_t sampled = 0;
-        cudaError_t e = launch_hub_select(d_idx, N, T, N, H, counts, rank, cand, hub_ids, info, &sampled,
-                                          ctx->stream, &ctx->launches);
-        count_launches(ctx);
-        PS_CUDA(ctx, e);
-        bool use = true;
-        if (ctx->pool_hubs < 0) {              // automatic: worth it when the hubs hold a third of the entries
-            long long info_h[2] = {0, 0};
-            PS_CUDA(ctx, cudaMemcpyAsync(info_h, info, 16, cudaMemcpyDeviceToHost, ctx->stream));
-            PS_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
-            use = info_h[0] > 0 && 3 * info_h[1] >= sampled;
+        PS_TRY(hub_select_begin(ctx, dt, N, T, K, layers, sample, sample_n, hp));
+    }
+    // (hub_select_finish follows S1 of the first layer, which hides the selection's read-back)
+    auto hub_finish = [&]() -> pinsage_status {
+        PS_TRY(hub_select_finish(ctx, N, T, K, layers, chunk, !h_idx, hp, &hubs_on));
+        if (hubs_on && !h_idx) PS_TRY(hub_remap_whole(ctx, hp, nbr_idx, N, T));
+        else if (hubs_on) hub_activate(ctx, hp, nullptr, nullptr, hp.hub_ids);
+        return PINSAGE_OK;
+    };
+
+    // ---- per-chunk plumbing of the layers -------------------------------------------------------------
+    const char *Hlast = nullptr;               // the last layer's output buffer (set when the loop reaches it)
+    void *d_out = h_out ? nullptr : out;
+    int layer = 0;                             // 0-based layer the lambdas below act for
+    std::vector<char> remapped((size_t)nchunks, 0), validated((size_t)nchunks, 0);
+    ChunkIO io;
+    if (h_feats) {
+        io.s1_in = [&](int64_t c, const void **src) { return sF.acquire(ctx, c, ctx->stream, src); };
+        io.s1_done = [&](int64_t c) { return sF.release(ctx, c, ctx->stream); };
+    }
+    io.tables_in = [&](int64_t c, cudaStream_t ps, const int32_t **ic, const float **wc) -> pinsage_status {
+        const int64_t r0 = c * chunk, rows = std::min(chunk, N - r0);
+        const void *p = nullptr;
+        if (h_idx) {
+            PS_TRY(sI.acquire(ctx, c, ps, &p));
+            *ic = static_cast<const int32_t *>(p);
         }
-        if (use) {
-            e = launch_hub_remap(d_idx, rank, N * (int64_t)T, idxm, ctx->stream, &ctx->launches);
+        if (h_w) {
+            PS_TRY(sW.acquire(ctx, c, ps, &p));
+            *wc = static_cast<const float *>(p);
+        }
+        if (ctx->check_indices && (h_idx || h_w) && !validated[(size_t)c]) {
+            if (ps != ctx->stream) {           // (the validation kernel runs on the context's main stream)
+                if (h_idx) PS_TRY(sI.acquire(ctx, c, ctx->stream, &p));
+                if (h_w) PS_TRY(sW.acquire(ctx, c, ctx->stream, &p));
+            }
+            int64_t bad = -1;                  // (synchronous; ids are still the caller's here)
+            pinsage_status st = pinsage_validate_graph(ctx, rows, N, T, *ic, *wc, &bad);
+            if (st != PINSAGE_OK) return st;
+            validated[(size_t)c] = 1;
+        }
+        if (io.hub_remapped && !(sI.whole && remapped[(size_t)c])) {
+            // in place in the staging slot (once when the table is staged whole, every pass through a ring)
+            int32_t *slot = const_cast<int32_t *>(*ic);
+            cudaError_t e = launch_hub_remap(slot, hp.rank, rows * (int64_t)T, slot, ps, &ctx->launches);
             count_launches(ctx);
             PS_CUDA(ctx, e);
-            ctx->hub.H = H;
-            ctx->hub.src_idx = d_idx;
-            ctx->hub.idxm = idxm;
-            ctx->hub.hub_ids = hub_ids;
-            char *after = reinterpret_cast<char *>(idxm) + tabB;
-            ctx->hub.A = after;
-            ctx->hub.Ph = after + AB;
-            ctx->hub.G = reinterpret_cast<float *>(after + AB + PhB);
-            ctx->hub.Wext = after + AB + PhB + GB;
+            remapped[(size_t)c] = 1;
         }
+        return PINSAGE_OK;
+    };
+    io.tables_done = [&](int64_t c, cudaStream_t ps) -> pinsage_status {
+        if (h_idx) PS_TRY(sI.release(ctx, c, ps));
+        if (h_w) PS_TRY(sW.release(ctx, c, ps));
+        return PINSAGE_OK;
+    };
+    if (!h_idx && !h_w) {
+        io.tables_in = nullptr;
+        io.tables_done = nullptr;
     }
-
-    const void *Hin = d_feats;
-    char *Hcur = nullptr;
-    // ---- head of rows [r0, r0 + rows) (the intermediate a never exists in full) -------------------
-    const char *Hlast = nullptr;              // the last layer's output buffer (set when the loop reaches it)
-    ChunkHook head_chunk = [&](int64_t r0, int64_t rows) -> pinsage_status {
+    io.self_in = [&](int64_t c, const void **self) -> pinsage_status {
+        if (layer == 0 && h_feats) return sF.acquire(ctx, c, ctx->stream, self);
+        return PINSAGE_OK;
+    };
+    // after S3 of chunk c: (layer 1, streamed features) the slot is free; (last layer) the head of the
+    // chunk -- the intermediate a never exists in full, and a host `out` streams home during the layer
+    io.after_chunk = [&](int64_t c, int64_t r0, int64_t rows) -> pinsage_status {
+        if (layer == 0 && h_feats) PS_TRY(sF.release(ctx, c, ctx->stream));
+        if (layer != K - 1) return PINSAGE_OK;
+        StepRange r45("S4+S5 head rows %lld+%lld", (long long)r0, (long long)rows);
         GemmArgs g;
         g.M = rows; g.K1 = head->d; g.N = head->g1;
         g.A1 = Hlast + (size_t)r0 * head->d * es;
         g.B = head->G1; g.bias = head->g; g.relu = 1; g.out = abuf;
-        StepRange r45("S4+S5 head rows %lld+%lld", (long long)r0, (long long)rows);
         PS_TRY(run_gemm(ctx, dt, g, nullptr, 0, ctx->stream, PROF_HEAD1));
+        if (h_out) PS_TRY(sO.acquire(ctx, c, ctx->stream));
         GemmArgs g2;
         g2.M = rows; g2.K1 = head->g1; g2.N = head->d_out; g2.A1 = abuf; g2.B = head->G2;
-        g2.out = static_cast<char *>(d_out) + (size_t)r0 * head->d_out * es;
+        g2.out = h_out ? sO.ptr(c) : static_cast<char *>(d_out) + (size_t)r0 * head->d_out * es;
         PS_TRY(run_gemm(ctx, dt, g2, nullptr, 0, ctx->stream, PROF_HEAD2));
-        if (out_ready) {                      // this chunk of out goes home while the next one is computed
-            const int64_t c = r0 / chunk;
-            const size_t rb = (size_t)head->d_out * es;
-            PS_CUDA(ctx, cudaEventRecord(out_ready[c], ctx->stream));
-            PS_CUDA(ctx, cudaStreamWaitEvent(ctx->d2h, out_ready[c], 0));
-            PS_CUDA(ctx, cudaMemcpyAsync(static_cast<char *>(out) + r0 * rb, static_cast<char *>(d_out) + r0 * rb,
-                                         rows * rb, cudaMemcpyDeviceToHost, ctx->d2h));
-        }
+        if (ctx->poison) PS_CUDA(ctx, cudaMemsetAsync(abuf, 0xFF, (size_t)rows * head->g1 * es, ctx->stream));
+        if (h_out) PS_TRY(sO.release(ctx, c, r0, rows, ctx->stream));
         return PINSAGE_OK;
     };
+
+    const void *Hin = h_feats ? nullptr : feats;
+    char *Hcur = nullptr;
     for (int k = 0; k < K; ++k) {
         const pinsage_layer_params *lp = &layers[k];
         const LayerWs plan = plan_layer_ws(ctx, dt, N, lp, chunk);
         ctx->cur_layer = k + 1;
+        layer = k;
         char *Hout;
         if (k == 0) Hout = Ha;
         else if (lp->d == lp->d_in) Hout = Hcur;           // in place (S1 has consumed all of H first)
         else Hout = (Hcur == Ha) ? Hb : Ha;
         if (k == K - 1) Hlast = Hout;
-        // host output: the head of a chunk follows its last S3 directly, so that finished chunks of
-        // `out` travel home while the rest of the last layer is still being computed
-        PS_TRY(layer_on_ws(ctx, dt, N, T, Hin, d_idx, d_w, lp, Hout, ws, plan, chunk,
-                           k == 0 ? feats_landed : nullptr, k == 0 ? tables_landed : nullptr, -1, nullptr,
-                           (k == K - 1 && out_ready) ? head_chunk : ChunkHook()));
+        // aliasing rules, as assertions: a layer runs in place only at equal widths;
+        // `out` doubles as H only when every row of H has out's stride; two H buffers otherwise
+        if ((Hout == Hcur && lp->d != lp->d_in) || (pl.H_is_out && lp->d != head->d_out) ||
+            (Hout != Hcur && k > 0 && !Hb))
+            return fail(ctx, PINSAGE_ERR_CUDA, "internal: buffer aliasing rule violated in layer %d", k + 1);
+        ChunkIO lio = io;
+        if (k > 0 || !h_feats) {
+            lio.s1_in = nullptr;
+            lio.s1_done = nullptr;
+        }
+        if (k == 0) PS_TRY(sF.begin_pass(ctx));                     // pass 1: S1 behind the feature chunks
+        PS_TRY(project_chunks(ctx, dt, N, lp, Hin, ws, plan, chunk, lio));
+        if (k == 0) {
+            PS_TRY(hub_finish());
+            io.hub_remapped = lio.hub_remapped = hubs_on && h_idx;
+        }
+        if (k == 0 && !sF.whole) PS_TRY(sF.begin_pass(ctx));        // streamed features, pass 2: the self rows of S3
+        PS_TRY(sI.begin_pass(ctx));                                 // (no-ops for device arrays and for
+        PS_TRY(sW.begin_pass(ctx));                                 //  tables already staged whole)
+        PS_TRY(pool_combine_chunks(ctx, dt, N, T, lp, Hin, ws + plan.P_off, nbr_idx, nbr_w, Hout, chunk,
+                                   ws + plan.n0_off, ws + plan.n1_off, ws + plan.scratch_off, plan.scratch_bytes,
+                                   N, lio));
+        if (ctx->poison && Hcur && Hout != Hcur)   // the previous H is dead once S1 and every S3 of this layer ran
+            PS_CUDA(ctx, cudaMemsetAsync(Hcur, 0xFF, (size_t)N * lp->d_in * es, ctx->stream));
         Hcur = Hout;
         Hin = Hout;
     }
-    if (!out_ready)
-        for (int64_t r0 = 0; r0 < N; r0 += chunk) PS_TRY(head_chunk(r0, std::min(chunk, N - r0)));
     if (any_host) {
         PS_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
         PS_CUDA(ctx, cudaStreamSynchronize(ctx->h2d));
@@ -1382,6 +1801,14 @@ pinsage_status pinsage_embed_nodes(pinsage_ctx *ctx, pinsage_dtype dtype, int64_
         chunk[k] = auto_chunk(n[k], 0, (size_t)std::max(lp->m, lp->d) * es);
         wsmax = std::max(wsmax, plan_layer_ws(ctx, dt, n[k - 1], lp, chunk[k]).total);
     }
+    // the hub-split pool, if the whole graph would take it: same hubs, same split, same bits as the rows
+    // of pinsage_embed_all
+    HubReset hub_reset{ctx};
+    HubPlan hp;
+    bool use_hubs = false;
+    PS_TRY(hub_select_begin(ctx, dt, N, T, K, layers, nbr_idx, N, hp));
+    PS_TRY(hub_select_finish(ctx, N, T, K, layers, *std::max_element(chunk.begin() + 1, chunk.end()), false, hp,
+                             &use_hubs));
     const size_t aB = align_up((size_t)n[K] * head->g1 * es, 256), oB = align_up((size_t)n[K] * head->d_out * es, 256);
     Hmax = align_up(Hmax, 256); selfmax = align_up(selfmax, 256); tabmax = align_up(tabmax, 256);
     wsmax = align_up(wsmax, 256);
@@ -1405,11 +1832,19 @@ pinsage_status pinsage_embed_nodes(pinsage_ctx *ctx, pinsage_dtype dtype, int64_
                                          &ctx->launches));
         PS_CUDA(ctx, subset_gather_rows(Hbuf[cur], list(k), pos(k - 1), n[k], (size_t)lp->d_in * es, Hself, st,
                                         &ctx->launches));
+        ctx->hub.H = 0;
+        if (use_hubs && !use_linear_pool(ctx, lp)) {
+            // entries that name a hub of the whole graph become -(rank + 1); the hubs' rows of the compact
+            // P are found through the previous set's positions
+            PS_CUDA(ctx, launch_hub_remap_sub(list(k), n[k], nbr_idx, T, hp.rank, idx_loc, st, &ctx->launches));
+            PS_CUDA(ctx, launch_hub_localize(hp.hub_ids, hp.H, mark(k - 1), pos(k - 1), hp.hub_loc, st, &ctx->launches));
+            hub_activate(ctx, hp, idx_loc, idx_loc, hp.hub_loc);
+        }
         count_launches(ctx);
         const LayerWs plan = plan_layer_ws(ctx, dt, n[k - 1], lp, chunk[k]);
         ctx->cur_layer = k;
         PS_TRY(layer_on_ws(ctx, dt, n[k], T, Hself, idx_loc, w_loc, lp, Hbuf[cur ^ 1], lws, plan, chunk[k],
-                           nullptr, nullptr, n[k - 1], Hbuf[cur]));
+                           n[k - 1], Hbuf[cur]));
         cur ^= 1;
     }
     // head on S^(K) (l.15-17), then one row per requested target, in the caller's order

@@ -47,21 +47,26 @@ __device__ __forceinline__ unsigned row_id(unsigned key, int t, unsigned n_src)
     return __umulhi(x, n_src);
 }
 
-// m1: every thread streams 16-byte words, 8 loads in flight, grid-stride; one word per thread is written.
+// m1: every warp streams contiguous 4 KB blocks (8 x 512-byte warp loads in flight per lane), block after
+// block in grid order, so that the front the grid reads at any time is one contiguous range of memory;
+// one word per thread is written at the end.
 __global__ void __launch_bounds__(256, 8)
 calib_stream_kernel(const uint4 *__restrict__ buf, long long words, uint4 *__restrict__ sink)
 {
     uint4 acc = make_uint4(0, 0, 0, 0);
-    const long long stride = (long long)gridDim.x * blockDim.x;
-    long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
-    for (; i + 7 * stride < words; i += 8 * stride) {
+    const int lane = threadIdx.x & 31;
+    const long long warps = (long long)gridDim.x * (blockDim.x >> 5);
+    const long long gwarp = (long long)blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5);
+    const long long blocks = words / 256;                  // whole 4 KB blocks (256 words)
+    for (long long b = gwarp; b < blocks; b += warps) {
+        const uint4 *p = buf + b * 256 + lane;
         uint4 r[8];
 #pragma unroll
-        for (int u = 0; u < 8; ++u) r[u] = ldg16_stream(buf + i + u * stride);
+        for (int u = 0; u < 8; ++u) r[u] = ldg16_stream(p + u * 32);
 #pragma unroll
         for (int u = 0; u < 8; ++u) xor16(acc, r[u]);
     }
-    for (; i < words; i += stride) xor16(acc, ldg16_stream(buf + i));
+    for (long long i = blocks * 256 + gwarp * 32 + lane; i < words; i += warps * 32) xor16(acc, ldg16_stream(buf + i));
     sink[(long long)blockIdx.x * blockDim.x + threadIdx.x] = acc;
 }
 

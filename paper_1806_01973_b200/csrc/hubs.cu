@@ -111,8 +111,37 @@ hub_remap_kernel(const int *__restrict__ idx, const int *__restrict__ rank, long
     }
 }
 
-// A [rows x H] bf16, A[u, h] = sum of the weights of u's entries that point at
-// hub h (mean aggregator: 1/T each).  One warp per node, the row is summed in shared memory.
+// Targeted inference (pinsage_embed_nodes): the sub-table idx_loc [n x T] of the members list[0..n) holds
+// positions inside the previous set; entries whose WHOLE-GRAPH id is a hub become -(rank + 1) instead, as
+// in the remapped whole-graph table, so that the closure runs the same split as the whole graph.
+__global__ void __launch_bounds__(256)
+hub_remap_sub_kernel(const int *__restrict__ list, long long n, const int *__restrict__ idx, int T,
+                     const int *__restrict__ rank, int *__restrict__ idx_loc)
+{
+    const long long total = n * T;
+    for (long long e = (long long)blockIdx.x * blockDim.x + threadIdx.x; e < total;
+         e += (long long)gridDim.x * blockDim.x) {
+        const long long i = e / T;
+        const int t = (int)(e - i * T);
+        const int r = rank[idx[(long long)list[i] * T + t]];
+        if (r >= 0) idx_loc[e] = -(r + 1);
+    }
+}
+
+// hub_loc[h] = position of hub h inside the previous set (its row of the compact P), or -1 when no member
+// lists it (its column of A is then zero, and so is the row of P_hub that stands for it)
+__global__ void hub_localize_kernel(const int *__restrict__ hub_ids, int H, const unsigned char *__restrict__ mark,
+                                    const int *__restrict__ pos, int *__restrict__ hub_loc)
+{
+    const int h = blockIdx.x * blockDim.x + threadIdx.x;
+    if (h >= H) return;
+    const int id = hub_ids[h];
+    hub_loc[h] = (id >= 0 && mark[id]) ? pos[id] : -1;
+}
+
+// A [rows x H] bf16, A[u, h] = sum of the weights of u's entries that point at hub h (mean aggregator:
+// 1/T each), summed in table order without atomics (the same scheme as pool.cu's hub_accumulate, so the
+// stand-alone kernel and the gather kernel's fused form give the same bits).  One warp per node.
 __global__ void __launch_bounds__(256)
 hub_matrix_kernel(const int *__restrict__ idxm, const float *__restrict__ w, long long rows, int T, int H, int mean,
                   __nv_bfloat16 *__restrict__ A)
@@ -125,11 +154,23 @@ hub_matrix_kernel(const int *__restrict__ idxm, const float *__restrict__ w, lon
     for (int h = lane; h < H; h += 32) buf[h] = 0.f;
     __syncwarp();
     const float wmean = 1.0f / (float)T;
-    for (int t = lane; t < T; t += 32) {
-        const int i = idxm[v * T + t];
-        if (i < 0) atomicAdd(buf - (i + 1), mean ? wmean : w[v * T + t]);   // (a list may name a hub twice)
+    for (int tb = 0; tb < T; tb += 32) {
+        const int t = tb + lane;
+        const int i = t < T ? idxm[v * T + t] : 0;
+        const bool is_hub = t < T && i < 0;
+        const float wt = is_hub ? (mean ? wmean : w[v * T + t]) : 0.f;
+        const unsigned hm = __ballot_sync(0xffffffffu, is_hub);
+        if (hm == 0) continue;
+        if (is_hub) {
+            const int r = -(i + 1);
+            const unsigned peers = __match_any_sync(hm, r);
+            const int leader = __ffs(peers) - 1;
+            float sum = lane == leader ? buf[r] : 0.f;
+            for (unsigned rem = peers; rem; rem &= rem - 1) sum += __shfl_sync(peers, wt, __ffs(rem) - 1);
+            if (lane == leader) buf[r] = sum;
+        }
+        __syncwarp();
     }
-    __syncwarp();
     __nv_bfloat16 *row = A + v * H;
     for (int h = lane; h < H; h += 32) row[h] = __float2bfloat16_rn(buf[h]);
 }
@@ -205,6 +246,23 @@ cudaError_t launch_hub_remap(const int32_t *idx, const int32_t *rank, int64_t to
                              cudaStream_t s, int *launches)
 {
     hub_remap_kernel<<<grid_for(total), 256, 0, s>>>(idx, rank, total, out);
+    if (launches) ++*launches;
+    return cudaGetLastError();
+}
+
+cudaError_t launch_hub_remap_sub(const int32_t *list, int64_t n, const int32_t *idx, int32_t T, const int32_t *rank,
+                                 int32_t *idx_loc, cudaStream_t s, int *launches)
+{
+    if (n <= 0) return cudaSuccess;
+    hub_remap_sub_kernel<<<grid_for(n * (long long)T), 256, 0, s>>>(list, n, idx, T, rank, idx_loc);
+    if (launches) ++*launches;
+    return cudaGetLastError();
+}
+
+cudaError_t launch_hub_localize(const int32_t *hub_ids, int32_t H, const unsigned char *mark, const int32_t *pos,
+                                int32_t *hub_loc, cudaStream_t s, int *launches)
+{
+    hub_localize_kernel<<<(H + 255) / 256, 256, 0, s>>>(hub_ids, H, mark, pos, hub_loc);
     if (launches) ++*launches;
     return cudaGetLastError();
 }

@@ -104,6 +104,10 @@ cudaError_t launch_hub_select(const int32_t *idx, int64_t N, int32_t T, int64_t 
 size_t hub_cand_bytes();
 cudaError_t launch_hub_remap(const int32_t *idx, const int32_t *rank, int64_t total, int32_t *out,
                              cudaStream_t s, int *launches);
+cudaError_t launch_hub_remap_sub(const int32_t *list, int64_t n, const int32_t *idx, int32_t T, const int32_t *rank,
+                                 int32_t *idx_loc, cudaStream_t s, int *launches);
+cudaError_t launch_hub_localize(const int32_t *hub_ids, int32_t H, const unsigned char *mark, const int32_t *pos,
+                                int32_t *hub_loc, cudaStream_t s, int *launches);
 cudaError_t launch_hub_matrix(const int32_t *idxm, const float *w, int64_t rows, int32_t T, int32_t H,
                               int mean, void *A, cudaStream_t s, int *launches);
 cudaError_t launch_hub_gather(const void *P, const int32_t *hub_ids, int32_t H, int32_t pw, void *Ph,

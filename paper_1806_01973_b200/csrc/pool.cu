@@ -127,6 +127,33 @@ struct Chunk<false> {  // 4 fp32 per 16 bytes
     }
 };
 
+// A[v, r] += w for the lanes of one 32-entry batch whose entry names hub r (idx = -(r + 1)), in TABLE
+// ORDER and without atomics: the lanes that name the same hub find each other with a match, the lowest
+// one adds their weights lane by lane to the running sum in shared memory.  Batches follow each other
+// in table order, so A[v, r] is the sum a sequential loop over t = 0..T-1 would form, bit for bit
+// (a list may legally name a hub several times: reading A7).  Called by all 32 lanes of the warp.
+__device__ __forceinline__ void hub_accumulate(float *hbuf, bool is_hub, int my_i, float my_w, int lane)
+{
+    const unsigned hm = __ballot_sync(0xffffffffu, is_hub);
+    if (hm == 0) return;                                   // (warp-uniform)
+    if (is_hub) {
+        const int r = -(my_i + 1);
+        const unsigned peers = __match_any_sync(hm, r);
+        const int leader = __ffs(peers) - 1;
+        if (peers == (1u << lane)) {                       // the usual case: named once in this batch
+            hbuf[r] += my_w;
+        } else {
+            float sum = lane == leader ? hbuf[r] : 0.f;
+            for (unsigned rem = peers; rem; rem &= rem - 1) {
+                const float wv = __shfl_sync(peers, my_w, __ffs(rem) - 1);
+                sum += wv;                                 // (only the leader's sum is used)
+            }
+            if (lane == leader) hbuf[r] = sum;
+        }
+    }
+    __syncwarp();                                          // the next batch may update the same sums from other lanes
+}
+
 // UU neighbour rows (slots j0 .. j0+UU-1 of the current batch) for one lane: every one of the
 // UU*CPL 16-byte loads is issued before the first FMA (memory-level parallelism).
 // MODE: 0 importance pooling (weighted sum), 1 element-wise mean (my_w holds 1/T in every lane),
@@ -206,8 +233,8 @@ pool_kernel(const uint4 *__restrict__ P, const int *__restrict__ idx, const floa
             if (MODE == 0) my_w = ld_stream_f32(wrow + t);
         }
         int cnt = min(LPN, T - tb);
-        if (hubA != nullptr && t < T && my_i < 0)          // hub entry -(rank + 1): its weight goes to A[v, rank]
-            atomicAdd(hbuf - (my_i + 1), my_w);
+        if (hubA != nullptr)                               // hub entry -(rank + 1): its weight goes to A[v, rank]
+            hub_accumulate(hbuf, t < T && my_i < 0, my_i, my_w, lane);
         if (skip_neg) {
             // entries with a negative id (hub neighbours, summed by the hub GEMM: hubs.cu) are squeezed
             // out of this batch: lane k of a node's group takes the k-th remaining entry.  Groups of

@@ -1,6 +1,6 @@
 """Parity of the hub-split pool (option ``pool_hubs``; hubs.cu): on a power-law graph the entries of the
 neighbour lists that point at the few hundred most listed nodes are not gathered; their term enters S3 as
-a third K segment on the tensor cores.  Same function as Algorithm 1 lines 1-2 (PAPER.md:101-106) in real arithmetic;
+a third K segment on the tensor cores.  Same function as Algorithm 1 lines 1-2 (PAPER.md:114-115) in real arithmetic;
 checked against the fp64 oracle on sampled destinations (Algorithm 2 on their K-hop closure) and against
 the plain pool on every row."""
 import numpy as np
@@ -17,7 +17,10 @@ DEV = "cuda:0"
 
 @pytest.fixture(scope="module")
 def ctx():
+    """The split is automatic by default (pool_hubs = -1); these tests start from "off" and switch it on
+    explicitly, so that each has the plain pool to compare with."""
     c = binding.Context(0)
+    c.pinsage_set_option("pool_hubs", 0)
     yield c
     c.close()
 
@@ -128,3 +131,45 @@ def test_hub_split_pool_odd_shapes(ctx, d0, hidden, T, hubs, chunk):
     rel, cos = row_errors(to_f64(out), to_f64(plain))
     assert rel.max() <= 1e-2 and cos.min() >= 0.999, (rel.max(), cos.min())
     assert not torch.equal(out.view(torch.int16), plain.view(torch.int16)), "the hub path did not run"
+
+
+def test_default_context_takes_the_split_and_all_paths_agree_bit_for_bit():
+    """A fresh context (pool_hubs = -1, the default) on the power-law graph: the split is taken, the result is
+    the same run to run (no atomics: the hub weights are summed in table order), and the one-call path, the
+    layer-by-layer path and targeted inference (pinsage_embed_nodes, which picks the hubs from the whole
+    graph's table and remaps only its sub-tables) agree bit for bit -- with lists that name a hub several
+    times (reading A7) and with the hub weights summed across 32-entry batches (T = 50)."""
+    cfg = synth.CONFIGS["cfg4"].scaled(140_000)
+    X, layers, head, idx, counts = _setup(cfg)
+    idx[7, 5] = idx[7, 0]            # node 7 names its first (hub) neighbour three times, across two batches
+    idx[7, 40] = idx[7, 0]
+    idx[9, :] = idx[9, 0]            # node 9 names one hub 50 times
+    with binding.Context(0) as c:
+        alpha = c.pinsage_normalize_counts(counts)
+        l0 = c.pinsage_launch_count()
+        a = c.pinsage_embed_all(X, idx, alpha, layers, head, chunk_nodes=40_000)
+        n_split = c.pinsage_launch_count() - l0
+        b = c.pinsage_embed_all(X, idx, alpha, layers, head)            # automatic chunk
+        torch.cuda.synchronize()
+        assert torch.equal(a.view(torch.int16), b.view(torch.int16))
+        for _ in range(3):
+            again = c.pinsage_embed_all(X, idx, alpha, layers, head, chunk_nodes=40_000)
+            assert torch.equal(a.view(torch.int16), again.view(torch.int16)), "not bit-reproducible"
+        H = X
+        for lp in layers:
+            H = c.pinsage_layer(H, idx, alpha, lp)
+        by_layer = c.pinsage_head(H, head)
+        assert torch.equal(a.view(torch.int16), by_layer.view(torch.int16)), "layer-by-layer path differs"
+        rows = np.concatenate([[0, 7, 9, 127, 128, cfg.N - 1], np.random.default_rng(11).integers(0, cfg.N, 200)])
+        t = torch.from_numpy(rows).to(DEV).to(torch.int32)
+        sub = c.pinsage_embed_nodes(X, idx, alpha, layers, head, t)
+        torch.cuda.synchronize()
+        assert torch.equal(sub.view(torch.int16), a[t.long()].view(torch.int16)), "targeted rows differ"
+        ref = _oracle_rows(X, idx, alpha, layers, head, rows[:70])
+        assert_rows_close(to_f64(a[t.long()[:70]]), ref, torch.bfloat16, "default (hub-split) path vs oracle")
+        c.pinsage_set_option("pool_hubs", 0)
+        l0 = c.pinsage_launch_count()
+        plain = c.pinsage_embed_all(X, idx, alpha, layers, head, chunk_nodes=40_000)
+        n_plain = c.pinsage_launch_count() - l0
+        assert n_split > n_plain + 4, "the default context did not take the hub-split pool"
+        assert not torch.equal(plain.view(torch.int16), a.view(torch.int16))

@@ -211,17 +211,17 @@ def test_full_cfg2_sampled_and_layerwise(ctx):
 
 def test_full_cfg3_paper_shaped(ctx):
     _need_memory(75)
-    _full_size(ctx, "cfg3", n_e2e=24, e2e_batch=64, n_layer=1024)
+    _full_size(ctx, "cfg3", n_e2e=256, e2e_batch=64, n_layer=4096)
 
 
 def test_full_cfg4_power_law(ctx):
     _need_memory(110)
-    _full_size(ctx, "cfg4", n_e2e=128, e2e_batch=128, n_layer=4096)
+    _full_size(ctx, "cfg4", n_e2e=1024, e2e_batch=256, n_layer=4096)
 
 
 def test_full_cfg5_deep_wide(ctx):
     _need_memory(150)
-    _full_size(ctx, "cfg5", n_e2e=2, e2e_batch=2, n_layer=2048, few=True)
+    _full_size(ctx, "cfg5", n_e2e=2, e2e_batch=2, n_layer=4096, few=True)
 
 
 def test_full_paper_geometry_linear_pool(ctx):

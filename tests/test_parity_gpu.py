@@ -289,6 +289,8 @@ def _to_dev(layers, head):
 
 
 def _check_whole_path(ctx, cfg, impl=0, chunk_nodes=0, cg=0):
+    """chunk_nodes may be a tuple: the one-call path is then run once per value against the same oracle
+    pass (0 = the automatic driver chunk, the launch configuration bench.py times)."""
     X, idx, counts, alpha, layers, head = _inputs(cfg)
     Lf, Hf = params_f64(layers, head)
     ref_out, ref_hidden = O.embed_all(to_f64(X), idx.numpy(), alpha, Lf, Hf, return_hidden=True)
@@ -307,8 +309,16 @@ def _check_whole_path(ctx, cfg, impl=0, chunk_nodes=0, cg=0):
         out_head = ctx.pinsage_head(H, Hd)
         assert_rows_close(to_f64(out_head), ref_out, dtype, f"{cfg.name} head impl={impl}")
         # and in one call
-        out = ctx.pinsage_embed_all(X.to(DEV), idx.to(DEV), w_dev, Ld, Hd, chunk_nodes=chunk_nodes)
-        stats = assert_rows_close(to_f64(out), ref_out, dtype, f"{cfg.name} embed_all impl={impl}")
+        chunks = chunk_nodes if isinstance(chunk_nodes, (tuple, list)) else (chunk_nodes,)
+        first = None
+        for cn in chunks:
+            out = ctx.pinsage_embed_all(X.to(DEV), idx.to(DEV), w_dev, Ld, Hd, chunk_nodes=cn)
+            stats = assert_rows_close(to_f64(out), ref_out, dtype, f"{cfg.name} embed_all impl={impl} chunk={cn}")
+            bits = torch.int16 if dtype == torch.bfloat16 else torch.int32
+            if first is None:
+                first = out
+            else:        # a row's arithmetic does not depend on the chunk it sits in
+                assert torch.equal(first.view(bits), out.view(bits)), f"chunk_nodes={cn} changes the result"
         return out, stats
     finally:
         ctx.pinsage_set_option("gemm_impl", 0)
@@ -327,17 +337,17 @@ def test_cfg2_small_exhaustive(ctx, impl, cg):
     _check_whole_path(ctx, synth.CONFIGS["cfg2"].scaled(20_011), impl=impl, chunk_nodes=4096, cg=cg)
 
 
-@pytest.mark.parametrize("name,N", [("cfg3", 3000), ("cfg4", 6000), ("cfg5", 5000)])
-def test_small_siblings_exhaustive(ctx, name, N):
-    """The "-small" siblings of configs 3-5 (same dims, T, K and value laws), every row."""
+@pytest.mark.parametrize("name,N,small_chunk", [("cfg3", 50_000, 6144), ("cfg4", 100_000, 12_800),
+                                                ("cfg5", 20_000, 2048)])
+def test_small_siblings_exhaustive(ctx, name, N, small_chunk):
+    """The "-small" siblings of configs 3-5 (same dims, T, K and value laws) at the sizes SURVEY.md 8(d)
+    fixes, EVERY row against the oracle, with the automatic driver chunk and with a small one.  At these
+    sizes the persistent GEMMs walk several tiles per CTA (pair): config 3's S3 (d = 1024, four 256-column
+    slabs, 36 lanes of CTA pairs) runs 196 row tiles = 5-6 per lane with the automatic chunk, so both
+    parities of the grid-wide norm exchange and its arrival-count targets for it >= 2 are compared with
+    the oracle on every row; the small chunk adds ragged last tiles and chunk edges off the tile grid."""
     cfg = synth.CONFIGS[name].scaled(N)
-    try:
-        _check_whole_path(ctx, cfg, impl=0, chunk_nodes=2048)
-    except binding.PinsageError as e:
-        if e.status_name != "UNSUPPORTED_SHAPE":
-            raise
-        _check_whole_path(ctx, cfg, impl=1, chunk_nodes=2048)
-        pytest.xfail(f"tcgen05 path does not cover {name} yet (SIMT reference path is green): {e}")
+    _check_whole_path(ctx, cfg, impl=0, chunk_nodes=(0, small_chunk))
 
 
 def test_embed_all_deterministic_and_overlap_invariant(ctx):
@@ -442,16 +452,17 @@ def test_argument_errors(ctx):
 # ------------------------------------------------------------------ random shapes (property test)
 def _random_case(rng, narrow_ok):
     """A random small instance: dims multiples of 8 with m != d != d_in, odd T, K in 1..3, ragged N.
-    narrow_ok=False keeps every normalised width >= 128 and output width >= 32: with 8-wide rows ReLU regularly
-    leaves a nearly dead row whose direction is ill-conditioned (a 1e-3 input rounding becomes a 3 %
-    change of z / ||z||), which measures the generator, not the kernels -- those widths are
-    exercised in fp32 mode, where they pass at 1e-4 ("degenerate rows")."""
+    narrow_ok=False keeps every normalised width >= 128 (the narrowest bf16 width of BASELINE.json's
+    configs is 256; fp32's is 64) and the output width >= 32: with 8-wide rows ReLU regularly leaves a
+    nearly dead row whose direction is ill-conditioned (a 1e-3 input rounding becomes a 3 % change of
+    z / ||z||), which measures the generator, not the kernels -- those widths are exercised in fp32 mode,
+    where they pass at 1e-4, and reported (not gated) in bf16 by test_narrow_bf16_rows_report_only."""
     K = int(rng.integers(1, 4))
-    wide = [128, 200, 256, 320]      # (at 64-72 columns the worst bf16 row sits at 0.96e-2, on the gate)
+    wide = [128, 200, 256, 320]
     any_w = [8, 24, 40, 64, 72] + wide
     dims = [int(rng.choice(any_w))] + [int(rng.choice(any_w if narrow_ok else wide)) for _ in range(K)]
-    ms = [int(rng.choice([8, 16, 48, 64, 136, 256, 512])) for _ in range(K)]
-    g1 = int(rng.choice([8, 32, 64, 128, 264] if narrow_ok else [64, 128, 264]))
+    ms = [int(rng.choice([8, 16, 48, 64, 136, 256, 512] if narrow_ok else [136, 256, 512])) for _ in range(K)]
+    g1 = int(rng.choice([8, 32, 64, 128, 264] if narrow_ok else [128, 264]))
     d_out = int(rng.choice([8, 16, 32, 128, 520] if narrow_ok else [32, 128, 520]))
     N = int(rng.integers(60, 3000))
     T = int(rng.choice([1, 2, 3, 7, 10, 33, 50]))
@@ -484,12 +495,48 @@ def test_random_shapes_whole_path(ctx, dtype, seed):
     Ld, Hd = _to_dev(layers, head)
     out = ctx.pinsage_embed_all(X.to(DEV), idx.to(DEV), torch.from_numpy(alpha).to(DEV), Ld, Hd,
                                 chunk_nodes=int(rng.choice([0, 128, 1024])))
-    # north_star's 1e-2 is stated for K = 2 chains of 8 bf16 roundings (P, n, H per layer; a, out).
-    # Deeper / linear-pool chains round more often: the per-row error grows like sqrt(#roundings).
-    R = 3 * len(ms) + 2 + sum(m > d for m, d in zip(ms, dims[1:]))
-    tol = None if dtype == torch.float32 else 1e-2 * max(1.0, (R / 8) ** 0.5)
-    assert_rows_close(to_f64(out), ref, dtype,
-                      f"random case {seed}: N={N} T={T} dims={dims} ms={ms}", tol=tol)
+    # north_star's tolerance as it stands (1e-2 bf16, 1e-4 fp32), for every K and either schedule
+    assert_rows_close(to_f64(out), ref, dtype, f"random case {seed}: N={N} T={T} dims={dims} ms={ms}")
+
+
+@pytest.mark.parametrize("seed", range(6))
+def test_narrow_bf16_rows_report_only(ctx, seed):
+    """NOT a gate of north_star's tolerance: bf16 with normalised widths below BASELINE.json's minimum
+    (8 .. 72 columns).  DESIGN.md sec. 9: with so few columns a row's error is an average over few
+    roundings and a nearly dead ReLU row is ill-conditioned, so the worst row of a few thousand sits at
+    or above 1e-2 although every stage rounds exactly once.  Asserted here: finite output, exact zero rows,
+    cosine >= 0.999 and a relative error below 5e-2 (a wrong index, sign or operand would give O(1));
+    the measured maximum is printed."""
+    rng = np.random.default_rng(3000 + seed)
+    K = int(rng.integers(1, 4))
+    narrow = [8, 24, 40, 64, 72]
+    dims = [int(rng.choice(narrow)) for _ in range(K + 1)]
+    ms = [int(rng.choice([8, 16, 48, 64])) for _ in range(K)]
+    g1, d_out = int(rng.choice([8, 32, 64])), int(rng.choice([8, 16, 32]))
+    N, T = int(rng.integers(60, 3000)), int(rng.choice([1, 3, 10, 50]))
+    g = torch.Generator().manual_seed(4000 + seed)
+
+    def rn(*shape, std=1.0):
+        return torch.randn(shape, generator=g) * std
+
+    dtype = torch.bfloat16
+    X = rn(N, dims[0]).to(dtype)
+    layers = [{"Q": rn(ms[k], dims[k], std=dims[k] ** -0.5).to(dtype), "q": rn(ms[k], std=0.01),
+               "W": rn(dims[k + 1], dims[k] + ms[k], std=(dims[k] + ms[k]) ** -0.5).to(dtype),
+               "w": rn(dims[k + 1], std=0.01)} for k in range(K)]
+    head = {"G1": rn(g1, dims[-1], std=dims[-1] ** -0.5).to(dtype), "g": rn(g1, std=0.01),
+            "G2": rn(d_out, g1, std=g1 ** -0.5).to(dtype)}
+    idx = torch.randint(0, N, (N, T), generator=g, dtype=torch.int32)
+    alpha = O.normalize_counts(torch.randint(1, 101, (N, T), generator=g, dtype=torch.int32).numpy())
+    Lf, Hf = params_f64(layers, head)
+    ref = O.embed_all(to_f64(X), idx.numpy(), alpha, Lf, Hf)
+    Ld, Hd = _to_dev(layers, head)
+    out = ctx.pinsage_embed_all(X.to(DEV), idx.to(DEV), torch.from_numpy(alpha).to(DEV), Ld, Hd)
+    rel, cos = row_errors(to_f64(out), ref)
+    live = np.linalg.norm(ref, axis=1) > 1e-3          # nearly dead rows: direction is ill-conditioned
+    print(f"narrow bf16 case {seed}: dims={dims} ms={ms} K={K} max rel L2 {rel[live].max():.3e} "
+          f"(north_star gate 1e-2 applies from 128 columns)")
+    assert np.isfinite(to_f64(out)).all() and rel[live].max() < 5e-2 and cos[live].min() >= 0.999
 
 
 # ------------------------------------------------------------------ aggregator variants (NEXT #1)
@@ -626,6 +673,9 @@ def test_grid_exchange_from_two_streams():
     c2 = binding.Context(0, stream=s2.cuda_stream)
     try:
         ref = c1.pinsage_combine(H, n, W, w).clone()
+        # many tiles per CTA pair (30 000 rows = 118 row tiles on 36 lanes): against the ORACLE first
+        assert_rows_close(to_f64(ref), O.combine(to_f64(H), to_f64(n), to_f64(W), to_f64(w)), torch.bfloat16,
+                          "d = 1024 combine, grid-wide norm exchange", tol=4e-3)
         o1, o2 = torch.empty_like(ref), torch.empty_like(ref)
         torch.cuda.synchronize()
         for _ in range(300):
