@@ -318,6 +318,7 @@ def run_config(cfg, args, steps, warmup, env, with_clocks=False, e2e_steps=0):
     ctx.pinsage_set_option("gemm_cg", args.gemm_cg)
     ctx.pinsage_set_option("pool_slab", args.pool_slab)
     ctx.pinsage_set_option("gemm_gx", args.gemm_gx)
+    ctx.pinsage_set_option("gemm_bres", args.gemm_bres)
     if args.pool_hubs is not None:
         ctx.pinsage_set_option("pool_hubs", args.pool_hubs)
     ctx.pinsage_set_option("linear_pool", args.linear_pool)
@@ -566,6 +567,7 @@ def main():
     ap.add_argument("--gemm-gx", type=int, default=1,
                     help="wide S3 row norms: 1 global-memory exchange (cooperative launch), 2 the same with a plain "
                          "launch (for ncu, which cannot replay a cooperative one), 0 cluster exchange")
+    ap.add_argument("--gemm-bres", type=int, default=1, help="1 stationary weights in shared memory at short K, 0 off")
     ap.add_argument("--pool-hubs", type=int, default=None,
                     help="hub-split pool: 0 off, -1 automatic, 64..512 forced (default: the library's)")
     ap.add_argument("--calib", action="store_true", help="run the calibration kernels with a single workload too")

@@ -150,6 +150,8 @@ const char *pinsage_version(void);
  *                    between the co-resident CTA pairs of a cooperative launch; 2 = the same with a plain
  *                    launch (Nsight Compute cannot replay a cooperative one; a wait longer than ~2 s traps);
  *                    0 = exchanged inside a thread-block cluster (512-column slabs)
+ *   "gemm_bres"      1 (default) = a GEMM with short K keeps each CTA's share of its weight slab in shared
+ *                    memory for the whole launch and streams only the activations; 0 = always stream both
  *   "pool_slab"      column-slab width in bytes of the S2 pool: -1 automatic (default: 128-byte slabs when
  *                    P exceeds L2 but n_src x 128 bytes fits in 0.7 of it), 0 = whole rows, 32 / 64 / 128 */
 pinsage_status pinsage_set_option(pinsage_ctx *ctx, const char *key, int64_t value);

@@ -1201,6 +1201,9 @@ pinsage_status pinsage_set_option(pinsage_ctx *ctx, const char *key, int64_t val
     } else if (!strcmp(key, "gemm_cg")) {
         if (value < 0 || value > 2) return fail(ctx, PINSAGE_ERR_INVALID_ARG, "gemm_cg must be 0, 1 or 2");
         ctx->tune.cg = (int)value;
+    } else if (!strcmp(key, "gemm_bres")) {
+        if (value != 0 && value != 1) return fail(ctx, PINSAGE_ERR_INVALID_ARG, "gemm_bres must be 0 or 1");
+        ctx->tune.bres = (int)value;
     } else if (!strcmp(key, "gemm_gx")) {
         if (value < 0 || value > 2) return fail(ctx, PINSAGE_ERR_INVALID_ARG, "gemm_gx must be 0, 1 or 2");
         ctx->tune.gx = (int)value;

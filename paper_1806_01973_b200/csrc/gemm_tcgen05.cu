@@ -26,6 +26,7 @@
 // per-row partial sums of squares through distributed shared memory.
 #include "internal.h"
 
+#include <algorithm>
 #include <new>
 #include <vector>
 
@@ -58,7 +59,10 @@ struct TcParams {
     int acc_cols;      // TMEM columns between accumulators = nchunks * CN rounded up to 64
     int tmem_cols;     // allocation (power of two >= 32)
     int stages;
-    int stage_bytes;   // A_BYTES + nchunks * CN * 128
+    int stage_bytes;   // A_BYTES + nchunks * CN * 128 (A_BYTES alone when B is stationary)
+    int bres_bytes;    // > 0: this CTA's share of its B slab stays in shared memory for the whole launch
+                       // ([KB][nchunks * CN / cg rows x 128 B] ahead of the operand ring) and only A streams
+    int b_kb_bytes;    // bytes of one K block of that share
     int epi_halves;    // 1: four epilogue warps own all columns; 2: eight warps, two per row quarter,
                        // each owning half of the slab's columns
     int c_split;       // first column of the second half (multiple of 64)
@@ -373,7 +377,8 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap tmA1, const __grid_constant__
     if ((sbase & 1023u) != 0) __trap();  // SWIZZLE_128B tiles need 1024-byte alignment
 
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-    const uint32_t stg_off = (uint32_t)p.stages * p.stage_bytes;
+    const uint32_t ring_off = (uint32_t)p.bres_bytes;          // the operand ring follows the stationary B
+    const uint32_t stg_off = ring_off + (uint32_t)p.stages * p.stage_bytes;
     const uint32_t bias_off = stg_off + (uint32_t)p.stg_bytes;
     const uint32_t bar_off = bias_off + BIAS_BYTES;
     const uint32_t half_off = bar_off + BAR_BYTES;
@@ -384,6 +389,7 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap tmA1, const __grid_constant__
     const uint32_t bar_tfull = bar_empty + 8 * MAX_STAGES;     // [2]
     const uint32_t bar_tempty = bar_tfull + 16;                // [2]           (CG 2: the leader's are used)
     const uint32_t bar_xchg = bar_tempty + 16;                 // [2]
+    const uint32_t bar_bres = bar_full + 184;                  // stationary B has landed (CG 2: the leader's)
     volatile uint32_t *tmem_slot = reinterpret_cast<volatile uint32_t *>(smem + bar_off + 8 * (2 * MAX_STAGES + 6));
 
     // A "unit" is the CTA (CG 1) or CTA pair (CG 2) that owns one (row tile, slab) at a time.
@@ -421,6 +427,7 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap tmA1, const __grid_constant__
             mbar_init(bar_tempty + 8 * a, 4 * CG * p.epi_halves);  // every epilogue warp of the unit
             mbar_init(bar_xchg + 8 * a, 1);                         // armed per tile with the expected bytes
         }
+        mbar_init(bar_bres, 1);
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
     if (warp == 2) {
@@ -457,6 +464,28 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap tmA1, const __grid_constant__
         // A is read once per slab: keep it in L2 while the other slabs of the same rows still need it
         const uint64_t pol_a = p.n_slabs > 1 ? pol_keep : pol_stream;
         const uint32_t leader_full = CG == 2 ? map_to_cta(bar_full, leader) : bar_full;
+        if (p.bres_bytes && lane0 < p.m_blocks) {
+            // this CTA's share of the slab of B, once: every K block into its place ahead of the ring
+            if (elect_one()) {
+                const uint32_t lbar = CG == 2 ? map_to_cta(bar_bres, leader) : bar_bres;
+                if (half == 0) mbar_expect_tx(bar_bres, (uint32_t)(CG * p.bres_bytes));
+                for (int kb = 0; kb < KB; ++kb) {
+                    const int seg = kb < p.kb1 ? 0 : kb < p.kb1 + p.kb2 ? 1 : 2;
+                    const int ka = (seg == 0 ? kb : seg == 1 ? kb - p.kb1 : kb - p.kb1 - p.kb2) * BK;
+                    const int kcol = (seg == 0 ? 0 : seg == 1 ? p.K1 : p.K12) + ka;
+                    const uint32_t sB = sbase + (uint32_t)kb * p.b_kb_bytes;
+#pragma unroll
+                    for (int j = 0; j < NCH; ++j) {
+                        if (CG == 2)
+                            tma_load_2d_pair(sB + (uint32_t)j * b_rows * 128, &tmB, kcol,
+                                             n0 + j * p.CN + (int)half * b_rows, lbar, pol_keep);
+                        else
+                            tma_load_2d(sB + (uint32_t)j * b_rows * 128, &tmB, kcol, n0 + j * p.CN, lbar, pol_keep);
+                    }
+                }
+            }
+            __syncwarp();
+        }
         int stage = 0;
         uint32_t phase = 0;
         for (long long mb = lane0; mb < p.m_blocks; mb += lanes) {
@@ -467,7 +496,7 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap tmA1, const __grid_constant__
                     const uint32_t full = bar_full + 8 * stage;
                     const int seg = kb < p.kb1 ? 0 : kb < p.kb1 + p.kb2 ? 1 : 2;
                     const int ka = (seg == 0 ? kb : seg == 1 ? kb - p.kb1 : kb - p.kb1 - p.kb2) * BK;
-                    const uint32_t sA = sbase + (uint32_t)stage * p.stage_bytes;
+                    const uint32_t sA = sbase + ring_off + (uint32_t)stage * p.stage_bytes;
                     const int kcol = (seg == 0 ? 0 : seg == 1 ? p.K1 : p.K12) + ka;
                     const CUtensorMap *tmA = seg == 0 ? &tmA1 : seg == 1 ? &tmA2 : &tmA3;
                     if (CG == 2) {
@@ -475,17 +504,21 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap tmA1, const __grid_constant__
                         if (half == 0) mbar_expect_tx(full, 2u * (uint32_t)p.stage_bytes);
                         const uint32_t lfull = leader_full + 8 * stage;
                         tma_load_2d_pair(sA, tmA, ka, m0, lfull, pol_a);
+                        if (!p.bres_bytes) {
 #pragma unroll
-                        for (int j = 0; j < NCH; ++j)
-                            tma_load_2d_pair(sA + A_BYTES + (uint32_t)j * b_rows * 128, &tmB, kcol,
-                                             n0 + j * p.CN + (int)half * b_rows, lfull, pol_keep);
+                            for (int j = 0; j < NCH; ++j)
+                                tma_load_2d_pair(sA + A_BYTES + (uint32_t)j * b_rows * 128, &tmB, kcol,
+                                                 n0 + j * p.CN + (int)half * b_rows, lfull, pol_keep);
+                        }
                     } else {
                         mbar_expect_tx(full, (uint32_t)p.stage_bytes);
                         tma_load_2d(sA, tmA, ka, m0, full, pol_a);
+                        if (!p.bres_bytes) {
 #pragma unroll
-                        for (int j = 0; j < NCH; ++j)
-                            tma_load_2d(sA + A_BYTES + (uint32_t)j * p.CN * 128, &tmB, kcol,
-                                        n0 + j * p.CN, full, pol_keep);
+                            for (int j = 0; j < NCH; ++j)
+                                tma_load_2d(sA + A_BYTES + (uint32_t)j * p.CN * 128, &tmB, kcol,
+                                            n0 + j * p.CN, full, pol_keep);
+                        }
                     }
                 }
                 __syncwarp();
@@ -503,6 +536,10 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap tmA1, const __grid_constant__
             const uint32_t b_step = (uint32_t)((b_rows * 128) >> 4);  // descriptor units between chunks
             int stage = 0, acc = 0;
             uint32_t phase = 0, accphase = 0;
+            if (p.bres_bytes && lane0 < p.m_blocks) {            // stationary B (both CTAs' shares) has landed
+                mbar_wait(bar_bres, 0);
+                tc_fence_after();
+            }
             for (long long mb = lane0; mb < p.m_blocks; mb += lanes) {
                 mbar_wait(bar_tempty + 8 * acc, accphase ^ 1);   // epilogue(s) drained this accumulator
                 tc_fence_after();
@@ -511,8 +548,9 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap tmA1, const __grid_constant__
                     mbar_wait(bar_full + 8 * stage, phase);      // TMA bytes have landed (both CTAs)
                     tc_fence_after();
                     if (elect_one()) {
-                        const uint32_t sA = sbase + (uint32_t)stage * p.stage_bytes;
-                        const uint64_t ad = make_desc(sA), bd = make_desc(sA + A_BYTES);
+                        const uint32_t sA = sbase + ring_off + (uint32_t)stage * p.stage_bytes;
+                        const uint64_t ad = make_desc(sA);
+                        const uint64_t bd = make_desc(p.bres_bytes ? sbase + (uint32_t)kb * p.b_kb_bytes : sA + A_BYTES);
 #pragma unroll
                         for (int k = 0; k < BK / 16; ++k)        // 32 bytes along K per UMMA_K = 16
 #pragma unroll
@@ -967,7 +1005,7 @@ const CUtensorMap *get_map(GemmTcState *st, const void *ptr, long long rows, int
 
 // cg: CTAs per tile (1 or 2).  Slabs without a row norm are 256 columns wide (double-buffered
 // accumulators: the epilogue of tile i overlaps the MMAs of tile i+1).
-bool plan(const GemmArgs &a, int cg, int gx_pref, TcParams &p, int &smem_bytes, const char **why)
+bool plan(const GemmArgs &a, int cg, int gx_pref, int bres_pref, TcParams &p, int &smem_bytes, const char **why)
 {
     auto no = [&](const char *msg) {
         if (why) *why = msg;
@@ -1013,7 +1051,8 @@ bool plan(const GemmArgs &a, int cg, int gx_pref, TcParams &p, int &smem_bytes, 
     int cols = p.nacc * p.acc_cols;
     p.tmem_cols = 32;
     while (p.tmem_cols < cols) p.tmem_cols *= 2;
-    p.stage_bytes = A_BYTES + p.nchunks * (p.CN / cg) * 128;
+    p.b_kb_bytes = p.nchunks * (p.CN / cg) * 128;
+    p.stage_bytes = A_BYTES + p.b_kb_bytes;
     // Eight epilogue warps (two per row quarter, half of the columns each) halve the two-pass row-norm
     // epilogue, which is exposed when the accumulator is single-buffered (measured: S3 +3 % at config 3,
     // +8 % at config 4; the one-pass epilogues lose more from the 32 KB of extra staging than they
@@ -1031,8 +1070,24 @@ bool plan(const GemmArgs &a, int cg, int gx_pref, TcParams &p, int &smem_bytes, 
         if (p.stages >= 3 || p.epi_halves == 1) break;
     }
     if (p.stages < 2) return no("tile does not fit shared memory");
+    // Stationary B: a persistent unit keeps its slab of B for all of its row tiles, so when the CTA's
+    // share of the slab (all K blocks) fits beside an A ring of at least four stages it is loaded once
+    // and only A streams -- half of the L2 -> shared memory traffic of a 256 x 256 tile (short K: S1 / S4 /
+    // S5 at K <= 512).  Not with the tile-major schedule (a unit's slab changes) or the selection epilogue.
+    {
+        const int kbt = p.kb1 + p.kb2 + p.kb3;
+        const long long bres = (long long)kbt * p.b_kb_bytes;
+        const long long room = (long long)SMEM_LIMIT - fixed - bres;
+        const bool tile_major = !a.l2norm && !a.bias && p.n_slabs > 148 / cg && p.m_blocks > 1 &&
+                                (long long)(148 / cg) * p.NS * (a.K1 + a.K2 + a.K3) * 2 > (48LL << 20);
+        if (bres_pref && !a.sel_state && !tile_major && room >= 4 * A_BYTES && p.m_blocks * p.n_slabs > 148 / cg) {
+            p.bres_bytes = (int)bres;
+            p.stage_bytes = A_BYTES;
+            p.stages = (int)std::min<long long>(room / A_BYTES, MAX_STAGES);
+        }
+    }
     p.c_split = round_up((p.NS + 1) / 2, 64);
-    smem_bytes = p.stages * p.stage_bytes + fixed;
+    smem_bytes = p.bres_bytes + p.stages * p.stage_bytes + fixed;
     p.bias = a.bias;
     p.addend = static_cast<const uint4 *>(a.addend);
     p.out_f32 = a.out_f32;
@@ -1062,12 +1117,12 @@ bool plan_auto(const GemmArgs &a, const GemmTune &t, TcParams &p, int &smem_byte
     // 256 x 256) single-CTA tiles keep more independent tiles in flight and are 15-35 % faster.
     const long long Kt = a.K1 + a.K2 + a.K3;
     const bool tensor_bound = Kt * a.N >= 160 * (Kt + a.N);
-    if ((t.cg == 2 || (t.cg == 0 && tensor_bound)) && plan(a, 2, t.gx, p, smem_bytes, nullptr)) return true;
+    if ((t.cg == 2 || (t.cg == 0 && tensor_bound)) && plan(a, 2, t.gx, t.bres, p, smem_bytes, nullptr)) return true;
     if (t.cg == 2) {
         if (why) *why = "shape not supported by the CTA-pair kernel";
         return false;
     }
-    return plan(a, 1, t.gx, p, smem_bytes, why);
+    return plan(a, 1, t.gx, t.bres, p, smem_bytes, why);
 }
 
 template <int CG, int NCH>

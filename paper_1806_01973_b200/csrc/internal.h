@@ -58,6 +58,7 @@ struct GemmTune {
                    // global memory between co-resident CTA pairs, cooperative launch; 2 = the same with a
                    // plain launch (Nsight Compute cannot replay a cooperative one; a wait that outlasts
                    // ~2 s traps instead of hanging); 0 = 512-column slabs exchanged inside a cluster
+    int bres = 1;  // 1 = keep the CTA's share of B in shared memory when it fits (short K), 0 = always stream it
 };
 // Per-context state of the launcher: function attributes already set, co-resident cluster counts, the
 // exchange buffers of the grid-wide row-norm exchange (one per stream used, sized from the SM count),

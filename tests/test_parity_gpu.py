@@ -222,6 +222,30 @@ def test_dense_matches_oracle(ctx, dtype, M, k, n_out):
     assert ran >= 3
 
 
+@pytest.mark.parametrize("M,k,n_out,cg", [(40_000, 512, 512, 2), (40_000, 512, 256, 0), (38_001, 256, 256, 1),
+                                          (50_000, 136, 264, 1), (50_000, 520, 200, 2)])
+def test_dense_stationary_weights_many_tiles(ctx, M, k, n_out, cg):
+    """Short K with more tiles than CTAs: the CTA's share of the weight slab stays in shared memory for the
+    whole launch and only the activations stream (diagnostic key gemm_bres; ragged K blocks, ragged slabs
+    and ragged last row tiles included).  Against the oracle on every row, and bit-identical to the
+    streaming form (the MMAs run in the same order)."""
+    A = _rand((M, k), torch.bfloat16, 23)
+    Wt = _rand((n_out, k), torch.bfloat16, 24, scale=k ** -0.5)
+    b = _rand((n_out,), torch.float32, 25, scale=0.1)
+    ref = O.dense(to_f64(A), to_f64(Wt), to_f64(b), True)
+    outs = []
+    with _impl(ctx, 0, cg):
+        for bres in (1, 0):
+            ctx.pinsage_set_option("gemm_bres", bres)
+            try:
+                outs.append(ctx.pinsage_dense(A.to(DEV), Wt.to(DEV), b.to(DEV), True))
+            finally:
+                ctx.pinsage_set_option("gemm_bres", 1)
+    err = np.abs(to_f64(outs[0]) - ref).max(axis=1) / (np.abs(ref).max(axis=1) + 1e-3)
+    assert err.max() < 8e-3, err.max()
+    assert torch.equal(outs[0].view(torch.int16), outs[1].view(torch.int16))
+
+
 # ------------------------------------------------------------------ S3 combine
 @pytest.mark.parametrize("dtype", DTYPES)
 @pytest.mark.parametrize("M,d_in,m,d", [(1, 8, 8, 8), (130, 64, 64, 64), (1000, 256, 256, 256),
