@@ -448,6 +448,67 @@ def run_config(cfg, args, steps, warmup, env, with_clocks=False, e2e_steps=0):
     return rec
 
 
+def run_extras(local, dev):
+    """The steps around the hot path, timed briefly so that their numbers reach
+    the same record: the neighbourhood builder (the step before the path), targeted inference (Algorithm 2
+    on a minibatch) and the exact top-K lookup (the step after it).  CUDA events, best of 3 after a warm-up."""
+    import torch
+    from paper_1806_01973_b200 import binding, synth
+    res = {}
+
+    def best_ms(fn, reps=3, warm=1):
+        best = float("inf")
+        for it in range(warm + reps):
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record()
+            fn()
+            e1.record()
+            torch.cuda.synchronize()
+            if it >= warm:
+                best = min(best, e0.elapsed_time(e1))
+        return best
+
+    with binding.Context(local) as ctx:
+        # pinsage_build_neighbourhoods: N = 10^6, out-degrees uniform on [1, 40], 200 walks x 5 steps, T = 50
+        N, walks, wlen, T = 1_000_000, 200, 5, 50
+        row_ptr, col = synth.make_csr(N, 1, 40, law="uniform", seed=1, device=dev)
+        ms = best_ms(lambda: ctx.pinsage_build_neighbourhoods(row_ptr, col, walks, wlen, T, 0))
+        res["build_neighbourhoods"] = {"value": N / (ms * 1e-3), "unit": "neighbourhoods/s", "ms": ms,
+                                       "walk_steps_per_s": N * walks * wlen / (ms * 1e-3),
+                                       "config": {"N": N, "edges": int(col.numel()), "n_walks": walks,
+                                                  "walk_len": wlen, "T": T}}
+        del row_ptr, col
+        # pinsage_embed_nodes on config 2's graph: 1 / 1024 / 16384 targets
+        cfg = synth.CONFIGS["cfg2"]
+        X = synth.make_features(cfg, device=dev)
+        layers, head = synth.make_params(cfg, device=dev)
+        idx, counts = synth.make_graph(cfg, device=dev)
+        alpha = ctx.pinsage_normalize_counts(counts)
+        del counts
+        res["embed_nodes"] = {"graph": "cfg2", "unit": "ms per call"}
+        g = torch.Generator(device=dev).manual_seed(5)
+        for m in (1, 1024, 16384):
+            t = torch.randint(0, cfg.N, (m,), generator=g, device=dev, dtype=torch.int32)
+            res["embed_nodes"][str(m)] = best_ms(lambda: ctx.pinsage_embed_nodes(X, idx, alpha, layers, head, t))
+        del X, idx, alpha, layers, head
+        torch.cuda.empty_cache()
+        # pinsage_topk at the paper's evaluation shape (PAPER.md:289): K = 500 of 5 * 10^6 candidates, d = 1024
+        nq, nc, d, k = 4096, 5_000_000, 1024, 500
+        Z = torch.empty((nc, d), dtype=torch.bfloat16, device=dev)
+        for s0 in range(0, nc, 1 << 20):
+            e1 = min(nc, s0 + (1 << 20))
+            z = torch.randn((e1 - s0, d), generator=g, device=dev)
+            Z[s0:e1] = (z / z.norm(dim=1, keepdim=True)).to(torch.bfloat16)
+        Q = Z[torch.randint(0, nc, (nq,), generator=g, device=dev)].clone()
+        ms = best_ms(lambda: ctx.pinsage_topk(Q, Z, k), reps=2)
+        res["topk"] = {"value": nq / (ms * 1e-3), "unit": "queries/s", "ms": ms,
+                       "gemm_tflops_incl_selection": 2.0 * nq * nc * d / (ms * 1e-3) / 1e12,
+                       "config": {"queries": nq, "candidates": nc, "dim": d, "k": k, "dtype": "bf16"}}
+        del Z, Q
+    torch.cuda.empty_cache()
+    return res
+
+
 def run_ours(args):
     import torch
     import torch.distributed as dist
@@ -540,6 +601,8 @@ def run_ours(args):
                 "kernels": {k: {"achieved": v["tflops"], "frac": v["tflops"] / sustained,
                                 "frac_of_nominal_2250": v["frac_of_nominal_2250"], "ms_per_step": v["ms_per_step"]}
                             for k, v in c3["gemm"].items()}}
+    if everything and world == 1 and not args.no_extras:
+        line["extras"] = run_extras(local, dev)
     if not args.no_cpu and world == 1:
         line["cpu_baseline"], _ = cpu_baseline(head_cfg, args.cpu_seconds)
     print(json.dumps(line))
@@ -572,6 +635,7 @@ def main():
                     help="hub-split pool: 0 off, -1 automatic, 64..512 forced (default: the library's)")
     ap.add_argument("--calib", action="store_true", help="run the calibration kernels with a single workload too")
     ap.add_argument("--no-calib", action="store_true")
+    ap.add_argument("--no-extras", action="store_true", help="skip the neighbourhood builder / embed_nodes / top-K legs")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu", action="store_true")
     ap.add_argument("--cpu-seconds", type=float, default=15.0)

@@ -1080,7 +1080,11 @@ bool plan(const GemmArgs &a, int cg, int gx_pref, int bres_pref, TcParams &p, in
         const long long room = (long long)SMEM_LIMIT - fixed - bres;
         const bool tile_major = !a.l2norm && !a.bias && p.n_slabs > 148 / cg && p.m_blocks > 1 &&
                                 (long long)(148 / cg) * p.NS * (a.K1 + a.K2 + a.K3) * 2 > (48LL << 20);
-        if (bres_pref && !a.sel_state && !tile_major && room >= 4 * A_BYTES && p.m_blocks * p.n_slabs > 148 / cg) {
+        // Measured on B200 (profiles/r02_gemm_bres.md): +4 % on the HBM-bound single-CTA shapes (K = 256,
+        // N = 256: config 2 / 5's S1, S4, S5); with CTA pairs at K = 512 the four A stages that are left do
+        // not cover the HBM latency of a tensor-bound tile stream (config 4 S1 -8 %, S3 at K = 512 -4 %).
+        if (bres_pref && cg == 1 && !a.l2norm && !a.sel_state && !tile_major && room >= 4 * A_BYTES &&
+            p.m_blocks * p.n_slabs > 148) {
             p.bres_bytes = (int)bres;
             p.stage_bytes = A_BYTES;
             p.stages = (int)std::min<long long>(room / A_BYTES, MAX_STAGES);

@@ -152,7 +152,7 @@ def test_hub_split_with_host_tables_matches_device_tables():
         ctx.pinsage_set_option("pool_hubs", -1)
         hI, hW = idx.cpu().pin_memory(), alpha.cpu().pin_memory()
         hO = torch.empty((cfg.N, cfg.d_out), dtype=torch.bfloat16).pin_memory()
-        for cap, chunk_nodes in ((0, 32_768), (380, 0)):
+        for cap, chunk_nodes in ((0, 32_768), (340, 0)):
             ctx.pinsage_set_option("mem_limit_mb", cap)
             hO.zero_()
             ctx.pinsage_embed_all(X, hI, hW, layers, head, out=hO, chunk_nodes=chunk_nodes)
