@@ -32,7 +32,9 @@
  *     legal; a short neighbourhood is padded with any valid id and weight 0.
  *   - nbr_w is used as given (weighted SUM).  The paper's weighted mean = rows that sum to 1,
  *     e.g. produced by pinsage_normalize_counts.
- *   - Identical inputs give bit-identical outputs run to run (no atomics, fixed summation order).
+ *   - Identical inputs give bit-identical outputs run to run (no floating-point atomics, fixed summation
+ *     order).  pinsage_embed_all, pinsage_layer + pinsage_head, and pinsage_embed_nodes give the same bits
+ *     for the same node, whatever the chunking and wherever the buffers live.
  *   - A context is not thread-safe: calls on one context must be serialised by the caller; different
  *     contexts (one per device or stream) may be used from different threads.
  */

@@ -224,13 +224,21 @@ pool_kernel(const uint4 *__restrict__ P, const int *__restrict__ idx, const floa
         for (int h = lane; h < H; h += 32) hbuf[h] = 0.f;
         __syncwarp();
     }
+    // the (id, weight) pairs of the NEXT batch are requested before the current batch's rows are gathered,
+    // so that the table load is off the node's chain of dependent memory latencies
+    int nx_i = 0;
+    float nx_w = 0.f;
+    if (sl < T) {
+        nx_i = ld_stream_i32(irow + sl);
+        if (MODE == 0) nx_w = ld_stream_f32(wrow + sl);
+    }
     for (int tb = 0; tb < T; tb += LPN) {
         const int t = tb + sl;
-        int my_i = 0;
-        float my_w = MODE == 1 ? 1.0f / (float)T : 0.f;
-        if (t < T) {
-            my_i = ld_stream_i32(irow + t);
-            if (MODE == 0) my_w = ld_stream_f32(wrow + t);
+        int my_i = t < T ? nx_i : 0;
+        float my_w = MODE == 1 ? 1.0f / (float)T : (t < T ? nx_w : 0.f);
+        if (t + LPN < T) {
+            nx_i = ld_stream_i32(irow + t + LPN);
+            if (MODE == 0) nx_w = ld_stream_f32(wrow + t + LPN);
         }
         int cnt = min(LPN, T - tb);
         if (hubA != nullptr)                               // hub entry -(rank + 1): its weight goes to A[v, rank]
@@ -252,6 +260,16 @@ pool_kernel(const uint4 *__restrict__ P, const int *__restrict__ idx, const floa
         int j0 = 0;
         for (; j0 + U <= cnt; j0 += U)
             gather_fma<BF16, LPN, CPL, U, EXACT, MODE>(P, my_i, my_w, j0, sl, chunks, acc);
+        // the remainder (< U rows) in at most three rounds of 4, 2 and 1 rows in flight, still in table
+        // order (one row at a time would cost a memory latency each: T = 100 leaves 4 rows, T = 50 two)
+        if (U > 4 && j0 + 4 <= cnt) {
+            gather_fma<BF16, LPN, CPL, 4, EXACT, MODE>(P, my_i, my_w, j0, sl, chunks, acc);
+            j0 += 4;
+        }
+        if (U > 2 && j0 + 2 <= cnt) {
+            gather_fma<BF16, LPN, CPL, 2, EXACT, MODE>(P, my_i, my_w, j0, sl, chunks, acc);
+            j0 += 2;
+        }
         for (; j0 < cnt; ++j0)
             gather_fma<BF16, LPN, CPL, 1, EXACT, MODE>(P, my_i, my_w, j0, sl, chunks, acc);
     }
