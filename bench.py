@@ -319,6 +319,7 @@ def run_config(cfg, args, steps, warmup, env, with_clocks=False, e2e_steps=0):
     ctx.pinsage_set_option("pool_slab", args.pool_slab)
     ctx.pinsage_set_option("gemm_gx", args.gemm_gx)
     ctx.pinsage_set_option("gemm_bres", args.gemm_bres)
+    ctx.pinsage_set_option("head_fused", args.head_fused)
     if args.pool_hubs is not None:
         ctx.pinsage_set_option("pool_hubs", args.pool_hubs)
     ctx.pinsage_set_option("linear_pool", args.linear_pool)
@@ -379,6 +380,11 @@ def run_config(cfg, args, steps, warmup, env, with_clocks=False, e2e_steps=0):
             "ms_per_step": pool_ms / steps,
             "traffic_over_algorithmic": (traffic / (pool_bytes_step * steps / max(pool_n, 1))) if traffic else None}
     gemm = {}
+    if gemm_ms["S5 head"][1] == 0 and gemm_ms["S4 head"][1] > 0:
+        # the head ran as ONE launch (gemm_head.cu): its bytes are H read + out written, `a` stays on chip / in L2
+        f4, f5 = kinds[-2][3], kinds[-1][3]
+        kinds = kinds[:-2] + [("S4+S5 head (one launch)", 3, kinds[-1][2], f4 + f5, (cfg.hidden + cfg.d_out) * e)]
+        gemm_ms["S4+S5 head (one launch)"] = gemm_ms["S4 head"]
     for name, kind, layer, flops, nbytes in kinds:
         kms, kn = gemm_ms[name]
         if kms <= 0:
@@ -630,6 +636,7 @@ def main():
     ap.add_argument("--gemm-gx", type=int, default=1,
                     help="wide S3 row norms: 1 global-memory exchange (cooperative launch), 2 the same with a plain "
                          "launch (for ncu, which cannot replay a cooperative one), 0 cluster exchange")
+    ap.add_argument("--head-fused", type=int, default=1, help="1 S4 -> S5 in one launch where the shape allows, 0 two launches")
     ap.add_argument("--gemm-bres", type=int, default=1, help="1 stationary weights in shared memory at short K, 0 off")
     ap.add_argument("--pool-hubs", type=int, default=None,
                     help="hub-split pool: 0 off, -1 automatic, 64..512 forced (default: the library's)")

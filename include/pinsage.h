@@ -152,6 +152,9 @@ const char *pinsage_version(void);
  *                    between the co-resident CTA pairs of a cooperative launch; 2 = the same with a plain
  *                    launch (Nsight Compute cannot replay a cooperative one; a wait longer than ~2 s traps);
  *                    0 = exchanged inside a thread-block cluster (512-column slabs)
+ *   "head_fused"     1 (default) = the head runs as one launch where the shape allows (BF16, g1 and d_out
+ *                    <= 256: the intermediate a = ReLU(h G1^T + g) stays in an L2-resident scratch and never
+ *                    reaches HBM), 0 = always S4 and S5 as two GEMM launches.  Same bits either way.
  *   "gemm_bres"      1 (default) = a GEMM with short K keeps each CTA's share of its weight slab in shared
  *                    memory for the whole launch and streams only the activations; 0 = always stream both
  *   "pool_slab"      column-slab width in bytes of the S2 pool: -1 automatic (default: 128-byte slabs when

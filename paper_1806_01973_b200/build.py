@@ -16,7 +16,7 @@ PKG = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(PKG, "csrc")
 OBJ = os.path.join(CSRC, "build")
 LIB = os.path.join(PKG, "libpinsage.so")
-SOURCES = ["api.cu", "pool.cu", "walks.cu", "subset.cu", "topk.cu", "split_f32.cu", "hubs.cu", "calib.cu", "gemm_simt.cu", "gemm_tcgen05.cu"]
+SOURCES = ["api.cu", "pool.cu", "walks.cu", "subset.cu", "topk.cu", "split_f32.cu", "hubs.cu", "calib.cu", "gemm_simt.cu", "gemm_tcgen05.cu", "gemm_head.cu"]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
               "-Xcompiler", "-fPIC", "--cudart", "static"]
 

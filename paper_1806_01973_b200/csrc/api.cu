@@ -71,6 +71,9 @@ struct pinsage_ctx {
     int f32_split = -1;              // fp32 GEMMs on the tensor cores by bf16 splitting: -1 automatic, 0 never, 1 always
     void *split_buf = nullptr;       // bf16 planes of the operands of a split fp32 GEMM (grown on demand)
     size_t split_bytes = 0;
+    int head_fused = 1;              // S4 -> S5 in one launch where the shape allows (gemm_head.cu)
+    void *head_scratch = nullptr;    // its L2-resident scratch for the a tiles
+    size_t head_scratch_bytes = 0;
     void *subA = nullptr, *subB = nullptr;   // scratch of pinsage_embed_nodes (sets / compact tensors)
     size_t subA_bytes = 0, subB_bytes = 0;
     // optional per-kernel timing ("profile" option): event pairs around every launch
@@ -420,6 +423,35 @@ pinsage_status run_gemm(pinsage_ctx *ctx, DType dt, const GemmArgs &a, void *scr
     prof_close(ctx, kind, e0, s);
     count_launches(ctx);
     PS_CUDA(ctx, e);
+    return PINSAGE_OK;
+}
+
+// The head of `rows` rows: out = ReLU(h G1^T + g) G2^T.  One launch with the intermediate
+// kept in an L2-resident scratch where the fused kernel covers the shape (BF16 on the tcgen05 path, g1 and
+// d_out <= 256), else S4 into `abuf` [rows x g1] and S5 from it: the same bits either way.
+pinsage_status run_head(pinsage_ctx *ctx, DType dt, int64_t rows, const void *h, const pinsage_head_params *head,
+                        void *abuf, void *out, cudaStream_t s)
+{
+    if (rows == 0) return PINSAGE_OK;
+    if (ctx->head_fused && dt == DType::BF16 && ctx->gemm_impl == 0 && head_tc_supported(head->d, head->g1, head->d_out)) {
+        PS_TRY(ensure_buf(ctx, &ctx->head_scratch, &ctx->head_scratch_bytes, head_tc_scratch_bytes(256, ctx->num_sms),
+                          "head scratch"));
+        const int e0 = prof_mark(ctx, s);
+        cudaError_t e = launch_head_tc(ctx->tc, rows, head->d, head->g1, head->d_out, h, head->G1, head->g, head->G2, out,
+                                       ctx->head_scratch, ctx->num_sms, s, &ctx->launches);
+        prof_close(ctx, PROF_HEAD1, e0, s);
+        count_launches(ctx);
+        PS_CUDA(ctx, e);
+        return PINSAGE_OK;
+    }
+    GemmArgs g;
+    g.M = rows; g.K1 = head->d; g.N = head->g1; g.A1 = h;
+    g.B = head->G1; g.bias = head->g; g.relu = 1; g.out = abuf;
+    PS_TRY(run_gemm(ctx, dt, g, nullptr, 0, s, PROF_HEAD1));
+    GemmArgs g2;
+    g2.M = rows; g2.K1 = head->g1; g2.N = head->d_out; g2.A1 = abuf; g2.B = head->G2; g2.out = out;
+    PS_TRY(run_gemm(ctx, dt, g2, nullptr, 0, s, PROF_HEAD2));
+    if (ctx->poison) PS_CUDA(ctx, cudaMemsetAsync(abuf, 0xFF, (size_t)rows * head->g1 * elem_size(dt), s));
     return PINSAGE_OK;
 }
 
@@ -1179,6 +1211,7 @@ void pinsage_destroy(pinsage_ctx *ctx)
     if (ctx->split_buf) cudaFree(ctx->split_buf);
     if (ctx->hub_buf) cudaFree(ctx->hub_buf);
     if (ctx->hub_tab) cudaFree(ctx->hub_tab);
+    if (ctx->head_scratch) cudaFree(ctx->head_scratch);
     if (ctx->hub_sample) cudaFree(ctx->hub_sample);
     if (ctx->hub_info_h) cudaFreeHost(ctx->hub_info_h);
     if (ctx->ev_hub) cudaEventDestroy(ctx->ev_hub);
@@ -1201,6 +1234,8 @@ pinsage_status pinsage_set_option(pinsage_ctx *ctx, const char *key, int64_t val
     } else if (!strcmp(key, "gemm_cg")) {
         if (value < 0 || value > 2) return fail(ctx, PINSAGE_ERR_INVALID_ARG, "gemm_cg must be 0, 1 or 2");
         ctx->tune.cg = (int)value;
+    } else if (!strcmp(key, "head_fused")) {
+        ctx->head_fused = value != 0;
     } else if (!strcmp(key, "gemm_bres")) {
         if (value != 0 && value != 1) return fail(ctx, PINSAGE_ERR_INVALID_ARG, "gemm_bres must be 0 or 1");
         ctx->tune.bres = (int)value;
@@ -1465,16 +1500,9 @@ pinsage_status pinsage_head(pinsage_ctx *ctx, pinsage_dtype dtype, int64_t N, co
     HintGuard hint(ctx, N);
     for (int64_t r0 = 0; r0 < N; r0 += chunk) {
         const int64_t rows = std::min(chunk, N - r0);
-        GemmArgs g;
-        g.M = rows; g.K1 = params->d; g.N = params->g1;
-        g.A1 = static_cast<const char *>(h) + (size_t)r0 * params->d * es;
-        g.B = params->G1; g.bias = params->g; g.relu = 1; g.out = ctx->ws;
         StepRange r45("S4+S5 head rows %lld+%lld", (long long)r0, (long long)rows);
-        PS_TRY(run_gemm(ctx, dt, g, nullptr, 0, ctx->stream, PROF_HEAD1));
-        GemmArgs g2;
-        g2.M = rows; g2.K1 = params->g1; g2.N = params->d_out; g2.A1 = ctx->ws; g2.B = params->G2;
-        g2.out = static_cast<char *>(out) + (size_t)r0 * params->d_out * es;
-        PS_TRY(run_gemm(ctx, dt, g2, nullptr, 0, ctx->stream, PROF_HEAD2));
+        PS_TRY(run_head(ctx, dt, rows, static_cast<const char *>(h) + (size_t)r0 * params->d * es, params, ctx->ws,
+                        static_cast<char *>(out) + (size_t)r0 * params->d_out * es, ctx->stream));
     }
     return PINSAGE_OK;
 }
@@ -1669,17 +1697,9 @@ pinsage_status pinsage_embed_all(pinsage_ctx *ctx, pinsage_dtype dtype, int64_t 
         if (layer == 0 && h_feats) PS_TRY(sF.release(ctx, c, ctx->stream));
         if (layer != K - 1) return PINSAGE_OK;
         StepRange r45("S4+S5 head rows %lld+%lld", (long long)r0, (long long)rows);
-        GemmArgs g;
-        g.M = rows; g.K1 = head->d; g.N = head->g1;
-        g.A1 = Hlast + (size_t)r0 * head->d * es;
-        g.B = head->G1; g.bias = head->g; g.relu = 1; g.out = abuf;
-        PS_TRY(run_gemm(ctx, dt, g, nullptr, 0, ctx->stream, PROF_HEAD1));
         if (h_out) PS_TRY(sO.acquire(ctx, c, ctx->stream));
-        GemmArgs g2;
-        g2.M = rows; g2.K1 = head->g1; g2.N = head->d_out; g2.A1 = abuf; g2.B = head->G2;
-        g2.out = h_out ? sO.ptr(c) : static_cast<char *>(d_out) + (size_t)r0 * head->d_out * es;
-        PS_TRY(run_gemm(ctx, dt, g2, nullptr, 0, ctx->stream, PROF_HEAD2));
-        if (ctx->poison) PS_CUDA(ctx, cudaMemsetAsync(abuf, 0xFF, (size_t)rows * head->g1 * es, ctx->stream));
+        PS_TRY(run_head(ctx, dt, rows, Hlast + (size_t)r0 * head->d * es, head, abuf,
+                        h_out ? sO.ptr(c) : static_cast<char *>(d_out) + (size_t)r0 * head->d_out * es, ctx->stream));
         if (h_out) PS_TRY(sO.release(ctx, c, r0, rows, ctx->stream));
         return PINSAGE_OK;
     };
@@ -1851,13 +1871,7 @@ pinsage_status pinsage_embed_nodes(pinsage_ctx *ctx, pinsage_dtype dtype, int64_
         cur ^= 1;
     }
     // head on S^(K) (l.15-17), then one row per requested target, in the caller's order
-    GemmArgs g;
-    g.M = n[K]; g.K1 = head->d; g.N = head->g1; g.A1 = Hbuf[cur]; g.B = head->G1; g.bias = head->g;
-    g.relu = 1; g.out = abuf;
-    PS_TRY(run_gemm(ctx, dt, g, nullptr, 0, st, PROF_HEAD1));
-    GemmArgs g2;
-    g2.M = n[K]; g2.K1 = head->g1; g2.N = head->d_out; g2.A1 = abuf; g2.B = head->G2; g2.out = obuf;
-    PS_TRY(run_gemm(ctx, dt, g2, nullptr, 0, st, PROF_HEAD2));
+    PS_TRY(run_head(ctx, dt, n[K], Hbuf[cur], head, abuf, obuf, st));
     PS_CUDA(ctx, subset_gather_rows(obuf, targets, pos(K), M, (size_t)head->d_out * es, out, st, &ctx->launches));
     count_launches(ctx);
     return PINSAGE_OK;

@@ -1,0 +1,325 @@
+// gemm_head.cu -- S4 -> S5 in one launch: out = ReLU(H G1^T + g) G2^T   (Alg. 2 l.16)
+//
+// The head's intermediate a = ReLU(H G1^T + g) [rows x g1] never reaches HBM: every CTA owns two 128-row
+// slots of a small scratch array (grid x 2 x 128 rows: ~19 MB, rewritten every few microseconds, so it
+// lives in L2), stores the a tile of a row tile there (bf16, the SAME rounding as the two-launch form) and
+// reads it back as the A operand of the second GEMM.  Row tiles are taken two at a time and their four
+// GEMM phases are software-pipelined over the two TMEM accumulators,
+//
+//      A(t0) -> acc0 | A(t1) -> acc1 | B(t0) -> acc0 | B(t1) -> acc1 |  A(t2) ...      (A: H G1^T, B: a G2^T)
+//
+// so that the only new dependency -- B(t) must not load a(t) before the epilogue of A(t) has stored it --
+// always has a whole MMA phase of slack, and every epilogue runs under the next phase's MMAs.
+// Result: bit-identical to pinsage_dense(G1, relu) followed by pinsage_dense(G2) (same K order, same
+// roundings), with H read and out written once and nothing else crossing HBM.
+//
+// Single-CTA tiles (these shapes -- g1, d_out <= 256 -- are HBM-bound); warp roles as in gemm_tcgen05.cu:
+// warp 0 TMA producer, warp 1 MMA issuer, warp 2 TMEM allocator, warps 4-7 epilogue.
+#include "internal.h"
+
+#include <algorithm>
+
+#include <cuda.h>
+
+#include "tc_ptx.cuh"
+
+namespace pinsage {
+namespace {
+
+constexpr int HEAD_THREADS = 256;
+constexpr int HEAD_MAX_STAGES = 8;
+constexpr int HEAD_BIAS_FLOATS = 320;          // g1 <= 256, read in 64-column chunks
+constexpr int HEAD_BAR_BYTES = 256;
+
+struct HeadTcParams {
+    long long M, m_blocks;
+    int kb1, kb2;          // 64-wide K blocks of GEMM 1 (over d) and GEMM 2 (over g1)
+    int N1, N2;            // g1, d_out
+    int CN1, CN2;          // MMA N of the two GEMMs (N rounded up to 16)
+    int stages, stage_bytes;
+    const float *bias;     // g [g1]
+    uint32_t idesc1, idesc2;
+};
+
+__device__ __forceinline__ void fence_proxy_async_global()
+{
+    asm volatile("fence.proxy.async.global;" ::: "memory");
+}
+
+__global__ void __launch_bounds__(HEAD_THREADS, 1)
+head_tc_kernel(const __grid_constant__ CUtensorMap tmH, const __grid_constant__ CUtensorMap tmG1,
+               const __grid_constant__ CUtensorMap tmScrOut, const __grid_constant__ CUtensorMap tmScrIn,
+               const __grid_constant__ CUtensorMap tmG2, const __grid_constant__ CUtensorMap tmOut,
+               const HeadTcParams p)
+{
+    extern __shared__ __align__(1024) uint8_t smem[];
+    const uint32_t sbase = smem_u32(smem);
+    if ((sbase & 1023u) != 0) __trap();
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const uint32_t stg_off = (uint32_t)p.stages * p.stage_bytes;
+    const uint32_t bias_off = stg_off + 4 * 2 * STG_WARP_BYTES;
+    const uint32_t bar_off = bias_off + HEAD_BIAS_FLOATS * 4;
+    float *sbias = reinterpret_cast<float *>(smem + bias_off);
+    const uint32_t bar_full = sbase + bar_off;                     // [8]
+    const uint32_t bar_empty = bar_full + 8 * HEAD_MAX_STAGES;     // [8]
+    const uint32_t bar_tfull = bar_empty + 8 * HEAD_MAX_STAGES;    // [2]
+    const uint32_t bar_tempty = bar_tfull + 16;                    // [2]
+    const uint32_t bar_aready = bar_tempty + 16;                   // [2]: a(t) of slot j is in the scratch
+    volatile uint32_t *tmem_slot = reinterpret_cast<volatile uint32_t *>(smem + bar_off + 8 * (2 * HEAD_MAX_STAGES + 6));
+
+    // this CTA's row tiles: blockIdx.x, + gridDim.x, ...; `cnt` of them
+    const long long cnt = p.m_blocks > blockIdx.x ? (p.m_blocks - blockIdx.x + gridDim.x - 1) / gridDim.x : 0;
+    const int scr_row0 = (int)blockIdx.x * 2 * BM;                 // this CTA's two slots of the scratch
+
+    if (warp == 0 && lane == 0) {
+        asm volatile("prefetch.tensormap [%0];" ::"l"(&tmH) : "memory");
+        asm volatile("prefetch.tensormap [%0];" ::"l"(&tmG1) : "memory");
+        asm volatile("prefetch.tensormap [%0];" ::"l"(&tmScrOut) : "memory");
+        asm volatile("prefetch.tensormap [%0];" ::"l"(&tmScrIn) : "memory");
+        asm volatile("prefetch.tensormap [%0];" ::"l"(&tmG2) : "memory");
+        asm volatile("prefetch.tensormap [%0];" ::"l"(&tmOut) : "memory");
+    }
+    if (warp == 1 && lane == 0) {
+        for (int s = 0; s < p.stages; ++s) {
+            mbar_init(bar_full + 8 * s, 1);
+            mbar_init(bar_empty + 8 * s, 1);
+        }
+        for (int a = 0; a < 2; ++a) {
+            mbar_init(bar_tfull + 8 * a, 1);
+            mbar_init(bar_tempty + 8 * a, 4);      // the four epilogue warps
+            mbar_init(bar_aready + 8 * a, 4);
+        }
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    if (warp == 2) {
+        asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(
+                         smem_u32(const_cast<uint32_t *>(tmem_slot))),
+                     "r"(512u)
+                     : "memory");
+        asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
+    }
+    if (warp >= 4) {
+        for (int c = threadIdx.x - 128; c < HEAD_BIAS_FLOATS; c += 128)
+            sbias[c] = (p.bias != nullptr && c < p.N1) ? __ldg(p.bias + c) : 0.f;
+    }
+    tc_fence_before();
+    __syncthreads();
+    tc_fence_after();
+    const uint32_t tmem_base = *tmem_slot;
+
+    // phase ph of pair pr: kind = ph >> 1 (0: H G1^T, 1: a G2^T), j = ph & 1 (tile of the pair = accumulator
+    // = scratch slot); a pair's second tile may not exist
+    if (warp == 0) {
+        // ===== TMA producer ===================================================================
+        uint64_t pol_stream, pol_keep;
+        asm volatile("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(pol_stream));
+        asm volatile("createpolicy.fractional.L2::evict_last.b64 %0, 1.0;" : "=l"(pol_keep));
+        int stage = 0;
+        uint32_t phase = 0;
+        for (long long pr = 0; 2 * pr < cnt; ++pr) {
+            for (int ph = 0; ph < 4; ++ph) {
+                const int kind = ph >> 1, j = ph & 1;
+                if (2 * pr + j >= cnt) continue;
+                const long long mb = blockIdx.x + (2 * pr + j) * (long long)gridDim.x;
+                const int m0 = (int)(mb * BM);
+                const int KB = kind ? p.kb2 : p.kb1, CN = kind ? p.CN2 : p.CN1;
+                if (kind) {                              // a(t) must have been stored by the epilogue
+                    mbar_wait(bar_aready + 8 * j, (uint32_t)(pr & 1));
+                    fence_proxy_async_global();
+                }
+                for (int kb = 0; kb < KB; ++kb) {
+                    mbar_wait(bar_empty + 8 * stage, phase ^ 1);
+                    if (elect_one()) {
+                        const uint32_t full = bar_full + 8 * stage;
+                        const uint32_t sA = sbase + (uint32_t)stage * p.stage_bytes;
+                        mbar_expect_tx(full, (uint32_t)(A_BYTES + CN * 128));
+                        if (kind) {
+                            tma_load_2d(sA, &tmScrIn, kb * BK, scr_row0 + j * BM, full, pol_keep);
+                            tma_load_2d(sA + A_BYTES, &tmG2, kb * BK, 0, full, pol_keep);
+                        } else {
+                            tma_load_2d(sA, &tmH, kb * BK, m0, full, pol_stream);
+                            tma_load_2d(sA + A_BYTES, &tmG1, kb * BK, 0, full, pol_keep);
+                        }
+                    }
+                    __syncwarp();
+                    if (++stage == p.stages) {
+                        stage = 0;
+                        phase ^= 1;
+                    }
+                }
+            }
+        }
+    } else if (warp == 1) {
+        // ===== MMA issuer =====================================================================
+        int stage = 0;
+        uint32_t phase = 0, use[2] = {0, 0};
+        for (long long pr = 0; 2 * pr < cnt; ++pr) {
+            for (int ph = 0; ph < 4; ++ph) {
+                const int kind = ph >> 1, j = ph & 1;
+                if (2 * pr + j >= cnt) continue;
+                const int KB = kind ? p.kb2 : p.kb1;
+                const uint32_t idesc = kind ? p.idesc2 : p.idesc1;
+                mbar_wait(bar_tempty + 8 * j, (use[j] & 1u) ^ 1u);    // the epilogue drained this accumulator
+                tc_fence_after();
+                const uint32_t d0 = tmem_base + (uint32_t)j * 256u;
+                for (int kb = 0; kb < KB; ++kb) {
+                    mbar_wait(bar_full + 8 * stage, phase);
+                    tc_fence_after();
+                    if (elect_one()) {
+                        const uint32_t sA = sbase + (uint32_t)stage * p.stage_bytes;
+                        const uint64_t ad = make_desc(sA), bd = make_desc(sA + A_BYTES);
+#pragma unroll
+                        for (int k = 0; k < BK / 16; ++k)
+                            tc_mma(d0, ad + 2 * k, bd + 2 * k, idesc, k == 0 ? (uint32_t)kb : 1u);
+                        tc_commit(bar_empty + 8 * stage);
+                        if (kb == KB - 1) tc_commit(bar_tfull + 8 * j);
+                    }
+                    __syncwarp();
+                    if (++stage == p.stages) {
+                        stage = 0;
+                        phase ^= 1;
+                    }
+                }
+                ++use[j];
+            }
+        }
+    } else if (warp >= 4) {
+        // ===== epilogue: thread (ew, lane) owns row 32 * ew + lane of the tile ==================
+        const int ew = warp & 3;
+        uint8_t *stg = smem + stg_off + ew * 2 * STG_WARP_BYTES;
+        int sbuf = 0;
+        uint32_t use[2] = {0, 0};
+        for (long long pr = 0; 2 * pr < cnt; ++pr) {
+            for (int ph = 0; ph < 4; ++ph) {
+                const int kind = ph >> 1, j = ph & 1;
+                if (2 * pr + j >= cnt) continue;
+                const long long mb = blockIdx.x + (2 * pr + j) * (long long)gridDim.x;
+                const long long m0 = mb * BM;
+                const int ncols = kind ? p.N2 : p.N1;
+                mbar_wait(bar_tfull + 8 * j, use[j] & 1u);
+                tc_fence_after();
+                const uint32_t t0 = tmem_base + ((uint32_t)(ew * 32) << 16) + (uint32_t)j * 256u;
+                for (int c0 = 0; c0 < ncols; c0 += OUT_CHUNK) {
+                    uint32_t v[2][32];
+                    tc_ld32(t0 + c0, v[0]);
+                    tc_ld32(t0 + c0 + 32, v[1]);
+                    tc_wait_ld();
+                    uint32_t pk[32];
+#pragma unroll
+                    for (int h = 0; h < 2; ++h)
+#pragma unroll
+                        for (int i = 0; i < 32; i += 2) {
+                            float2 z2 = make_float2(__uint_as_float(v[h][i]), __uint_as_float(v[h][i + 1]));
+                            if (!kind) {                 // a = ReLU(acc + g)
+                                z2 = __fadd2_rn(z2, *reinterpret_cast<const float2 *>(sbias + c0 + 32 * h + i));
+                                z2.x = fmaxf(z2.x, 0.f);
+                                z2.y = fmaxf(z2.y, 0.f);
+                            }
+                            __nv_bfloat162 b = __floats2bfloat162_rn(z2.x, z2.y);
+                            pk[16 * h + i / 2] = *reinterpret_cast<uint32_t *>(&b);
+                        }
+                    if (lane == 0) tma_store_wait_read<1>();      // the buffer used two stores ago is free
+                    __syncwarp();
+                    uint8_t *buf = stg + sbuf * STG_WARP_BYTES;
+                    uint8_t *rowp = buf + lane * 128;
+#pragma unroll
+                    for (int q = 0; q < 8; ++q)                   // 16-byte chunk q of the row, XOR-swizzled
+                        *reinterpret_cast<uint4 *>(rowp + ((q ^ (lane & 7)) << 4)) =
+                            make_uint4(pk[4 * q], pk[4 * q + 1], pk[4 * q + 2], pk[4 * q + 3]);
+                    fence_proxy_async();
+                    __syncwarp();
+                    if (lane == 0) {
+                        if (!kind) {
+                            tma_store_2d(&tmScrOut, c0, scr_row0 + j * BM + ew * 32, smem_u32(buf));
+                            tma_store_commit();
+                        } else if (m0 + ew * 32 < p.M) {
+                            tma_store_2d(&tmOut, c0, (int)(m0 + ew * 32), smem_u32(buf));
+                            tma_store_commit();
+                        }
+                    }
+                    sbuf ^= 1;
+                }
+                tc_fence_before();
+                __syncwarp();
+                if (lane == 0) {
+                    mbar_arrive(bar_tempty + 8 * j);
+                    if (!kind) {
+                        // the a tile is in the scratch (complete, not just read out of shared memory)
+                        // before the producer may load it
+                        tma_store_wait_all();
+                        fence_proxy_async_global();
+                        mbar_arrive(bar_aready + 8 * j);
+                    }
+                }
+                ++use[j];
+            }
+        }
+        if (lane == 0) tma_store_wait_all();
+    }
+
+    __syncwarp();
+    tc_fence_before();
+    __syncthreads();
+    if (warp == 2) {
+        tc_fence_after();
+        asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem_base), "r"(512u) : "memory");
+    }
+}
+
+inline int round_up_i(int x, int a) { return (x + a - 1) / a * a; }
+
+}  // namespace
+
+bool head_tc_supported(int32_t d, int32_t g1, int32_t d_out)
+{
+    return d >= 8 && d % 8 == 0 && g1 >= 8 && g1 % 8 == 0 && g1 <= 256 && d_out >= 8 && d_out % 8 == 0 && d_out <= 256;
+}
+
+size_t head_tc_scratch_bytes(int32_t g1, int num_sms) { return (size_t)num_sms * 2 * BM * g1 * 2; }
+
+cudaError_t launch_head_tc(GemmTcState *st, int64_t M, int32_t d, int32_t g1, int32_t d_out, const void *H,
+                           const void *G1, const float *g, const void *G2, void *out, void *scratch, int num_sms,
+                           cudaStream_t s, int *launches)
+{
+    if (!head_tc_supported(d, g1, d_out) || M < 1 || M >= (1LL << 31)) return cudaErrorNotSupported;
+    HeadTcParams p{};
+    p.M = M;
+    p.m_blocks = (M + BM - 1) / BM;
+    p.kb1 = (d + BK - 1) / BK;
+    p.kb2 = (g1 + BK - 1) / BK;
+    p.N1 = g1;
+    p.N2 = d_out;
+    p.CN1 = round_up_i(g1, 16);
+    p.CN2 = round_up_i(d_out, 16);
+    p.stage_bytes = A_BYTES + std::max(p.CN1, p.CN2) * 128;
+    const int fixed = 4 * 2 * STG_WARP_BYTES + HEAD_BIAS_FLOATS * 4 + HEAD_BAR_BYTES;
+    p.stages = std::min((SMEM_LIMIT - fixed) / p.stage_bytes, HEAD_MAX_STAGES);
+    if (p.stages < 2) return cudaErrorNotSupported;
+    p.bias = g;
+    p.idesc1 = (1u << 4) | (1u << 7) | (1u << 10) | ((uint32_t)(p.CN1 >> 3) << 17) | ((uint32_t)(BM >> 4) << 24);
+    p.idesc2 = (1u << 4) | (1u << 7) | (1u << 10) | ((uint32_t)(p.CN2 >> 3) << 17) | ((uint32_t)(BM >> 4) << 24);
+    const int grid = (int)std::min<long long>(num_sms, p.m_blocks);
+    const long long scr_rows = (long long)grid * 2 * BM;
+    const CUtensorMap *m;
+    if (!(m = gemm_tc_map(st, H, M, d, BM, 0, false))) return cudaErrorInvalidValue;
+    const CUtensorMap tmH = *m;
+    if (!(m = gemm_tc_map(st, G1, g1, d, p.CN1, 0, false))) return cudaErrorInvalidValue;
+    const CUtensorMap tmG1 = *m;
+    if (!(m = gemm_tc_map(st, scratch, scr_rows, g1, 32, 0, false))) return cudaErrorInvalidValue;
+    const CUtensorMap tmScrOut = *m;
+    if (!(m = gemm_tc_map(st, scratch, scr_rows, g1, BM, 0, false))) return cudaErrorInvalidValue;
+    const CUtensorMap tmScrIn = *m;
+    if (!(m = gemm_tc_map(st, G2, d_out, g1, p.CN2, 0, false))) return cudaErrorInvalidValue;
+    const CUtensorMap tmG2 = *m;
+    if (!(m = gemm_tc_map(st, out, M, d_out, 32, 0, false))) return cudaErrorInvalidValue;
+    const CUtensorMap tmOut = *m;
+    static_assert(sizeof(CUtensorMap) == 128, "tensor map size");
+    cudaError_t e = cudaFuncSetAttribute(head_tc_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_LIMIT);
+    if (e != cudaSuccess) return e;
+    const int smem = p.stages * p.stage_bytes + fixed;
+    if (launches) ++*launches;
+    head_tc_kernel<<<grid, HEAD_THREADS, smem, s>>>(tmH, tmG1, tmScrOut, tmScrIn, tmG2, tmOut, p);
+    return cudaGetLastError();
+}
+
+}  // namespace pinsage

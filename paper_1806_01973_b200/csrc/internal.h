@@ -7,6 +7,8 @@
 #include <stddef.h>
 #include <stdint.h>
 
+struct CUtensorMap_st;   // (cuda.h's tensor map; only gemm_*.cu include the driver header)
+
 namespace pinsage {
 
 enum class DType : int { BF16 = 0, F32 = 1 };
@@ -70,6 +72,18 @@ void gemm_tc_state_destroy(GemmTcState *st);
 // (the caller reports PINSAGE_ERR_UNSUPPORTED_SHAPE).
 bool gemm_tc_supported(const GemmArgs &a, const GemmTune &t, const char **why);
 cudaError_t launch_gemm_tc(const GemmArgs &a, const GemmTune &t, GemmTcState *st, cudaStream_t s, int *launches);
+// A (cached) tensor map of the row-major matrix [rows x cols] at ptr (bf16, or fp32 with f32), box =
+// box_rows x 128 bytes, SWIZZLE_128B; ld = row stride in elements (0 = cols).  Null when the driver entry
+// point is missing or the encoding fails.  The pointer is valid until the next call on this state.
+const ::CUtensorMap_st *gemm_tc_map(GemmTcState *st, const void *ptr, long long rows, int cols, int box_rows, int ld,
+                                  bool f32);
+
+// ---- gemm_head.cu: S4 -> S5 in one launch, the intermediate a kept in an L2-resident scratch -------------
+bool head_tc_supported(int32_t d, int32_t g1, int32_t d_out);
+size_t head_tc_scratch_bytes(int32_t g1, int num_sms);
+cudaError_t launch_head_tc(GemmTcState *st, int64_t M, int32_t d, int32_t g1, int32_t d_out, const void *H,
+                           const void *G1, const float *g, const void *G2, void *out, void *scratch, int num_sms,
+                           cudaStream_t s, int *launches);
 
 // ---- split_f32.cu: fp32 operands as K-concatenated bf16 planes (fp32 mode on the tensor cores) ----
 // out [rows x 6 (K1 + K2)] bf16 from [S1 | S2] (fp32, row strides ld1 / ld2; all multiples of 4).
