@@ -396,7 +396,12 @@ def run_config(cfg, args, steps, warmup, env, with_clocks=False, e2e_steps=0):
                       "ai_flop_per_byte": ai, "bound_tflops": bound,
                       "bound": "tensor" if bound == sustained else "hbm", "frac_of_bound": tf / bound,
                       "frac_of_nominal_2250": tf / 2250.0}
-    rec = {"workload": workload_config(cfg, args)["workload"], "steps": steps, "warmup": warmup,
+    plan = ctx.pinsage_last_plan()
+    if "hubs=" in plan and "hubs=off" not in plan:
+        roof["note"] = ("hub-split pool: the list entries that name a hub are not gathered (they enter S3 as a third K "
+                        "segment), so `achieved` -- the plain definition's bytes over the pool's time -- is not a "
+                        "bandwidth; the launch itself moves `traffic` bytes")
+    rec = {"workload": workload_config(cfg, args)["workload"], "steps": steps, "warmup": warmup, "plan": plan,
            "ms_per_step": ms_max / steps, "value": job_throughput(cfg.N, steps, world, ms_max), "unit": UNIT,
            "roofline": roof, "gemm": gemm, "gpu_launches": int(launches), "gen_s": round(t_gen, 1)}
     if clocks is not None:

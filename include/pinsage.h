@@ -165,8 +165,8 @@ pinsage_status pinsage_set_option(pinsage_ctx *ctx, const char *key, int64_t val
 int64_t pinsage_launch_count(const pinsage_ctx *ctx);
 
 /* Context-owned description of the memory plan the last pinsage_embed_all call chose, e.g.
- * "chunk=1048576 chunks=48 H=out feats=staged tables=ring out=ring workspace=... staging=..." ("" before
- * the first call).  Valid until the next pinsage_embed_all on this context. */
+ * "chunk=1048576 chunks=48 H=out feats=staged tables=ring out=ring workspace=... staging=... hubs=off"
+ * (hubs=H when the hub-split pool was taken; "" before the first call).  Valid until the next pinsage_embed_all on this context. */
 const char *pinsage_last_plan(const pinsage_ctx *ctx);
 
 /* Per-kernel device time gathered while option "profile" is 1.  Synchronises the context's streams,

@@ -1731,6 +1731,7 @@ pinsage_status pinsage_embed_all(pinsage_ctx *ctx, pinsage_dtype dtype, int64_t 
         if (k == 0) {
             PS_TRY(hub_finish());
             io.hub_remapped = lio.hub_remapped = hubs_on && h_idx;
+            ctx->plan += hubs_on ? " hubs=" + std::to_string(hp.H) : std::string(" hubs=off");
         }
         if (k == 0 && !sF.whole) PS_TRY(sF.begin_pass(ctx));        // streamed features, pass 2: the self rows of S3
         PS_TRY(sI.begin_pass(ctx));                                 // (no-ops for device arrays and for
