@@ -33,12 +33,16 @@ def compute():
     head = {"G1": rng.normal(size=(g1, d)) / np.sqrt(d), "g": rng.normal(size=g1) * 0.01,
             "G2": rng.normal(size=(d_out, g1)) / np.sqrt(g1)}
     out = O.embed_all(X, idx, alpha, layers, head, mode="literal")
-    return out[[0, 1, 17, N - 1]]
+    # four live rows and, last, node 49, whose output is legitimately all zero (its ReLUs are all dead:
+    # reading A3) -- kept as the explicit zero-row case, not as a fourth of the tripwire
+    rows = [0, 1, 17, 33, N - 1]
+    assert all(np.abs(out[r]).max() > 1e-3 for r in rows[:-1])
+    return out[rows]
 
 
 if __name__ == "__main__":
     path = os.path.join(os.path.dirname(os.path.abspath(__file__)), "tiny_rows.txt")
     np.savetxt(path, compute(), fmt="%.17g",
-               header="rows 0, 1, 17, 49 of oracle.embed_all(mode=literal); "
+               header="rows 0, 1, 17, 33, 49 of oracle.embed_all(mode=literal); "
                       "written by tests/golden/make_golden.py")
     print("wrote", path)
