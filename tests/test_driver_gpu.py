@@ -158,3 +158,33 @@ def test_hub_split_with_host_tables_matches_device_tables():
             ctx.pinsage_embed_all(X, hI, hW, layers, head, out=hO, chunk_nodes=chunk_nodes)
             assert torch.equal(hO.view(torch.int16), dev.cpu().view(torch.int16)), ctx.pinsage_last_plan()
         assert "tables=ring" in ctx.pinsage_last_plan(), ctx.pinsage_last_plan()
+
+
+@pytest.mark.parametrize("K,chunk_nodes,cap", [(1, 700, 0), (2, 512, 14), (3, 1000, 14), (2, 0, 0)])
+def test_host_pipeline_rings_many_chunks_repeated(K, chunk_nodes, cap):
+    """The copy / compute pipeline of host buffers under stress: many small chunks (ragged last one), rings
+    forced by a small memory cap, every mix of host and device arrays, K = 1 (layer 1 is also the last
+    layer: the head follows the S3 that consumed a streamed feature chunk), pageable as well as pinned
+    host memory -- ten calls in a row on one context, each bit-identical to the device-buffer result."""
+    cfg = dataclasses.replace(synth.CONFIGS["cfg2"].scaled(9_973), K=K)
+    X, idx, alpha, layers, head, Ld, Hd = _inputs(cfg)
+    with binding.Context(0) as ctx:
+        dev = ctx.pinsage_embed_all(X.to(DEV), idx.to(DEV), alpha.to(DEV), Ld, Hd).cpu()
+        ctx.pinsage_set_option("mem_limit_mb", cap)
+        ctx.pinsage_set_option("debug_poison", 1)
+        hO = torch.empty((cfg.N, cfg.d_out), dtype=X.dtype).pin_memory()
+        pinned = (X.pin_memory(), idx.pin_memory(), alpha.pin_memory())
+        for it in range(10):
+            if it % 5 == 4:      # pageable host memory
+                args = (X.clone(), idx.clone(), alpha.clone())
+            elif it % 5 == 3:    # device features, host tables
+                args = (X.to(DEV), pinned[1], pinned[2])
+            elif it % 5 == 2:    # host features, device tables
+                args = (pinned[0], idx.to(DEV), alpha.to(DEV))
+            else:
+                args = pinned
+            hO.zero_()
+            ctx.pinsage_embed_all(*args, Ld, Hd, out=hO, chunk_nodes=chunk_nodes)
+            assert torch.equal(hO.view(torch.int16), dev.view(torch.int16)), (it, ctx.pinsage_last_plan())
+        if cap:
+            assert "ring" in ctx.pinsage_last_plan().split("out=")[0], ctx.pinsage_last_plan()
