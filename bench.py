@@ -595,7 +595,7 @@ def run_ours(args):
         "ms_per_step": head["ms_per_step"], "higher_is_better": True, "scaling": "weak",
         "vs_baseline": None, "dtype": "bf16" if head_cfg.dtype == "bf16" else "f32",
         "data": "synthetic", "config": workload_config(head_cfg, args),
-        "roofline": head["roofline"], "gemm": head["gemm"],
+        "roofline": head["roofline"], "gemm": head["gemm"], "plan": head.get("plan"),
         "e2e": head.get("e2e"), "gpu_launches": head["gpu_launches"], "clocks": head.get("clocks"),
         "gemm_impl": "tcgen05" if args.gemm_impl == 0 and head_cfg.dtype == "bf16" else "simt",
         "peaks": {"hbm_gbs": hbm, "bf16_tflops_burst": burst, "bf16_tflops_sustained": sustained, "source": src},

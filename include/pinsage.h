@@ -133,7 +133,7 @@ const char *pinsage_version(void);
  *                    tensor cores (A and P_hub W2^T rounded to bf16, exact products, fp32 sum).  The same
  *                    function in real arithmetic and the same error level as the plain pool (which rounds
  *                    all of n to bf16), but a different rounding.  0 = off, H = 64 .. 512 (multiple of 64)
- *                    = on, -1 = on (H = 128) when the sampled hubs hold at least a third of all entries
+ *                    = on, -1 = on (H = 256) when the sampled hubs hold at least a third of all entries
  *                    (one stream synchronisation per call).  Power-law config: 1.45 x faster.
  *   "topk_fused"     pinsage_topk: 1 (default) = once every running list is full, scores are tested against
  *                    the query's k-th score in the GEMM's epilogue and only the keepers leave the SM (no

@@ -1020,7 +1020,8 @@ pinsage_status hub_select_begin(pinsage_ctx *ctx, DType dt, int64_t N, int32_t T
 {
     hp = HubPlan{};
     if (!hub_eligible(ctx, dt, N, T, K, layers)) return PINSAGE_OK;
-    const int H = ctx->pool_hubs > 0 ? ctx->pool_hubs : 128;
+    // automatic: 256 hubs (config 4, step ms with H = 64 / 128 / 192 / 256: 131.7 / 119.6 / 118.4 / 117.4)
+    const int H = ctx->pool_hubs > 0 ? ctx->pool_hubs : 256;
     const size_t nB = align_up((size_t)N * 4, 256), candB = align_up(hub_cand_bytes(), 256);
     const size_t idsB = align_up((size_t)H * 4, 256);
     PS_TRY(ensure_buf(ctx, &ctx->hub_buf, &ctx->hub_bytes, 2 * nB + candB + 2 * idsB + 256, "hub selection scratch"));
