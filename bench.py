@@ -459,10 +459,11 @@ def run_config(cfg, args, steps, warmup, env, with_clocks=False, e2e_steps=0):
     return rec
 
 
-def run_extras(local, dev):
+def run_extras(local, dev, which=("walks", "embed_nodes", "topk")):
     """The steps around the hot path, timed briefly so that their numbers reach
     the same record: the neighbourhood builder (the step before the path), targeted inference (Algorithm 2
-    on a minibatch) and the exact top-K lookup (the step after it).  CUDA events, best of 3 after a warm-up."""
+    on a minibatch) and the exact top-K lookup (the step after it).  CUDA events, best of 3 after a warm-up.
+    `--workload extras [--extras walks,topk]` runs these legs alone (the command the ncu captures use)."""
     import torch
     from paper_1806_01973_b200 import binding, synth
     res = {}
@@ -479,43 +480,46 @@ def run_extras(local, dev):
                 best = min(best, e0.elapsed_time(e1))
         return best
 
+    g = torch.Generator(device=dev).manual_seed(5)
     with binding.Context(local) as ctx:
-        # pinsage_build_neighbourhoods: N = 10^6, out-degrees uniform on [1, 40], 200 walks x 5 steps, T = 50
-        N, walks, wlen, T = 1_000_000, 200, 5, 50
-        row_ptr, col = synth.make_csr(N, 1, 40, law="uniform", seed=1, device=dev)
-        ms = best_ms(lambda: ctx.pinsage_build_neighbourhoods(row_ptr, col, walks, wlen, T, 0))
-        res["build_neighbourhoods"] = {"value": N / (ms * 1e-3), "unit": "neighbourhoods/s", "ms": ms,
-                                       "walk_steps_per_s": N * walks * wlen / (ms * 1e-3),
-                                       "config": {"N": N, "edges": int(col.numel()), "n_walks": walks,
-                                                  "walk_len": wlen, "T": T}}
-        del row_ptr, col
-        # pinsage_embed_nodes on config 2's graph: 1 / 1024 / 16384 targets
-        cfg = synth.CONFIGS["cfg2"]
-        X = synth.make_features(cfg, device=dev)
-        layers, head = synth.make_params(cfg, device=dev)
-        idx, counts = synth.make_graph(cfg, device=dev)
-        alpha = ctx.pinsage_normalize_counts(counts)
-        del counts
-        res["embed_nodes"] = {"graph": "cfg2", "unit": "ms per call"}
-        g = torch.Generator(device=dev).manual_seed(5)
-        for m in (1, 1024, 16384):
-            t = torch.randint(0, cfg.N, (m,), generator=g, device=dev, dtype=torch.int32)
-            res["embed_nodes"][str(m)] = best_ms(lambda: ctx.pinsage_embed_nodes(X, idx, alpha, layers, head, t))
-        del X, idx, alpha, layers, head
-        torch.cuda.empty_cache()
-        # pinsage_topk at the paper's evaluation shape: K = 500 of 5 * 10^6 candidates, d = 1024
-        nq, nc, d, k = 4096, 5_000_000, 1024, 500
-        Z = torch.empty((nc, d), dtype=torch.bfloat16, device=dev)
-        for s0 in range(0, nc, 1 << 20):
-            e1 = min(nc, s0 + (1 << 20))
-            z = torch.randn((e1 - s0, d), generator=g, device=dev)
-            Z[s0:e1] = (z / z.norm(dim=1, keepdim=True)).to(torch.bfloat16)
-        Q = Z[torch.randint(0, nc, (nq,), generator=g, device=dev)].clone()
-        ms = best_ms(lambda: ctx.pinsage_topk(Q, Z, k), reps=2)
-        res["topk"] = {"value": nq / (ms * 1e-3), "unit": "queries/s", "ms": ms,
-                       "gemm_tflops_incl_selection": 2.0 * nq * nc * d / (ms * 1e-3) / 1e12,
-                       "config": {"queries": nq, "candidates": nc, "dim": d, "k": k, "dtype": "bf16"}}
-        del Z, Q
+        if "walks" in which:
+            # pinsage_build_neighbourhoods: N = 10^6, out-degrees uniform on [1, 40], 200 walks x 5 steps, T = 50
+            N, walks, wlen, T = 1_000_000, 200, 5, 50
+            row_ptr, col = synth.make_csr(N, 1, 40, law="uniform", seed=1, device=dev)
+            ms = best_ms(lambda: ctx.pinsage_build_neighbourhoods(row_ptr, col, walks, wlen, T, 0))
+            res["build_neighbourhoods"] = {"value": N / (ms * 1e-3), "unit": "neighbourhoods/s", "ms": ms,
+                                           "walk_steps_per_s": N * walks * wlen / (ms * 1e-3),
+                                           "config": {"N": N, "edges": int(col.numel()), "n_walks": walks,
+                                                      "walk_len": wlen, "T": T}}
+            del row_ptr, col
+        if "embed_nodes" in which:
+            # pinsage_embed_nodes on config 2's graph: 1 / 1024 / 16384 targets
+            cfg = synth.CONFIGS["cfg2"]
+            X = synth.make_features(cfg, device=dev)
+            layers, head = synth.make_params(cfg, device=dev)
+            idx, counts = synth.make_graph(cfg, device=dev)
+            alpha = ctx.pinsage_normalize_counts(counts)
+            del counts
+            res["embed_nodes"] = {"graph": "cfg2", "unit": "ms per call"}
+            for m in (1, 1024, 16384):
+                t = torch.randint(0, cfg.N, (m,), generator=g, device=dev, dtype=torch.int32)
+                res["embed_nodes"][str(m)] = best_ms(lambda: ctx.pinsage_embed_nodes(X, idx, alpha, layers, head, t))
+            del X, idx, alpha, layers, head
+            torch.cuda.empty_cache()
+        if "topk" in which:
+            # pinsage_topk at the paper's evaluation shape: K = 500 of 5 * 10^6 candidates, d = 1024
+            nq, nc, d, k = 4096, 5_000_000, 1024, 500
+            Z = torch.empty((nc, d), dtype=torch.bfloat16, device=dev)
+            for s0 in range(0, nc, 1 << 20):
+                e1 = min(nc, s0 + (1 << 20))
+                z = torch.randn((e1 - s0, d), generator=g, device=dev)
+                Z[s0:e1] = (z / z.norm(dim=1, keepdim=True)).to(torch.bfloat16)
+            Q = Z[torch.randint(0, nc, (nq,), generator=g, device=dev)].clone()
+            ms = best_ms(lambda: ctx.pinsage_topk(Q, Z, k), reps=2)
+            res["topk"] = {"value": nq / (ms * 1e-3), "unit": "queries/s", "ms": ms,
+                           "gemm_tflops_incl_selection": 2.0 * nq * nc * d / (ms * 1e-3) / 1e12,
+                           "config": {"queries": nq, "candidates": nc, "dim": d, "k": k, "dtype": "bf16"}}
+            del Z, Q
     torch.cuda.empty_cache()
     return res
 
@@ -542,6 +546,12 @@ def run_ours(args):
             dist.barrier()
         torch.cuda.synchronize()
 
+    if args.workload == "extras":      # the legs around the path alone (profiles/: the ncu captures of walks / top-K)
+        if rank == 0:
+            print(json.dumps({"extras": run_extras(local, dev, tuple(args.extras.split(",")))}))
+        if world > 1:
+            dist.destroy_process_group()
+        return
     env = (rank, world, local, dev, barrier)
     everything = args.workload == "all"
     head_cfg = synth.CONFIGS[HEADLINE if everything else args.workload]
@@ -629,7 +639,8 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--workload", default="all",
                     help="all (default: cfg5 headline + cfg2-4 in per_config + calibration) | tiny | cfg2 | cfg3 | "
-                         "cfg4 | cfg5 | paper (one workload at full N)")
+                         "cfg4 | cfg5 | paper (one workload at full N) | extras (only the legs around the path, "
+                         "one JSON object; not the contract line)")
     ap.add_argument("--side-steps", type=int, default=5, help="timed steps of each per_config entry")
     ap.add_argument("--nodes", type=int, default=0, help="override N (a '-small' sibling)")
     ap.add_argument("--chunk-nodes", type=int, default=0)
@@ -648,6 +659,8 @@ def main():
     ap.add_argument("--calib", action="store_true", help="run the calibration kernels with a single workload too")
     ap.add_argument("--no-calib", action="store_true")
     ap.add_argument("--no-extras", action="store_true", help="skip the neighbourhood builder / embed_nodes / top-K legs")
+    ap.add_argument("--extras", default="walks,embed_nodes,topk",
+                    help="with --workload extras: which of the legs to run (comma-separated)")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu", action="store_true")
     ap.add_argument("--cpu-seconds", type=float, default=15.0)
@@ -656,7 +669,7 @@ def main():
         args.warmup = 3          # timing rule: at least 3 warm-up steps
     if args.impl == "reference":
         from paper_1806_01973_b200 import synth
-        cfg = synth.CONFIGS[HEADLINE if args.workload == "all" else args.workload]
+        cfg = synth.CONFIGS[HEADLINE if args.workload in ("all", "extras") else args.workload]
         if args.nodes:
             cfg = cfg.scaled(args.nodes)
         run_reference(args, cfg)

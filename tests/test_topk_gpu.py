@@ -125,7 +125,7 @@ def test_topk_argument_errors(ctx):
 
 
 def test_topk_full_size_sampled(ctx):
-    """The shape topk_bench times (K = 500 among 5 million candidates; 4 096 queries,
+    """The shape bench.py's `extras` leg times (K = 500 among 5 million candidates; 4 096 queries,
     d = 1024, bf16), in the launch configuration it times (88 candidate blocks, 87 of them through the
     GEMM's selection epilogue).  Sampled queries are checked against fp64 scores computed on the host
     from the stored bf16 values, block of candidates by block of candidates (numpy), then ordered as
