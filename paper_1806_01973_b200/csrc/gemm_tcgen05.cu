@@ -813,13 +813,13 @@ bool plan(const GemmArgs &a, int cg, int gx_pref, int bres_pref, TcParams &p, in
         const int kbt = p.kb1 + p.kb2 + p.kb3;
         const long long bres = (long long)kbt * p.b_kb_bytes;
         const long long room = (long long)SMEM_LIMIT - fixed - bres;
-        const bool tile_major = !a.l2norm && !a.bias && p.n_slabs > 148 / cg && p.m_blocks > 1 &&
-                                (long long)(148 / cg) * p.NS * (a.K1 + a.K2 + a.K3) * 2 > (48LL << 20);
+        const bool tile_major = !a.l2norm && !a.bias && p.n_slabs > TUNED_SMS / cg && p.m_blocks > 1 &&
+                                (long long)(TUNED_SMS / cg) * p.NS * (a.K1 + a.K2 + a.K3) * 2 > (48LL << 20);
         // Measured on B200 (profiles/r02_gemm_bres.md): +4 % on the HBM-bound single-CTA shapes (K = 256,
         // N = 256: config 2 / 5's S1, S4, S5); with CTA pairs at K = 512 the four A stages that are left do
         // not cover the HBM latency of a tensor-bound tile stream (config 4 S1 -8 %, S3 at K = 512 -4 %).
         if (bres_pref && cg == 1 && !a.l2norm && !a.sel_state && !tile_major && room >= 4 * A_BYTES &&
-            p.m_blocks * p.n_slabs > 148) {
+            p.m_blocks * p.n_slabs > TUNED_SMS) {
             p.bres_bytes = (int)bres;
             p.stage_bytes = A_BYTES;
             p.stages = (int)std::min<long long>(room / A_BYTES, MAX_STAGES);
@@ -837,8 +837,8 @@ bool plan(const GemmArgs &a, int cg, int gx_pref, int bres_pref, TcParams &p, in
     p.sel_id0 = a.sel_id0;
     // slabs in flight (one per resident unit) against half of L2; only without per-slab state (bias,
     // row-norm exchange), i.e. the top-K lookup's products
-    p.tile_major = !a.l2norm && !a.bias && p.n_slabs > 148 / cg && p.m_blocks > 1 &&
-                   (long long)(148 / cg) * p.NS * (a.K1 + a.K2 + a.K3) * 2 > (48LL << 20);
+    p.tile_major = !a.l2norm && !a.bias && p.n_slabs > TUNED_SMS / cg && p.m_blocks > 1 &&
+                   (long long)(TUNED_SMS / cg) * p.NS * (a.K1 + a.K2 + a.K3) * 2 > (48LL << 20);
     p.relu = a.relu;
     p.l2norm = a.l2norm;
     // instruction descriptor, kind::f16: D fp32 (bit 4), A and B bf16 (bits 7, 10), both K-major,

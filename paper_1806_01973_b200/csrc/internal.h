@@ -11,6 +11,11 @@ struct CUtensorMap_st;   // (cuda.h's tensor map; only gemm_*.cu include the dri
 
 namespace pinsage {
 
+// SM count of the part the size heuristics were tuned on (B200: 148).  Heuristics only -- grids and buffers that
+// must match the device are sized from the context's num_sms.
+constexpr int TUNED_SMS = 148;
+
+
 enum class DType : int { BF16 = 0, F32 = 1 };
 
 inline size_t elem_size(DType t) { return t == DType::BF16 ? 2 : 4; }

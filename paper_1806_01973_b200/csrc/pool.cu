@@ -529,7 +529,7 @@ cudaError_t launch_validate(int64_t n_dst, int64_t n_src, int32_t T, const int32
     const long long total = n_dst * (long long)T;
     set_ll<<<1, 1, 0, s>>>(first_bad, LLONG_MAX);
     long long blocks = (total + 255) / 256;
-    if (blocks > 148 * 16) blocks = 148 * 16;
+    if (blocks > TUNED_SMS * 16) blocks = TUNED_SMS * 16;
     if (blocks < 1) blocks = 1;
     validate_kernel<<<(unsigned)blocks, 256, 0, s>>>(idx, w, total, n_src, first_bad);
     fix_first_bad<<<1, 1, 0, s>>>(first_bad);
