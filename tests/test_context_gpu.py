@@ -143,3 +143,55 @@ def test_fp32_kernel_choice_follows_the_call_not_the_chunk():
         assert not torch.equal(simt.view(torch.int32), whole.view(torch.int32))
         rows = np.array([0, 17, 69_999])
         assert_rows_close(to_f64(whole[rows]), to_f64(simt[rows]), torch.float32, "split vs SIMT rows")
+
+
+def test_two_contexts_on_two_threads_share_nothing():
+    """include/pinsage.h: different contexts may be used from different threads.  Two threads, each with its
+    own context on its own stream, run different graphs at the same time (ctypes releases the GIL during a
+    call) -- a uniform graph at d = 1024 (CTA pairs, the cooperative grid-wide norm exchange, cached tensor
+    maps) and a skewed one (hub selection with its pinned read-back, hub-split pool, fused head) -- several
+    times over; every result equals, bit for bit, what the same context configuration gives when it runs
+    alone."""
+    import threading
+    jobs = []
+    for name, N, opts in (("cfg3", 20_000, {}), ("cfg4", 150_000, {"pool_hubs": 64})):
+        cfg = synth.CONFIGS[name].scaled(N)
+        X = synth.make_features(cfg, device=DEV)
+        layers, head = synth.make_params(cfg, device=DEV)
+        idx, counts = synth.make_graph(cfg, device=DEV)
+        with binding.Context(0) as ctx:
+            for k, v in opts.items():
+                ctx.pinsage_set_option(k, v)
+            alpha = ctx.pinsage_normalize_counts(counts)
+            alone = ctx.pinsage_embed_all(X, idx, alpha, layers, head, chunk_nodes=8192).clone()
+        torch.cuda.synchronize()
+        jobs.append(dict(X=X, idx=idx, alpha=alpha, layers=layers, head=head, opts=opts, alone=alone,
+                         outs=[torch.empty_like(alone) for _ in range(4)], err=None))
+
+    start = threading.Barrier(len(jobs))
+
+    def work(job):
+        try:
+            s = torch.cuda.Stream(device=DEV)
+            with binding.Context(0, stream=s.cuda_stream) as ctx:
+                for k, v in job["opts"].items():
+                    ctx.pinsage_set_option(k, v)
+                start.wait()
+                for out in job["outs"]:
+                    ctx.pinsage_embed_all(job["X"], job["idx"], job["alpha"], job["layers"], job["head"],
+                                          chunk_nodes=8192, out=out)
+                s.synchronize()
+        except Exception as ex:     # surfaced in the main thread
+            job["err"] = ex
+
+    threads = [threading.Thread(target=work, args=(j,)) for j in jobs]
+    for t in threads:
+        t.start()
+    for t in threads:
+        t.join(timeout=300)
+        assert not t.is_alive(), "a worker thread hangs"
+    torch.cuda.synchronize()
+    for j in jobs:
+        assert j["err"] is None, j["err"]
+        for out in j["outs"]:
+            assert torch.equal(out.view(torch.int16), j["alone"].view(torch.int16))
