@@ -652,7 +652,7 @@ def main():
     ap.add_argument("--gemm-gx", type=int, default=1,
                     help="wide S3 row norms: 1 global-memory exchange (cooperative launch), 2 the same with a plain "
                          "launch (for ncu, which cannot replay a cooperative one), 0 cluster exchange")
-    ap.add_argument("--head-fused", type=int, default=1, help="1 S4 -> S5 in one launch where the shape allows, 0 two launches")
+    ap.add_argument("--head-fused", type=int, default=1, help="1 S4 -> S5 in one launch where the shape allows, 2 its single-CTA form only, 0 two launches")
     ap.add_argument("--gemm-bres", type=int, default=1, help="1 stationary weights in shared memory at short K, 0 off")
     ap.add_argument("--pool-hubs", type=int, default=None,
                     help="hub-split pool: 0 off, -1 automatic, 64..512 forced (default: the library's)")

@@ -154,7 +154,9 @@ const char *pinsage_version(void);
  *                    0 = exchanged inside a thread-block cluster (512-column slabs)
  *   "head_fused"     1 (default) = the head runs as one launch where the shape allows (BF16, g1 and d_out
  *                    <= 256: the intermediate a = ReLU(h G1^T + g) stays in an L2-resident scratch and never
- *                    reaches HBM), 0 = always S4 and S5 as two GEMM launches.  Same bits either way.
+ *                    reaches HBM; CTA pairs that keep the weights in shared memory for the whole launch where
+ *                    those fit, else single CTAs that stream them), 2 = the single-CTA form only, 0 = always S4
+ *                    and S5 as two GEMM launches.  Same bits in every form.
  *   "gemm_bres"      1 (default) = a GEMM with short K keeps each CTA's share of its weight slab in shared
  *                    memory for the whole launch and streams only the activations; 0 = always stream both
  *   "pool_slab"      column-slab width in bytes of the S2 pool: -1 automatic (default: 128-byte slabs when

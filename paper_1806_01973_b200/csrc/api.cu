@@ -71,7 +71,7 @@ struct pinsage_ctx {
     int f32_split = -1;              // fp32 GEMMs on the tensor cores by bf16 splitting: -1 automatic, 0 never, 1 always
     void *split_buf = nullptr;       // bf16 planes of the operands of a split fp32 GEMM (grown on demand)
     size_t split_bytes = 0;
-    int head_fused = 1;              // S4 -> S5 in one launch where the shape allows (gemm_head.cu)
+    int head_fused = 1;              // S4 -> S5 in one launch where the shape allows (gemm_head.cu); 2 = its single-CTA form only
     void *head_scratch = nullptr;    // its L2-resident scratch for the a tiles
     size_t head_scratch_bytes = 0;
     void *subA = nullptr, *subB = nullptr;   // scratch of pinsage_embed_nodes (sets / compact tensors)
@@ -438,7 +438,7 @@ pinsage_status run_head(pinsage_ctx *ctx, DType dt, int64_t rows, const void *h,
                           "head scratch"));
         const int e0 = prof_mark(ctx, s);
         cudaError_t e = launch_head_tc(ctx->tc, rows, head->d, head->g1, head->d_out, h, head->G1, head->g, head->G2, out,
-                                       ctx->head_scratch, ctx->num_sms, s, &ctx->launches);
+                                       ctx->head_scratch, ctx->num_sms, s, &ctx->launches, ctx->head_fused != 2);
         prof_close(ctx, PROF_HEAD1, e0, s);
         count_launches(ctx);
         PS_CUDA(ctx, e);
@@ -1236,7 +1236,8 @@ pinsage_status pinsage_set_option(pinsage_ctx *ctx, const char *key, int64_t val
         if (value < 0 || value > 2) return fail(ctx, PINSAGE_ERR_INVALID_ARG, "gemm_cg must be 0, 1 or 2");
         ctx->tune.cg = (int)value;
     } else if (!strcmp(key, "head_fused")) {
-        ctx->head_fused = value != 0;
+        if (value < 0 || value > 2) return fail(ctx, PINSAGE_ERR_INVALID_ARG, "head_fused = %lld outside {0, 1, 2}", (long long)value);
+        ctx->head_fused = (int)value;
     } else if (!strcmp(key, "gemm_bres")) {
         if (value != 0 && value != 1) return fail(ctx, PINSAGE_ERR_INVALID_ARG, "gemm_bres must be 0 or 1");
         ctx->tune.bres = (int)value;

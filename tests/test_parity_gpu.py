@@ -248,31 +248,36 @@ def test_dense_stationary_weights_many_tiles(ctx, M, k, n_out, cg):
 
 @pytest.mark.parametrize("M,d,g1,d_out", [(1, 64, 64, 32), (130, 256, 256, 128), (20_011, 256, 256, 128),
                                           (50_000, 256, 256, 256), (3_001, 136, 72, 40), (100_000, 512, 256, 256),
-                                          (777, 1024, 128, 8), (40_000, 264, 200, 136)])
+                                          (777, 1024, 128, 8), (40_000, 264, 200, 136),
+                                          (256 * 74 + 100, 256, 256, 256), (256 * 74 * 3 + 129, 128, 256, 64),
+                                          (300_000, 256, 256, 256)])
 def test_head_one_launch_matches_oracle_and_two_launches(ctx, M, d, g1, d_out):
     """S4 -> S5 in one launch (gemm_head.cu; the intermediate a lives in an L2-resident scratch, two row
     tiles software-pipelined over the two TMEM accumulators): against the oracle's head on every row, and
-    bit-identical to the two-launch form (same K order, same roundings) -- one tile, a trailing single tile of
-    a pair, many tiles per CTA, ragged K blocks and ragged widths."""
+    bit-identical to the two-launch form (same K order, same roundings) -- in both of its forms: CTA pairs
+    with the weights stationary in shared memory (taken from ~19 000 rows where the weights fit) and single
+    CTAs that stream them.  One tile, a trailing single tile of a pair, a last pair tile whose second half is
+    empty, many tiles per CTA, ragged K blocks and ragged widths."""
     h = _rand((M, d), torch.bfloat16, 60)
     hp = {"G1": _rand((g1, d), torch.bfloat16, 61, scale=d ** -0.5), "g": _rand((g1,), torch.float32, 62, scale=0.05),
           "G2": _rand((d_out, g1), torch.bfloat16, 63, scale=g1 ** -0.5)}
     Hd = {k: v.to(DEV) for k, v in hp.items()}
-    l0 = ctx.pinsage_launch_count()
-    one = ctx.pinsage_head(h.to(DEV), Hd)
-    n_one = ctx.pinsage_launch_count() - l0
-    ctx.pinsage_set_option("head_fused", 0)
+    hd = h.to(DEV)
+    outs, counts = {}, {}
     try:
-        l0 = ctx.pinsage_launch_count()
-        two = ctx.pinsage_head(h.to(DEV), Hd)
-        n_two = ctx.pinsage_launch_count() - l0
+        for mode in (1, 2, 0):
+            ctx.pinsage_set_option("head_fused", mode)
+            l0 = ctx.pinsage_launch_count()
+            outs[mode] = ctx.pinsage_head(hd, Hd)
+            counts[mode] = ctx.pinsage_launch_count() - l0
     finally:
         ctx.pinsage_set_option("head_fused", 1)
     torch.cuda.synchronize()
-    assert n_one == 1 and n_two == 2, (n_one, n_two)
-    assert torch.equal(one.view(torch.int16), two.view(torch.int16))
+    assert counts == {1: 1, 2: 1, 0: 2}, counts
+    assert torch.equal(outs[1].view(torch.int16), outs[0].view(torch.int16))
+    assert torch.equal(outs[2].view(torch.int16), outs[0].view(torch.int16))
     ref = O.head(to_f64(h), {k: to_f64(v) for k, v in hp.items()})
-    err = np.abs(to_f64(one) - ref).max(axis=1) / (np.abs(ref).max(axis=1) + 1e-3)
+    err = np.abs(to_f64(outs[1]) - ref).max(axis=1) / (np.abs(ref).max(axis=1) + 1e-3)
     assert err.max() < 1.2e-2, err.max()          # two bf16 roundings (a, out) of O(1) values, per element
 
 
