@@ -28,6 +28,8 @@ namespace {
 
 constexpr int HEAD_THREADS = 256;
 constexpr int HEAD_PAIR_THREADS = 384;          // the pair kernel runs eight epilogue warps
+constexpr int HEAD_LAG = 2;                     // ... and issues a G2^T of tile t after H G1^T of tile t + HEAD_LAG
+constexpr int HEAD_SLOTS = HEAD_LAG + 1;        // a tiles a CTA has in the scratch at one time
 constexpr int HEAD_MAX_STAGES = 8;
 constexpr int HEAD_BIAS_FLOATS = 320;          // g1 <= 256, read in 64-column chunks
 constexpr int HEAD_BAR_BYTES = 256;
@@ -305,14 +307,15 @@ head_tc_pair_kernel(const __grid_constant__ CUtensorMap tmH, const __grid_consta
     const uint32_t bar_empty = bar_full + 8 * HEAD_MAX_STAGES;     // [8]
     const uint32_t bar_tfull = bar_empty + 8 * HEAD_MAX_STAGES;    // [2]
     const uint32_t bar_tempty = bar_tfull + 16;                    // [2]  the leader's are used
-    const uint32_t bar_aready = bar_tempty + 16;                   // [2]
-    const uint32_t bar_w = bar_aready + 16;                        // weights have landed (the leader's)
-    volatile uint32_t *tmem_slot = reinterpret_cast<volatile uint32_t *>(smem + bar_off + 8 * (2 * HEAD_MAX_STAGES + 7));
+    const uint32_t bar_aready = bar_tempty + 16;                   // [HEAD_SLOTS]: a(t) of that slot is in the scratch
+    const uint32_t bar_w = bar_aready + 8 * HEAD_SLOTS;            // weights have landed (the leader's)
+    volatile uint32_t *tmem_slot =
+        reinterpret_cast<volatile uint32_t *>(smem + bar_off + 8 * (2 * HEAD_MAX_STAGES + 4 + HEAD_SLOTS + 1));
 
     const uint32_t half = cluster_ctarank();                       // which 128 rows of the 256-row tile
     const long long unit = blockIdx.x >> 1, units = gridDim.x >> 1;
     const long long cnt = p.m_blocks > unit ? (p.m_blocks - unit + units - 1) / units : 0;
-    const int scr_row0 = (int)blockIdx.x * 2 * BM;                 // this CTA's two slots of the scratch
+    const int scr_row0 = (int)blockIdx.x * HEAD_SLOTS * BM;        // this CTA's slots of the scratch
 
     if (warp == 0 && lane == 0) {
         asm volatile("prefetch.tensormap [%0];" ::"l"(&tmH) : "memory");
@@ -330,8 +333,8 @@ head_tc_pair_kernel(const __grid_constant__ CUtensorMap tmH, const __grid_consta
         for (int a = 0; a < 2; ++a) {
             mbar_init(bar_tfull + 8 * a, 1);
             mbar_init(bar_tempty + 8 * a, 16);     // the eight epilogue warps of both CTAs
-            mbar_init(bar_aready + 8 * a, 8);      // this CTA's own epilogue warps
         }
+        for (int a = 0; a < HEAD_SLOTS; ++a) mbar_init(bar_aready + 8 * a, 8);   // this CTA's own epilogue warps
         mbar_init(bar_w, 1);
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
@@ -369,15 +372,16 @@ head_tc_pair_kernel(const __grid_constant__ CUtensorMap tmH, const __grid_consta
         __syncwarp();
         int stage = 0;
         uint32_t phase = 0;
-        for (long long pr = 0; 2 * pr < cnt; ++pr) {
-            for (int ph = 0; ph < 4; ++ph) {
-                const int kind = ph >> 1, j = ph & 1;
-                if (2 * pr + j >= cnt) continue;
-                const long long mb = unit + (2 * pr + j) * units;
+        for (long long st = 0; st < cnt + HEAD_LAG; ++st) {
+            for (int kind = 0; kind < 2; ++kind) {
+                const long long t = kind ? st - HEAD_LAG : st;       // this CTA pair's t-th tile
+                if (t < 0 || t >= cnt) continue;
+                const long long mb = unit + t * units;
                 const int m0 = (int)(mb * (2 * BM)) + (int)half * BM;
                 const int KB = kind ? p.kb2 : p.kb1;
+                const int slot = (int)(t % HEAD_SLOTS);
                 if (kind) {                              // this CTA's rows of a(t) are in the scratch
-                    mbar_wait(bar_aready + 8 * j, (uint32_t)(pr & 1));
+                    mbar_wait(bar_aready + 8 * slot, (uint32_t)((t / HEAD_SLOTS) & 1));
                     fence_proxy_async_global();
                 }
                 for (int kb = 0; kb < KB; ++kb) {
@@ -385,7 +389,7 @@ head_tc_pair_kernel(const __grid_constant__ CUtensorMap tmH, const __grid_consta
                     if (elect_one()) {
                         if (half == 0) mbar_expect_tx(bar_full + 8 * stage, 2u * A_BYTES);   // both CTAs' bytes
                         const uint32_t sA = sbase + ring_off + (uint32_t)stage * A_BYTES;
-                        if (kind) tma_load_2d_pair(sA, &tmScrIn, kb * BK, scr_row0 + j * BM, leader_full + 8 * stage, pol_keep);
+                        if (kind) tma_load_2d_pair(sA, &tmScrIn, kb * BK, scr_row0 + slot * BM, leader_full + 8 * stage, pol_keep);
                         else tma_load_2d_pair(sA, &tmH, kb * BK, m0, leader_full + 8 * stage, pol_stream);
                     }
                     __syncwarp();
@@ -401,12 +405,13 @@ head_tc_pair_kernel(const __grid_constant__ CUtensorMap tmH, const __grid_consta
         if (half == 0 && cnt > 0) {
             int stage = 0;
             uint32_t phase = 0, use[2] = {0, 0};
+            int j = 0;                                   // accumulators alternate from phase to phase
             mbar_wait(bar_w, 0);
             tc_fence_after();
-            for (long long pr = 0; 2 * pr < cnt; ++pr) {
-                for (int ph = 0; ph < 4; ++ph) {
-                    const int kind = ph >> 1, j = ph & 1;
-                    if (2 * pr + j >= cnt) continue;
+            for (long long st = 0; st < cnt + HEAD_LAG; ++st) {
+                for (int kind = 0; kind < 2; ++kind) {
+                    const long long t = kind ? st - HEAD_LAG : st;
+                    if (t < 0 || t >= cnt) continue;
                     const int KB = kind ? p.kb2 : p.kb1;
                     const uint32_t idesc = kind ? p.idesc2 : p.idesc1;
                     const uint32_t wbase = sbase + (kind ? w2_off : 0u), wblk = (uint32_t)(kind ? p.w2_blk : p.w1_blk);
@@ -432,6 +437,7 @@ head_tc_pair_kernel(const __grid_constant__ CUtensorMap tmH, const __grid_consta
                         }
                     }
                     ++use[j];
+                    j ^= 1;
                 }
             }
         }
@@ -442,13 +448,15 @@ head_tc_pair_kernel(const __grid_constant__ CUtensorMap tmH, const __grid_consta
         uint8_t *buf = smem + stg_off + (eh * 4 + ew) * STG_WARP_BYTES;     // one staging buffer per warp
         const uint32_t tempty_leader = map_to_cta(bar_tempty, 0);
         uint32_t use[2] = {0, 0};
-        for (long long pr = 0; 2 * pr < cnt; ++pr) {
-            for (int ph = 0; ph < 4; ++ph) {
-                const int kind = ph >> 1, j = ph & 1;
-                if (2 * pr + j >= cnt) continue;
-                const long long mb = unit + (2 * pr + j) * units;
+        int j = 0;
+        for (long long st = 0; st < cnt + HEAD_LAG; ++st) {
+            for (int kind = 0; kind < 2; ++kind) {
+                const long long t = kind ? st - HEAD_LAG : st;
+                if (t < 0 || t >= cnt) continue;
+                const long long mb = unit + t * units;
                 const long long m0 = mb * (2 * BM) + (long long)half * BM;
                 const int ncols = kind ? p.N2 : p.N1;
+                const int slot = (int)(t % HEAD_SLOTS);
                 const int c_split = ((ncols + 1) / 2 + OUT_CHUNK - 1) / OUT_CHUNK * OUT_CHUNK;
                 const int c_lo = eh ? c_split : 0, c_hi = eh ? ncols : min(c_split, ncols);
                 mbar_wait(bar_tfull + 8 * j, use[j] & 1u);
@@ -484,7 +492,7 @@ head_tc_pair_kernel(const __grid_constant__ CUtensorMap tmH, const __grid_consta
                     __syncwarp();
                     if (lane == 0) {
                         if (!kind) {
-                            tma_store_2d(&tmScrOut, c0, scr_row0 + j * BM + ew * 32, smem_u32(buf));
+                            tma_store_2d(&tmScrOut, c0, scr_row0 + slot * BM + ew * 32, smem_u32(buf));
                             tma_store_commit();
                         } else if (m0 + ew * 32 < p.M) {
                             tma_store_2d(&tmOut, c0, (int)(m0 + ew * 32), smem_u32(buf));
@@ -499,10 +507,11 @@ head_tc_pair_kernel(const __grid_constant__ CUtensorMap tmH, const __grid_consta
                     if (!kind) {
                         tma_store_wait_all();
                         fence_proxy_async_global();
-                        mbar_arrive(bar_aready + 8 * j);
+                        mbar_arrive(bar_aready + 8 * slot);
                     }
                 }
                 ++use[j];
+                j ^= 1;
             }
         }
         if (lane == 0) tma_store_wait_all();
@@ -526,7 +535,7 @@ bool head_tc_supported(int32_t d, int32_t g1, int32_t d_out)
     return d >= 8 && d % 8 == 0 && g1 >= 8 && g1 % 8 == 0 && g1 <= 256 && d_out >= 8 && d_out % 8 == 0 && d_out <= 256;
 }
 
-size_t head_tc_scratch_bytes(int32_t g1, int num_sms) { return (size_t)num_sms * 2 * BM * g1 * 2; }
+size_t head_tc_scratch_bytes(int32_t g1, int num_sms) { return (size_t)num_sms * HEAD_SLOTS * BM * g1 * 2; }
 
 namespace {
 
@@ -557,7 +566,7 @@ cudaError_t launch_head_pair(GemmTcState *st, int64_t M, int32_t d, int32_t g1, 
     p.idesc1 = (1u << 4) | (1u << 7) | (1u << 10) | ((uint32_t)(p.CN1 >> 3) << 17) | ((uint32_t)((2 * BM) >> 4) << 24);
     p.idesc2 = (1u << 4) | (1u << 7) | (1u << 10) | ((uint32_t)(p.CN2 >> 3) << 17) | ((uint32_t)((2 * BM) >> 4) << 24);
     const int grid = 2 * pairs;
-    const long long scr_rows = (long long)grid * 2 * BM;
+    const long long scr_rows = (long long)grid * HEAD_SLOTS * BM;
     const CUtensorMap *m;
     if (!(m = gemm_tc_map(st, H, M, d, BM, 0, false))) return cudaErrorInvalidValue;
     const CUtensorMap tmH = *m;
