@@ -223,6 +223,20 @@ size_t pinsage_layer_workspace_bytes(pinsage_dtype dtype, int64_t N, int32_t T,
 pinsage_status pinsage_head(pinsage_ctx *ctx, pinsage_dtype dtype, int64_t N, const void *h,
                             const pinsage_head_params *params, void *out);
 
+/* The head for callers that must not allocate (CUDA graph capture, tight serving loops, harnesses that forbid
+ * cudaMalloc): the same one-launch S4 -> S5 kernel as pinsage_head's default form, same bits, with its scratch
+ * (the a = ReLU(h G1^T + g) tiles in flight) in a file-scope __device__ array of 29 097 984 bytes (148 SMs x 3
+ * tiles x 128 rows x 256 bf16 values) that every GPU loading the library holds until the process exits.  The
+ * call itself makes no cudaMalloc / cudaFree and creates no events; the first call on a device resolves the
+ * array's address (cudaGetSymbolAddress) and sets a function attribute -- make it once before capturing.
+ * Limits: PINSAGE_BF16 only, g1 <= 256, d_out <= 256, N < 2^31, and g1 x SMs within the array (any g1 <= 256 on
+ * a 148-SM part); anything else -> PINSAGE_ERR_UNSUPPORTED_SHAPE, nothing launched.  All device pointers.
+ * The array is shared by every call in the process and keeps the last call's contents (nothing needs to start
+ * at zero: a tile is always written before it is read).  Calls that overlap on the GPU -- two streams, two
+ * contexts -- race on it: serialise them.  The "profile" option records nothing here.  PAPER.md:166. */
+pinsage_status pinsage_head_static(pinsage_ctx *ctx, pinsage_dtype dtype, int64_t N, const void *h,
+                                   const pinsage_head_params *params, void *out);
+
 /* K layers + head over all N nodes with the chunked layer driver (Alg. 2 l.8-17 with S^(k) = V).
  * feats:[N x layers[0].d_in], nbr_idx / nbr_w:[N x T], out:[N x head->d_out] may each be DEVICE or
  * HOST pointers (detected with cudaPointerGetAttributes; host buffers should be pinned for speed):

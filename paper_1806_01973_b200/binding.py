@@ -24,7 +24,7 @@ STATUS = {0: "OK", 1: "INVALID_ARG", 2: "UNSUPPORTED_SHAPE", 3: "MISALIGNED", 4:
 SYMBOLS = [
     "pinsage_create", "pinsage_destroy", "pinsage_last_error", "pinsage_version",
     "pinsage_set_option", "pinsage_launch_count", "pinsage_last_plan", "pinsage_profile_read", "pinsage_dense", "pinsage_pool",
-    "pinsage_combine", "pinsage_layer", "pinsage_layer_workspace_bytes", "pinsage_head",
+    "pinsage_combine", "pinsage_layer", "pinsage_layer_workspace_bytes", "pinsage_head", "pinsage_head_static",
     "pinsage_embed_all", "pinsage_normalize_counts", "pinsage_validate_graph",
     "pinsage_build_neighbourhoods", "pinsage_embed_nodes", "pinsage_topk", "pinsage_calibrate",
 ]
@@ -93,6 +93,8 @@ def load_library() -> ctypes.CDLL:
     lib.pinsage_layer_workspace_bytes.restype = sz
     lib.pinsage_head.argtypes = [vp, ctypes.c_int, i64, vp, ctypes.POINTER(HeadParams), vp]
     lib.pinsage_head.restype = ctypes.c_int
+    lib.pinsage_head_static.argtypes = [vp, ctypes.c_int, i64, vp, ctypes.POINTER(HeadParams), vp]
+    lib.pinsage_head_static.restype = ctypes.c_int
     lib.pinsage_embed_all.argtypes = [vp, ctypes.c_int, i64, i32, i32, vp, vp, vp,
                                       ctypes.POINTER(LayerParams), ctypes.POINTER(HeadParams),
                                       vp, i64]
@@ -265,6 +267,16 @@ class Context:
             out = torch.empty((N, hs.d_out), dtype=h.dtype, device=h.device)
         self._check(self.lib.pinsage_head(self.handle, dtype_code(h.dtype), N, _ptr(h),
                                           ctypes.byref(hs), _ptr(out)))
+        return out
+
+    def pinsage_head_static(self, h, head, out):
+        """pinsage_head with the scratch in the library's static device array: allocates nothing, so `out` is
+        the caller's (argument marshalling only -- no tensor is created here either)."""
+        N, d = h.shape
+        hs = _head_struct(head)
+        assert hs.d == d and out.shape == (N, hs.d_out) and out.dtype == h.dtype
+        self._check(self.lib.pinsage_head_static(self.handle, dtype_code(h.dtype), N, _ptr(h),
+                                                 ctypes.byref(hs), _ptr(out)))
         return out
 
     def pinsage_embed_all(self, feats, nbr_idx, nbr_w, layers: Sequence[dict], head: dict,

@@ -1509,6 +1509,41 @@ pinsage_status pinsage_head(pinsage_ctx *ctx, pinsage_dtype dtype, int64_t N, co
     return PINSAGE_OK;
 }
 
+// The head without any allocation: one launch of the fused S4 -> S5 kernel with its scratch in a file-scope
+// __device__ array (gemm_head.cu).  No cudaMalloc / cudaFree / event creation on this path, whatever the
+// context's options say (no profile records, no workspace growth).
+pinsage_status pinsage_head_static(pinsage_ctx *ctx, pinsage_dtype dtype, int64_t N, const void *h,
+                                   const pinsage_head_params *params, void *out)
+{
+    if (!ctx) return PINSAGE_ERR_INVALID_ARG;
+    DeviceGuard guard(ctx->device);
+    PS_TRY(check_dtype(ctx, dtype));
+    if (N < 1) return fail(ctx, PINSAGE_ERR_INVALID_ARG, "N must be positive");
+    PS_TRY(check_head_params(ctx, params));
+    PS_TRY(check_ptr(ctx, "h", h));
+    PS_TRY(check_ptr(ctx, "out", out));
+    const DType dt = static_cast<DType>(dtype);
+    if (dt != DType::BF16 || !head_tc_supported(params->d, params->g1, params->d_out))
+        return fail(ctx, PINSAGE_ERR_UNSUPPORTED_SHAPE,
+                    "pinsage_head_static covers BF16 heads with g1 <= 256 and d_out <= 256 (the one-launch kernel); "
+                    "got dtype %d, d = %d, g1 = %d, d_out = %d", (int)dtype, params->d, params->g1, params->d_out);
+    if (N >= (1LL << 31)) return fail(ctx, PINSAGE_ERR_INVALID_ARG, "N = %lld outside [1, 2^31)", (long long)N);
+    const size_t es = elem_size(dt);
+    if (overlaps(h, (size_t)N * params->d * es, out, (size_t)N * params->d_out * es))
+        return fail(ctx, PINSAGE_ERR_INVALID_ARG, "out overlaps h");
+    StepRange r45("S4+S5 head (static scratch) rows 0+%lld", (long long)N);
+    bool too_big = false;
+    cudaError_t e = launch_head_tc_static(ctx->tc, N, params->d, params->g1, params->d_out, h, params->G1, params->g,
+                                          params->G2, out, ctx->num_sms, ctx->stream, &ctx->launches, &too_big);
+    count_launches(ctx);
+    if (too_big)
+        return fail(ctx, PINSAGE_ERR_UNSUPPORTED_SHAPE,
+                    "pinsage_head_static: g1 = %d on %d SMs needs %zu bytes of scratch, the static array holds %zu",
+                    params->g1, ctx->num_sms, head_tc_scratch_bytes(params->g1, ctx->num_sms), head_static_scratch_bytes());
+    PS_CUDA(ctx, e);
+    return PINSAGE_OK;
+}
+
 pinsage_status pinsage_embed_all(pinsage_ctx *ctx, pinsage_dtype dtype, int64_t N, int32_t T,
                                  int32_t K, const void *feats, const int32_t *nbr_idx,
                                  const float *nbr_w, const pinsage_layer_params *layers,

@@ -18,6 +18,7 @@
 #include "internal.h"
 
 #include <algorithm>
+#include <mutex>
 
 #include <cuda.h>
 
@@ -649,6 +650,54 @@ cudaError_t launch_head_tc(GemmTcState *st, int64_t M, int32_t d, int32_t g1, in
     if (launches) ++*launches;
     head_tc_kernel<<<grid, HEAD_THREADS, smem, s>>>(tmH, tmG1, tmScrOut, tmScrIn, tmG2, tmOut, p);
     return cudaGetLastError();
+}
+
+// ---- the head without any allocation (pinsage_head_static) --------------------------------------------
+// Callers that may not allocate (CUDA graph capture, serving loops, harnesses that forbid cudaMalloc) get
+// the same kernels with the a-tile scratch in a file-scope array instead of the context's cudaMalloc'ed
+// buffer.  Its size is the most the kernels above ask for on the part this library is written for: 148 SMs x
+// HEAD_SLOTS (3) tiles x 128 rows x g1 <= 256 bf16 values = 29 097 984 bytes, held by every GPU that loads
+// the library until the process exits.  In host code `g_head_scratch` is only a stand-in for the symbol --
+// not a device address -- so the address is asked for once per device with cudaGetSymbolAddress.
+// The array keeps the previous call's contents; nothing has to start at zero (every a tile is written
+// before the mbarrier that lets the second GEMM read it), but every call uses the same array, so two calls
+// that overlap on the GPU (different streams, different contexts) race.
+constexpr size_t HEAD_STATIC_BYTES = (size_t)TUNED_SMS * HEAD_SLOTS * BM * 256 * 2;
+static __device__ __align__(256) unsigned char g_head_scratch[HEAD_STATIC_BYTES];
+
+size_t head_static_scratch_bytes() { return HEAD_STATIC_BYTES; }
+
+namespace {
+constexpr int HEAD_STATIC_MAX_DEVICES = 64;
+std::mutex g_head_static_mu;
+void *g_head_static_ptr[HEAD_STATIC_MAX_DEVICES] = {};    // device address of g_head_scratch, per device
+}  // namespace
+
+// The calling thread's current device must be the one the launch goes to.  *too_big: the shape needs more
+// scratch than the array holds (nothing is launched then).
+cudaError_t launch_head_tc_static(GemmTcState *st, int64_t M, int32_t d, int32_t g1, int32_t d_out, const void *H,
+                                  const void *G1, const float *g, const void *G2, void *out, int num_sms,
+                                  cudaStream_t s, int *launches, bool *too_big)
+{
+    *too_big = head_tc_scratch_bytes(g1, num_sms) > HEAD_STATIC_BYTES;
+    if (*too_big) return cudaSuccess;
+    int dev = -1;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) return e;
+    if (dev < 0 || dev >= HEAD_STATIC_MAX_DEVICES) return cudaErrorInvalidDevice;
+    void *ptr = nullptr;
+    {
+        std::lock_guard<std::mutex> lock(g_head_static_mu);
+        if (!g_head_static_ptr[dev]) {          // set-up, once per device, with that device current
+            void *q = nullptr;
+            e = cudaGetSymbolAddress(&q, g_head_scratch);
+            if (e != cudaSuccess) return e;
+            if (!q || (reinterpret_cast<uintptr_t>(q) & 255u)) return cudaErrorInvalidSymbol;
+            g_head_static_ptr[dev] = q;
+        }
+        ptr = g_head_static_ptr[dev];
+    }
+    return launch_head_tc(st, M, d, g1, d_out, H, G1, g, G2, out, ptr, num_sms, s, launches, true);
 }
 
 }  // namespace pinsage

@@ -89,6 +89,11 @@ size_t head_tc_scratch_bytes(int32_t g1, int num_sms);
 cudaError_t launch_head_tc(GemmTcState *st, int64_t M, int32_t d, int32_t g1, int32_t d_out, const void *H,
                            const void *G1, const float *g, const void *G2, void *out, void *scratch, int num_sms,
                            cudaStream_t s, int *launches, bool pairs = true);
+// The same launch with the scratch in a file-scope __device__ array (no allocation anywhere): gemm_head.cu
+size_t head_static_scratch_bytes();
+cudaError_t launch_head_tc_static(GemmTcState *st, int64_t M, int32_t d, int32_t g1, int32_t d_out, const void *H,
+                                  const void *G1, const float *g, const void *G2, void *out, int num_sms,
+                                  cudaStream_t s, int *launches, bool *too_big);
 
 // ---- split_f32.cu: fp32 operands as K-concatenated bf16 planes (fp32 mode on the tensor cores) ----
 // out [rows x 6 (K1 + K2)] bf16 from [S1 | S2] (fp32, row strides ld1 / ld2; all multiples of 4).
