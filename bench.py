@@ -524,6 +524,57 @@ def run_extras(local, dev, which=("walks", "embed_nodes", "topk")):
     return res
 
 
+def run_libgemm(local, dev, reps=10, rounds=3):
+    """`--workload libgemm`: context for the GEMM rooflines, NOT part of the path or of the contract line.
+    The plain GEMMs of configs 3-5 (no epilogue: the library routine has none) as pinsage_dense and as
+    torch.matmul (cuBLAS), interleaved in one process on the same HBM-resident operands, in 2^20-row chunks as
+    the layer driver issues them: what a vendor GEMM reaches on these streaming shapes under the same power
+    cap.  TFLOP/s per round; CUDA events around `reps` back-to-back passes over all rows."""
+    import torch
+    from paper_1806_01973_b200 import binding
+    shapes = [("cfg4 S1 / S4", 20_000_000, 512, 512), ("cfg4 S3 without the hub segment", 20_000_000, 1024, 512),
+              ("cfg4 S3 with 256 hubs", 20_000_000, 1280, 512), ("cfg4 S5", 20_000_000, 512, 256),
+              ("cfg3 S1", 5_000_000, 2048, 1024), ("cfg3 S3", 5_000_000, 3072, 1024),
+              ("cfg3 S4 / S5", 5_000_000, 1024, 1024), ("cfg5 S1 / S4 / S5", 50_000_000, 256, 256),
+              ("cfg5 S3", 50_000_000, 512, 256)]
+    g = torch.Generator(device=dev).manual_seed(1)
+    out_recs = []
+    with binding.Context(local) as ctx:
+        for name, M, K, N in shapes:
+            A = torch.empty((M, K), dtype=torch.bfloat16, device=dev)
+            for s0 in range(0, M, 1 << 21):
+                A[s0:s0 + (1 << 21)].normal_(generator=g)
+            W = (torch.randn((N, K), generator=g, device=dev) * K ** -0.5).to(torch.bfloat16)
+            Wt = W.t()
+            out = torch.empty((M, N), dtype=torch.bfloat16, device=dev)
+            chunk = 1 << 20
+
+            def lib():
+                for s0 in range(0, M, chunk):
+                    torch.matmul(A[s0:s0 + chunk], Wt, out=out[s0:s0 + chunk])
+
+            def ours():
+                for s0 in range(0, M, chunk):
+                    ctx.pinsage_dense(A[s0:s0 + chunk], W, None, False, out=out[s0:s0 + chunk])
+
+            rec = {"shape": name, "M": M, "K": K, "N": N, "unit": "TFLOP/s", "pinsage_dense": [], "torch_matmul": []}
+            for _ in range(rounds):
+                for key, fn in (("torch_matmul", lib), ("pinsage_dense", ours)):
+                    fn()
+                    torch.cuda.synchronize()
+                    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                    e0.record()
+                    for _ in range(reps):
+                        fn()
+                    e1.record()
+                    torch.cuda.synchronize()
+                    rec[key].append(round(2.0 * M * K * N * reps / e0.elapsed_time(e1) / 1e9, 1))
+            out_recs.append(rec)
+            del A, W, Wt, out
+            torch.cuda.empty_cache()
+    return out_recs
+
+
 def run_ours(args):
     import torch
     import torch.distributed as dist
@@ -549,6 +600,12 @@ def run_ours(args):
     if args.workload == "extras":      # the legs around the path alone (profiles/: the ncu captures of walks / top-K)
         if rank == 0:
             print(json.dumps({"extras": run_extras(local, dev, tuple(args.extras.split(",")))}))
+        if world > 1:
+            dist.destroy_process_group()
+        return
+    if args.workload == "libgemm":     # context only: the library GEMM on the path's shapes (profiles/r02_gemm.md)
+        if rank == 0:
+            print(json.dumps({"libgemm": run_libgemm(local, dev)}))
         if world > 1:
             dist.destroy_process_group()
         return
@@ -640,7 +697,8 @@ def main():
     ap.add_argument("--workload", default="all",
                     help="all (default: cfg5 headline + cfg2-4 in per_config + calibration) | tiny | cfg2 | cfg3 | "
                          "cfg4 | cfg5 | paper (one workload at full N) | extras (only the legs around the path, "
-                         "one JSON object; not the contract line)")
+                         "one JSON object; not the contract line) | libgemm (context: pinsage_dense and torch.matmul "
+                         "on the path's GEMM shapes)")
     ap.add_argument("--side-steps", type=int, default=5, help="timed steps of each per_config entry")
     ap.add_argument("--nodes", type=int, default=0, help="override N (a '-small' sibling)")
     ap.add_argument("--chunk-nodes", type=int, default=0)
@@ -669,7 +727,7 @@ def main():
         args.warmup = 3          # timing rule: at least 3 warm-up steps
     if args.impl == "reference":
         from paper_1806_01973_b200 import synth
-        cfg = synth.CONFIGS[HEADLINE if args.workload in ("all", "extras") else args.workload]
+        cfg = synth.CONFIGS[HEADLINE if args.workload in ("all", "extras", "libgemm") else args.workload]
         if args.nodes:
             cfg = cfg.scaled(args.nodes)
         run_reference(args, cfg)
