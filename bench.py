@@ -524,7 +524,7 @@ def run_extras(local, dev, which=("walks", "embed_nodes", "topk")):
     return res
 
 
-def run_libgemm(local, dev, reps=10, rounds=3):
+def run_libgemm(local, dev, reps=10, rounds=3, only=None):
     """`--workload libgemm`: context for the GEMM rooflines, NOT part of the path or of the contract line.
     The plain GEMMs of configs 3-5 (no epilogue: the library routine has none) as pinsage_dense and as
     torch.matmul (cuBLAS), interleaved in one process on the same HBM-resident operands, in 2^20-row chunks as
@@ -540,7 +540,9 @@ def run_libgemm(local, dev, reps=10, rounds=3):
     g = torch.Generator(device=dev).manual_seed(1)
     out_recs = []
     with binding.Context(local) as ctx:
-        for name, M, K, N in shapes:
+        for si, (name, M, K, N) in enumerate(shapes):
+            if only is not None and si not in only:
+                continue
             A = torch.empty((M, K), dtype=torch.bfloat16, device=dev)
             for s0 in range(0, M, 1 << 21):
                 A[s0:s0 + (1 << 21)].normal_(generator=g)
@@ -605,7 +607,8 @@ def run_ours(args):
         return
     if args.workload == "libgemm":     # context only: the library GEMM on the path's shapes (profiles/r02_gemm.md)
         if rank == 0:
-            print(json.dumps({"libgemm": run_libgemm(local, dev)}))
+            only = None if args.libgemm_shapes == "all" else {int(x) for x in args.libgemm_shapes.split(",")}
+            print(json.dumps({"libgemm": run_libgemm(local, dev, reps=args.libgemm_reps, only=only)}))
         if world > 1:
             dist.destroy_process_group()
         return
@@ -719,6 +722,8 @@ def main():
     ap.add_argument("--no-extras", action="store_true", help="skip the neighbourhood builder / embed_nodes / top-K legs")
     ap.add_argument("--extras", default="walks,embed_nodes,topk",
                     help="with --workload extras: which of the legs to run (comma-separated)")
+    ap.add_argument("--libgemm-shapes", default="all", help="with --workload libgemm: indices 0..8 of the shapes to run")
+    ap.add_argument("--libgemm-reps", type=int, default=10, help="with --workload libgemm: passes per timed figure")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu", action="store_true")
     ap.add_argument("--cpu-seconds", type=float, default=15.0)
