@@ -199,7 +199,8 @@ pool_kernel(const uint4 *__restrict__ P, const int *__restrict__ idx, const floa
             uint4 *__restrict__ out, long long n_dst, int T, int chunks, int skip_neg,
             __nv_bfloat16 *__restrict__ hubA, int H)
 {
-    extern __shared__ float hub_acc[];                     // hub mode (LPN == 32): H sums per warp
+    extern __shared__ __align__(16) float hub_acc[];       // hub mode (LPN == 32): H sums per warp
+    __shared__ int2 squeeze[8][32];                        // skip_neg: the (id, weight) pairs that remain, per warp
     using C = Chunk<BF16>;
     constexpr int NPW = 32 / LPN;
     static_assert(LPN % U == 0, "U must divide LPN");
@@ -220,8 +221,8 @@ pool_kernel(const uint4 *__restrict__ P, const int *__restrict__ idx, const floa
     const int *irow = idx + v * T;
     const float *wrow = w + v * T;
     float *hbuf = hub_acc + (size_t)(threadIdx.x >> 5) * H;
-    if (hubA != nullptr) {                                 // (one node per warp: LPN == 32)
-        for (int h = lane; h < H; h += 32) hbuf[h] = 0.f;
+    if (hubA != nullptr) {                                 // (one node per warp: LPN == 32; H % 64 == 0)
+        for (int h = lane * 4; h < H; h += 128) *reinterpret_cast<float4 *>(hbuf + h) = make_float4(0.f, 0.f, 0.f, 0.f);
         __syncwarp();
     }
     // the (id, weight) pairs of the NEXT batch are requested before the current batch's rows are gathered,
@@ -248,14 +249,21 @@ pool_kernel(const uint4 *__restrict__ P, const int *__restrict__ idx, const floa
             // out of this batch: lane k of a node's group takes the k-th remaining entry.  Groups of
             // one warp run the same number of steps (the shuffles below are warp-wide); a group that
             // has fewer entries pads with weight 0 on row 0.
-            const unsigned live = __ballot_sync(0xffffffffu, t < T && my_i >= 0);
-            const unsigned gm = LPN == 32 ? live : (live >> (lane / LPN * LPN)) & ((1u << (LPN & 31)) - 1u);
-            const unsigned src = __fns(gm, 0, sl + 1);             // position of the (sl+1)-th live entry
-            const int ci = __shfl_sync(0xffffffffu, my_i, src & (LPN - 1), LPN);
-            const float cw = __shfl_sync(0xffffffffu, my_w, src & (LPN - 1), LPN);
-            my_i = src != 0xffffffffu ? ci : 0;
-            my_w = src != 0xffffffffu ? cw : 0.f;
-            cnt = __reduce_max_sync(0xffffffffu, __popc(gm));
+            // (through shared memory: a live entry knows its rank among the live ones, i.e. where it goes;
+            // __fns, which finds where an entry comes from, is a software loop of ~60 instructions)
+            const bool lv = t < T && my_i >= 0;
+            const unsigned live = __ballot_sync(0xffffffffu, lv);
+            const int g0 = lane / LPN * LPN;
+            const unsigned gm = LPN == 32 ? live : (live >> g0) & ((1u << (LPN & 31)) - 1u);
+            int2 *sq = squeeze[threadIdx.x >> 5];
+            __syncwarp();                                          // the previous batch has been read
+            if (lv) sq[g0 + __popc(gm & ((1u << sl) - 1u))] = make_int2(my_i, __float_as_int(my_w));
+            __syncwarp();
+            const int n_live = __popc(gm);
+            const int2 e = sq[g0 + sl];
+            my_i = sl < n_live ? e.x : 0;
+            my_w = sl < n_live ? __int_as_float(e.y) : 0.f;
+            cnt = LPN == 32 ? n_live : __reduce_max_sync(0xffffffffu, n_live);
         }
         int j0 = 0;
         for (; j0 + U <= cnt; j0 += U)
@@ -276,7 +284,15 @@ pool_kernel(const uint4 *__restrict__ P, const int *__restrict__ idx, const floa
     if (hubA != nullptr) {                                 // A[v, :] = bf16 of the sums (hubs.cu)
         __syncwarp();
         __nv_bfloat16 *arow = hubA + (size_t)v * H;
-        for (int h = lane; h < H; h += 32) arow[h] = __float2bfloat16_rn(hbuf[h]);
+        for (int h = lane * 8; h < H; h += 256) {          // eight sums per lane: one 16-byte store
+            const float4 a = *reinterpret_cast<const float4 *>(hbuf + h);
+            const float4 b = *reinterpret_cast<const float4 *>(hbuf + h + 4);
+            const __nv_bfloat162 p0 = __floats2bfloat162_rn(a.x, a.y), p1 = __floats2bfloat162_rn(a.z, a.w);
+            const __nv_bfloat162 p2 = __floats2bfloat162_rn(b.x, b.y), p3 = __floats2bfloat162_rn(b.z, b.w);
+            *reinterpret_cast<uint4 *>(arow + h) =
+                make_uint4(*reinterpret_cast<const uint32_t *>(&p0), *reinterpret_cast<const uint32_t *>(&p1),
+                           *reinterpret_cast<const uint32_t *>(&p2), *reinterpret_cast<const uint32_t *>(&p3));
+        }
     }
     if (active) {
         uint4 *orow = out + (size_t)v * (size_t)chunks;
