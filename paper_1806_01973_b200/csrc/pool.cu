@@ -11,6 +11,7 @@
 // Also here: the L1-normalisation of visit counts and table validation.
 #include "internal.h"
 
+#include <algorithm>
 #include <climits>
 
 namespace pinsage {
@@ -206,12 +207,20 @@ pool_kernel(const uint4 *__restrict__ P, const int *__restrict__ idx, const floa
     static_assert(LPN % U == 0, "U must divide LPN");
     const int lane = threadIdx.x & 31;
     const int sl = lane % LPN;
+    // LOOP (the hub-split instantiations, one node per warp at a time): a warp walks nodes warp, warp + stride,
+    // ... and requests the first table batch of its next node during the last batch of the current one, so that
+    // no node starts with an exposed table latency.  Elsewhere: one pass, one node (group) per lane group.
+    constexpr bool LOOP = U == 1 && CPL <= 2 && LPN == 32;
     const long long warp = (long long)blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5);
-    const long long v_raw = warp * NPW + lane / LPN;
+    const long long wstride = (long long)gridDim.x * (blockDim.x >> 5);
     if (warp * NPW >= n_dst) return;                       // whole warp out of range
+    const long long v_raw = warp * NPW + lane / LPN;
     const bool active = v_raw < n_dst;
-    const long long v = active ? v_raw : n_dst - 1;        // idle groups shadow the last node
-
+    long long v = active ? v_raw : n_dst - 1;              // idle groups shadow the last node
+    int nx_i = 0;
+    float nx_w = 0.f;
+    bool first = true;
+  for (;;) {
     float acc[CPL][C::E];
 #pragma unroll
     for (int c = 0; c < CPL; ++c)
@@ -227,12 +236,12 @@ pool_kernel(const uint4 *__restrict__ P, const int *__restrict__ idx, const floa
     }
     // the (id, weight) pairs of the NEXT batch are requested before the current batch's rows are gathered,
     // so that the table load is off the node's chain of dependent memory latencies
-    int nx_i = 0;
-    float nx_w = 0.f;
-    if (sl < T) {
+    if ((!LOOP || first) && sl < T) {
         nx_i = ld_stream_i32(irow + sl);
         if (MODE == 0) nx_w = ld_stream_f32(wrow + sl);
     }
+    first = false;
+    const long long v_next = v + wstride;                  // (LOOP only)
     for (int tb = 0; tb < T; tb += LPN) {
         const int t = tb + sl;
         int my_i = t < T ? nx_i : 0;
@@ -240,6 +249,10 @@ pool_kernel(const uint4 *__restrict__ P, const int *__restrict__ idx, const floa
         if (t + LPN < T) {
             nx_i = ld_stream_i32(irow + t + LPN);
             if (MODE == 0) nx_w = ld_stream_f32(wrow + t + LPN);
+        }
+        if (LOOP && tb + LPN >= T && v_next < n_dst && sl < T) {      // last batch: the next node's first one
+            nx_i = ld_stream_i32(idx + v_next * T + sl);
+            if (MODE == 0) nx_w = ld_stream_f32(w + v_next * T + sl);
         }
         int cnt = min(LPN, T - tb);
         if (hubA != nullptr)                               // hub entry -(rank + 1): its weight goes to A[v, rank]
@@ -302,6 +315,10 @@ pool_kernel(const uint4 *__restrict__ P, const int *__restrict__ idx, const floa
             if (EXACT || ch < chunks) st_stream16(orow + ch, C::pack(acc[c]));
         }
     }
+    if (!LOOP || v_next >= n_dst) break;
+    v = v_next;
+    __syncwarp();                                          // hbuf / squeeze of this node have been read
+  }
 }
 
 template <bool BF16, int LPN, int CPL, int U, int MODE>
@@ -313,7 +330,10 @@ cudaError_t run_pool(const void *P, const int *idx, const float *w, void *out, l
     __nv_bfloat16 *hA = static_cast<__nv_bfloat16 *>(hubA);
     constexpr int NPW = 32 / LPN;
     const long long warps = (n_dst + NPW - 1) / NPW;
-    const long long blocks = (warps + 7) / 8;
+    long long blocks = (warps + 7) / 8;
+    // the looping (hub-split) instantiations: enough blocks to fill every SM a few times over, each warp
+    // then walks ~16 nodes or more
+    if (U == 1 && CPL <= 2 && LPN == 32) blocks = std::min<long long>(blocks, (long long)TUNED_SMS * 5 * 8);
     if (blocks > 0x7fffffffLL) return cudaErrorInvalidConfiguration;
     if (chunks == LPN * CPL)
         pool_kernel<BF16, LPN, CPL, U, true, MODE><<<(unsigned)blocks, 256, smem, s>>>(
