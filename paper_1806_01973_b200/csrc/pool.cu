@@ -133,24 +133,28 @@ struct Chunk<false> {  // 4 fp32 per 16 bytes
 // one adds their weights lane by lane to the running sum in shared memory.  Batches follow each other
 // in table order, so A[v, r] is the sum a sequential loop over t = 0..T-1 would form, bit for bit
 // (a list may legally name a hub several times: reading A7).  Called by all 32 lanes of the warp.
-__device__ __forceinline__ void hub_accumulate(float *hbuf, bool is_hub, int my_i, float my_w, int lane)
+__device__ __forceinline__ void hub_accumulate(float *hbuf, int *claim, bool is_hub, int my_i, float my_w, int lane)
 {
     const unsigned hm = __ballot_sync(0xffffffffu, is_hub);
     if (hm == 0) return;                                   // (warp-uniform)
-    if (is_hub) {
-        const int r = -(my_i + 1);
+    // Is any hub named twice in this batch?  Every hub lane signs claim[r]; a hub named by two lanes leaves at
+    // least one of them reading the other's signature.  (A shared-memory round trip instead of a MATCH.ANY,
+    // whose result was the largest single stall of the kernel; lists rarely repeat an id.)
+    const int r = is_hub ? -(my_i + 1) : 0;
+    if (is_hub) claim[r] = lane;
+    __syncwarp();
+    const unsigned dup = __ballot_sync(0xffffffffu, is_hub && claim[r] != lane);
+    if (dup == 0) {                                        // the usual case: every hub named once
+        if (is_hub) hbuf[r] += my_w;
+    } else if (is_hub) {
         const unsigned peers = __match_any_sync(hm, r);
         const int leader = __ffs(peers) - 1;
-        if (peers == (1u << lane)) {                       // the usual case: named once in this batch
-            hbuf[r] += my_w;
-        } else {
-            float sum = lane == leader ? hbuf[r] : 0.f;
-            for (unsigned rem = peers; rem; rem &= rem - 1) {
-                const float wv = __shfl_sync(peers, my_w, __ffs(rem) - 1);
-                sum += wv;                                 // (only the leader's sum is used)
-            }
-            if (lane == leader) hbuf[r] = sum;
+        float sum = lane == leader ? hbuf[r] : 0.f;
+        for (unsigned rem = peers; rem; rem &= rem - 1) {
+            const float wv = __shfl_sync(peers, my_w, __ffs(rem) - 1);
+            sum += wv;                                     // (only the leader's sum is used)
         }
+        if (lane == leader) hbuf[r] = sum;
     }
     __syncwarp();                                          // the next batch may update the same sums from other lanes
 }
@@ -230,6 +234,7 @@ pool_kernel(const uint4 *__restrict__ P, const int *__restrict__ idx, const floa
     const int *irow = idx + v * T;
     const float *wrow = w + v * T;
     float *hbuf = hub_acc + (size_t)(threadIdx.x >> 5) * H;
+    int *claim = reinterpret_cast<int *>(hub_acc + (size_t)8 * H) + (size_t)(threadIdx.x >> 5) * H;   // (see hub_accumulate)
     if (hubA != nullptr) {                                 // (one node per warp: LPN == 32; H % 64 == 0)
         for (int h = lane * 4; h < H; h += 128) *reinterpret_cast<float4 *>(hbuf + h) = make_float4(0.f, 0.f, 0.f, 0.f);
         __syncwarp();
@@ -256,7 +261,7 @@ pool_kernel(const uint4 *__restrict__ P, const int *__restrict__ idx, const floa
         }
         int cnt = min(LPN, T - tb);
         if (hubA != nullptr)                               // hub entry -(rank + 1): its weight goes to A[v, rank]
-            hub_accumulate(hbuf, t < T && my_i < 0, my_i, my_w, lane);
+            hub_accumulate(hbuf, claim, t < T && my_i < 0, my_i, my_w, lane);
         if (skip_neg) {
             // entries with a negative id (hub neighbours, summed by the hub GEMM: hubs.cu) are squeezed
             // out of this batch: lane k of a node's group takes the k-th remaining entry.  Groups of
@@ -326,7 +331,7 @@ cudaError_t run_pool(const void *P, const int *idx, const float *w, void *out, l
                      int T, int chunks, cudaStream_t s, int skip_neg = 0, void *hubA = nullptr, int H = 0)
 {
     if (hubA != nullptr && LPN != 32) return cudaErrorNotSupported;
-    const size_t smem = hubA != nullptr ? (size_t)8 * H * 4 : 0;
+    const size_t smem = hubA != nullptr ? (size_t)8 * H * 8 : 0;      // per warp: H sums and H signatures
     __nv_bfloat16 *hA = static_cast<__nv_bfloat16 *>(hubA);
     constexpr int NPW = 32 / LPN;
     const long long warps = (n_dst + NPW - 1) / NPW;
